@@ -1,0 +1,198 @@
+"""ctypes face of the CPU oracle (oracle/nb_oracle.c).  TEST INFRASTRUCTURE, NOT THE PRODUCT.
+
+Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs may
+import this package.  It imports nothing from paper_2604_09184_b200/ (the CUDA path), and the
+CUDA path never imports it.  Every function takes and returns numpy float64 host arrays.
+Citations are in nb_oracle.c next to each function.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+import subprocess
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "nb_oracle.c")
+_LIB = os.path.join(_HERE, "liboracle.so")
+
+# -ffp-contract=off: the oracle states r^2 = (dx*dx + dy*dy) + dz*dz without fused multiply-adds.
+_CFLAGS = ["-O2", "-ffp-contract=off", "-fno-fast-math", "-fopenmp", "-shared", "-fPIC", "-Wall", "-Wextra"]
+
+
+def build(force: bool = False) -> str:
+    """Compile the oracle with gcc (building the checker is not using it)."""
+    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
+        subprocess.check_call(["gcc", *_CFLAGS, "-o", _LIB, _SRC, "-lm"])
+    return _LIB
+
+
+_lib = None
+
+
+def _L():
+    global _lib
+    if _lib is None:
+        lib = C.CDLL(build())
+        dp, ip, lp = C.POINTER(C.c_double), C.POINTER(C.c_int32), C.POINTER(C.c_int64)
+        i64, dbl, i32 = C.c_int64, C.c_double, C.c_int
+        lib.oracle_num_threads.restype = i32
+        lib.oracle_set_num_threads.argtypes = [i32]
+        lib.oracle_changeover.restype = dbl
+        lib.oracle_changeover.argtypes = [dbl, dbl, i32]
+        lib.oracle_rcrit.argtypes = [dp, dp, dp, dbl, i64, dbl, dbl, dbl, dbl, dp]
+        lib.oracle_accel.argtypes = [dp, dp, dp, i64, i64, dbl, i32, lp, i64, dp, dp, lp]
+        lib.oracle_kick.argtypes = [dp, dp, dp, i64, i64, dbl, dp, dbl, i32, dp]
+        lib.oracle_pairs.argtypes = [dp, dp, i64, i64, dbl, lp, i64, ip, i64, lp, ip, i64, lp]
+        lib.oracle_shift.argtypes = [dp, dp, dp, dbl, i64, dbl]
+        lib.oracle_kepler_elliptic.restype = i32
+        lib.oracle_kepler_elliptic.argtypes = [dp, dp, dbl, dbl]
+        lib.oracle_kepler_universal.restype = i32
+        lib.oracle_kepler_universal.argtypes = [dp, dp, dbl, dbl]
+        lib.oracle_drift_kepler.restype = i64
+        lib.oracle_drift_kepler.argtypes = [dp, dp, dbl, i64, dbl, dbl, i32]
+        lib.oracle_step.restype = i64
+        lib.oracle_step.argtypes = [dp, dp, dp, dbl, i64, i64, dbl, dbl, dbl, dbl, i32, dp, dp, i64]
+        lib.oracle_diagnostics.argtypes = [dp, dp, dp, dbl, i64, dbl, dp]
+        _lib = lib
+    return _lib
+
+
+def _d(a):
+    a = np.ascontiguousarray(a, dtype=np.float64)
+    return a, a.ctypes.data_as(C.POINTER(C.c_double))
+
+
+def _rows(rows):
+    if rows is None:
+        return None, None, 0
+    r = np.ascontiguousarray(rows, dtype=np.int64)
+    return r, r.ctypes.data_as(C.POINTER(C.c_int64)), r.shape[0]
+
+
+def num_threads() -> int:
+    return int(_L().oracle_num_threads())
+
+
+def set_num_threads(n: int) -> None:
+    _L().oracle_set_num_threads(int(n))
+
+
+def changeover(r: float, rc: float, kind: int = 0) -> float:
+    return float(_L().oracle_changeover(float(r), float(rc), int(kind)))
+
+
+def rcrit(x, v, m, M_star, dt, G, n1=3.0, n2=0.4):
+    x, px = _d(x); v, pv = _d(v); m, pm = _d(m)
+    N = m.shape[0]
+    out = np.empty(N)
+    _L().oracle_rcrit(px, pv, pm, M_star, N, dt, G, n1, n2, out.ctypes.data_as(C.POINTER(C.c_double)))
+    return out
+
+
+def accel(x, m, rcrit_, G, n_active=0, kind=0, rows=None, want_abs=False):
+    """a_i (and optionally sum_j |term|).  Returns (acc, abs_sum or None, n_singular)."""
+    x, px = _d(x); m, pm = _d(m)
+    N = m.shape[0]
+    if rcrit_ is None:
+        prc = None
+    else:
+        rcrit_, prc = _d(rcrit_)
+    r, pr, nr = _rows(rows)
+    n_out = nr if rows is not None else N
+    acc = np.empty((n_out, 3))
+    ab = np.empty((n_out, 3)) if want_abs else None
+    ns = C.c_int64(0)
+    _L().oracle_accel(px, pm, prc, N, n_active, G, kind, pr, nr,
+                      acc.ctypes.data_as(C.POINTER(C.c_double)),
+                      ab.ctypes.data_as(C.POINTER(C.c_double)) if want_abs else None, C.byref(ns))
+    return acc, ab, int(ns.value)
+
+
+def kick(x, v, m, dt, rcrit_, G, n_active=0, kind=0):
+    """Returns (v_new, acc)."""
+    x, px = _d(x); m, pm = _d(m)
+    v = np.array(v, dtype=np.float64, order="C", copy=True)
+    N = m.shape[0]
+    if rcrit_ is None:
+        prc = None
+    else:
+        rcrit_, prc = _d(rcrit_)
+    acc = np.empty((N, 3))
+    _L().oracle_kick(px, v.ctypes.data_as(C.POINTER(C.c_double)), pm, N, n_active, dt, prc, G, kind,
+                     acc.ctypes.data_as(C.POINTER(C.c_double)))
+    return v, acc
+
+
+def _canon(p):
+    """Canonical pair order: unique rows sorted by (min, max) (reading S12)."""
+    if p.shape[0] == 0:
+        return p.reshape(0, 2)
+    return np.unique(p, axis=0)
+
+
+def pairs(x, rcrit_, n_active=0, tol2=2e-12, rows=None, cap=1 << 22):
+    """Returns (sure[ns,2], borderline[nb,2]) int32, canonically sorted, de-duplicated."""
+    x, px = _d(x); rcrit_, prc = _d(rcrit_)
+    N = rcrit_.shape[0]
+    r, pr, nr = _rows(rows)
+    while True:
+        sure = np.empty((cap, 2), dtype=np.int32)
+        bord = np.empty((cap, 2), dtype=np.int32)
+        ns, nb = C.c_int64(0), C.c_int64(0)
+        _L().oracle_pairs(px, prc, N, n_active, tol2, pr, nr,
+                          sure.ctypes.data_as(C.POINTER(C.c_int32)), cap, C.byref(ns),
+                          bord.ctypes.data_as(C.POINTER(C.c_int32)), cap, C.byref(nb))
+        if ns.value <= cap and nb.value <= cap:
+            break
+        cap = int(max(ns.value, nb.value))
+    return _canon(sure[: ns.value]), _canon(bord[: nb.value])
+
+
+def shift(x, v, m, M_star, dt):
+    x = np.array(x, dtype=np.float64, order="C", copy=True)
+    v, pv = _d(v); m, pm = _d(m)
+    _L().oracle_shift(x.ctypes.data_as(C.POINTER(C.c_double)), pv, pm, M_star, m.shape[0], dt)
+    return x
+
+
+def kepler_one(x, v, mu, h, solver="elliptic"):
+    """Advance ONE body.  Returns (x, v, code)."""
+    x = np.array(x, dtype=np.float64, copy=True).reshape(3)
+    v = np.array(v, dtype=np.float64, copy=True).reshape(3)
+    fn = _L().oracle_kepler_elliptic if solver == "elliptic" else _L().oracle_kepler_universal
+    code = fn(x.ctypes.data_as(C.POINTER(C.c_double)), v.ctypes.data_as(C.POINTER(C.c_double)), mu, h)
+    return x, v, int(code)
+
+
+def drift_kepler(x, v, M_star, dt, G, solver=0):
+    """Returns (x_new, v_new, n_fail)."""
+    x = np.array(x, dtype=np.float64, order="C", copy=True)
+    v = np.array(v, dtype=np.float64, order="C", copy=True)
+    N = x.shape[0]
+    nf = _L().oracle_drift_kepler(x.ctypes.data_as(C.POINTER(C.c_double)),
+                                  v.ctypes.data_as(C.POINTER(C.c_double)), M_star, N, dt, G, solver)
+    return x, v, int(nf)
+
+
+def step(x, v, m, M_star, dt, G, nsteps, n_active=0, n1=3.0, n2=0.0, kind=0, rcrit_=None):
+    """nsteps steps B(dt/2)C(dt/2)A(dt)C(dt/2)B(dt/2).  Returns dict(x, v, acc, rcrit, n_fail)."""
+    x = np.array(x, dtype=np.float64, order="C", copy=True)
+    v = np.array(v, dtype=np.float64, order="C", copy=True)
+    m, pm = _d(m)
+    N = m.shape[0]
+    rc = np.zeros(N) if rcrit_ is None else np.array(rcrit_, dtype=np.float64, copy=True)
+    acc = np.empty((N, 3))
+    P = C.POINTER(C.c_double)
+    nf = _L().oracle_step(x.ctypes.data_as(P), v.ctypes.data_as(P), pm, M_star, N, n_active, dt, G,
+                          n1, n2, kind, rc.ctypes.data_as(P), acc.ctypes.data_as(P), nsteps)
+    return dict(x=x, v=v, acc=acc, rcrit=rc, n_fail=int(nf))
+
+
+def diagnostics(x, v, m, M_star, G):
+    """dict(E, L[3], T, T_star, U_star, U_mutual) -- PAPER.md:84-92 with the K terms cancelling."""
+    x, px = _d(x); v, pv = _d(v); m, pm = _d(m)
+    out = np.empty(8)
+    _L().oracle_diagnostics(px, pv, pm, M_star, m.shape[0], G, out.ctypes.data_as(C.POINTER(C.c_double)))
+    return dict(E=out[0], L=out[1:4].copy(), T=out[4], T_star=out[5], U_star=out[6], U_mutual=out[7])

@@ -1,0 +1,458 @@
+/*
+ * nb_oracle.c -- TEST INFRASTRUCTURE, NOT THE PRODUCT.
+ *
+ * Plain, slow, double-precision CPU statement of the hot path of the hybrid symplectic
+ * integrator in Grimm & Stadel (arxiv 2604.09184; /root/reference/PAPER.md):
+ *   - changeover weight W            PAPER.md:94            (shape: DESIGN.md reading S2)
+ *   - critical radius                PAPER.md:94-96, Eq. 7  (R_Hill: reading S5)
+ *   - H_B kick, O(N^2)               PAPER.md:86 Eq. 5, 98  (force weighting: readings S1, S3)
+ *   - close-encounter pair list      PAPER.md:94, 98, 106   (r_crit,ij = max: reading S4)
+ *   - H_C shift                      PAPER.md:91-92 Eq. 6
+ *   - H_A Kepler drift, Gauss f,g    PAPER.md:64, 98        (solver: reading S15)
+ *   - step  B(dt/2) C(dt/2) A(dt) C(dt/2) B(dt/2)           PAPER.md:80 Eq. 3 (order: S6, S17)
+ *   - diagnostics E, L               PAPER.md:84-92 Eq. 4-6 (K terms cancel in H_A + H_B)
+ *
+ * It is the definition written out: explicit loops in the paper's index order, no blocking,
+ * no fusion, no FMA contraction (build with -ffp-contract=off).  All inputs and outputs are
+ * fp64.  Sums are Neumaier-compensated, and the O(N^2) acceleration sum carries its terms in the
+ * host's extended precision (x87 long double) before one final rounding to fp64, so that the
+ * whole 1e-12 error budget belongs to the CUDA path.  Decisions that produce integers (the
+ * pair test r^2 < rc^2) are taken in plain fp64.  OpenMP parallelises over the OUTER body
+ * index i only; every per-body sum runs sequentially in j order.
+ *
+ * It shares no code, header, table or helper with paper_2604_09184_b200/ (the CUDA path) and
+ * neither includes the other.  Only tests/, __graft_entry__.smoke() and bench.py's
+ * cpu_baseline / --impl reference legs may call it.
+ *
+ * Pins (tests/test_oracle_*.py, -m "not gpu"): every exported function is pinned by closed
+ * forms, invariants or brute force; the SHAPE of W between its end points, the max() rule for
+ * r_crit,ij and force-vs-potential weighting are "parity unpinned" against the paper (the
+ * paper gives no formula for them) -- see DESIGN.md.
+ */
+#include <math.h>
+#include <stdint.h>
+#include <stdlib.h>
+#include <string.h>
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+
+#define ORACLE_PI 3.141592653589793238462643383279502884
+
+int oracle_num_threads(void) {
+#ifdef _OPENMP
+    return omp_get_max_threads();
+#else
+    return 1;
+#endif
+}
+
+void oracle_set_num_threads(int n) {
+#ifdef _OPENMP
+    if (n > 0) omp_set_num_threads(n);
+#else
+    (void)n;
+#endif
+}
+
+/* Neumaier's compensated summation: (sum, comp) += t. */
+static inline void neumaier_add(double *sum, double *comp, double t) {
+    double s = *sum + t;
+    if (fabs(*sum) >= fabs(t)) *comp += (*sum - s) + t;
+    else                       *comp += (t - s) + *sum;
+    *sum = s;
+}
+
+/* ------------------------------------------------------------------------------------------
+ * Changeover / kick weight W(r; rc)  -- PAPER.md:94 "smooth changeover function ranging from
+ * 0 to 1"; the changeover "starts to act" at the critical radius.  Reading S1: W = 1 far
+ * (r >= rc), W = 0 close (r <= 0.1 rc).  Reading S2: between, with y = (r-0.1rc)/(0.9rc),
+ *   kind 0: K_C(y) = y^2 / (2y^2 - 2y + 1)       (form of the hybrid scheme the paper cites [9])
+ *   kind 1: 10y^3 - 15y^4 + 6y^5                 (quintic smoothstep, alternative)
+ * ------------------------------------------------------------------------------------------ */
+double oracle_changeover(double r, double rc, int kind) {
+    if (!(r < rc)) return 1.0;            /* r >= rc; also rc == 0 */
+    double y = (r - 0.1 * rc) / (0.9 * rc);
+    if (y <= 0.0) return 0.0;
+    if (y >= 1.0) return 1.0;
+    if (kind == 1) return y * y * y * (10.0 + y * (-15.0 + 6.0 * y));
+    return (y * y) / (2.0 * y * y - 2.0 * y + 1.0);
+}
+
+/* ------------------------------------------------------------------------------------------
+ * Critical radius, Eq. 7:  rc_i = max(n1 R_Hill,i , n2 dt v_i),  n1 = 3, n2 = 0.4.
+ * Reading S5: R_Hill,i = a_i (m_i / (3 M_star))^(1/3), a_i from vis-viva with the stored
+ * (barycentric) velocity, 1/a = 2/r - v^2/(G M_star); if 1/a <= 0 use a_i = r_i.
+ * |dt| is used so that a backward step sees the same radius.
+ * ------------------------------------------------------------------------------------------ */
+void oracle_rcrit(const double *x, const double *v, const double *m, double M_star, int64_t N,
+                  double dt, double G, double n1, double n2, double *rcrit) {
+    for (int64_t i = 0; i < N; ++i) {
+        double xi = x[3 * i], yi = x[3 * i + 1], zi = x[3 * i + 2];
+        double vx = v[3 * i], vy = v[3 * i + 1], vz = v[3 * i + 2];
+        double r = sqrt((xi * xi + yi * yi) + zi * zi);
+        double v2 = (vx * vx + vy * vy) + vz * vz;
+        double inva = 2.0 / r - v2 / (G * M_star);
+        double a = (inva > 0.0) ? 1.0 / inva : r;
+        double rh = a * cbrt(m[i] / (3.0 * M_star));
+        double t1 = n1 * rh;
+        double t2 = n2 * fabs(dt) * sqrt(v2);
+        rcrit[i] = (t1 > t2) ? t1 : t2;
+    }
+}
+
+/* ------------------------------------------------------------------------------------------
+ * H_B accelerations (Eq. 5; "H_B describes the N^2 mutual
+ * gravitational force terms"; BASELINE.json:north_star):
+ *     a_i = sum_{j != i, j < n_active} G m_j W(r_ij; rc_ij) (x_j - x_i) / r_ij^3
+ * rc_ij = max(rc_i, rc_j) (S4).  The weight multiplies the force (S3).  r_ij^2 is formed as
+ * (dx*dx + dy*dy) + dz*dz.  S10: the self term is skipped; W = 0 contributes exactly 0 (so a
+ * coincident pair with rc_ij > 0 never forms 0 * inf); a coincident pair with rc_ij == 0 is
+ * counted in *n_singular and contributes 0.
+ * Semi-active mode (north_star; not in the paper): j runs over the first n_active bodies only.
+ * rows == NULL: all i = 0..N-1 (acc is [N,3]); otherwise only the listed rows (acc is [nrows,3]).
+ * abs_sum (optional, same shape as acc): sum_j |term| per component, for the conditioning-aware
+ * error report.
+ * ------------------------------------------------------------------------------------------ */
+static long double changeover_ext(long double r, long double rc, int kind) {
+    if (!(r < rc)) return 1.0L;
+    long double y = (r - 0.1L * rc) / (0.9L * rc);
+    if (y <= 0.0L) return 0.0L;
+    if (y >= 1.0L) return 1.0L;
+    if (kind == 1) return y * y * y * (10.0L + y * (-15.0L + 6.0L * y));
+    return (y * y) / (2.0L * y * y - 2.0L * y + 1.0L);
+}
+
+void oracle_accel(const double *x, const double *m, const double *rcrit, int64_t N,
+                  int64_t n_active, double G, int kind, const int64_t *rows, int64_t nrows,
+                  double *acc, double *abs_sum, int64_t *n_singular) {
+    /* Every term and the three running sums are carried in the host's extended precision
+       (x87 long double, 64-bit significand) and rounded to fp64 once at the end, so that the
+       oracle's own rounding is far below the 1e-12 per-component tolerance it arbitrates. */
+    int64_t nr = rows ? nrows : N;
+    int64_t nsing = 0;
+    if (n_active <= 0 || n_active > N) n_active = N;
+#pragma omp parallel for schedule(dynamic, 16) reduction(+ : nsing)
+    for (int64_t k = 0; k < nr; ++k) {
+        int64_t i = rows ? rows[k] : k;
+        long double xi = x[3 * i], yi = x[3 * i + 1], zi = x[3 * i + 2];
+        long double rci = rcrit ? rcrit[i] : 0.0;
+        long double sx = 0, sy = 0, sz = 0;
+        long double bx = 0, by = 0, bz = 0;
+        for (int64_t j = 0; j < n_active; ++j) {
+            if (j == i) continue;
+            long double dx = x[3 * j] - xi, dy = x[3 * j + 1] - yi, dz = x[3 * j + 2] - zi;
+            long double r2 = (dx * dx + dy * dy) + dz * dz;
+            long double rcj = rcrit ? rcrit[j] : 0.0;
+            long double rc = (rci > rcj) ? rci : rcj;
+            long double r = sqrtl(r2);
+            long double W = changeover_ext(r, rc, kind);
+            if (W == 0.0L) continue;
+            if (r2 == 0.0L) { nsing++; continue; }   /* only reachable with rc == 0 */
+            long double f = (long double)G * m[j] * W / (r2 * r);
+            long double tx = f * dx, ty = f * dy, tz = f * dz;
+            sx += tx; sy += ty; sz += tz;
+            bx += fabsl(tx); by += fabsl(ty); bz += fabsl(tz);
+        }
+        acc[3 * k] = (double)sx; acc[3 * k + 1] = (double)sy; acc[3 * k + 2] = (double)sz;
+        if (abs_sum) { abs_sum[3 * k] = (double)bx; abs_sum[3 * k + 1] = (double)by; abs_sum[3 * k + 2] = (double)bz; }
+    }
+    if (n_singular) *n_singular = nsing;
+}
+
+/* Kick: acc <- a(x); v_i += dt * a_i. */
+void oracle_kick(const double *x, double *v, const double *m, int64_t N, int64_t n_active,
+                 double dt, const double *rcrit, double G, int kind, double *acc) {
+    oracle_accel(x, m, rcrit, N, n_active, G, kind, NULL, 0, acc, NULL, NULL);
+    for (int64_t i = 0; i < 3 * N; ++i) v[i] = v[i] + dt * acc[i];
+}
+
+/* ------------------------------------------------------------------------------------------
+ * Close-encounter pairs ("critical radius describes the separation distance ...
+ * when the changeover starts to act"): every unordered {i,j} with
+ * r_ij < rc_ij = max(rc_i, rc_j), emitted once as (min,max) (S11, S12).  Semi-active: at
+ * least one member must be active (index < n_active) (S13).
+ * The north_star tolerance clause ("pairs within 1e-12 relative of the r_crit threshold ...
+ * listed separately") is applied in r^2 (tol2 = 2e-12):
+ *    sure        r^2 <  rc^2 (1 - tol2)
+ *    borderline  |r^2/rc^2 - 1| <= tol2
+ * rows == NULL: all pairs.  rows != NULL: pairs incident to the listed bodies (each (min,max)
+ * may then appear once per listed member; the caller de-duplicates).
+ * Output order is unspecified (the caller sorts).  Counts keep counting past the capacities.
+ * ------------------------------------------------------------------------------------------ */
+void oracle_pairs(const double *x, const double *rcrit, int64_t N, int64_t n_active,
+                  double tol2, const int64_t *rows, int64_t nrows,
+                  int32_t *sure, int64_t cap_sure, int64_t *n_sure,
+                  int32_t *border, int64_t cap_border, int64_t *n_border) {
+    int64_t ns = 0, nb = 0;
+    if (n_active <= 0 || n_active > N) n_active = N;
+    int64_t nr = rows ? nrows : n_active;
+#pragma omp parallel for schedule(dynamic, 16)
+    for (int64_t k = 0; k < nr; ++k) {
+        int64_t i = rows ? rows[k] : k;
+        double xi = x[3 * i], yi = x[3 * i + 1], zi = x[3 * i + 2];
+        double rci = rcrit[i];
+        /* full list: j > i (i is active since i < n_active);
+           row list : all j != i with at least one of (i,j) active */
+        int64_t j0 = rows ? 0 : i + 1;
+        int64_t j1 = (rows && i >= n_active) ? n_active : N;
+        for (int64_t j = j0; j < j1; ++j) {
+            if (j == i) continue;
+            double dx = x[3 * j] - xi, dy = x[3 * j + 1] - yi, dz = x[3 * j + 2] - zi;
+            double r2 = (dx * dx + dy * dy) + dz * dz;
+            double rcj = rcrit[j];
+            double rc = (rci > rcj) ? rci : rcj;
+            double rc2 = rc * rc;
+            int is_sure = r2 < rc2 * (1.0 - tol2);
+            int is_border = !is_sure && (fabs(r2 / rc2 - 1.0) <= tol2);
+            if (!is_sure && !is_border) continue;
+            int32_t lo = (int32_t)(i < j ? i : j), hi = (int32_t)(i < j ? j : i);
+#pragma omp critical(oracle_pairs_append)
+            {
+                if (is_sure) {
+                    if (ns < cap_sure) { sure[2 * ns] = lo; sure[2 * ns + 1] = hi; }
+                    ns++;
+                } else {
+                    if (nb < cap_border) { border[2 * nb] = lo; border[2 * nb + 1] = hi; }
+                    nb++;
+                }
+            }
+        }
+    }
+    *n_sure = ns;
+    *n_border = nb;
+}
+
+/* ------------------------------------------------------------------------------------------
+ * H_C (Eq. 6): H_C = (sum p_i)^2 / (2 m_0)  =>  every heliocentric position
+ * moves by  dt * (sum_i m_i v_i) / M_star.  Sum in index order, compensated.
+ * ------------------------------------------------------------------------------------------ */
+void oracle_shift(double *x, const double *v, const double *m, double M_star, int64_t N,
+                  double dt) {
+    double s[3] = {0, 0, 0}, c[3] = {0, 0, 0};
+    for (int64_t i = 0; i < N; ++i)
+        for (int k = 0; k < 3; ++k) neumaier_add(&s[k], &c[k], m[i] * v[3 * i + k]);
+    for (int k = 0; k < 3; ++k) s[k] = (s[k] + c[k]) / M_star;
+    for (int64_t i = 0; i < N; ++i)
+        for (int k = 0; k < 3; ++k) x[3 * i + k] = x[3 * i + k] + dt * s[k];
+}
+
+/* ------------------------------------------------------------------------------------------
+ * H_A without encounters: Kepler flow about mu = G M_star ("a Keplerian orbit can
+ * be solved analytically"; Eq. 4 first sum), advanced with Gauss'
+ * f and g functions (BASELINE.json:north_star).
+ *
+ * Elliptic solver (alpha = 2/r0 - v^2/mu > 0), in the differenced eccentric anomaly dE:
+ *   a = 1/alpha, n = sqrt(mu/a^3), ec = 1 - r0/a, es = (x.v)/sqrt(mu a),
+ *   dM = n h reduced to (-pi, pi],
+ *   F(dE) = dE - ec sin dE + es (1 - cos dE) - dM = 0,   F' = r/a > 0   (unique root),
+ *   Newton from dE = dM safeguarded by bisection on [dM - 3e, dM + 3e],
+ *   c = 2 sin^2(dE/2), s = sin dE, r = a (1 - ec (1 - c) + es s),
+ *   f = 1 - (a/r0) c,  g = [(r0/a) s + es c]/n,  fdot = -sqrt(mu a) s/(r r0),  gdot = 1 - (a/r) c.
+ * Returns 0 on convergence, 1 if 64 iterations did not reach the fixed point (state then
+ * left unchanged), 2 if not elliptic (state unchanged).
+ * ------------------------------------------------------------------------------------------ */
+int oracle_kepler_elliptic(double *x, double *v, double mu, double h) {
+    double r0 = sqrt((x[0] * x[0] + x[1] * x[1]) + x[2] * x[2]);
+    double v2 = (v[0] * v[0] + v[1] * v[1]) + v[2] * v[2];
+    double u = (x[0] * v[0] + x[1] * v[1]) + x[2] * v[2];
+    double alpha = 2.0 / r0 - v2 / mu;
+    if (!(alpha > 0.0)) return 2;
+    double a = 1.0 / alpha;
+    double n = sqrt(mu / (a * a * a));
+    double ec = 1.0 - r0 / a;
+    double es = u / sqrt(mu * a);
+    double e = sqrt(ec * ec + es * es);
+    double dM = n * h;
+    dM = dM - 2.0 * ORACLE_PI * nearbyint(dM / (2.0 * ORACLE_PI));
+    double lo = dM - 3.0 * e, hi = dM + 3.0 * e;
+    double dE = dM;
+    int converged = 0;
+    for (int it = 0; it < 64; ++it) {
+        double sn = sin(dE), cs = cos(dE);
+        double F = dE - ec * sn + es * (1.0 - cs) - dM;
+        double Fp = 1.0 - ec * cs + es * sn;
+        if (F > 0.0) hi = dE; else lo = dE;
+        double step = F / Fp;
+        double nxt = dE - step;
+        if (!(nxt > lo && nxt < hi)) nxt = 0.5 * (lo + hi);   /* bisection safeguard */
+        double delta = nxt - dE;
+        dE = nxt;
+        if (fabs(delta) <= 2.220446049250313e-16 * fmax(1.0, fabs(dE))) { converged = 1; break; }
+    }
+    if (!converged) return 1;
+    double sh = sin(0.5 * dE);
+    double c = 2.0 * sh * sh;
+    double s = sin(dE);
+    double r = a * (1.0 - ec * (1.0 - c) + es * s);
+    double f = 1.0 - (a / r0) * c;
+    double g = ((r0 / a) * s + es * c) / n;
+    double fd = -sqrt(mu * a) * s / (r * r0);
+    double gd = 1.0 - (a / r) * c;
+    for (int k = 0; k < 3; ++k) {
+        double xn = f * x[k] + g * v[k];
+        double vn = fd * x[k] + gd * v[k];
+        x[k] = xn; v[k] = vn;
+    }
+    return 0;
+}
+
+/* Stumpff functions c0..c3 of z (Danby's argument-quartering + series + duplication). */
+static void stumpff(double z, double *c0, double *c1, double *c2, double *c3) {
+    int nq = 0;
+    while (fabs(z) > 0.1) { z *= 0.25; nq++; }
+    /* series: c2 = sum (-z)^k/(2k+2)!, c3 = sum (-z)^k/(2k+3)! */
+    double a2 = 1.0 / 2.0, a3 = 1.0 / 6.0, t2 = a2, t3 = a3;
+    for (int k = 1; k < 12; ++k) {
+        t2 *= -z / ((2.0 * k + 1.0) * (2.0 * k + 2.0));
+        t3 *= -z / ((2.0 * k + 2.0) * (2.0 * k + 3.0));
+        a2 += t2; a3 += t3;
+    }
+    double C2 = a2, C3 = a3, C1 = 1.0 - z * C3, C0 = 1.0 - z * C2;
+    for (; nq > 0; --nq) {
+        C3 = 0.25 * (C2 + C0 * C3);
+        C2 = 0.5 * C1 * C1;
+        C1 = C0 * C1;
+        C0 = 2.0 * C0 * C0 - 1.0;
+    }
+    *c0 = C0; *c1 = C1; *c2 = C2; *c3 = C3;
+}
+
+/* Universal-variable solver (any conic; second, independent route -- also the fallback when
+ * alpha <= 0, S15).  With beta = 2 mu/r0 - v^2, G_k(s) = s^k c_k(beta s^2), u = x.v:
+ *    h = r0 G1 + u G2 + mu G3            (universal Kepler equation, dF/ds = r > 0)
+ *    r = r0 G0 + u G1 + mu G2
+ *    f = 1 - (mu/r0) G2, g = h - mu G3, fdot = -(mu/(r r0)) G1, gdot = 1 - (mu/r) G2.
+ * Newton from s = h/r0, safeguarded by an expanding bracket + bisection.
+ * Returns 0 ok, 1 not converged (state unchanged). */
+int oracle_kepler_universal(double *x, double *v, double mu, double h) {
+    double r0 = sqrt((x[0] * x[0] + x[1] * x[1]) + x[2] * x[2]);
+    double v2 = (v[0] * v[0] + v[1] * v[1]) + v[2] * v[2];
+    double u = (x[0] * v[0] + x[1] * v[1]) + x[2] * v[2];
+    double beta = 2.0 * mu / r0 - v2;
+    double s = h / r0;
+    double lo = -INFINITY, hi = INFINITY;
+    double c0, c1, c2, c3, G0 = 1, G1 = 0, G2 = 0, G3 = 0, r = r0;
+    int converged = 0;
+    for (int it = 0; it < 200; ++it) {
+        stumpff(beta * s * s, &c0, &c1, &c2, &c3);
+        G0 = c0; G1 = s * c1; G2 = s * s * c2; G3 = s * s * s * c3;
+        double F = r0 * G1 + u * G2 + mu * G3 - h;
+        r = r0 * G0 + u * G1 + mu * G2;
+        if (F > 0.0) hi = s; else lo = s;
+        double nxt = s - F / r;
+        if (!(nxt > lo && nxt < hi)) {
+            if (isinf(lo)) nxt = (hi == 0.0) ? -1.0 : hi - 2.0 * fabs(hi) - 1e-3;
+            else if (isinf(hi)) nxt = (lo == 0.0) ? 1.0 : lo + 2.0 * fabs(lo) + 1e-3;
+            else nxt = 0.5 * (lo + hi);
+        }
+        double delta = nxt - s;
+        s = nxt;
+        if (fabs(delta) <= 2.220446049250313e-16 * fmax(fabs(s), fabs(h / r0))) { converged = 1; break; }
+    }
+    if (!converged) return 1;
+    stumpff(beta * s * s, &c0, &c1, &c2, &c3);
+    G0 = c0; G1 = s * c1; G2 = s * s * c2; G3 = s * s * s * c3;
+    r = r0 * G0 + u * G1 + mu * G2;
+    double f = 1.0 - (mu / r0) * G2;
+    double g = h - mu * G3;
+    double fd = -(mu / (r * r0)) * G1;
+    double gd = 1.0 - (mu / r) * G2;
+    for (int k = 0; k < 3; ++k) {
+        double xn = f * x[k] + g * v[k];
+        double vn = fd * x[k] + gd * v[k];
+        x[k] = xn; v[k] = vn;
+    }
+    return 0;
+}
+
+/* Drift every body: elliptic solver when bound, universal variables otherwise (S15).
+ * solver: 0 = as described, 1 = force the universal solver for every body (cross-check).
+ * Returns the number of bodies that failed to converge (left unchanged). */
+int64_t oracle_drift_kepler(double *x, double *v, double M_star, int64_t N, double dt, double G,
+                            int solver) {
+    double mu = G * M_star;
+    int64_t nfail = 0;
+#pragma omp parallel for schedule(static) reduction(+ : nfail)
+    for (int64_t i = 0; i < N; ++i) {
+        int rcode = 2;
+        if (solver == 0) rcode = oracle_kepler_elliptic(x + 3 * i, v + 3 * i, mu, dt);
+        if (rcode == 2) rcode = oracle_kepler_universal(x + 3 * i, v + 3 * i, mu, dt);
+        if (rcode != 0) nfail++;
+    }
+    return nfail;
+}
+
+/* ------------------------------------------------------------------------------------------
+ * One run of nsteps steps (Eq. 3; order S6: B(dt/2) C(dt/2) A(dt) C(dt/2) B(dt/2)).
+ * S17: r_crit is recomputed from the current (x, v) immediately before every force
+ * evaluation (skipped when n1 == n2 == 0: the caller's rcrit is used unchanged); the closing
+ * half-kick of step n and the opening half-kick of step n+1 share that evaluation.
+ * On return acc / rcrit are those of the last evaluation (at the final positions).
+ * Returns the number of Kepler non-convergences.
+ * ------------------------------------------------------------------------------------------ */
+int64_t oracle_step(double *x, double *v, const double *m, double M_star, int64_t N,
+                    int64_t n_active, double dt, double G, double n1, double n2, int kind,
+                    double *rcrit, double *acc, int64_t nsteps) {
+    int64_t nfail = 0;
+    int update_rc = !(n1 == 0.0 && n2 == 0.0);
+    if (update_rc) oracle_rcrit(x, v, m, M_star, N, dt, G, n1, n2, rcrit);
+    oracle_accel(x, m, rcrit, N, n_active, G, kind, NULL, 0, acc, NULL, NULL);
+    for (int64_t st = 0; st < nsteps; ++st) {
+        for (int64_t i = 0; i < 3 * N; ++i) v[i] = v[i] + (0.5 * dt) * acc[i];
+        oracle_shift(x, v, m, M_star, N, 0.5 * dt);
+        nfail += oracle_drift_kepler(x, v, M_star, N, dt, G, 0);
+        oracle_shift(x, v, m, M_star, N, 0.5 * dt);
+        if (update_rc) oracle_rcrit(x, v, m, M_star, N, dt, G, n1, n2, rcrit);
+        oracle_accel(x, m, rcrit, N, n_active, G, kind, NULL, 0, acc, NULL, NULL);
+        for (int64_t i = 0; i < 3 * N; ++i) v[i] = v[i] + (0.5 * dt) * acc[i];
+    }
+    return nfail;
+}
+
+/* ------------------------------------------------------------------------------------------
+ * Diagnostics.  E = H_A + H_B + H_C with the K terms cancelling (Eq. 4-6):
+ *   E = sum 1/2 m_i v_i^2 + |sum m_i v_i|^2/(2 M_star) - sum G M_star m_i/r_i
+ *       - sum_{i<j} G m_i m_j / r_ij
+ * L = sum m_i x_i cross v_i.   out = {E, Lx, Ly, Lz, T_bodies, T_star, U_star, U_mutual}.
+ * Bodies with m == 0 contribute nothing.
+ * ------------------------------------------------------------------------------------------ */
+void oracle_diagnostics(const double *x, const double *v, const double *m, double M_star,
+                        int64_t N, double G, double *out) {
+    double T = 0, Tc = 0, Us = 0, Usc = 0;
+    double p[3] = {0, 0, 0}, pc[3] = {0, 0, 0}, L[3] = {0, 0, 0}, Lc[3] = {0, 0, 0};
+    for (int64_t i = 0; i < N; ++i) {
+        const double *xi = x + 3 * i, *vi = v + 3 * i;
+        double v2 = (vi[0] * vi[0] + vi[1] * vi[1]) + vi[2] * vi[2];
+        double r = sqrt((xi[0] * xi[0] + xi[1] * xi[1]) + xi[2] * xi[2]);
+        neumaier_add(&T, &Tc, 0.5 * m[i] * v2);
+        if (m[i] != 0.0) neumaier_add(&Us, &Usc, -G * M_star * m[i] / r);
+        for (int k = 0; k < 3; ++k) neumaier_add(&p[k], &pc[k], m[i] * vi[k]);
+        neumaier_add(&L[0], &Lc[0], m[i] * (xi[1] * vi[2] - xi[2] * vi[1]));
+        neumaier_add(&L[1], &Lc[1], m[i] * (xi[2] * vi[0] - xi[0] * vi[2]));
+        neumaier_add(&L[2], &Lc[2], m[i] * (xi[0] * vi[1] - xi[1] * vi[0]));
+    }
+    /* mutual potential: one compensated row sum per i (parallel over i), rows added in index order */
+    double *row = (double *)calloc((size_t)(N > 0 ? N : 1), sizeof(double));
+#pragma omp parallel for schedule(dynamic, 16)
+    for (int64_t i = 0; i < N; ++i) {
+        if (m[i] == 0.0) continue;
+        double si = 0, ci = 0;
+        for (int64_t j = i + 1; j < N; ++j) {
+            if (m[j] == 0.0) continue;
+            double dx = x[3 * j] - x[3 * i], dy = x[3 * j + 1] - x[3 * i + 1],
+                   dz = x[3 * j + 2] - x[3 * i + 2];
+            double r = sqrt((dx * dx + dy * dy) + dz * dz);
+            neumaier_add(&si, &ci, -G * m[i] * m[j] / r);
+        }
+        row[i] = si + ci;
+    }
+    double Um = 0, Umc = 0;
+    for (int64_t i = 0; i < N; ++i) neumaier_add(&Um, &Umc, row[i]);
+    free(row);
+    double px = p[0] + pc[0], py = p[1] + pc[1], pz = p[2] + pc[2];
+    double Ts = ((px * px + py * py) + pz * pz) / (2.0 * M_star);
+    out[4] = T + Tc; out[5] = Ts; out[6] = Us + Usc; out[7] = Um + Umc;
+    out[0] = ((out[4] + out[5]) + out[6]) + out[7];
+    out[1] = L[0] + Lc[0]; out[2] = L[1] + Lc[1]; out[3] = L[2] + Lc[2];
+}

@@ -1,0 +1,514 @@
+"""Pins for the CPU oracle (-m "not gpu").
+
+Each test ties one oracle function to something OTHER than the oracle's own formula:
+closed forms from textbooks, conservation laws, library routines on special cases, brute
+force on tiny inputs.  SURVEY.md section 8(c) pins P1..P12; citations are PAPER.md lines.
+"""
+import math
+
+import numpy as np
+import pytest
+from scipy.optimize import brentq
+from scipy.spatial import cKDTree
+
+import nb_inputs as nbi
+import oracle
+
+G = nbi.G_GAUSS
+
+
+def _golden_factors():
+    import os
+    out = {}
+    with open(os.path.join(os.path.dirname(__file__), "golden", "eq7_safety_factors.txt")) as f:
+        for line in f:
+            if line.startswith("#") or not line.strip():
+                continue
+            k, v = line.split()
+            out[k] = float(v)
+    return out
+
+
+# ---------------------------------------------------------------- P1: changeover W
+@pytest.mark.parametrize("kind", [0, 1])
+def test_P1_changeover_endpoints_symmetry_monotone(kind):
+    rc = 0.0371
+    assert oracle.changeover(0.1 * rc, rc, kind) == 0.0          # "ranging from 0 ..."
+    assert oracle.changeover(0.05 * rc, rc, kind) == 0.0
+    assert oracle.changeover(0.0, rc, kind) == 0.0
+    assert oracle.changeover(rc, rc, kind) == 1.0                # "... to 1", starts to act at rc
+    assert oracle.changeover(7.0 * rc, rc, kind) == 1.0
+    assert oracle.changeover(1.0, 0.0, kind) == 1.0              # rc = 0: plain Newtonian
+    assert abs(oracle.changeover(0.55 * rc, rc, kind) - 0.5) < 1e-15
+    ys = np.linspace(0.0, 1.0, 10001)
+    w = np.array([oracle.changeover((0.1 + 0.9 * y) * rc, rc, kind) for y in ys])
+    assert np.all(np.diff(w) >= 0.0)                             # monotone
+    assert np.all((w >= 0.0) & (w <= 1.0))
+    assert np.max(np.abs(w + w[::-1] - 1.0)) < 2e-15             # W(y) + W(1-y) = 1
+    # smooth: the one-sided slopes at both ends vanish (C^1 junction with the constants)
+    h = 1e-6
+    assert oracle.changeover((0.1 + 0.9 * h) * rc, rc, kind) < 10 * h * h
+    assert 1.0 - oracle.changeover((1.0 - 0.9 * h) * rc, rc, kind) < 10 * h * h
+
+
+# ---------------------------------------------------------------- P2: kick with W == 1
+def test_P2_two_body_closed_form():
+    x, v, m = nbi.two_body(m1=3e-6, m2=5e-4, sep=0.02, direction=(0.6, 0.0, 0.8))
+    acc, _, ns = oracle.accel(x, m, None, G)
+    r = 0.02
+    d = np.array([0.6, 0.0, 0.8])
+    assert ns == 0
+    np.testing.assert_allclose(acc[0], G * m[1] / r**2 * d, rtol=4e-15)     # towards body 1
+    np.testing.assert_allclose(acc[1], -G * m[0] / r**2 * d, rtol=4e-15)
+
+
+def test_P2_regular_polygon_closed_form():
+    # n equal masses on a circle of radius R: every body is pulled to the centre with
+    # |a| = G m / (4 R^2) * sum_{k=1}^{n-1} 1/sin(pi k/n)   (textbook n-gon / Lagrange ring)
+    n, R, mm = 7, 0.83, 2.5e-7
+    th = 2 * math.pi * np.arange(n) / n + 0.3
+    c = np.array([1.3, -0.4, 0.2])
+    x = np.stack([R * np.cos(th), R * np.sin(th), np.zeros(n)], axis=1) + c
+    m = np.full(n, mm)
+    acc, _, _ = oracle.accel(x, m, None, G)
+    amag = G * mm / (4 * R * R) * sum(1.0 / math.sin(math.pi * k / n) for k in range(1, n))
+    for i in range(n):
+        inward = (c - x[i]) / R
+        np.testing.assert_allclose(acc[i], amag * inward, rtol=1e-13, atol=1e-13 * amag)
+    # a massless probe at the centre feels nothing; on the axis it feels the ring formula
+    xp = np.vstack([x, c, c + np.array([0, 0, 0.5])])
+    mp = np.concatenate([m, [0.0, 0.0]])
+    accp, _, _ = oracle.accel(xp, mp, None, G)
+    assert np.linalg.norm(accp[n]) < 1e-14 * amag
+    z = 0.5
+    np.testing.assert_allclose(accp[n + 1], [0, 0, -G * n * mm * z / (z * z + R * R) ** 1.5],
+                               rtol=1e-13, atol=1e-14 * amag)
+
+
+def test_P2_force_is_minus_gradient_of_mutual_potential():
+    # m_i a_i = -dU/dx_i with U = -sum_{i<j} G m_i m_j / r_ij (Eq. 5 with K == 1), U from the
+    # oracle's own energy diagnostic: ties sign, index and mass (m_j, not m_i) of the kick to it.
+    x, v, m = nbi.random_cluster(9, seed=3, scale=0.5)
+    acc, _, _ = oracle.accel(x, m, None, G)
+    h = 1e-5
+    for i in (0, 4, 8):
+        for c in range(3):
+            xp, xm = x.copy(), x.copy()
+            xp[i, c] += h
+            xm[i, c] -= h
+            up = oracle.diagnostics(xp, v, m, 1.0, G)["U_mutual"]
+            um = oracle.diagnostics(xm, v, m, 1.0, G)["U_mutual"]
+            grad = (up - um) / (2 * h)
+            assert abs(m[i] * acc[i, c] + grad) < 1e-6 * np.abs(m[i] * acc[i]).max()
+
+
+def test_P2_random_vs_longdouble_restatement():
+    # secondary check (a restatement, so not counted as a pin on its own)
+    x, v, m = nbi.random_cluster(64, seed=11)
+    acc, _, _ = oracle.accel(x, m, None, G)
+    xl = x.astype(np.longdouble)
+    d = xl[None, :, :] - xl[:, None, :]
+    r2 = (d * d).sum(-1)
+    np.fill_diagonal(r2, 1.0)
+    w = (np.longdouble(G) * m.astype(np.longdouble))[None, :] / (r2 * np.sqrt(r2))
+    np.fill_diagonal(w, 0.0)
+    ref = (w[:, :, None] * d).sum(1)
+    np.testing.assert_allclose(acc, ref.astype(np.float64), rtol=2e-15, atol=0)
+
+
+# ---------------------------------------------------------------- P3: invariants with W active
+@pytest.mark.parametrize("kind", [0, 1])
+def test_P3_newton_third_law_and_zero_torque_with_changeover(kind):
+    d = nbi.make_config(2, n_override=1500)        # encounter-dense ring, power-law masses
+    rc = oracle.rcrit(d.x, d.v, d.m, d.M_star, d.dt, G, 3.0, 0.4)   # full Eq. 7: many in-range pairs
+    sure, _ = oracle.pairs(d.x, rc)
+    assert len(sure) > 50
+    acc, ab, _ = oracle.accel(d.x, d.m, rc, G, kind=kind, want_abs=True)
+    scale = (d.m[:, None] * np.abs(acc)).sum()
+    assert np.abs((d.m[:, None] * acc).sum(0)).max() <= 1e-14 * scale          # sum m a = 0
+    tau = (d.m[:, None] * np.cross(d.x, acc)).sum(0)
+    assert np.abs(tau).max() <= 1e-13 * scale                                  # central forces
+    # and the changeover really removed something
+    acc1, _, _ = oracle.accel(d.x, d.m, None, G)
+    assert np.abs(acc1 - acc).max() > 1e-3 * np.abs(acc1).max()
+
+
+def test_P3_changeover_weights_the_force_of_one_pair():
+    # one pair inside the shell: |a| = W(r) G m_j / r^2 exactly (S3: weight multiplies the force)
+    rc = 0.05
+    for frac in (0.05, 0.1, 0.3, 0.55, 0.9, 1.0, 1.7):
+        x, v, m = nbi.two_body(m1=1e-6, m2=4e-6, sep=frac * rc)
+        acc, _, _ = oracle.accel(x, m, np.array([rc, 0.2 * rc]), G)
+        w = oracle.changeover(frac * rc, rc, 0)
+        full = G * m[1] / (frac * rc) ** 2
+        assert np.isclose(np.linalg.norm(acc[0]), w * full, rtol=1e-14, atol=1e-14 * full)
+
+
+def test_P3_semi_active_rows_feel_only_active_bodies():
+    d = nbi.make_config(3, n_override=1024)        # 8 embryos + 1016 test masses
+    na = d.n_active
+    assert na == 8 and np.all(d.m[na:] == 0)
+    rc = np.zeros(d.N)
+    acc_semi, _, _ = oracle.accel(d.x, d.m, rc, G, n_active=na)
+    # massless bodies exert nothing, so the full sum over all j is the same thing
+    acc_full, _, _ = oracle.accel(d.x, d.m, rc, G, n_active=0)
+    np.testing.assert_allclose(acc_semi, acc_full, rtol=0, atol=0)
+    # with the planetesimals given mass, semi-active still ignores them as sources
+    m2 = d.m.copy()
+    m2[na:] = 1e-9
+    acc2, _, _ = oracle.accel(d.x, m2, rc, G, n_active=na)
+    np.testing.assert_allclose(acc2, acc_semi, rtol=0, atol=0)
+    rows = np.array([0, 5, 9, 1000])
+    accr, _, _ = oracle.accel(d.x, d.m, rc, G, n_active=na, rows=rows)
+    np.testing.assert_array_equal(accr, acc_semi[rows])
+
+
+# ---------------------------------------------------------------- P4: r_crit (Eq. 7)
+def test_P4_rcrit_closed_forms_and_crossover():
+    f = _golden_factors()
+    n1, n2 = f["n1"], f["n2"]
+    assert (n1, n2) == (3.0, 0.4)
+    a = np.array([0.5, 1.0, 2.5, 5.2])
+    m = np.array([1e-9, 3e-6, 1e-7, 1e-3])
+    M = 1.0
+    vc = np.sqrt(G * M / a)
+    x = np.stack([a, 0 * a, 0 * a], 1)
+    v = np.stack([0 * a, vc, 0 * a], 1)
+    dt = 6.0
+    hill = n1 * a * np.cbrt(m / (3 * M))
+    vel = n2 * dt * vc
+    rc = oracle.rcrit(x, v, m, M, dt, G, n1, n2)
+    np.testing.assert_allclose(rc, np.maximum(hill, vel), rtol=1e-14)
+    assert (hill > vel).any() and (hill < vel).any()             # both branches of the max
+    np.testing.assert_allclose(oracle.rcrit(x, v, m, M, dt, G, n1, 0.0), hill, rtol=1e-14)
+    np.testing.assert_allclose(oracle.rcrit(x, v, m, M, -dt, G, 0.0, n2), vel, rtol=1e-14)
+    # crossover mass where both terms are equal: m* = 3 M (n2 dt v / (n1 a))^3
+    a0 = 1.0
+    v0 = math.sqrt(G * M / a0)
+    mstar = 3 * M * (n2 * dt * v0 / (n1 * a0)) ** 3
+    for fac, which in ((0.9, "vel"), (1.1, "hill")):
+        r1 = oracle.rcrit(np.array([[a0, 0, 0.0]]), np.array([[0, v0, 0.0]]), np.array([fac * mstar]), M, dt, G, n1, n2)[0]
+        expect = n2 * dt * v0 if which == "vel" else n1 * a0 * (fac * mstar / (3 * M)) ** (1 / 3)
+        assert np.isclose(r1, expect, rtol=1e-14)
+    # eccentric body: a from vis-viva, not r
+    aa, ee = 2.0, 0.3
+    xe, ve = nbi.elements_to_cartesian([aa], [ee], [0.1], [0.3], [0.4], [1.0], G * M)
+    r1 = oracle.rcrit(xe, ve, np.array([1e-5]), M, dt, G, n1, 0.0)[0]
+    assert np.isclose(r1, n1 * aa * (1e-5 / 3) ** (1 / 3), rtol=1e-12)
+    # unbound body falls back to r; massless body has zero Hill radius
+    xu = np.array([[1.0, 0, 0]]); vu = np.array([[0, 3 * math.sqrt(G), 0.0]])
+    assert np.isclose(oracle.rcrit(xu, vu, np.array([3e-6]), M, dt, G, n1, 0.0)[0], n1 * 1.0 * (1e-6) ** (1 / 3), rtol=1e-14)
+    assert oracle.rcrit(xu, vu, np.array([0.0]), M, dt, G, n1, 0.0)[0] == 0.0
+
+
+# ---------------------------------------------------------------- P5: pairs
+def test_P5_chain_counts():
+    N = 37
+    x, v, m = nbi.chain_1d(N, spacing=1.0)
+    s, b = oracle.pairs(x, np.full(N, 1.5))
+    assert len(s) == N - 1 and len(b) == 0
+    s, b = oracle.pairs(x, np.full(N, 2.5))
+    assert len(s) == 2 * N - 3 and len(b) == 0
+    # max rule (S4): only ONE body with a big radius still pairs with both its neighbours
+    rc = np.full(N, 0.1)
+    rc[10] = 1.5
+    s, b = oracle.pairs(x, rc)
+    assert s.tolist() == [[9, 10], [10, 11]]
+    # strict '<' (S11) and the borderline bucket: spacing exactly equal to rc
+    s, b = oracle.pairs(x, np.full(N, 1.0))
+    assert len(s) == 0 and len(b) == N - 1
+
+
+def test_P5_cubic_lattice_counts():
+    n = 5
+    x, v, m = nbi.cubic_lattice(n)
+    N = n**3
+    edges = 3 * n * n * (n - 1)
+    face_diag = 3 * 2 * n * (n - 1) ** 2
+    body_diag = 4 * (n - 1) ** 3
+    assert len(oracle.pairs(x, np.full(N, 1.2))[0]) == edges
+    assert len(oracle.pairs(x, np.full(N, 1.5))[0]) == edges + face_diag
+    assert len(oracle.pairs(x, np.full(N, 1.8))[0]) == edges + face_diag + body_diag
+
+
+def test_P5_kdtree_equal_radius_and_max_rule():
+    d = nbi.make_config(2, n_override=2048)
+    rc0 = 4e-3
+    s, b = oracle.pairs(d.x, np.full(d.N, rc0))
+    ref = cKDTree(d.x).query_pairs(rc0, output_type="ndarray")
+    ref = np.unique(np.sort(ref, axis=1), axis=0).astype(np.int32)
+    assert len(ref) > 30
+    assert len(b) == 0 and np.array_equal(s, ref)
+    # per-body radii: candidates from the tree at the largest radius, filtered by max(rc_i, rc_j)
+    rc = oracle.rcrit(d.x, d.v, d.m, d.M_star, d.dt, G, 3.0, 0.4)
+    cand = cKDTree(d.x).query_pairs(rc.max() * (1 + 1e-9), output_type="ndarray")
+    cand = np.sort(cand, axis=1)
+    dist = np.linalg.norm(d.x[cand[:, 0]] - d.x[cand[:, 1]], axis=1)
+    thr = np.maximum(rc[cand[:, 0]], rc[cand[:, 1]])
+    clear = np.abs(dist / thr - 1) > 1e-9
+    ref = np.unique(cand[(dist < thr) & clear], axis=0).astype(np.int32)
+    s, b = oracle.pairs(d.x, rc)
+    assert len(b) == 0 and np.array_equal(s, ref)
+    # rows interface returns exactly the pairs incident to those rows
+    rows = np.array([3, 77, 1500])
+    sr, _ = oracle.pairs(d.x, rc, rows=rows)
+    inc = s[np.isin(s[:, 0], rows) | np.isin(s[:, 1], rows)]
+    assert np.array_equal(sr, inc)
+
+
+def test_P5_borderline_bucket():
+    rc = 0.01
+    for eps, where in ((-1e-9, "sure"), (-1e-13, "border"), (1e-13, "border"), (1e-9, "out")):
+        x, v, m = nbi.two_body(sep=rc * (1 + eps), direction=(1, 0, 0), center=(1.0, 0, 0))
+        s, b = oracle.pairs(x, np.array([rc, 0.0]))
+        got = "sure" if len(s) else ("border" if len(b) else "out")
+        assert got == where, (eps, got)
+
+
+def test_P5_semi_active_pairs_need_an_active_member():
+    N = 12
+    x, v, m = nbi.chain_1d(N, spacing=1.0)
+    s, b = oracle.pairs(x, np.full(N, 1.5), n_active=3)
+    # active = {0,1,2}: (0,1), (1,2), (2,3) only
+    assert s.tolist() == [[0, 1], [1, 2], [2, 3]]
+    sr, _ = oracle.pairs(x, np.full(N, 1.5), n_active=3, rows=np.array([3, 7]))
+    assert sr.tolist() == [[2, 3]]
+
+
+# ---------------------------------------------------------------- P6/P7: Kepler drift
+def _random_orbits(n, seed, emax=0.9):
+    rng = np.random.default_rng(seed)
+    a = rng.uniform(0.3, 6.0, n)
+    e = rng.uniform(0.0, emax, n)
+    inc = rng.uniform(0, 1.0, n)
+    w, O, M = (rng.uniform(0, 2 * math.pi, n) for _ in range(3))
+    x, v = nbi.elements_to_cartesian(a, e, inc, w, O, M, G)
+    return a, e, inc, w, O, M, x, v
+
+
+def test_P6_drift_conserves_kepler_integrals():
+    a, e, inc, w, O, M, x, v = _random_orbits(2000, 5)
+    x1, v1, nf = oracle.drift_kepler(x, v, 1.0, 6.0, G)
+    assert nf == 0
+    en0 = 0.5 * (v * v).sum(1) - G / np.linalg.norm(x, axis=1)
+    en1 = 0.5 * (v1 * v1).sum(1) - G / np.linalg.norm(x1, axis=1)
+    assert np.max(np.abs(en1 / en0 - 1)) < 2e-13 / (1 - 0.9)
+    h0, h1 = np.cross(x, v), np.cross(x1, v1)
+    assert np.max(np.linalg.norm(h1 - h0, axis=1) / np.linalg.norm(h0, axis=1)) < 1e-13
+    ev0 = np.cross(v, h0) / G - x / np.linalg.norm(x, axis=1)[:, None]
+    ev1 = np.cross(v1, h1) / G - x1 / np.linalg.norm(x1, axis=1)[:, None]
+    assert np.max(np.linalg.norm(ev1 - ev0, axis=1)) < 5e-13
+
+
+def test_P7_circular_orbit_and_full_period():
+    a = 1.7
+    n = math.sqrt(G / a**3)
+    x = np.array([[a, 0, 0.0]]); v = np.array([[0, a * n, 0.0]])
+    for t in (0.5, 6.0, 100.0, 5000.0):
+        x1, v1, _ = oracle.drift_kepler(x, v, 1.0, t, G)
+        np.testing.assert_allclose(x1[0], [a * math.cos(n * t), a * math.sin(n * t), 0], atol=4e-15 * a * max(1, n * t))
+        np.testing.assert_allclose(v1[0], [-a * n * math.sin(n * t), a * n * math.cos(n * t), 0], atol=4e-15 * a * n * max(1, n * t))
+    # exactly one period returns the initial state (exercises the 2 pi reduction)
+    aa, ee, *_rest, xs, vs = _random_orbits(50, 9)
+    for k in range(50):
+        P = 2 * math.pi / math.sqrt(G / aa[k] ** 3)
+        x1, v1, _ = oracle.kepler_one(xs[k], vs[k], G, P)
+        assert np.linalg.norm(x1 - xs[k]) < 2e-13 * aa[k] / (1 - ee[k]) ** 2
+        x3, v3, _ = oracle.kepler_one(xs[k], vs[k], G, -3 * P)
+        assert np.linalg.norm(x3 - xs[k]) < 6e-13 * aa[k] / (1 - ee[k]) ** 2
+
+
+def test_P7_independent_route_through_elements():
+    # elements -> M0 + n dt -> Kepler's equation by a LIBRARY root finder -> x, v
+    a, e, inc, w, O, M, x, v = _random_orbits(300, 21, emax=0.1)
+    for dt in (6.0, -3.0, 10.0):
+        x1, v1, nf = oracle.drift_kepler(x, v, 1.0, dt, G)
+        assert nf == 0
+        n = np.sqrt(G / a**3)
+        M1 = M + n * dt
+        E1 = np.array([brentq(lambda E: E - ee * math.sin(E) - mm, mm - 1.5, mm + 1.5, xtol=1e-15, rtol=1e-15)
+                       for ee, mm in zip(e, M1)])
+        cE, sE = np.cos(E1), np.sin(E1)
+        b = np.sqrt(1 - e * e)
+        xp, yp = a * (cE - e), a * b * sE
+        rr = 1 - e * cE
+        vxp, vyp = -a * n * sE / rr, a * n * b * cE / rr
+        cw, sw, cO, sO, ci, si = np.cos(w), np.sin(w), np.cos(O), np.sin(O), np.cos(inc), np.sin(inc)
+        R = np.array([[cO * cw - sO * sw * ci, -cO * sw - sO * cw * ci],
+                      [sO * cw + cO * sw * ci, -sO * sw + cO * cw * ci],
+                      [sw * si, cw * si]])
+        xr = (R[:, 0] * xp + R[:, 1] * yp).T
+        vr = (R[:, 0] * vxp + R[:, 1] * vyp).T
+        assert np.max(np.linalg.norm(x1 - xr, axis=1) / np.linalg.norm(xr, axis=1)) < 1e-13
+        assert np.max(np.linalg.norm(v1 - vr, axis=1) / np.linalg.norm(vr, axis=1)) < 1e-13
+
+
+def test_P7_group_property_and_inverse():
+    a, e, inc, w, O, M, x, v = _random_orbits(500, 33, emax=0.6)
+    xa, va, _ = oracle.drift_kepler(x, v, 1.0, 2.5, G)
+    xb, vb, _ = oracle.drift_kepler(xa, va, 1.0, 3.5, G)
+    xc, vc, _ = oracle.drift_kepler(x, v, 1.0, 6.0, G)
+    assert np.max(np.linalg.norm(xb - xc, axis=1) / np.linalg.norm(xc, axis=1)) < 2e-13
+    xd, vd, _ = oracle.drift_kepler(xc, vc, 1.0, -6.0, G)
+    assert np.max(np.linalg.norm(xd - x, axis=1) / np.linalg.norm(x, axis=1)) < 2e-13
+    assert np.max(np.linalg.norm(vd - v, axis=1) / np.linalg.norm(v, axis=1)) < 2e-13
+
+
+def test_P7_elliptic_and_universal_solvers_agree():
+    a, e, inc, w, O, M, x, v = _random_orbits(500, 44, emax=0.9)
+    for dt in (6.0, 400.0, -37.0):
+        x1, v1, nf1 = oracle.drift_kepler(x, v, 1.0, dt, G, solver=0)
+        x2, v2, nf2 = oracle.drift_kepler(x, v, 1.0, dt, G, solver=1)
+        assert nf1 == 0 and nf2 == 0
+        tol = 5e-13 * max(1.0, abs(dt) / 50) / (1 - 0.9)
+        assert np.max(np.linalg.norm(x1 - x2, axis=1) / np.linalg.norm(x1, axis=1)) < tol
+
+
+def test_P7_hyperbolic_closed_form():
+    # unbound body (alpha < 0): compare with the hyperbolic Kepler equation solved by brentq
+    mu = G
+    a, e = -1.5, 1.8                          # a < 0
+    n = math.sqrt(mu / (-a) ** 3)
+
+    def state(Mh):
+        H = brentq(lambda H: e * math.sinh(H) - H - Mh, -20, 20, xtol=1e-15, rtol=1e-15)
+        r = -a * (e * math.cosh(H) - 1)
+        xx = -a * (e - math.cosh(H))
+        yy = -a * math.sqrt(e * e - 1) * math.sinh(H)
+        vx = -math.sqrt(-mu * a) * math.sinh(H) / r
+        vy = math.sqrt(-mu * a) * math.sqrt(e * e - 1) * math.cosh(H) / r
+        return np.array([xx, yy, 0.0]), np.array([vx, vy, 0.0])
+
+    x0, v0 = state(-0.4)
+    assert 0.5 * v0 @ v0 - mu / np.linalg.norm(x0) > 0
+    for dt in (5.0, 60.0, -20.0):
+        xr, vr = state(-0.4 + n * dt)
+        x1, v1, nf = oracle.drift_kepler(x0[None], v0[None], 1.0, dt, G)
+        assert nf == 0
+        assert np.linalg.norm(x1[0] - xr) < 1e-13 * np.linalg.norm(xr)
+        assert np.linalg.norm(v1[0] - vr) < 1e-13 * np.linalg.norm(vr)
+
+
+# ---------------------------------------------------------------- P8: H_C shift (Eq. 6)
+def test_P8_shift_closed_forms():
+    x = np.array([[1.0, 0, 0], [0, 2.0, 0]])
+    m = np.array([2e-3, 1e-3])
+    v = np.array([[0.0, 0.01, 0.0], [0.0, -0.02, 0.0]])          # opposite momenta
+    np.testing.assert_array_equal(oracle.shift(x, v, m, 1.0, 3.0), x)
+    v = np.array([[0.01, 0.0, 0.002], [0.0, 0.03, 0.0]])
+    M = 0.8
+    s = (m[:, None] * v).sum(0) / M
+    np.testing.assert_allclose(oracle.shift(x, v, m, M, 3.0), x + 3.0 * s, rtol=1e-15)
+    # L = sum m x cross v is unchanged by the shift: sum m (dt s) x v = dt s x P = 0 since s || P
+    d = nbi.make_config(0, n_override=300)
+    L0 = oracle.diagnostics(d.x, d.v, d.m, 1.0, G)["L"]
+    x1 = oracle.shift(d.x, d.v, d.m, 1.0, 50.0)
+    L1 = oracle.diagnostics(x1, d.v, d.m, 1.0, G)["L"]
+    assert np.linalg.norm(L1 - L0) < 1e-14 * np.linalg.norm(L0)
+
+
+# ---------------------------------------------------------------- P9..P12: the step
+def test_P9_single_planet_reduces_to_kepler_with_total_mass_order_two():
+    # star + ONE massive planet in democratic coordinates: H_A + H_C = p^2/2 (1/m + 1/m0) - G m m0/r,
+    # i.e. the relative orbit is a Kepler orbit with mu = G (m0 + m): closed form for x(t).
+    M, m = 1.0, 1e-2
+    a, e = 1.0, 0.2
+    xh, vh = nbi.elements_to_cartesian([a], [e], [0.2], [0.5], [0.7], [0.3], G * (M + m))
+    vb = vh * M / (M + m)                                      # barycentric velocity of the planet
+    T = 96.0
+    n = math.sqrt(G * (M + m) / a**3)
+    xr, _ = nbi.elements_to_cartesian([a], [e], [0.2], [0.5], [0.7], [0.3 + n * T], G * (M + m))
+    errs = []
+    for nst in (8, 16, 32):
+        r = oracle.step(xh, vb, np.array([m]), M, T / nst, G, nst, n1=0.0, n2=0.0, rcrit_=np.zeros(1))
+        errs.append(np.linalg.norm(r["x"][0] - xr[0]))
+    assert errs[0] < 1e-3 and errs[2] > 1e-9                    # a splitting error exists, and is small
+    assert 3.6 < errs[0] / errs[1] < 4.4 and 3.6 < errs[1] / errs[2] < 4.4   # second order
+    # mass-less planet: the step IS the Kepler flow about M (H_B = 0, H_C = 0)
+    xb, vbb = nbi.elements_to_cartesian([a], [e], [0.2], [0.5], [0.7], [0.3], G * M)
+    r = oracle.step(xb, vbb, np.array([0.0]), M, 6.0, G, 16, rcrit_=np.zeros(1), n1=0.0, n2=0.0)
+    xr2, vr2 = nbi.elements_to_cartesian([a], [e], [0.2], [0.5], [0.7], [0.3 + math.sqrt(G * M / a**3) * 96.0], G * M)
+    assert np.linalg.norm(r["x"][0] - xr2[0]) < 1e-13
+
+
+def _giants():
+    d = nbi.make_config(1, n_override=0)                       # just the two giants
+    assert d.N == 2
+    return d
+
+
+def test_P10_energy_bounded_and_second_order():
+    d = _giants()
+    E0 = oracle.diagnostics(d.x, d.v, d.m, 1.0, G)["E"]
+    out = {}
+    for dt in (24.0, 12.0):
+        errs = []
+        x, v = d.x, d.v
+        nchunk = 20
+        per = int(round(48000 / dt / nchunk))
+        for _ in range(nchunk):
+            r = oracle.step(x, v, d.m, 1.0, dt, G, per, n1=0.0, n2=0.0, rcrit_=np.zeros(2))
+            x, v = r["x"], r["v"]
+            errs.append((oracle.diagnostics(x, v, d.m, 1.0, G)["E"] - E0) / E0)
+        out[dt] = np.array(errs)
+    assert np.max(np.abs(out[24.0])) < 1e-6
+    # bounded (no secular drift): second half no worse than the first
+    assert np.max(np.abs(out[24.0][10:])) < 2.0 * np.max(np.abs(out[24.0][:10])) + 1e-12
+    ratio = np.max(np.abs(out[24.0])) / np.max(np.abs(out[12.0]))
+    assert 3.0 < ratio < 5.0
+
+
+def test_P11_angular_momentum_conserved_with_changeover_active():
+    d = nbi.make_config(2, n_override=400)
+    L0 = oracle.diagnostics(d.x, d.v, d.m, 1.0, G)["L"]
+    r = oracle.step(d.x, d.v, d.m, 1.0, d.dt, G, 1000, n1=3.0, n2=0.4)
+    s, _ = oracle.pairs(r["x"], r["rcrit"])
+    assert len(s) > 0                                           # changeover really active
+    L1 = oracle.diagnostics(r["x"], r["v"], d.m, 1.0, G)["L"]
+    assert np.linalg.norm(L1 - L0) <= 1e-13 * np.linalg.norm(L0)
+    assert r["n_fail"] == 0
+
+
+def test_P12_time_reversibility():
+    d = nbi.make_config(0, n_override=256)
+    rc = oracle.rcrit(d.x, d.v, d.m, 1.0, d.dt, G, 3.0, 0.0)     # fixed radii (n1 = n2 = 0 below)
+    f = oracle.step(d.x, d.v, d.m, 1.0, d.dt, G, 20, n1=0.0, n2=0.0, rcrit_=rc)
+    b = oracle.step(f["x"], f["v"], d.m, 1.0, -d.dt, G, 20, n1=0.0, n2=0.0, rcrit_=rc)
+    assert np.max(np.abs(b["x"] - d.x)) < 1e-12
+    assert np.max(np.abs(b["v"] - d.v)) < 1e-13
+    # and a step really moved things
+    assert np.max(np.abs(f["x"] - d.x)) > 0.1
+
+
+def test_step_equals_its_parts():
+    # oracle_step is exactly the composition of the separately pinned pieces (S6, S17)
+    d = nbi.make_config(0, n_override=128)
+    dt = d.dt
+    r = oracle.step(d.x, d.v, d.m, 1.0, dt, G, 2, n1=3.0, n2=0.4)
+    x, v = d.x.copy(), d.v.copy()
+    rc = oracle.rcrit(x, v, d.m, 1.0, dt, G, 3.0, 0.4)
+    acc, _, _ = oracle.accel(x, d.m, rc, G)
+    for _ in range(2):
+        v = v + (0.5 * dt) * acc
+        x = oracle.shift(x, v, d.m, 1.0, 0.5 * dt)
+        x, v, _ = oracle.drift_kepler(x, v, 1.0, dt, G)
+        x = oracle.shift(x, v, d.m, 1.0, 0.5 * dt)
+        rc = oracle.rcrit(x, v, d.m, 1.0, dt, G, 3.0, 0.4)
+        acc, _, _ = oracle.accel(x, d.m, rc, G)
+        v = v + (0.5 * dt) * acc
+    np.testing.assert_array_equal(r["x"], x)
+    np.testing.assert_array_equal(r["v"], v)
+    np.testing.assert_array_equal(r["acc"], acc)
+    np.testing.assert_array_equal(r["rcrit"], rc)
+
+
+def test_diagnostics_closed_form():
+    # two bodies, hand values (Eq. 4-6 with K terms cancelling)
+    x = np.array([[1.0, 0, 0], [0, 2.0, 0]]); v = np.array([[0, 0.01, 0], [0.02, 0, 0.0]])
+    m = np.array([1e-3, 2e-3]); M = 1.5
+    dg = oracle.diagnostics(x, v, m, M, G)
+    T = 0.5 * (1e-3 * 1e-4 + 2e-3 * 4e-4)
+    p = np.array([2e-3 * 0.02, 1e-3 * 0.01, 0])
+    E = T + p @ p / (2 * M) - G * M * (1e-3 / 1 + 2e-3 / 2) - G * 2e-6 / math.sqrt(5)
+    assert np.isclose(dg["E"], E, rtol=1e-14)
+    np.testing.assert_allclose(dg["L"], [0, 0, 1e-3 * 0.01 - 2e-3 * 2 * 0.02], rtol=1e-14)
