@@ -1,0 +1,177 @@
+/*
+ * nbkick.h -- C ABI of libnbkick.so: the data-parallel hot path of the hybrid symplectic
+ * planet-formation integrator of Grimm & Stadel (arxiv 2604.09184; cited as PAPER.md:<line>),
+ * hand-written CUDA for NVIDIA B200 (sm_100a).  One GPU, no sharding, no CPU fallback.
+ *
+ * State ("democratic coordinates"): heliocentric positions x[N,3], barycentric
+ * velocities v[N,3], masses m[N] of the N non-star bodies; the star (mass M_star) sits at the
+ * origin and is not in the arrays.  Everything is fp64, contiguous, row-major.  Pair indices
+ * are int32.  Units are the caller's; G is set with nb_configure (default: Gaussian k^2 in
+ * AU, day, solar mass).
+ *
+ * Pointers.  Every array argument of the nb_* calls below is a DEVICE pointer unless the
+ * function name ends in _host (those take HOST pointers and copy in and out themselves).
+ * Ownership: the caller owns every buffer, including the scratch workspace handed over with
+ * nb_configure; the library allocates no device memory in the device-pointer calls.  (The
+ * _host calls keep one private, lazily grown device arena, released by nb_release.)
+ *
+ * Asynchrony.  Device-pointer calls enqueue work on the configured CUDA stream and return
+ * without synchronising; results are ordered on that stream.  _host calls and nb_status
+ * synchronise the stream before they return.
+ *
+ * Errors.  Every int-returning call returns NB_OK (0) or a negative NB_E_* code for
+ * conditions detectable on the host at call time; nb_last_error() then holds a message.
+ * Conditions only the device can see (pair list overflow, Kepler non-convergence,
+ * non-finite input, coincident bodies) are counted lazily and read with nb_status.
+ *
+ * Semi-active mode (BASELINE.json:north_star; not in the paper): with n_active = A < N the
+ * first A bodies are fully interacting and the remaining N-A "feel but do not exert" force:
+ * the j-sum runs over j < A only, and a pair is listed only if at least one member is active.
+ */
+#ifndef NBKICK_H
+#define NBKICK_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define NB_OK 0
+#define NB_E_NULL (-1)      /* a required pointer is NULL */
+#define NB_E_BADN (-2)      /* N <= 0 or N > 2^31 - 1 */
+#define NB_E_BADARG (-3)    /* non-finite dt, M_star <= 0, n_active > N, nsteps < 0, bad config value */
+#define NB_E_WORKSPACE (-4) /* no workspace configured or it is smaller than nb_workspace_bytes(N) */
+#define NB_E_CUDA (-5)      /* a CUDA runtime call failed (message in nb_last_error) */
+
+/* Changeover shapes for the transition 0.1 r_crit < r < r_crit (PAPER.md:94 says only
+ * "smooth changeover function ranging from 0 to 1"; reading S2). */
+#define NB_CHANGEOVER_RATIONAL 0 /* y^2 / (2y^2 - 2y + 1), y = (r - 0.1 rc) / (0.9 rc) */
+#define NB_CHANGEOVER_QUINTIC 1  /* 10y^3 - 15y^4 + 6y^5 */
+
+/* Process-wide settings.  nb_default_config fills the defaults named below. */
+typedef struct nb_config {
+    void *stream;            /* cudaStream_t the calls enqueue on; NULL = legacy default stream */
+    void *workspace;         /* DEVICE scratch owned by the caller, 256-byte aligned */
+    size_t workspace_bytes;  /* its size; must be >= nb_workspace_bytes(N) of every call */
+    int64_t pair_capacity;   /* rows of the caller's pairs[cap,2] buffer (default 0) */
+    int64_t n_active;        /* semi-active: number of force-exerting bodies; 0 = all N */
+    double G;                /* gravitational constant (default 0.01720209895^2) */
+    double n1;               /* Eq. 7 safety factor on R_Hill (default 3) */
+    double n2;               /* Eq. 7 safety factor on dt*v   (default 0.4) */
+    int changeover_kind;     /* NB_CHANGEOVER_* (default rational) */
+    int i_per_thread;        /* tuning: i-bodies held in registers per thread, 0 = auto (1,2,4) */
+    int j_splits;            /* tuning: number of j-chunks the force grid is split into, 0 = auto */
+    int use_graph;           /* nb_step: replay one captured CUDA graph per step (default 1) */
+} nb_config;
+
+void nb_default_config(nb_config *cfg);
+/* Copies *cfg; validates G > 0, n1,n2 >= 0 and finite, pair_capacity >= 0, n_active >= 0. */
+int nb_configure(const nb_config *cfg);
+/* Bytes of scratch the device-pointer calls need for N bodies under the current tuning. */
+size_t nb_workspace_bytes(int64_t N);
+
+/*
+ * a0 -- critical radius, Eq. 7:  rcrit_i = max(n1 R_Hill,i , n2 |dt| |v_i|),
+ * R_Hill,i = a_i (m_i / (3 M_star))^(1/3), a_i from vis-viva 1/a = 2/r - v^2/(G M_star) with the
+ * stored velocity (a_i = r_i if 1/a <= 0)  [DESIGN.md reading S5].
+ * x,v: [N,3] in; m: [N] in; rcrit: [N] out.
+ */
+int nb_rcrit(const double *x, const double *v, const double *m, double M_star, int64_t N, double dt,
+             double *rcrit);
+
+/*
+ * a1-a4 -- H_B kick (Eq. 5; "H_B describes the N^2 mutual gravitational
+ * force terms"; BASELINE.json:north_star):
+ *     acc_i = sum_{j != i, j < n_active} G m_j W(r_ij; rc_ij) (x_j - x_i) / r_ij^3 ,
+ *     v_i  += dt * acc_i                                  (dt = 0: accelerations and pairs only)
+ * W = kick weight = 1 for r >= rc_ij, 0 for r <= 0.1 rc_ij, changeover_kind between (readings
+ * S1-S3); rc_ij = max(rcrit_i, rcrit_j) (S4).  From the same tiles: every unordered pair with
+ * r_ij < rc_ij (strict, decided in fp64 on r^2 < rc^2) is appended once as (min,max) to pairs
+ * (PAPER.md:94, 98, 106), in unspecified order.
+ *   x [N,3] in; v [N,3] in/out; m [N] in; rcrit [N] in, or NULL => computed internally by a0 from
+ *   (x, v, m, M_star, dt) with the configured n1, n2 into workspace scratch (M_star is used for
+ *   nothing else: H_B has no star term); acc [N,3] out; pairs [pair_capacity,2] int32 out or NULL
+ *   (=> detection skipped); npairs: device int64[1] out, total number of pairs found -- it keeps
+ *   counting past pair_capacity, only the first pair_capacity rows are written (required iff
+ *   pairs != NULL).
+ */
+int nb_kick(const double *x, double *v, const double *m, double M_star, int64_t N, double dt,
+            const double *rcrit, double *acc, int32_t *pairs, int64_t *npairs);
+
+/*
+ * a5 -- H_C (Eq. 6): x_i += dt * (sum_k m_k v_k) / M_star for every body.
+ * The sum is a fixed-shape tree reduction (deterministic, run-to-run reproducible).
+ */
+int nb_shift(double *x, const double *v, const double *m, double M_star, int64_t N, double dt);
+
+/*
+ * a6 -- H_A without encounters ("a Keplerian orbit can be solved analytically";
+ * PAPER.md:84 Eq. 4 first sum): every body follows the Kepler flow about
+ * mu = G M_star for dt, advanced with Gauss' f and g functions (BASELINE.json:north_star).
+ * Bound orbits: Newton on the differenced Kepler equation; otherwise universal variables
+ * (reading S15).  A body whose solver does not converge is left unchanged and counted.
+ * x, v: [N,3] in/out.
+ */
+int nb_drift_kepler(double *x, double *v, double M_star, int64_t N, double dt);
+
+/*
+ * a7 -- nsteps steps of B(dt/2) C(dt/2) A(dt) C(dt/2) B(dt/2) (Eq. 3; order: reading
+ * S6) with the adjacent half-kicks of consecutive steps sharing one force evaluation: one O(N^2)
+ * evaluation per step plus one at the start.  rcrit is recomputed by a0 from the current (x, v)
+ * immediately before every force evaluation (S17) unless n1 == n2 == 0, in which case the
+ * caller's rcrit is used unchanged.  On return acc, rcrit, pairs, npairs are those of the last
+ * evaluation (at the final positions).  nsteps = 0: one evaluation, no motion.
+ *   x, v [N,3] in/out; m [N] in; rcrit [N] in/out; acc [N,3] out; pairs/npairs as in nb_kick.
+ */
+int nb_step(double *x, double *v, const double *m, double M_star, int64_t N, double dt, double *rcrit,
+            double *acc, int32_t *pairs, int64_t *npairs, int64_t nsteps);
+
+/*
+ * Host-buffer forms of nb_kick and nb_step: same semantics, every pointer is a HOST pointer
+ * (pairs has room for pair_capacity rows; npairs is a host int64).  Inputs are copied to the
+ * library's private device arena, the device path above runs, outputs are copied back, the
+ * stream is synchronised.  rcrit may be NULL in nb_kick_host (as in nb_kick) and in
+ * nb_step_host (then it is neither read nor returned; needs n1 or n2 > 0).
+ */
+int nb_kick_host(const double *x, double *v, const double *m, double M_star, int64_t N, double dt,
+                 const double *rcrit, double *acc, int32_t *pairs, int64_t *npairs);
+int nb_step_host(double *x, double *v, const double *m, double M_star, int64_t N, double dt,
+                 double *rcrit, double *acc, int32_t *pairs, int64_t *npairs, int64_t nsteps);
+
+/*
+ * Lazy device-side conditions accumulated since the last nb_status_reset; synchronises the
+ * stream.  flags (host int64[4]):
+ *   [0] pairs dropped because the list was full (sum over evaluations)
+ *   [1] Kepler solver non-convergences (body left unchanged)
+ *   [2] non-finite positions / masses / radii seen while staging j-bodies
+ *   [3] coincident bodies (r_ij == 0, i != j) that contributed nothing
+ */
+int nb_status(int64_t *flags);
+int nb_status_reset(void);
+
+/* Milliseconds the most recent force-tile kernel of nb_kick / nb_step(nsteps=0) took, timed with
+ * CUDA events on the configured stream (synchronises).  Negative if none was recorded. */
+double nb_last_force_ms(void);
+/* Launch geometry the force kernel would use for (N, n_active): out[0] = i-bodies per thread,
+ * out[1] = i-blocks, out[2] = j-splits, out[3] = threads per CTA, out[4] = j-tile length. */
+int nb_force_geometry(int64_t N, int64_t *out5);
+
+/*
+ * Measurement aid: runs a register-only chain of independent fp64 FMAs on every SM and returns
+ * the achieved rate in *tflops (2 flops per FMA), the roofline denominator for the kick.
+ * Synchronises.  iters = FMAs per chain step; 0 = default.
+ */
+int nb_fp64_peak(int64_t iters, double *tflops, double *ms);
+
+/* Frees the private arena, cached graphs and events. */
+void nb_release(void);
+
+const char *nb_last_error(void);
+const char *nb_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* NBKICK_H */

@@ -1,0 +1,265 @@
+"""Thin ctypes face of libnbkick.so (include/nbkick.h): argument marshalling only.
+
+Every step of the path runs in the library's CUDA kernels.  PyTorch is used for device memory and
+streams only: tensors are passed as raw device pointers.  There is no CPU fallback; if the shared
+library is missing or cannot be loaded this module raises at import of the first call.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+from dataclasses import dataclass
+
+import numpy as np
+
+from . import build as _build
+
+NB_OK = 0
+NB_E_NULL, NB_E_BADN, NB_E_BADARG, NB_E_WORKSPACE, NB_E_CUDA = -1, -2, -3, -4, -5
+CHANGEOVER_RATIONAL, CHANGEOVER_QUINTIC = 0, 1
+
+# every symbol include/nbkick.h declares (tests check the library exports each of them)
+SYMBOLS = (
+    "nb_default_config", "nb_configure", "nb_workspace_bytes", "nb_rcrit", "nb_kick", "nb_shift",
+    "nb_drift_kepler", "nb_step", "nb_kick_host", "nb_step_host", "nb_status", "nb_status_reset",
+    "nb_last_force_ms", "nb_force_geometry", "nb_fp64_peak", "nb_release", "nb_last_error", "nb_version",
+)
+
+
+class NbConfig(C.Structure):
+    _fields_ = [
+        ("stream", C.c_void_p),
+        ("workspace", C.c_void_p),
+        ("workspace_bytes", C.c_size_t),
+        ("pair_capacity", C.c_int64),
+        ("n_active", C.c_int64),
+        ("G", C.c_double),
+        ("n1", C.c_double),
+        ("n2", C.c_double),
+        ("changeover_kind", C.c_int),
+        ("i_per_thread", C.c_int),
+        ("j_splits", C.c_int),
+        ("use_graph", C.c_int),
+    ]
+
+
+class NbError(RuntimeError):
+    def __init__(self, code: int, msg: str):
+        super().__init__(f"libnbkick error {code}: {msg}")
+        self.code = code
+
+
+_lib = None
+
+
+def lib_path() -> str:
+    return _build.LIB
+
+
+def load():
+    """Load libnbkick.so (built in-tree by paper_2604_09184_b200/build.py).  Fails loudly."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    path = lib_path()
+    if not os.path.exists(path):
+        raise ImportError(f"{path} is missing: run `python -m paper_2604_09184_b200.build` "
+                          "(or __graft_entry__.build()); there is no CPU fallback")
+    lib = C.CDLL(path)
+    vp, dbl, i64, sz = C.c_void_p, C.c_double, C.c_int64, C.c_size_t
+    lib.nb_default_config.argtypes = [C.POINTER(NbConfig)]
+    lib.nb_default_config.restype = None
+    lib.nb_configure.argtypes = [C.POINTER(NbConfig)]
+    lib.nb_workspace_bytes.argtypes = [i64]
+    lib.nb_workspace_bytes.restype = sz
+    lib.nb_rcrit.argtypes = [vp, vp, vp, dbl, i64, dbl, vp]
+    lib.nb_kick.argtypes = [vp, vp, vp, dbl, i64, dbl, vp, vp, vp, vp]
+    lib.nb_shift.argtypes = [vp, vp, vp, dbl, i64, dbl]
+    lib.nb_drift_kepler.argtypes = [vp, vp, dbl, i64, dbl]
+    lib.nb_step.argtypes = [vp, vp, vp, dbl, i64, dbl, vp, vp, vp, vp, i64]
+    lib.nb_kick_host.argtypes = [vp, vp, vp, dbl, i64, dbl, vp, vp, vp, vp]
+    lib.nb_step_host.argtypes = [vp, vp, vp, dbl, i64, dbl, vp, vp, vp, vp, i64]
+    lib.nb_status.argtypes = [C.POINTER(C.c_int64)]
+    lib.nb_status_reset.argtypes = []
+    lib.nb_last_force_ms.argtypes = []
+    lib.nb_last_force_ms.restype = dbl
+    lib.nb_force_geometry.argtypes = [i64, C.POINTER(C.c_int64)]
+    lib.nb_fp64_peak.argtypes = [i64, C.POINTER(dbl), C.POINTER(dbl)]
+    lib.nb_release.argtypes = []
+    lib.nb_release.restype = None
+    lib.nb_last_error.restype = C.c_char_p
+    lib.nb_version.restype = C.c_char_p
+    _lib = lib
+    return lib
+
+
+def _check(rc: int):
+    if rc != NB_OK:
+        raise NbError(rc, load().nb_last_error().decode())
+
+
+def _dev(t, n_elem=None, dtype=None):
+    """Raw device pointer of a contiguous CUDA tensor (None -> NULL)."""
+    if t is None:
+        return None
+    import torch
+    if not (isinstance(t, torch.Tensor) and t.is_cuda and t.is_contiguous()):
+        raise TypeError("expected a contiguous CUDA tensor")
+    if dtype is not None and t.dtype != dtype:
+        raise TypeError(f"expected dtype {dtype}, got {t.dtype}")
+    if n_elem is not None and t.numel() < n_elem:
+        raise ValueError(f"tensor has {t.numel()} elements, need {n_elem}")
+    return C.c_void_p(t.data_ptr())
+
+
+def _host(a, n_elem=None, dtype=np.float64):
+    if a is None:
+        return None
+    if not (isinstance(a, np.ndarray) and a.flags.c_contiguous and a.dtype == dtype):
+        raise TypeError(f"expected a C-contiguous numpy array of {dtype}")
+    if n_elem is not None and a.size < n_elem:
+        raise ValueError("host array too small")
+    return C.c_void_p(a.ctypes.data)
+
+
+@dataclass
+class Geometry:
+    i_per_thread: int
+    i_blocks: int
+    j_splits: int
+    threads: int
+    tile_j: int
+
+
+_state = dict(cfg=None, workspace=None)
+
+
+def default_config() -> NbConfig:
+    cfg = NbConfig()
+    load().nb_default_config(C.byref(cfg))
+    return cfg
+
+
+def configure(N=None, *, stream=None, pair_capacity=0, n_active=0, G=None, n1=3.0, n2=0.4, changeover_kind=0,
+              i_per_thread=0, j_splits=0, use_graph=True, device="cuda"):
+    """nb_configure with a torch-allocated workspace sized for N bodies (N=None: no workspace,
+    enough for the _host calls).  Keeps the workspace tensor alive."""
+    lib = load()
+    cfg = default_config()
+    if G is not None:
+        cfg.G = float(G)
+    cfg.n1, cfg.n2 = float(n1), float(n2)
+    cfg.pair_capacity = int(pair_capacity)
+    cfg.n_active = int(n_active)
+    cfg.changeover_kind = int(changeover_kind)
+    cfg.i_per_thread, cfg.j_splits = int(i_per_thread), int(j_splits)
+    cfg.use_graph = 1 if use_graph else 0
+    if N is not None:
+        import torch
+        if stream is None:
+            stream = torch.cuda.current_stream().cuda_stream
+        cfg.stream = C.c_void_p(int(stream)) if stream else None
+        _check(lib.nb_configure(C.byref(cfg)))  # tuning first: the workspace size depends on it
+        nbytes = int(lib.nb_workspace_bytes(int(N)))
+        ws = torch.zeros(nbytes + 256, dtype=torch.uint8, device=device)
+        off = (-ws.data_ptr()) % 256
+        cfg.workspace = C.c_void_p(ws.data_ptr() + off)
+        cfg.workspace_bytes = nbytes
+        _state["workspace"] = ws
+    else:
+        cfg.stream = C.c_void_p(int(stream)) if stream else None
+        _state["workspace"] = None
+    _check(lib.nb_configure(C.byref(cfg)))
+    _state["cfg"] = cfg
+    return cfg
+
+
+def workspace_bytes(N: int) -> int:
+    return int(load().nb_workspace_bytes(int(N)))
+
+
+def force_geometry(N: int) -> Geometry:
+    out = (C.c_int64 * 5)()
+    _check(load().nb_force_geometry(int(N), out))
+    return Geometry(*[int(v) for v in out])
+
+
+def nb_rcrit(x, v, m, M_star, dt, rcrit):
+    import torch
+    N = m.numel()
+    _check(load().nb_rcrit(_dev(x, 3 * N, torch.float64), _dev(v, 3 * N, torch.float64), _dev(m, N, torch.float64),
+                           float(M_star), N, float(dt), _dev(rcrit, N, torch.float64)))
+
+
+def nb_kick(x, v, m, M_star, dt, rcrit, acc, pairs=None, npairs=None):
+    import torch
+    N = m.numel()
+    _check(load().nb_kick(_dev(x, 3 * N, torch.float64), _dev(v, 3 * N, torch.float64), _dev(m, N, torch.float64),
+                          float(M_star), N, float(dt), _dev(rcrit, N, torch.float64), _dev(acc, 3 * N, torch.float64),
+                          _dev(pairs, None, torch.int32), _dev(npairs, 1, torch.int64)))
+
+
+def nb_shift(x, v, m, M_star, dt):
+    import torch
+    N = m.numel()
+    _check(load().nb_shift(_dev(x, 3 * N, torch.float64), _dev(v, 3 * N, torch.float64), _dev(m, N, torch.float64),
+                           float(M_star), N, float(dt)))
+
+
+def nb_drift_kepler(x, v, M_star, dt):
+    import torch
+    N = x.numel() // 3
+    _check(load().nb_drift_kepler(_dev(x, 3 * N, torch.float64), _dev(v, 3 * N, torch.float64), float(M_star), N,
+                                  float(dt)))
+
+
+def nb_step(x, v, m, M_star, dt, rcrit, acc, pairs=None, npairs=None, nsteps=1):
+    import torch
+    N = m.numel()
+    _check(load().nb_step(_dev(x, 3 * N, torch.float64), _dev(v, 3 * N, torch.float64), _dev(m, N, torch.float64),
+                          float(M_star), N, float(dt), _dev(rcrit, N, torch.float64), _dev(acc, 3 * N, torch.float64),
+                          _dev(pairs, None, torch.int32), _dev(npairs, 1, torch.int64), int(nsteps)))
+
+
+def nb_kick_host(x, v, m, M_star, dt, rcrit, acc, pairs=None, npairs=None):
+    N = m.size
+    _check(load().nb_kick_host(_host(x, 3 * N), _host(v, 3 * N), _host(m, N), float(M_star), N, float(dt),
+                               _host(rcrit, N), _host(acc, 3 * N), _host(pairs, None, np.int32),
+                               _host(npairs, 1, np.int64)))
+
+
+def nb_step_host(x, v, m, M_star, dt, rcrit, acc, pairs=None, npairs=None, nsteps=1):
+    N = m.size
+    _check(load().nb_step_host(_host(x, 3 * N), _host(v, 3 * N), _host(m, N), float(M_star), N, float(dt),
+                               _host(rcrit, N), _host(acc, 3 * N), _host(pairs, None, np.int32),
+                               _host(npairs, 1, np.int64), int(nsteps)))
+
+
+def nb_status() -> dict:
+    f = (C.c_int64 * 4)()
+    _check(load().nb_status(f))
+    return dict(pairs_dropped=int(f[0]), kepler_fail=int(f[1]), nonfinite=int(f[2]), singular=int(f[3]))
+
+
+def nb_status_reset():
+    _check(load().nb_status_reset())
+
+
+def nb_last_force_ms() -> float:
+    return float(load().nb_last_force_ms())
+
+
+def nb_fp64_peak(iters: int = 0):
+    """(TFLOP/s, ms) of a register-only fp64 FMA chain on every SM."""
+    t, ms = C.c_double(0.0), C.c_double(0.0)
+    _check(load().nb_fp64_peak(int(iters), C.byref(t), C.byref(ms)))
+    return float(t.value), float(ms.value)
+
+
+def nb_release():
+    load().nb_release()
+    _state["workspace"] = None
+
+
+def nb_version() -> str:
+    return load().nb_version().decode()

@@ -1,0 +1,196 @@
+// body_kernels.cuh -- the O(N) kernels around the force tiles: critical radius + j-record staging
+// (a0), partial-sum reduce + velocity kick (a4), H_C shift (a5), Kepler drift (a6).
+// One thread per body, kBodyThreads per CTA.  The total momentum needed by H_C travels between
+// kernels as per-CTA partial sums that every consumer CTA re-reduces in a fixed order, so a step
+// needs no separate reduction launch and stays bit-reproducible.
+#pragma once
+#include "kepler.cuh"
+#include "nb_common.cuh"
+
+namespace nbk {
+
+// Eq. 7 with reading S5 for R_Hill.
+__device__ __forceinline__ double critical_radius(const double x, const double y, const double z, const double vx,
+                                                  const double vy, const double vz, const double m,
+                                                  const double M_star, const double G, const double n1,
+                                                  const double n2, const double absdt) {
+    const double r = sqrt(x * x + y * y + z * z);
+    const double v2 = vx * vx + vy * vy + vz * vz;
+    const double inva = 2.0 / r - v2 / (G * M_star);
+    const double a = (inva > 0.0) ? 1.0 / inva : r;
+    const double rh = a * cbrt(m / (3.0 * M_star));
+    return fmax(n1 * rh, n2 * absdt * sqrt(v2));
+}
+
+struct PrepParams {
+    double *x;              // [N,3]; written only when mv_in != nullptr (second H_C half-shift)
+    const double *v;        // [N,3]; needed when update_rc
+    const double *m;        // [N]
+    double *rcrit;          // [N]; written when update_rc, read otherwise
+    JRec *jrec;             // [Njpad]
+    const double *mv_in;    // [nblk_in,3] momentum partials or nullptr
+    unsigned long long *npairs;  // reset to 0 here (nullptr: skip)
+    long long *status;
+    double dtc;             // shift time (dt/2)
+    double M_star, G, n1, n2, absdt;
+    int nblk_in;
+    int N, Nj, Njpad;
+    int update_rc;
+};
+
+// a5 (second half) + a0 + staging: x += dtc * P/M_star; rcrit from the shifted state; JRec for j < Nj.
+__global__ void __launch_bounds__(kBodyThreads) nb_prep_kernel(const PrepParams p) {
+    __shared__ double sm[3 * kBodyThreads];
+    double sx = 0.0, sy = 0.0, sz = 0.0;
+    if (p.mv_in != nullptr) {
+        reduce_partials3(p.mv_in, p.nblk_in, sx, sy, sz, sm);
+        sx /= p.M_star; sy /= p.M_star; sz /= p.M_star;
+    }
+    const int i = blockIdx.x * kBodyThreads + threadIdx.x;
+    if (i == 0 && p.npairs != nullptr) *p.npairs = 0ull;
+    // padding record: zero mass, far away => contributes exactly 0 and never votes for the slow path
+    JRec r;
+    r.x = kFarJ; r.y = kFarJ; r.z = kFarJ; r.gm = 0.0; r.c1 = 0.0; r.c2 = 0.0; r.rc2 = 0.0; r.rc = 0.0;
+    if (i < p.N) {
+        double x = p.x[3 * (size_t)i], y = p.x[3 * (size_t)i + 1], z = p.x[3 * (size_t)i + 2];
+        if (p.mv_in != nullptr) {
+            x = x + p.dtc * sx; y = y + p.dtc * sy; z = z + p.dtc * sz;
+            p.x[3 * (size_t)i] = x; p.x[3 * (size_t)i + 1] = y; p.x[3 * (size_t)i + 2] = z;
+        }
+        const double m = p.m[i];
+        double rc;
+        if (p.update_rc) {
+            rc = critical_radius(x, y, z, p.v[3 * (size_t)i], p.v[3 * (size_t)i + 1], p.v[3 * (size_t)i + 2], m,
+                                 p.M_star, p.G, p.n1, p.n2, p.absdt);
+            p.rcrit[i] = rc;
+        } else {
+            rc = p.rcrit[i];
+        }
+        if (i < p.Nj) {
+            const double gm = p.G * m;
+            r.x = x; r.y = y; r.z = z; r.gm = gm;
+            r.c1 = 1.5 * gm; r.c2 = 1.875 * gm; r.rc2 = rc * rc; r.rc = rc;
+            if (!(isfinite(x) && isfinite(y) && isfinite(z) && isfinite(gm) && isfinite(rc) && rc >= 0.0))
+                status_add(p.status, ST_NONFINITE, 1);
+        }
+    }
+    if (i < p.Njpad) p.jrec[i] = r;  // grid covers max(N, Njpad)
+}
+
+// standalone a0
+__global__ void __launch_bounds__(kBodyThreads) nb_rcrit_kernel(const double *__restrict__ x, const double *__restrict__ v,
+                                                               const double *__restrict__ m, double *__restrict__ rcrit,
+                                                               int N, double M_star, double G, double n1, double n2,
+                                                               double absdt) {
+    const int i = blockIdx.x * kBodyThreads + threadIdx.x;
+    if (i >= N) return;
+    rcrit[i] = critical_radius(x[3 * (size_t)i], x[3 * (size_t)i + 1], x[3 * (size_t)i + 2], v[3 * (size_t)i],
+                               v[3 * (size_t)i + 1], v[3 * (size_t)i + 2], m[i], M_star, G, n1, n2, absdt);
+}
+
+// a4: acc_i = sum over j-splits (in split order) of the partial sums; v_i = v_i + hk*acc_i, applied
+// nhalf times (the closing half-kick of one step and the opening half-kick of the next are two
+// separate roundings, as in the step definition).  Optionally emits momentum partials of the new v.
+__global__ void __launch_bounds__(kBodyThreads) nb_kickv_kernel(const double *__restrict__ part, int nsplit,
+                                                               double *__restrict__ acc, double *__restrict__ v,
+                                                               const double *__restrict__ m, int N, double hk,
+                                                               int nhalf, double *__restrict__ mv_out) {
+    __shared__ double sm[3 * kBodyThreads];
+    const int i = blockIdx.x * kBodyThreads + threadIdx.x;
+    double px = 0.0, py = 0.0, pz = 0.0;
+    if (i < N) {
+        double ax = 0.0, ay = 0.0, az = 0.0;
+        for (int s = 0; s < nsplit; ++s) {
+            const double *q = part + ((size_t)s * N + i) * 3;
+            ax += q[0]; ay += q[1]; az += q[2];
+        }
+        acc[3 * (size_t)i] = ax; acc[3 * (size_t)i + 1] = ay; acc[3 * (size_t)i + 2] = az;
+        double vx = v[3 * (size_t)i], vy = v[3 * (size_t)i + 1], vz = v[3 * (size_t)i + 2];
+        for (int h = 0; h < nhalf; ++h) {
+            vx = vx + hk * ax; vy = vy + hk * ay; vz = vz + hk * az;
+        }
+        if (nhalf > 0) { v[3 * (size_t)i] = vx; v[3 * (size_t)i + 1] = vy; v[3 * (size_t)i + 2] = vz; }
+        if (mv_out != nullptr) { const double mi = m[i]; px = mi * vx; py = mi * vy; pz = mi * vz; }
+    }
+    if (mv_out != nullptr) {
+        block_sum3(px, py, pz, sm);
+        if (threadIdx.x == 0) {
+            mv_out[3 * blockIdx.x] = px; mv_out[3 * blockIdx.x + 1] = py; mv_out[3 * blockIdx.x + 2] = pz;
+        }
+    }
+}
+
+// momentum partials of the current v (standalone nb_shift)
+__global__ void __launch_bounds__(kBodyThreads) nb_momentum_kernel(const double *__restrict__ v, const double *__restrict__ m,
+                                                                  int N, double *__restrict__ mv_out) {
+    __shared__ double sm[3 * kBodyThreads];
+    const int i = blockIdx.x * kBodyThreads + threadIdx.x;
+    double px = 0.0, py = 0.0, pz = 0.0;
+    if (i < N) { const double mi = m[i]; px = mi * v[3 * (size_t)i]; py = mi * v[3 * (size_t)i + 1]; pz = mi * v[3 * (size_t)i + 2]; }
+    block_sum3(px, py, pz, sm);
+    if (threadIdx.x == 0) { mv_out[3 * blockIdx.x] = px; mv_out[3 * blockIdx.x + 1] = py; mv_out[3 * blockIdx.x + 2] = pz; }
+}
+
+// standalone a5: x += dtc * P / M_star
+__global__ void __launch_bounds__(kBodyThreads) nb_shift_kernel(double *__restrict__ x, const double *__restrict__ mv_in,
+                                                               int nblk_in, int N, double dtc, double M_star) {
+    __shared__ double sm[3 * kBodyThreads];
+    double sx, sy, sz;
+    reduce_partials3(mv_in, nblk_in, sx, sy, sz, sm);
+    sx /= M_star; sy /= M_star; sz /= M_star;
+    const int i = blockIdx.x * kBodyThreads + threadIdx.x;
+    if (i < N) {
+        x[3 * (size_t)i] = x[3 * (size_t)i] + dtc * sx;
+        x[3 * (size_t)i + 1] = x[3 * (size_t)i + 1] + dtc * sy;
+        x[3 * (size_t)i + 2] = x[3 * (size_t)i + 2] + dtc * sz;
+    }
+}
+
+// a5 (first half, optional) + a6: x += dtc*P/M_star, then the Kepler flow for dt; optionally emits the
+// momentum partials of the drifted velocities for the second half-shift.
+__global__ void __launch_bounds__(kBodyThreads) nb_drift_kernel(double *__restrict__ x, double *__restrict__ v,
+                                                               const double *__restrict__ m, int N, double mu, double dt,
+                                                               const double *__restrict__ mv_in, int nblk_in,
+                                                               double dtc, double M_star, double *__restrict__ mv_out,
+                                                               long long *status) {
+    __shared__ double sm[3 * kBodyThreads];
+    double sx = 0.0, sy = 0.0, sz = 0.0;
+    if (mv_in != nullptr) {
+        reduce_partials3(mv_in, nblk_in, sx, sy, sz, sm);
+        sx /= M_star; sy /= M_star; sz /= M_star;
+    }
+    const int i = blockIdx.x * kBodyThreads + threadIdx.x;
+    double px = 0.0, py = 0.0, pz = 0.0;
+    if (i < N) {
+        double X[3] = {x[3 * (size_t)i], x[3 * (size_t)i + 1], x[3 * (size_t)i + 2]};
+        double V[3] = {v[3 * (size_t)i], v[3 * (size_t)i + 1], v[3 * (size_t)i + 2]};
+        if (mv_in != nullptr) { X[0] = X[0] + dtc * sx; X[1] = X[1] + dtc * sy; X[2] = X[2] + dtc * sz; }
+        int rcode = kepler_elliptic(X, V, mu, dt);
+        if (rcode == 2) rcode = kepler_universal(X, V, mu, dt);
+        if (rcode != 0) status_add(status, ST_KEPLER_FAIL, 1);
+        x[3 * (size_t)i] = X[0]; x[3 * (size_t)i + 1] = X[1]; x[3 * (size_t)i + 2] = X[2];
+        v[3 * (size_t)i] = V[0]; v[3 * (size_t)i + 1] = V[1]; v[3 * (size_t)i + 2] = V[2];
+        if (mv_out != nullptr) { const double mi = m[i]; px = mi * V[0]; py = mi * V[1]; pz = mi * V[2]; }
+    }
+    if (mv_out != nullptr) {
+        block_sum3(px, py, pz, sm);
+        if (threadIdx.x == 0) { mv_out[3 * blockIdx.x] = px; mv_out[3 * blockIdx.x + 1] = py; mv_out[3 * blockIdx.x + 2] = pz; }
+    }
+}
+
+// fp64 FMA-rate microbenchmark: 8 independent chains per thread, register only.
+__global__ void __launch_bounds__(256) nb_fp64_peak_kernel(double *out, long long iters, double a, double b) {
+    double c0 = threadIdx.x, c1 = c0 + 1, c2 = c0 + 2, c3 = c0 + 3, c4 = c0 + 4, c5 = c0 + 5, c6 = c0 + 6, c7 = c0 + 7;
+#pragma unroll 1
+    for (long long k = 0; k < iters; ++k) {
+#pragma unroll
+        for (int r = 0; r < 8; ++r) {
+            c0 = __fma_rn(c0, a, b); c1 = __fma_rn(c1, a, b); c2 = __fma_rn(c2, a, b); c3 = __fma_rn(c3, a, b);
+            c4 = __fma_rn(c4, a, b); c5 = __fma_rn(c5, a, b); c6 = __fma_rn(c6, a, b); c7 = __fma_rn(c7, a, b);
+        }
+    }
+    const double s = ((c0 + c1) + (c2 + c3)) + ((c4 + c5) + (c6 + c7));
+    if (s == 123.456) out[0] = s;  // keeps the chains alive; practically never true
+}
+
+}  // namespace nbk

@@ -1,0 +1,73 @@
+// nb_common.cuh -- shared device-side types and helpers of libnbkick (CUDA path only).
+// Nothing here is shared with oracle/ (the CPU checker); see DESIGN.md "independence".
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace nbk {
+
+// One staged j-body, 64 bytes = four 16-byte shared-memory broadcasts.
+// Built once per force evaluation by nb_prep_kernel (O(N)), consumed by the O(N^2) tile kernel.
+//   gm = G m_j, c1 = 3/2 G m_j, c2 = 15/8 G m_j : coefficients of the rsqrt-cube correction
+//   polynomial G m_j (1 + 3/2 e + 15/8 e^2)     (see force_tiles.cuh)
+//   rc2 = rcrit_j^2, rc = rcrit_j                (pair test / changeover)
+struct __align__(16) JRec {
+    double x, y, z, gm;
+    double c1, c2, rc2, rc;
+};
+static_assert(sizeof(JRec) == 64, "JRec must be 64 bytes");
+
+constexpr int kForceThreads = 128;  // threads per force CTA
+constexpr int kTileJ = 128;         // j-bodies per shared-memory stage (8 KB)
+constexpr int kStages = 2;          // TMA double buffer
+constexpr int kBodyThreads = 256;   // threads per CTA of the O(N) kernels
+constexpr double kFarJ = 1.0e30;    // padding j-records sit here with zero mass
+constexpr double kFarI = -1.0e30;   // padding i-lanes sit here; their sums are discarded
+
+// status counters (device int64[4]); meanings in include/nbkick.h nb_status
+enum { ST_PAIR_DROPPED = 0, ST_KEPLER_FAIL = 1, ST_NONFINITE = 2, ST_SINGULAR = 3, ST_COUNT = 4 };
+
+__device__ __forceinline__ void status_add(long long *status, int which, long long n) {
+    atomicAdd(reinterpret_cast<unsigned long long *>(status + which), static_cast<unsigned long long>(n));
+}
+
+// Deterministic block-wide sum of three doubles (fixed tree, blockDim.x == kBodyThreads).
+// Every thread returns the same totals.
+__device__ __forceinline__ void block_sum3(double &a, double &b, double &c, double *sm /* [3*kBodyThreads] */) {
+    const int t = threadIdx.x;
+    sm[t] = a;
+    sm[kBodyThreads + t] = b;
+    sm[2 * kBodyThreads + t] = c;
+    __syncthreads();
+#pragma unroll
+    for (int s = kBodyThreads / 2; s > 0; s >>= 1) {
+        if (t < s) {
+            sm[t] += sm[t + s];
+            sm[kBodyThreads + t] += sm[kBodyThreads + t + s];
+            sm[2 * kBodyThreads + t] += sm[2 * kBodyThreads + t + s];
+        }
+        __syncthreads();
+    }
+    a = sm[0];
+    b = sm[kBodyThreads];
+    c = sm[2 * kBodyThreads];
+    __syncthreads();
+}
+
+// Sum of per-block momentum partials part[nblk,3] in a fixed order: every CTA that calls this
+// gets bit-identical totals (thread t adds blocks t, t+256, ... in order; then the fixed tree).
+__device__ __forceinline__ void reduce_partials3(const double *__restrict__ part, int nblk, double &sx, double &sy,
+                                                 double &sz, double *sm) {
+    double a = 0.0, b = 0.0, c = 0.0;
+    for (int k = threadIdx.x; k < nblk; k += kBodyThreads) {
+        a += part[3 * k];
+        b += part[3 * k + 1];
+        c += part[3 * k + 2];
+    }
+    block_sum3(a, b, c, sm);
+    sx = a;
+    sy = b;
+    sz = c;
+}
+
+}  // namespace nbk

@@ -1,0 +1,540 @@
+// nbkick.cu -- host side of libnbkick.so: the C ABI declared in include/nbkick.h.
+// Argument validation, workspace carving, launch geometry, the step driver (a7) with CUDA-graph
+// replay, the host-buffer entry points and the measurement aids.  All arithmetic of the method runs
+// in the kernels of force_tiles.cuh / body_kernels.cuh; nothing here computes on the CPU.
+#include "../../include/nbkick.h"
+
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <mutex>
+
+#include "body_kernels.cuh"
+#include "force_tiles.cuh"
+
+namespace {
+
+using namespace nbk;
+
+std::mutex g_mu;
+nb_config g_cfg = {nullptr, nullptr, 0, 0, 0, 0.01720209895 * 0.01720209895, 3.0, 0.4, 0, 0, 0, 1};
+char g_err[512] = "";
+int g_sm_count = 0;
+cudaEvent_t g_ev0 = nullptr, g_ev1 = nullptr;
+bool g_force_timed = false;
+
+// private arena of the _host entry points
+void *g_arena = nullptr;
+size_t g_arena_bytes = 0;
+
+// cached CUDA graph of one interior step of nb_step
+struct StepKey {
+    const void *x, *v, *m, *rcrit, *acc, *pairs, *npairs, *ws, *stream;
+    int64_t N, n_active, cap;
+    double dt, M_star, G, n1, n2;
+    int kind, ipt, jsplit;
+    size_t ws_bytes;
+};
+StepKey g_graph_key;
+cudaGraphExec_t g_graph_exec = nullptr;
+
+int fail(int code, const char *fmt, ...) {
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(g_err, sizeof(g_err), fmt, ap);
+    va_end(ap);
+    return code;
+}
+
+#define NB_CUDA(call)                                                                                   \
+    do {                                                                                                \
+        cudaError_t e_ = (call);                                                                        \
+        if (e_ != cudaSuccess) return fail(NB_E_CUDA, "%s failed: %s", #call, cudaGetErrorString(e_)); \
+    } while (0)
+
+inline size_t align_up(size_t a, size_t b) { return (a + b - 1) / b * b; }
+inline cudaStream_t stream() { return static_cast<cudaStream_t>(g_cfg.stream); }
+
+int sm_count() {
+    if (g_sm_count == 0) {
+        int dev = 0, n = 0;
+        if (cudaGetDevice(&dev) == cudaSuccess &&
+            cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess && n > 0)
+            g_sm_count = n;
+        else
+            g_sm_count = 148;  // B200; only reached with no device (geometry queries on a CPU box)
+    }
+    return g_sm_count;
+}
+
+// Launch geometry of the force kernel.
+struct Geometry {
+    int ipt;              // i-bodies per thread
+    int iblocks;          // CTAs along i
+    int tiles_total;      // ceil(Nj / kTileJ)
+    int tiles_per_split;  // j-tiles per CTA
+    int nsplit;           // CTAs along j
+    int Nj, Njpad;
+};
+
+Geometry geometry(int64_t N, int64_t n_active) {
+    Geometry g;
+    g.Nj = (int)((n_active > 0 && n_active < N) ? n_active : N);
+    g.tiles_total = (g.Nj + kTileJ - 1) / kTileJ;
+    g.Njpad = g.tiles_total * kTileJ;
+    const int sms = sm_count();
+    // I: the largest register tile (i-bodies per thread) that still leaves enough (i-block, j-tile)
+    // work items to cover every SM a few times; small N falls back to a narrower tile.
+    int ipt = g_cfg.i_per_thread;
+    if (ipt != 1 && ipt != 2 && ipt != 4) {
+        ipt = 4;
+        while (ipt > 1 &&
+               ((N + (int64_t)kForceThreads * ipt - 1) / ((int64_t)kForceThreads * ipt)) * g.tiles_total < (int64_t)4 * sms)
+            ipt >>= 1;
+    }
+    g.ipt = ipt;
+    g.iblocks = (int)((N + (int64_t)kForceThreads * ipt - 1) / ((int64_t)kForceThreads * ipt));
+    int nsplit = g_cfg.j_splits;
+    if (nsplit <= 0) {
+        // aim for >= 8 waves of (4 CTAs per SM) so the tail is small; keep a few tiles per CTA so the
+        // prologue/epilogue and the partial-sum traffic stay negligible
+        const int64_t target = (int64_t)8 * 4 * sms;
+        nsplit = (int)((target + g.iblocks - 1) / g.iblocks);
+        const int min_tiles = g.tiles_total <= 32 ? 1 : (g.tiles_total <= 256 ? 2 : 4);
+        const int max_split = (g.tiles_total + min_tiles - 1) / min_tiles;
+        if (nsplit > max_split) nsplit = max_split;
+        if (nsplit < 1) nsplit = 1;
+    }
+    if (nsplit > g.tiles_total) nsplit = g.tiles_total;
+    if (nsplit > 65535) nsplit = 65535;
+    g.tiles_per_split = (g.tiles_total + nsplit - 1) / nsplit;
+    g.nsplit = (g.tiles_total + g.tiles_per_split - 1) / g.tiles_per_split;
+    return g;
+}
+
+// Workspace carving (all offsets 256-byte aligned).
+struct Workspace {
+    long long *status;  // ST_COUNT
+    unsigned long long *npairs_dummy;
+    double *mvA, *mvB;  // momentum partials [nblk,3]
+    double *rc_scratch; // [N]
+    JRec *jrec;         // [Njpad]
+    double *part;       // [nsplit, N, 3]
+    size_t bytes;
+};
+
+Workspace carve(void *base, int64_t N, const Geometry &g) {
+    Workspace w;
+    size_t off = 0;
+    char *b = static_cast<char *>(base);
+    const size_t nblk = (size_t)((N + kBodyThreads - 1) / kBodyThreads);
+    w.status = reinterpret_cast<long long *>(b + off); off += 256;
+    w.npairs_dummy = reinterpret_cast<unsigned long long *>(b + off); off += 256;
+    w.mvA = reinterpret_cast<double *>(b + off); off += align_up(nblk * 3 * sizeof(double), 256);
+    w.mvB = reinterpret_cast<double *>(b + off); off += align_up(nblk * 3 * sizeof(double), 256);
+    w.rc_scratch = reinterpret_cast<double *>(b + off); off += align_up((size_t)N * sizeof(double), 256);
+    w.jrec = reinterpret_cast<JRec *>(b + off); off += align_up((size_t)g.Njpad * sizeof(JRec), 256);
+    w.part = reinterpret_cast<double *>(b + off); off += align_up((size_t)g.nsplit * (size_t)N * 3 * sizeof(double), 256);
+    w.bytes = off;
+    return w;
+}
+
+int check_common(int64_t N, double dt, double M_star) {
+    if (N <= 0 || N > 2147483647LL) return fail(NB_E_BADN, "N = %lld out of range (1 .. 2^31-1)", (long long)N);
+    if (!std::isfinite(dt)) return fail(NB_E_BADARG, "dt is not finite");
+    if (!(M_star > 0.0) || !std::isfinite(M_star)) return fail(NB_E_BADARG, "M_star must be finite and > 0");
+    if (g_cfg.n_active > N) return fail(NB_E_BADARG, "n_active = %lld > N = %lld", (long long)g_cfg.n_active, (long long)N);
+    return NB_OK;
+}
+
+int check_workspace(int64_t N, const Geometry &g, Workspace *w) {
+    if (g_cfg.workspace == nullptr) return fail(NB_E_WORKSPACE, "no workspace configured (nb_configure)");
+    if ((reinterpret_cast<uintptr_t>(g_cfg.workspace) & 255u) != 0) return fail(NB_E_WORKSPACE, "workspace is not 256-byte aligned");
+    *w = carve(g_cfg.workspace, N, g);
+    if (w->bytes > g_cfg.workspace_bytes)
+        return fail(NB_E_WORKSPACE, "workspace has %zu bytes, N = %lld needs %zu", g_cfg.workspace_bytes, (long long)N, w->bytes);
+    return NB_OK;
+}
+
+inline int body_blocks(int64_t n) { return (int)((n + kBodyThreads - 1) / kBodyThreads); }
+
+template <int I>
+void launch_force_I(const ForceParams &fp, const Geometry &g, bool pairs) {
+    dim3 grid(g.iblocks, g.nsplit);
+    if (pairs) nb_force_tiles_kernel<I, true><<<grid, kForceThreads, 0, stream()>>>(fp);
+    else nb_force_tiles_kernel<I, false><<<grid, kForceThreads, 0, stream()>>>(fp);
+}
+
+void launch_force(const ForceParams &fp, const Geometry &g, bool pairs) {
+    if (g.ipt == 4) launch_force_I<4>(fp, g, pairs);
+    else if (g.ipt == 2) launch_force_I<2>(fp, g, pairs);
+    else launch_force_I<1>(fp, g, pairs);
+}
+
+// One force evaluation: [second half-shift] + rcrit + staging, tiles, reduce + kick.
+//   mv_in  : momentum partials for the half-shift folded into prep (nullptr: none)
+//   rc_io  : rcrit array read (update_rc = 0) or written (update_rc = 1)
+//   nhalf  : number of half-kicks hk applied to v after the evaluation
+//   mv_out : momentum partials of the kicked v (nullptr: none)
+int enqueue_eval(const Workspace &w, const Geometry &g, double *x, double *v, const double *m, double M_star, int64_t N,
+                 double dt_for_rc, double *rc_io, int update_rc, const double *mv_in, double dtc, double *acc,
+                 int32_t *pairs, int64_t *npairs, double hk, int nhalf, double *mv_out, bool time_force) {
+    const int nblk = body_blocks(N);
+    PrepParams pp;
+    pp.x = x; pp.v = v; pp.m = m; pp.rcrit = rc_io; pp.jrec = w.jrec; pp.mv_in = mv_in;
+    pp.npairs = pairs ? reinterpret_cast<unsigned long long *>(npairs) : nullptr;
+    pp.status = w.status; pp.dtc = dtc; pp.M_star = M_star; pp.G = g_cfg.G; pp.n1 = g_cfg.n1; pp.n2 = g_cfg.n2;
+    pp.absdt = std::fabs(dt_for_rc); pp.nblk_in = nblk; pp.N = (int)N; pp.Nj = g.Nj; pp.Njpad = g.Njpad;
+    pp.update_rc = update_rc;
+    const int64_t cover = N > g.Njpad ? N : g.Njpad;
+    nb_prep_kernel<<<body_blocks(cover), kBodyThreads, 0, stream()>>>(pp);
+
+    ForceParams fp;
+    fp.jrec = w.jrec; fp.x = x; fp.rcrit = rc_io; fp.part = w.part; fp.pairs = pairs;
+    fp.npairs = pairs ? reinterpret_cast<unsigned long long *>(npairs) : w.npairs_dummy;
+    fp.status = w.status; fp.cap = pairs ? g_cfg.pair_capacity : 0; fp.N = (int)N; fp.Nj = g.Nj;
+    fp.tiles_total = g.tiles_total; fp.tiles_per_split = g.tiles_per_split; fp.kind = g_cfg.changeover_kind;
+    if (time_force) {
+        if (!g_ev0) { NB_CUDA(cudaEventCreate(&g_ev0)); NB_CUDA(cudaEventCreate(&g_ev1)); }
+        NB_CUDA(cudaEventRecord(g_ev0, stream()));
+    }
+    launch_force(fp, g, pairs != nullptr);
+    if (time_force) { NB_CUDA(cudaEventRecord(g_ev1, stream())); g_force_timed = true; }
+
+    nb_kickv_kernel<<<nblk, kBodyThreads, 0, stream()>>>(w.part, g.nsplit, acc, v, m, (int)N, hk, nhalf, mv_out);
+    NB_CUDA(cudaGetLastError());
+    return NB_OK;
+}
+
+int check_pairs_args(const int32_t *pairs, const int64_t *npairs) {
+    if (pairs != nullptr && npairs == nullptr) return fail(NB_E_NULL, "npairs is NULL but pairs is not");
+    if (pairs != nullptr && g_cfg.pair_capacity <= 0) return fail(NB_E_BADARG, "pairs given but pair_capacity is 0 (nb_configure)");
+    return NB_OK;
+}
+
+int ensure_arena(size_t bytes) {
+    if (bytes <= g_arena_bytes) return NB_OK;
+    if (g_arena) { cudaFree(g_arena); g_arena = nullptr; g_arena_bytes = 0; }
+    const size_t want = align_up(bytes + bytes / 8, 1 << 20);
+    NB_CUDA(cudaMalloc(&g_arena, want));
+    NB_CUDA(cudaMemset(g_arena, 0, 512));
+    g_arena_bytes = want;
+    return NB_OK;
+}
+
+void drop_graph() {
+    if (g_graph_exec) { cudaGraphExecDestroy(g_graph_exec); g_graph_exec = nullptr; }
+}
+
+int step_impl(double *x, double *v, const double *m, double M_star, int64_t N, double dt, double *rcrit, double *acc,
+              int32_t *pairs, int64_t *npairs, int64_t nsteps) {
+    int rc = check_common(N, dt, M_star);
+    if (rc) return rc;
+    if (!x || !v || !m || !acc) return fail(NB_E_NULL, "nb_step: x, v, m, acc must not be NULL");
+    if (nsteps < 0) return fail(NB_E_BADARG, "nsteps < 0");
+    const int update_rc = !(g_cfg.n1 == 0.0 && g_cfg.n2 == 0.0);
+    if (!rcrit && !update_rc) return fail(NB_E_NULL, "nb_step: rcrit is NULL and n1 == n2 == 0");
+    if ((rc = check_pairs_args(pairs, npairs))) return rc;
+    const Geometry g = geometry(N, g_cfg.n_active);
+    Workspace w;
+    if ((rc = check_workspace(N, g, &w))) return rc;
+    double *rc_io = rcrit ? rcrit : w.rc_scratch;
+    const double hk = 0.5 * dt, dtc = 0.5 * dt, mu = g_cfg.G * M_star;
+    const int nblk = body_blocks(N);
+
+    // evaluation at t0 (+ opening half-kick of the first step)
+    if ((rc = enqueue_eval(w, g, x, v, m, M_star, N, dt, rc_io, update_rc, nullptr, 0.0, acc, pairs, npairs, hk,
+                           nsteps > 0 ? 1 : 0, w.mvA, nsteps == 0)))
+        return rc;
+
+    auto enqueue_step = [&](int nhalf) -> int {
+        // C(dt/2) A(dt): first half-shift folded into the drift kernel
+        nb_drift_kernel<<<nblk, kBodyThreads, 0, stream()>>>(x, v, m, (int)N, mu, dt, w.mvA, nblk, dtc, M_star, w.mvB,
+                                                             w.status);
+        // C(dt/2) folded into prep; force; B(dt/2) [+ B(dt/2) of the next step]
+        return enqueue_eval(w, g, x, v, m, M_star, N, dt, rc_io, update_rc, w.mvB, dtc, acc, pairs, npairs, hk, nhalf,
+                            w.mvA, false);
+    };
+
+    const int64_t interior = nsteps > 0 ? nsteps - 1 : 0;
+    if (interior > 0 && g_cfg.use_graph) {
+        StepKey key;
+        std::memset(&key, 0, sizeof(key));
+        key.x = x; key.v = v; key.m = m; key.rcrit = rc_io; key.acc = acc; key.pairs = pairs; key.npairs = npairs;
+        key.ws = g_cfg.workspace; key.stream = g_cfg.stream; key.N = N; key.n_active = g_cfg.n_active;
+        key.cap = g_cfg.pair_capacity; key.dt = dt; key.M_star = M_star; key.G = g_cfg.G; key.n1 = g_cfg.n1;
+        key.n2 = g_cfg.n2; key.kind = g_cfg.changeover_kind; key.ipt = g.ipt; key.jsplit = g.nsplit;
+        key.ws_bytes = g_cfg.workspace_bytes;
+        if (!g_graph_exec || std::memcmp(&key, &g_graph_key, sizeof(key)) != 0) {
+            drop_graph();
+            cudaGraph_t graph = nullptr;
+            NB_CUDA(cudaStreamBeginCapture(stream(), cudaStreamCaptureModeRelaxed));
+            const int erc = enqueue_step(2);
+            cudaError_t ce = cudaStreamEndCapture(stream(), &graph);
+            if (erc) { if (graph) cudaGraphDestroy(graph); return erc; }
+            if (ce != cudaSuccess) return fail(NB_E_CUDA, "cudaStreamEndCapture failed: %s", cudaGetErrorString(ce));
+            ce = cudaGraphInstantiate(&g_graph_exec, graph, 0);
+            cudaGraphDestroy(graph);
+            if (ce != cudaSuccess) { g_graph_exec = nullptr; return fail(NB_E_CUDA, "cudaGraphInstantiate failed: %s", cudaGetErrorString(ce)); }
+            g_graph_key = key;
+        }
+        for (int64_t s = 0; s < interior; ++s) NB_CUDA(cudaGraphLaunch(g_graph_exec, stream()));
+    } else {
+        for (int64_t s = 0; s < interior; ++s)
+            if ((rc = enqueue_step(2))) return rc;
+    }
+    if (nsteps > 0 && (rc = enqueue_step(1))) return rc;
+    NB_CUDA(cudaGetLastError());
+    return NB_OK;
+}
+
+int kick_impl(const double *x, double *v, const double *m, double M_star, int64_t N, double dt, const double *rcrit,
+              double *acc, int32_t *pairs, int64_t *npairs) {
+    int rc = check_common(N, dt, M_star);
+    if (rc) return rc;
+    if (!x || !v || !m || !acc) return fail(NB_E_NULL, "nb_kick: x, v, m, acc must not be NULL");
+    if ((rc = check_pairs_args(pairs, npairs))) return rc;
+    const Geometry g = geometry(N, g_cfg.n_active);
+    Workspace w;
+    if ((rc = check_workspace(N, g, &w))) return rc;
+    double *rc_io = rcrit ? const_cast<double *>(rcrit) : w.rc_scratch;
+    return enqueue_eval(w, g, const_cast<double *>(x), v, m, M_star, N, dt, rc_io, rcrit ? 0 : 1, nullptr, 0.0, acc, pairs,
+                        npairs, dt, dt != 0.0 ? 1 : 0, nullptr, true);
+}
+
+}  // namespace
+
+extern "C" {
+
+void nb_default_config(nb_config *cfg) {
+    if (!cfg) return;
+    std::memset(cfg, 0, sizeof(*cfg));
+    cfg->G = 0.01720209895 * 0.01720209895;
+    cfg->n1 = 3.0;
+    cfg->n2 = 0.4;
+    cfg->changeover_kind = NB_CHANGEOVER_RATIONAL;
+    cfg->use_graph = 1;
+}
+
+int nb_configure(const nb_config *cfg) {
+    std::lock_guard<std::mutex> lk(g_mu);
+    if (!cfg) return fail(NB_E_NULL, "nb_configure: cfg is NULL");
+    if (!(cfg->G > 0.0) || !std::isfinite(cfg->G)) return fail(NB_E_BADARG, "G must be finite and > 0");
+    if (!(cfg->n1 >= 0.0) || !(cfg->n2 >= 0.0) || !std::isfinite(cfg->n1) || !std::isfinite(cfg->n2))
+        return fail(NB_E_BADARG, "n1, n2 must be finite and >= 0");
+    if (cfg->pair_capacity < 0 || cfg->n_active < 0) return fail(NB_E_BADARG, "pair_capacity and n_active must be >= 0");
+    if (cfg->changeover_kind != NB_CHANGEOVER_RATIONAL && cfg->changeover_kind != NB_CHANGEOVER_QUINTIC)
+        return fail(NB_E_BADARG, "unknown changeover_kind %d", cfg->changeover_kind);
+    if (cfg->i_per_thread != 0 && cfg->i_per_thread != 1 && cfg->i_per_thread != 2 && cfg->i_per_thread != 4)
+        return fail(NB_E_BADARG, "i_per_thread must be 0, 1, 2 or 4");
+    if (cfg->j_splits < 0) return fail(NB_E_BADARG, "j_splits must be >= 0");
+    g_cfg = *cfg;
+    return NB_OK;
+}
+
+size_t nb_workspace_bytes(int64_t N) {
+    std::lock_guard<std::mutex> lk(g_mu);
+    if (N <= 0 || N > 2147483647LL) return 0;
+    const Geometry g = geometry(N, g_cfg.n_active <= N ? g_cfg.n_active : 0);
+    return carve(nullptr, N, g).bytes;
+}
+
+int nb_force_geometry(int64_t N, int64_t *out5) {
+    std::lock_guard<std::mutex> lk(g_mu);
+    if (!out5) return fail(NB_E_NULL, "out5 is NULL");
+    if (N <= 0 || N > 2147483647LL) return fail(NB_E_BADN, "N out of range");
+    const Geometry g = geometry(N, g_cfg.n_active <= N ? g_cfg.n_active : 0);
+    out5[0] = g.ipt; out5[1] = g.iblocks; out5[2] = g.nsplit; out5[3] = kForceThreads; out5[4] = kTileJ;
+    return NB_OK;
+}
+
+int nb_rcrit(const double *x, const double *v, const double *m, double M_star, int64_t N, double dt, double *rcrit) {
+    std::lock_guard<std::mutex> lk(g_mu);
+    int rc = check_common(N, dt, M_star);
+    if (rc) return rc;
+    if (!x || !v || !m || !rcrit) return fail(NB_E_NULL, "nb_rcrit: NULL argument");
+    nb_rcrit_kernel<<<body_blocks(N), kBodyThreads, 0, stream()>>>(x, v, m, rcrit, (int)N, M_star, g_cfg.G, g_cfg.n1,
+                                                                   g_cfg.n2, std::fabs(dt));
+    NB_CUDA(cudaGetLastError());
+    return NB_OK;
+}
+
+int nb_kick(const double *x, double *v, const double *m, double M_star, int64_t N, double dt, const double *rcrit,
+            double *acc, int32_t *pairs, int64_t *npairs) {
+    std::lock_guard<std::mutex> lk(g_mu);
+    return kick_impl(x, v, m, M_star, N, dt, rcrit, acc, pairs, npairs);
+}
+
+int nb_shift(double *x, const double *v, const double *m, double M_star, int64_t N, double dt) {
+    std::lock_guard<std::mutex> lk(g_mu);
+    int rc = check_common(N, dt, M_star);
+    if (rc) return rc;
+    if (!x || !v || !m) return fail(NB_E_NULL, "nb_shift: NULL argument");
+    const Geometry g = geometry(N, g_cfg.n_active);
+    Workspace w;
+    if ((rc = check_workspace(N, g, &w))) return rc;
+    const int nblk = body_blocks(N);
+    nb_momentum_kernel<<<nblk, kBodyThreads, 0, stream()>>>(v, m, (int)N, w.mvA);
+    nb_shift_kernel<<<nblk, kBodyThreads, 0, stream()>>>(x, w.mvA, nblk, (int)N, dt, M_star);
+    NB_CUDA(cudaGetLastError());
+    return NB_OK;
+}
+
+int nb_drift_kepler(double *x, double *v, double M_star, int64_t N, double dt) {
+    std::lock_guard<std::mutex> lk(g_mu);
+    int rc = check_common(N, dt, M_star);
+    if (rc) return rc;
+    if (!x || !v) return fail(NB_E_NULL, "nb_drift_kepler: NULL argument");
+    const Geometry g = geometry(N, g_cfg.n_active);
+    Workspace w;
+    if ((rc = check_workspace(N, g, &w))) return rc;
+    nb_drift_kernel<<<body_blocks(N), kBodyThreads, 0, stream()>>>(x, v, nullptr, (int)N, g_cfg.G * M_star, dt, nullptr, 0,
+                                                                   0.0, M_star, nullptr, w.status);
+    NB_CUDA(cudaGetLastError());
+    return NB_OK;
+}
+
+int nb_step(double *x, double *v, const double *m, double M_star, int64_t N, double dt, double *rcrit, double *acc,
+            int32_t *pairs, int64_t *npairs, int64_t nsteps) {
+    std::lock_guard<std::mutex> lk(g_mu);
+    return step_impl(x, v, m, M_star, N, dt, rcrit, acc, pairs, npairs, nsteps);
+}
+
+// ---- host-buffer forms: copy in, run the device path on the private arena, copy out ----
+static int host_run(bool is_step, double *x, double *v, const double *m, double M_star, int64_t N, double dt,
+                    double *rcrit, bool rcrit_out, double *acc, int32_t *pairs, int64_t *npairs, int64_t nsteps) {
+    int rc = check_common(N, dt, M_star);
+    if (rc) return rc;
+    if (!x || !v || !m || !acc) return fail(NB_E_NULL, "host call: x, v, m, acc must not be NULL");
+    if ((rc = check_pairs_args(pairs, npairs))) return rc;
+    const Geometry g = geometry(N, g_cfg.n_active);
+    const size_t ws_bytes = carve(nullptr, N, g).bytes;
+    const size_t n3 = align_up((size_t)N * 3 * sizeof(double), 256), n1 = align_up((size_t)N * sizeof(double), 256);
+    const size_t pb = pairs ? align_up((size_t)g_cfg.pair_capacity * 2 * sizeof(int32_t), 256) : 0;
+    const size_t total = ws_bytes + 3 * n3 + 2 * n1 + pb + 256;
+    if ((rc = ensure_arena(total))) return rc;
+    char *b = static_cast<char *>(g_arena);
+    void *ws = b; b += ws_bytes;
+    double *dx = reinterpret_cast<double *>(b); b += n3;
+    double *dv = reinterpret_cast<double *>(b); b += n3;
+    double *dacc = reinterpret_cast<double *>(b); b += n3;
+    double *dm = reinterpret_cast<double *>(b); b += n1;
+    double *drc = reinterpret_cast<double *>(b); b += n1;
+    int32_t *dpairs = pairs ? reinterpret_cast<int32_t *>(b) : nullptr; b += pb;
+    int64_t *dnp = reinterpret_cast<int64_t *>(b);
+
+    const nb_config saved = g_cfg;
+    g_cfg.workspace = ws;
+    g_cfg.workspace_bytes = ws_bytes;
+    cudaStream_t s = stream();
+    const size_t b3 = (size_t)N * 3 * sizeof(double), b1 = (size_t)N * sizeof(double);
+    auto body = [&]() -> int {
+        NB_CUDA(cudaMemcpyAsync(dx, x, b3, cudaMemcpyHostToDevice, s));
+        NB_CUDA(cudaMemcpyAsync(dv, v, b3, cudaMemcpyHostToDevice, s));
+        NB_CUDA(cudaMemcpyAsync(dm, m, b1, cudaMemcpyHostToDevice, s));
+        if (rcrit) NB_CUDA(cudaMemcpyAsync(drc, rcrit, b1, cudaMemcpyHostToDevice, s));
+        int r;
+        if (is_step) r = step_impl(dx, dv, dm, M_star, N, dt, rcrit ? drc : nullptr, dacc, dpairs, pairs ? dnp : nullptr, nsteps);
+        else r = kick_impl(dx, dv, dm, M_star, N, dt, rcrit ? drc : nullptr, dacc, dpairs, pairs ? dnp : nullptr);
+        if (r) return r;
+        if (is_step) NB_CUDA(cudaMemcpyAsync(x, dx, b3, cudaMemcpyDeviceToHost, s));
+        NB_CUDA(cudaMemcpyAsync(v, dv, b3, cudaMemcpyDeviceToHost, s));
+        NB_CUDA(cudaMemcpyAsync(acc, dacc, b3, cudaMemcpyDeviceToHost, s));
+        if (rcrit && rcrit_out) NB_CUDA(cudaMemcpyAsync(rcrit, drc, b1, cudaMemcpyDeviceToHost, s));
+        if (pairs) {
+            NB_CUDA(cudaMemcpyAsync(npairs, dnp, sizeof(int64_t), cudaMemcpyDeviceToHost, s));
+            NB_CUDA(cudaStreamSynchronize(s));
+            int64_t keep = *npairs < g_cfg.pair_capacity ? *npairs : g_cfg.pair_capacity;
+            if (keep > 0) NB_CUDA(cudaMemcpyAsync(pairs, dpairs, (size_t)keep * 2 * sizeof(int32_t), cudaMemcpyDeviceToHost, s));
+        }
+        NB_CUDA(cudaStreamSynchronize(s));
+        return NB_OK;
+    };
+    rc = body();
+    // the arena is private: restore the caller's workspace, keep everything else
+    g_cfg.workspace = saved.workspace;
+    g_cfg.workspace_bytes = saved.workspace_bytes;
+    return rc;
+}
+
+int nb_kick_host(const double *x, double *v, const double *m, double M_star, int64_t N, double dt, const double *rcrit,
+                 double *acc, int32_t *pairs, int64_t *npairs) {
+    std::lock_guard<std::mutex> lk(g_mu);
+    return host_run(false, const_cast<double *>(x), v, m, M_star, N, dt, const_cast<double *>(rcrit), false, acc, pairs,
+                    npairs, 0);
+}
+
+int nb_step_host(double *x, double *v, const double *m, double M_star, int64_t N, double dt, double *rcrit, double *acc,
+                 int32_t *pairs, int64_t *npairs, int64_t nsteps) {
+    std::lock_guard<std::mutex> lk(g_mu);
+    return host_run(true, x, v, m, M_star, N, dt, rcrit, true, acc, pairs, npairs, nsteps);
+}
+
+int nb_status(int64_t *flags) {
+    std::lock_guard<std::mutex> lk(g_mu);
+    if (!flags) return fail(NB_E_NULL, "flags is NULL");
+    if (!g_cfg.workspace && !g_arena) return fail(NB_E_WORKSPACE, "no workspace configured");
+    int64_t a[ST_COUNT] = {0, 0, 0, 0}, b[ST_COUNT] = {0, 0, 0, 0};
+    if (g_cfg.workspace) NB_CUDA(cudaMemcpyAsync(a, g_cfg.workspace, sizeof(a), cudaMemcpyDeviceToHost, stream()));
+    if (g_arena) NB_CUDA(cudaMemcpyAsync(b, g_arena, sizeof(b), cudaMemcpyDeviceToHost, stream()));  // _host calls
+    NB_CUDA(cudaStreamSynchronize(stream()));
+    for (int k = 0; k < ST_COUNT; ++k) flags[k] = a[k] + b[k];
+    return NB_OK;
+}
+
+int nb_status_reset(void) {
+    std::lock_guard<std::mutex> lk(g_mu);
+    if (!g_cfg.workspace && !g_arena) return fail(NB_E_WORKSPACE, "no workspace configured");
+    if (g_cfg.workspace) NB_CUDA(cudaMemsetAsync(g_cfg.workspace, 0, 512, stream()));
+    if (g_arena) NB_CUDA(cudaMemsetAsync(g_arena, 0, 512, stream()));
+    return NB_OK;
+}
+
+double nb_last_force_ms(void) {
+    std::lock_guard<std::mutex> lk(g_mu);
+    if (!g_force_timed) return -1.0;
+    if (cudaEventSynchronize(g_ev1) != cudaSuccess) return -1.0;
+    float ms = -1.0f;
+    if (cudaEventElapsedTime(&ms, g_ev0, g_ev1) != cudaSuccess) return -1.0;
+    return (double)ms;
+}
+
+int nb_fp64_peak(int64_t iters, double *tflops, double *ms_out) {
+    std::lock_guard<std::mutex> lk(g_mu);
+    if (!tflops) return fail(NB_E_NULL, "tflops is NULL");
+    if (iters <= 0) iters = 4096;
+    double *d = nullptr;
+    NB_CUDA(cudaMalloc(&d, 256));
+    const int ctas = sm_count() * 8, threads = 256;
+    cudaEvent_t e0, e1;
+    NB_CUDA(cudaEventCreate(&e0));
+    NB_CUDA(cudaEventCreate(&e1));
+    nb_fp64_peak_kernel<<<ctas, threads, 0, stream()>>>(d, iters / 8 + 1, 0.999999, 1e-7);  // warm-up
+    NB_CUDA(cudaEventRecord(e0, stream()));
+    nb_fp64_peak_kernel<<<ctas, threads, 0, stream()>>>(d, iters, 0.999999, 1e-7);
+    NB_CUDA(cudaEventRecord(e1, stream()));
+    NB_CUDA(cudaEventSynchronize(e1));
+    float ms = 0.f;
+    NB_CUDA(cudaEventElapsedTime(&ms, e0, e1));
+    cudaEventDestroy(e0);
+    cudaEventDestroy(e1);
+    cudaFree(d);
+    const double fmas = (double)ctas * threads * (double)iters * 64.0;
+    *tflops = 2.0 * fmas / ((double)ms * 1e-3) / 1e12;
+    if (ms_out) *ms_out = ms;
+    return NB_OK;
+}
+
+void nb_release(void) {
+    std::lock_guard<std::mutex> lk(g_mu);
+    drop_graph();
+    if (g_arena) { cudaFree(g_arena); g_arena = nullptr; g_arena_bytes = 0; }
+    if (g_ev0) { cudaEventDestroy(g_ev0); cudaEventDestroy(g_ev1); g_ev0 = g_ev1 = nullptr; }
+    g_force_timed = false;
+}
+
+const char *nb_last_error(void) { return g_err; }
+const char *nb_version(void) { return "nbkick 0.1 (sm_100a)"; }
+
+}  // extern "C"
