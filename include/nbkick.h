@@ -64,6 +64,12 @@ typedef struct nb_config {
     int i_per_thread;        /* tuning: i-bodies held in registers per thread, 0 = auto (1,2,4) */
     int j_splits;            /* tuning: number of j-chunks the force grid is split into, 0 = auto */
     int use_graph;           /* nb_step: replay one captured CUDA graph per step (default 1) */
+    int reuse_acc;           /* nb_step: acc (and rcrit, pairs) already hold the evaluation at the current x,
+                                as left by the previous nb_step/nb_kick(dt=0) call on this state: skip the
+                                evaluation at t0, so a run stepped in chunks costs one evaluation per step
+                                (default 0) */
+    int time_force;          /* bracket every force-tile launch with CUDA events (nb_force_time); implies
+                                no graph replay (default 0) */
 } nb_config;
 
 void nb_default_config(nb_config *cfg);
@@ -154,6 +160,11 @@ int nb_status_reset(void);
 /* Milliseconds the most recent force-tile kernel of nb_kick / nb_step(nsteps=0) took, timed with
  * CUDA events on the configured stream (synchronises).  Negative if none was recorded. */
 double nb_last_force_ms(void);
+/* Sum over the force-tile launches recorded since the last nb_force_time_reset (time_force = 1):
+ * *launches and *total_ms (CUDA events on the configured stream; synchronises).  At most 4096
+ * launches are kept between resets; later ones are not recorded. */
+int nb_force_time(int64_t *launches, double *total_ms);
+int nb_force_time_reset(void);
 /* Launch geometry the force kernel would use for (N, n_active): out[0] = i-bodies per thread,
  * out[1] = i-blocks, out[2] = j-splits, out[3] = threads per CTA, out[4] = j-tile length. */
 int nb_force_geometry(int64_t N, int64_t *out5);

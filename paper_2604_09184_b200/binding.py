@@ -22,7 +22,7 @@ CHANGEOVER_RATIONAL, CHANGEOVER_QUINTIC = 0, 1
 SYMBOLS = (
     "nb_default_config", "nb_configure", "nb_workspace_bytes", "nb_rcrit", "nb_kick", "nb_shift",
     "nb_drift_kepler", "nb_step", "nb_kick_host", "nb_step_host", "nb_status", "nb_status_reset",
-    "nb_last_force_ms", "nb_force_geometry", "nb_fp64_peak", "nb_release", "nb_last_error", "nb_version",
+    "nb_last_force_ms", "nb_force_time", "nb_force_time_reset", "nb_force_geometry", "nb_fp64_peak", "nb_release", "nb_last_error", "nb_version",
 )
 
 
@@ -40,6 +40,8 @@ class NbConfig(C.Structure):
         ("i_per_thread", C.c_int),
         ("j_splits", C.c_int),
         ("use_graph", C.c_int),
+        ("reuse_acc", C.c_int),
+        ("time_force", C.c_int),
     ]
 
 
@@ -83,6 +85,8 @@ def load():
     lib.nb_status_reset.argtypes = []
     lib.nb_last_force_ms.argtypes = []
     lib.nb_last_force_ms.restype = dbl
+    lib.nb_force_time.argtypes = [C.POINTER(C.c_int64), C.POINTER(dbl)]
+    lib.nb_force_time_reset.argtypes = []
     lib.nb_force_geometry.argtypes = [i64, C.POINTER(C.c_int64)]
     lib.nb_fp64_peak.argtypes = [i64, C.POINTER(dbl), C.POINTER(dbl)]
     lib.nb_release.argtypes = []
@@ -141,7 +145,7 @@ def default_config() -> NbConfig:
 
 
 def configure(N=None, *, stream=None, pair_capacity=0, n_active=0, G=None, n1=3.0, n2=0.4, changeover_kind=0,
-              i_per_thread=0, j_splits=0, use_graph=True, device="cuda"):
+              i_per_thread=0, j_splits=0, use_graph=True, reuse_acc=False, time_force=False, device="cuda"):
     """nb_configure with a torch-allocated workspace sized for N bodies (N=None: no workspace,
     enough for the _host calls).  Keeps the workspace tensor alive."""
     lib = load()
@@ -154,6 +158,8 @@ def configure(N=None, *, stream=None, pair_capacity=0, n_active=0, G=None, n1=3.
     cfg.changeover_kind = int(changeover_kind)
     cfg.i_per_thread, cfg.j_splits = int(i_per_thread), int(j_splits)
     cfg.use_graph = 1 if use_graph else 0
+    cfg.reuse_acc = 1 if reuse_acc else 0
+    cfg.time_force = 1 if time_force else 0
     if N is not None:
         import torch
         if stream is None:
@@ -247,6 +253,27 @@ def nb_status_reset():
 
 def nb_last_force_ms() -> float:
     return float(load().nb_last_force_ms())
+
+
+def nb_force_time():
+    """(launches, total_ms) of the force-tile launches recorded since nb_force_time_reset."""
+    n, ms = C.c_int64(0), C.c_double(0.0)
+    _check(load().nb_force_time(C.byref(n), C.byref(ms)))
+    return int(n.value), float(ms.value)
+
+
+def nb_force_time_reset():
+    _check(load().nb_force_time_reset())
+
+
+def set_flags(**kw):
+    """Re-issue nb_configure with some fields of the current config changed (same workspace)."""
+    cfg = _state["cfg"]
+    if cfg is None:
+        raise RuntimeError("configure() first")
+    for k, v in kw.items():
+        setattr(cfg, k, int(v) if isinstance(v, bool) else v)
+    _check(load().nb_configure(C.byref(cfg)))
 
 
 def nb_fp64_peak(iters: int = 0):

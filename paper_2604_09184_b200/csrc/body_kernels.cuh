@@ -91,8 +91,8 @@ __global__ void __launch_bounds__(kBodyThreads) nb_rcrit_kernel(const double *__
 // a4: acc_i = sum over j-splits (in split order) of the partial sums; v_i = v_i + hk*acc_i, applied
 // nhalf times (the closing half-kick of one step and the opening half-kick of the next are two
 // separate roundings, as in the step definition).  Optionally emits momentum partials of the new v.
-__global__ void __launch_bounds__(kBodyThreads) nb_kickv_kernel(const double *__restrict__ part, int nsplit,
-                                                               double *__restrict__ acc, double *__restrict__ v,
+__global__ void __launch_bounds__(kBodyThreads) nb_kickv_kernel(const double *part, int nsplit,
+                                                               double *acc, double *__restrict__ v,
                                                                const double *__restrict__ m, int N, double hk,
                                                                int nhalf, double *__restrict__ mv_out) {
     __shared__ double sm[3 * kBodyThreads];

@@ -18,11 +18,14 @@ namespace {
 using namespace nbk;
 
 std::mutex g_mu;
-nb_config g_cfg = {nullptr, nullptr, 0, 0, 0, 0.01720209895 * 0.01720209895, 3.0, 0.4, 0, 0, 0, 1};
+nb_config g_cfg = {nullptr, nullptr, 0, 0, 0, 0.01720209895 * 0.01720209895, 3.0, 0.4, 0, 0, 0, 1, 0, 0};
 char g_err[512] = "";
 int g_sm_count = 0;
 cudaEvent_t g_ev0 = nullptr, g_ev1 = nullptr;
 bool g_force_timed = false;
+constexpr int kMaxTimed = 4096;
+cudaEvent_t g_tev[2 * kMaxTimed];
+int g_tev_created = 0, g_tev_used = 0;
 
 // private arena of the _host entry points
 void *g_arena = nullptr;
@@ -195,12 +198,21 @@ int enqueue_eval(const Workspace &w, const Geometry &g, double *x, double *v, co
     fp.npairs = pairs ? reinterpret_cast<unsigned long long *>(npairs) : w.npairs_dummy;
     fp.status = w.status; fp.cap = pairs ? g_cfg.pair_capacity : 0; fp.N = (int)N; fp.Nj = g.Nj;
     fp.tiles_total = g.tiles_total; fp.tiles_per_split = g.tiles_per_split; fp.kind = g_cfg.changeover_kind;
-    if (time_force) {
+    const bool pool = g_cfg.time_force && g_tev_used < kMaxTimed;
+    if (pool) {
+        while (g_tev_created <= g_tev_used) {
+            NB_CUDA(cudaEventCreate(&g_tev[2 * g_tev_created]));
+            NB_CUDA(cudaEventCreate(&g_tev[2 * g_tev_created + 1]));
+            ++g_tev_created;
+        }
+        NB_CUDA(cudaEventRecord(g_tev[2 * g_tev_used], stream()));
+    } else if (time_force) {
         if (!g_ev0) { NB_CUDA(cudaEventCreate(&g_ev0)); NB_CUDA(cudaEventCreate(&g_ev1)); }
         NB_CUDA(cudaEventRecord(g_ev0, stream()));
     }
     launch_force(fp, g, pairs != nullptr);
-    if (time_force) { NB_CUDA(cudaEventRecord(g_ev1, stream())); g_force_timed = true; }
+    if (pool) { NB_CUDA(cudaEventRecord(g_tev[2 * g_tev_used + 1], stream())); ++g_tev_used; }
+    else if (time_force) { NB_CUDA(cudaEventRecord(g_ev1, stream())); g_force_timed = true; }
 
     nb_kickv_kernel<<<nblk, kBodyThreads, 0, stream()>>>(w.part, g.nsplit, acc, v, m, (int)N, hk, nhalf, mv_out);
     NB_CUDA(cudaGetLastError());
@@ -243,10 +255,15 @@ int step_impl(double *x, double *v, const double *m, double M_star, int64_t N, d
     const double hk = 0.5 * dt, dtc = 0.5 * dt, mu = g_cfg.G * M_star;
     const int nblk = body_blocks(N);
 
-    // evaluation at t0 (+ opening half-kick of the first step)
-    if ((rc = enqueue_eval(w, g, x, v, m, M_star, N, dt, rc_io, update_rc, nullptr, 0.0, acc, pairs, npairs, hk,
-                           nsteps > 0 ? 1 : 0, w.mvA, nsteps == 0)))
-        return rc;
+    if (g_cfg.reuse_acc && nsteps > 0) {
+        // acc already is the force at the current x: opening half-kick only (reads acc as a 1-split partial)
+        nb_kickv_kernel<<<nblk, kBodyThreads, 0, stream()>>>(acc, 1, acc, v, m, (int)N, hk, 1, w.mvA);
+    } else {
+        // evaluation at t0 (+ opening half-kick of the first step)
+        if ((rc = enqueue_eval(w, g, x, v, m, M_star, N, dt, rc_io, update_rc, nullptr, 0.0, acc, pairs, npairs, hk,
+                               nsteps > 0 ? 1 : 0, w.mvA, nsteps == 0)))
+            return rc;
+    }
 
     auto enqueue_step = [&](int nhalf) -> int {
         // C(dt/2) A(dt): first half-shift folded into the drift kernel
@@ -258,7 +275,7 @@ int step_impl(double *x, double *v, const double *m, double M_star, int64_t N, d
     };
 
     const int64_t interior = nsteps > 0 ? nsteps - 1 : 0;
-    if (interior > 0 && g_cfg.use_graph) {
+    if (interior > 0 && g_cfg.use_graph && !g_cfg.time_force) {
         StepKey key;
         std::memset(&key, 0, sizeof(key));
         key.x = x; key.v = v; key.m = m; key.rcrit = rc_io; key.acc = acc; key.pairs = pairs; key.npairs = npairs;
@@ -315,6 +332,8 @@ void nb_default_config(nb_config *cfg) {
     cfg->n2 = 0.4;
     cfg->changeover_kind = NB_CHANGEOVER_RATIONAL;
     cfg->use_graph = 1;
+    cfg->reuse_acc = 0;
+    cfg->time_force = 0;
 }
 
 int nb_configure(const nb_config *cfg) {
@@ -500,6 +519,27 @@ double nb_last_force_ms(void) {
     return (double)ms;
 }
 
+int nb_force_time(int64_t *launches, double *total_ms) {
+    std::lock_guard<std::mutex> lk(g_mu);
+    if (!launches || !total_ms) return fail(NB_E_NULL, "nb_force_time: NULL argument");
+    double tot = 0.0;
+    for (int k = 0; k < g_tev_used; ++k) {
+        NB_CUDA(cudaEventSynchronize(g_tev[2 * k + 1]));
+        float ms = 0.f;
+        NB_CUDA(cudaEventElapsedTime(&ms, g_tev[2 * k], g_tev[2 * k + 1]));
+        tot += ms;
+    }
+    *launches = g_tev_used;
+    *total_ms = tot;
+    return NB_OK;
+}
+
+int nb_force_time_reset(void) {
+    std::lock_guard<std::mutex> lk(g_mu);
+    g_tev_used = 0;
+    return NB_OK;
+}
+
 int nb_fp64_peak(int64_t iters, double *tflops, double *ms_out) {
     std::lock_guard<std::mutex> lk(g_mu);
     if (!tflops) return fail(NB_E_NULL, "tflops is NULL");
@@ -531,6 +571,8 @@ void nb_release(void) {
     drop_graph();
     if (g_arena) { cudaFree(g_arena); g_arena = nullptr; g_arena_bytes = 0; }
     if (g_ev0) { cudaEventDestroy(g_ev0); cudaEventDestroy(g_ev1); g_ev0 = g_ev1 = nullptr; }
+    for (int k = 0; k < 2 * g_tev_created; ++k) cudaEventDestroy(g_tev[k]);
+    g_tev_created = g_tev_used = 0;
     g_force_timed = false;
 }
 
