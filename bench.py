@@ -1,0 +1,344 @@
+#!/usr/bin/env python
+"""bench.py -- whole hot path (one nb_step = rcrit + O(N^2) kick tiles + pair list + H_C shifts + Kepler
+drift) on the synthetic N = 65536 ring of BASELINE.json:configs[2], the configuration the metric
+("fp64 pairwise interactions/sec ...; steps/sec at N=65536") is quoted on.
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl cuda|reference] [--config k]
+
+Prints ONE JSON line (rank 0).  `value` = ordered (i,j) interactions evaluated per second by all ranks,
+inputs resident in HBM; `e2e` = the same through the host-buffer C-ABI call (nb_step_host) with the
+host<->device copies inside the timed region; `roofline` = the force-tile kernel against the B200 fp64
+FMA peak (bound "alu"); `cpu_baseline` = the CPU oracle timed beside it on a bounded sample.
+--impl reference times the CPU oracle alone (test infrastructure; the one other place that runs it).
+The path does not shard (BASELINE.json:north_star: one GPU, no collectives): --gpus N runs N
+independent replicas ("replicas only"), one process per GPU, no data-path collective.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import nb_inputs  # noqa: E402  (seeded input generators only; none of the method's arithmetic)
+from nb_inputs import G_GAUSS  # noqa: E402
+
+METRIC = "fp64_pairwise_interactions_per_sec"
+UNIT = "interactions/s"
+FLOPS_PER_INTERACTION = 20.0  # BASELINE.json:north_star "about 20 flops counted per interaction"
+# fp64 FMA peak of a B200 from unit counts and clocks: 148 SMs x 64 fp64 lanes
+# x 2 flop x 1.965 GHz (clocks.max.sm)
+FP64_PEAK_NOMINAL_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12
+N1, N2 = 3.0, 0.0  # headline radius: 3 Hill radii (BASELINE.json:configs[0]; S7)
+
+
+def parse_args():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=100)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
+    ap.add_argument("--config", type=int, default=2, help="index into BASELINE.json:configs (default 2: N=65536)")
+    ap.add_argument("--n", type=int, default=None, help="override the body count (debugging only)")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    return ap.parse_args()
+
+
+class ClockSampler:
+    """nvidia-smi clocks + throttle reasons sampled every 100 ms while the timed region runs."""
+
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index = index
+        self.proc = None
+        self.path = f"/tmp/nb_clocks_{os.getpid()}.csv"
+
+    def start(self):
+        try:
+            self.fh = open(self.path, "w")
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}",
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=self.fh, stderr=subprocess.DEVNULL)
+        except Exception:
+            self.proc = None
+
+    def stop(self) -> dict:
+        out = dict(sm_mhz=None, sm_max_mhz=None, power_w_max=None, reasons=[], samples=0)
+        if self.proc is None:
+            return out
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except Exception:
+            self.proc.kill()
+        self.fh.close()
+        sm, mx, pw, reasons = [], [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        try:
+            for line in open(self.path):
+                f = [t.strip() for t in line.split(",")]
+                if len(f) < 7:
+                    continue
+                try:
+                    sm.append(float(f[0])); mx.append(float(f[1])); pw.append(float(f[2]))
+                except ValueError:
+                    continue
+                for nm, val in zip(names, f[3:7]):
+                    if val.lower().startswith("active"):
+                        reasons.add(nm)
+            os.remove(self.path)
+        except Exception:
+            pass
+        if sm:
+            out.update(sm_mhz=statistics.median(sm), sm_max_mhz=max(mx), power_w_max=max(pw), samples=len(sm))
+        out["reasons"] = sorted(reasons)
+        return out
+
+
+def workload(args):
+    d = nb_inputs.make_config(args.config, n_override=args.n)
+    na = d.n_active if d.n_active < d.N else 0
+    return d, na
+
+
+def workload_name(d, na):
+    return (f"{d.name}: N={d.N}" + (f" (n_active={na})" if na else "") +
+            f", dt={d.dt:g} d, rcrit = {N1:g} R_Hill (n2={N2:g}), seed {d.seed}, synthetic disk (DESIGN.md input recipe)")
+
+
+# ------------------------------------------------------------------------------------------------
+# CPU oracle legs (test infrastructure, timed as it stands; never tuned for this)
+# ------------------------------------------------------------------------------------------------
+def oracle_sample_step(d, na, rows, state):
+    """One pass of the hot path by the oracle with the O(N^2) parts restricted to `rows` i-bodies
+    (all j): rcrit, accelerations + pairs of the sampled rows, half-kicks, H_C shifts, Kepler drift.
+    Returns (seconds, interactions evaluated)."""
+    import oracle
+    x, v = state
+    t0 = time.perf_counter()
+    rc = oracle.rcrit(x, v, d.m, d.M_star, d.dt, G_GAUSS, N1, N2)
+    acc, _, _ = oracle.accel(x, d.m, rc, G_GAUSS, n_active=na, rows=rows)
+    oracle.pairs(x, rc, n_active=na, rows=rows)
+    v = v.copy()
+    v[rows] = v[rows] + (0.5 * d.dt) * acc
+    x = oracle.shift(x, v, d.m, d.M_star, 0.5 * d.dt)
+    x, v, _ = oracle.drift_kepler(x, v, d.M_star, d.dt, G_GAUSS)
+    x = oracle.shift(x, v, d.m, d.M_star, 0.5 * d.dt)
+    dt = time.perf_counter() - t0
+    state[0], state[1] = x, v
+    return dt, rows.size * (na or d.N)
+
+
+def cpu_baseline(d, na, budget_s=12.0):
+    import oracle
+    rng = np.random.default_rng(77)
+    state = [d.x.copy(), d.v.copy()]
+    probe = np.sort(rng.choice(d.N, size=min(256, d.N), replace=False))
+    t, n = oracle_sample_step(d, na, probe, state)
+    rate = n / t
+    R = int(min(d.N, max(256, budget_s * rate / (na or d.N))))
+    rows = np.sort(rng.choice(d.N, size=R, replace=False))
+    t, n = oracle_sample_step(d, na, rows, state)
+    return dict(value=n / t, unit=UNIT, cores=oracle.num_threads(), kind="oracle",
+                sample=f"one oracle step with the O(N^2) kick + pair test on {R} seeded-random i-rows x all "
+                       f"{na or d.N} j (rcrit, shifts, Kepler drift on all N): {n:.3e} interactions in {t:.2f} s")
+
+
+def run_reference(args):
+    """--impl reference: the CPU oracle as it stands on this box's host cores; each step a bounded sample."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    import oracle
+    d, na = workload(args)
+    rng = np.random.default_rng(78)
+    state = [d.x.copy(), d.v.copy()]
+    probe = np.sort(rng.choice(d.N, size=min(128, d.N), replace=False))
+    t, n = oracle_sample_step(d, na, probe, state)
+    total_steps = args.steps + args.warmup
+    budget = 150.0  # seconds for the whole run
+    R = int(min(d.N, max(32, budget / total_steps * (n / t) / (na or d.N))))
+    rows = np.sort(rng.choice(d.N, size=R, replace=False))
+    for _ in range(args.warmup):
+        oracle_sample_step(d, na, rows, state)
+    tt, nn = 0.0, 0
+    for _ in range(args.steps):
+        t, n = oracle_sample_step(d, na, rows, state)
+        tt += t
+        nn += n
+    value = nn / tt
+    sample = (f"each step: oracle O(N^2) kick + pair test on {R} seeded-random i-rows x all {na or d.N} j, "
+              f"O(N) parts on all N; {args.steps} steps, {nn:.3e} interactions in {tt:.2f} s")
+    line = dict(impl="reference", metric=METRIC, value=value, unit=UNIT, n_gpus=args.gpus, steps=args.steps,
+                warmup=args.warmup, ms_per_step=1e3 * tt / max(args.steps, 1), higher_is_better=True, scaling="weak",
+                vs_baseline=None, dtype="f64 (x87 extended accumulators)", data="synthetic",
+                config=dict(workload=workload_name(d, na), sample=sample),
+                cpu_baseline=dict(value=value, unit=UNIT, cores=oracle.num_threads(), kind="oracle", sample=sample),
+                e2e=dict(value=value, unit=UNIT, h2d_bytes_per_step=0, d2h_bytes_per_step=0), gpu_launches=0)
+    print(json.dumps(line), flush=True)
+
+
+# ------------------------------------------------------------------------------------------------
+# CUDA arm
+# ------------------------------------------------------------------------------------------------
+def _traffic_from_profile():
+    """dram bytes per force-kernel launch from the committed ncu capture (profiles/), or None."""
+    p = os.path.join(ROOT, "profiles", "force_kernel_traffic.json")
+    try:
+        return json.load(open(p)).get("dram_bytes_per_launch")
+    except Exception:
+        return None
+
+
+def run_cuda(args):
+    import torch
+    import torch.distributed as dist
+    import paper_2604_09184_b200 as nb
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py --impl cuda needs a CUDA device: there is no CPU fallback")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    d, na = workload(args)
+    N, Nj = d.N, (na or d.N)
+    inter_per_step = float(N) * float(Nj)
+    cap = 1 << 22
+    K, W = args.steps, max(args.warmup, 0)
+
+    # ---- device-resident arm: inputs in HBM before the timed region -------------------------------
+    nb.configure(N, pair_capacity=cap, n_active=na, G=G_GAUSS, n1=N1, n2=N2, reuse_acc=False, time_force=True)
+    nb.nb_status_reset()
+    x = torch.from_numpy(d.x).cuda(); v = torch.from_numpy(d.v).cuda(); m = torch.from_numpy(d.m).cuda()
+    acc = torch.zeros_like(x); rc = torch.zeros(N, dtype=torch.float64, device="cuda")
+    pairs = torch.zeros((cap, 2), dtype=torch.int32, device="cuda")
+    npairs = torch.zeros(1, dtype=torch.int64, device="cuda")
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")  # > 126 MB L2
+    geom = nb.force_geometry(N)
+
+    nb.nb_step(x, v, m, d.M_star, d.dt, rc, acc, pairs, npairs, 0)  # evaluation at t0 (start-up, untimed)
+    nb.set_flags(reuse_acc=1)  # from here on: exactly one force evaluation per step
+    for _ in range(W):
+        nb.nb_step(x, v, m, d.M_star, d.dt, rc, acc, pairs, npairs, 1)
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(K)]
+    sampler = ClockSampler(local)
+    barrier()
+    nb.nb_force_time_reset()
+    sampler.start()
+    wall0 = time.perf_counter()
+    for k in range(K):
+        flush.fill_(k & 0xFF)  # L2 flush between timed iterations (outside the per-step events)
+        ev[k][0].record()
+        nb.nb_step(x, v, m, d.M_star, d.dt, rc, acc, pairs, npairs, 1)
+        ev[k][1].record()
+    barrier()
+    wall = time.perf_counter() - wall0
+    clocks = sampler.stop()
+    step_ms = [a.elapsed_time(b) for a, b in ev]
+    total_ms = float(sum(step_ms))
+    n_force, force_ms = nb.nb_force_time()
+    status = nb.nb_status()
+    npairs_last = int(npairs.item())
+    peak_tf, _ = nb.nb_fp64_peak(8192)
+
+    # ---- end-to-end arm: host buffers through nb_step_host, copies inside the timed region ---------
+    e2e = None
+    if not args.no_e2e:
+        Ke = max(3, min(K, 20))
+        nb.set_flags(reuse_acc=0, time_force=0)
+        hx, hv, hm = d.x.copy(), d.v.copy(), d.m.copy()
+        hacc, hrc = np.zeros((N, 3)), np.zeros(N)
+        hpairs, hnp = np.zeros((cap, 2), dtype=np.int32), np.zeros(1, dtype=np.int64)
+        nb.nb_step_host(hx, hv, hm, d.M_star, d.dt, hrc, hacc, hpairs, hnp, 0)  # t0 evaluation, result lands on the host
+        nb.set_flags(reuse_acc=1)
+        for _ in range(min(W, 3)):
+            nb.nb_step_host(hx, hv, hm, d.M_star, d.dt, hrc, hacc, hpairs, hnp, 1)
+        barrier()
+        t0 = time.perf_counter()
+        for _ in range(Ke):
+            nb.nb_step_host(hx, hv, hm, d.M_star, d.dt, hrc, hacc, hpairs, hnp, 1)  # synchronises
+        barrier()
+        te = time.perf_counter() - t0
+        h2d = 8 * (3 * N + 3 * N + N + N + 3 * N)            # x, v, m, rcrit, acc (cached force)
+        d2h = 8 * (3 * N + 3 * N + 3 * N + N) + 8 + 8 * int(hnp[0])  # x, v, acc, rcrit, npairs, pairs
+        e2e = dict(te=te, Ke=Ke, h2d=h2d, d2h=d2h)
+        nb.set_flags(reuse_acc=0)
+
+    # ---- max over ranks (replicas: no data-path collective; this is only the timing reduction) -----
+    if world > 1:
+        t = torch.tensor([total_ms, e2e["te"] if e2e else 0.0], dtype=torch.float64, device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        total_ms = float(t[0].item())
+        if e2e:
+            e2e["te"] = float(t[1].item())
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+
+    value = world * K * inter_per_step / (total_ms * 1e-3)
+    force_avg_ms = force_ms / max(n_force, 1)
+    achieved_tf = FLOPS_PER_INTERACTION * inter_per_step / (force_avg_ms * 1e-3) / 1e12
+    line = dict(
+        metric=METRIC, value=value, unit=UNIT, n_gpus=world, steps=K, warmup=W, ms_per_step=total_ms / K,
+        higher_is_better=True, scaling="weak", vs_baseline=None, dtype="f64", data="synthetic",
+        config=dict(workload=workload_name(d, na), parallelism="replicas only (path does not shard)" if world > 1 else "1 GPU",
+                    l2="256 MiB buffer written between timed steps (L2 flush), outside the per-step CUDA events",
+                    force_evaluations_per_step=1, interactions_per_step=inter_per_step,
+                    geometry=dict(i_per_thread=geom.i_per_thread, i_blocks=geom.i_blocks, j_splits=geom.j_splits,
+                                  threads=geom.threads, tile_j=geom.tile_j),
+                    pairs_last_step=npairs_last, status=status, wall_s_incl_flush=wall),
+        steps_per_sec=world * K / (total_ms * 1e-3),
+        roofline=dict(bound="alu", achieved=achieved_tf, peak=FP64_PEAK_NOMINAL_TFLOPS, unit="TFLOP/s",
+                      frac=achieved_tf / FP64_PEAK_NOMINAL_TFLOPS, traffic=_traffic_from_profile(),
+                      kernel="nb_force_tiles_kernel", launches_timed=n_force, avg_launch_ms=force_avg_ms,
+                      flops_per_interaction=FLOPS_PER_INTERACTION,
+                      peak_source="nominal: 148 SM x 64 fp64 lanes x 2 x 1.965 GHz (DESIGN.md); MEASURED_PEAKS.json has no fp64 entry",
+                      peak_measured_dfma=peak_tf, frac_of_measured_dfma=achieved_tf / peak_tf if peak_tf > 0 else None,
+                      fp64_pipe_instr_per_interaction=15,
+                      fp64_pipe_util_est=15.0 * inter_per_step / (force_avg_ms * 1e-3) / (peak_tf * 1e12 / 2.0) if peak_tf > 0 else None),
+        clocks=clocks, gpu_launches=4 * K,
+    )
+    if e2e:
+        line["e2e"] = dict(value=world * e2e["Ke"] * inter_per_step / e2e["te"], unit=UNIT,
+                           h2d_bytes_per_step=e2e["h2d"], d2h_bytes_per_step=e2e["d2h"], steps=e2e["Ke"],
+                           call="nb_step_host(nsteps=1, reuse_acc=1): pageable numpy buffers in, results out, stream synchronised")
+    if not args.no_cpu_baseline:
+        line["cpu_baseline"] = cpu_baseline(d, na)
+    print(json.dumps(line), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    args = parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_cuda(args)
+
+
+if __name__ == "__main__":
+    main()

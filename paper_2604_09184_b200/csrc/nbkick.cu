@@ -453,6 +453,7 @@ static int host_run(bool is_step, double *x, double *v, const double *m, double 
         NB_CUDA(cudaMemcpyAsync(dv, v, b3, cudaMemcpyHostToDevice, s));
         NB_CUDA(cudaMemcpyAsync(dm, m, b1, cudaMemcpyHostToDevice, s));
         if (rcrit) NB_CUDA(cudaMemcpyAsync(drc, rcrit, b1, cudaMemcpyHostToDevice, s));
+        if (is_step && g_cfg.reuse_acc) NB_CUDA(cudaMemcpyAsync(dacc, acc, b3, cudaMemcpyHostToDevice, s));  // cached force
         int r;
         if (is_step) r = step_impl(dx, dv, dm, M_star, N, dt, rcrit ? drc : nullptr, dacc, dpairs, pairs ? dnp : nullptr, nsteps);
         else r = kick_impl(dx, dv, dm, M_star, N, dt, rcrit ? drc : nullptr, dacc, dpairs, pairs ? dnp : nullptr);
