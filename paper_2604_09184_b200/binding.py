@@ -41,6 +41,8 @@ class NbConfig(C.Structure):
         ("j_splits", C.c_int),
         ("use_graph", C.c_int),
         ("reuse_acc", C.c_int),
+        ("ctas_per_sm", C.c_int),
+        ("pipeline_j", C.c_int),
         ("time_force", C.c_int),
     ]
 
@@ -145,7 +147,8 @@ def default_config() -> NbConfig:
 
 
 def configure(N=None, *, stream=None, pair_capacity=0, n_active=0, G=None, n1=3.0, n2=0.4, changeover_kind=0,
-              i_per_thread=0, j_splits=0, use_graph=True, reuse_acc=False, time_force=False, device="cuda"):
+              i_per_thread=0, j_splits=0, use_graph=True, reuse_acc=False, time_force=False, ctas_per_sm=0,
+              pipeline_j=0, device="cuda"):
     """nb_configure with a torch-allocated workspace sized for N bodies (N=None: no workspace,
     enough for the _host calls).  Keeps the workspace tensor alive."""
     lib = load()
@@ -160,6 +163,7 @@ def configure(N=None, *, stream=None, pair_capacity=0, n_active=0, G=None, n1=3.
     cfg.use_graph = 1 if use_graph else 0
     cfg.reuse_acc = 1 if reuse_acc else 0
     cfg.time_force = 1 if time_force else 0
+    cfg.ctas_per_sm, cfg.pipeline_j = int(ctas_per_sm), int(pipeline_j)
     if N is not None:
         import torch
         if stream is None:

@@ -5,7 +5,7 @@
 //
 // Grid: blockIdx.x = i-block of kForceThreads*I bodies (I bodies per thread, in registers),
 //       blockIdx.y = j-split (a contiguous range of j-tiles).  Each CTA streams its j-range through
-//       a two-stage shared-memory ring filled by TMA bulk copies (cp.async.bulk + mbarrier) of
+//       a four-stage shared-memory ring filled by TMA bulk copies (cp.async.bulk, full/empty mbarriers) of
 //       64-byte JRec records; every lane of a warp reads the same j => pure broadcasts.
 // Out:  part[split][i][3], summed in split order by nb_kickv_kernel (deterministic two-level sum).
 //
@@ -150,10 +150,41 @@ __device__ __forceinline__ void slow_path(const ForceParams &p, const double4 A,
     }
 }
 
-template <int I, bool PAIRS>
-__global__ void __launch_bounds__(kForceThreads) nb_force_tiles_kernel(const ForceParams p) {
+__device__ __forceinline__ void mbar_arrive(uint64_t *bar) {
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
+
+// One j against the thread's I bodies: differences, r^2 and the running minimum of the high words.
+template <int I>
+struct JWork {
+    double4 A, B;  // A = x, y, z, G m ; B = 3/2 G m, 15/8 G m, rc^2, rc
+    double dx[I], dy[I], dz[I], r2[I];
+    int mn, thr;
+    __device__ __forceinline__ void load(const JRec *rec, const double (&xi)[I], const double (&yi)[I],
+                                         const double (&zi)[I], const int thr_i) {
+        const double4 *q = reinterpret_cast<const double4 *>(rec);
+        A = q[0];
+        B = q[1];
+        thr = max(thr_i, __double2hiint(B.z) + 1);
+        mn = 0x7fffffff;
+#pragma unroll
+        for (int k = 0; k < I; ++k) {
+            dx[k] = __dsub_rn(A.x, xi[k]);
+            dy[k] = __dsub_rn(A.y, yi[k]);
+            dz[k] = __dsub_rn(A.z, zi[k]);
+            r2[k] = __fma_rn(dz[k], dz[k], __fma_rn(dy[k], dy[k], __dmul_rn(dx[k], dx[k])));
+            mn = min(mn, __double2hiint(r2[k]));
+        }
+    }
+};
+
+// MINB = CTAs per SM the register allocation is capped for; PIPE = software-pipeline the j loop
+// (differences and r^2 of j+1 are issued between the vote on j and its branch).
+template <int I, bool PAIRS, int MINB, bool PIPE>
+__global__ void __launch_bounds__(kForceThreads, MINB) nb_force_tiles_kernel(const ForceParams p) {
     __shared__ __align__(128) JRec sm[kStages][kTileJ];
-    __shared__ __align__(8) uint64_t bar[kStages];
+    __shared__ __align__(8) uint64_t full[kStages];
+    __shared__ __align__(8) uint64_t empty[kStages];
 
     const int t = threadIdx.x;
     const int i0 = blockIdx.x * (kForceThreads * I) + t;
@@ -161,19 +192,26 @@ __global__ void __launch_bounds__(kForceThreads) nb_force_tiles_kernel(const For
     int tile_end = tile_begin + p.tiles_per_split;
     if (tile_end > p.tiles_total) tile_end = p.tiles_total;
     const int ntiles = tile_end - tile_begin;
+    constexpr unsigned kTileBytes = kTileJ * sizeof(JRec);
+    constexpr int kAhead = kStages - 2;  // tiles in flight ahead of the one being consumed
 
     if (t == 0) {
 #pragma unroll
-        for (int s = 0; s < kStages; ++s) mbar_init(&bar[s], 1);
+        for (int s = 0; s < kStages; ++s) {
+            mbar_init(&full[s], 1);
+            mbar_init(&empty[s], kForceThreads / 32);
+        }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
         asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
     }
     __syncthreads();
-
-    constexpr unsigned kTileBytes = kTileJ * sizeof(JRec);
-    if (t == 0 && ntiles > 0) {
-        mbar_expect_tx(&bar[0], kTileBytes);
-        tma_bulk_g2s(&sm[0][0], p.jrec + (size_t)tile_begin * kTileJ, kTileBytes, &bar[0]);
+    if (t == 0) {
+#pragma unroll
+        for (int n = 0; n < kAhead; ++n)
+            if (n < ntiles) {
+                mbar_expect_tx(&full[n], kTileBytes);
+                tma_bulk_g2s(&sm[n][0], p.jrec + (size_t)(tile_begin + n) * kTileJ, kTileBytes, &full[n]);
+            }
     }
 
     // i-bodies in registers
@@ -199,53 +237,73 @@ __global__ void __launch_bounds__(kForceThreads) nb_force_tiles_kernel(const For
     for (int k = 0; k < I; ++k) { ox[k] = 0.0; oy[k] = 0.0; oz[k] = 0.0; }
 
     for (int it = 0; it < ntiles; ++it) {
-        const int st = it & 1;
-        if (t == 0 && it + 1 < ntiles) {  // stage st^1 was released by the __syncthreads of iteration it-1
-            mbar_expect_tx(&bar[st ^ 1], kTileBytes);
-            tma_bulk_g2s(&sm[st ^ 1][0], p.jrec + (size_t)(tile_begin + it + 1) * kTileJ, kTileBytes, &bar[st ^ 1]);
+        const int st = it % kStages;
+        {
+            // refill the stage that tile it - 2 used.  Every thread takes the (almost always already
+            // satisfied) wait so that control flow stays warp-uniform; one thread issues the copy.
+            const int n = it + kAhead;
+            if (n < ntiles) {
+                const int sn = n % kStages;
+                if (n >= kStages) mbar_wait(&empty[sn], (unsigned)((n / kStages - 1) & 1));
+                if (t == 0) {
+                    mbar_expect_tx(&full[sn], kTileBytes);
+                    tma_bulk_g2s(&sm[sn][0], p.jrec + (size_t)(tile_begin + n) * kTileJ, kTileBytes, &full[sn]);
+                }
+            }
         }
-        mbar_wait(&bar[st], (unsigned)((it >> 1) & 1));
+        mbar_wait(&full[st], (unsigned)((it / kStages) & 1));
 
         double ax[I], ay[I], az[I];
 #pragma unroll
         for (int k = 0; k < I; ++k) { ax[k] = 0.0; ay[k] = 0.0; az[k] = 0.0; }
         const int jbase = (tile_begin + it) * kTileJ;
+        const JRec *tile = &sm[st][0];
 
-#pragma unroll 2
-        for (int jj = 0; jj < kTileJ; ++jj) {
-            const double4 *rec = reinterpret_cast<const double4 *>(&sm[st][jj]);
-            const double4 A = rec[0];  // x, y, z, G m
-            const double4 B = rec[1];  // 3/2 G m, 15/8 G m, rc^2, rc
-            const int thr = max(thr_i, __double2hiint(B.z) + 1);
-            double dx[I], dy[I], dz[I], r2[I];
-            int mn = 0x7fffffff;
+        auto fast = [&](const JWork<I> &w, const double (&y0)[I]) {
 #pragma unroll
             for (int k = 0; k < I; ++k) {
-                dx[k] = __dsub_rn(A.x, xi[k]);
-                dy[k] = __dsub_rn(A.y, yi[k]);
-                dz[k] = __dsub_rn(A.z, zi[k]);
-                r2[k] = __fma_rn(dz[k], dz[k], __fma_rn(dy[k], dy[k], __dmul_rn(dx[k], dx[k])));
-                mn = min(mn, __double2hiint(r2[k]));
+                const double u = __dmul_rn(y0[k], y0[k]);
+                const double e = __fma_rn(-w.r2[k], u, 1.0);
+                const double h = __fma_rn(e, __fma_rn(e, w.B.y, w.B.x), w.A.w);
+                const double s = __dmul_rn(__dmul_rn(u, y0[k]), h);
+                ax[k] = __fma_rn(s, w.dx[k], ax[k]);
+                ay[k] = __fma_rn(s, w.dy[k], ay[k]);
+                az[k] = __fma_rn(s, w.dz[k], az[k]);
             }
-            if (__any_sync(0xffffffffu, mn <= thr)) {
-                slow_path<I, PAIRS>(p, A, B, jbase + jj, xi, yi, zi, rci, i0, ax, ay, az);
-            } else {
+        };
+
+        if (PIPE) {
+            JWork<I> cur, nxt;
+            cur.load(tile, xi, yi, zi, thr_i);
+#pragma unroll 2
+            for (int jj = 0; jj < kTileJ; ++jj) {
+                double y0[I];
 #pragma unroll
-                for (int k = 0; k < I; ++k) {
-                    const double y0 = rsqrt_seed(r2[k]);
-                    const double u = __dmul_rn(y0, y0);
-                    const double e = __fma_rn(-r2[k], u, 1.0);
-                    const double h = __fma_rn(e, __fma_rn(e, B.y, B.x), A.w);
-                    const double s = __dmul_rn(__dmul_rn(u, y0), h);
-                    ax[k] = __fma_rn(s, dx[k], ax[k]);
-                    ay[k] = __fma_rn(s, dy[k], ay[k]);
-                    az[k] = __fma_rn(s, dz[k], az[k]);
-                }
+                for (int k = 0; k < I; ++k) y0[k] = rsqrt_seed(cur.r2[k]);  // speculative: unused on the slow path
+                const bool hit = __any_sync(0xffffffffu, cur.mn <= cur.thr);
+                if (jj + 1 < kTileJ) nxt.load(tile + jj + 1, xi, yi, zi, thr_i);
+                if (hit) slow_path<I, PAIRS>(p, cur.A, cur.B, jbase + jj, xi, yi, zi, rci, i0, ax, ay, az);
+                else fast(cur, y0);
+                cur = nxt;
+            }
+        } else {
+#pragma unroll 2
+            for (int jj = 0; jj < kTileJ; ++jj) {
+                JWork<I> cur;
+                cur.load(tile + jj, xi, yi, zi, thr_i);
+                double y0[I];
+#pragma unroll
+                for (int k = 0; k < I; ++k) y0[k] = rsqrt_seed(cur.r2[k]);
+                if (__any_sync(0xffffffffu, cur.mn <= cur.thr))
+                    slow_path<I, PAIRS>(p, cur.A, cur.B, jbase + jj, xi, yi, zi, rci, i0, ax, ay, az);
+                else
+                    fast(cur, y0);
             }
         }
 #pragma unroll
         for (int k = 0; k < I; ++k) { ox[k] += ax[k]; oy[k] += ay[k]; oz[k] += az[k]; }
-        __syncthreads();  // everyone is done with stage st before TMA refills it
+        __syncwarp();
+        if ((t & 31) == 0) mbar_arrive(&empty[st]);  // this warp is done with stage st
     }
 
     double *out = p.part + (size_t)blockIdx.y * p.N * 3;

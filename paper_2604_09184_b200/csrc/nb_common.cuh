@@ -19,7 +19,7 @@ static_assert(sizeof(JRec) == 64, "JRec must be 64 bytes");
 
 constexpr int kForceThreads = 128;  // threads per force CTA
 constexpr int kTileJ = 128;         // j-bodies per shared-memory stage (8 KB)
-constexpr int kStages = 2;          // TMA double buffer
+constexpr int kStages = 4;          // TMA ring depth (2 tiles in flight ahead of the consumer)
 constexpr int kBodyThreads = 256;   // threads per CTA of the O(N) kernels
 constexpr double kFarJ = 1.0e30;    // padding j-records sit here with zero mass
 constexpr double kFarI = -1.0e30;   // padding i-lanes sit here; their sums are discarded

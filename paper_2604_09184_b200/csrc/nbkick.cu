@@ -18,7 +18,7 @@ namespace {
 using namespace nbk;
 
 std::mutex g_mu;
-nb_config g_cfg = {nullptr, nullptr, 0, 0, 0, 0.01720209895 * 0.01720209895, 3.0, 0.4, 0, 0, 0, 1, 0, 0};
+nb_config g_cfg = {nullptr, nullptr, 0, 0, 0, 0.01720209895 * 0.01720209895, 3.0, 0.4, 0, 0, 0, 1, 0, 0, 0, 0};
 char g_err[512] = "";
 int g_sm_count = 0;
 cudaEvent_t g_ev0 = nullptr, g_ev1 = nullptr;
@@ -57,7 +57,17 @@ int fail(int code, const char *fmt, ...) {
     } while (0)
 
 inline size_t align_up(size_t a, size_t b) { return (a + b - 1) / b * b; }
-inline cudaStream_t stream() { return static_cast<cudaStream_t>(g_cfg.stream); }
+// Graph capture needs a capturable stream; the legacy default stream (what torch hands out unless the
+// caller made its own) is not.  Graph replay then runs on a private stream ordered against the
+// caller's stream with events, so the calls stay stream-ordered as include/nbkick.h promises.
+cudaStream_t g_own_stream = nullptr;
+cudaEvent_t g_ev_in = nullptr, g_ev_out = nullptr;
+bool g_on_own_stream = false;
+inline cudaStream_t stream() { return g_on_own_stream ? g_own_stream : static_cast<cudaStream_t>(g_cfg.stream); }
+inline bool stream_capturable() {
+    const uintptr_t h = reinterpret_cast<uintptr_t>(g_cfg.stream);
+    return h > 2;  // 0 = legacy default, 1 = cudaStreamLegacy, 2 = cudaStreamPerThread
+}
 
 int sm_count() {
     if (g_sm_count == 0) {
@@ -79,6 +89,8 @@ struct Geometry {
     int tiles_per_split;  // j-tiles per CTA
     int nsplit;           // CTAs along j
     int Nj, Njpad;
+    int minb;             // register cap: CTAs per SM the kernel variant is compiled for (3..6)
+    int pipe;             // software-pipelined j loop
 };
 
 Geometry geometry(int64_t N, int64_t n_active) {
@@ -87,16 +99,19 @@ Geometry geometry(int64_t N, int64_t n_active) {
     g.tiles_total = (g.Nj + kTileJ - 1) / kTileJ;
     g.Njpad = g.tiles_total * kTileJ;
     const int sms = sm_count();
-    // I: the largest register tile (i-bodies per thread) that still leaves enough (i-block, j-tile)
-    // work items to cover every SM a few times; small N falls back to a narrower tile.
+    // I: register tile (i-bodies per thread).  I = 2 at 5 CTAs/SM (96 registers, 20 warps/SM) measured
+    // fastest on B200 (profiles/); small N falls back to I = 1 so that enough (i-block, j-tile) work
+    // items exist to cover every SM a few times.  I = 4 stays selectable (fewer shared-memory reads).
     int ipt = g_cfg.i_per_thread;
     if (ipt != 1 && ipt != 2 && ipt != 4) {
-        ipt = 4;
+        ipt = 2;
         while (ipt > 1 &&
                ((N + (int64_t)kForceThreads * ipt - 1) / ((int64_t)kForceThreads * ipt)) * g.tiles_total < (int64_t)4 * sms)
             ipt >>= 1;
     }
     g.ipt = ipt;
+    g.minb = g_cfg.ctas_per_sm >= 3 && g_cfg.ctas_per_sm <= 6 ? g_cfg.ctas_per_sm : (ipt == 4 ? 3 : 5);
+    g.pipe = g_cfg.pipeline_j > 0 ? 1 : 0;
     g.iblocks = (int)((N + (int64_t)kForceThreads * ipt - 1) / ((int64_t)kForceThreads * ipt));
     int nsplit = g_cfg.j_splits;
     if (nsplit <= 0) {
@@ -162,11 +177,27 @@ int check_workspace(int64_t N, const Geometry &g, Workspace *w) {
 
 inline int body_blocks(int64_t n) { return (int)((n + kBodyThreads - 1) / kBodyThreads); }
 
+template <int I, int MINB, bool PIPE>
+void launch_force_IMP(const ForceParams &fp, const Geometry &g, bool pairs) {
+    dim3 grid(g.iblocks, g.nsplit);
+    if (pairs) nb_force_tiles_kernel<I, true, MINB, PIPE><<<grid, kForceThreads, 0, stream()>>>(fp);
+    else nb_force_tiles_kernel<I, false, MINB, PIPE><<<grid, kForceThreads, 0, stream()>>>(fp);
+}
+
+template <int I, int MINB>
+void launch_force_IM(const ForceParams &fp, const Geometry &g, bool pairs) {
+    if (g.pipe) launch_force_IMP<I, MINB, true>(fp, g, pairs);
+    else launch_force_IMP<I, MINB, false>(fp, g, pairs);
+}
+
 template <int I>
 void launch_force_I(const ForceParams &fp, const Geometry &g, bool pairs) {
-    dim3 grid(g.iblocks, g.nsplit);
-    if (pairs) nb_force_tiles_kernel<I, true><<<grid, kForceThreads, 0, stream()>>>(fp);
-    else nb_force_tiles_kernel<I, false><<<grid, kForceThreads, 0, stream()>>>(fp);
+    switch (g.minb) {
+        case 3: launch_force_IM<I, 3>(fp, g, pairs); break;
+        case 4: launch_force_IM<I, 4>(fp, g, pairs); break;
+        case 5: launch_force_IM<I, 5>(fp, g, pairs); break;
+        default: launch_force_IM<I, 6>(fp, g, pairs); break;
+    }
 }
 
 void launch_force(const ForceParams &fp, const Geometry &g, bool pairs) {
@@ -281,22 +312,44 @@ int step_impl(double *x, double *v, const double *m, double M_star, int64_t N, d
         key.x = x; key.v = v; key.m = m; key.rcrit = rc_io; key.acc = acc; key.pairs = pairs; key.npairs = npairs;
         key.ws = g_cfg.workspace; key.stream = g_cfg.stream; key.N = N; key.n_active = g_cfg.n_active;
         key.cap = g_cfg.pair_capacity; key.dt = dt; key.M_star = M_star; key.G = g_cfg.G; key.n1 = g_cfg.n1;
-        key.n2 = g_cfg.n2; key.kind = g_cfg.changeover_kind; key.ipt = g.ipt; key.jsplit = g.nsplit;
+        key.n2 = g_cfg.n2; key.kind = g_cfg.changeover_kind; key.ipt = g.ipt * 100 + g.minb * 10 + g.pipe; key.jsplit = g.nsplit;
         key.ws_bytes = g_cfg.workspace_bytes;
-        if (!g_graph_exec || std::memcmp(&key, &g_graph_key, sizeof(key)) != 0) {
-            drop_graph();
-            cudaGraph_t graph = nullptr;
-            NB_CUDA(cudaStreamBeginCapture(stream(), cudaStreamCaptureModeRelaxed));
-            const int erc = enqueue_step(2);
-            cudaError_t ce = cudaStreamEndCapture(stream(), &graph);
-            if (erc) { if (graph) cudaGraphDestroy(graph); return erc; }
-            if (ce != cudaSuccess) return fail(NB_E_CUDA, "cudaStreamEndCapture failed: %s", cudaGetErrorString(ce));
-            ce = cudaGraphInstantiate(&g_graph_exec, graph, 0);
-            cudaGraphDestroy(graph);
-            if (ce != cudaSuccess) { g_graph_exec = nullptr; return fail(NB_E_CUDA, "cudaGraphInstantiate failed: %s", cudaGetErrorString(ce)); }
-            g_graph_key = key;
+        const bool hop = !stream_capturable();
+        if (hop) {
+            if (!g_own_stream) {
+                NB_CUDA(cudaStreamCreateWithFlags(&g_own_stream, cudaStreamNonBlocking));
+                NB_CUDA(cudaEventCreateWithFlags(&g_ev_in, cudaEventDisableTiming));
+                NB_CUDA(cudaEventCreateWithFlags(&g_ev_out, cudaEventDisableTiming));
+            }
+            NB_CUDA(cudaEventRecord(g_ev_in, stream()));
+            NB_CUDA(cudaStreamWaitEvent(g_own_stream, g_ev_in, 0));
+            g_on_own_stream = true;
         }
-        for (int64_t s = 0; s < interior; ++s) NB_CUDA(cudaGraphLaunch(g_graph_exec, stream()));
+        auto replay = [&]() -> int {
+            if (!g_graph_exec || std::memcmp(&key, &g_graph_key, sizeof(key)) != 0) {
+                drop_graph();
+                cudaGraph_t graph = nullptr;
+                NB_CUDA(cudaStreamBeginCapture(stream(), cudaStreamCaptureModeRelaxed));
+                const int erc = enqueue_step(2);
+                cudaError_t ce = cudaStreamEndCapture(stream(), &graph);
+                if (erc) { if (graph) cudaGraphDestroy(graph); return erc; }
+                if (ce != cudaSuccess) return fail(NB_E_CUDA, "cudaStreamEndCapture failed: %s", cudaGetErrorString(ce));
+                ce = cudaGraphInstantiate(&g_graph_exec, graph, 0);
+                cudaGraphDestroy(graph);
+                if (ce != cudaSuccess) { g_graph_exec = nullptr; return fail(NB_E_CUDA, "cudaGraphInstantiate failed: %s", cudaGetErrorString(ce)); }
+                g_graph_key = key;
+            }
+            for (int64_t s = 0; s < interior; ++s) NB_CUDA(cudaGraphLaunch(g_graph_exec, stream()));
+            return NB_OK;
+        };
+        rc = replay();
+        if (hop) {
+            cudaError_t ce = cudaEventRecord(g_ev_out, g_own_stream);
+            g_on_own_stream = false;
+            if (ce == cudaSuccess) ce = cudaStreamWaitEvent(stream(), g_ev_out, 0);
+            if (!rc && ce != cudaSuccess) rc = fail(NB_E_CUDA, "stream hand-back failed: %s", cudaGetErrorString(ce));
+        }
+        if (rc) return rc;
     } else {
         for (int64_t s = 0; s < interior; ++s)
             if ((rc = enqueue_step(2))) return rc;
@@ -348,6 +401,7 @@ int nb_configure(const nb_config *cfg) {
     if (cfg->i_per_thread != 0 && cfg->i_per_thread != 1 && cfg->i_per_thread != 2 && cfg->i_per_thread != 4)
         return fail(NB_E_BADARG, "i_per_thread must be 0, 1, 2 or 4");
     if (cfg->j_splits < 0) return fail(NB_E_BADARG, "j_splits must be >= 0");
+    if (cfg->ctas_per_sm != 0 && (cfg->ctas_per_sm < 3 || cfg->ctas_per_sm > 6)) return fail(NB_E_BADARG, "ctas_per_sm must be 0 or 3..6");
     g_cfg = *cfg;
     return NB_OK;
 }
@@ -574,6 +628,7 @@ void nb_release(void) {
     if (g_ev0) { cudaEventDestroy(g_ev0); cudaEventDestroy(g_ev1); g_ev0 = g_ev1 = nullptr; }
     for (int k = 0; k < 2 * g_tev_created; ++k) cudaEventDestroy(g_tev[k]);
     g_tev_created = g_tev_used = 0;
+    if (g_own_stream) { cudaStreamDestroy(g_own_stream); cudaEventDestroy(g_ev_in); cudaEventDestroy(g_ev_out); g_own_stream = nullptr; }
     g_force_timed = false;
 }
 
