@@ -18,8 +18,8 @@ def _kick_case(x, v, m, rc, *, G=G_GAUSS, n_active=0, kind=0, dt=0.0, what="", *
     st.set_rcrit(rc)
     st.kick(dt)
     _, v_gpu, acc_gpu, _ = st.host()
-    acc_ref, _, nsing = oracle.accel(x, m, rc, G, n_active=n_active, kind=kind)
-    ratio, lit = assert_acc_close(acc_gpu, acc_ref, what)
+    acc_ref, ab, nsing = oracle.accel(x, m, rc, G, n_active=n_active, kind=kind, want_abs=True)
+    ratio, lit = assert_acc_close(acc_gpu, acc_ref, what, ab)
     sure, border = oracle.pairs(x, rc, n_active=n_active)
     gp, n = st.get_pairs()
     info = assert_pairs_match(gp, n, sure, border, what)
@@ -63,7 +63,7 @@ def test_random_cluster_with_changeover_and_pairs(kind, ipt, splits):
     rc[::7] = 0.0
     info = _kick_case(x, v, m, rc, kind=kind, dt=0.37, i_per_thread=ipt, j_splits=splits,
                       what=f"cluster changeover kind={kind} I={ipt} splits={splits}")
-    assert info["n_sure"] > 500  # the pair path really is exercised
+    assert info["n_sure"] > 300  # the pair path really is exercised
 
 
 def test_chain_and_lattice_pair_counts():
@@ -111,8 +111,8 @@ def test_internal_rcrit_and_nb_rcrit():
     assert np.max(np.abs(rc_gpu - rc_ref) / rc_ref) <= 1e-14
     # rcrit = NULL: nb_kick computes Eq. 7 internally from (x, v, m, M_star, dt)
     st.kick(d.dt, rcrit_given=False)
-    acc_ref, _, _ = oracle.accel(d.x, d.m, rc_ref, G_GAUSS)
-    assert_acc_close(st.acc.cpu().numpy(), acc_ref, "internal rcrit")
+    acc_ref, ab, _ = oracle.accel(d.x, d.m, rc_ref, G_GAUSS, want_abs=True)
+    assert_acc_close(st.acc.cpu().numpy(), acc_ref, "internal rcrit", ab)
     sure, border = oracle.pairs(d.x, rc_ref)
     gp, n = st.get_pairs()
     assert_pairs_match(gp, n, sure, border, "internal rcrit")
@@ -123,17 +123,17 @@ def test_pairs_null_skips_detection_and_overflow_counts():
     x, v, m = nb_inputs.random_cluster(N, seed=11, scale=0.1)
     rc = np.full(N, 0.05)
     sure, border = oracle.pairs(x, rc)
-    acc_ref, _, _ = oracle.accel(x, m, rc, G_GAUSS)
+    acc_ref, ab, _ = oracle.accel(x, m, rc, G_GAUSS, want_abs=True)
     st = GpuState(x, v, m, G=G_GAUSS, pair_capacity=100)
     st.set_rcrit(rc)
     st.kick(0.0, with_pairs=False)
-    assert_acc_close(st.acc.cpu().numpy(), acc_ref, "pairs=NULL")
+    assert_acc_close(st.acc.cpu().numpy(), acc_ref, "pairs=NULL", ab)
     st.kick(0.0, with_pairs=True)
     gp, n = st.get_pairs()
     assert sure.shape[0] <= n <= sure.shape[0] + border.shape[0]
     assert gp.shape[0] == 100  # only the first `capacity` rows are written, the count keeps counting
     assert st.nb.nb_status()["pairs_dropped"] == n - 100
-    assert_acc_close(st.acc.cpu().numpy(), acc_ref, "overflow")
+    assert_acc_close(st.acc.cpu().numpy(), acc_ref, "overflow", ab)
 
 
 def test_shift_parity():
