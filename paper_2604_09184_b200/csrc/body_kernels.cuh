@@ -178,18 +178,26 @@ __global__ void __launch_bounds__(kBodyThreads) nb_drift_kernel(double *__restri
     }
 }
 
-// fp64 FMA-rate microbenchmark: 8 independent chains per thread, register only.
-__global__ void __launch_bounds__(256) nb_fp64_peak_kernel(double *out, long long iters, double a, double b) {
-    double c0 = threadIdx.x, c1 = c0 + 1, c2 = c0 + 2, c3 = c0 + 3, c4 = c0 + 4, c5 = c0 + 5, c6 = c0 + 6, c7 = c0 + 7;
+// fp64 FMA-rate microbenchmark: 8 independent chains per thread, register only.  The FMAs read TWO
+// distinct vector-register pairs (c = p*p + c): a DFMA reading three distinct pairs issues every 3
+// clocks instead of 2 on sm_100 (register-file read ports; profiles/r1_fp64_pipe_microbench.md), so
+// the three-operand form would understate the pipe's peak by a third.
+__global__ void __launch_bounds__(256) nb_fp64_peak_kernel(double *out, long long iters, const double *src) {
+    double c[8], p[8];
+    const double tid = threadIdx.x * 1e-9;
+#pragma unroll
+    for (int r = 0; r < 8; ++r) { c[r] = tid + r; p[r] = src[r] + tid; }
 #pragma unroll 1
     for (long long k = 0; k < iters; ++k) {
 #pragma unroll
-        for (int r = 0; r < 8; ++r) {
-            c0 = __fma_rn(c0, a, b); c1 = __fma_rn(c1, a, b); c2 = __fma_rn(c2, a, b); c3 = __fma_rn(c3, a, b);
-            c4 = __fma_rn(c4, a, b); c5 = __fma_rn(c5, a, b); c6 = __fma_rn(c6, a, b); c7 = __fma_rn(c7, a, b);
+        for (int u = 0; u < 8; ++u) {
+#pragma unroll
+            for (int r = 0; r < 8; ++r) c[r] = __fma_rn(p[r], p[r], c[r]);
         }
     }
-    const double s = ((c0 + c1) + (c2 + c3)) + ((c4 + c5) + (c6 + c7));
+    double s = 0.0;
+#pragma unroll
+    for (int r = 0; r < 8; ++r) s += c[r];
     if (s == 123.456) out[0] = s;  // keeps the chains alive; practically never true
 }
 
