@@ -50,6 +50,18 @@ extern "C" {
 #define NB_CHANGEOVER_RATIONAL 0 /* y^2 / (2y^2 - 2y + 1), y = (r - 0.1 rc) / (0.9 rc) */
 #define NB_CHANGEOVER_QUINTIC 1  /* 10y^3 - 15y^4 + 6y^5 */
 
+/* The O(N^2) sum has two kernels that compute the same accelerations and the same pair list
+ * (summation order, hence the last bits, differ):
+ *   NB_FORCE_TILES      one-sided: every ordered interaction (i,j) is evaluated for body i;
+ *                       any n_active, any N.
+ *   NB_FORCE_SYMMETRIC  Newton's third law: every unordered pair is evaluated once and its r^-3
+ *                       serves both bodies (two thirds of the fp64 instructions); fully active case
+ *                       only -- with n_active < N the call falls back to NB_FORCE_TILES.
+ *   NB_FORCE_AUTO       symmetric when fully active and N >= 12288, else tiles. */
+#define NB_FORCE_AUTO 0
+#define NB_FORCE_TILES 1
+#define NB_FORCE_SYMMETRIC 2
+
 /* Process-wide settings.  nb_default_config fills the defaults named below. */
 typedef struct nb_config {
     void *stream;            /* cudaStream_t the calls enqueue on; NULL = legacy default stream */
@@ -68,10 +80,12 @@ typedef struct nb_config {
                                 as left by the previous nb_step/nb_kick(dt=0) call on this state: skip the
                                 evaluation at t0, so a run stepped in chunks costs one evaluation per step
                                 (default 0) */
-    int ctas_per_sm;         /* tuning: register cap of the force kernel, CTAs of 128 threads per SM (3..6), 0 = auto */
+    int ctas_per_sm;         /* tuning: register cap of the force kernel, CTAs of 128 threads per SM (2..6), 0 = auto */
     int pipeline_j;          /* tuning: 1 = software-pipelined j loop in the force kernel (default 0) */
     int time_force;          /* bracket every force-tile launch with CUDA events (nb_force_time); implies
                                 no graph replay (default 0) */
+    int force_kernel;        /* NB_FORCE_AUTO (default), NB_FORCE_TILES, NB_FORCE_SYMMETRIC (see below) */
+    int sym_block;           /* tuning: super-block size S of the symmetric kernel (256, 512, 1024, 2048), 0 = auto */
 } nb_config;
 
 void nb_default_config(nb_config *cfg);
@@ -168,7 +182,8 @@ double nb_last_force_ms(void);
 int nb_force_time(int64_t *launches, double *total_ms);
 int nb_force_time_reset(void);
 /* Launch geometry the force kernel would use for (N, n_active): out[0] = i-bodies per thread,
- * out[1] = i-blocks, out[2] = j-splits, out[3] = threads per CTA, out[4] = j-tile length. */
+ * out[1] = i-blocks, out[2] = j-splits, out[3] = threads per CTA, out[4] = j-tile length
+ * (one-sided kernel) or minus the super-block size S (symmetric kernel; out[1] = out[2] = super-blocks). */
 int nb_force_geometry(int64_t N, int64_t *out5);
 
 /*

@@ -17,6 +17,7 @@ from . import build as _build
 NB_OK = 0
 NB_E_NULL, NB_E_BADN, NB_E_BADARG, NB_E_WORKSPACE, NB_E_CUDA = -1, -2, -3, -4, -5
 CHANGEOVER_RATIONAL, CHANGEOVER_QUINTIC = 0, 1
+FORCE_AUTO, FORCE_TILES, FORCE_SYMMETRIC = 0, 1, 2
 
 # every symbol include/nbkick.h declares (tests check the library exports each of them)
 SYMBOLS = (
@@ -44,6 +45,8 @@ class NbConfig(C.Structure):
         ("ctas_per_sm", C.c_int),
         ("pipeline_j", C.c_int),
         ("time_force", C.c_int),
+        ("force_kernel", C.c_int),
+        ("sym_block", C.c_int),
     ]
 
 
@@ -148,7 +151,7 @@ def default_config() -> NbConfig:
 
 def configure(N=None, *, stream=None, pair_capacity=0, n_active=0, G=None, n1=3.0, n2=0.4, changeover_kind=0,
               i_per_thread=0, j_splits=0, use_graph=True, reuse_acc=False, time_force=False, ctas_per_sm=0,
-              pipeline_j=0, device="cuda"):
+              pipeline_j=0, force_kernel=0, sym_block=0, device="cuda"):
     """nb_configure with a torch-allocated workspace sized for N bodies (N=None: no workspace,
     enough for the _host calls).  Keeps the workspace tensor alive."""
     lib = load()
@@ -164,6 +167,7 @@ def configure(N=None, *, stream=None, pair_capacity=0, n_active=0, G=None, n1=3.
     cfg.reuse_acc = 1 if reuse_acc else 0
     cfg.time_force = 1 if time_force else 0
     cfg.ctas_per_sm, cfg.pipeline_j = int(ctas_per_sm), int(pipeline_j)
+    cfg.force_kernel, cfg.sym_block = int(force_kernel), int(sym_block)
     if N is not None:
         import torch
         if stream is None:

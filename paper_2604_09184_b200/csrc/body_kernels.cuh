@@ -27,7 +27,10 @@ struct PrepParams {
     const double *v;        // [N,3]; needed when update_rc
     const double *m;        // [N]
     double *rcrit;          // [N]; written when update_rc, read otherwise
-    JRec *jrec;             // [Njpad]
+    JRec *jrec;             // [Njpad] one-sided kernel's records (nullptr: not staged)
+    double2 *sxy, *szg;     // [Npad_sym] symmetric kernel's (x,y) and (z,Gm) (nullptr: not staged)
+    int *sthr;              // [Npad_sym] hi32(rcrit^2) + 1
+    int Npad_sym;
     const double *mv_in;    // [nblk_in,3] momentum partials or nullptr
     unsigned long long *npairs;  // reset to 0 here (nullptr: skip)
     long long *status;
@@ -74,7 +77,16 @@ __global__ void __launch_bounds__(kBodyThreads) nb_prep_kernel(const PrepParams 
                 status_add(p.status, ST_NONFINITE, 1);
         }
     }
-    if (i < p.Njpad) p.jrec[i] = r;  // grid covers max(N, Njpad)
+    if (p.jrec != nullptr && i < p.Njpad) p.jrec[i] = r;  // grid covers max(N, Njpad, Npad_sym)
+    if (p.sxy != nullptr && i < p.Npad_sym) {
+        // symmetric kernel: every body is both an i- and a j-body; padding bodies get distinct far
+        // positions (pad-pad distances stay huge and finite) and zero mass
+        double sx_ = r.x, sy_ = r.y, sz_ = r.z;
+        if (i >= p.N) { sx_ = kFarJ + 1.0e27 * (double)(i - p.N + 1); sy_ = kFarJ; sz_ = kFarJ; }
+        p.sxy[i] = make_double2(sx_, sy_);
+        p.szg[i] = make_double2(sz_, r.gm);
+        p.sthr[i] = __double2hiint(r.rc2) + 1;
+    }
 }
 
 // standalone a0

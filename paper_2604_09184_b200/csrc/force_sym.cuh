@@ -1,0 +1,285 @@
+// force_sym.cuh -- Newton-III form of the O(N^2) kick for the fully active case (Eq. 5,
+// PAPER.md:98; pair list PAPER.md:94, 98, 106).  Each unordered pair {i,j} is evaluated ONCE and
+// its r^-3 serves both bodies: 20 FP64-pipe instructions per unordered pair = 10 per ordered
+// interaction, against 15 in the one-sided tile kernel (force_tiles.cuh), which stays the kernel of
+// the semi-active mode and of small N.
+//
+// Work unit: a super-tile (A, B), A <= B, of S x S bodies; one CTA of 4 warps per super-tile.
+//   * B's bodies (x, y | z, Gm | threshold word) are staged ONCE in shared memory by three TMA bulk
+//     copies; B's accelerations accumulate in shared memory (jS).
+//   * A's bodies are taken in chunks of 128*I; every lane holds I of them in registers together
+//     with their accumulators.
+//   * A warp meets a block of 32 j-bodies by ROTATION: lane l starts with j = l, evaluates its I
+//     pairs, then the three j-accumulators move one lane down (6 SHFL) while the next j's constants
+//     come from shared memory; after 32 rotations every (i, j) pair of the 32I x 32 block has been
+//     visited exactly once and the j-accumulators are back in their home lanes.  No reduction
+//     arithmetic is spent on the j side.
+//   * Warps of a CTA work on different j-units in a skewed order (unit = (step + warp) mod units)
+//     with one __syncthreads per step, so shared accumulators are never touched by two warps at a
+//     time and the summation order is fixed: results are bit-reproducible, no atomics.
+// Output: part[slot][n][3]; super-tile (A,B) writes slot B for A's bodies (i side) and slot A for
+// B's bodies (j side); every (slot, body) is written exactly once per evaluation and
+// nb_kickv_kernel adds the slots in order.
+//
+// Diagonal super-tiles (A == B): a warp's 32I-block against a 32-block q is evaluated symmetrically
+// if q lies above the block, skipped if below (the mirrored visit covers it), and "mixed" if q is one
+// of the block's own 32-blocks: all ordered pairs are evaluated, only the i side is kept.
+#pragma once
+#include "force_tiles.cuh"
+
+namespace nbk {
+
+struct SymParams {
+    const double2 *sxy;          // [Npad] (x, y)      staged by nb_prep_kernel; padding bodies sit far
+    const double2 *szg;          // [Npad] (z, G m)    away at distinct places with zero mass
+    const int *sthr;             // [Npad] hi32(rcrit^2) + 1
+    const double *rcrit;         // [N]    exact critical radii (slow path only)
+    double *part;                // [nsb, N, 3]
+    int32_t *pairs;              // [cap,2] or nullptr
+    unsigned long long *npairs;  // device counter
+    long long *status;           // device int64[ST_COUNT]
+    long long cap;
+    int N;
+    int S;      // super-block size: multiple of 128*I and of 128*U
+    int nsb;    // super-blocks = Npad / S
+    int U;      // 32-blocks per skew unit (S / (32 U) >= 4)
+    int kind;   // changeover shape
+};
+
+constexpr int kSymThreads = 128;
+__host__ __device__ constexpr size_t sym_smem_bytes(int S) { return (size_t)S * (16 + 16 + 24 + 4) + 16; }
+
+// Exact evaluation of the lane's I pairs against body j (deferred pass; entered by the lanes that
+// flagged rotation r, whose fast-path contributions were forced to exactly 0).  Returns the j-side
+// contribution in (cx,cy,cz); emit[k] says whether pair k goes on the list.
+//   mixed: only the i side is kept by the caller and a pair is emitted from its i < j visit only.
+template <int I>
+__device__ __forceinline__ void sym_exact(const SymParams &p, const double2 xy, const double2 zg, const int j,
+                                          const bool mixed, const double (&xi)[I], const double (&yi)[I],
+                                          const double (&zi)[I], const double (&ngi)[I], const int i0,
+                                          double (&ax)[I], double (&ay)[I], double (&az)[I], double &cx, double &cy,
+                                          double &cz, bool (&emit)[I]) {
+    const double rcj = j < p.N ? p.rcrit[j] : 0.0;
+#pragma unroll
+    for (int k = 0; k < I; ++k) {
+        const int i = i0 + 32 * k;
+        emit[k] = false;
+        const bool valid = (i < p.N) && (j < p.N) && (i != j);
+        if (!valid) continue;  // padding bodies have zero mass both ways; the self term is skipped
+        const double dx = __dsub_rn(xy.x, xi[k]), dy = __dsub_rn(xy.y, yi[k]), dz = __dsub_rn(zg.x, zi[k]);
+        const double r2 = __fma_rn(dz, dz, __fma_rn(dy, dy, __dmul_rn(dx, dx)));
+        const double rc = fmax(p.rcrit[i], rcj);
+        const bool inside = r2 < rc * rc;
+        if (r2 == 0.0) {
+            // rc == 0 and coincident: contributes 0; counted once per ordered interaction
+            if (!inside) status_add(p.status, ST_SINGULAR, mixed ? 1 : 2);
+        } else {
+            const double r = sqrt(r2);
+            const double W = inside ? changeover_weight(r, rc, p.kind) : 1.0;
+            if (W != 0.0) {
+                const double f = W / (r2 * r);
+                const double si = zg.y * f, sj = ngi[k] * f;
+                ax[k] = __fma_rn(si, dx, ax[k]); ay[k] = __fma_rn(si, dy, ay[k]); az[k] = __fma_rn(si, dz, az[k]);
+                cx = __fma_rn(sj, dx, cx); cy = __fma_rn(sj, dy, cy); cz = __fma_rn(sj, dz, cz);
+            }
+        }
+        emit[k] = inside && (!mixed || i < j);
+    }
+}
+
+// One warp, one block of 32 j-bodies (shared-memory arrays qxy/qzg/qthr of the block), 32 rotations.
+// On return (bx,by,bz) of lane l hold the sums for j = jbase + l.
+//
+// The rotation loop is branch-free so that consecutive rotations overlap in the FP64 pipe: a lane
+// whose smallest r^2 is within reach of a critical radius (integer test on the high words; always
+// true for the self term, r^2 = 0) replaces its rsqrt seeds by 0 -- u = 0, e = 1, r^-3 = 0: its I pairs
+// contribute exactly 0 to both sides -- and sets bit r of a mask.  After the 32 rotations the
+// (rare) flagged rotations are evaluated exactly, and their j-side contributions are handed to the
+// home lanes of the j-bodies.
+template <int I, bool PAIRS>
+__device__ __forceinline__ void sym_block(const SymParams &p, const double2 *__restrict__ qxy,
+                                          const double2 *__restrict__ qzg, const int *__restrict__ qthr,
+                                          const int jbase, const bool mixed, const double (&xi)[I],
+                                          const double (&yi)[I], const double (&zi)[I], const double (&ngi)[I],
+                                          const int thr_lane, const int i0, double (&ax)[I], double (&ay)[I],
+                                          double (&az)[I], double &bx, double &by, double &bz) {
+    const int lane = threadIdx.x & 31;
+    const int down = (lane + 1) & 31;  // the lane whose j-sums this lane takes over after each rotation
+    bx = 0.0; by = 0.0; bz = 0.0;
+    unsigned bits = 0u;
+#pragma unroll 4
+    for (int r = 0; r < 32; ++r) {
+        const int src = (lane + r) & 31;
+        const double2 xy = qxy[src];
+        const double2 zg = qzg[src];
+        const int thrj = qthr[src];
+        double dx[I], dy[I], dz[I], r2[I];
+        int mn = 0x7fffffff;
+#pragma unroll
+        for (int k = 0; k < I; ++k) {
+            dx[k] = __dsub_rn(xy.x, xi[k]);
+            dy[k] = __dsub_rn(xy.y, yi[k]);
+            dz[k] = __dsub_rn(zg.x, zi[k]);
+            r2[k] = __fma_rn(dz[k], dz[k], __fma_rn(dy[k], dy[k], __dmul_rn(dx[k], dx[k])));
+            mn = min(mn, __double2hiint(r2[k]));
+        }
+        const bool hit = mn <= max(thr_lane, thrj);
+        if (hit) bits |= 1u << r;
+#pragma unroll
+        for (int k = 0; k < I; ++k) {
+            const int yh = hit ? 0 : __double2hiint(rsqrt_seed(r2[k]));
+            const double y0 = __hiloint2double(yh, 0);
+            const double u = __dmul_rn(y0, y0);                          // exact (y0 has 21 bits)
+            const double e = __fma_rn(-r2[k], u, 1.0);                   // 1 - r2 y0^2
+            const double q = __fma_rn(e, __fma_rn(e, 1.875, 1.5), 1.0);  // (1-e)^(-3/2), next term < 2^-56
+            const double b = __dmul_rn(__dmul_rn(u, y0), q);             // r^-3
+            const double si = __dmul_rn(b, zg.y);                        // G m_j / r^3
+            const double sj = __dmul_rn(b, ngi[k]);                      // -G m_i / r^3
+            ax[k] = __fma_rn(si, dx[k], ax[k]);
+            bx = __fma_rn(sj, dx[k], bx);
+            by = __fma_rn(sj, dy[k], by);
+            ay[k] = __fma_rn(si, dy[k], ay[k]);
+            az[k] = __fma_rn(si, dz[k], az[k]);
+            bz = __fma_rn(sj, dz[k], bz);
+        }
+        bx = __shfl_sync(0xffffffffu, bx, down);
+        by = __shfl_sync(0xffffffffu, by, down);
+        bz = __shfl_sync(0xffffffffu, bz, down);
+    }
+    unsigned any = __reduce_or_sync(0xffffffffu, bits);
+    while (any) {
+        const int r = __ffs(any) - 1;
+        any &= any - 1u;
+        const int src = (lane + r) & 31;
+        double cx = 0.0, cy = 0.0, cz = 0.0;
+        bool emit[I];
+#pragma unroll
+        for (int k = 0; k < I; ++k) emit[k] = false;
+        if ((bits >> r) & 1u)
+            sym_exact<I>(p, qxy[src], qzg[src], jbase + src, mixed, xi, yi, zi, ngi, i0, ax, ay, az, cx, cy, cz, emit);
+        if (PAIRS) {
+#pragma unroll
+            for (int k = 0; k < I; ++k) pair_append(p.pairs, p.npairs, p.status, p.cap, emit[k], i0 + 32 * k, jbase + src);
+        }
+        // body j = jbase + h met lane (h - r) & 31 in rotation r; its sums live in lane h
+        const int from = (lane - r) & 31;
+        bx += __shfl_sync(0xffffffffu, cx, from);
+        by += __shfl_sync(0xffffffffu, cy, from);
+        bz += __shfl_sync(0xffffffffu, cz, from);
+    }
+}
+
+
+template <int I, bool PAIRS, int MINB>
+__global__ void __launch_bounds__(kSymThreads, MINB) nb_force_sym_kernel(const SymParams p) {
+    extern __shared__ __align__(16) unsigned char sym_smem[];
+    const int S = p.S;
+    double2 *bxy = reinterpret_cast<double2 *>(sym_smem);
+    double2 *bzg = bxy + S;
+    double *jsx = reinterpret_cast<double *>(bzg + S);
+    double *jsy = jsx + S;
+    double *jsz = jsy + S;
+    int *bthr = reinterpret_cast<int *>(jsz + S);
+    uint64_t *bar = reinterpret_cast<uint64_t *>(bthr + S);  // S*60 bytes in: 8-byte aligned (S % 128 == 0)
+
+    const int t = threadIdx.x, lane = t & 31, w = t >> 5;
+
+    // super-tile of this CTA: strict pairs A < B first (all of equal cost), diagonal tiles (about half
+    // the work each) last, where they fill the tail wave
+    const int T = p.nsb;
+    const long long nstrict = (long long)T * (T - 1) / 2;
+    const long long idx = blockIdx.x;
+    int A, B;
+    if (idx < nstrict) {
+        B = (int)((1.0 + sqrt(1.0 + 8.0 * (double)idx)) * 0.5);
+        while ((long long)B * (B - 1) / 2 > idx) --B;
+        while ((long long)(B + 1) * B / 2 <= idx) ++B;
+        A = (int)(idx - (long long)B * (B - 1) / 2);
+    } else {
+        A = B = (int)(idx - nstrict);
+    }
+    const bool diag = (A == B);
+
+    if (t == 0) {
+        mbar_init(bar, 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+        const unsigned b16 = (unsigned)S * 16u, b4 = (unsigned)S * 4u;
+        mbar_expect_tx(bar, 2u * b16 + b4);
+        tma_bulk_g2s(bxy, p.sxy + (size_t)B * S, b16, bar);
+        tma_bulk_g2s(bzg, p.szg + (size_t)B * S, b16, bar);
+        tma_bulk_g2s(bthr, p.sthr + (size_t)B * S, b4, bar);
+    }
+    for (int n = t; n < S; n += kSymThreads) { jsx[n] = 0.0; jsy[n] = 0.0; jsz[n] = 0.0; }
+    __syncthreads();  // barrier initialised and accumulators zeroed before anyone proceeds
+    mbar_wait(bar, 0);
+
+    const int nunits = S / (32 * p.U);
+    const int nchunks = S / (kSymThreads * I);
+    for (int c = 0; c < nchunks; ++c) {
+        const int P = (c * 4 + w) * I;                  // first 32-block of this warp's i-block within A
+        const int i0 = A * S + P * 32 + lane;           // global index of the lane's first i-body
+        double xi[I], yi[I], zi[I], ngi[I], ax[I], ay[I], az[I];
+        int thr_lane = 0;
+#pragma unroll
+        for (int k = 0; k < I; ++k) {
+            const double2 a = p.sxy[i0 + 32 * k];
+            const double2 b = p.szg[i0 + 32 * k];
+            xi[k] = a.x; yi[k] = a.y; zi[k] = b.x; ngi[k] = -b.y;
+            thr_lane = max(thr_lane, p.sthr[i0 + 32 * k]);
+            ax[k] = 0.0; ay[k] = 0.0; az[k] = 0.0;
+        }
+        for (int step = 0; step < nunits; ++step) {
+            int unit = step + w;
+            if (unit >= nunits) unit -= nunits;
+            for (int uu = 0; uu < p.U; ++uu) {
+                const int q = unit * p.U + uu;  // 32-block of B
+                bool mixed = false;
+                if (diag) {
+                    if (q < P) continue;          // the mirrored visit covers it
+                    mixed = q < P + I;
+                }
+                double bx, by, bz;
+                sym_block<I, PAIRS>(p, bxy + q * 32, bzg + q * 32, bthr + q * 32, B * S + q * 32, mixed, xi, yi, zi,
+                                    ngi, thr_lane, i0, ax, ay, az, bx, by, bz);
+                if (!mixed) {
+                    const int n = q * 32 + lane;
+                    jsx[n] += bx; jsy[n] += by; jsz[n] += bz;
+                }
+            }
+            __syncthreads();
+        }
+        if (diag) {
+            // A's bodies are B's bodies: both sides of the diagonal tile go to the same slot
+#pragma unroll
+            for (int k = 0; k < I; ++k) {
+                const int n = P * 32 + 32 * k + lane;
+                jsx[n] += ax[k]; jsy[n] += ay[k]; jsz[n] += az[k];
+            }
+            __syncthreads();
+        } else {
+            double *out = p.part + (size_t)B * p.N * 3;
+#pragma unroll
+            for (int k = 0; k < I; ++k) {
+                const int i = i0 + 32 * k;
+                if (i < p.N) {
+                    out[3 * (size_t)i] = ax[k];
+                    out[3 * (size_t)i + 1] = ay[k];
+                    out[3 * (size_t)i + 2] = az[k];
+                }
+            }
+        }
+    }
+    // j side (and, on the diagonal, both sides) -> slot A for B's bodies
+    double *out = p.part + (size_t)A * p.N * 3;
+    for (int n = t; n < S; n += kSymThreads) {
+        const long long g = (long long)B * S + n;
+        if (g < p.N) {
+            out[3 * g] = jsx[n];
+            out[3 * g + 1] = jsy[n];
+            out[3 * g + 2] = jsz[n];
+        }
+    }
+}
+
+}  // namespace nbk

@@ -91,6 +91,35 @@ __device__ __forceinline__ double changeover_weight(double r, double rc, int kin
     return (y * y) / (2.0 * y * y - 2.0 * y + 1.0);
 }
 
+// Warp-aggregated append of encounter pairs (a3): one atomicAdd per warp-hit reserves the slots,
+// lanes take them in lane order; overflow keeps counting, drops the writes and is reported.
+// Must be called by all 32 lanes.
+__device__ __forceinline__ void pair_append(int32_t *pairs, unsigned long long *npairs, long long *status,
+                                            const long long cap, const bool emit, const int i, const int j) {
+    const unsigned lane = threadIdx.x & 31u;
+    const unsigned mask = __ballot_sync(0xffffffffu, emit);
+    if (mask) {
+        const int leader = __ffs(mask) - 1;
+        const int cnt = __popc(mask);
+        unsigned long long base = 0;
+        if ((int)lane == leader) {
+            base = atomicAdd(npairs, (unsigned long long)cnt);
+            const long long end = (long long)base + cnt;
+            const long long kept_end = end < cap ? end : cap;
+            const long long kept = kept_end > (long long)base ? kept_end - (long long)base : 0;
+            if (kept < cnt) status_add(status, ST_PAIR_DROPPED, cnt - kept);
+        }
+        base = __shfl_sync(0xffffffffu, base, leader);
+        if (emit) {
+            const long long pos = (long long)base + __popc(mask & ((1u << lane) - 1u));
+            if (pos < cap) {
+                const int lo = i < j ? i : j, hi = i < j ? j : i;
+                reinterpret_cast<int2 *>(pairs)[pos] = make_int2(lo, hi);
+            }
+        }
+    }
+}
+
 // Exact path for one j against this thread's I bodies: self term, strict r2 < rc_ij^2 pair test,
 // changeover weight, IEEE sqrt/divide, warp-aggregated pair append.  Entered warp-uniformly.
 template <int I, bool PAIRS>
@@ -98,7 +127,6 @@ __device__ __forceinline__ void slow_path(const ForceParams &p, const double4 A,
                                           const double (&xi)[I], const double (&yi)[I], const double (&zi)[I],
                                           const double (&rci)[I], const int i0, double (&ax)[I], double (&ay)[I],
                                           double (&az)[I]) {
-    const unsigned lane = threadIdx.x & 31u;
 #pragma unroll
     for (int k = 0; k < I; ++k) {
         const int i = i0 + k * kForceThreads;
@@ -124,28 +152,7 @@ __device__ __forceinline__ void slow_path(const ForceParams &p, const double4 A,
         }
         if (PAIRS) {
             // each unordered pair once: (i<j) among active bodies; passive i (>= Nj) sees j once only
-            const bool emit = inside && (i < j || i >= p.Nj);
-            const unsigned mask = __ballot_sync(0xffffffffu, emit);
-            if (mask) {
-                const int leader = __ffs(mask) - 1;
-                const int cnt = __popc(mask);
-                unsigned long long base = 0;
-                if ((int)lane == leader) {
-                    base = atomicAdd(p.npairs, (unsigned long long)cnt);
-                    const long long end = (long long)base + cnt;
-                    const long long kept_end = end < p.cap ? end : p.cap;
-                    const long long kept = kept_end > (long long)base ? kept_end - (long long)base : 0;
-                    if (kept < cnt) status_add(p.status, ST_PAIR_DROPPED, cnt - kept);
-                }
-                base = __shfl_sync(0xffffffffu, base, leader);
-                if (emit) {
-                    const long long pos = (long long)base + __popc(mask & ((1u << lane) - 1u));
-                    if (pos < p.cap) {
-                        const int lo = i < j ? i : j, hi = i < j ? j : i;
-                        reinterpret_cast<int2 *>(p.pairs)[pos] = make_int2(lo, hi);
-                    }
-                }
-            }
+            pair_append(p.pairs, p.npairs, p.status, p.cap, inside && (i < j || i >= p.Nj), i, j);
         }
     }
 }

@@ -11,6 +11,7 @@
 #include <mutex>
 
 #include "body_kernels.cuh"
+#include "force_sym.cuh"
 #include "force_tiles.cuh"
 
 namespace {
@@ -18,7 +19,7 @@ namespace {
 using namespace nbk;
 
 std::mutex g_mu;
-nb_config g_cfg = {nullptr, nullptr, 0, 0, 0, 0.01720209895 * 0.01720209895, 3.0, 0.4, 0, 0, 0, 1, 0, 0, 0, 0};
+nb_config g_cfg = {nullptr, nullptr, 0, 0, 0, 0.01720209895 * 0.01720209895, 3.0, 0.4, 0, 0, 0, 1, 0, 0, 0, 0, 0, 0};
 char g_err[512] = "";
 int g_sm_count = 0;
 cudaEvent_t g_ev0 = nullptr, g_ev1 = nullptr;
@@ -91,6 +92,8 @@ struct Geometry {
     int Nj, Njpad;
     int minb;             // register cap: CTAs per SM the kernel variant is compiled for (3..6)
     int pipe;             // software-pipelined j loop
+    int sym;              // 1: Newton-III super-tile kernel (force_sym.cuh); nsplit = number of super-blocks
+    int S, U, Npad_sym;   // super-block size, 32-blocks per skew unit, N padded to a multiple of S
 };
 
 Geometry geometry(int64_t N, int64_t n_active) {
@@ -99,6 +102,33 @@ Geometry geometry(int64_t N, int64_t n_active) {
     g.tiles_total = (g.Nj + kTileJ - 1) / kTileJ;
     g.Njpad = g.tiles_total * kTileJ;
     const int sms = sm_count();
+    g.sym = 0; g.S = 0; g.U = 0; g.Npad_sym = 0;
+    // Newton-III kernel: fully active case only (a passive body exerts nothing, so there is no second
+    // side to serve), and only when there are enough super-tiles to fill the machine several times.
+    const bool fully_active = (g.Nj == N);
+    if (fully_active && g_cfg.force_kernel != NB_FORCE_TILES && (g_cfg.force_kernel == NB_FORCE_SYMMETRIC || N >= 12288)) {
+        // I = 4 at 3 CTAs/SM (168 registers, no spills) measured fastest on B200 (profiles/); smaller
+        // problems take I = 2 so that S = 256 super-blocks (more CTAs) stay possible.
+        int ipt = g_cfg.i_per_thread;
+        if (ipt != 1 && ipt != 2 && ipt != 4) ipt = N >= 32768 ? 4 : 2;
+        int minb = g_cfg.ctas_per_sm >= 2 && g_cfg.ctas_per_sm <= 6 ? g_cfg.ctas_per_sm : (ipt == 4 ? 3 : 4);
+        int S = g_cfg.sym_block;
+        if (S != 256 && S != 512 && S != 1024 && S != 2048) {
+            // largest super-block (fewest partial slots, least staging) that still gives >= 8 waves
+            S = 1024;
+            while (S > 256 && S > 128 * ipt) {
+                const int64_t T = (N + S - 1) / S;
+                if (T * (T + 1) / 2 >= (int64_t)8 * minb * sms) break;
+                S >>= 1;
+            }
+        }
+        if (S < 128 * ipt) S = 128 * ipt;
+        g.sym = 1; g.S = S; g.U = S / 128; g.ipt = ipt; g.minb = minb; g.pipe = 0;
+        g.Npad_sym = (int)(((N + S - 1) / S) * S);
+        g.nsplit = g.Npad_sym / S;
+        g.iblocks = g.nsplit; g.tiles_per_split = 0;
+        return g;
+    }
     // I: register tile (i-bodies per thread).  I = 2 at 5 CTAs/SM (96 registers, 20 warps/SM) measured
     // fastest on B200 (profiles/); small N falls back to I = 1 so that enough (i-block, j-tile) work
     // items exist to cover every SM a few times.  I = 4 stays selectable (fewer shared-memory reads).
@@ -150,7 +180,9 @@ struct Workspace {
     unsigned long long *npairs_dummy;
     double *mvA, *mvB;  // momentum partials [nblk,3]
     double *rc_scratch; // [N]
-    JRec *jrec;         // [Njpad]
+    JRec *jrec;         // [Njpad]                 (one-sided kernel)
+    double2 *sxy, *szg; // [Npad_sym]              (symmetric kernel)
+    int *sthr;          // [Npad_sym]
     double *part;       // [nsplit, N, 3]
     size_t bytes;
 };
@@ -165,7 +197,10 @@ Workspace carve(void *base, int64_t N, const Geometry &g) {
     w.mvA = reinterpret_cast<double *>(b + off); off += align_up(nblk * 3 * sizeof(double), 256);
     w.mvB = reinterpret_cast<double *>(b + off); off += align_up(nblk * 3 * sizeof(double), 256);
     w.rc_scratch = reinterpret_cast<double *>(b + off); off += align_up((size_t)N * sizeof(double), 256);
-    w.jrec = reinterpret_cast<JRec *>(b + off); off += align_up((size_t)g.Njpad * sizeof(JRec), 256);
+    w.jrec = reinterpret_cast<JRec *>(b + off); off += align_up((size_t)(g.sym ? 0 : g.Njpad) * sizeof(JRec), 256);
+    w.sxy = reinterpret_cast<double2 *>(b + off); off += align_up((size_t)g.Npad_sym * sizeof(double2), 256);
+    w.szg = reinterpret_cast<double2 *>(b + off); off += align_up((size_t)g.Npad_sym * sizeof(double2), 256);
+    w.sthr = reinterpret_cast<int *>(b + off); off += align_up((size_t)g.Npad_sym * sizeof(int), 256);
     w.part = reinterpret_cast<double *>(b + off); off += align_up((size_t)g.nsplit * (size_t)N * 3 * sizeof(double), 256);
     w.bytes = off;
     return w;
@@ -219,6 +254,36 @@ void launch_force(const ForceParams &fp, const Geometry &g, bool pairs) {
     else launch_force_I<1>(fp, g, pairs);
 }
 
+template <int I, int MINB>
+int launch_sym_IM(const SymParams &sp, const Geometry &g, bool pairs) {
+    const size_t smem = sym_smem_bytes(g.S);
+    const long long T = g.nsplit;
+    const unsigned ctas = (unsigned)(T * (T + 1) / 2);
+    auto go = [&](auto kern) -> int {
+        NB_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        kern<<<ctas, kSymThreads, smem, stream()>>>(sp);
+        return NB_OK;
+    };
+    return pairs ? go(nb_force_sym_kernel<I, true, MINB>) : go(nb_force_sym_kernel<I, false, MINB>);
+}
+
+template <int I>
+int launch_sym_I(const SymParams &sp, const Geometry &g, bool pairs) {
+    switch (g.minb) {
+        case 2: return launch_sym_IM<I, 2>(sp, g, pairs);
+        case 3: return launch_sym_IM<I, 3>(sp, g, pairs);
+        case 4: return launch_sym_IM<I, 4>(sp, g, pairs);
+        case 5: return launch_sym_IM<I, 5>(sp, g, pairs);
+        default: return launch_sym_IM<I, 6>(sp, g, pairs);
+    }
+}
+
+int launch_sym(const SymParams &sp, const Geometry &g, bool pairs) {
+    if (g.ipt == 4) return launch_sym_I<4>(sp, g, pairs);
+    if (g.ipt == 2) return launch_sym_I<2>(sp, g, pairs);
+    return launch_sym_I<1>(sp, g, pairs);
+}
+
 // One force evaluation: [second half-shift] + rcrit + staging, tiles, reduce + kick.
 //   mv_in  : momentum partials for the half-shift folded into prep (nullptr: none)
 //   rc_io  : rcrit array read (update_rc = 0) or written (update_rc = 1)
@@ -229,12 +294,14 @@ int enqueue_eval(const Workspace &w, const Geometry &g, double *x, double *v, co
                  int32_t *pairs, int64_t *npairs, double hk, int nhalf, double *mv_out, bool time_force) {
     const int nblk = body_blocks(N);
     PrepParams pp;
-    pp.x = x; pp.v = v; pp.m = m; pp.rcrit = rc_io; pp.jrec = w.jrec; pp.mv_in = mv_in;
+    pp.x = x; pp.v = v; pp.m = m; pp.rcrit = rc_io; pp.jrec = g.sym ? nullptr : w.jrec; pp.mv_in = mv_in;
+    pp.sxy = g.sym ? w.sxy : nullptr; pp.szg = w.szg; pp.sthr = w.sthr; pp.Npad_sym = g.Npad_sym;
     pp.npairs = pairs ? reinterpret_cast<unsigned long long *>(npairs) : nullptr;
     pp.status = w.status; pp.dtc = dtc; pp.M_star = M_star; pp.G = g_cfg.G; pp.n1 = g_cfg.n1; pp.n2 = g_cfg.n2;
     pp.absdt = std::fabs(dt_for_rc); pp.nblk_in = nblk; pp.N = (int)N; pp.Nj = g.Nj; pp.Njpad = g.Njpad;
     pp.update_rc = update_rc;
-    const int64_t cover = N > g.Njpad ? N : g.Njpad;
+    int64_t cover = N > g.Njpad ? N : g.Njpad;
+    if (g.Npad_sym > cover) cover = g.Npad_sym;
     nb_prep_kernel<<<body_blocks(cover), kBodyThreads, 0, stream()>>>(pp);
 
     ForceParams fp;
@@ -254,7 +321,16 @@ int enqueue_eval(const Workspace &w, const Geometry &g, double *x, double *v, co
         if (!g_ev0) { NB_CUDA(cudaEventCreate(&g_ev0)); NB_CUDA(cudaEventCreate(&g_ev1)); }
         NB_CUDA(cudaEventRecord(g_ev0, stream()));
     }
-    launch_force(fp, g, pairs != nullptr);
+    if (g.sym) {
+        SymParams sp;
+        sp.sxy = w.sxy; sp.szg = w.szg; sp.sthr = w.sthr; sp.rcrit = rc_io; sp.part = w.part; sp.pairs = pairs;
+        sp.npairs = fp.npairs; sp.status = w.status; sp.cap = fp.cap; sp.N = (int)N; sp.S = g.S; sp.nsb = g.nsplit;
+        sp.U = g.U; sp.kind = g_cfg.changeover_kind;
+        const int lrc = launch_sym(sp, g, pairs != nullptr);
+        if (lrc) return lrc;
+    } else {
+        launch_force(fp, g, pairs != nullptr);
+    }
     if (pool) { NB_CUDA(cudaEventRecord(g_tev[2 * g_tev_used + 1], stream())); ++g_tev_used; }
     else if (time_force) { NB_CUDA(cudaEventRecord(g_ev1, stream())); g_force_timed = true; }
 
@@ -325,7 +401,7 @@ int step_impl(double *x, double *v, const double *m, double M_star, int64_t N, d
         key.x = x; key.v = v; key.m = m; key.rcrit = rc_io; key.acc = acc; key.pairs = pairs; key.npairs = npairs;
         key.ws = g_cfg.workspace; key.stream = g_cfg.stream; key.N = N; key.n_active = g_cfg.n_active;
         key.cap = g_cfg.pair_capacity; key.dt = dt; key.M_star = M_star; key.G = g_cfg.G; key.n1 = g_cfg.n1;
-        key.n2 = g_cfg.n2; key.kind = g_cfg.changeover_kind; key.ipt = g.ipt * 100 + g.minb * 10 + g.pipe; key.jsplit = g.nsplit;
+        key.n2 = g_cfg.n2; key.kind = g_cfg.changeover_kind; key.ipt = g.S * 1000 + g.ipt * 100 + g.minb * 10 + g.pipe; key.jsplit = g.nsplit;
         key.ws_bytes = g_cfg.workspace_bytes;
         const bool hop = !stream_capturable();
         if (hop) {
@@ -400,6 +476,8 @@ void nb_default_config(nb_config *cfg) {
     cfg->use_graph = 1;
     cfg->reuse_acc = 0;
     cfg->time_force = 0;
+    cfg->force_kernel = NB_FORCE_AUTO;
+    cfg->sym_block = 0;
 }
 
 int nb_configure(const nb_config *cfg) {
@@ -414,7 +492,11 @@ int nb_configure(const nb_config *cfg) {
     if (cfg->i_per_thread != 0 && cfg->i_per_thread != 1 && cfg->i_per_thread != 2 && cfg->i_per_thread != 4)
         return fail(NB_E_BADARG, "i_per_thread must be 0, 1, 2 or 4");
     if (cfg->j_splits < 0) return fail(NB_E_BADARG, "j_splits must be >= 0");
-    if (cfg->ctas_per_sm != 0 && (cfg->ctas_per_sm < 3 || cfg->ctas_per_sm > 6)) return fail(NB_E_BADARG, "ctas_per_sm must be 0 or 3..6");
+    if (cfg->ctas_per_sm != 0 && (cfg->ctas_per_sm < 2 || cfg->ctas_per_sm > 6)) return fail(NB_E_BADARG, "ctas_per_sm must be 0 or 2..6");
+    if (cfg->force_kernel != NB_FORCE_AUTO && cfg->force_kernel != NB_FORCE_TILES && cfg->force_kernel != NB_FORCE_SYMMETRIC)
+        return fail(NB_E_BADARG, "unknown force_kernel %d", cfg->force_kernel);
+    if (cfg->sym_block != 0 && cfg->sym_block != 256 && cfg->sym_block != 512 && cfg->sym_block != 1024 && cfg->sym_block != 2048)
+        return fail(NB_E_BADARG, "sym_block must be 0, 256, 512, 1024 or 2048");
     g_cfg = *cfg;
     return NB_OK;
 }
@@ -431,7 +513,7 @@ int nb_force_geometry(int64_t N, int64_t *out5) {
     if (!out5) return fail(NB_E_NULL, "out5 is NULL");
     if (N <= 0 || N > 2147483647LL) return fail(NB_E_BADN, "N out of range");
     const Geometry g = geometry(N, g_cfg.n_active <= N ? g_cfg.n_active : 0);
-    out5[0] = g.ipt; out5[1] = g.iblocks; out5[2] = g.nsplit; out5[3] = kForceThreads; out5[4] = kTileJ;
+    out5[0] = g.ipt; out5[1] = g.iblocks; out5[2] = g.nsplit; out5[3] = kForceThreads; out5[4] = g.sym ? -g.S : kTileJ;
     return NB_OK;
 }
 

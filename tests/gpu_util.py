@@ -85,7 +85,7 @@ class GpuState:
     """Device copies of one workload + output buffers, configured library."""
 
     def __init__(self, x, v, m, M_star=1.0, *, G, n_active=0, n1=3.0, n2=0.0, kind=0, pair_capacity=1 << 20,
-                 i_per_thread=0, j_splits=0, use_graph=True):
+                 i_per_thread=0, j_splits=0, use_graph=True, **tune):
         import paper_2604_09184_b200 as nb
         torch = torch_mod()
         self.nb = nb
@@ -98,7 +98,7 @@ class GpuState:
         self.pairs = torch.full((max(self.cap, 1), 2), -1, dtype=torch.int32, device="cuda")
         self.npairs = torch.zeros(1, dtype=torch.int64, device="cuda")
         nb.configure(self.N, pair_capacity=self.cap, n_active=n_active, G=G, n1=n1, n2=n2, changeover_kind=kind,
-                     i_per_thread=i_per_thread, j_splits=j_splits, use_graph=use_graph)
+                     i_per_thread=i_per_thread, j_splits=j_splits, use_graph=use_graph, **tune)
         nb.nb_status_reset()
 
     def set_rcrit(self, rc):

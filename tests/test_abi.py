@@ -93,19 +93,41 @@ def test_geometry_and_workspace(nb):
         c.n_active = n_active
         assert lib.nb_configure(C.byref(c)) == 0
         g = nb.force_geometry(N)
-        assert g.threads == 128 and g.tile_j == 128 and g.i_per_thread in (1, 2, 4)
-        assert g.i_blocks * g.threads * g.i_per_thread >= N > (g.i_blocks - 1) * g.threads * g.i_per_thread
+        assert g.threads == 128 and g.i_per_thread in (1, 2, 4)
         nj = n_active or N
-        tiles = -(-nj // g.tile_j)
-        per = -(-tiles // g.j_splits)
-        assert (g.j_splits - 1) * per < tiles <= g.j_splits * per
-        assert g.i_blocks * g.j_splits >= 148
         ws = nb.workspace_bytes(N)
-        assert ws >= 64 * nj + 24 * N * g.j_splits
+        if g.tile_j < 0:
+            # Newton-III kernel: fully active and large enough; super-blocks of S bodies cover N, one CTA
+            # per unordered pair of super-blocks, one partial slot per super-block
+            S = -g.tile_j
+            assert not n_active and N >= 12288
+            assert S in (256, 512, 1024, 2048) and S % (128 * g.i_per_thread) == 0
+            assert g.i_blocks == g.j_splits == -(-N // S)
+            assert g.i_blocks * (g.i_blocks + 1) // 2 >= 8 * 148 or S == max(256, 128 * g.i_per_thread)
+            assert ws >= 36 * N + 24 * N * g.j_splits
+        else:
+            assert g.tile_j == 128
+            assert g.i_blocks * g.threads * g.i_per_thread >= N > (g.i_blocks - 1) * g.threads * g.i_per_thread
+            tiles = -(-nj // g.tile_j)
+            per = -(-tiles // g.j_splits)
+            assert (g.j_splits - 1) * per < tiles <= g.j_splits * per
+            assert g.i_blocks * g.j_splits >= 148
+            assert ws >= 64 * nj + 24 * N * g.j_splits
         if not n_active:
             assert ws > prev
             prev = ws
     assert nb.workspace_bytes(0) == 0
+    # the kernel choice can be forced either way; semi-active requests fall back to the one-sided kernel
+    c = nb.default_config()
+    c.force_kernel = 1
+    assert lib.nb_configure(C.byref(c)) == 0 and nb.force_geometry(65536).tile_j == 128
+    c.force_kernel, c.sym_block, c.i_per_thread = 2, 256, 1
+    assert lib.nb_configure(C.byref(c)) == 0 and nb.force_geometry(700).tile_j == -256
+    c.n_active = 100
+    assert lib.nb_configure(C.byref(c)) == 0 and nb.force_geometry(700).tile_j == 128
+    c = nb.default_config()
+    c.sym_block = 300
+    assert lib.nb_configure(C.byref(c)) == nb.binding.NB_E_BADARG
     assert lib.nb_configure(C.byref(nb.default_config())) == 0
 
 

@@ -1,0 +1,134 @@
+"""-m gpu parity of the Newton-III force kernel (force_sym.cuh; nb_config.force_kernel =
+NB_FORCE_SYMMETRIC) against the CPU oracle: same bar as the one-sided kernel (test_gpu_kick.py) --
+accelerations within the north_star tolerance, pair lists bit-exact after the canonical sort.
+Sizes straddle the super-block size S, the 128*I chunk and the 32-body rotation block; the
+diagonal ("mixed") blocks, the padding bodies and the deferred exact pass are all exercised."""
+import numpy as np
+import pytest
+
+import nb_inputs
+import oracle
+from nb_inputs import G_GAUSS
+
+from gpu_util import GpuState, assert_acc_close, assert_pairs_match
+from test_gpu_kick import _kick_case
+
+pytestmark = pytest.mark.gpu
+
+SYM = 2  # NB_FORCE_SYMMETRIC
+
+
+def _geometry_is_symmetric(N):
+    import paper_2604_09184_b200 as nb
+    return nb.force_geometry(N).tile_j < 0
+
+
+@pytest.mark.parametrize("ipt,S", [(1, 256), (2, 256), (2, 512), (4, 512), (4, 1024)])
+@pytest.mark.parametrize("N", [1, 2, 31, 32, 33, 255, 256, 257, 700, 1100])
+def test_sym_random_cluster_newtonian(N, ipt, S):
+    x, v, m = nb_inputs.random_cluster(N, seed=100 + N)
+    info = _kick_case(x, v, m, np.zeros(N), force_kernel=SYM, i_per_thread=ipt, sym_block=S,
+                      what=f"sym cluster N={N} I={ipt} S={S}")
+    assert _geometry_is_symmetric(N)
+    assert info["n_gpu"] == 0
+
+
+@pytest.mark.parametrize("kind", [0, 1])
+@pytest.mark.parametrize("ipt,S", [(1, 256), (2, 256), (4, 512)])
+def test_sym_cluster_with_changeover_and_pairs(kind, ipt, S):
+    N = 1000
+    x, v, m = nb_inputs.random_cluster(N, seed=5, scale=0.2)
+    rng = np.random.default_rng(9)
+    rc = rng.uniform(0.0, 0.06, N)
+    rc[::7] = 0.0
+    info = _kick_case(x, v, m, rc, kind=kind, dt=0.37, force_kernel=SYM, i_per_thread=ipt, sym_block=S,
+                      what=f"sym changeover kind={kind} I={ipt} S={S}")
+    assert info["n_sure"] > 300
+
+
+@pytest.mark.parametrize("ipt,S", [(2, 256), (4, 512)])
+def test_sym_chain_lattice_and_all_pairs(ipt, S):
+    tune = dict(force_kernel=SYM, i_per_thread=ipt, sym_block=S)
+    N = 300
+    x, v, m = nb_inputs.chain_1d(N)
+    for rcv, expect in ((1.5, N - 1), (2.5, 2 * N - 3)):
+        info = _kick_case(x, v, m, np.full(N, rcv), G=1.0, what=f"sym chain rc={rcv}", **tune)
+        assert info["n_gpu"] == expect
+    n = 7
+    x, v, m = nb_inputs.cubic_lattice(n)
+    info = _kick_case(x, v, m, np.full(n ** 3, 1.2), G=1.0, what="sym lattice", **tune)
+    assert info["n_gpu"] == 3 * n * n * (n - 1)
+    # every pair inside every critical radius: the deferred exact pass does all the work
+    N = 333
+    x, v, m = nb_inputs.random_cluster(N, seed=17, scale=0.05)
+    info = _kick_case(x, v, m, np.full(N, 10.0), what="sym all pairs", pair_capacity=1 << 17, **tune)
+    assert info["n_gpu"] == N * (N - 1) // 2
+
+
+@pytest.mark.parametrize("ipt,S", [(1, 256), (4, 512)])
+def test_sym_coincident_bodies(ipt, S):
+    tune = dict(force_kernel=SYM, i_per_thread=ipt, sym_block=S)
+    x, v, m = nb_inputs.random_cluster(300, seed=3)
+    x[7] = x[21]      # same 32-block (mixed visit)
+    x[40] = x[290]    # different blocks (symmetric visit)
+    rc = np.full(300, 0.01)
+    info = _kick_case(x, v, m, rc, what="sym coincident rc>0", **tune)
+    assert info["n_gpu"] >= 2
+    _kick_case(x, v, m, np.zeros(300), what="sym coincident rc=0", **tune)  # checks the singular count
+
+
+@pytest.mark.parametrize("cfg,n_override", [(0, 2048), (1, 3000), (2, 4096), (4, 5000)])
+@pytest.mark.parametrize("n1,n2", [(3.0, 0.0), (3.0, 0.4), (30.0, 0.0)])
+def test_sym_disk_configs_reduced(cfg, n_override, n1, n2):
+    d = nb_inputs.make_config(cfg, n_override=n_override)
+    rc = oracle.rcrit(d.x, d.v, d.m, d.M_star, d.dt, G_GAUSS, n1, n2)
+    info = _kick_case(d.x, d.v, d.m, rc, dt=0.5 * d.dt, force_kernel=SYM, what=f"sym {d.name} n1={n1} n2={n2}")
+    assert _geometry_is_symmetric(d.N)
+    if n1 == 30.0 or n2 > 0:
+        assert info["n_sure"] > 0
+
+
+def test_sym_semi_active_falls_back_to_tiles():
+    import paper_2604_09184_b200 as nb
+    d = nb_inputs.make_config(3, n_override=4096)
+    assert d.n_active < d.N
+    rc = oracle.rcrit(d.x, d.v, d.m, d.M_star, d.dt, G_GAUSS, 3.0, 0.4)
+    _kick_case(d.x, d.v, d.m, rc, n_active=d.n_active, force_kernel=SYM, what="sym requested, semi-active")
+    assert nb.force_geometry(d.N).tile_j > 0  # a passive body has no second side to serve
+
+
+def test_sym_bitwise_reproducible_and_close_to_tiles():
+    d = nb_inputs.make_config(2, n_override=6000)
+    rc = oracle.rcrit(d.x, d.v, d.m, d.M_star, d.dt, G_GAUSS, 3.0, 0.4)
+    out = []
+    for fk in (SYM, SYM, 1):
+        st = GpuState(d.x, d.v, d.m, G=G_GAUSS, force_kernel=fk)
+        st.set_rcrit(rc)
+        st.kick(0.0)
+        gp, n = st.get_pairs()
+        out.append((st.acc.cpu().numpy().copy(), {tuple(p) for p in gp.tolist()}))
+    assert np.array_equal(out[0][0], out[1][0]), "the symmetric kernel is not run-to-run reproducible"
+    assert out[0][1] == out[1][1] == out[2][1]
+    scale = np.linalg.norm(out[2][0], axis=1, keepdims=True)
+    assert np.max(np.abs(out[0][0] - out[2][0]) / scale) < 1e-12
+
+
+@pytest.mark.parametrize("nsteps", [1, 3, 100])
+def test_sym_step_matches_oracle(nsteps):
+    d = nb_inputs.make_config(1, n_override=1498)
+    st = GpuState(d.x, d.v, d.m, d.M_star, G=G_GAUSS, n1=3.0, n2=0.4, force_kernel=SYM, sym_block=256)
+    st.step(d.dt, nsteps)
+    xg, vg, ag, rcg = st.host()
+    ref = oracle.step(d.x, d.v, d.m, d.M_star, d.dt, G_GAUSS, nsteps, n1=3.0, n2=0.4)
+    tol = 1e-13 if nsteps <= 3 else 1e-9
+    assert np.max(np.abs(xg - ref["x"])) <= tol * np.max(np.abs(ref["x"]))
+    assert np.max(np.abs(vg - ref["v"])) <= tol * np.max(np.abs(ref["v"]))
+    acc_ref, ab, _ = oracle.accel(xg, d.m, rcg, G_GAUSS, want_abs=True)
+    assert_acc_close(ag, acc_ref, f"sym step x{nsteps}: final acc", ab)
+    sure, border = oracle.pairs(xg, rcg)
+    gp, n = st.get_pairs()
+    assert_pairs_match(gp, n, sure, border, f"sym step x{nsteps}")
+    D0 = oracle.diagnostics(d.x, d.v, d.m, d.M_star, G_GAUSS)
+    Dg = oracle.diagnostics(xg, vg, d.m, d.M_star, G_GAUSS)
+    Dr = oracle.diagnostics(ref["x"], ref["v"], d.m, d.M_star, G_GAUSS)
+    assert abs((Dg["E"] - D0["E"]) / D0["E"] - (Dr["E"] - D0["E"]) / D0["E"]) <= 1e-9
