@@ -51,6 +51,8 @@ def parse_args():
     ap.add_argument("--n", type=int, default=None, help="override the body count (debugging only)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--force-kernel", type=int, default=0, choices=[0, 1, 2],
+                    help="nb_config.force_kernel: 0 auto, 1 one-sided tiles, 2 Newton-III (comparison runs)")
     return ap.parse_args()
 
 
@@ -194,11 +196,12 @@ def run_reference(args):
 # ------------------------------------------------------------------------------------------------
 # CUDA arm
 # ------------------------------------------------------------------------------------------------
-def _traffic_from_profile():
-    """dram bytes per force-kernel launch from the committed ncu capture (profiles/), or None."""
+def _traffic_from_profile(kernel):
+    """dram bytes per launch of `kernel` at N = 65536 from the committed ncu capture (profiles/), or None."""
     p = os.path.join(ROOT, "profiles", "force_kernel_traffic.json")
     try:
-        return json.load(open(p)).get("dram_bytes_per_launch")
+        j = json.load(open(p))
+        return j.get(kernel, {}).get("dram_bytes_per_launch")
     except Exception:
         return None
 
@@ -229,7 +232,8 @@ def run_cuda(args):
     K, W = args.steps, max(args.warmup, 0)
 
     # ---- device-resident arm: inputs in HBM before the timed region -------------------------------
-    nb.configure(N, pair_capacity=cap, n_active=na, G=G_GAUSS, n1=N1, n2=N2, reuse_acc=False, time_force=True)
+    nb.configure(N, pair_capacity=cap, n_active=na, G=G_GAUSS, n1=N1, n2=N2, reuse_acc=False, time_force=True,
+                 force_kernel=args.force_kernel)
     nb.nb_status_reset()
     x = torch.from_numpy(d.x).cuda(); v = torch.from_numpy(d.v).cuda(); m = torch.from_numpy(d.m).cuda()
     acc = torch.zeros_like(x); rc = torch.zeros(N, dtype=torch.float64, device="cuda")
@@ -299,6 +303,11 @@ def run_cuda(args):
         return
 
     value = world * K * inter_per_step / (total_ms * 1e-3)
+    symmetric = geom.tile_j < 0
+    kernel = "nb_force_sym_kernel" if symmetric else "nb_force_tiles_kernel"
+    # FP64-pipe instructions per ORDERED interaction on the fast path: 20 per unordered pair (Newton III)
+    # or 15 (one-sided); DESIGN.md section 5
+    pipe_instr = 10.0 if symmetric else 15.0
     force_avg_ms = force_ms / max(n_force, 1)
     achieved_tf = FLOPS_PER_INTERACTION * inter_per_step / (force_avg_ms * 1e-3) / 1e12
     line = dict(
@@ -312,13 +321,13 @@ def run_cuda(args):
                     pairs_last_step=npairs_last, status=status, wall_s_incl_flush=wall),
         steps_per_sec=world * K / (total_ms * 1e-3),
         roofline=dict(bound="alu", achieved=achieved_tf, peak=FP64_PEAK_NOMINAL_TFLOPS, unit="TFLOP/s",
-                      frac=achieved_tf / FP64_PEAK_NOMINAL_TFLOPS, traffic=_traffic_from_profile(),
-                      kernel="nb_force_tiles_kernel", launches_timed=n_force, avg_launch_ms=force_avg_ms,
+                      frac=achieved_tf / FP64_PEAK_NOMINAL_TFLOPS, traffic=_traffic_from_profile(kernel) if N == 65536 else None,
+                      kernel=kernel, launches_timed=n_force, avg_launch_ms=force_avg_ms,
                       flops_per_interaction=FLOPS_PER_INTERACTION,
                       peak_source="nominal: 148 SM x 64 fp64 lanes x 2 x 1.965 GHz (DESIGN.md); MEASURED_PEAKS.json has no fp64 entry",
                       peak_measured_dfma=peak_tf, frac_of_measured_dfma=achieved_tf / peak_tf if peak_tf > 0 else None,
-                      fp64_pipe_instr_per_interaction=15,
-                      fp64_pipe_util_est=15.0 * inter_per_step / (force_avg_ms * 1e-3) / (peak_tf * 1e12 / 2.0) if peak_tf > 0 else None),
+                      fp64_pipe_instr_per_interaction=pipe_instr,
+                      fp64_pipe_util_est=pipe_instr * inter_per_step / (force_avg_ms * 1e-3) / (peak_tf * 1e12 / 2.0) if peak_tf > 0 else None),
         clocks=clocks, gpu_launches=4 * K,
     )
     if e2e:

@@ -28,8 +28,8 @@ struct PrepParams {
     const double *m;        // [N]
     double *rcrit;          // [N]; written when update_rc, read otherwise
     JRec *jrec;             // [Njpad] one-sided kernel's records (nullptr: not staged)
-    double2 *sxy, *szg;     // [Npad_sym] symmetric kernel's (x,y) and (z,Gm) (nullptr: not staged)
-    int *sthr;              // [Npad_sym] hi32(rcrit^2) + 1
+    double2 *sxy, *szg;     // [2 Npad_sym] symmetric kernel's (x,y) and (z,Gm), doubled-block layout (nullptr: not staged)
+    int *sthr;              // [2 Npad_sym] hi32(rcrit^2) + 1
     int Npad_sym;
     const double *mv_in;    // [nblk_in,3] momentum partials or nullptr
     unsigned long long *npairs;  // reset to 0 here (nullptr: skip)
@@ -83,9 +83,11 @@ __global__ void __launch_bounds__(kBodyThreads) nb_prep_kernel(const PrepParams 
         // positions (pad-pad distances stay huge and finite) and zero mass
         double sx_ = r.x, sy_ = r.y, sz_ = r.z;
         if (i >= p.N) { sx_ = kFarJ + 1.0e27 * (double)(i - p.N + 1); sy_ = kFarJ; sz_ = kFarJ; }
-        p.sxy[i] = make_double2(sx_, sy_);
-        p.szg[i] = make_double2(sz_, r.gm);
-        p.sthr[i] = __double2hiint(r.rc2) + 1;
+        const size_t en = (size_t)(i >> 5) * 64 + (i & 31);  // doubled-block layout (force_sym.cuh)
+        const int thr = __double2hiint(r.rc2) + 1;
+        p.sxy[en] = make_double2(sx_, sy_); p.sxy[en + 32] = make_double2(sx_, sy_);
+        p.szg[en] = make_double2(sz_, r.gm); p.szg[en + 32] = make_double2(sz_, r.gm);
+        p.sthr[en] = thr; p.sthr[en + 32] = thr;
     }
 }
 

@@ -5,8 +5,8 @@
 // the semi-active mode and of small N.
 //
 // Work unit: a super-tile (A, B), A <= B, of S x S bodies; one CTA of 4 warps per super-tile.
-//   * B's bodies (x, y | z, Gm | threshold word) are staged ONCE in shared memory by three TMA bulk
-//     copies; B's accelerations accumulate in shared memory (jS).
+//   * B's bodies (x, y | z, Gm | threshold word; doubled-block layout, see SymParams) are staged
+//     ONCE in shared memory by three TMA bulk copies; B's accelerations accumulate in shared memory (jS).
 //   * A's bodies are taken in chunks of 128*I; every lane holds I of them in registers together
 //     with their accumulators.
 //   * A warp meets a block of 32 j-bodies by ROTATION: lane l starts with j = l, evaluates its I
@@ -30,9 +30,13 @@
 namespace nbk {
 
 struct SymParams {
-    const double2 *sxy;          // [Npad] (x, y)      staged by nb_prep_kernel; padding bodies sit far
-    const double2 *szg;          // [Npad] (z, G m)    away at distinct places with zero mass
-    const int *sthr;             // [Npad] hi32(rcrit^2) + 1
+    // staged by nb_prep_kernel in the DOUBLED-BLOCK layout: every block of 32 bodies is stored twice in a
+    // row (entry of body n, copy h: (n >> 5) * 64 + 32 h + (n & 31)), so that the j-body lane l meets in
+    // rotation r sits at block + l + r with no wrap-around arithmetic.  Padding bodies sit far away at
+    // distinct places with zero mass.
+    const double2 *sxy;          // [2 Npad] (x, y)
+    const double2 *szg;          // [2 Npad] (z, G m)
+    const int *sthr;             // [2 Npad] hi32(rcrit^2) + 1
     const double *rcrit;         // [N]    exact critical radii (slow path only)
     double *part;                // [nsb, N, 3]
     int32_t *pairs;              // [cap,2] or nullptr
@@ -47,7 +51,11 @@ struct SymParams {
 };
 
 constexpr int kSymThreads = 128;
-__host__ __device__ constexpr size_t sym_smem_bytes(int S) { return (size_t)S * (16 + 16 + 24 + 4) + 16; }
+#ifndef NB_SYM_UNROLL
+#define NB_SYM_UNROLL 4
+#endif
+constexpr int kSymUnroll = NB_SYM_UNROLL;  // rotations unrolled in the hot loop
+__host__ __device__ constexpr size_t sym_smem_bytes(int S) { return (size_t)S * (32 + 32 + 24 + 8) + 16; }
 
 // Exact evaluation of the lane's I pairs against body j (deferred pass; entered by the lanes that
 // flagged rotation r, whose fast-path contributions were forced to exactly 0).  Returns the j-side
@@ -87,7 +95,8 @@ __device__ __forceinline__ void sym_exact(const SymParams &p, const double2 xy, 
     }
 }
 
-// One warp, one block of 32 j-bodies (shared-memory arrays qxy/qzg/qthr of the block), 32 rotations.
+// One warp, one block of 32 j-bodies (shared-memory arrays qxy/qzg/qthr of the doubled block: 64
+// entries each), 32 rotations.
 // On return (bx,by,bz) of lane l hold the sums for j = jbase + l.
 //
 // The rotation loop is branch-free so that consecutive rotations overlap in the FP64 pipe: a lane
@@ -106,13 +115,15 @@ __device__ __forceinline__ void sym_block(const SymParams &p, const double2 *__r
     const int lane = threadIdx.x & 31;
     const int down = (lane + 1) & 31;  // the lane whose j-sums this lane takes over after each rotation
     bx = 0.0; by = 0.0; bz = 0.0;
-    unsigned bits = 0u;
-#pragma unroll 4
+    unsigned bits = 0u, rbit = 1u;
+    const double2 *__restrict__ lxy = qxy + lane;
+    const double2 *__restrict__ lzg = qzg + lane;
+    const int *__restrict__ lthr = qthr + lane;
+#pragma unroll kSymUnroll
     for (int r = 0; r < 32; ++r) {
-        const int src = (lane + r) & 31;
-        const double2 xy = qxy[src];
-        const double2 zg = qzg[src];
-        const int thrj = qthr[src];
+        const double2 xy = lxy[r];
+        const double2 zg = lzg[r];
+        const int thrj = lthr[r];
         double dx[I], dy[I], dz[I], r2[I];
         int mn = 0x7fffffff;
 #pragma unroll
@@ -124,11 +135,13 @@ __device__ __forceinline__ void sym_block(const SymParams &p, const double2 *__r
             mn = min(mn, __double2hiint(r2[k]));
         }
         const bool hit = mn <= max(thr_lane, thrj);
-        if (hit) bits |= 1u << r;
+        if (hit) bits |= rbit;
+        rbit <<= 1;
+        // a flagged lane feeds +inf to the seed: rsqrt(+inf) = +0, so y0 = u = r^-3 = 0 for its I pairs
+        const int kill = hit ? 0x7ff00000 : 0;
 #pragma unroll
         for (int k = 0; k < I; ++k) {
-            const int yh = hit ? 0 : __double2hiint(rsqrt_seed(r2[k]));
-            const double y0 = __hiloint2double(yh, 0);
+            const double y0 = rsqrt_seed(__hiloint2double(max(__double2hiint(r2[k]), kill), 0));
             const double u = __dmul_rn(y0, y0);                          // exact (y0 has 21 bits)
             const double e = __fma_rn(-r2[k], u, 1.0);                   // 1 - r2 y0^2
             const double q = __fma_rn(e, __fma_rn(e, 1.875, 1.5), 1.0);  // (1-e)^(-3/2), next term < 2^-56
@@ -156,7 +169,7 @@ __device__ __forceinline__ void sym_block(const SymParams &p, const double2 *__r
 #pragma unroll
         for (int k = 0; k < I; ++k) emit[k] = false;
         if ((bits >> r) & 1u)
-            sym_exact<I>(p, qxy[src], qzg[src], jbase + src, mixed, xi, yi, zi, ngi, i0, ax, ay, az, cx, cy, cz, emit);
+            sym_exact<I>(p, lxy[r], lzg[r], jbase + src, mixed, xi, yi, zi, ngi, i0, ax, ay, az, cx, cy, cz, emit);
         if (PAIRS) {
 #pragma unroll
             for (int k = 0; k < I; ++k) pair_append(p.pairs, p.npairs, p.status, p.cap, emit[k], i0 + 32 * k, jbase + src);
@@ -175,12 +188,12 @@ __global__ void __launch_bounds__(kSymThreads, MINB) nb_force_sym_kernel(const S
     extern __shared__ __align__(16) unsigned char sym_smem[];
     const int S = p.S;
     double2 *bxy = reinterpret_cast<double2 *>(sym_smem);
-    double2 *bzg = bxy + S;
-    double *jsx = reinterpret_cast<double *>(bzg + S);
+    double2 *bzg = bxy + 2 * S;
+    double *jsx = reinterpret_cast<double *>(bzg + 2 * S);
     double *jsy = jsx + S;
     double *jsz = jsy + S;
     int *bthr = reinterpret_cast<int *>(jsz + S);
-    uint64_t *bar = reinterpret_cast<uint64_t *>(bthr + S);  // S*60 bytes in: 8-byte aligned (S % 128 == 0)
+    uint64_t *bar = reinterpret_cast<uint64_t *>(bthr + 2 * S);  // S*96 bytes in: 8-byte aligned
 
     const int t = threadIdx.x, lane = t & 31, w = t >> 5;
 
@@ -204,11 +217,11 @@ __global__ void __launch_bounds__(kSymThreads, MINB) nb_force_sym_kernel(const S
         mbar_init(bar, 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
         asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-        const unsigned b16 = (unsigned)S * 16u, b4 = (unsigned)S * 4u;
+        const unsigned b16 = (unsigned)S * 32u, b4 = (unsigned)S * 8u;
         mbar_expect_tx(bar, 2u * b16 + b4);
-        tma_bulk_g2s(bxy, p.sxy + (size_t)B * S, b16, bar);
-        tma_bulk_g2s(bzg, p.szg + (size_t)B * S, b16, bar);
-        tma_bulk_g2s(bthr, p.sthr + (size_t)B * S, b4, bar);
+        tma_bulk_g2s(bxy, p.sxy + (size_t)B * S * 2, b16, bar);
+        tma_bulk_g2s(bzg, p.szg + (size_t)B * S * 2, b16, bar);
+        tma_bulk_g2s(bthr, p.sthr + (size_t)B * S * 2, b4, bar);
     }
     for (int n = t; n < S; n += kSymThreads) { jsx[n] = 0.0; jsy[n] = 0.0; jsz[n] = 0.0; }
     __syncthreads();  // barrier initialised and accumulators zeroed before anyone proceeds
@@ -223,10 +236,11 @@ __global__ void __launch_bounds__(kSymThreads, MINB) nb_force_sym_kernel(const S
         int thr_lane = 0;
 #pragma unroll
         for (int k = 0; k < I; ++k) {
-            const double2 a = p.sxy[i0 + 32 * k];
-            const double2 b = p.szg[i0 + 32 * k];
+            const size_t en = (size_t)((i0 >> 5) + k) * 64 + lane;  // first copy of body i0 + 32 k
+            const double2 a = p.sxy[en];
+            const double2 b = p.szg[en];
             xi[k] = a.x; yi[k] = a.y; zi[k] = b.x; ngi[k] = -b.y;
-            thr_lane = max(thr_lane, p.sthr[i0 + 32 * k]);
+            thr_lane = max(thr_lane, p.sthr[en]);
             ax[k] = 0.0; ay[k] = 0.0; az[k] = 0.0;
         }
         for (int step = 0; step < nunits; ++step) {
@@ -240,7 +254,7 @@ __global__ void __launch_bounds__(kSymThreads, MINB) nb_force_sym_kernel(const S
                     mixed = q < P + I;
                 }
                 double bx, by, bz;
-                sym_block<I, PAIRS>(p, bxy + q * 32, bzg + q * 32, bthr + q * 32, B * S + q * 32, mixed, xi, yi, zi,
+                sym_block<I, PAIRS>(p, bxy + q * 64, bzg + q * 64, bthr + q * 64, B * S + q * 32, mixed, xi, yi, zi,
                                     ngi, thr_lane, i0, ax, ay, az, bx, by, bz);
                 if (!mixed) {
                     const int n = q * 32 + lane;

@@ -181,8 +181,8 @@ struct Workspace {
     double *mvA, *mvB;  // momentum partials [nblk,3]
     double *rc_scratch; // [N]
     JRec *jrec;         // [Njpad]                 (one-sided kernel)
-    double2 *sxy, *szg; // [Npad_sym]              (symmetric kernel)
-    int *sthr;          // [Npad_sym]
+    double2 *sxy, *szg; // [2 Npad_sym]            (symmetric kernel, doubled-block layout)
+    int *sthr;          // [2 Npad_sym]
     double *part;       // [nsplit, N, 3]
     size_t bytes;
 };
@@ -198,9 +198,9 @@ Workspace carve(void *base, int64_t N, const Geometry &g) {
     w.mvB = reinterpret_cast<double *>(b + off); off += align_up(nblk * 3 * sizeof(double), 256);
     w.rc_scratch = reinterpret_cast<double *>(b + off); off += align_up((size_t)N * sizeof(double), 256);
     w.jrec = reinterpret_cast<JRec *>(b + off); off += align_up((size_t)(g.sym ? 0 : g.Njpad) * sizeof(JRec), 256);
-    w.sxy = reinterpret_cast<double2 *>(b + off); off += align_up((size_t)g.Npad_sym * sizeof(double2), 256);
-    w.szg = reinterpret_cast<double2 *>(b + off); off += align_up((size_t)g.Npad_sym * sizeof(double2), 256);
-    w.sthr = reinterpret_cast<int *>(b + off); off += align_up((size_t)g.Npad_sym * sizeof(int), 256);
+    w.sxy = reinterpret_cast<double2 *>(b + off); off += align_up((size_t)2 * g.Npad_sym * sizeof(double2), 256);
+    w.szg = reinterpret_cast<double2 *>(b + off); off += align_up((size_t)2 * g.Npad_sym * sizeof(double2), 256);
+    w.sthr = reinterpret_cast<int *>(b + off); off += align_up((size_t)2 * g.Npad_sym * sizeof(int), 256);
     w.part = reinterpret_cast<double *>(b + off); off += align_up((size_t)g.nsplit * (size_t)N * 3 * sizeof(double), 256);
     w.bytes = off;
     return w;
