@@ -114,13 +114,16 @@ Geometry geometry(int64_t N, int64_t n_active) {
         int minb = g_cfg.ctas_per_sm >= 2 && g_cfg.ctas_per_sm <= 6 ? g_cfg.ctas_per_sm : (ipt == 4 ? 3 : 4);
         int S = g_cfg.sym_block;
         if (S != 256 && S != 512 && S != 1024 && S != 2048) {
-            // largest super-block (fewest partial slots, least staging) that still gives >= 8 waves
-            S = 1024;
+            // S = 512 runs 3 CTAs/SM at I = 4 (48 KB of shared memory each) and measured fastest; smaller when
+            // that would leave fewer than 8 waves of CTAs; larger only to keep the N/S partial slots
+            // (24 N^2 / S bytes of workspace) under 16 GiB
+            S = 512;
             while (S > 256 && S > 128 * ipt) {
                 const int64_t T = (N + S - 1) / S;
                 if (T * (T + 1) / 2 >= (int64_t)8 * minb * sms) break;
                 S >>= 1;
             }
+            while (S < 2048 && ((N + S - 1) / S) * N * 24 > ((int64_t)16 << 30)) S <<= 1;
         }
         if (S < 128 * ipt) S = 128 * ipt;
         g.sym = 1; g.S = S; g.U = S / 128; g.ipt = ipt; g.minb = minb; g.pipe = 0;
