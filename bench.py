@@ -51,6 +51,7 @@ def parse_args():
     ap.add_argument("--n", type=int, default=None, help="override the body count (debugging only)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-drift-point", action="store_true", help="skip the N = 2^24 drift-only HBM point")
     ap.add_argument("--force-kernel", type=int, default=0, choices=[0, 1, 2],
                     help="nb_config.force_kernel: 0 auto, 1 one-sided tiles, 2 Newton-III (comparison runs)")
     return ap.parse_args()
@@ -206,6 +207,43 @@ def _traffic_from_profile(kernel):
         return None
 
 
+def _hbm_peak_gbs():
+    """(GB/s, source): the driver-measured copy bandwidth, else the profiling guide's fallback."""
+    try:
+        return float(json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))["hbm_gbs"]), "MEASURED_PEAKS.json (burst copy)"
+    except Exception:
+        return 6650.0, "fallback of B200_PROFILING.md (MEASURED_PEAKS.json absent)"
+
+
+def drift_roofline(d, n_bodies=1 << 24, launches=5):
+    """HBM point of the Kepler drift (a6): the workload's bodies tiled to n_bodies (x, v: 96 bytes per
+    body in and out, 1.6 GB -- far beyond L2), nb_drift_kepler timed alone with CUDA events."""
+    import torch
+    import paper_2604_09184_b200 as nb
+    reps = -(-n_bodies // d.N)
+    x = torch.from_numpy(np.tile(d.x, (reps, 1))[:n_bodies].copy()).cuda()
+    v = torch.from_numpy(np.tile(d.v, (reps, 1))[:n_bodies].copy()).cuda()
+    nb.configure(n_bodies, G=G_GAUSS, workspace_bytes=4096)  # the O(N) calls need only the workspace head
+    nb.nb_status_reset()
+    for _ in range(2):
+        nb.nb_drift_kepler(x, v, d.M_star, d.dt)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    torch.cuda.synchronize()
+    e0.record()
+    for _ in range(launches):
+        nb.nb_drift_kepler(x, v, d.M_star, d.dt)
+    e1.record()
+    torch.cuda.synchronize()
+    ms = e0.elapsed_time(e1) / launches
+    fails = nb.nb_status()["kepler_fail"]
+    peak, src = _hbm_peak_gbs()
+    gbs = 96.0 * n_bodies / (ms * 1e-3) / 1e9
+    del x, v
+    return dict(kernel="nb_drift_kernel", bound="hbm", bodies=n_bodies, bytes_per_body=96, avg_launch_ms=ms,
+                achieved=gbs, peak=peak, unit="GB/s", frac=gbs / peak, peak_source=src, kepler_fail=fails,
+                bodies_per_sec=n_bodies / (ms * 1e-3))
+
+
 def run_cuda(args):
     import torch
     import torch.distributed as dist
@@ -334,6 +372,8 @@ def run_cuda(args):
         line["e2e"] = dict(value=world * e2e["Ke"] * inter_per_step / e2e["te"], unit=UNIT,
                            h2d_bytes_per_step=e2e["h2d"], d2h_bytes_per_step=e2e["d2h"], steps=e2e["Ke"],
                            call="nb_step_host(nsteps=1, reuse_acc=1): pageable numpy buffers in, results out, stream synchronised")
+    if not args.no_drift_point:
+        line["drift_roofline"] = drift_roofline(d)
     if not args.no_cpu_baseline:
         line["cpu_baseline"] = cpu_baseline(d, na)
     print(json.dumps(line), flush=True)

@@ -91,7 +91,9 @@ typedef struct nb_config {
 void nb_default_config(nb_config *cfg);
 /* Copies *cfg; validates G > 0, n1,n2 >= 0 and finite, pair_capacity >= 0, n_active >= 0. */
 int nb_configure(const nb_config *cfg);
-/* Bytes of scratch the device-pointer calls need for N bodies under the current tuning. */
+/* Bytes of scratch the device-pointer calls need for N bodies under the current tuning (the force
+ * kernels' partial sums dominate: 24 N x slots).  The O(N) calls need only its head: nb_rcrit none,
+ * nb_drift_kepler the first 512 bytes (status words), nb_shift 512 + 2 x roundup256(24 ceil(N/256)) bytes. */
 size_t nb_workspace_bytes(int64_t N);
 
 /*

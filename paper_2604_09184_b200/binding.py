@@ -151,9 +151,10 @@ def default_config() -> NbConfig:
 
 def configure(N=None, *, stream=None, pair_capacity=0, n_active=0, G=None, n1=3.0, n2=0.4, changeover_kind=0,
               i_per_thread=0, j_splits=0, use_graph=True, reuse_acc=False, time_force=False, ctas_per_sm=0,
-              pipeline_j=0, force_kernel=0, sym_block=0, device="cuda"):
+              pipeline_j=0, force_kernel=0, sym_block=0, workspace_bytes=None, device="cuda"):
     """nb_configure with a torch-allocated workspace sized for N bodies (N=None: no workspace,
-    enough for the _host calls).  Keeps the workspace tensor alive."""
+    enough for the _host calls; workspace_bytes: explicit size, e.g. the head that the O(N) calls
+    need).  Keeps the workspace tensor alive."""
     lib = load()
     cfg = default_config()
     if G is not None:
@@ -174,7 +175,7 @@ def configure(N=None, *, stream=None, pair_capacity=0, n_active=0, G=None, n1=3.
             stream = torch.cuda.current_stream().cuda_stream
         cfg.stream = C.c_void_p(int(stream)) if stream else None
         _check(lib.nb_configure(C.byref(cfg)))  # tuning first: the workspace size depends on it
-        nbytes = int(lib.nb_workspace_bytes(int(N)))
+        nbytes = int(lib.nb_workspace_bytes(int(N))) if workspace_bytes is None else int(workspace_bytes)
         ws = torch.zeros(nbytes + 256, dtype=torch.uint8, device=device)
         off = (-ws.data_ptr()) % 256
         cfg.workspace = C.c_void_p(ws.data_ptr() + off)

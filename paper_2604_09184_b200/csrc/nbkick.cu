@@ -226,6 +226,20 @@ int check_workspace(int64_t N, const Geometry &g, Workspace *w) {
     return NB_OK;
 }
 
+// The O(N) calls touch only the head of the workspace (status words, momentum partials): they must not
+// demand the O(N^2 / S) partial-sum area of the force kernels.
+int check_workspace_head(int64_t N, bool momentum, Workspace *w) {
+    if (g_cfg.workspace == nullptr) return fail(NB_E_WORKSPACE, "no workspace configured (nb_configure)");
+    if ((reinterpret_cast<uintptr_t>(g_cfg.workspace) & 255u) != 0) return fail(NB_E_WORKSPACE, "workspace is not 256-byte aligned");
+    Geometry g0;
+    std::memset(&g0, 0, sizeof(g0));
+    *w = carve(g_cfg.workspace, N, g0);
+    const size_t need = momentum ? (size_t)(reinterpret_cast<char *>(w->rc_scratch) - static_cast<char *>(g_cfg.workspace)) : 512;
+    if (need > g_cfg.workspace_bytes)
+        return fail(NB_E_WORKSPACE, "workspace has %zu bytes, this call needs %zu", g_cfg.workspace_bytes, need);
+    return NB_OK;
+}
+
 inline int body_blocks(int64_t n) { return (int)((n + kBodyThreads - 1) / kBodyThreads); }
 
 template <int I, int MINB, bool PIPE>
@@ -542,9 +556,8 @@ int nb_shift(double *x, const double *v, const double *m, double M_star, int64_t
     int rc = check_common(N, dt, M_star);
     if (rc) return rc;
     if (!x || !v || !m) return fail(NB_E_NULL, "nb_shift: NULL argument");
-    const Geometry g = geometry(N, g_cfg.n_active);
     Workspace w;
-    if ((rc = check_workspace(N, g, &w))) return rc;
+    if ((rc = check_workspace_head(N, true, &w))) return rc;
     const int nblk = body_blocks(N);
     nb_momentum_kernel<<<nblk, kBodyThreads, 0, stream()>>>(v, m, (int)N, w.mvA);
     nb_shift_kernel<<<nblk, kBodyThreads, 0, stream()>>>(x, w.mvA, nblk, (int)N, dt, M_star);
@@ -557,9 +570,8 @@ int nb_drift_kepler(double *x, double *v, double M_star, int64_t N, double dt) {
     int rc = check_common(N, dt, M_star);
     if (rc) return rc;
     if (!x || !v) return fail(NB_E_NULL, "nb_drift_kepler: NULL argument");
-    const Geometry g = geometry(N, g_cfg.n_active);
     Workspace w;
-    if ((rc = check_workspace(N, g, &w))) return rc;
+    if ((rc = check_workspace_head(N, false, &w))) return rc;
     nb_drift_kernel<<<body_blocks(N), kBodyThreads, 0, stream()>>>(x, v, nullptr, (int)N, g_cfg.G * M_star, dt, nullptr, 0,
                                                                    0.0, M_star, nullptr, w.status);
     NB_CUDA(cudaGetLastError());
