@@ -176,15 +176,20 @@ __global__ void __launch_bounds__(kBodyThreads) nb_drift_kernel(double *__restri
     const int i = blockIdx.x * kBodyThreads + threadIdx.x;
     double px = 0.0, py = 0.0, pz = 0.0;
     if (i < N) {
-        double X[3] = {x[3 * (size_t)i], x[3 * (size_t)i + 1], x[3 * (size_t)i + 2]};
-        double V[3] = {v[3 * (size_t)i], v[3 * (size_t)i + 1], v[3 * (size_t)i + 2]};
-        if (mv_in != nullptr) { X[0] = X[0] + dtc * sx; X[1] = X[1] + dtc * sy; X[2] = X[2] + dtc * sz; }
-        int rcode = kepler_elliptic(X, V, mu, dt);
-        if (rcode == 2) rcode = kepler_universal(X, V, mu, dt);
-        if (rcode != 0) status_add(status, ST_KEPLER_FAIL, 1);
-        x[3 * (size_t)i] = X[0]; x[3 * (size_t)i + 1] = X[1]; x[3 * (size_t)i + 2] = X[2];
-        v[3 * (size_t)i] = V[0]; v[3 * (size_t)i + 1] = V[1]; v[3 * (size_t)i + 2] = V[2];
-        if (mv_out != nullptr) { const double mi = m[i]; px = mi * V[0]; py = mi * V[1]; pz = mi * V[2]; }
+        double X0 = x[3 * (size_t)i], X1 = x[3 * (size_t)i + 1], X2 = x[3 * (size_t)i + 2];
+        double V0 = v[3 * (size_t)i], V1 = v[3 * (size_t)i + 1], V2 = v[3 * (size_t)i + 2];
+        if (mv_in != nullptr) { X0 = X0 + dtc * sx; X1 = X1 + dtc * sy; X2 = X2 + dtc * sz; }
+        if (kepler_elliptic_fast(X0, X1, X2, V0, V1, V2, mu, dt) != 0) {
+            // rare: not bound, or the fast iteration did not settle -> bracketed solvers (state untouched so far)
+            double X[3] = {X0, X1, X2}, V[3] = {V0, V1, V2};
+            int rcode = kepler_elliptic(X, V, mu, dt);
+            if (rcode == 2) rcode = kepler_universal(X, V, mu, dt);
+            if (rcode != 0) status_add(status, ST_KEPLER_FAIL, 1);
+            X0 = X[0]; X1 = X[1]; X2 = X[2]; V0 = V[0]; V1 = V[1]; V2 = V[2];
+        }
+        x[3 * (size_t)i] = X0; x[3 * (size_t)i + 1] = X1; x[3 * (size_t)i + 2] = X2;
+        v[3 * (size_t)i] = V0; v[3 * (size_t)i + 1] = V1; v[3 * (size_t)i + 2] = V2;
+        if (mv_out != nullptr) { const double mi = m[i]; px = mi * V0; py = mi * V1; pz = mi * V2; }
     }
     if (mv_out != nullptr) {
         block_sum3(px, py, pz, sm);

@@ -9,11 +9,108 @@ namespace nbk {
 constexpr double kTwoPi = 6.283185307179586476925286766559;
 constexpr double kEps = 2.220446049250313e-16;
 
+
+// ---- fast path of the bound-orbit solver -------------------------------------------------------
+// Same equations as kepler_elliptic below (differenced Kepler equation, Gauss f and g), arranged
+// for the FP64 pipe: no IEEE divide or sqrt (MUFU seeds + one third-order correction, ~1 ulp), ONE
+// library sincos -- of the half angle dE/2, which gives sin dE = 2SC and 1 - cos dE = 2S^2 without
+// cancellation -- and Halley steps whose trigonometric update is a rotation of (S, C) by the small
+// correction.  Anything unusual (not bound, no convergence in 8 steps, non-finite) returns nonzero
+// with the state untouched, and the caller falls back to the bracketed solver.
+
+__device__ __forceinline__ double rcp_fast(const double x) {
+    double y;
+    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));  // MUFU.RCP64H, ~2^-20
+    const double e = __fma_rn(-x, y, 1.0);
+    return __fma_rn(y, __fma_rn(e, e, e), y);               // y (1 + e + e^2): ~2^-60
+}
+// 1/sqrt(x) to ~2^-60 for normal x > 0
+__device__ __forceinline__ double rsqrt_fast(const double x) {
+    double y;
+    asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));  // MUFU.RSQ64H, ~2^-20
+    const double e = __fma_rn(-x, y * y, 1.0);
+    return __fma_rn(y * e, __fma_rn(e, 0.375, 0.5), y);       // y (1 + e/2 + 3 e^2/8)
+}
+// sqrt(x) from y = 1/sqrt(x): one Markstein correction
+__device__ __forceinline__ double sqrt_from_rsqrt(const double x, const double y) {
+    const double s = x * y;
+    return __fma_rn(__fma_rn(-s, s, x), 0.5 * y, s);
+}
+
+// Returns 0 ok (x, v advanced), nonzero: not handled here (state untouched).
+__device__ __forceinline__ int kepler_elliptic_fast(double &x0, double &x1, double &x2, double &v0, double &v1,
+                                                    double &v2, const double mu, const double h) {
+    const double rr = __fma_rn(x2, x2, __fma_rn(x1, x1, x0 * x0));
+    const double vv = __fma_rn(v2, v2, __fma_rn(v1, v1, v0 * v0));
+    const double u = __fma_rn(x2, v2, __fma_rn(x1, v1, x0 * v0));
+    if (!(rr > 1e-200 && rr < 1e200)) return 2;
+    const double ir0 = rsqrt_fast(rr);
+    const double r0 = sqrt_from_rsqrt(rr, ir0);
+    const double imu = rcp_fast(mu);
+    const double alpha = __fma_rn(-vv, imu, 2.0 * ir0);  // 1/a
+    if (!(alpha > 1e-100 && alpha < 1e100)) return 2;
+    const double a = rcp_fast(alpha);
+    const double t = mu * alpha;
+    const double irt = rsqrt_fast(t);                    // 1/sqrt(mu/a)
+    const double n = alpha * sqrt_from_rsqrt(t, irt);    // sqrt(mu/a^3)
+    const double inv_n = a * irt;
+    const double sma = mu * irt;                         // sqrt(mu a)
+    const double ec = __fma_rn(-r0, alpha, 1.0);
+    const double es = u * (irt * alpha);                 // u / sqrt(mu a)
+    double dM = n * h;
+    dM = __fma_rn(-kTwoPi, rint(dM * (1.0 / kTwoPi)), dM);
+    double dE = dM, S, C;
+    sincos(0.5 * dE, &S, &C);
+    const double omec = 1.0 - ec;
+    bool converged = false;
+#pragma unroll 1
+    for (int it = 0; it < 8; ++it) {
+        const double sd = 2.0 * S * C, cd = 2.0 * S * S;  // sin dE, 1 - cos dE
+        const double F = __fma_rn(es, cd, __fma_rn(-ec, sd, dE - dM));
+        const double Fp = __fma_rn(es, sd, __fma_rn(ec, cd, omec));          // r/a > 0
+        const double Fpp = __fma_rn(es, 1.0 - cd, ec * sd);
+        const double iFp = rcp_fast(Fp);
+        const double dN = -F * iFp;                                          // Newton
+        const double delta = __fma_rn(-dN, 0.5 * dN * Fpp * iFp, dN);        // Halley, expanded to first order
+        if (!(fabs(delta) < 1.0)) return 1;                                  // wild step or NaN: leave it to the bracketed solver
+        dE += delta;
+        const double hh = 0.5 * delta;
+        if (fabs(hh) <= 0.05) {
+            // rotate (S, C) by hh: Taylor series, next terms hh^11/11! and hh^12/12! < 1e-22
+            const double h2 = hh * hh;
+            const double sh = hh * __fma_rn(h2, __fma_rn(h2, __fma_rn(h2, __fma_rn(h2, 1.0 / 362880.0, -1.0 / 5040.0), 1.0 / 120.0), -1.0 / 6.0), 1.0);
+            const double chm1 = h2 * __fma_rn(h2, __fma_rn(h2, __fma_rn(h2, __fma_rn(h2, -1.0 / 3628800.0, 1.0 / 40320.0), -1.0 / 720.0), 1.0 / 24.0), -0.5);
+            const double Sn = __fma_rn(C, sh, __fma_rn(S, chm1, S));
+            const double Cn = __fma_rn(-S, sh, __fma_rn(C, chm1, C));
+            S = Sn; C = Cn;
+        } else {
+            sincos(0.5 * dE, &S, &C);
+        }
+        // cubic convergence: once |delta| < 2e-7 the next correction is below 1e-18 even for e = 0.9
+        if (fabs(delta) <= 2e-7 * fmax(1.0, fabs(dE))) { converged = true; break; }
+    }
+    if (!converged) return 1;
+    const double sd = 2.0 * S * C, cd = 2.0 * S * S;
+    const double Fp = __fma_rn(es, sd, __fma_rn(ec, cd, omec));  // r/a
+    const double iFp = rcp_fast(Fp);
+    const double ir = iFp * alpha;                               // 1/r
+    const double f = __fma_rn(-(a * ir0), cd, 1.0);
+    const double g = __fma_rn(r0 * alpha, sd, es * cd) * inv_n;
+    const double fd = -sma * sd * ir * ir0;
+    const double gd = __fma_rn(-iFp, cd, 1.0);
+    if (!(isfinite(f) && isfinite(g) && isfinite(fd) && isfinite(gd))) return 1;
+    const double n0 = __fma_rn(f, x0, g * v0), n1 = __fma_rn(f, x1, g * v1), n2 = __fma_rn(f, x2, g * v2);
+    const double w0 = __fma_rn(fd, x0, gd * v0), w1 = __fma_rn(fd, x1, gd * v1), w2 = __fma_rn(fd, x2, gd * v2);
+    x0 = n0; x1 = n1; x2 = n2;
+    v0 = w0; v1 = w1; v2 = w2;
+    return 0;
+}
+
 // Bound orbit (alpha = 2/r0 - v^2/mu > 0), differenced eccentric anomaly dE:
 //   F(dE) = dE - ec sin dE + es (1 - cos dE) - dM = 0,  F' = r/a > 0
 // Newton from dE = dM, kept inside a shrinking bracket [dM - 3e, dM + 3e] by bisection.
 // Returns 0 ok, 1 not converged (state untouched), 2 not elliptic (state untouched).
-__device__ __forceinline__ int kepler_elliptic(double (&x)[3], double (&v)[3], const double mu, const double h) {
+__device__ __noinline__ int kepler_elliptic(double (&x)[3], double (&v)[3], const double mu, const double h) {
     const double r0 = sqrt(x[0] * x[0] + x[1] * x[1] + x[2] * x[2]);
     const double v2 = v[0] * v[0] + v[1] * v[1] + v[2] * v[2];
     const double u = x[0] * v[0] + x[1] * v[1] + x[2] * v[2];
