@@ -55,6 +55,8 @@ def _L():
         lib.oracle_step.restype = i64
         lib.oracle_step.argtypes = [dp, dp, dp, dbl, i64, i64, dbl, dbl, dbl, dbl, i32, dp, dp, i64]
         lib.oracle_diagnostics.argtypes = [dp, dp, dp, dbl, i64, dbl, dp]
+        lib.oracle_groups.restype = i32
+        lib.oracle_groups.argtypes = [ip, i64, i64, ip, ip, ip, lp]
         _lib = lib
     return _lib
 
@@ -196,3 +198,22 @@ def diagnostics(x, v, m, M_star, G):
     out = np.empty(8)
     _L().oracle_diagnostics(px, pv, pm, M_star, m.shape[0], G, out.ctypes.data_as(C.POINTER(C.c_double)))
     return dict(E=out[0], L=out[1:4].copy(), T=out[4], T_star=out[5], U_star=out[6], U_mutual=out[7])
+
+
+def groups(pairs_, N):
+    """Independent encounter groups = connected components of the pair graph.
+    Returns dict(label[N], members[nmembers], gstart[ngroups+1], ngroups, nmembers, largest)."""
+    p = np.ascontiguousarray(np.asarray(pairs_, dtype=np.int32).reshape(-1, 2))
+    N = int(N)
+    label = np.empty(N, dtype=np.int32)
+    members = np.empty(max(N, 1), dtype=np.int32)
+    gstart = np.empty(N // 2 + 2, dtype=np.int32)
+    gstat = np.zeros(4, dtype=np.int64)
+    ip, lp = C.POINTER(C.c_int32), C.POINTER(C.c_int64)
+    rc = _L().oracle_groups(p.ctypes.data_as(ip), p.shape[0], N, label.ctypes.data_as(ip), members.ctypes.data_as(ip),
+                            gstart.ctypes.data_as(ip), gstat.ctypes.data_as(lp))
+    if rc != 0:
+        raise ValueError("oracle.groups: a pair holds an index outside [0, N) or i == j")
+    ng, nm = int(gstat[0]), int(gstat[1])
+    return dict(label=label, members=members[:nm].copy(), gstart=gstart[:ng + 1].copy(), ngroups=ng, nmembers=nm,
+                largest=int(gstat[2]))

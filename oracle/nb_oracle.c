@@ -11,6 +11,7 @@
  *   - H_A Kepler drift, Gauss f,g    PAPER.md:64, 98        (solver: reading S15)
  *   - step  B(dt/2) C(dt/2) A(dt) C(dt/2) B(dt/2)           PAPER.md:80 Eq. 3 (order: S6, S17)
  *   - diagnostics E, L               PAPER.md:84-92 Eq. 4-6 (K terms cancel in H_A + H_B)
+ *   - independent encounter groups   PAPER.md:106           (connected components of the pair graph)
  *
  * It is the definition written out: explicit loops in the paper's index order, no blocking,
  * no fusion, no FMA contraction (build with -ffp-contract=off).  All inputs and outputs are
@@ -455,4 +456,73 @@ void oracle_diagnostics(const double *x, const double *v, const double *m, doubl
     out[4] = T + Tc; out[5] = Ts; out[6] = Us + Usc; out[7] = Um + Umc;
     out[0] = ((out[4] + out[5]) + out[6]) + out[7];
     out[1] = L[0] + Lc[0]; out[2] = L[1] + Lc[1]; out[3] = L[2] + Lc[2];
+}
+
+
+/* ---------------------------------------------------------------------------------------------
+ * Independent close-encounter groups ("finding independent close encounter groups
+ * and integrating them independently"; the direct solver "propagates the involved
+ * bodies through the close encounter phase").  Two bodies belong to the same group when a chain of
+ * close-encounter pairs connects them: the groups are the connected components of the undirected
+ * graph (bodies, pairs).  This is the textbook statement: breadth-first search from every not yet
+ * visited body, taken in index order, over adjacency lists.
+ *
+ *   pairs  [npairs,2] int32 (any order inside a pair, duplicates allowed)
+ *   label  [N]  out: smallest body index of the body's group (a body without pairs: itself)
+ *   members[N]  out: the bodies of all groups with >= 2 members, group after group, groups ordered by
+ *               label, members ascending inside a group; the tail is filled with -1
+ *   gstart [N/2 + 2] out: members[gstart[g] .. gstart[g+1]) is group g; entries past ngroups+1: -1
+ *   gstat  [4]  out: number of groups (>= 2 members), number of member bodies, largest group,
+ *               number of pairs read
+ * Returns 0, or -1 if a pair holds an index outside [0, N) or i == j.
+ */
+static int cmp_i32(const void *a, const void *b) {
+    const int32_t x = *(const int32_t *)a, y = *(const int32_t *)b;
+    return (x > y) - (x < y);
+}
+
+int oracle_groups(const int32_t *pairs, int64_t npairs, int64_t N, int32_t *label, int32_t *members,
+                  int32_t *gstart, int64_t *gstat) {
+    int64_t *deg = (int64_t *)calloc((size_t)N + 1, sizeof(int64_t));
+    for (int64_t k = 0; k < npairs; ++k) {
+        const int64_t a = pairs[2 * k], b = pairs[2 * k + 1];
+        if (a < 0 || b < 0 || a >= N || b >= N || a == b) { free(deg); return -1; }
+        deg[a + 1]++; deg[b + 1]++;
+    }
+    for (int64_t i = 0; i < N; ++i) deg[i + 1] += deg[i];              /* CSR offsets */
+    int32_t *adj = (int32_t *)malloc(sizeof(int32_t) * (size_t)(2 * npairs + 1));
+    int64_t *fill = (int64_t *)malloc(sizeof(int64_t) * (size_t)(N + 1));
+    memcpy(fill, deg, sizeof(int64_t) * (size_t)(N + 1));
+    for (int64_t k = 0; k < npairs; ++k) {
+        const int32_t a = pairs[2 * k], b = pairs[2 * k + 1];
+        adj[fill[a]++] = b; adj[fill[b]++] = a;
+    }
+    int32_t *queue = (int32_t *)malloc(sizeof(int32_t) * (size_t)(N + 1));
+    for (int64_t i = 0; i < N; ++i) { label[i] = -1; members[i] = -1; }
+    for (int64_t g = 0; g < N / 2 + 2; ++g) gstart[g] = -1;
+    int64_t ngroups = 0, nmembers = 0, largest = 0;
+    for (int64_t i = 0; i < N; ++i) {
+        if (label[i] >= 0) continue;
+        label[i] = (int32_t)i;                    /* i is the smallest index of a new group */
+        if (deg[i + 1] == deg[i]) continue;       /* no pairs: a group of one, not listed */
+        int64_t head = 0, tail = 0;
+        queue[tail++] = (int32_t)i;
+        while (head < tail) {
+            const int32_t a = queue[head++];
+            for (int64_t e = deg[a]; e < deg[a + 1]; ++e) {
+                const int32_t b = adj[e];
+                if (label[b] < 0) { label[b] = (int32_t)i; queue[tail++] = b; }
+            }
+        }
+        qsort(queue, (size_t)tail, sizeof(int32_t), cmp_i32);
+        gstart[ngroups] = (int32_t)nmembers;
+        for (int64_t k = 0; k < tail; ++k) members[nmembers + k] = queue[k];
+        nmembers += tail;
+        ngroups++;
+        if (tail > largest) largest = tail;
+    }
+    gstart[ngroups] = (int32_t)nmembers;
+    gstat[0] = ngroups; gstat[1] = nmembers; gstat[2] = largest; gstat[3] = npairs;
+    free(deg); free(adj); free(fill); free(queue);
+    return 0;
 }
