@@ -305,6 +305,22 @@ def run_cuda(args):
     npairs_last = int(npairs.item())
     peak_tf, _ = nb.nb_fp64_peak(8192)
 
+    # ---- encounter groups of the last step's pair list: reported beside
+    # the step, not part of the timed region
+    g_label = torch.empty(N, dtype=torch.int32, device="cuda"); g_members = torch.empty(N, dtype=torch.int32, device="cuda")
+    g_start = torch.empty(N // 2 + 2, dtype=torch.int32, device="cuda"); g_stat = torch.zeros(4, dtype=torch.int64, device="cuda")
+    for _ in range(2):
+        nb.nb_groups(pairs, npairs, N, g_label, g_members, g_start, g_stat)
+    ge0, ge1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    ge0.record()
+    for _ in range(10):
+        nb.nb_groups(pairs, npairs, N, g_label, g_members, g_start, g_stat)
+    ge1.record()
+    torch.cuda.synchronize()
+    gs = [int(t) for t in g_stat.cpu().tolist()]
+    groups_info = dict(call="nb_groups", ms=ge0.elapsed_time(ge1) / 10, launches_per_call=9, pairs=gs[3], groups=gs[0],
+                       members=gs[1], largest=gs[2])
+
     # ---- end-to-end arm: host buffers through nb_step_host, copies inside the timed region ---------
     e2e = None
     if not args.no_e2e:
@@ -366,7 +382,7 @@ def run_cuda(args):
                       peak_measured_dfma=peak_tf, frac_of_measured_dfma=achieved_tf / peak_tf if peak_tf > 0 else None,
                       fp64_pipe_instr_per_interaction=pipe_instr,
                       fp64_pipe_util_est=pipe_instr * inter_per_step / (force_avg_ms * 1e-3) / (peak_tf * 1e12 / 2.0) if peak_tf > 0 else None),
-        clocks=clocks, gpu_launches=4 * K,
+        clocks=clocks, gpu_launches=4 * K, groups=groups_info,
     )
     if e2e:
         line["e2e"] = dict(value=world * e2e["Ke"] * inter_per_step / e2e["te"], unit=UNIT,

@@ -153,6 +153,25 @@ int nb_step(double *x, double *v, const double *m, double M_star, int64_t N, dou
             double *acc, int32_t *pairs, int64_t *npairs, int64_t nsteps);
 
 /*
+ * Independent close-encounter groups ("finding independent close encounter groups and
+ * integrating them independently"): the connected components of the graph whose edges
+ * are the rows of a pair list as written by nb_kick / nb_step.  Integer work, every output unique
+ * (bit-reproducible):
+ *   pairs   [pair_capacity,2] int32 in; npairs: device int64[1] in -- min(*npairs, pair_capacity) rows
+ *           are read (order inside a row and duplicates do not matter; a row with an index outside
+ *           [0,N) or i == j is skipped and counted in nb_status[2])
+ *   label   [N] int32 out: smallest body index of the body's group (a body without pairs: itself)
+ *   members [N] int32 out: the bodies of all groups with >= 2 members, group after group, groups
+ *           ordered by label, members ascending inside a group; the tail is -1
+ *   gstart  [N/2 + 2] int32 out: members[gstart[g] .. gstart[g+1]) is group g; entries past the last: -1
+ *   gstat   device int64[4] out: groups (>= 2 members), member bodies, largest group, pair rows read
+ * Needs the first 512 + 2 x roundup256(24 ceil(N/256)) + 5 x roundup256(4 N) + ~8 N/1024 + 768 bytes of
+ * the workspace (always inside nb_workspace_bytes(N)).
+ */
+int nb_groups(const int32_t *pairs, const int64_t *npairs, int64_t N, int32_t *label, int32_t *members,
+              int32_t *gstart, int64_t *gstat);
+
+/*
  * Host-buffer forms of nb_kick and nb_step: same semantics, every pointer is a HOST pointer
  * (pairs has room for pair_capacity rows; npairs is a host int64).  Inputs are copied to the
  * library's private device arena, the device path above runs, outputs are copied back, the

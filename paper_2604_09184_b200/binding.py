@@ -22,7 +22,7 @@ FORCE_AUTO, FORCE_TILES, FORCE_SYMMETRIC = 0, 1, 2
 # every symbol include/nbkick.h declares (tests check the library exports each of them)
 SYMBOLS = (
     "nb_default_config", "nb_configure", "nb_workspace_bytes", "nb_rcrit", "nb_kick", "nb_shift",
-    "nb_drift_kepler", "nb_step", "nb_kick_host", "nb_step_host", "nb_status", "nb_status_reset",
+    "nb_drift_kepler", "nb_step", "nb_groups", "nb_kick_host", "nb_step_host", "nb_status", "nb_status_reset",
     "nb_last_force_ms", "nb_force_time", "nb_force_time_reset", "nb_force_geometry", "nb_fp64_peak", "nb_release", "nb_last_error", "nb_version",
 )
 
@@ -84,6 +84,7 @@ def load():
     lib.nb_shift.argtypes = [vp, vp, vp, dbl, i64, dbl]
     lib.nb_drift_kepler.argtypes = [vp, vp, dbl, i64, dbl]
     lib.nb_step.argtypes = [vp, vp, vp, dbl, i64, dbl, vp, vp, vp, vp, i64]
+    lib.nb_groups.argtypes = [vp, vp, i64, vp, vp, vp, vp]
     lib.nb_kick_host.argtypes = [vp, vp, vp, dbl, i64, dbl, vp, vp, vp, vp]
     lib.nb_step_host.argtypes = [vp, vp, vp, dbl, i64, dbl, vp, vp, vp, vp, i64]
     lib.nb_status.argtypes = [C.POINTER(C.c_int64)]
@@ -234,6 +235,13 @@ def nb_step(x, v, m, M_star, dt, rcrit, acc, pairs=None, npairs=None, nsteps=1):
     _check(load().nb_step(_dev(x, 3 * N, torch.float64), _dev(v, 3 * N, torch.float64), _dev(m, N, torch.float64),
                           float(M_star), N, float(dt), _dev(rcrit, N, torch.float64), _dev(acc, 3 * N, torch.float64),
                           _dev(pairs, None, torch.int32), _dev(npairs, 1, torch.int64), int(nsteps)))
+
+
+def nb_groups(pairs, npairs, N, label, members, gstart, gstat):
+    import torch
+    _check(load().nb_groups(_dev(pairs, None, torch.int32), _dev(npairs, 1, torch.int64), int(N),
+                            _dev(label, N, torch.int32), _dev(members, N, torch.int32),
+                            _dev(gstart, N // 2 + 2, torch.int32), _dev(gstat, 4, torch.int64)))
 
 
 def nb_kick_host(x, v, m, M_star, dt, rcrit, acc, pairs=None, npairs=None):

@@ -13,6 +13,7 @@
 #include "body_kernels.cuh"
 #include "force_sym.cuh"
 #include "force_tiles.cuh"
+#include "groups.cuh"
 
 namespace {
 
@@ -182,6 +183,8 @@ struct Workspace {
     long long *status;  // ST_COUNT
     unsigned long long *npairs_dummy;
     double *mvA, *mvB;  // momentum partials [nblk,3]
+    GroupScratch grp;   // encounter groups (groups.cuh): 5 N + 2 ceil(N/1024) + N/2048 + 3 ints
+    char *head_mv_end, *head_grp_end;  // ends of the geometry-independent head
     double *rc_scratch; // [N]
     JRec *jrec;         // [Njpad]                 (one-sided kernel)
     double2 *sxy, *szg; // [2 Npad_sym]            (symmetric kernel, doubled-block layout)
@@ -199,6 +202,20 @@ Workspace carve(void *base, int64_t N, const Geometry &g) {
     w.npairs_dummy = reinterpret_cast<unsigned long long *>(b + off); off += 256;
     w.mvA = reinterpret_cast<double *>(b + off); off += align_up(nblk * 3 * sizeof(double), 256);
     w.mvB = reinterpret_cast<double *>(b + off); off += align_up(nblk * 3 * sizeof(double), 256);
+    w.head_mv_end = b + off;
+    {
+        const size_t n4 = align_up((size_t)N * sizeof(int), 256);
+        const size_t gblk = (size_t)((N + kGrpScanBlock - 1) / kGrpScanBlock);
+        w.grp.parent = reinterpret_cast<int *>(b + off); off += n4;
+        w.grp.size = reinterpret_cast<int *>(b + off); off += n4;
+        w.grp.segstart = reinterpret_cast<int *>(b + off); off += n4;
+        w.grp.cursor = reinterpret_cast<int *>(b + off); off += n4;
+        w.grp.tmp = reinterpret_cast<int *>(b + off); off += n4;
+        w.grp.bsum = reinterpret_cast<int *>(b + off); off += align_up(2 * gblk * sizeof(int), 256);
+        w.grp.giant = reinterpret_cast<int *>(b + off); off += align_up(((size_t)N / kGiant + 2) * sizeof(int), 256);
+        w.grp.ngiant = reinterpret_cast<int *>(b + off); off += 256;
+    }
+    w.head_grp_end = b + off;
     w.rc_scratch = reinterpret_cast<double *>(b + off); off += align_up((size_t)N * sizeof(double), 256);
     w.jrec = reinterpret_cast<JRec *>(b + off); off += align_up((size_t)(g.sym ? 0 : g.Njpad) * sizeof(JRec), 256);
     w.sxy = reinterpret_cast<double2 *>(b + off); off += align_up((size_t)2 * g.Npad_sym * sizeof(double2), 256);
@@ -228,13 +245,14 @@ int check_workspace(int64_t N, const Geometry &g, Workspace *w) {
 
 // The O(N) calls touch only the head of the workspace (status words, momentum partials): they must not
 // demand the O(N^2 / S) partial-sum area of the force kernels.
-int check_workspace_head(int64_t N, bool momentum, Workspace *w) {
+int check_workspace_head(int64_t N, int level /* 0 status, 1 + momentum partials, 2 + group scratch */, Workspace *w) {
     if (g_cfg.workspace == nullptr) return fail(NB_E_WORKSPACE, "no workspace configured (nb_configure)");
     if ((reinterpret_cast<uintptr_t>(g_cfg.workspace) & 255u) != 0) return fail(NB_E_WORKSPACE, "workspace is not 256-byte aligned");
     Geometry g0;
     std::memset(&g0, 0, sizeof(g0));
     *w = carve(g_cfg.workspace, N, g0);
-    const size_t need = momentum ? (size_t)(reinterpret_cast<char *>(w->rc_scratch) - static_cast<char *>(g_cfg.workspace)) : 512;
+    const char *base = static_cast<char *>(g_cfg.workspace);
+    const size_t need = level == 0 ? 512 : (size_t)((level == 1 ? w->head_mv_end : w->head_grp_end) - base);
     if (need > g_cfg.workspace_bytes)
         return fail(NB_E_WORKSPACE, "workspace has %zu bytes, this call needs %zu", g_cfg.workspace_bytes, need);
     return NB_OK;
@@ -557,7 +575,7 @@ int nb_shift(double *x, const double *v, const double *m, double M_star, int64_t
     if (rc) return rc;
     if (!x || !v || !m) return fail(NB_E_NULL, "nb_shift: NULL argument");
     Workspace w;
-    if ((rc = check_workspace_head(N, true, &w))) return rc;
+    if ((rc = check_workspace_head(N, 1, &w))) return rc;
     const int nblk = body_blocks(N);
     nb_momentum_kernel<<<nblk, kBodyThreads, 0, stream()>>>(v, m, (int)N, w.mvA);
     nb_shift_kernel<<<nblk, kBodyThreads, 0, stream()>>>(x, w.mvA, nblk, (int)N, dt, M_star);
@@ -571,7 +589,7 @@ int nb_drift_kepler(double *x, double *v, double M_star, int64_t N, double dt) {
     if (rc) return rc;
     if (!x || !v) return fail(NB_E_NULL, "nb_drift_kepler: NULL argument");
     Workspace w;
-    if ((rc = check_workspace_head(N, false, &w))) return rc;
+    if ((rc = check_workspace_head(N, 0, &w))) return rc;
     nb_drift_kernel<<<body_blocks(N), kBodyThreads, 0, stream()>>>(x, v, nullptr, (int)N, g_cfg.G * M_star, dt, nullptr, 0,
                                                                    0.0, M_star, nullptr, w.status);
     NB_CUDA(cudaGetLastError());
@@ -582,6 +600,37 @@ int nb_step(double *x, double *v, const double *m, double M_star, int64_t N, dou
             int32_t *pairs, int64_t *npairs, int64_t nsteps) {
     std::lock_guard<std::mutex> lk(g_mu);
     return step_impl(x, v, m, M_star, N, dt, rcrit, acc, pairs, npairs, nsteps);
+}
+
+int nb_groups(const int32_t *pairs, const int64_t *npairs, int64_t N, int32_t *label, int32_t *members, int32_t *gstart,
+              int64_t *gstat) {
+    std::lock_guard<std::mutex> lk(g_mu);
+    if (N <= 0 || N > 2147483647LL) return fail(NB_E_BADN, "N = %lld out of range (1 .. 2^31-1)", (long long)N);
+    if (!pairs || !npairs || !label || !members || !gstart || !gstat) return fail(NB_E_NULL, "nb_groups: NULL argument");
+    if (g_cfg.pair_capacity <= 0) return fail(NB_E_BADARG, "nb_groups: pair_capacity is 0 (nb_configure)");
+    Workspace w;
+    int rc = check_workspace_head(N, 2, &w);
+    if (rc) return rc;
+    const int n = (int)N;
+    const int nb256 = (n + kGrpThreads - 1) / kGrpThreads, nb1024 = (n + kGrpScanBlock - 1) / kGrpScanBlock;
+    long long *gs = reinterpret_cast<long long *>(gstat);
+    const long long cap = g_cfg.pair_capacity;
+    long long hook_blocks = (cap + kGrpThreads - 1) / kGrpThreads;
+    const long long max_blocks = (long long)sm_count() * 16;
+    if (hook_blocks > max_blocks) hook_blocks = max_blocks;
+    nb_grp_init_kernel<<<nb256, kGrpThreads, 0, stream()>>>(w.grp, label, members, gstart, gs, n);
+    nb_grp_hook_kernel<<<(unsigned)hook_blocks, kGrpThreads, 0, stream()>>>(w.grp, reinterpret_cast<const int2 *>(pairs),
+                                                                            reinterpret_cast<const long long *>(npairs), cap, n, gs,
+                                                                            w.status);
+    nb_grp_compress_kernel<<<nb256, kGrpThreads, 0, stream()>>>(w.grp, label, n);
+    nb_grp_blocksum_kernel<<<nb1024, kGrpScanBlock, 0, stream()>>>(w.grp, label, n);
+    nb_grp_topscan_kernel<<<1, kGrpScanBlock, 0, stream()>>>(w.grp, nb1024, gstart, gs);
+    nb_grp_offsets_kernel<<<nb1024, kGrpScanBlock, 0, stream()>>>(w.grp, label, n, gstart, gs);
+    nb_grp_scatter_kernel<<<nb256, kGrpThreads, 0, stream()>>>(w.grp, label, n);
+    nb_grp_ranksort_kernel<<<nb256, kGrpThreads, 0, stream()>>>(w.grp, label, gs, members);
+    nb_grp_giant_kernel<<<sm_count(), kGrpScanBlock, 0, stream()>>>(w.grp, label, n, members);
+    NB_CUDA(cudaGetLastError());
+    return NB_OK;
 }
 
 // ---- host-buffer forms: copy in, run the device path on the private arena, copy out ----
