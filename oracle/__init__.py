@@ -55,6 +55,7 @@ def _L():
         lib.oracle_step.restype = i64
         lib.oracle_step.argtypes = [dp, dp, dp, dbl, i64, i64, dbl, dbl, dbl, dbl, i32, dp, dp, i64]
         lib.oracle_diagnostics.argtypes = [dp, dp, dp, dbl, i64, dbl, dp]
+        lib.oracle_encounter.argtypes = [dp, dp, dp, dp, i64, dbl, dbl, dbl, i32, dbl, ip, ip, i64, i64, lp]
         lib.oracle_groups.restype = i32
         lib.oracle_groups.argtypes = [ip, i64, i64, ip, ip, ip, lp]
         _lib = lib
@@ -217,3 +218,60 @@ def groups(pairs_, N):
     ng, nm = int(gstat[0]), int(gstat[1])
     return dict(label=label, members=members[:nm].copy(), gstart=gstart[:ng + 1].copy(), ngroups=ng, nmembers=nm,
                 largest=int(gstat[2]))
+
+
+def encounter(x, v, m, rcrit_, M_star, dt, G, grp, kind=0, tol=1e-12, max_group=1024):
+    """H_A with encounters (Eq. 4, 98, 106): the members of every group of `grp` (a dict from
+    groups()) are advanced by dt with the Bulirsch-Stoer integrator; returns (x, v, stats) with
+    stats = dict(integrated, skipped, failed, steps)."""
+    x = np.array(x, dtype=np.float64, order="C"); v = np.array(v, dtype=np.float64, order="C")
+    m = np.ascontiguousarray(m, dtype=np.float64); rc = np.ascontiguousarray(rcrit_, dtype=np.float64)
+    N = m.shape[0]
+    members = np.ascontiguousarray(grp["members"], dtype=np.int32)
+    gstart = np.ascontiguousarray(grp["gstart"], dtype=np.int32)
+    stats = np.zeros(4, dtype=np.int64)
+    dp, ip, lp = C.POINTER(C.c_double), C.POINTER(C.c_int32), C.POINTER(C.c_int64)
+    _L().oracle_encounter(x.ctypes.data_as(dp), v.ctypes.data_as(dp), m.ctypes.data_as(dp), rc.ctypes.data_as(dp), N,
+                          float(M_star), float(G), float(dt), int(kind), float(tol), members.ctypes.data_as(ip),
+                          gstart.ctypes.data_as(ip), int(grp["ngroups"]), int(max_group), stats.ctypes.data_as(lp))
+    return x, v, dict(integrated=int(stats[0]), skipped=int(stats[1]), failed=int(stats[2]), steps=int(stats[3]))
+
+
+def step_enc(x, v, m, M_star, dt, G, nsteps, n1=3.0, n2=0.4, kind=0, tol=1e-12, max_group=1024):
+    """nsteps of B(dt/2) C(dt/2) A(dt) C(dt/2) B(dt/2) with close encounters resolved:
+    in A the members of the encounter groups of the step's opening pair list (groups of at most max_group
+    bodies) are propagated by encounter(), every other body by the Kepler drift.  Composed of the pinned
+    pieces above; rcrit is recomputed before every force evaluation (S17) and held through the step.
+    Returns dict(x, v, acc, rcrit, pairs, stats)."""
+    x = np.array(x, dtype=np.float64, order="C"); v = np.array(v, dtype=np.float64, order="C")
+    m = np.ascontiguousarray(m, dtype=np.float64)
+    N = m.shape[0]
+    tot = dict(integrated=0, skipped=0, failed=0, steps=0, border=0)
+
+    def evaluate(x, v):
+        rc = rcrit(x, v, m, M_star, dt, G, n1, n2)
+        acc, _, _ = accel(x, m, rc, G, kind=kind)
+        sure, border = pairs(x, rc)
+        tot["border"] += border.shape[0]
+        return rc, acc, sure
+
+    rc, acc, pr = evaluate(x, v)
+    for _ in range(int(nsteps)):
+        v = v + (0.5 * dt) * acc
+        x = shift(x, v, m, M_star, 0.5 * dt)
+        grp = groups(pr, N)
+        xk, vk, nfail = drift_kepler(x, v, M_star, dt, G)
+        xe, ve, st = encounter(x, v, m, rc, M_star, dt, G, grp, kind=kind, tol=tol, max_group=max_group)
+        moved = np.zeros(N, dtype=bool)
+        for g in range(grp["ngroups"]):
+            seg = grp["members"][grp["gstart"][g]:grp["gstart"][g + 1]]
+            if seg.shape[0] <= max_group:
+                moved[seg] = True
+        x = np.where(moved[:, None], xe, xk)
+        v = np.where(moved[:, None], ve, vk)
+        for k in ("integrated", "skipped", "failed", "steps"):
+            tot[k] += st[k]
+        x = shift(x, v, m, M_star, 0.5 * dt)
+        rc, acc, pr = evaluate(x, v)
+        v = v + (0.5 * dt) * acc
+    return dict(x=x, v=v, acc=acc, rcrit=rc, pairs=pr, stats=tot)

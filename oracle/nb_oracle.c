@@ -526,3 +526,156 @@ int oracle_groups(const int32_t *pairs, int64_t npairs, int64_t N, int32_t *labe
     free(deg); free(adj); free(fill); free(queue);
     return 0;
 }
+
+/* ---------------------------------------------------------------------------------------------
+ * Close-encounter propagation of one group (Eq. 4: H_A = Kepler terms + the pair terms
+ * weighted by [1 - K]; "when there is a close encounter, a direct solver is needed which
+ * propagates the involved bodies through the close encounter phase ... must not necessarily be
+ * symplectic"; groups are integrated independently).
+ *
+ * Equations of motion of the n members of a group under H_A (democratic coordinates; the weight
+ * multiplies the force, reading S3, so that kick + this = the full Newtonian pair force):
+ *     dx_i/dt = v_i
+ *     dv_i/dt = - G M_star x_i / r_i^3 + sum_{j in group, j != i} G m_j [1 - W(r_ij; rc_ij)] (x_j - x_i) / r_ij^3
+ * with W the kick weight of oracle_changeover and rc_ij = max(rc_i, rc_j) (S4), rc held fixed.
+ *
+ * Integrator (the paper prescribes none; reading S19): Bulirsch-Stoer -- Gragg's modified
+ * midpoint rule with 2, 4, ..., 16 substeps, polynomial (Aitken-Neville) extrapolation in h^2, at
+ * most 8 columns.  Error of a column = max over members of |dx|^2/|x|^2 and |dv|^2/max(|v|^2, mu/|x|)
+ * between the last two diagonal entries (x, v at the start of the step), accepted when <= tol^2.  Step control: accepted in <= 6 columns: next
+ * h = 1.3 h; in 8 columns: next h = 0.55 h; not accepted after 8 columns: retry with h/2.  The first
+ * trial step is the whole interval.  Returns the number of accepted steps, or -1 if h underflows.
+ * --------------------------------------------------------------------------------------------- */
+static double one_minus_changeover(double r, double rc, int kind) {
+    if (!(r < rc)) return 0.0;
+    double y = (r - 0.1 * rc) / (0.9 * rc);
+    if (y <= 0.0) return 1.0;
+    if (y >= 1.0) return 0.0;
+    double z = 1.0 - y;
+    if (kind == 1) return z * z * z * (1.0 + y * (3.0 + 6.0 * y));   /* 1 - (10y^3 - 15y^4 + 6y^5) */
+    return (z * z) / (2.0 * y * y - 2.0 * y + 1.0);                    /* 1 - y^2/(2y^2 - 2y + 1)   */
+}
+
+/* y = (x[3n], v[3n]) -> f = (v, a) */
+static void group_rhs(const double *y, double *f, int n, const double *gm, const double *rc, double mu, int kind) {
+    const double *x = y, *v = y + 3 * n;
+    for (int i = 0; i < n; ++i) {
+        double r2 = (x[3 * i] * x[3 * i] + x[3 * i + 1] * x[3 * i + 1]) + x[3 * i + 2] * x[3 * i + 2];
+        double s = -mu / (r2 * sqrt(r2));
+        double ax = s * x[3 * i], ay = s * x[3 * i + 1], az = s * x[3 * i + 2];
+        for (int j = 0; j < n; ++j) {
+            if (j == i) continue;
+            double dx = x[3 * j] - x[3 * i], dy = x[3 * j + 1] - x[3 * i + 1], dz = x[3 * j + 2] - x[3 * i + 2];
+            double d2 = (dx * dx + dy * dy) + dz * dz;
+            if (d2 == 0.0) continue;                       /* coincident: no direction, contributes nothing */
+            double d = sqrt(d2);
+            double rcij = rc[i] > rc[j] ? rc[i] : rc[j];
+            double w = one_minus_changeover(d, rcij, kind);
+            if (w == 0.0) continue;
+            double t = gm[j] * w / (d2 * d);
+            ax += t * dx; ay += t * dy; az += t * dz;
+        }
+        f[3 * i] = v[3 * i]; f[3 * i + 1] = v[3 * i + 1]; f[3 * i + 2] = v[3 * i + 2];
+        f[3 * n + 3 * i] = ax; f[3 * n + 3 * i + 1] = ay; f[3 * n + 3 * i + 2] = az;
+    }
+}
+
+#define BS_COLS 8
+
+int64_t oracle_encounter_group(double *y, int n, const double *gm, const double *rc, double mu, int kind,
+                               double dt, double tol) {
+    const int dim = 6 * n;
+    double *buf = (double *)malloc(sizeof(double) * (size_t)dim * (5 + BS_COLS));
+    double *f = buf, *ym = buf + dim, *yn = buf + 2 * dim, *tmp = buf + 3 * dim, *f0 = buf + 4 * dim;
+    double *T = buf + 5 * dim;                             /* T[c*dim + k]: current row of the tableau */
+    double t = 0.0, h = dt;
+    int64_t steps = 0;
+    const double tol2 = tol * tol;
+    while (t != dt) {
+        if (fabs(h) > fabs(dt - t)) h = dt - t;
+        if (fabs(h) < 1e-14 * fabs(dt)) { free(buf); return -1; }
+        group_rhs(y, f0, n, gm, rc, mu, kind);
+        int accepted = 0, cols = 0;
+        for (int c = 1; c <= BS_COLS && !accepted; ++c) {
+            const int nsub = 2 * c;
+            const double hs = h / nsub;
+            for (int k = 0; k < dim; ++k) { ym[k] = y[k]; yn[k] = y[k] + hs * f0[k]; }
+            for (int s = 2; s <= nsub; ++s) {
+                group_rhs(yn, f, n, gm, rc, mu, kind);
+                for (int k = 0; k < dim; ++k) { tmp[k] = ym[k] + 2.0 * hs * f[k]; ym[k] = yn[k]; yn[k] = tmp[k]; }
+            }
+            group_rhs(yn, f, n, gm, rc, mu, kind);
+            /* new tableau row: tmp[] runs along the row, T[] holds the previous row */
+            double err2 = 0.0;
+            for (int k = 0; k < dim; ++k) {
+                double cur = 0.5 * (ym[k] + yn[k] + hs * f[k]);     /* T_{c,0} */
+                double last_diag = c >= 2 ? T[(c - 2) * dim + k] : 0.0;  /* T_{c-1,c-2} */
+                for (int mcol = 1; mcol < c; ++mcol) {
+                    double ratio = (double)nsub / (double)(2 * (c - mcol));
+                    double old = T[(mcol - 1) * dim + k];               /* T_{c-1,mcol-1} */
+                    T[(mcol - 1) * dim + k] = cur;                      /* becomes T_{c,mcol-1} */
+                    cur = cur + (cur - old) / (ratio * ratio - 1.0);    /* T_{c,mcol} */
+                }
+                T[(c - 1) * dim + k] = cur;                             /* T_{c,c-1}: the diagonal */
+                tmp[k] = cur - last_diag;
+            }
+            if (c >= 2) {
+                for (int i = 0; i < n; ++i) {
+                    const double *dx = tmp + 3 * i, *dv = tmp + 3 * n + 3 * i;
+                    const double *xx = y + 3 * i, *vv = y + 3 * n + 3 * i;
+                    double ex = (dx[0] * dx[0] + dx[1] * dx[1]) + dx[2] * dx[2];
+                    double ev = (dv[0] * dv[0] + dv[1] * dv[1]) + dv[2] * dv[2];
+                    /* scales: heliocentric distance^2; speed^2, not below the circular speed^2 mu/r */
+                    double sx = (xx[0] * xx[0] + xx[1] * xx[1]) + xx[2] * xx[2];
+                    double sv = (vv[0] * vv[0] + vv[1] * vv[1]) + vv[2] * vv[2];
+                    double vc2 = mu / sqrt(sx);
+                    if (sv < vc2) sv = vc2;
+                    if (ex > err2 * sx) err2 = ex / sx;
+                    if (ev > err2 * sv) err2 = ev / sv;
+                }
+                if (err2 <= tol2) { accepted = 1; cols = c; }
+            }
+        }
+        if (accepted) {
+            for (int k = 0; k < dim; ++k) y[k] = T[(cols - 1) * dim + k];
+            t = (fabs(dt - (t + h)) <= 1e-15 * fabs(dt)) ? dt : t + h;
+            steps++;
+            if (cols <= 6) h *= 1.3; else if (cols == 8) h *= 0.55;
+        } else {
+            h *= 0.5;
+        }
+    }
+    free(buf);
+    return steps;
+}
+
+
+/* All listed groups of at most max_group members (members / gstart / ngroups as oracle_groups writes
+ * them), one after the other; x, v of the members are advanced in place by dt under H_A with
+ * encounters, every other body is left alone.  stats = {groups integrated, groups skipped because they
+ * exceed max_group, groups whose step size underflowed (left unchanged), accepted steps in total}. */
+void oracle_encounter(double *x, double *v, const double *m, const double *rcrit, int64_t N, double M_star,
+                      double G, double dt, int kind, double tol, const int32_t *members, const int32_t *gstart,
+                      int64_t ngroups, int64_t max_group, int64_t *stats) {
+    (void)N;
+    stats[0] = stats[1] = stats[2] = stats[3] = 0;
+    for (int64_t g = 0; g < ngroups; ++g) {
+        const int n = gstart[g + 1] - gstart[g];
+        if (n > max_group) { stats[1]++; continue; }
+        double *y = (double *)malloc(sizeof(double) * (size_t)(8 * n));
+        double *gm = y + 6 * n, *rc = y + 7 * n;
+        for (int k = 0; k < n; ++k) {
+            const int32_t b = members[gstart[g] + k];
+            for (int c = 0; c < 3; ++c) { y[3 * k + c] = x[3 * (int64_t)b + c]; y[3 * n + 3 * k + c] = v[3 * (int64_t)b + c]; }
+            gm[k] = G * m[b]; rc[k] = rcrit[b];
+        }
+        const int64_t st = oracle_encounter_group(y, n, gm, rc, G * M_star, kind, dt, tol);
+        if (st < 0) { stats[2]++; free(y); continue; }
+        for (int k = 0; k < n; ++k) {
+            const int32_t b = members[gstart[g] + k];
+            for (int c = 0; c < 3; ++c) { x[3 * (int64_t)b + c] = y[3 * k + c]; v[3 * (int64_t)b + c] = y[3 * n + 3 * k + c]; }
+        }
+        stats[0]++; stats[3] += st;
+        free(y);
+    }
+}
