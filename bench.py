@@ -320,6 +320,18 @@ def run_cuda(args):
     gs = [int(t) for t in g_stat.cpu().tolist()]
     groups_info = dict(call="nb_groups", ms=ge0.elapsed_time(ge1) / 10, launches_per_call=9, pairs=gs[3], groups=gs[0],
                        members=gs[1], largest=gs[2])
+    # direct solver of those groups for one dt, on copies of the state
+    xe, ve = x.clone(), v.clone()
+    nb.nb_encounter(xe, ve, m, rc, d.M_star, d.dt, g_members, g_start, g_stat)
+    xe.copy_(x); ve.copy_(v)
+    ge0.record()
+    nb.nb_encounter(xe, ve, m, rc, d.M_star, d.dt, g_members, g_start, g_stat)
+    ge1.record()
+    torch.cuda.synchronize()
+    st_enc = nb.nb_status()
+    groups_info.update(encounter_call="nb_encounter", encounter_ms=ge0.elapsed_time(ge1), bs_tol=1e-12,
+                       groups_skipped=st_enc["groups_skipped"], bs_fail=st_enc["bs_fail"])
+    del xe, ve
 
     # ---- end-to-end arm: host buffers through nb_step_host, copies inside the timed region ---------
     e2e = None

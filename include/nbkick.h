@@ -86,6 +86,10 @@ typedef struct nb_config {
                                 no graph replay (default 0) */
     int force_kernel;        /* NB_FORCE_AUTO (default), NB_FORCE_TILES, NB_FORCE_SYMMETRIC (see below) */
     int sym_block;           /* tuning: super-block size S of the symmetric kernel (256, 512, 1024, 2048), 0 = auto */
+    int resolve_encounters;  /* nb_step: 1 = the members of the encounter groups of each step's pair list are
+                                propagated through A(dt) by the direct solver (nb_encounter) instead of the Kepler
+                                drift; needs pairs != NULL (default 0: pure Kepler drift) */
+    double bs_tol;           /* relative tolerance of the direct solver's Bulirsch-Stoer steps (default 1e-12) */
 } nb_config;
 
 void nb_default_config(nb_config *cfg);
@@ -172,6 +176,24 @@ int nb_groups(const int32_t *pairs, const int64_t *npairs, int64_t N, int32_t *l
               int32_t *gstart, int64_t *gstat);
 
 /*
+ * H_A with close encounters (Eq. 4: Kepler terms plus the pair terms weighted by [1 - K];
+ * PAPER.md:98 "a direct solver is needed which propagates the involved bodies through the close
+ * encounter phase"; PAPER.md:106 groups are integrated independently).  The members of every listed
+ * group (members / gstart / gstat as nb_groups writes them) are advanced by dt under
+ *     dx_i/dt = v_i,
+ *     dv_i/dt = -G M_star x_i/r_i^3 + sum_{j in group, j != i} G m_j [1 - W(r_ij; rc_ij)] (x_j - x_i)/r_ij^3
+ * (W, rc_ij as in nb_kick, rcrit held fixed; weight on the force: reading S3) with a Bulirsch-Stoer
+ * integrator of relative tolerance bs_tol (reading S19: the paper prescribes no method); every other body
+ * is left alone.  Groups of more than NB_MAX_GROUP members are left alone as well and counted in
+ * nb_status[4] (the regime for which the paper proposes multi-level changeovers); a group
+ * whose step size underflows is left unchanged and counted in nb_status[5].
+ * x, v [N,3] in/out; m, rcrit [N] in.  Needs the first 512 bytes of the workspace.
+ */
+#define NB_MAX_GROUP 1024
+int nb_encounter(double *x, double *v, const double *m, const double *rcrit, double M_star, int64_t N,
+                 double dt, const int32_t *members, const int32_t *gstart, const int64_t *gstat);
+
+/*
  * Host-buffer forms of nb_kick and nb_step: same semantics, every pointer is a HOST pointer
  * (pairs has room for pair_capacity rows; npairs is a host int64).  Inputs are copied to the
  * library's private device arena, the device path above runs, outputs are copied back, the
@@ -185,11 +207,13 @@ int nb_step_host(double *x, double *v, const double *m, double M_star, int64_t N
 
 /*
  * Lazy device-side conditions accumulated since the last nb_status_reset; synchronises the
- * stream.  flags (host int64[4]):
+ * stream.  flags (host int64[6]):
  *   [0] pairs dropped because the list was full (sum over evaluations)
  *   [1] Kepler solver non-convergences (body left unchanged)
- *   [2] non-finite positions / masses / radii seen while staging j-bodies
+ *   [2] non-finite positions / masses / radii seen while staging j-bodies; invalid rows of a pair list
  *   [3] coincident bodies (r_ij == 0, i != j) that contributed nothing
+ *   [4] encounter groups larger than NB_MAX_GROUP, left to the Kepler drift
+ *   [5] encounter groups whose Bulirsch-Stoer step size underflowed (left unchanged)
  */
 int nb_status(int64_t *flags);
 int nb_status_reset(void);

@@ -22,7 +22,7 @@ FORCE_AUTO, FORCE_TILES, FORCE_SYMMETRIC = 0, 1, 2
 # every symbol include/nbkick.h declares (tests check the library exports each of them)
 SYMBOLS = (
     "nb_default_config", "nb_configure", "nb_workspace_bytes", "nb_rcrit", "nb_kick", "nb_shift",
-    "nb_drift_kepler", "nb_step", "nb_groups", "nb_kick_host", "nb_step_host", "nb_status", "nb_status_reset",
+    "nb_drift_kepler", "nb_step", "nb_groups", "nb_encounter", "nb_kick_host", "nb_step_host", "nb_status", "nb_status_reset",
     "nb_last_force_ms", "nb_force_time", "nb_force_time_reset", "nb_force_geometry", "nb_fp64_peak", "nb_release", "nb_last_error", "nb_version",
 )
 
@@ -47,6 +47,8 @@ class NbConfig(C.Structure):
         ("time_force", C.c_int),
         ("force_kernel", C.c_int),
         ("sym_block", C.c_int),
+        ("resolve_encounters", C.c_int),
+        ("bs_tol", C.c_double),
     ]
 
 
@@ -85,6 +87,7 @@ def load():
     lib.nb_drift_kepler.argtypes = [vp, vp, dbl, i64, dbl]
     lib.nb_step.argtypes = [vp, vp, vp, dbl, i64, dbl, vp, vp, vp, vp, i64]
     lib.nb_groups.argtypes = [vp, vp, i64, vp, vp, vp, vp]
+    lib.nb_encounter.argtypes = [vp, vp, vp, vp, dbl, i64, dbl, vp, vp, vp]
     lib.nb_kick_host.argtypes = [vp, vp, vp, dbl, i64, dbl, vp, vp, vp, vp]
     lib.nb_step_host.argtypes = [vp, vp, vp, dbl, i64, dbl, vp, vp, vp, vp, i64]
     lib.nb_status.argtypes = [C.POINTER(C.c_int64)]
@@ -152,7 +155,8 @@ def default_config() -> NbConfig:
 
 def configure(N=None, *, stream=None, pair_capacity=0, n_active=0, G=None, n1=3.0, n2=0.4, changeover_kind=0,
               i_per_thread=0, j_splits=0, use_graph=True, reuse_acc=False, time_force=False, ctas_per_sm=0,
-              pipeline_j=0, force_kernel=0, sym_block=0, workspace_bytes=None, device="cuda"):
+              pipeline_j=0, force_kernel=0, sym_block=0, resolve_encounters=False, bs_tol=1e-12, workspace_bytes=None,
+              device="cuda"):
     """nb_configure with a torch-allocated workspace sized for N bodies (N=None: no workspace,
     enough for the _host calls; workspace_bytes: explicit size, e.g. the head that the O(N) calls
     need).  Keeps the workspace tensor alive."""
@@ -170,6 +174,7 @@ def configure(N=None, *, stream=None, pair_capacity=0, n_active=0, G=None, n1=3.
     cfg.time_force = 1 if time_force else 0
     cfg.ctas_per_sm, cfg.pipeline_j = int(ctas_per_sm), int(pipeline_j)
     cfg.force_kernel, cfg.sym_block = int(force_kernel), int(sym_block)
+    cfg.resolve_encounters, cfg.bs_tol = (1 if resolve_encounters else 0), float(bs_tol)
     if N is not None:
         import torch
         if stream is None:
@@ -244,6 +249,14 @@ def nb_groups(pairs, npairs, N, label, members, gstart, gstat):
                             _dev(gstart, N // 2 + 2, torch.int32), _dev(gstat, 4, torch.int64)))
 
 
+def nb_encounter(x, v, m, rcrit, M_star, dt, members, gstart, gstat):
+    import torch
+    N = m.numel()
+    _check(load().nb_encounter(_dev(x, 3 * N, torch.float64), _dev(v, 3 * N, torch.float64), _dev(m, N, torch.float64),
+                               _dev(rcrit, N, torch.float64), float(M_star), N, float(dt), _dev(members, N, torch.int32),
+                               _dev(gstart, N // 2 + 2, torch.int32), _dev(gstat, 4, torch.int64)))
+
+
 def nb_kick_host(x, v, m, M_star, dt, rcrit, acc, pairs=None, npairs=None):
     N = m.size
     _check(load().nb_kick_host(_host(x, 3 * N), _host(v, 3 * N), _host(m, N), float(M_star), N, float(dt),
@@ -259,9 +272,10 @@ def nb_step_host(x, v, m, M_star, dt, rcrit, acc, pairs=None, npairs=None, nstep
 
 
 def nb_status() -> dict:
-    f = (C.c_int64 * 4)()
+    f = (C.c_int64 * 6)()
     _check(load().nb_status(f))
-    return dict(pairs_dropped=int(f[0]), kepler_fail=int(f[1]), nonfinite=int(f[2]), singular=int(f[3]))
+    return dict(pairs_dropped=int(f[0]), kepler_fail=int(f[1]), nonfinite=int(f[2]), singular=int(f[3]),
+                groups_skipped=int(f[4]), bs_fail=int(f[5]))
 
 
 def nb_status_reset():

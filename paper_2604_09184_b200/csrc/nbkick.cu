@@ -11,6 +11,7 @@
 #include <mutex>
 
 #include "body_kernels.cuh"
+#include "encounter.cuh"
 #include "force_sym.cuh"
 #include "force_tiles.cuh"
 #include "groups.cuh"
@@ -20,7 +21,7 @@ namespace {
 using namespace nbk;
 
 std::mutex g_mu;
-nb_config g_cfg = {nullptr, nullptr, 0, 0, 0, 0.01720209895 * 0.01720209895, 3.0, 0.4, 0, 0, 0, 1, 0, 0, 0, 0, 0, 0};
+nb_config g_cfg = {nullptr, nullptr, 0, 0, 0, 0.01720209895 * 0.01720209895, 3.0, 0.4, 0, 0, 0, 1, 0, 0, 0, 0, 0, 0, 0, 1e-12};
 char g_err[512] = "";
 int g_sm_count = 0;
 cudaEvent_t g_ev0 = nullptr, g_ev1 = nullptr;
@@ -37,8 +38,8 @@ size_t g_arena_bytes = 0;
 struct StepKey {
     const void *x, *v, *m, *rcrit, *acc, *pairs, *npairs, *ws, *stream;
     int64_t N, n_active, cap;
-    double dt, M_star, G, n1, n2;
-    int kind, ipt, jsplit;
+    double dt, M_star, G, n1, n2, bs_tol;
+    int kind, ipt, jsplit, enc;
     size_t ws_bytes;
 };
 StepKey g_graph_key;
@@ -184,6 +185,8 @@ struct Workspace {
     unsigned long long *npairs_dummy;
     double *mvA, *mvB;  // momentum partials [nblk,3]
     GroupScratch grp;   // encounter groups (groups.cuh): 5 N + 2 ceil(N/1024) + N/2048 + 3 ints
+    int32_t *g_label, *g_members, *g_start;  // the step driver's own group lists
+    int64_t *g_stat;
     char *head_mv_end, *head_grp_end;  // ends of the geometry-independent head
     double *rc_scratch; // [N]
     JRec *jrec;         // [Njpad]                 (one-sided kernel)
@@ -214,6 +217,13 @@ Workspace carve(void *base, int64_t N, const Geometry &g) {
         w.grp.bsum = reinterpret_cast<int *>(b + off); off += align_up(2 * gblk * sizeof(int), 256);
         w.grp.giant = reinterpret_cast<int *>(b + off); off += align_up(((size_t)N / kGiant + 2) * sizeof(int), 256);
         w.grp.ngiant = reinterpret_cast<int *>(b + off); off += 256;
+    }
+    {   // group outputs of the step driver (resolve_encounters): label, members, gstart, gstat
+        const size_t n4 = align_up((size_t)N * sizeof(int), 256);
+        w.g_label = reinterpret_cast<int32_t *>(b + off); off += n4;
+        w.g_members = reinterpret_cast<int32_t *>(b + off); off += n4;
+        w.g_start = reinterpret_cast<int32_t *>(b + off); off += align_up(((size_t)N / 2 + 2) * sizeof(int), 256);
+        w.g_stat = reinterpret_cast<int64_t *>(b + off); off += 256;
     }
     w.head_grp_end = b + off;
     w.rc_scratch = reinterpret_cast<double *>(b + off); off += align_up((size_t)N * sizeof(double), 256);
@@ -394,6 +404,51 @@ void drop_graph() {
     if (g_graph_exec) { cudaGraphExecDestroy(g_graph_exec); g_graph_exec = nullptr; }
 }
 
+// the nine launches of nb_groups (groups.cuh)
+void enqueue_groups(const Workspace &w, const int32_t *pairs, const int64_t *npairs, int64_t N, int32_t *label,
+                    int32_t *members, int32_t *gstart, int64_t *gstat) {
+    const int n = (int)N;
+    const int nb256 = (n + kGrpThreads - 1) / kGrpThreads, nb1024 = (n + kGrpScanBlock - 1) / kGrpScanBlock;
+    long long *gs = reinterpret_cast<long long *>(gstat);
+    const long long cap = g_cfg.pair_capacity;
+    long long hook_blocks = (cap + kGrpThreads - 1) / kGrpThreads;
+    const long long max_blocks = (long long)sm_count() * 16;
+    if (hook_blocks > max_blocks) hook_blocks = max_blocks;
+    nb_grp_init_kernel<<<nb256, kGrpThreads, 0, stream()>>>(w.grp, label, members, gstart, gs, n);
+    nb_grp_hook_kernel<<<(unsigned)hook_blocks, kGrpThreads, 0, stream()>>>(w.grp, reinterpret_cast<const int2 *>(pairs),
+                                                                            reinterpret_cast<const long long *>(npairs), cap, n, gs,
+                                                                            w.status);
+    nb_grp_compress_kernel<<<nb256, kGrpThreads, 0, stream()>>>(w.grp, label, n);
+    nb_grp_blocksum_kernel<<<nb1024, kGrpScanBlock, 0, stream()>>>(w.grp, label, n);
+    nb_grp_topscan_kernel<<<1, kGrpScanBlock, 0, stream()>>>(w.grp, nb1024, gstart, gs);
+    nb_grp_offsets_kernel<<<nb1024, kGrpScanBlock, 0, stream()>>>(w.grp, label, n, gstart, gs);
+    nb_grp_scatter_kernel<<<nb256, kGrpThreads, 0, stream()>>>(w.grp, label, n);
+    nb_grp_ranksort_kernel<<<nb256, kGrpThreads, 0, stream()>>>(w.grp, label, gs, members);
+    nb_grp_giant_kernel<<<sm_count(), kGrpScanBlock, 0, stream()>>>(w.grp, label, n, members);
+}
+
+// H_A with encounters for the listed groups (encounter.cuh): groups of up to 32 members by CTAs of one warp,
+// up to kMaxGroup members by CTAs of kMaxGroup threads
+void enqueue_encounter(const Workspace &w, double *x, double *v, const double *m, const double *rcrit, double M_star,
+                       int64_t N, double dt, const int32_t *members, const int32_t *gstart, const int64_t *gstat) {
+    EncParams ep;
+    ep.x = x; ep.v = v; ep.m = m; ep.rcrit = rcrit; ep.members = members; ep.gstart = gstart;
+    ep.gstat = reinterpret_cast<const long long *>(gstat); ep.status = w.status; ep.mu = g_cfg.G * M_star; ep.G = g_cfg.G;
+    ep.dt = dt; ep.tol = g_cfg.bs_tol > 0.0 ? g_cfg.bs_tol : 1e-12; ep.kind = g_cfg.changeover_kind;
+    long long small_blocks = N / 2 + 1;
+    const long long cap_blocks = (long long)sm_count() * 32;
+    if (small_blocks > cap_blocks) small_blocks = cap_blocks;
+    ep.min_size = 2; ep.max_size = 32;
+    nb_encounter_kernel<32><<<(unsigned)small_blocks, 32, (5 * 32 + 32) * sizeof(double), stream()>>>(ep);
+    ep.min_size = 33; ep.max_size = kMaxGroup;
+    static bool attr_set = false;
+    const size_t big_smem = (5 * (size_t)kMaxGroup + 32) * sizeof(double);
+    if (!attr_set) { cudaFuncSetAttribute(nb_encounter_kernel<kMaxGroup>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)big_smem); attr_set = true; }
+    long long big_blocks = N / 33 + 1;
+    if (big_blocks > 2LL * sm_count()) big_blocks = 2LL * sm_count();
+    nb_encounter_kernel<kMaxGroup><<<(unsigned)big_blocks, kMaxGroup, big_smem, stream()>>>(ep);
+}
+
 int step_impl(double *x, double *v, const double *m, double M_star, int64_t N, double dt, double *rcrit, double *acc,
               int32_t *pairs, int64_t *npairs, int64_t nsteps) {
     int rc = check_common(N, dt, M_star);
@@ -420,10 +475,20 @@ int step_impl(double *x, double *v, const double *m, double M_star, int64_t N, d
             return rc;
     }
 
+    const bool enc = g_cfg.resolve_encounters != 0;
+    if (enc && !pairs) return fail(NB_E_BADARG, "nb_step: resolve_encounters needs the pair list (pairs != NULL)");
     auto enqueue_step = [&](int nhalf) -> int {
-        // C(dt/2) A(dt): first half-shift folded into the drift kernel
-        nb_drift_kernel<<<nblk, kBodyThreads, 0, stream()>>>(x, v, m, (int)N, mu, dt, w.mvA, nblk, dtc, M_star, w.mvB,
-                                                             w.status);
+        // groups of the pair list of the evaluation that opened this step
+        if (enc) enqueue_groups(w, pairs, npairs, N, w.g_label, w.g_members, w.g_start, w.g_stat);
+        // C(dt/2) A(dt): first half-shift folded into the drift kernel; members of groups are only shifted there
+        // and then propagated through their encounter by the direct solver
+        nb_drift_kernel<<<nblk, kBodyThreads, 0, stream()>>>(x, v, m, (int)N, mu, dt, w.mvA, nblk, dtc, M_star,
+                                                             enc ? nullptr : w.mvB, w.status, enc ? w.g_label : nullptr,
+                                                             enc ? w.grp.size : nullptr);
+        if (enc) {
+            enqueue_encounter(w, x, v, m, rc_io, M_star, N, dt, w.g_members, w.g_start, w.g_stat);
+            nb_momentum_kernel<<<nblk, kBodyThreads, 0, stream()>>>(v, m, (int)N, w.mvB);
+        }
         // C(dt/2) folded into prep; force; B(dt/2) [+ B(dt/2) of the next step]
         return enqueue_eval(w, g, x, v, m, M_star, N, dt, rc_io, update_rc, w.mvB, dtc, acc, pairs, npairs, hk, nhalf,
                             w.mvA, false);
@@ -436,7 +501,7 @@ int step_impl(double *x, double *v, const double *m, double M_star, int64_t N, d
         key.x = x; key.v = v; key.m = m; key.rcrit = rc_io; key.acc = acc; key.pairs = pairs; key.npairs = npairs;
         key.ws = g_cfg.workspace; key.stream = g_cfg.stream; key.N = N; key.n_active = g_cfg.n_active;
         key.cap = g_cfg.pair_capacity; key.dt = dt; key.M_star = M_star; key.G = g_cfg.G; key.n1 = g_cfg.n1;
-        key.n2 = g_cfg.n2; key.kind = g_cfg.changeover_kind; key.ipt = g.S * 1000 + g.ipt * 100 + g.minb * 10 + g.pipe; key.jsplit = g.nsplit;
+        key.n2 = g_cfg.n2; key.kind = g_cfg.changeover_kind; key.bs_tol = g_cfg.bs_tol; key.enc = enc ? 1 : 0; key.ipt = g.S * 1000 + g.ipt * 100 + g.minb * 10 + g.pipe; key.jsplit = g.nsplit;
         key.ws_bytes = g_cfg.workspace_bytes;
         const bool hop = !stream_capturable();
         if (hop) {
@@ -513,6 +578,8 @@ void nb_default_config(nb_config *cfg) {
     cfg->time_force = 0;
     cfg->force_kernel = NB_FORCE_AUTO;
     cfg->sym_block = 0;
+    cfg->resolve_encounters = 0;
+    cfg->bs_tol = 1e-12;
 }
 
 int nb_configure(const nb_config *cfg) {
@@ -532,6 +599,7 @@ int nb_configure(const nb_config *cfg) {
         return fail(NB_E_BADARG, "unknown force_kernel %d", cfg->force_kernel);
     if (cfg->sym_block != 0 && cfg->sym_block != 256 && cfg->sym_block != 512 && cfg->sym_block != 1024 && cfg->sym_block != 2048)
         return fail(NB_E_BADARG, "sym_block must be 0, 256, 512, 1024 or 2048");
+    if (!(cfg->bs_tol >= 0.0) || !std::isfinite(cfg->bs_tol)) return fail(NB_E_BADARG, "bs_tol must be finite and >= 0");
     g_cfg = *cfg;
     return NB_OK;
 }
@@ -591,7 +659,7 @@ int nb_drift_kepler(double *x, double *v, double M_star, int64_t N, double dt) {
     Workspace w;
     if ((rc = check_workspace_head(N, 0, &w))) return rc;
     nb_drift_kernel<<<body_blocks(N), kBodyThreads, 0, stream()>>>(x, v, nullptr, (int)N, g_cfg.G * M_star, dt, nullptr, 0,
-                                                                   0.0, M_star, nullptr, w.status);
+                                                                   0.0, M_star, nullptr, w.status, nullptr, nullptr);
     NB_CUDA(cudaGetLastError());
     return NB_OK;
 }
@@ -611,24 +679,20 @@ int nb_groups(const int32_t *pairs, const int64_t *npairs, int64_t N, int32_t *l
     Workspace w;
     int rc = check_workspace_head(N, 2, &w);
     if (rc) return rc;
-    const int n = (int)N;
-    const int nb256 = (n + kGrpThreads - 1) / kGrpThreads, nb1024 = (n + kGrpScanBlock - 1) / kGrpScanBlock;
-    long long *gs = reinterpret_cast<long long *>(gstat);
-    const long long cap = g_cfg.pair_capacity;
-    long long hook_blocks = (cap + kGrpThreads - 1) / kGrpThreads;
-    const long long max_blocks = (long long)sm_count() * 16;
-    if (hook_blocks > max_blocks) hook_blocks = max_blocks;
-    nb_grp_init_kernel<<<nb256, kGrpThreads, 0, stream()>>>(w.grp, label, members, gstart, gs, n);
-    nb_grp_hook_kernel<<<(unsigned)hook_blocks, kGrpThreads, 0, stream()>>>(w.grp, reinterpret_cast<const int2 *>(pairs),
-                                                                            reinterpret_cast<const long long *>(npairs), cap, n, gs,
-                                                                            w.status);
-    nb_grp_compress_kernel<<<nb256, kGrpThreads, 0, stream()>>>(w.grp, label, n);
-    nb_grp_blocksum_kernel<<<nb1024, kGrpScanBlock, 0, stream()>>>(w.grp, label, n);
-    nb_grp_topscan_kernel<<<1, kGrpScanBlock, 0, stream()>>>(w.grp, nb1024, gstart, gs);
-    nb_grp_offsets_kernel<<<nb1024, kGrpScanBlock, 0, stream()>>>(w.grp, label, n, gstart, gs);
-    nb_grp_scatter_kernel<<<nb256, kGrpThreads, 0, stream()>>>(w.grp, label, n);
-    nb_grp_ranksort_kernel<<<nb256, kGrpThreads, 0, stream()>>>(w.grp, label, gs, members);
-    nb_grp_giant_kernel<<<sm_count(), kGrpScanBlock, 0, stream()>>>(w.grp, label, n, members);
+    enqueue_groups(w, pairs, npairs, N, label, members, gstart, gstat);
+    NB_CUDA(cudaGetLastError());
+    return NB_OK;
+}
+
+int nb_encounter(double *x, double *v, const double *m, const double *rcrit, double M_star, int64_t N, double dt,
+                 const int32_t *members, const int32_t *gstart, const int64_t *gstat) {
+    std::lock_guard<std::mutex> lk(g_mu);
+    int rc = check_common(N, dt, M_star);
+    if (rc) return rc;
+    if (!x || !v || !m || !rcrit || !members || !gstart || !gstat) return fail(NB_E_NULL, "nb_encounter: NULL argument");
+    Workspace w;
+    if ((rc = check_workspace_head(N, 0, &w))) return rc;
+    enqueue_encounter(w, x, v, m, rcrit, M_star, N, dt, members, gstart, gstat);
     NB_CUDA(cudaGetLastError());
     return NB_OK;
 }
@@ -708,7 +772,7 @@ int nb_status(int64_t *flags) {
     std::lock_guard<std::mutex> lk(g_mu);
     if (!flags) return fail(NB_E_NULL, "flags is NULL");
     if (!g_cfg.workspace && !g_arena) return fail(NB_E_WORKSPACE, "no workspace configured");
-    int64_t a[ST_COUNT] = {0, 0, 0, 0}, b[ST_COUNT] = {0, 0, 0, 0};
+    int64_t a[ST_COUNT] = {0}, b[ST_COUNT] = {0};
     if (g_cfg.workspace) NB_CUDA(cudaMemcpyAsync(a, g_cfg.workspace, sizeof(a), cudaMemcpyDeviceToHost, stream()));
     if (g_arena) NB_CUDA(cudaMemcpyAsync(b, g_arena, sizeof(b), cudaMemcpyDeviceToHost, stream()));  // _host calls
     NB_CUDA(cudaStreamSynchronize(stream()));
