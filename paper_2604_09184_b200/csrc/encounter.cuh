@@ -13,6 +13,7 @@
 // rejected: h /= 2; the first trial step is the whole interval.  Every thread of the CTA takes the same
 // decisions (the error is a CTA-wide maximum), so the control flow is uniform.
 #pragma once
+#include "kepler.cuh"  // rcp_fast, rsqrt_fast, sqrt_from_rsqrt (MUFU seed + one third-order correction, ~1 ulp)
 #include "nb_common.cuh"
 
 namespace nbk {
@@ -20,14 +21,43 @@ namespace nbk {
 constexpr int kBsCols = 8;
 constexpr int kMaxGroup = 1024;  // larger groups are left to the Kepler drift and counted (NB_MAX_GROUP)
 
-__device__ __forceinline__ double one_minus_changeover(const double r, const double rc, const int kind) {
-    if (!(r < rc)) return 0.0;
-    const double y = (r - 0.1 * rc) / (0.9 * rc);
-    if (y <= 0.0) return 1.0;
-    if (y >= 1.0) return 0.0;
-    const double z = 1.0 - y;
-    if (kind == 1) return z * z * z * (1.0 + y * (3.0 + 6.0 * y));
-    return (z * z) / (2.0 * y * y - 2.0 * y + 1.0);
+// Acceleration of a body at q = (x, y, z) with critical radius my_rc: star term plus the [1 - W] pair terms of
+// the n members whose positions / G m / rc sit in the given (shared-memory) arrays; `self` is skipped.
+// No IEEE divide or sqrt on the common path (latency is what a small group pays for).
+__device__ __forceinline__ void enc_accel(const double qx, const double qy, const double qz, const double my_rc,
+                                          const int self, const int n, const double *__restrict__ px,
+                                          const double *__restrict__ py, const double *__restrict__ pz,
+                                          const double *__restrict__ sgm, const double *__restrict__ src,
+                                          const double mu, const int kind, double &ax, double &ay, double &az) {
+    const double r2 = (qx * qx + qy * qy) + qz * qz;
+    const double ir = rsqrt_fast(r2);
+    const double s = -mu * (ir * ir * ir);
+    ax = s * qx; ay = s * qy; az = s * qz;
+    for (int j = 0; j < n; ++j) {
+        if (j == self) continue;
+        const double dx = px[j] - qx, dy = py[j] - qy, dz = pz[j] - qz;
+        const double d2 = (dx * dx + dy * dy) + dz * dz;
+        const double rc = fmax(my_rc, src[j]);
+        if (!(d2 < rc * rc) || d2 == 0.0) continue;      // 1 - W = 0 outside rc; coincident: no direction
+        const double id = rsqrt_fast(d2);
+        const double d = sqrt_from_rsqrt(d2, id);
+        double w = 1.0;
+        const double t0 = d - 0.1 * rc;
+        if (t0 > 0.0) {
+            const double y = t0 * rcp_fast(0.9 * rc);
+            if (y >= 1.0) continue;
+            const double z = 1.0 - y;
+            w = kind == 1 ? z * z * z * (1.0 + y * (3.0 + 6.0 * y)) : (z * z) * rcp_fast(2.0 * y * y - 2.0 * y + 1.0);
+        }
+        const double tt = sgm[j] * w * (id * id * id);
+        ax += tt * dx; ay += tt * dy; az += tt * dz;
+    }
+}
+
+// 1 / ((n_c / n_{c-m})^2 - 1) of the Aitken-Neville extrapolation, n_k = 2k
+__device__ __forceinline__ double bs_weight(const int c, const int mc) {
+    const double ratio = (double)(2 * c) / (double)(2 * (c - mc));
+    return 1.0 / (ratio * ratio - 1.0);
 }
 
 struct EncParams {
@@ -91,20 +121,8 @@ __global__ void __launch_bounds__(THREADS) nb_encounter_kernel(const EncParams p
             if (act) { px[t] = q[0]; py[t] = q[1]; pz[t] = q[2]; }
             __syncthreads();
             if (act) {
-                const double r2 = (q[0] * q[0] + q[1] * q[1]) + q[2] * q[2];
-                const double s = -p.mu / (r2 * sqrt(r2));
-                double ax = s * q[0], ay = s * q[1], az = s * q[2];
-                for (int j = 0; j < n; ++j) {
-                    if (j == t) continue;
-                    const double dx = px[j] - q[0], dy = py[j] - q[1], dz = pz[j] - q[2];
-                    const double d2 = (dx * dx + dy * dy) + dz * dz;
-                    if (d2 == 0.0) continue;
-                    const double d = sqrt(d2);
-                    const double w = one_minus_changeover(d, fmax(my_rc, src[j]), p.kind);
-                    if (w == 0.0) continue;
-                    const double tt = sgm[j] * w / (d2 * d);
-                    ax += tt * dx; ay += tt * dy; az += tt * dz;
-                }
+                double ax, ay, az;
+                enc_accel(q[0], q[1], q[2], my_rc, t, n, px, py, pz, sgm, src, p.mu, p.kind, ax, ay, az);
                 f[0] = q[3]; f[1] = q[4]; f[2] = q[5]; f[3] = ax; f[4] = ay; f[5] = az;
             }
         };
@@ -136,10 +154,9 @@ __global__ void __launch_bounds__(THREADS) nb_encounter_kernel(const EncParams p
                     double cur = 0.5 * (ym[k] + yn[k] + hs * f[k]);
                     const double last_diag = c >= 2 ? T[c - 2][k] : 0.0;
                     for (int mc = 1; mc < c; ++mc) {
-                        const double ratio = (double)nsub / (double)(2 * (c - mc));
                         const double old = T[mc - 1][k];
                         T[mc - 1][k] = cur;
-                        cur = cur + (cur - old) / (ratio * ratio - 1.0);
+                        cur = cur + (cur - old) * bs_weight(c, mc);
                     }
                     T[c - 1][k] = cur;
                     dif[k] = cur - last_diag;
@@ -174,6 +191,143 @@ __global__ void __launch_bounds__(THREADS) nb_encounter_kernel(const EncParams p
         } else if (act) {
 #pragma unroll
             for (int c = 0; c < 3; ++c) { p.x[3 * (size_t)b + c] = y[c]; p.v[3 * (size_t)b + c] = y[3 + c]; }
+        }
+    }
+}
+
+// Groups of up to 32 members: latency is everything (a hard pair takes tens of serial Bulirsch-Stoer steps),
+// so the 8 extrapolation columns of a trial step -- independent modified-midpoint integrations with 2, 4,
+// ..., 16 substeps -- run CONCURRENTLY, one warp per column, lane = member; warp 0 then builds the tableau
+// column by column exactly as the sequential algorithm does and accepts the first column that passes, so
+// the result is the sequential algorithm's, bit for bit.  Critical path per step: 17 right-hand sides
+// instead of up to 80.
+__global__ void __launch_bounds__(32 * kBsCols) nb_encounter_small_kernel(const EncParams p) {
+    __shared__ double px[kBsCols][32], py[kBsCols][32], pz[kBsCols][32];
+    __shared__ double sgm[32], src[32];
+    __shared__ double col[kBsCols][6][32];   // T_{c,0} of every column
+    __shared__ double ycur[6][32];
+    __shared__ double ctrl_h, ctrl_t;
+    __shared__ int ctrl_done;                // 0 running, 1 finished, 2 failed
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    const long long ngroups = p.gstat[0];
+    const double tol2 = p.tol * p.tol;
+    for (long long g = blockIdx.x; g < ngroups; g += gridDim.x) {
+        const int g0 = p.gstart[g], n = p.gstart[g + 1] - g0;
+        if (n < p.min_size || n > p.max_size) continue;
+        const bool act = lane < n;
+        const int b = act ? p.members[g0 + lane] : 0;
+        __syncthreads();
+        if (w == 0) {
+            if (act) {
+#pragma unroll
+                for (int c = 0; c < 3; ++c) { ycur[c][lane] = p.x[3 * (size_t)b + c]; ycur[3 + c][lane] = p.v[3 * (size_t)b + c]; }
+                sgm[lane] = p.G * p.m[b];
+                src[lane] = p.rcrit[b];
+            }
+            if (lane == 0) { ctrl_h = p.dt; ctrl_t = 0.0; ctrl_done = (p.dt == 0.0) ? 1 : 0; }
+        }
+        __syncthreads();
+        const double my_rc = act ? src[lane] : 0.0;
+        double T[kBsCols][6];                // warp 0: current row of the tableau
+        while (true) {
+            if (ctrl_done != 0) break;
+            double h = ctrl_h;
+            const double tcur = ctrl_t;
+            if (fabs(h) > fabs(p.dt - tcur)) h = p.dt - tcur;
+            const bool underflow = fabs(h) < 1e-14 * fabs(p.dt);
+            double y[6];
+#pragma unroll
+            for (int k = 0; k < 6; ++k) y[k] = act ? ycur[k][lane] : 0.0;
+            if (!underflow) {
+                // column c = w + 1: modified midpoint with 2c substeps
+                auto rhs = [&](const double (&q)[6], double (&f)[6]) {
+                    __syncwarp();
+                    if (act) { px[w][lane] = q[0]; py[w][lane] = q[1]; pz[w][lane] = q[2]; }
+                    __syncwarp();
+                    if (act) {
+                        double ax, ay, az;
+                        enc_accel(q[0], q[1], q[2], my_rc, lane, n, px[w], py[w], pz[w], sgm, src, p.mu, p.kind, ax, ay, az);
+                        f[0] = q[3]; f[1] = q[4]; f[2] = q[5]; f[3] = ax; f[4] = ay; f[5] = az;
+                    }
+                };
+                const int c = w + 1, nsub = 2 * c;
+                const double hs = h / nsub;
+                double f0[6] = {0, 0, 0, 0, 0, 0}, f[6] = {0, 0, 0, 0, 0, 0}, ym[6], yn[6];
+                rhs(y, f0);
+#pragma unroll
+                for (int k = 0; k < 6; ++k) { ym[k] = y[k]; yn[k] = y[k] + hs * f0[k]; }
+                for (int s = 2; s <= nsub; ++s) {
+                    rhs(yn, f);
+#pragma unroll
+                    for (int k = 0; k < 6; ++k) { const double tmp = ym[k] + 2.0 * hs * f[k]; ym[k] = yn[k]; yn[k] = tmp; }
+                }
+                rhs(yn, f);
+#pragma unroll
+                for (int k = 0; k < 6; ++k) col[w][k][lane] = 0.5 * (ym[k] + yn[k] + hs * f[k]);
+            }
+            __syncthreads();
+            if (w == 0) {
+                bool accepted = false;
+                int cols = 0;
+                if (!underflow) {
+                    for (int c = 1; c <= kBsCols && !accepted; ++c) {
+                        double dif[6];
+#pragma unroll
+                        for (int k = 0; k < 6; ++k) {
+                            double cur = col[c - 1][k][lane];
+                            const double last_diag = c >= 2 ? T[c - 2][k] : 0.0;
+                            for (int mc = 1; mc < c; ++mc) {
+                                const double old = T[mc - 1][k];
+                                T[mc - 1][k] = cur;
+                                cur = cur + (cur - old) * bs_weight(c, mc);
+                            }
+                            T[c - 1][k] = cur;
+                            dif[k] = cur - last_diag;
+                        }
+                        if (c >= 2) {
+                            double e2 = 0.0;
+                            if (act) {
+                                const double ex = (dif[0] * dif[0] + dif[1] * dif[1]) + dif[2] * dif[2];
+                                const double ev = (dif[3] * dif[3] + dif[4] * dif[4]) + dif[5] * dif[5];
+                                const double sx = (y[0] * y[0] + y[1] * y[1]) + y[2] * y[2];
+                                double sv = (y[3] * y[3] + y[4] * y[4]) + y[5] * y[5];
+                                const double vc2 = p.mu / sqrt(sx);
+                                if (sv < vc2) sv = vc2;
+                                e2 = fmax(ex / sx, ev / sv);
+                                if (!(e2 == e2)) e2 = INFINITY;
+                            }
+#pragma unroll
+                            for (int o = 16; o > 0; o >>= 1) e2 = fmax(e2, __shfl_xor_sync(0xffffffffu, e2, o));
+                            if (e2 <= tol2) { accepted = true; cols = c; }
+                        }
+                    }
+                }
+                if (accepted && act) {
+#pragma unroll
+                    for (int k = 0; k < 6; ++k) ycur[k][lane] = T[cols - 1][k];
+                }
+                if (lane == 0) {
+                    if (underflow) {
+                        ctrl_done = 2;
+                    } else if (accepted) {
+                        const double tn = (fabs(p.dt - (tcur + h)) <= 1e-15 * fabs(p.dt)) ? p.dt : tcur + h;
+                        ctrl_t = tn;
+                        ctrl_h = cols <= 6 ? h * 1.3 : (cols == 8 ? h * 0.55 : h);
+                        if (tn == p.dt) ctrl_done = 1;
+                    } else {
+                        ctrl_h = h * 0.5;
+                    }
+                }
+            }
+            __syncthreads();
+        }
+        if (w == 0) {
+            if (ctrl_done == 2) {
+                if (lane == 0) status_add(p.status, ST_BS_FAIL, 1);  // group left unchanged
+            } else if (act) {
+#pragma unroll
+                for (int c = 0; c < 3; ++c) { p.x[3 * (size_t)b + c] = ycur[c][lane]; p.v[3 * (size_t)b + c] = ycur[3 + c][lane]; }
+            }
         }
     }
 }

@@ -427,8 +427,8 @@ void enqueue_groups(const Workspace &w, const int32_t *pairs, const int64_t *npa
     nb_grp_giant_kernel<<<sm_count(), kGrpScanBlock, 0, stream()>>>(w.grp, label, n, members);
 }
 
-// H_A with encounters for the listed groups (encounter.cuh): groups of up to 32 members by CTAs of one warp,
-// up to kMaxGroup members by CTAs of kMaxGroup threads
+// H_A with encounters for the listed groups (encounter.cuh): groups of up to 32 members by CTAs of 8 warps (one per
+// extrapolation column), up to kMaxGroup members by CTAs of kMaxGroup threads (one thread per member)
 void enqueue_encounter(const Workspace &w, double *x, double *v, const double *m, const double *rcrit, double M_star,
                        int64_t N, double dt, const int32_t *members, const int32_t *gstart, const int64_t *gstat) {
     EncParams ep;
@@ -436,10 +436,10 @@ void enqueue_encounter(const Workspace &w, double *x, double *v, const double *m
     ep.gstat = reinterpret_cast<const long long *>(gstat); ep.status = w.status; ep.mu = g_cfg.G * M_star; ep.G = g_cfg.G;
     ep.dt = dt; ep.tol = g_cfg.bs_tol > 0.0 ? g_cfg.bs_tol : 1e-12; ep.kind = g_cfg.changeover_kind;
     long long small_blocks = N / 2 + 1;
-    const long long cap_blocks = (long long)sm_count() * 32;
+    const long long cap_blocks = (long long)sm_count() * 8;
     if (small_blocks > cap_blocks) small_blocks = cap_blocks;
     ep.min_size = 2; ep.max_size = 32;
-    nb_encounter_kernel<32><<<(unsigned)small_blocks, 32, (5 * 32 + 32) * sizeof(double), stream()>>>(ep);
+    nb_encounter_small_kernel<<<(unsigned)small_blocks, 32 * kBsCols, 0, stream()>>>(ep);
     ep.min_size = 33; ep.max_size = kMaxGroup;
     static bool attr_set = false;
     const size_t big_smem = (5 * (size_t)kMaxGroup + 32) * sizeof(double);
