@@ -237,11 +237,12 @@ def encounter(x, v, m, rcrit_, M_star, dt, G, grp, kind=0, tol=1e-12, max_group=
     return x, v, dict(integrated=int(stats[0]), skipped=int(stats[1]), failed=int(stats[2]), steps=int(stats[3]))
 
 
-def step_enc(x, v, m, M_star, dt, G, nsteps, n1=3.0, n2=0.4, kind=0, tol=1e-12, max_group=1024):
+def step_enc(x, v, m, M_star, dt, G, nsteps, n1=3.0, n2=0.4, kind=0, tol=1e-12, max_group=1024, n_active=0):
     """nsteps of B(dt/2) C(dt/2) A(dt) C(dt/2) B(dt/2) with close encounters resolved:
     in A the members of the encounter groups of the step's opening pair list (groups of at most max_group
     bodies) are propagated by encounter(), every other body by the Kepler drift.  Composed of the pinned
-    pieces above; rcrit is recomputed before every force evaluation (S17) and held through the step.
+    pieces above; rcrit is recomputed before every force evaluation (S17) and held through the step.  With
+    n_active (semi-active mode) only the first n_active bodies exert force and every pair has an active member.
     Returns dict(x, v, acc, rcrit, pairs, stats)."""
     x = np.array(x, dtype=np.float64, order="C"); v = np.array(v, dtype=np.float64, order="C")
     m = np.ascontiguousarray(m, dtype=np.float64)
@@ -250,8 +251,8 @@ def step_enc(x, v, m, M_star, dt, G, nsteps, n1=3.0, n2=0.4, kind=0, tol=1e-12, 
 
     def evaluate(x, v):
         rc = rcrit(x, v, m, M_star, dt, G, n1, n2)
-        acc, _, _ = accel(x, m, rc, G, kind=kind)
-        sure, border = pairs(x, rc)
+        acc, _, _ = accel(x, m, rc, G, n_active=n_active, kind=kind)
+        sure, border = pairs(x, rc, n_active=n_active)
         tot["border"] += border.shape[0]
         return rc, acc, sure
 

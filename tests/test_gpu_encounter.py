@@ -169,3 +169,25 @@ def test_step_with_encounters_is_bitwise_reproducible():
         out.append((xg.copy(), vg.copy(), ag.copy(), {tuple(p) for p in gp.tolist()}))
     assert np.array_equal(out[0][0], out[1][0]) and np.array_equal(out[0][1], out[1][1])
     assert np.array_equal(out[0][2], out[1][2]) and out[0][3] == out[1][3]
+
+
+def test_step_with_encounters_semi_active():
+    """Semi-active mode with encounters resolved: test-mass planetesimals that meet an embryo join its group (they
+    feel the [1 - W] part of the embryo's pull in the direct solver, and exert nothing)."""
+    d = nb_inputs.make_config(3, n_override=3000)
+    assert 0 < d.n_active < d.N
+    st = GpuState(d.x, d.v, d.m, d.M_star, G=G_GAUSS, n_active=d.n_active, n1=3.0, n2=0.4, resolve_encounters=True,
+                  pair_capacity=1 << 16)
+    st.step(d.dt, 10)
+    xg, vg, ag, rcg = st.host()
+    ref = oracle.step_enc(d.x, d.v, d.m, d.M_star, d.dt, G_GAUSS, 10, n1=3.0, n2=0.4, n_active=d.n_active)
+    assert ref["stats"]["integrated"] > 0 and ref["stats"]["border"] == 0
+    status = st.nb.nb_status()
+    assert status["bs_fail"] == 0 and status["kepler_fail"] == 0 and status["groups_skipped"] == ref["stats"]["skipped"]
+    ex = np.max(np.abs(xg - ref["x"])) / np.max(np.abs(ref["x"]))
+    ev = np.max(np.abs(vg - ref["v"])) / np.max(np.abs(ref["v"]))
+    print(f"semi-active step_enc x10: groups integrated {ref['stats']['integrated']}, rel dx {ex:.2e} dv {ev:.2e}")
+    assert ex <= 1e-9 and ev <= 1e-9
+    sure, border = oracle.pairs(xg, rcg, n_active=d.n_active)
+    gp, n = st.get_pairs()
+    assert_pairs_match(gp, n, sure, border, "semi-active step_enc")
