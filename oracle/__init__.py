@@ -276,3 +276,50 @@ def step_enc(x, v, m, M_star, dt, G, nsteps, n1=3.0, n2=0.4, kind=0, tol=1e-12, 
         rc, acc, pr = evaluate(x, v)
         v = v + (0.5 * dt) * acc
     return dict(x=x, v=v, acc=acc, rcrit=rc, pairs=pr, stats=tot)
+
+
+def merge(x, v, m, radius, pairs_, f=1.0):
+    """Perfect merging ("N-body simulations often treat collisions as perfect mergers"; PAPER.md:168:
+    radii may be inflated by a constant factor f).  DESIGN.md reading S21:
+      * two bodies of a listed pair collide iff r_ij < f (R_i + R_j) (strict, decided in fp64 on r^2);
+      * colliding bodies that are linked by a chain of collisions merge into ONE body, the one with the smallest
+        index: m <- sum m_k, x <- sum m_k x_k / sum m_k, v <- sum m_k v_k / sum m_k (mass and momentum of the
+        democratic coordinates conserved; members in index order), R <- (sum R_k^3)^(1/3) (volume conserved);
+        if all masses are zero the survivor keeps its x, v;
+      * every other member is removed; the arrays are then compacted in index order (a stable partition, so a
+        semi-active ordering survives).
+    Returns dict(x, v, m, radius, N, alive[N_old] bool, survivor_of[N_old] int32 (label of the merged body, own
+    index for untouched bodies), n_collisions (colliding pair rows), n_merged (bodies removed))."""
+    x = np.array(x, dtype=np.float64, order="C"); v = np.array(v, dtype=np.float64, order="C")
+    m = np.array(m, dtype=np.float64); R = np.array(radius, dtype=np.float64)
+    N = m.shape[0]
+    p = np.asarray(pairs_, dtype=np.int32).reshape(-1, 2)
+    hits = []
+    for i, j in p:
+        dx = x[j] - x[i]
+        r2 = (dx[0] * dx[0] + dx[1] * dx[1]) + dx[2] * dx[2]
+        s = f * (R[i] + R[j])
+        if r2 < s * s:
+            hits.append((i, j))
+    hits = np.array(hits, dtype=np.int32).reshape(-1, 2)
+    g = groups(hits, N)
+    alive = np.ones(N, dtype=bool)
+    for k in range(g["ngroups"]):
+        seg = g["members"][g["gstart"][k]:g["gstart"][k + 1]]
+        s = int(seg[0])
+        mt = 0.0; mx = np.zeros(3); mv = np.zeros(3); vol = 0.0
+        for b in seg:                      # index order
+            mt = mt + m[b]
+            mx = mx + m[b] * x[b]
+            mv = mv + m[b] * v[b]
+            vol = vol + R[b] * R[b] * R[b]
+        if mt > 0.0:
+            x[s] = mx / mt
+            v[s] = mv / mt
+        m[s] = mt
+        R[s] = np.cbrt(vol)
+        alive[seg[1:]] = False
+    keep = np.flatnonzero(alive)
+    return dict(x=x[keep].copy(), v=v[keep].copy(), m=m[keep].copy(), radius=R[keep].copy(), N=int(keep.shape[0]),
+                alive=alive, survivor_of=g["label"].copy(), n_collisions=int(hits.shape[0]),
+                n_merged=int(N - keep.shape[0]))
