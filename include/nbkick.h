@@ -90,6 +90,7 @@ typedef struct nb_config {
                                 propagated through A(dt) by the direct solver (nb_encounter) instead of the Kepler
                                 drift; needs pairs != NULL (default 0: pure Kepler drift) */
     double bs_tol;           /* relative tolerance of the direct solver's Bulirsch-Stoer steps (default 1e-12) */
+    double radius_factor;    /* nb_merge: factor f by which the physical radii are inflated (default 1) */
 } nb_config;
 
 void nb_default_config(nb_config *cfg);
@@ -192,6 +193,25 @@ int nb_groups(const int32_t *pairs, const int64_t *npairs, int64_t N, int32_t *l
 #define NB_MAX_GROUP 1024
 int nb_encounter(double *x, double *v, const double *m, const double *rcrit, double M_star, int64_t N,
                  double dt, const int32_t *members, const int32_t *gstart, const int64_t *gstat);
+
+/*
+ * Perfect merging ("N-body simulations often treat collisions as perfect mergers";
+ * PAPER.md:168 radii inflated by a constant factor f = radius_factor; reading S21).  For every
+ * row (i, j) of the pair list (as nb_kick / nb_step wrote it for the CURRENT positions) the bodies collide
+ * iff r_ij < f (R_i + R_j) (strict, fp64 on r^2).  Bodies linked by a chain of collisions merge into the one
+ * with the smallest index: m <- sum m_k, x <- sum m_k x_k / sum m_k, v <- sum m_k v_k / sum m_k (members
+ * in index order; mass and momentum conserved), R <- cbrt(sum R_k^3); if all masses are zero the survivor
+ * keeps its x, v.  The other members are removed and x, v, m, radius are compacted in index order (stable:
+ * a semi-active ordering survives); rows past the new N are undefined.
+ *   x, v [N,3], m, radius [N] in/out; pairs / npairs in (device, as in nb_groups);
+ *   survivor_of [N] int32 out: index (before compaction) of the body each body ended up in (itself if untouched);
+ *   mstat device int64[4] out: new N, colliding pair rows, bodies removed, new n_active (alive among the
+ *   first n_active; = new N when n_active is 0).
+ * acc, rcrit and the pair list refer to the old indexing afterwards: re-evaluate (nb_kick / nb_step with
+ * reuse_acc = 0) with the new N, and re-issue nb_configure if n_active changed.  Needs nb_workspace_bytes(N).
+ */
+int nb_merge(double *x, double *v, double *m, double *radius, int64_t N, const int32_t *pairs,
+             const int64_t *npairs, int32_t *survivor_of, int64_t *mstat);
 
 /*
  * Host-buffer forms of nb_kick and nb_step: same semantics, every pointer is a HOST pointer

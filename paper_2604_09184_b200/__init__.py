@@ -7,5 +7,5 @@ its thin Python binding.  No CPU fallback exists: the calls raise if the library
 from . import build  # noqa: F401
 from .binding import *  # noqa: F401,F403
 from .binding import (NbConfig, NbError, SYMBOLS, configure, default_config, force_geometry, lib_path, load,  # noqa: F401
-                      nb_drift_kepler, nb_encounter, nb_fp64_peak, nb_groups, nb_kick, nb_kick_host, nb_force_time, nb_force_time_reset, nb_last_force_ms, nb_rcrit, set_flags, nb_release,
+                      nb_drift_kepler, nb_encounter, nb_fp64_peak, nb_groups, nb_kick, nb_merge, nb_kick_host, nb_force_time, nb_force_time_reset, nb_last_force_ms, nb_rcrit, set_flags, nb_release,
                       nb_shift, nb_status, nb_status_reset, nb_step, nb_step_host, nb_version, workspace_bytes)

@@ -22,7 +22,7 @@ FORCE_AUTO, FORCE_TILES, FORCE_SYMMETRIC = 0, 1, 2
 # every symbol include/nbkick.h declares (tests check the library exports each of them)
 SYMBOLS = (
     "nb_default_config", "nb_configure", "nb_workspace_bytes", "nb_rcrit", "nb_kick", "nb_shift",
-    "nb_drift_kepler", "nb_step", "nb_groups", "nb_encounter", "nb_kick_host", "nb_step_host", "nb_status", "nb_status_reset",
+    "nb_drift_kepler", "nb_step", "nb_groups", "nb_encounter", "nb_merge", "nb_kick_host", "nb_step_host", "nb_status", "nb_status_reset",
     "nb_last_force_ms", "nb_force_time", "nb_force_time_reset", "nb_force_geometry", "nb_fp64_peak", "nb_release", "nb_last_error", "nb_version",
 )
 
@@ -49,6 +49,7 @@ class NbConfig(C.Structure):
         ("sym_block", C.c_int),
         ("resolve_encounters", C.c_int),
         ("bs_tol", C.c_double),
+        ("radius_factor", C.c_double),
     ]
 
 
@@ -88,6 +89,7 @@ def load():
     lib.nb_step.argtypes = [vp, vp, vp, dbl, i64, dbl, vp, vp, vp, vp, i64]
     lib.nb_groups.argtypes = [vp, vp, i64, vp, vp, vp, vp]
     lib.nb_encounter.argtypes = [vp, vp, vp, vp, dbl, i64, dbl, vp, vp, vp]
+    lib.nb_merge.argtypes = [vp, vp, vp, vp, i64, vp, vp, vp, vp]
     lib.nb_kick_host.argtypes = [vp, vp, vp, dbl, i64, dbl, vp, vp, vp, vp]
     lib.nb_step_host.argtypes = [vp, vp, vp, dbl, i64, dbl, vp, vp, vp, vp, i64]
     lib.nb_status.argtypes = [C.POINTER(C.c_int64)]
@@ -155,7 +157,7 @@ def default_config() -> NbConfig:
 
 def configure(N=None, *, stream=None, pair_capacity=0, n_active=0, G=None, n1=3.0, n2=0.4, changeover_kind=0,
               i_per_thread=0, j_splits=0, use_graph=True, reuse_acc=False, time_force=False, ctas_per_sm=0,
-              pipeline_j=0, force_kernel=0, sym_block=0, resolve_encounters=False, bs_tol=1e-12, workspace_bytes=None,
+              pipeline_j=0, force_kernel=0, sym_block=0, resolve_encounters=False, bs_tol=1e-12, radius_factor=1.0, workspace_bytes=None,
               device="cuda"):
     """nb_configure with a torch-allocated workspace sized for N bodies (N=None: no workspace,
     enough for the _host calls; workspace_bytes: explicit size, e.g. the head that the O(N) calls
@@ -175,6 +177,7 @@ def configure(N=None, *, stream=None, pair_capacity=0, n_active=0, G=None, n1=3.
     cfg.ctas_per_sm, cfg.pipeline_j = int(ctas_per_sm), int(pipeline_j)
     cfg.force_kernel, cfg.sym_block = int(force_kernel), int(sym_block)
     cfg.resolve_encounters, cfg.bs_tol = (1 if resolve_encounters else 0), float(bs_tol)
+    cfg.radius_factor = float(radius_factor)
     if N is not None:
         import torch
         if stream is None:
@@ -255,6 +258,14 @@ def nb_encounter(x, v, m, rcrit, M_star, dt, members, gstart, gstat):
     _check(load().nb_encounter(_dev(x, 3 * N, torch.float64), _dev(v, 3 * N, torch.float64), _dev(m, N, torch.float64),
                                _dev(rcrit, N, torch.float64), float(M_star), N, float(dt), _dev(members, N, torch.int32),
                                _dev(gstart, N // 2 + 2, torch.int32), _dev(gstat, 4, torch.int64)))
+
+
+def nb_merge(x, v, m, radius, pairs, npairs, survivor_of, mstat):
+    import torch
+    N = m.numel()
+    _check(load().nb_merge(_dev(x, 3 * N, torch.float64), _dev(v, 3 * N, torch.float64), _dev(m, N, torch.float64),
+                           _dev(radius, N, torch.float64), N, _dev(pairs, None, torch.int32), _dev(npairs, 1, torch.int64),
+                           _dev(survivor_of, N, torch.int32), _dev(mstat, 4, torch.int64)))
 
 
 def nb_kick_host(x, v, m, M_star, dt, rcrit, acc, pairs=None, npairs=None):

@@ -54,10 +54,19 @@ __global__ void __launch_bounds__(kGrpThreads) nb_grp_init_kernel(GroupScratch s
     if (i == 0) *s.ngiant = 0;
 }
 
+// Optional edge filter of the hooking kernel (merge.cuh): an edge counts only if the two bodies are in
+// contact, r_ij < f (R_i + R_j); x == nullptr: every row is an edge.
+struct GroupFilter {
+    const double *x;       // [N,3] or nullptr
+    const double *radius;  // [N]
+    double f;
+    long long *nhit;       // rows that passed the filter
+};
+
 __global__ void __launch_bounds__(kGrpThreads) nb_grp_hook_kernel(GroupScratch s, const int2 *__restrict__ pairs,
                                                                  const long long *__restrict__ npairs, long long cap,
                                                                  int N, long long *__restrict__ gstat,
-                                                                 long long *__restrict__ status) {
+                                                                 long long *__restrict__ status, const GroupFilter flt) {
     long long n = *npairs;
     if (n > cap) n = cap;
     if (n < 0) n = 0;
@@ -66,6 +75,15 @@ __global__ void __launch_bounds__(kGrpThreads) nb_grp_hook_kernel(GroupScratch s
     for (long long e = (long long)blockIdx.x * kGrpThreads + threadIdx.x; e < n; e += (long long)gridDim.x * kGrpThreads) {
         const int2 ab = pairs[e];
         if (ab.x < 0 || ab.y < 0 || ab.x >= N || ab.y >= N || ab.x == ab.y) { status_add(status, ST_NONFINITE, 1); continue; }
+        if (flt.x != nullptr) {
+            const double dx = flt.x[3 * (size_t)ab.y] - flt.x[3 * (size_t)ab.x];
+            const double dy = flt.x[3 * (size_t)ab.y + 1] - flt.x[3 * (size_t)ab.x + 1];
+            const double dz = flt.x[3 * (size_t)ab.y + 2] - flt.x[3 * (size_t)ab.x + 2];
+            const double r2 = __dadd_rn(__dadd_rn(__dmul_rn(dx, dx), __dmul_rn(dy, dy)), __dmul_rn(dz, dz));
+            const double sr = flt.f * (flt.radius[ab.x] + flt.radius[ab.y]);
+            if (!(r2 < sr * sr)) continue;
+            atomicAdd(reinterpret_cast<unsigned long long *>(flt.nhit), 1ull);
+        }
         int ra = ab.x, rb = ab.y;
         while (true) {
             ra = grp_find(parent, ra);

@@ -15,13 +15,14 @@
 #include "force_sym.cuh"
 #include "force_tiles.cuh"
 #include "groups.cuh"
+#include "merge.cuh"
 
 namespace {
 
 using namespace nbk;
 
 std::mutex g_mu;
-nb_config g_cfg = {nullptr, nullptr, 0, 0, 0, 0.01720209895 * 0.01720209895, 3.0, 0.4, 0, 0, 0, 1, 0, 0, 0, 0, 0, 0, 0, 1e-12};
+nb_config g_cfg = {nullptr, nullptr, 0, 0, 0, 0.01720209895 * 0.01720209895, 3.0, 0.4, 0, 0, 0, 1, 0, 0, 0, 0, 0, 0, 0, 1e-12, 1.0};
 char g_err[512] = "";
 int g_sm_count = 0;
 cudaEvent_t g_ev0 = nullptr, g_ev1 = nullptr;
@@ -231,7 +232,11 @@ Workspace carve(void *base, int64_t N, const Geometry &g) {
     w.sxy = reinterpret_cast<double2 *>(b + off); off += align_up((size_t)2 * g.Npad_sym * sizeof(double2), 256);
     w.szg = reinterpret_cast<double2 *>(b + off); off += align_up((size_t)2 * g.Npad_sym * sizeof(double2), 256);
     w.sthr = reinterpret_cast<int *>(b + off); off += align_up((size_t)2 * g.Npad_sym * sizeof(int), 256);
-    w.part = reinterpret_cast<double *>(b + off); off += align_up((size_t)g.nsplit * (size_t)N * 3 * sizeof(double), 256);
+    {   // partial accelerations; never smaller than 64 bytes per body (nb_merge's compaction buffer)
+        size_t pb = (size_t)g.nsplit * (size_t)N * 3 * sizeof(double);
+        if (pb < (size_t)N * 64) pb = (size_t)N * 64;
+        w.part = reinterpret_cast<double *>(b + off); off += align_up(pb, 256);
+    }
     w.bytes = off;
     return w;
 }
@@ -406,7 +411,7 @@ void drop_graph() {
 
 // the nine launches of nb_groups (groups.cuh)
 void enqueue_groups(const Workspace &w, const int32_t *pairs, const int64_t *npairs, int64_t N, int32_t *label,
-                    int32_t *members, int32_t *gstart, int64_t *gstat) {
+                    int32_t *members, int32_t *gstart, int64_t *gstat, const GroupFilter flt = GroupFilter{nullptr, nullptr, 1.0, nullptr}) {
     const int n = (int)N;
     const int nb256 = (n + kGrpThreads - 1) / kGrpThreads, nb1024 = (n + kGrpScanBlock - 1) / kGrpScanBlock;
     long long *gs = reinterpret_cast<long long *>(gstat);
@@ -417,7 +422,7 @@ void enqueue_groups(const Workspace &w, const int32_t *pairs, const int64_t *npa
     nb_grp_init_kernel<<<nb256, kGrpThreads, 0, stream()>>>(w.grp, label, members, gstart, gs, n);
     nb_grp_hook_kernel<<<(unsigned)hook_blocks, kGrpThreads, 0, stream()>>>(w.grp, reinterpret_cast<const int2 *>(pairs),
                                                                             reinterpret_cast<const long long *>(npairs), cap, n, gs,
-                                                                            w.status);
+                                                                            w.status, flt);
     nb_grp_compress_kernel<<<nb256, kGrpThreads, 0, stream()>>>(w.grp, label, n);
     nb_grp_blocksum_kernel<<<nb1024, kGrpScanBlock, 0, stream()>>>(w.grp, label, n);
     nb_grp_topscan_kernel<<<1, kGrpScanBlock, 0, stream()>>>(w.grp, nb1024, gstart, gs);
@@ -580,6 +585,7 @@ void nb_default_config(nb_config *cfg) {
     cfg->sym_block = 0;
     cfg->resolve_encounters = 0;
     cfg->bs_tol = 1e-12;
+    cfg->radius_factor = 1.0;
 }
 
 int nb_configure(const nb_config *cfg) {
@@ -600,6 +606,7 @@ int nb_configure(const nb_config *cfg) {
     if (cfg->sym_block != 0 && cfg->sym_block != 256 && cfg->sym_block != 512 && cfg->sym_block != 1024 && cfg->sym_block != 2048)
         return fail(NB_E_BADARG, "sym_block must be 0, 256, 512, 1024 or 2048");
     if (!(cfg->bs_tol >= 0.0) || !std::isfinite(cfg->bs_tol)) return fail(NB_E_BADARG, "bs_tol must be finite and >= 0");
+    if (!(cfg->radius_factor >= 0.0) || !std::isfinite(cfg->radius_factor)) return fail(NB_E_BADARG, "radius_factor must be finite and >= 0");
     g_cfg = *cfg;
     return NB_OK;
 }
@@ -680,6 +687,38 @@ int nb_groups(const int32_t *pairs, const int64_t *npairs, int64_t N, int32_t *l
     int rc = check_workspace_head(N, 2, &w);
     if (rc) return rc;
     enqueue_groups(w, pairs, npairs, N, label, members, gstart, gstat);
+    NB_CUDA(cudaGetLastError());
+    return NB_OK;
+}
+
+int nb_merge(double *x, double *v, double *m, double *radius, int64_t N, const int32_t *pairs, const int64_t *npairs,
+             int32_t *survivor_of, int64_t *mstat) {
+    std::lock_guard<std::mutex> lk(g_mu);
+    if (N <= 0 || N > 2147483647LL) return fail(NB_E_BADN, "N = %lld out of range (1 .. 2^31-1)", (long long)N);
+    if (!x || !v || !m || !radius || !pairs || !npairs || !survivor_of || !mstat) return fail(NB_E_NULL, "nb_merge: NULL argument");
+    if (g_cfg.pair_capacity <= 0) return fail(NB_E_BADARG, "nb_merge: pair_capacity is 0 (nb_configure)");
+    if (g_cfg.n_active > N) return fail(NB_E_BADARG, "n_active = %lld > N = %lld", (long long)g_cfg.n_active, (long long)N);
+    const Geometry g = geometry(N, g_cfg.n_active);
+    Workspace w;
+    int rc = check_workspace(N, g, &w);  // the partial-sum area doubles as the compaction buffer (64 bytes per body)
+    if (rc) return rc;
+    const int n = (int)N;
+    const int nb256 = (n + kGrpThreads - 1) / kGrpThreads, nb1024 = (n + kGrpScanBlock - 1) / kGrpScanBlock;
+    long long *ms = reinterpret_cast<long long *>(mstat);
+    long long *ncoll = reinterpret_cast<long long *>(w.npairs_dummy) + 8;   // spare words of the 256-byte slot
+    NB_CUDA(cudaMemsetAsync(ncoll, 0, sizeof(long long), stream()));
+    GroupFilter flt{x, radius, g_cfg.radius_factor > 0.0 ? g_cfg.radius_factor : 1.0, ncoll};
+    enqueue_groups(w, pairs, npairs, N, survivor_of, w.g_members, w.g_start, w.g_stat, flt);
+    int *alive = w.grp.cursor;                                              // free again after the member lists are built
+    nb_mrg_alive_init_kernel<<<nb256, kGrpThreads, 0, stream()>>>(alive, n);
+    nb_mrg_merge_kernel<<<(n / 2 + kGrpThreads) / kGrpThreads, kGrpThreads, 0, stream()>>>(
+        x, v, m, radius, w.g_members, w.g_start, reinterpret_cast<const long long *>(w.g_stat), alive);
+    const int na = (int)((g_cfg.n_active > 0 && g_cfg.n_active < N) ? g_cfg.n_active : N);
+    nb_mrg_blocksum_kernel<<<nb1024, kGrpScanBlock, 0, stream()>>>(alive, n, na, w.grp.bsum);
+    nb_mrg_topscan_kernel<<<1, kGrpScanBlock, 0, stream()>>>(w.grp.bsum, nb1024, n, reinterpret_cast<const long long *>(w.g_stat),
+                                                             ncoll, ms);
+    nb_mrg_scatter_kernel<<<nb1024, kGrpScanBlock, 0, stream()>>>(x, v, m, radius, alive, w.grp.bsum, n, w.part);
+    nb_mrg_copyback_kernel<<<nb256, kGrpThreads, 0, stream()>>>(x, v, m, radius, w.part, ms);
     NB_CUDA(cudaGetLastError());
     return NB_OK;
 }
