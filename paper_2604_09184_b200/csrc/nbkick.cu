@@ -433,7 +433,8 @@ void enqueue_groups(const Workspace &w, const int32_t *pairs, const int64_t *npa
 }
 
 // H_A with encounters for the listed groups (encounter.cuh): groups of up to 32 members by CTAs of 8 warps (one per
-// extrapolation column), up to kMaxGroup members by CTAs of kMaxGroup threads (one thread per member)
+// extrapolation column), 33 .. 128 members by CTAs of 128 threads, up to kMaxGroup members by CTAs of kMaxGroup threads
+// (one thread per member, columns in sequence)
 void enqueue_encounter(const Workspace &w, double *x, double *v, const double *m, const double *rcrit, double M_star,
                        int64_t N, double dt, const int32_t *members, const int32_t *gstart, const int64_t *gstat) {
     EncParams ep;
@@ -445,11 +446,16 @@ void enqueue_encounter(const Workspace &w, double *x, double *v, const double *m
     if (small_blocks > cap_blocks) small_blocks = cap_blocks;
     ep.min_size = 2; ep.max_size = 32;
     nb_encounter_small_kernel<<<(unsigned)small_blocks, 32 * kBsCols, 0, stream()>>>(ep);
-    ep.min_size = 33; ep.max_size = kMaxGroup;
+    // mid-size groups: CTAs of 128 threads (no register cap: the 1024-thread variant is held to 64 registers and spills)
+    ep.min_size = 33; ep.max_size = 128;
+    long long mid_blocks = N / 33 + 1;
+    if (mid_blocks > 8LL * sm_count()) mid_blocks = 8LL * sm_count();
+    nb_encounter_kernel<128><<<(unsigned)mid_blocks, 128, (5 * 128 + 32) * sizeof(double), stream()>>>(ep);
+    ep.min_size = 129; ep.max_size = kMaxGroup;
     static bool attr_set = false;
     const size_t big_smem = (5 * (size_t)kMaxGroup + 32) * sizeof(double);
     if (!attr_set) { cudaFuncSetAttribute(nb_encounter_kernel<kMaxGroup>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)big_smem); attr_set = true; }
-    long long big_blocks = N / 33 + 1;
+    long long big_blocks = N / 129 + 1;
     if (big_blocks > 2LL * sm_count()) big_blocks = 2LL * sm_count();
     nb_encounter_kernel<kMaxGroup><<<(unsigned)big_blocks, kMaxGroup, big_smem, stream()>>>(ep);
 }
