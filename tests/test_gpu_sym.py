@@ -132,3 +132,50 @@ def test_sym_step_matches_oracle(nsteps):
     Dg = oracle.diagnostics(xg, vg, d.m, d.M_star, G_GAUSS)
     Dr = oracle.diagnostics(ref["x"], ref["v"], d.m, d.M_star, G_GAUSS)
     assert abs((Dg["E"] - D0["E"]) / D0["E"] - (Dr["E"] - D0["E"]) / D0["E"]) <= 1e-9
+
+
+def test_sym_pair_overflow_counts_and_null_pairs():
+    N = 900
+    x, v, m = nb_inputs.random_cluster(N, seed=11, scale=0.1)
+    rc = np.full(N, 0.05)
+    sure, border = oracle.pairs(x, rc)
+    acc_ref, ab, _ = oracle.accel(x, m, rc, G_GAUSS, want_abs=True)
+    st = GpuState(x, v, m, G=G_GAUSS, pair_capacity=100, force_kernel=SYM, sym_block=256, i_per_thread=2)
+    st.set_rcrit(rc)
+    st.kick(0.0, with_pairs=False)                       # pairs = NULL: detection skipped, weights still applied
+    assert_acc_close(st.acc.cpu().numpy(), acc_ref, "sym pairs=NULL", ab)
+    st.kick(0.0, with_pairs=True)
+    gp, n = st.get_pairs()
+    assert sure.shape[0] <= n <= sure.shape[0] + border.shape[0] and n > 100
+    assert gp.shape[0] == 100 and st.nb.nb_status()["pairs_dropped"] == n - 100
+    assert_acc_close(st.acc.cpu().numpy(), acc_ref, "sym overflow", ab)
+    allowed = {tuple(p) for p in np.concatenate([sure, border]).tolist()}
+    assert all(tuple(p) in allowed for p in gp.tolist())
+
+
+def test_sym_everything_in_the_exact_path_at_larger_n():
+    """rc larger than the cluster: every one of the N(N-1)/2 pairs goes through the deferred exact pass."""
+    N = 1500
+    x, v, m = nb_inputs.random_cluster(N, seed=23, scale=0.05)
+    info = _kick_case(x, v, m, np.full(N, 10.0), force_kernel=SYM, sym_block=512, i_per_thread=4,
+                      pair_capacity=1 << 21, what="sym all pairs N=1500")
+    assert info["n_gpu"] == N * (N - 1) // 2
+
+
+def test_auto_selection_threshold():
+    import paper_2604_09184_b200 as nb
+    for N, want_sym in ((12287, False), (12288, True)):
+        nb.configure(N, G=G_GAUSS)
+        assert (nb.force_geometry(N).tile_j < 0) == want_sym
+    d = nb_inputs.make_config(1, n_override=12300)       # just above the threshold, ragged: N = 12302
+    rc = oracle.rcrit(d.x, d.v, d.m, d.M_star, d.dt, G_GAUSS, 3.0, 0.4)
+    rows = np.unique(np.concatenate([np.arange(0, d.N, 97), [d.N - 1, d.N - 2]]))
+    st = GpuState(d.x, d.v, d.m, d.M_star, G=G_GAUSS, pair_capacity=1 << 20)
+    assert _geometry_is_symmetric(d.N)
+    st.set_rcrit(rc)
+    st.kick(0.0)
+    acc_ref, ab, _ = oracle.accel(d.x, d.m, rc, G_GAUSS, rows=rows, want_abs=True)
+    assert_acc_close(st.acc.cpu().numpy()[rows], acc_ref, "auto sym N=12302 sampled rows", ab)
+    sure, border = oracle.pairs(d.x, rc)
+    gp, n = st.get_pairs()
+    assert_pairs_match(gp, n, sure, border, "auto sym N=12302")
