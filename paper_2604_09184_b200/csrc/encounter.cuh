@@ -34,7 +34,7 @@ __device__ __forceinline__ void enc_accel(const double qx, const double qy, cons
     const double s = -mu * (ir * ir * ir);
     ax = s * qx; ay = s * qy; az = s * qz;
     for (int j = 0; j < n; ++j) {
-        if (j == self) continue;
+        if (j == self || sgm[j] == 0.0) continue;        // a massless member (semi-active mode) pulls on nobody
         const double dx = px[j] - qx, dy = py[j] - qy, dz = pz[j] - qz;
         const double d2 = (dx * dx + dy * dy) + dz * dz;
         const double rc = fmax(my_rc, src[j]);
