@@ -149,7 +149,7 @@ def cpu_baseline(d, na, budget_s=12.0):
     import oracle
     rng = np.random.default_rng(77)
     state = [d.x.copy(), d.v.copy()]
-    probe = np.sort(rng.choice(d.N, size=min(256, d.N), replace=False))
+    probe = np.sort(rng.choice(d.N, size=min(2048, d.N), replace=False))  # large enough that thread start-up does not bias the rate
     t, n = oracle_sample_step(d, na, probe, state)
     rate = n / t
     R = int(min(d.N, max(256, budget_s * rate / (na or d.N))))
