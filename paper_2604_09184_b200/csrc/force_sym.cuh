@@ -62,8 +62,8 @@ __host__ __device__ constexpr size_t sym_smem_bytes(int S) { return (size_t)S * 
 // contribution in (cx,cy,cz); emit[k] says whether pair k goes on the list.
 //   mixed: only the i side is kept by the caller and a pair is emitted from its i < j visit only.
 template <int I>
-__device__ __forceinline__ void sym_exact(const SymParams &p, const double2 xy, const double2 zg, const int j,
-                                          const bool mixed, const double (&xi)[I], const double (&yi)[I],
+__device__ __forceinline__ void sym_exact(const SymParams &p, const double2 xy, const double2 zg, const int thrj,
+                                          const int j, const bool mixed, const double (&xi)[I], const double (&yi)[I],
                                           const double (&zi)[I], const double (&ngi)[I], const int i0,
                                           double (&ax)[I], double (&ay)[I], double (&az)[I], double &cx, double &cy,
                                           double &cz, bool (&emit)[I]) {
@@ -76,6 +76,21 @@ __device__ __forceinline__ void sym_exact(const SymParams &p, const double2 xy, 
         if (!valid) continue;  // padding bodies have zero mass both ways; the self term is skipped
         const double dx = __dsub_rn(xy.x, xi[k]), dy = __dsub_rn(xy.y, yi[k]), dz = __dsub_rn(zg.x, zi[k]);
         const double r2 = __fma_rn(dz, dz, __fma_rn(dy, dy, __dmul_rn(dx, dx)));
+        // the body's own threshold word, reloaded from the staged array (kept out of the rotation loop's registers)
+        const int thr_i = p.sthr[(size_t)(i >> 5) * 64 + (i & 31)];
+        if (__double2hiint(r2) > max(thr_i, thrj)) {
+            // flagged only because a lane-mate (say a giant planet) has a large critical radius: this pair is out of
+            // reach, W = 1 -- same arithmetic as the rotation loop, no divide or square root
+            const double y0 = rsqrt_seed(r2);
+            const double u = __dmul_rn(y0, y0);
+            const double e = __fma_rn(-r2, u, 1.0);
+            const double q = __fma_rn(e, __fma_rn(e, 1.875, 1.5), 1.0);
+            const double b = __dmul_rn(__dmul_rn(u, y0), q);
+            const double si = __dmul_rn(b, zg.y), sj = __dmul_rn(b, ngi[k]);
+            ax[k] = __fma_rn(si, dx, ax[k]); ay[k] = __fma_rn(si, dy, ay[k]); az[k] = __fma_rn(si, dz, az[k]);
+            cx = __fma_rn(sj, dx, cx); cy = __fma_rn(sj, dy, cy); cz = __fma_rn(sj, dz, cz);
+            continue;
+        }
         const double rc = fmax(p.rcrit[i], rcj);
         const bool inside = r2 < rc * rc;
         if (r2 == 0.0) {
@@ -169,7 +184,7 @@ __device__ __forceinline__ void sym_block(const SymParams &p, const double2 *__r
 #pragma unroll
         for (int k = 0; k < I; ++k) emit[k] = false;
         if ((bits >> r) & 1u)
-            sym_exact<I>(p, lxy[r], lzg[r], jbase + src, mixed, xi, yi, zi, ngi, i0, ax, ay, az, cx, cy, cz, emit);
+            sym_exact<I>(p, lxy[r], lzg[r], lthr[r], jbase + src, mixed, xi, yi, zi, ngi, i0, ax, ay, az, cx, cy, cz, emit);
         if (PAIRS) {
 #pragma unroll
             for (int k = 0; k < I; ++k) pair_append(p.pairs, p.npairs, p.status, p.cap, emit[k], i0 + 32 * k, jbase + src);
