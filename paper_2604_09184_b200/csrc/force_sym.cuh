@@ -97,10 +97,8 @@ __device__ __forceinline__ void sym_exact(const SymParams &p, const double2 xy, 
             // rc == 0 and coincident: contributes 0; counted once per ordered interaction
             if (!inside) status_add(p.status, ST_SINGULAR, mixed ? 1 : 2);
         } else {
-            const double r = sqrt(r2);
-            const double W = inside ? changeover_weight(r, rc, p.kind) : 1.0;
-            if (W != 0.0) {
-                const double f = W / (r2 * r);
+            const double f = weighted_inv_r3(r2, rc, inside, p.kind);
+            if (f != 0.0) {
                 const double si = zg.y * f, sj = ngi[k] * f;
                 ax[k] = __fma_rn(si, dx, ax[k]); ay[k] = __fma_rn(si, dy, ay[k]); az[k] = __fma_rn(si, dz, az[k]);
                 cx = __fma_rn(sj, dx, cx); cy = __fma_rn(sj, dy, cy); cz = __fma_rn(sj, dz, cz);

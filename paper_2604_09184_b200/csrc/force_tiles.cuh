@@ -22,6 +22,7 @@
 // min_k hi32(r2_k) <= max(hi32(rc_i^2), hi32(rc_j^2)) + 1 is a conservative integer pre-filter; a
 // warp vote sends the (rare) hits, and every self term (r2 = 0), to the exact slow path.
 #pragma once
+#include "kepler.cuh"  // rcp_fast, rsqrt_fast, sqrt_from_rsqrt
 #include "nb_common.cuh"
 
 namespace nbk {
@@ -82,13 +83,22 @@ __device__ __forceinline__ double rsqrt_seed(double a) {
     return y;
 }
 
-// Kick weight W(r; rc) between the end points (readings S1, S2).
+// Kick weight W(r; rc) between the end points (readings S1, S2).  Reciprocals from the MUFU
+// seed with one third-order correction (~1 ulp, kepler.cuh): the exact path is not rare with the full Eq. 7 radius.
 __device__ __forceinline__ double changeover_weight(double r, double rc, int kind) {
-    const double y = (r - 0.1 * rc) / (0.9 * rc);
-    if (y <= 0.0) return 0.0;
+    const double t0 = r - 0.1 * rc;
+    if (t0 <= 0.0) return 0.0;
+    const double y = t0 * rcp_fast(0.9 * rc);
     if (y >= 1.0) return 1.0;
     if (kind == 1) return y * y * y * (10.0 + y * (-15.0 + 6.0 * y));
-    return (y * y) / (2.0 * y * y - 2.0 * y + 1.0);
+    return (y * y) * rcp_fast(2.0 * y * y - 2.0 * y + 1.0);
+}
+
+// W / r^3 for a pair inside rc (r2 > 0): no IEEE divide or square root
+__device__ __forceinline__ double weighted_inv_r3(const double r2, const double rc, const bool inside, const int kind) {
+    const double id = rsqrt_fast(r2);
+    const double W = inside ? changeover_weight(sqrt_from_rsqrt(r2, id), rc, kind) : 1.0;
+    return W * (id * id * id);
 }
 
 // Warp-aggregated append of encounter pairs (a3): one atomicAdd per warp-hit reserves the slots,
@@ -140,10 +150,9 @@ __device__ __forceinline__ void slow_path(const ForceParams &p, const double4 A,
             if (r2 == 0.0) {
                 if (!inside) status_add(p.status, ST_SINGULAR, 1);  // rc == 0 and coincident: contributes 0
             } else {
-                const double r = sqrt(r2);
-                const double W = inside ? changeover_weight(r, rc, p.kind) : 1.0;
-                if (W != 0.0) {
-                    const double f = A.w * W / (r2 * r);
+                const double wr3 = weighted_inv_r3(r2, rc, inside, p.kind);
+                if (wr3 != 0.0) {
+                    const double f = A.w * wr3;
                     ax[k] = __fma_rn(f, dx, ax[k]);
                     ay[k] = __fma_rn(f, dy, ay[k]);
                     az[k] = __fma_rn(f, dz, az[k]);
