@@ -78,33 +78,28 @@ __device__ __forceinline__ void sym_exact(const SymParams &p, const double2 xy, 
         const double r2 = __fma_rn(dz, dz, __fma_rn(dy, dy, __dmul_rn(dx, dx)));
         // the body's own threshold word, reloaded from the staged array (kept out of the rotation loop's registers)
         const int thr_i = p.sthr[(size_t)(i >> 5) * 64 + (i & 31)];
+        double f;  // W / r^3
         if (__double2hiint(r2) > max(thr_i, thrj)) {
             // flagged only because a lane-mate (say a giant planet) has a large critical radius: this pair is out of
-            // reach, W = 1 -- same arithmetic as the rotation loop, no divide or square root
+            // reach, W = 1 -- same arithmetic as the rotation loop
             const double y0 = rsqrt_seed(r2);
             const double u = __dmul_rn(y0, y0);
             const double e = __fma_rn(-r2, u, 1.0);
-            const double q = __fma_rn(e, __fma_rn(e, 1.875, 1.5), 1.0);
-            const double b = __dmul_rn(__dmul_rn(u, y0), q);
-            const double si = __dmul_rn(b, zg.y), sj = __dmul_rn(b, ngi[k]);
-            ax[k] = __fma_rn(si, dx, ax[k]); ay[k] = __fma_rn(si, dy, ay[k]); az[k] = __fma_rn(si, dz, az[k]);
-            cx = __fma_rn(sj, dx, cx); cy = __fma_rn(sj, dy, cy); cz = __fma_rn(sj, dz, cz);
-            continue;
-        }
-        const double rc = fmax(p.rcrit[i], rcj);
-        const bool inside = r2 < rc * rc;
-        if (r2 == 0.0) {
-            // rc == 0 and coincident: contributes 0; counted once per ordered interaction
-            if (!inside) status_add(p.status, ST_SINGULAR, mixed ? 1 : 2);
+            f = __dmul_rn(__dmul_rn(u, y0), __fma_rn(e, __fma_rn(e, 1.875, 1.5), 1.0));
         } else {
-            const double f = weighted_inv_r3(r2, rc, inside, p.kind);
-            if (f != 0.0) {
-                const double si = zg.y * f, sj = ngi[k] * f;
-                ax[k] = __fma_rn(si, dx, ax[k]); ay[k] = __fma_rn(si, dy, ay[k]); az[k] = __fma_rn(si, dz, az[k]);
-                cx = __fma_rn(sj, dx, cx); cy = __fma_rn(sj, dy, cy); cz = __fma_rn(sj, dz, cz);
+            const double rc = fmax(p.rcrit[i], rcj);
+            const bool inside = r2 < rc * rc;
+            emit[k] = inside && (!mixed || i < j);
+            if (r2 == 0.0) {
+                // rc == 0 and coincident: contributes 0; counted once per ordered interaction
+                if (!inside) status_add(p.status, ST_SINGULAR, mixed ? 1 : 2);
+                continue;
             }
+            f = weighted_inv_r3(r2, rc, inside, p.kind);
         }
-        emit[k] = inside && (!mixed || i < j);
+        const double si = zg.y * f, sj = ngi[k] * f;
+        ax[k] = __fma_rn(si, dx, ax[k]); ay[k] = __fma_rn(si, dy, ay[k]); az[k] = __fma_rn(si, dz, az[k]);
+        cx = __fma_rn(sj, dx, cx); cy = __fma_rn(sj, dy, cy); cz = __fma_rn(sj, dz, cz);
     }
 }
 
