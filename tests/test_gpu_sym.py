@@ -179,3 +179,23 @@ def test_auto_selection_threshold():
     sure, border = oracle.pairs(d.x, rc)
     gp, n = st.get_pairs()
     assert_pairs_match(gp, n, sure, border, "auto sym N=12302")
+
+
+@pytest.mark.parametrize("seed", range(16))
+def test_sym_randomized_shapes_against_oracle(seed):
+    """Random N, mass spectrum, clustering and critical radii (including zero radii, a few huge ones and test
+    particles): both force kernels against the oracle, same pair list from both."""
+    rng = np.random.default_rng(1000 + seed)
+    N = int(rng.integers(2, 1400))
+    scale = float(rng.choice([0.02, 0.2, 2.0]))
+    x, v, m = nb_inputs.random_cluster(N, seed=seed, scale=scale)
+    m = m * rng.choice([0.0, 1.0, 1.0, 30.0], size=N)            # test particles and a few heavy bodies
+    rc = rng.uniform(0.0, 0.08 * scale, N) * rng.choice([0.0, 1.0, 1.0, 1.0], size=N)
+    big = rng.choice(N, size=max(1, N // 200), replace=False)
+    rc[big] = 0.5 * scale                                         # a "giant": large radius next to small ones
+    ipt = int(rng.choice([1, 2, 4])); S = int(rng.choice([256, 512, 1024]))
+    kind = int(rng.integers(0, 2))
+    info_s = _kick_case(x, v, m, rc, kind=kind, force_kernel=SYM, i_per_thread=ipt, sym_block=S,
+                        what=f"random seed={seed} N={N} I={ipt} S={S} (Newton III)")
+    info_t = _kick_case(x, v, m, rc, kind=kind, force_kernel=1, what=f"random seed={seed} N={N} (one-sided)")
+    assert info_s["n_gpu"] == info_t["n_gpu"]
