@@ -56,6 +56,7 @@ def _L():
         lib.oracle_step.argtypes = [dp, dp, dp, dbl, i64, i64, dbl, dbl, dbl, dbl, i32, dp, dp, i64]
         lib.oracle_diagnostics.argtypes = [dp, dp, dp, dbl, i64, dbl, dp]
         lib.oracle_encounter.argtypes = [dp, dp, dp, dp, i64, dbl, dbl, dbl, i32, dbl, ip, ip, i64, i64, lp]
+        lib.oracle_encounter_split.argtypes = [dp, dp, dp, dp, i64, i64, dbl, dbl, dbl, i32, dbl, ip, ip, i64, i64, lp]
         lib.oracle_groups.restype = i32
         lib.oracle_groups.argtypes = [ip, i64, i64, ip, ip, ip, lp]
         _lib = lib
@@ -220,7 +221,7 @@ def groups(pairs_, N):
                 largest=int(gstat[2]))
 
 
-def encounter(x, v, m, rcrit_, M_star, dt, G, grp, kind=0, tol=1e-12, max_group=1024):
+def encounter(x, v, m, rcrit_, M_star, dt, G, grp, kind=0, tol=1e-12, max_group=1024, n_active=0):
     """H_A with encounters (Eq. 4, 98, 106): the members of every group of `grp` (a dict from
     groups()) are advanced by dt with the Bulirsch-Stoer integrator; returns (x, v, stats) with
     stats = dict(integrated, skipped, failed, steps)."""
@@ -231,9 +232,16 @@ def encounter(x, v, m, rcrit_, M_star, dt, G, grp, kind=0, tol=1e-12, max_group=
     gstart = np.ascontiguousarray(grp["gstart"], dtype=np.int32)
     stats = np.zeros(4, dtype=np.int64)
     dp, ip, lp = C.POINTER(C.c_double), C.POINTER(C.c_int32), C.POINTER(C.c_int64)
-    _L().oracle_encounter(x.ctypes.data_as(dp), v.ctypes.data_as(dp), m.ctypes.data_as(dp), rc.ctypes.data_as(dp), N,
-                          float(M_star), float(G), float(dt), int(kind), float(tol), members.ctypes.data_as(ip),
-                          gstart.ctypes.data_as(ip), int(grp["ngroups"]), int(max_group), stats.ctypes.data_as(lp))
+    if 0 < int(n_active) < N:
+        # semi-active mode: cores and test particles are integrated separately (oracle_encounter_split)
+        _L().oracle_encounter_split(x.ctypes.data_as(dp), v.ctypes.data_as(dp), m.ctypes.data_as(dp), rc.ctypes.data_as(dp),
+                                    N, int(n_active), float(M_star), float(G), float(dt), int(kind), float(tol),
+                                    members.ctypes.data_as(ip), gstart.ctypes.data_as(ip), int(grp["ngroups"]),
+                                    int(max_group), stats.ctypes.data_as(lp))
+    else:
+        _L().oracle_encounter(x.ctypes.data_as(dp), v.ctypes.data_as(dp), m.ctypes.data_as(dp), rc.ctypes.data_as(dp), N,
+                              float(M_star), float(G), float(dt), int(kind), float(tol), members.ctypes.data_as(ip),
+                              gstart.ctypes.data_as(ip), int(grp["ngroups"]), int(max_group), stats.ctypes.data_as(lp))
     return x, v, dict(integrated=int(stats[0]), skipped=int(stats[1]), failed=int(stats[2]), steps=int(stats[3]))
 
 
@@ -262,11 +270,16 @@ def step_enc(x, v, m, M_star, dt, G, nsteps, n1=3.0, n2=0.4, kind=0, tol=1e-12, 
         x = shift(x, v, m, M_star, 0.5 * dt)
         grp = groups(pr, N)
         xk, vk, nfail = drift_kepler(x, v, M_star, dt, G)
-        xe, ve, st = encounter(x, v, m, rc, M_star, dt, G, grp, kind=kind, tol=tol, max_group=max_group)
+        xe, ve, st = encounter(x, v, m, rc, M_star, dt, G, grp, kind=kind, tol=tol, max_group=max_group, n_active=n_active)
         moved = np.zeros(N, dtype=bool)
         for g in range(grp["ngroups"]):
             seg = grp["members"][grp["gstart"][g]:grp["gstart"][g + 1]]
-            if seg.shape[0] <= max_group:
+            size = seg.shape[0]
+            if 0 < n_active < N:
+                nc = int(np.count_nonzero(seg < n_active))
+                if nc <= 31 and nc < size:
+                    size = nc                      # split group: only the core counts against max_group
+            if size <= max_group:
                 moved[seg] = True
         x = np.where(moved[:, None], xe, xk)
         v = np.where(moved[:, None], ve, vk)

@@ -679,3 +679,53 @@ void oracle_encounter(double *x, double *v, const double *m, const double *rcrit
         free(y);
     }
 }
+
+/* Semi-active mode (the first n_active bodies exert force, the others only feel it; BASELINE.json:north_star,
+ * DESIGN.md readings S13, S22).  A test particle pulls on nobody, so inside a group the active members (the
+ * "core"; the first members of the group, since members ascend) move exactly as if the test particles were not
+ * there, and the test particles are mutually independent.  A group with at most 31 active members is therefore
+ * split: the core is integrated alone, and every test particle s is integrated together with the core
+ * (core + s, from the same initial state), of which only s is kept.  Groups whose core is larger are treated as
+ * one problem, as in oracle_encounter.  max_group bounds the core (split groups) or the group (unsplit ones).
+ * stats = {groups integrated, groups skipped, sub-integrations whose step size underflowed (body/core left
+ * unchanged), accepted steps in total}. */
+void oracle_encounter_split(double *x, double *v, const double *m, const double *rcrit, int64_t N, int64_t n_active,
+                            double M_star, double G, double dt, int kind, double tol, const int32_t *members,
+                            const int32_t *gstart, int64_t ngroups, int64_t max_group, int64_t *stats) {
+    (void)N;
+    stats[0] = stats[1] = stats[2] = stats[3] = 0;
+    for (int64_t g = 0; g < ngroups; ++g) {
+        const int g0 = gstart[g], n = gstart[g + 1] - g0;
+        int nc = 0;
+        while (nc < n && members[g0 + nc] < n_active) ++nc;
+        const int split = (nc <= 31 && nc < n);
+        if ((split ? nc : n) > max_group) { stats[1]++; continue; }
+        const int nn = split ? nc + 1 : n;                   /* size of the largest sub-problem */
+        double *y = (double *)malloc(sizeof(double) * (size_t)(8 * nn));
+        double *gm = y + 6 * nn, *rc = y + 7 * nn;
+        double *x0 = (double *)malloc(sizeof(double) * (size_t)(6 * n)), *v0 = x0 + 3 * n;
+        for (int k = 0; k < n; ++k)
+            for (int c = 0; c < 3; ++c) { x0[3 * k + c] = x[3 * (int64_t)members[g0 + k] + c]; v0[3 * k + c] = v[3 * (int64_t)members[g0 + k] + c]; }
+        const int nsub = split ? 1 + (n - nc) : 1;          /* sub-problem 0: the core (or the whole group) */
+        for (int sub = 0; sub < nsub; ++sub) {
+            const int nb = split ? (sub == 0 ? nc : nc + 1) : n;
+            for (int k = 0; k < nb; ++k) {
+                const int src = (split && k == nc) ? nc + sub - 1 : k;   /* the satellite of this sub-problem */
+                const int32_t b = members[g0 + src];
+                for (int c = 0; c < 3; ++c) { y[3 * k + c] = x0[3 * src + c]; y[3 * nb + 3 * k + c] = v0[3 * src + c]; }
+                gm[k] = G * m[b]; rc[k] = rcrit[b];
+            }
+            const int64_t st = oracle_encounter_group(y, nb, gm, rc, G * M_star, kind, dt, tol);
+            if (st < 0) { stats[2]++; continue; }
+            stats[3] += st;
+            const int first = (split && sub > 0) ? nc : 0;   /* a satellite sub-problem keeps only the satellite */
+            for (int k = first; k < nb; ++k) {
+                const int src = (split && k == nc) ? nc + sub - 1 : k;
+                const int32_t b = members[g0 + src];
+                for (int c = 0; c < 3; ++c) { x[3 * (int64_t)b + c] = y[3 * k + c]; v[3 * (int64_t)b + c] = y[3 * nb + 3 * k + c]; }
+            }
+        }
+        stats[0]++;
+        free(y); free(x0);
+    }
+}

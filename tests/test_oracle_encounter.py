@@ -145,3 +145,50 @@ def test_resolving_encounters_restores_energy_conservation():
     a = oracle.step(far_x, far_v, m, 1.0, dt, G, 5, n1=3.0, n2=0.4)
     b = oracle.step_enc(far_x, far_v, m, 1.0, dt, G, 5, n1=3.0, n2=0.4)
     assert np.array_equal(a["x"], b["x"]) and np.array_equal(a["v"], b["v"]) and b["stats"]["integrated"] == 0
+
+
+def test_semi_active_groups_are_split_into_core_and_independent_test_particles():
+    """Semi-active mode (reading S22): test particles pull on nobody, so the core of a group must move exactly as
+    if they were absent, every test particle exactly as in the problem {core + that particle}, and a single
+    embryo with a test particle deep inside its changeover radius around a negligible star is a Kepler problem
+    about the embryo."""
+    G = G_GAUSS
+    rng = np.random.default_rng(9)
+    n_act, n_sat = 3, 12
+    N = n_act + n_sat + 2
+    # embryos and test particles on a jittered 4 x 4 lattice (spacing 3e-3): close, but nobody on top of anybody
+    gi, gj = np.divmod(rng.permutation(16)[: n_act + n_sat], 4)
+    a = np.concatenate([1.0 + 3e-3 * (gi - 1.5) + rng.uniform(-5e-4, 5e-4, n_act + n_sat), [2.0, 2.5]])
+    M = np.concatenate([0.4 + 3e-3 * (gj - 1.5) + rng.uniform(-5e-4, 5e-4, n_act + n_sat), [1.0, 3.0]])
+    x, v = nb_inputs.elements_to_cartesian(a, np.full(N, 1e-3), np.full(N, 5e-4), np.zeros(N), np.zeros(N), M, G)
+    x = np.ascontiguousarray(x); v = np.ascontiguousarray(v)
+    m = np.zeros(N); m[:n_act] = [2e-7, 1e-7, 3e-7]
+    rc = np.full(N, 0.05)
+    pairs = [[0, 1], [1, 2]] + [[int(rng.integers(0, n_act)), k] for k in range(n_act, n_act + n_sat)]
+    grp = oracle.groups(np.array(pairs, dtype=np.int32), N)
+    assert grp["ngroups"] == 1 and grp["largest"] == n_act + n_sat
+    xs, vs, st = oracle.encounter(x, v, m, rc, 1.0, 3.0, G, grp, n_active=n_act, tol=1e-13)
+    assert st["integrated"] == 1 and st["failed"] == 0
+    # core: identical to the core integrated alone (bit for bit: it IS that integration)
+    core = oracle.groups(np.array([[0, 1], [1, 2]], dtype=np.int32), N)
+    xc, vc, _ = oracle.encounter(x, v, m, rc, 1.0, 3.0, G, core, tol=1e-13)
+    assert np.array_equal(xs[:n_act], xc[:n_act]) and np.array_equal(vs[:n_act], vc[:n_act])
+    # every test particle: identical to the problem {core + particle}
+    for k in (n_act, n_act + 7, n_act + n_sat - 1):
+        one = oracle.groups(np.array([[0, 1], [1, 2], [0, k]], dtype=np.int32), N)
+        xo, vo, _ = oracle.encounter(x, v, m, rc, 1.0, 3.0, G, one, tol=1e-13)
+        assert np.array_equal(xs[k], xo[k]) and np.array_equal(vs[k], vo[k])
+    # bodies outside the group untouched; the unsplit treatment agrees to the tolerance (same physics)
+    assert np.array_equal(xs[-2:], x[-2:])
+    xu, vu, _ = oracle.encounter(x, v, m, rc, 1.0, 3.0, G, grp, tol=1e-13)
+    assert np.max(np.abs(xu[:n_act] - xs[:n_act])) <= 1e-11 and np.median(np.abs(xu - xs)) <= 1e-11
+    # closed form: embryo + test particle, star switched off => Kepler orbit of the particle about the embryo
+    m2 = np.array([3e-6, 0.0]); mu = G * m2[0]
+    xr, vr = nb_inputs.elements_to_cartesian(np.array([0.01]), np.array([0.3]), np.array([0.2]), np.array([1.0]),
+                                             np.array([2.0]), np.array([0.5]), mu)
+    x2 = np.stack([np.array([1.0, 0.2, 0.0]), np.array([1.0, 0.2, 0.0]) + xr[0]]); v2 = np.stack([np.array([0.0, 1e-3, 0.0]), np.array([0.0, 1e-3, 0.0]) + vr[0]])
+    P = 2 * np.pi * np.sqrt(0.01 ** 3 / mu)
+    xe, ve, _ = oracle.encounter(x2, v2, m2, np.full(2, 10.0), 1e-30, 0.8 * P, G, oracle.groups(np.array([[0, 1]]), 2), n_active=1, tol=1e-13)
+    xk, vk, code = oracle.kepler_one(xr[0], vr[0], mu, 0.8 * P)
+    assert code == 0 and np.max(np.abs((xe[1] - xe[0]) - xk)) <= 1e-10 * 0.01
+    assert np.max(np.abs(xe[0] - (x2[0] + 0.8 * P * v2[0]))) <= 1e-13      # the embryo does not feel the particle
