@@ -188,7 +188,11 @@ int nb_groups(const int32_t *pairs, const int64_t *npairs, int64_t N, int32_t *l
  * is left alone.  Groups of more than NB_MAX_GROUP members are left alone as well and counted in
  * nb_status[4] (the regime for which the paper proposes multi-level changeovers); a group
  * whose step size underflows is left unchanged and counted in nb_status[5].
- * x, v [N,3] in/out; m, rcrit [N] in.  Needs the first 512 bytes of the workspace.
+ * Semi-active mode (n_active < N; reading S22): a test particle pulls on nobody, so a group with at most 31 active
+ * members is split -- its active core is integrated alone and every test particle together with the core, of
+ * which only the particle is kept; NB_MAX_GROUP then bounds the core, not the group (an embryo may carry
+ * thousands of test particles).  Groups with a larger core are treated as one problem.
+ * x, v [N,3] in/out; m, rcrit [N] in.  Needs the same head of the workspace as nb_groups.
  */
 #define NB_MAX_GROUP 1024
 int nb_encounter(double *x, double *v, const double *m, const double *rcrit, double M_star, int64_t N,

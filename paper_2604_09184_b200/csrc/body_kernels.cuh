@@ -161,14 +161,13 @@ __global__ void __launch_bounds__(kBodyThreads) nb_shift_kernel(double *__restri
 }
 
 // a5 (first half, optional) + a6: x += dtc*P/M_star, then the Kepler flow for dt; optionally emits the
-// momentum partials of the drifted velocities for the second half-shift.  With grp_label / grp_size (the
-// label and root-size arrays of groups.cuh) the members of encounter groups are shifted but not drifted.
+// momentum partials of the drifted velocities for the second half-shift.  With enc_flag (nb_enc_plan_kernel) the
+// bodies the direct solver will move are shifted but not drifted.
 __global__ void __launch_bounds__(kBodyThreads) nb_drift_kernel(double *__restrict__ x, double *__restrict__ v,
                                                                const double *__restrict__ m, int N, double mu, double dt,
                                                                const double *__restrict__ mv_in, int nblk_in,
                                                                double dtc, double M_star, double *__restrict__ mv_out,
-                                                               long long *status, const int *__restrict__ grp_label,
-                                                               const int *__restrict__ grp_size) {
+                                                               long long *status, const int *__restrict__ enc_flag) {
     __shared__ double sm[3 * kBodyThreads];
     double sx = 0.0, sy = 0.0, sz = 0.0;
     if (mv_in != nullptr) {
@@ -181,9 +180,8 @@ __global__ void __launch_bounds__(kBodyThreads) nb_drift_kernel(double *__restri
         double X0 = x[3 * (size_t)i], X1 = x[3 * (size_t)i + 1], X2 = x[3 * (size_t)i + 2];
         double V0 = v[3 * (size_t)i], V1 = v[3 * (size_t)i + 1], V2 = v[3 * (size_t)i + 2];
         if (mv_in != nullptr) { X0 = X0 + dtc * sx; X1 = X1 + dtc * sy; X2 = X2 + dtc * sz; }
-        // members of an encounter group (2 .. kMaxGroup bodies) are left to the direct solver (encounter.cuh)
-        bool in_group = false;
-        if (grp_label != nullptr) { const int gs = grp_size[grp_label[i]]; in_group = gs >= 2 && gs <= 1024; }
+        // bodies of the encounter groups the direct solver takes (encounter.cuh) are left to it
+        const bool in_group = enc_flag != nullptr && enc_flag[i] != 0;
         if (!in_group && kepler_elliptic_fast(X0, X1, X2, V0, V1, V2, mu, dt) != 0) {
             // rare: not bound, or the fast iteration did not settle -> bracketed solvers (state untouched so far)
             double X[3] = {X0, X1, X2}, V[3] = {V0, V1, V2};

@@ -69,7 +69,10 @@ struct EncParams {
     double mu, G, dt, tol;
     int kind;
     int min_size, max_size;   // this launch handles groups with min_size <= n <= max_size
+    const int *gcore;         // [ngroups] active members per group (semi-active mode) or nullptr
 };
+
+__device__ __forceinline__ int enc_group_size(const EncParams &p, const long long g, const int n, bool &split);
 
 // CTA-wide maximum of a non-negative double; every thread gets it.
 template <int THREADS>
@@ -97,7 +100,9 @@ __global__ void __launch_bounds__(THREADS) nb_encounter_kernel(const EncParams p
     const int t = threadIdx.x;
     const long long ngroups = p.gstat[0];
     for (long long g = blockIdx.x; g < ngroups; g += gridDim.x) {
-        const int g0 = p.gstart[g], n = p.gstart[g + 1] - g0;
+        const int g0 = p.gstart[g];
+        bool split;
+        const int n = enc_group_size(p, g, p.gstart[g + 1] - g0, split);
         if (n < p.min_size) continue;
         if (n > p.max_size) {
             if (n > kMaxGroup && p.max_size == kMaxGroup && t == 0) status_add(p.status, ST_GROUP_SKIPPED, 1);
@@ -201,7 +206,34 @@ __global__ void __launch_bounds__(THREADS) nb_encounter_kernel(const EncParams p
 // column by column exactly as the sequential algorithm does and accepts the first column that passes, so
 // the result is the sequential algorithm's, bit for bit.  Critical path per step: 17 right-hand sides
 // instead of up to 80.
-__global__ void __launch_bounds__(32 * kBsCols) nb_encounter_small_kernel(const EncParams p) {
+// Plan of the direct solver for one pair list: per group the number of active members (gcore; the whole group when
+// everybody is active) and per body whether the solver will move it (flag; nb_drift_kernel then leaves it alone).
+// A group is taken if its effective size -- the core of a split semi-active group, else the whole group -- is at
+// most kMaxGroup.  One warp per group.
+__global__ void __launch_bounds__(256) nb_enc_plan_kernel(const int *__restrict__ members, const int *__restrict__ gstart,
+                                                         const long long *__restrict__ gstat, const int n_active,
+                                                         int *__restrict__ gcore, int *__restrict__ flag) {
+    const int lane = threadIdx.x & 31;
+    const long long ngroups = gstat[0];
+    for (long long g = ((long long)blockIdx.x * 256 + threadIdx.x) >> 5; g < ngroups; g += ((long long)gridDim.x * 256) >> 5) {
+        const int g0 = gstart[g], n = gstart[g + 1] - g0;
+        int nc = 0;
+        for (int base = 0; base < n; base += 32) {  // members ascend: the active ones come first
+            const bool a = base + lane < n && members[g0 + base + lane] < n_active;
+            const int c = __popc(__ballot_sync(0xffffffffu, a));
+            nc += c;
+            if (c < 32) break;
+        }
+        const bool split = nc <= 31 && nc < n;
+        const int take = (split ? nc : n) <= kMaxGroup;
+        if (lane == 0) gcore[g] = nc;
+        for (int k = lane; k < n; k += 32) flag[members[g0 + k]] = take;
+    }
+}
+
+// One problem of up to 32 bodies, solved by the whole CTA (8 warps = 8 columns; lane = member, b = the lane's body).
+// Lanes >= keep_from write their final state back (0: everybody; nc: only the test particle of a split group).
+__device__ __forceinline__ void bs_small_problem(const EncParams &p, const int b, const int n, const int keep_from) {
     __shared__ double px[kBsCols][32], py[kBsCols][32], pz[kBsCols][32];
     __shared__ double sgm[32], src[32];
     __shared__ double col[kBsCols][6][32];   // T_{c,0} of every column
@@ -209,126 +241,166 @@ __global__ void __launch_bounds__(32 * kBsCols) nb_encounter_small_kernel(const 
     __shared__ double ctrl_h, ctrl_t;
     __shared__ int ctrl_done;                // 0 running, 1 finished, 2 failed
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
-    const long long ngroups = p.gstat[0];
     const double tol2 = p.tol * p.tol;
-    for (long long g = blockIdx.x; g < ngroups; g += gridDim.x) {
-        const int g0 = p.gstart[g], n = p.gstart[g + 1] - g0;
-        if (n < p.min_size || n > p.max_size) continue;
-        const bool act = lane < n;
-        const int b = act ? p.members[g0 + lane] : 0;
-        __syncthreads();
-        if (w == 0) {
-            if (act) {
+    const bool act = lane < n;
+    __syncthreads();
+    if (w == 0) {
+        if (act) {
 #pragma unroll
-                for (int c = 0; c < 3; ++c) { ycur[c][lane] = p.x[3 * (size_t)b + c]; ycur[3 + c][lane] = p.v[3 * (size_t)b + c]; }
-                sgm[lane] = p.G * p.m[b];
-                src[lane] = p.rcrit[b];
-            }
-            if (lane == 0) { ctrl_h = p.dt; ctrl_t = 0.0; ctrl_done = (p.dt == 0.0) ? 1 : 0; }
+            for (int c = 0; c < 3; ++c) { ycur[c][lane] = p.x[3 * (size_t)b + c]; ycur[3 + c][lane] = p.v[3 * (size_t)b + c]; }
+            sgm[lane] = p.G * p.m[b];
+            src[lane] = p.rcrit[b];
         }
-        __syncthreads();
-        const double my_rc = act ? src[lane] : 0.0;
-        double T[kBsCols][6];                // warp 0: current row of the tableau
-        while (true) {
-            if (ctrl_done != 0) break;
-            double h = ctrl_h;
-            const double tcur = ctrl_t;
-            if (fabs(h) > fabs(p.dt - tcur)) h = p.dt - tcur;
-            const bool underflow = fabs(h) < 1e-14 * fabs(p.dt);
-            double y[6];
+        if (lane == 0) { ctrl_h = p.dt; ctrl_t = 0.0; ctrl_done = (p.dt == 0.0) ? 1 : 0; }
+    }
+    __syncthreads();
+    const double my_rc = act ? src[lane] : 0.0;
+    double T[kBsCols][6];                // warp 0: current row of the tableau
+    while (true) {
+        if (ctrl_done != 0) break;
+        double h = ctrl_h;
+        const double tcur = ctrl_t;
+        if (fabs(h) > fabs(p.dt - tcur)) h = p.dt - tcur;
+        const bool underflow = fabs(h) < 1e-14 * fabs(p.dt);
+        double y[6];
 #pragma unroll
-            for (int k = 0; k < 6; ++k) y[k] = act ? ycur[k][lane] : 0.0;
-            if (!underflow) {
-                // column c = w + 1: modified midpoint with 2c substeps
-                auto rhs = [&](const double (&q)[6], double (&f)[6]) {
-                    __syncwarp();
-                    if (act) { px[w][lane] = q[0]; py[w][lane] = q[1]; pz[w][lane] = q[2]; }
-                    __syncwarp();
-                    if (act) {
-                        double ax, ay, az;
-                        enc_accel(q[0], q[1], q[2], my_rc, lane, n, px[w], py[w], pz[w], sgm, src, p.mu, p.kind, ax, ay, az);
-                        f[0] = q[3]; f[1] = q[4]; f[2] = q[5]; f[3] = ax; f[4] = ay; f[5] = az;
-                    }
-                };
-                const int c = w + 1, nsub = 2 * c;
-                const double hs = h / nsub;
-                double f0[6] = {0, 0, 0, 0, 0, 0}, f[6] = {0, 0, 0, 0, 0, 0}, ym[6], yn[6];
-                rhs(y, f0);
-#pragma unroll
-                for (int k = 0; k < 6; ++k) { ym[k] = y[k]; yn[k] = y[k] + hs * f0[k]; }
-                for (int s = 2; s <= nsub; ++s) {
-                    rhs(yn, f);
-#pragma unroll
-                    for (int k = 0; k < 6; ++k) { const double tmp = ym[k] + 2.0 * hs * f[k]; ym[k] = yn[k]; yn[k] = tmp; }
+        for (int k = 0; k < 6; ++k) y[k] = act ? ycur[k][lane] : 0.0;
+        if (!underflow) {
+            // column c = w + 1: modified midpoint with 2c substeps
+            auto rhs = [&](const double (&q)[6], double (&f)[6]) {
+                __syncwarp();
+                if (act) { px[w][lane] = q[0]; py[w][lane] = q[1]; pz[w][lane] = q[2]; }
+                __syncwarp();
+                if (act) {
+                    double ax, ay, az;
+                    enc_accel(q[0], q[1], q[2], my_rc, lane, n, px[w], py[w], pz[w], sgm, src, p.mu, p.kind, ax, ay, az);
+                    f[0] = q[3]; f[1] = q[4]; f[2] = q[5]; f[3] = ax; f[4] = ay; f[5] = az;
                 }
+            };
+            const int c = w + 1, nsub = 2 * c;
+            const double hs = h / nsub;
+            double f0[6] = {0, 0, 0, 0, 0, 0}, f[6] = {0, 0, 0, 0, 0, 0}, ym[6], yn[6];
+            rhs(y, f0);
+#pragma unroll
+            for (int k = 0; k < 6; ++k) { ym[k] = y[k]; yn[k] = y[k] + hs * f0[k]; }
+            for (int s = 2; s <= nsub; ++s) {
                 rhs(yn, f);
 #pragma unroll
-                for (int k = 0; k < 6; ++k) col[w][k][lane] = 0.5 * (ym[k] + yn[k] + hs * f[k]);
+                for (int k = 0; k < 6; ++k) { const double tmp = ym[k] + 2.0 * hs * f[k]; ym[k] = yn[k]; yn[k] = tmp; }
             }
-            __syncthreads();
-            if (w == 0) {
-                bool accepted = false;
-                int cols = 0;
-                if (!underflow) {
-                    for (int c = 1; c <= kBsCols && !accepted; ++c) {
-                        double dif[6];
+            rhs(yn, f);
 #pragma unroll
-                        for (int k = 0; k < 6; ++k) {
-                            double cur = col[c - 1][k][lane];
-                            const double last_diag = c >= 2 ? T[c - 2][k] : 0.0;
-                            for (int mc = 1; mc < c; ++mc) {
-                                const double old = T[mc - 1][k];
-                                T[mc - 1][k] = cur;
-                                cur = cur + (cur - old) * bs_weight(c, mc);
-                            }
-                            T[c - 1][k] = cur;
-                            dif[k] = cur - last_diag;
-                        }
-                        if (c >= 2) {
-                            double e2 = 0.0;
-                            if (act) {
-                                const double ex = (dif[0] * dif[0] + dif[1] * dif[1]) + dif[2] * dif[2];
-                                const double ev = (dif[3] * dif[3] + dif[4] * dif[4]) + dif[5] * dif[5];
-                                const double sx = (y[0] * y[0] + y[1] * y[1]) + y[2] * y[2];
-                                double sv = (y[3] * y[3] + y[4] * y[4]) + y[5] * y[5];
-                                const double vc2 = p.mu / sqrt(sx);
-                                if (sv < vc2) sv = vc2;
-                                e2 = fmax(ex / sx, ev / sv);
-                                if (!(e2 == e2)) e2 = INFINITY;
-                            }
-#pragma unroll
-                            for (int o = 16; o > 0; o >>= 1) e2 = fmax(e2, __shfl_xor_sync(0xffffffffu, e2, o));
-                            if (e2 <= tol2) { accepted = true; cols = c; }
-                        }
-                    }
-                }
-                if (accepted && act) {
-#pragma unroll
-                    for (int k = 0; k < 6; ++k) ycur[k][lane] = T[cols - 1][k];
-                }
-                if (lane == 0) {
-                    if (underflow) {
-                        ctrl_done = 2;
-                    } else if (accepted) {
-                        const double tn = (fabs(p.dt - (tcur + h)) <= 1e-15 * fabs(p.dt)) ? p.dt : tcur + h;
-                        ctrl_t = tn;
-                        ctrl_h = cols <= 6 ? h * 1.3 : (cols == 8 ? h * 0.55 : h);
-                        if (tn == p.dt) ctrl_done = 1;
-                    } else {
-                        ctrl_h = h * 0.5;
-                    }
-                }
-            }
-            __syncthreads();
+            for (int k = 0; k < 6; ++k) col[w][k][lane] = 0.5 * (ym[k] + yn[k] + hs * f[k]);
         }
+        __syncthreads();
         if (w == 0) {
-            if (ctrl_done == 2) {
-                if (lane == 0) status_add(p.status, ST_BS_FAIL, 1);  // group left unchanged
-            } else if (act) {
+            bool accepted = false;
+            int cols = 0;
+            if (!underflow) {
+                for (int c = 1; c <= kBsCols && !accepted; ++c) {
+                    double dif[6];
 #pragma unroll
-                for (int c = 0; c < 3; ++c) { p.x[3 * (size_t)b + c] = ycur[c][lane]; p.v[3 * (size_t)b + c] = ycur[3 + c][lane]; }
+                    for (int k = 0; k < 6; ++k) {
+                        double cur = col[c - 1][k][lane];
+                        const double last_diag = c >= 2 ? T[c - 2][k] : 0.0;
+                        for (int mc = 1; mc < c; ++mc) {
+                            const double old = T[mc - 1][k];
+                            T[mc - 1][k] = cur;
+                            cur = cur + (cur - old) * bs_weight(c, mc);
+                        }
+                        T[c - 1][k] = cur;
+                        dif[k] = cur - last_diag;
+                    }
+                    if (c >= 2) {
+                        double e2 = 0.0;
+                        if (act) {
+                            const double ex = (dif[0] * dif[0] + dif[1] * dif[1]) + dif[2] * dif[2];
+                            const double ev = (dif[3] * dif[3] + dif[4] * dif[4]) + dif[5] * dif[5];
+                            const double sx = (y[0] * y[0] + y[1] * y[1]) + y[2] * y[2];
+                            double sv = (y[3] * y[3] + y[4] * y[4]) + y[5] * y[5];
+                            const double vc2 = p.mu / sqrt(sx);
+                            if (sv < vc2) sv = vc2;
+                            e2 = fmax(ex / sx, ev / sv);
+                            if (!(e2 == e2)) e2 = INFINITY;
+                        }
+#pragma unroll
+                        for (int o = 16; o > 0; o >>= 1) e2 = fmax(e2, __shfl_xor_sync(0xffffffffu, e2, o));
+                        if (e2 <= tol2) { accepted = true; cols = c; }
+                    }
+                }
+            }
+            if (accepted && act) {
+#pragma unroll
+                for (int k = 0; k < 6; ++k) ycur[k][lane] = T[cols - 1][k];
+            }
+            if (lane == 0) {
+                if (underflow) {
+                    ctrl_done = 2;
+                } else if (accepted) {
+                    const double tn = (fabs(p.dt - (tcur + h)) <= 1e-15 * fabs(p.dt)) ? p.dt : tcur + h;
+                    ctrl_t = tn;
+                    ctrl_h = cols <= 6 ? h * 1.3 : (cols == 8 ? h * 0.55 : h);
+                    if (tn == p.dt) ctrl_done = 1;
+                } else {
+                    ctrl_h = h * 0.5;
+                }
             }
         }
+        __syncthreads();
+    }
+    if (w == 0) {
+        if (ctrl_done == 2) {
+            if (lane == 0) status_add(p.status, ST_BS_FAIL, 1);  // group left unchanged
+        } else if (act && lane >= keep_from) {
+#pragma unroll
+            for (int c = 0; c < 3; ++c) { p.x[3 * (size_t)b + c] = ycur[c][lane]; p.v[3 * (size_t)b + c] = ycur[3 + c][lane]; }
+        }
+    }
+
+}
+
+// effective size of group g: its core in a split semi-active group (gcore), else the whole group
+__device__ __forceinline__ int enc_group_size(const EncParams &p, const long long g, const int n, bool &split) {
+    split = false;
+    if (p.gcore == nullptr) return n;
+    const int nc = p.gcore[g];
+    split = nc <= 31 && nc < n;
+    return split ? nc : n;
+}
+
+__global__ void __launch_bounds__(32 * kBsCols) nb_encounter_small_kernel(const EncParams p) {
+    const int lane = threadIdx.x & 31;
+    const long long ngroups = p.gstat[0];
+    for (long long g = blockIdx.x; g < ngroups; g += gridDim.x) {
+        const int g0 = p.gstart[g];
+        bool split;
+        const int n = enc_group_size(p, g, p.gstart[g + 1] - g0, split);
+        if (n < p.min_size || n > p.max_size) continue;
+        bs_small_problem(p, lane < n ? p.members[g0 + lane] : 0, n, 0);
+    }
+}
+
+// Semi-active mode: the test particles of split groups, one CTA per particle: {core + particle} from the initial
+// state, only the particle is kept (reading S22).  Must run BEFORE the kernels that advance the cores.
+__global__ void __launch_bounds__(32 * kBsCols) nb_encounter_sat_kernel(const EncParams p) {
+    __shared__ int sh_g;
+    const int lane = threadIdx.x & 31;
+    const long long ngroups = p.gstat[0], nslots = p.gstat[1];
+    for (long long k = blockIdx.x; k < nslots; k += gridDim.x) {
+        __syncthreads();
+        if (threadIdx.x == 0) {  // group of member slot k: last g with gstart[g] <= k
+            long long lo = 0, hi = ngroups - 1;
+            while (lo < hi) { const long long mid = (lo + hi + 1) >> 1; if (p.gstart[mid] <= k) lo = mid; else hi = mid - 1; }
+            sh_g = (int)lo;
+        }
+        __syncthreads();
+        const long long g = sh_g;
+        const int g0 = p.gstart[g];
+        bool split;
+        const int nc = enc_group_size(p, g, p.gstart[g + 1] - g0, split);
+        if (!split || k < g0 + nc) continue;  // not a test particle of a split group
+        const int b = lane < nc ? p.members[g0 + lane] : (lane == nc ? p.members[k] : 0);
+        bs_small_problem(p, b, nc + 1, nc);
     }
 }
 

@@ -188,6 +188,7 @@ struct Workspace {
     GroupScratch grp;   // encounter groups (groups.cuh): 5 N + 2 ceil(N/1024) + N/2048 + 3 ints
     int32_t *g_label, *g_members, *g_start;  // the step driver's own group lists
     int64_t *g_stat;
+    int *g_core, *enc_flag;                  // direct-solver plan: active members per group, per-body flag
     char *head_mv_end, *head_grp_end;  // ends of the geometry-independent head
     double *rc_scratch; // [N]
     JRec *jrec;         // [Njpad]                 (one-sided kernel)
@@ -225,6 +226,8 @@ Workspace carve(void *base, int64_t N, const Geometry &g) {
         w.g_members = reinterpret_cast<int32_t *>(b + off); off += n4;
         w.g_start = reinterpret_cast<int32_t *>(b + off); off += align_up(((size_t)N / 2 + 2) * sizeof(int), 256);
         w.g_stat = reinterpret_cast<int64_t *>(b + off); off += 256;
+        w.g_core = reinterpret_cast<int *>(b + off); off += align_up(((size_t)N / 2 + 2) * sizeof(int), 256);
+        w.enc_flag = reinterpret_cast<int *>(b + off); off += n4;
     }
     w.head_grp_end = b + off;
     w.rc_scratch = reinterpret_cast<double *>(b + off); off += align_up((size_t)N * sizeof(double), 256);
@@ -432,19 +435,39 @@ void enqueue_groups(const Workspace &w, const int32_t *pairs, const int64_t *npa
     nb_grp_giant_kernel<<<sm_count(), kGrpScanBlock, 0, stream()>>>(w.grp, label, n, members);
 }
 
+// Which groups the direct solver takes, and the per-body flag nb_drift_kernel obeys (encounter.cuh).
+void enqueue_encounter_plan(const Workspace &w, int64_t N, const int32_t *members, const int32_t *gstart, const int64_t *gstat) {
+    const int na = (int)((g_cfg.n_active > 0 && g_cfg.n_active < N) ? g_cfg.n_active : N);
+    cudaMemsetAsync(w.enc_flag, 0, (size_t)N * sizeof(int), stream());
+    long long blocks = (N / 2 + 8) / 8;
+    if (blocks > 16LL * sm_count()) blocks = 16LL * sm_count();
+    nb_enc_plan_kernel<<<(unsigned)blocks, 256, 0, stream()>>>(members, gstart, reinterpret_cast<const long long *>(gstat), na,
+                                                              w.g_core, w.enc_flag);
+}
+
 // H_A with encounters for the listed groups (encounter.cuh): groups of up to 32 members by CTAs of 8 warps (one per
 // extrapolation column), 33 .. 128 members by CTAs of 128 threads, up to kMaxGroup members by CTAs of kMaxGroup threads
 // (one thread per member, columns in sequence)
 void enqueue_encounter(const Workspace &w, double *x, double *v, const double *m, const double *rcrit, double M_star,
-                       int64_t N, double dt, const int32_t *members, const int32_t *gstart, const int64_t *gstat) {
+                       int64_t N, double dt, const int32_t *members, const int32_t *gstart, const int64_t *gstat,
+                       bool plan_done) {
+    const long long *gs = reinterpret_cast<const long long *>(gstat);
+    if (!plan_done) enqueue_encounter_plan(w, N, members, gstart, gstat);
     EncParams ep;
     ep.x = x; ep.v = v; ep.m = m; ep.rcrit = rcrit; ep.members = members; ep.gstart = gstart;
-    ep.gstat = reinterpret_cast<const long long *>(gstat); ep.status = w.status; ep.mu = g_cfg.G * M_star; ep.G = g_cfg.G;
+    ep.gstat = gs; ep.status = w.status; ep.mu = g_cfg.G * M_star; ep.G = g_cfg.G;
     ep.dt = dt; ep.tol = g_cfg.bs_tol > 0.0 ? g_cfg.bs_tol : 1e-12; ep.kind = g_cfg.changeover_kind;
+    ep.gcore = w.g_core;
     long long small_blocks = N / 2 + 1;
     const long long cap_blocks = (long long)sm_count() * 8;
     if (small_blocks > cap_blocks) small_blocks = cap_blocks;
-    ep.min_size = 2; ep.max_size = 32;
+    ep.min_size = 1; ep.max_size = 32;
+    if (g_cfg.n_active > 0 && g_cfg.n_active < N) {
+        // semi-active: the test particles of split groups first (they read the cores' initial state)
+        long long sat_blocks = N;
+        if (sat_blocks > cap_blocks) sat_blocks = cap_blocks;
+        nb_encounter_sat_kernel<<<(unsigned)sat_blocks, 32 * kBsCols, 0, stream()>>>(ep);
+    }
     nb_encounter_small_kernel<<<(unsigned)small_blocks, 32 * kBsCols, 0, stream()>>>(ep);
     // mid-size groups: CTAs of 128 threads (no register cap: the 1024-thread variant is held to 64 registers and spills)
     ep.min_size = 33; ep.max_size = 128;
@@ -490,14 +513,16 @@ int step_impl(double *x, double *v, const double *m, double M_star, int64_t N, d
     if (enc && !pairs) return fail(NB_E_BADARG, "nb_step: resolve_encounters needs the pair list (pairs != NULL)");
     auto enqueue_step = [&](int nhalf) -> int {
         // groups of the pair list of the evaluation that opened this step
-        if (enc) enqueue_groups(w, pairs, npairs, N, w.g_label, w.g_members, w.g_start, w.g_stat);
+        if (enc) {
+            enqueue_groups(w, pairs, npairs, N, w.g_label, w.g_members, w.g_start, w.g_stat);
+            enqueue_encounter_plan(w, N, w.g_members, w.g_start, w.g_stat);
+        }
         // C(dt/2) A(dt): first half-shift folded into the drift kernel; members of groups are only shifted there
         // and then propagated through their encounter by the direct solver
         nb_drift_kernel<<<nblk, kBodyThreads, 0, stream()>>>(x, v, m, (int)N, mu, dt, w.mvA, nblk, dtc, M_star,
-                                                             enc ? nullptr : w.mvB, w.status, enc ? w.g_label : nullptr,
-                                                             enc ? w.grp.size : nullptr);
+                                                             enc ? nullptr : w.mvB, w.status, enc ? w.enc_flag : nullptr);
         if (enc) {
-            enqueue_encounter(w, x, v, m, rc_io, M_star, N, dt, w.g_members, w.g_start, w.g_stat);
+            enqueue_encounter(w, x, v, m, rc_io, M_star, N, dt, w.g_members, w.g_start, w.g_stat, true);
             nb_momentum_kernel<<<nblk, kBodyThreads, 0, stream()>>>(v, m, (int)N, w.mvB);
         }
         // C(dt/2) folded into prep; force; B(dt/2) [+ B(dt/2) of the next step]
@@ -672,7 +697,7 @@ int nb_drift_kepler(double *x, double *v, double M_star, int64_t N, double dt) {
     Workspace w;
     if ((rc = check_workspace_head(N, 0, &w))) return rc;
     nb_drift_kernel<<<body_blocks(N), kBodyThreads, 0, stream()>>>(x, v, nullptr, (int)N, g_cfg.G * M_star, dt, nullptr, 0,
-                                                                   0.0, M_star, nullptr, w.status, nullptr, nullptr);
+                                                                   0.0, M_star, nullptr, w.status, nullptr);
     NB_CUDA(cudaGetLastError());
     return NB_OK;
 }
@@ -736,8 +761,8 @@ int nb_encounter(double *x, double *v, const double *m, const double *rcrit, dou
     if (rc) return rc;
     if (!x || !v || !m || !rcrit || !members || !gstart || !gstat) return fail(NB_E_NULL, "nb_encounter: NULL argument");
     Workspace w;
-    if ((rc = check_workspace_head(N, 0, &w))) return rc;
-    enqueue_encounter(w, x, v, m, rcrit, M_star, N, dt, members, gstart, gstat);
+    if ((rc = check_workspace_head(N, 2, &w))) return rc;
+    enqueue_encounter(w, x, v, m, rcrit, M_star, N, dt, members, gstart, gstat, false);
     NB_CUDA(cudaGetLastError());
     return NB_OK;
 }

@@ -21,11 +21,11 @@ pytestmark = pytest.mark.gpu
 ENC_TOL = 1e-9
 
 
-def _gpu_encounter(x, v, m, rc, M_star, dt, grp, kind=0, tol=1e-12):
+def _gpu_encounter(x, v, m, rc, M_star, dt, grp, kind=0, tol=1e-12, n_active=0):
     import paper_2604_09184_b200 as nb
     torch = torch_mod()
     N = m.shape[0]
-    nb.configure(N, G=G_GAUSS, changeover_kind=kind, bs_tol=tol, pair_capacity=16)
+    nb.configure(N, G=G_GAUSS, changeover_kind=kind, bs_tol=tol, pair_capacity=16, n_active=n_active)
     nb.nb_status_reset()
     xd, vd, md, rcd = to_dev(x), to_dev(v), to_dev(m), to_dev(rc)
     members = torch.full((N,), -1, dtype=torch.int32, device="cuda")
@@ -191,3 +191,42 @@ def test_step_with_encounters_semi_active():
     sure, border = oracle.pairs(xg, rcg, n_active=d.n_active)
     gp, n = st.get_pairs()
     assert_pairs_match(gp, n, sure, border, "semi-active step_enc")
+
+
+def test_encounter_semi_active_split_groups():
+    """Semi-active mode (reading S22): star-shaped groups -- a few embryos, each with many test particles, one group far
+    beyond NB_MAX_GROUP bodies whose core is two embryos -- are split into the core and independent test particles."""
+    rng = np.random.default_rng(31)
+    n_act = 6
+    sat_per = [1500, 40, 3, 0, 25, 1]                      # embryo 0 and 1 share a group: 1540 + 2 bodies
+    N = n_act + sum(sat_per) + 30
+    a = np.empty(N); M = np.empty(N)
+    a[:n_act] = 1.0 + 0.2 * np.arange(n_act); M[:n_act] = 0.7 * np.arange(n_act)
+    a[1] = a[0] + 1.5e-3; M[1] = M[0] + 1.5e-3             # embryos 0 and 1 in encounter (mid-way between lattice cells)
+    pairs = [[0, 1]]
+    pos = n_act
+    for e, ns in enumerate(sat_per):
+        # test particles on a jittered lattice around their embryo, never closer than ~1e-3
+        side = int(np.ceil(np.sqrt(ns + 1))) | 1
+        cells = [(i, j) for i in range(side) for j in range(side) if (i, j) != (side // 2, side // 2)][:ns]
+        for (i, j) in cells:
+            a[pos] = a[e] + 3e-3 * (i - side // 2) + rng.uniform(-4e-4, 4e-4)
+            M[pos] = M[e] + 3e-3 * (j - side // 2) + rng.uniform(-4e-4, 4e-4)
+            pairs.append([e, pos]); pos += 1
+    a[pos:] = rng.uniform(3.0, 4.0, N - pos); M[pos:] = rng.uniform(0, 6, N - pos)
+    x, v = nb_inputs.elements_to_cartesian(a, rng.uniform(0, 1e-4, N), rng.uniform(0, 5e-5, N), np.zeros(N), np.zeros(N), M, G_GAUSS)
+    x = np.ascontiguousarray(x); v = np.ascontiguousarray(v)
+    m = np.zeros(N); m[:n_act] = rng.uniform(1e-9, 1e-8, n_act)       # Hill radii ~1e-3: no deep fly-by in 3 days
+    rc = np.full(N, 0.2)
+    grp = oracle.groups(np.array(pairs, dtype=np.int32), N)
+    assert grp["largest"] == 1542 and grp["ngroups"] == 4
+    xg, vg, status = _gpu_encounter(x, v, m, rc, 1.0, 3.0, grp, n_active=n_act)
+    xr, vr, st = oracle.encounter(x, v, m, rc, 1.0, 3.0, G_GAUSS, grp, tol=1e-12, n_active=n_act)
+    assert st["skipped"] == 0 and st["failed"] == 0 and status["groups_skipped"] == 0 and status["bs_fail"] == 0
+    moved = np.zeros(N, dtype=bool); moved[grp["members"]] = True
+    assert np.array_equal(xg[~moved], x[~moved]) and np.array_equal(vg[~moved], v[~moved])
+    ex = np.max(np.abs(xg[moved] - xr[moved]) / np.linalg.norm(xr[moved], axis=1, keepdims=True))
+    ev = np.max(np.abs(vg[moved] - vr[moved]) / np.linalg.norm(vr[moved], axis=1, keepdims=True))
+    print(f"semi-active split: {int(moved.sum())} bodies in {grp['ngroups']} groups, BS steps {st['steps']}, max rel dx {ex:.2e} dv {ev:.2e}")
+    assert ex <= ENC_TOL and ev <= ENC_TOL
+    assert np.max(np.abs(xr[moved] - x[moved])) > 0
