@@ -382,7 +382,9 @@ __global__ void __launch_bounds__(32 * kBsCols) nb_encounter_small_kernel(const 
 
 // Semi-active mode: the test particles of split groups, one CTA per particle: {core + particle} from the initial
 // state, only the particle is kept (reading S22).  Must run BEFORE the kernels that advance the cores.
-__global__ void __launch_bounds__(32 * kBsCols) nb_encounter_sat_kernel(const EncParams p) {
+// Thousands of easy problems: throughput-bound, so the register allocation is capped for 4 CTAs per SM (the
+// latency-bound kernel above is faster uncapped).
+__global__ void __launch_bounds__(32 * kBsCols, 4) nb_encounter_sat_kernel(const EncParams p) {
     __shared__ int sh_g;
     const int lane = threadIdx.x & 31;
     const long long ngroups = p.gstat[0], nslots = p.gstat[1];
