@@ -244,6 +244,23 @@ def drift_roofline(d, n_bodies=1 << 24, launches=5):
                 bodies_per_sec=n_bodies / (ms * 1e-3))
 
 
+def max_over_ranks(values, device="cuda"):
+    """Replicas only: the single cross-rank step of the benchmark is this MAX over the ranks' timings (no
+    data-path collective).  Works with any initialised backend (nccl on the GPUs, gloo in the CPU tests)."""
+    import torch
+    import torch.distributed as dist
+    if not (dist.is_available() and dist.is_initialized()) or dist.get_world_size() == 1:
+        return [float(v) for v in values]
+    t = torch.tensor([float(v) for v in values], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return [float(v) for v in t.cpu().tolist()]
+
+
+def whole_job_value(world, steps, interactions_per_step, max_total_ms):
+    """Whole-job aggregate: every replica does `steps` steps in the slowest rank's time."""
+    return world * steps * interactions_per_step / (max_total_ms * 1e-3)
+
+
 def run_cuda(args):
     import torch
     import torch.distributed as dist
@@ -362,17 +379,16 @@ def run_cuda(args):
 
     # ---- max over ranks (replicas: no data-path collective; this is only the timing reduction) -----
     if world > 1:
-        t = torch.tensor([total_ms, e2e["te"] if e2e else 0.0], dtype=torch.float64, device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        total_ms = float(t[0].item())
+        red = max_over_ranks([total_ms, e2e["te"] if e2e else 0.0])
+        total_ms = red[0]
         if e2e:
-            e2e["te"] = float(t[1].item())
+            e2e["te"] = red[1]
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()
         return
 
-    value = world * K * inter_per_step / (total_ms * 1e-3)
+    value = whole_job_value(world, K, inter_per_step, total_ms)
     symmetric = geom.tile_j < 0
     kernel = "nb_force_sym_kernel" if symmetric else "nb_force_tiles_kernel"
     # FP64-pipe instructions per ORDERED interaction on the fast path: 20 per unordered pair (Newton III)
