@@ -58,6 +58,9 @@ extern "C" {
  *                       serves both bodies (two thirds of the fp64 instructions); fully active case
  *                       only -- with n_active < N the call falls back to NB_FORCE_TILES.
  *   NB_FORCE_AUTO       symmetric when fully active and N >= 12288, else tiles. */
+#define NB_SORT_AUTO 0
+#define NB_SORT_ON 1
+#define NB_SORT_OFF 2
 #define NB_FORCE_AUTO 0
 #define NB_FORCE_TILES 1
 #define NB_FORCE_SYMMETRIC 2
@@ -91,6 +94,9 @@ typedef struct nb_config {
                                 drift; needs pairs != NULL (default 0: pure Kepler drift) */
     double bs_tol;           /* relative tolerance of the direct solver's Bulirsch-Stoer steps (default 1e-12) */
     double radius_factor;    /* nb_merge: factor f by which the physical radii are inflated (default 1) */
+    int sort_staging;        /* tuning (symmetric kernel): NB_SORT_ON stages the bodies sorted by azimuth, so that super-tiles whose
+                                arcs cannot hold an encounter pair skip the test (results keep the caller's indexing);
+                                NB_SORT_AUTO (default): on for N >= 32768; NB_SORT_OFF */
 } nb_config;
 
 void nb_default_config(nb_config *cfg);

@@ -50,6 +50,7 @@ class NbConfig(C.Structure):
         ("resolve_encounters", C.c_int),
         ("bs_tol", C.c_double),
         ("radius_factor", C.c_double),
+        ("sort_staging", C.c_int),
     ]
 
 
@@ -157,7 +158,7 @@ def default_config() -> NbConfig:
 
 def configure(N=None, *, stream=None, pair_capacity=0, n_active=0, G=None, n1=3.0, n2=0.4, changeover_kind=0,
               i_per_thread=0, j_splits=0, use_graph=True, reuse_acc=False, time_force=False, ctas_per_sm=0,
-              pipeline_j=0, force_kernel=0, sym_block=0, resolve_encounters=False, bs_tol=1e-12, radius_factor=1.0, workspace_bytes=None,
+              pipeline_j=0, force_kernel=0, sym_block=0, resolve_encounters=False, bs_tol=1e-12, radius_factor=1.0, sort_staging=0, workspace_bytes=None,
               device="cuda"):
     """nb_configure with a torch-allocated workspace sized for N bodies (N=None: no workspace,
     enough for the _host calls; workspace_bytes: explicit size, e.g. the head that the O(N) calls
@@ -178,6 +179,7 @@ def configure(N=None, *, stream=None, pair_capacity=0, n_active=0, G=None, n1=3.
     cfg.force_kernel, cfg.sym_block = int(force_kernel), int(sym_block)
     cfg.resolve_encounters, cfg.bs_tol = (1 if resolve_encounters else 0), float(bs_tol)
     cfg.radius_factor = float(radius_factor)
+    cfg.sort_staging = int(sort_staging)
     if N is not None:
         import torch
         if stream is None:

@@ -31,6 +31,7 @@ struct PrepParams {
     double2 *sxy, *szg;     // [2 Npad_sym] symmetric kernel's (x,y) and (z,Gm), doubled-block layout (nullptr: not staged)
     int *sthr;              // [2 Npad_sym] hi32(rcrit^2) + 1
     int Npad_sym;
+    const int *pos_of;      // [N] staged position of each body (sort_staging.cuh) or nullptr: position = index
     const double *mv_in;    // [nblk_in,3] momentum partials or nullptr
     unsigned long long *npairs;  // reset to 0 here (nullptr: skip)
     long long *status;
@@ -83,7 +84,8 @@ __global__ void __launch_bounds__(kBodyThreads) nb_prep_kernel(const PrepParams 
         // positions (pad-pad distances stay huge and finite) and zero mass
         double sx_ = r.x, sy_ = r.y, sz_ = r.z;
         if (i >= p.N) { sx_ = kFarJ + 1.0e27 * (double)(i - p.N + 1); sy_ = kFarJ; sz_ = kFarJ; }
-        const size_t en = (size_t)(i >> 5) * 64 + (i & 31);  // doubled-block layout (force_sym.cuh)
+        const int pos = (p.pos_of != nullptr && i < p.N) ? p.pos_of[i] : i;   // padding bodies keep the tail positions
+        const size_t en = (size_t)(pos >> 5) * 64 + (pos & 31);  // doubled-block layout (force_sym.cuh)
         const int thr = __double2hiint(r.rc2) + 1;
         p.sxy[en] = make_double2(sx_, sy_); p.sxy[en + 32] = make_double2(sx_, sy_);
         p.szg[en] = make_double2(sz_, r.gm); p.szg[en + 32] = make_double2(sz_, r.gm);
@@ -105,17 +107,21 @@ __global__ void __launch_bounds__(kBodyThreads) nb_rcrit_kernel(const double *__
 // a4: acc_i = sum over j-splits (in split order) of the partial sums; v_i = v_i + hk*acc_i, applied
 // nhalf times (the closing half-kick of one step and the opening half-kick of the next are two
 // separate roundings, as in the step definition).  Optionally emits momentum partials of the new v.
+// perm != nullptr: the partial sums are indexed by staged position (sort_staging.cuh); thread t then serves
+// position t (coalesced slot reads) and writes the body perm[t] (the real bodies hold positions 0 .. N-1).
 __global__ void __launch_bounds__(kBodyThreads) nb_kickv_kernel(const double *part, int nsplit,
                                                                double *acc, double *__restrict__ v,
                                                                const double *__restrict__ m, int N, double hk,
-                                                               int nhalf, double *__restrict__ mv_out) {
+                                                               int nhalf, double *__restrict__ mv_out,
+                                                               const int *__restrict__ perm) {
     __shared__ double sm[3 * kBodyThreads];
-    const int i = blockIdx.x * kBodyThreads + threadIdx.x;
+    const int t = blockIdx.x * kBodyThreads + threadIdx.x;
+    const int i = (perm != nullptr && t < N) ? perm[t] : t;
     double px = 0.0, py = 0.0, pz = 0.0;
-    if (i < N) {
+    if (t < N && i < N) {
         double ax = 0.0, ay = 0.0, az = 0.0;
         for (int s = 0; s < nsplit; ++s) {
-            const double *q = part + ((size_t)s * N + i) * 3;
+            const double *q = part + ((size_t)s * N + t) * 3;
             ax += q[0]; ay += q[1]; az += q[2];
         }
         acc[3 * (size_t)i] = ax; acc[3 * (size_t)i + 1] = ay; acc[3 * (size_t)i + 2] = az;

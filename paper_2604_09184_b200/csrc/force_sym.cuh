@@ -26,6 +26,7 @@
 // of the block's own 32-blocks: all ordered pairs are evaluated, only the i side is kept.
 #pragma once
 #include "force_tiles.cuh"
+#include "sort_staging.cuh"
 
 namespace nbk {
 
@@ -37,7 +38,9 @@ struct SymParams {
     const double2 *sxy;          // [2 Npad] (x, y)
     const double2 *szg;          // [2 Npad] (z, G m)
     const int *sthr;             // [2 Npad] hi32(rcrit^2) + 1
-    const double *rcrit;         // [N]    exact critical radii (slow path only)
+    const double *rcrit;         // [N]    exact critical radii (slow path only), indexed by BODY
+    const int *perm;             // [Npad] staged position -> body (sorted staging, sort_staging.cuh) or nullptr
+    const BlockBound *bnd;       // [nsb]  azimuth / radius / rc bounds of every staged super-block, or nullptr
     double *part;                // [nsb, N, 3]
     int32_t *pairs;              // [cap,2] or nullptr
     unsigned long long *npairs;  // device counter
@@ -61,13 +64,14 @@ __host__ __device__ constexpr size_t sym_smem_bytes(int S) { return (size_t)S * 
 // flagged rotation r, whose fast-path contributions were forced to exactly 0).  Returns the j-side
 // contribution in (cx,cy,cz); emit[k] says whether pair k goes on the list.
 //   mixed: only the i side is kept by the caller and a pair is emitted from its i < j visit only.
-template <int I>
+template <int I, bool SORTED>
 __device__ __forceinline__ void sym_exact(const SymParams &p, const double2 xy, const double2 zg, const int thrj,
                                           const int j, const bool mixed, const double (&xi)[I], const double (&yi)[I],
                                           const double (&zi)[I], const double (&ngi)[I], const int i0,
                                           double (&ax)[I], double (&ay)[I], double (&az)[I], double &cx, double &cy,
                                           double &cz, bool (&emit)[I]) {
-    const double rcj = j < p.N ? p.rcrit[j] : 0.0;
+    // i, j are STAGED POSITIONS (the real bodies hold positions 0 .. N-1); with sorted staging perm gives the body
+    const double rcj = j < p.N ? p.rcrit[SORTED ? p.perm[j] : j] : 0.0;
 #pragma unroll
     for (int k = 0; k < I; ++k) {
         const int i = i0 + 32 * k;
@@ -87,7 +91,7 @@ __device__ __forceinline__ void sym_exact(const SymParams &p, const double2 xy, 
             const double e = __fma_rn(-r2, u, 1.0);
             f = __dmul_rn(__dmul_rn(u, y0), __fma_rn(e, __fma_rn(e, 1.875, 1.5), 1.0));
         } else {
-            const double rc = fmax(p.rcrit[i], rcj);
+            const double rc = fmax(p.rcrit[SORTED ? p.perm[i] : i], rcj);
             const bool inside = r2 < rc * rc;
             emit[k] = inside && (!mixed || i < j);
             if (r2 == 0.0) {
@@ -113,7 +117,9 @@ __device__ __forceinline__ void sym_exact(const SymParams &p, const double2 xy, 
 // contribute exactly 0 to both sides -- and sets bit r of a mask.  After the 32 rotations the
 // (rare) flagged rotations are evaluated exactly, and their j-side contributions are handed to the
 // home lanes of the j-bodies.
-template <int I, bool PAIRS>
+//
+// TEST = false (sorted staging, super-tiles whose arcs are out of each other's reach): no test, no mask, no exact pass.
+template <int I, bool PAIRS, bool TEST, bool SORTED>
 __device__ __forceinline__ void sym_block(const SymParams &p, const double2 *__restrict__ qxy,
                                           const double2 *__restrict__ qzg, const int *__restrict__ qthr,
                                           const int jbase, const bool mixed, const double (&xi)[I],
@@ -131,7 +137,7 @@ __device__ __forceinline__ void sym_block(const SymParams &p, const double2 *__r
     for (int r = 0; r < 32; ++r) {
         const double2 xy = lxy[r];
         const double2 zg = lzg[r];
-        const int thrj = lthr[r];
+        const int thrj = TEST ? lthr[r] : 0;
         double dx[I], dy[I], dz[I], r2[I];
         int mn = 0x7fffffff;
 #pragma unroll
@@ -140,16 +146,19 @@ __device__ __forceinline__ void sym_block(const SymParams &p, const double2 *__r
             dy[k] = __dsub_rn(xy.y, yi[k]);
             dz[k] = __dsub_rn(zg.x, zi[k]);
             r2[k] = __fma_rn(dz[k], dz[k], __fma_rn(dy[k], dy[k], __dmul_rn(dx[k], dx[k])));
-            mn = min(mn, __double2hiint(r2[k]));
+            if (TEST) mn = min(mn, __double2hiint(r2[k]));
         }
-        const bool hit = mn <= max(thr_lane, thrj);
-        if (hit) bits |= rbit;
-        rbit <<= 1;
-        // a flagged lane feeds +inf to the seed: rsqrt(+inf) = +0, so y0 = u = r^-3 = 0 for its I pairs
-        const int kill = hit ? 0x7ff00000 : 0;
+        int kill = 0;
+        if (TEST) {
+            const bool hit = mn <= max(thr_lane, thrj);
+            if (hit) bits |= rbit;
+            rbit <<= 1;
+            // a flagged lane feeds +inf to the seed: rsqrt(+inf) = +0, so y0 = u = r^-3 = 0 for its I pairs
+            kill = hit ? 0x7ff00000 : 0;
+        }
 #pragma unroll
         for (int k = 0; k < I; ++k) {
-            const double y0 = rsqrt_seed(__hiloint2double(max(__double2hiint(r2[k]), kill), 0));
+            const double y0 = TEST ? rsqrt_seed(__hiloint2double(max(__double2hiint(r2[k]), kill), 0)) : rsqrt_seed(r2[k]);
             const double u = __dmul_rn(y0, y0);                          // exact (y0 has 21 bits)
             const double e = __fma_rn(-r2[k], u, 1.0);                   // 1 - r2 y0^2
             const double q = __fma_rn(e, __fma_rn(e, 1.875, 1.5), 1.0);  // (1-e)^(-3/2), next term < 2^-56
@@ -167,7 +176,7 @@ __device__ __forceinline__ void sym_block(const SymParams &p, const double2 *__r
         by = __shfl_sync(0xffffffffu, by, down);
         bz = __shfl_sync(0xffffffffu, bz, down);
     }
-    unsigned any = __reduce_or_sync(0xffffffffu, bits);
+    unsigned any = TEST ? __reduce_or_sync(0xffffffffu, bits) : 0u;
     while (any) {
         const int r = __ffs(any) - 1;
         any &= any - 1u;
@@ -177,10 +186,14 @@ __device__ __forceinline__ void sym_block(const SymParams &p, const double2 *__r
 #pragma unroll
         for (int k = 0; k < I; ++k) emit[k] = false;
         if ((bits >> r) & 1u)
-            sym_exact<I>(p, lxy[r], lzg[r], lthr[r], jbase + src, mixed, xi, yi, zi, ngi, i0, ax, ay, az, cx, cy, cz, emit);
+            sym_exact<I, SORTED>(p, lxy[r], lzg[r], lthr[r], jbase + src, mixed, xi, yi, zi, ngi, i0, ax, ay, az, cx, cy, cz, emit);
         if (PAIRS) {
 #pragma unroll
-            for (int k = 0; k < I; ++k) pair_append(p.pairs, p.npairs, p.status, p.cap, emit[k], i0 + 32 * k, jbase + src);
+            for (int k = 0; k < I; ++k) {
+                int ib = i0 + 32 * k, jb = jbase + src;
+                if (SORTED && emit[k]) { ib = p.perm[ib]; jb = p.perm[jb]; }  // the list holds BODY indices
+                pair_append(p.pairs, p.npairs, p.status, p.cap, emit[k], ib, jb);
+            }
         }
         // body j = jbase + h met lane (h - r) & 31 in rotation r; its sums live in lane h
         const int from = (lane - r) & 31;
@@ -191,7 +204,82 @@ __device__ __forceinline__ void sym_block(const SymParams &p, const double2 *__r
 }
 
 
-template <int I, bool PAIRS, int MINB>
+// The work of one super-tile after B is staged: chunks of A against the blocks of B, then the slot writes.
+template <int I, bool PAIRS, bool TEST, bool SORTED>
+__device__ __forceinline__ void sym_tile(const SymParams &p, const int A, const int B, const bool diag, const int S,
+                                         const double2 *bxy, const double2 *bzg, const int *bthr, double *jsx, double *jsy,
+                                         double *jsz) {
+    const int t = threadIdx.x, lane = t & 31, w = t >> 5;
+    const int nunits = S / (32 * p.U);
+    const int nchunks = S / (kSymThreads * I);
+    for (int c = 0; c < nchunks; ++c) {
+        const int P = (c * 4 + w) * I;                  // first 32-block of this warp's i-block within A
+        const int i0 = A * S + P * 32 + lane;           // global index of the lane's first i-body
+        double xi[I], yi[I], zi[I], ngi[I], ax[I], ay[I], az[I];
+        int thr_lane = 0;
+#pragma unroll
+        for (int k = 0; k < I; ++k) {
+            const size_t en = (size_t)((i0 >> 5) + k) * 64 + lane;  // first copy of body i0 + 32 k
+            const double2 a = p.sxy[en];
+            const double2 b = p.szg[en];
+            xi[k] = a.x; yi[k] = a.y; zi[k] = b.x; ngi[k] = -b.y;
+            thr_lane = max(thr_lane, p.sthr[en]);
+            ax[k] = 0.0; ay[k] = 0.0; az[k] = 0.0;
+        }
+        for (int step = 0; step < nunits; ++step) {
+            int unit = step + w;
+            if (unit >= nunits) unit -= nunits;
+            for (int uu = 0; uu < p.U; ++uu) {
+                const int q = unit * p.U + uu;  // 32-block of B
+                bool mixed = false;
+                if (diag) {
+                    if (q < P) continue;          // the mirrored visit covers it
+                    mixed = q < P + I;
+                }
+                double bx, by, bz;
+                sym_block<I, PAIRS, TEST, SORTED>(p, bxy + q * 64, bzg + q * 64, bthr + q * 64, B * S + q * 32, mixed, xi, yi, zi,
+                                    ngi, thr_lane, i0, ax, ay, az, bx, by, bz);
+                if (!mixed) {
+                    const int n = q * 32 + lane;
+                    jsx[n] += bx; jsy[n] += by; jsz[n] += bz;
+                }
+            }
+            __syncthreads();
+        }
+        if (diag) {
+            // A's bodies are B's bodies: both sides of the diagonal tile go to the same slot
+#pragma unroll
+            for (int k = 0; k < I; ++k) {
+                const int n = P * 32 + 32 * k + lane;
+                jsx[n] += ax[k]; jsy[n] += ay[k]; jsz[n] += az[k];
+            }
+            __syncthreads();
+        } else {
+            double *out = p.part + (size_t)B * p.N * 3;
+#pragma unroll
+            for (int k = 0; k < I; ++k) {
+                const int i = i0 + 32 * k;
+                if (i < p.N) {
+                    out[3 * (size_t)i] = ax[k];
+                    out[3 * (size_t)i + 1] = ay[k];
+                    out[3 * (size_t)i + 2] = az[k];
+                }
+            }
+        }
+    }
+    // j side (and, on the diagonal, both sides) -> slot A for B's bodies
+    double *out = p.part + (size_t)A * p.N * 3;
+    for (int n = t; n < S; n += kSymThreads) {
+        const long long g = (long long)B * S + n;
+        if (g < p.N) {
+            out[3 * g] = jsx[n];
+            out[3 * g + 1] = jsy[n];
+            out[3 * g + 2] = jsz[n];
+        }
+    }
+}
+
+template <int I, bool PAIRS, int MINB, bool SORTED>
 __global__ void __launch_bounds__(kSymThreads, MINB) nb_force_sym_kernel(const SymParams p) {
     extern __shared__ __align__(16) unsigned char sym_smem[];
     const int S = p.S;
@@ -235,73 +323,15 @@ __global__ void __launch_bounds__(kSymThreads, MINB) nb_force_sym_kernel(const S
     __syncthreads();  // barrier initialised and accumulators zeroed before anyone proceeds
     mbar_wait(bar, 0);
 
-    const int nunits = S / (32 * p.U);
-    const int nchunks = S / (kSymThreads * I);
-    for (int c = 0; c < nchunks; ++c) {
-        const int P = (c * 4 + w) * I;                  // first 32-block of this warp's i-block within A
-        const int i0 = A * S + P * 32 + lane;           // global index of the lane's first i-body
-        double xi[I], yi[I], zi[I], ngi[I], ax[I], ay[I], az[I];
-        int thr_lane = 0;
-#pragma unroll
-        for (int k = 0; k < I; ++k) {
-            const size_t en = (size_t)((i0 >> 5) + k) * 64 + lane;  // first copy of body i0 + 32 k
-            const double2 a = p.sxy[en];
-            const double2 b = p.szg[en];
-            xi[k] = a.x; yi[k] = a.y; zi[k] = b.x; ngi[k] = -b.y;
-            thr_lane = max(thr_lane, p.sthr[en]);
-            ax[k] = 0.0; ay[k] = 0.0; az[k] = 0.0;
-        }
-        for (int step = 0; step < nunits; ++step) {
-            int unit = step + w;
-            if (unit >= nunits) unit -= nunits;
-            for (int uu = 0; uu < p.U; ++uu) {
-                const int q = unit * p.U + uu;  // 32-block of B
-                bool mixed = false;
-                if (diag) {
-                    if (q < P) continue;          // the mirrored visit covers it
-                    mixed = q < P + I;
-                }
-                double bx, by, bz;
-                sym_block<I, PAIRS>(p, bxy + q * 64, bzg + q * 64, bthr + q * 64, B * S + q * 32, mixed, xi, yi, zi,
-                                    ngi, thr_lane, i0, ax, ay, az, bx, by, bz);
-                if (!mixed) {
-                    const int n = q * 32 + lane;
-                    jsx[n] += bx; jsy[n] += by; jsz[n] += bz;
-                }
-            }
-            __syncthreads();
-        }
-        if (diag) {
-            // A's bodies are B's bodies: both sides of the diagonal tile go to the same slot
-#pragma unroll
-            for (int k = 0; k < I; ++k) {
-                const int n = P * 32 + 32 * k + lane;
-                jsx[n] += ax[k]; jsy[n] += ay[k]; jsz[n] += az[k];
-            }
-            __syncthreads();
-        } else {
-            double *out = p.part + (size_t)B * p.N * 3;
-#pragma unroll
-            for (int k = 0; k < I; ++k) {
-                const int i = i0 + 32 * k;
-                if (i < p.N) {
-                    out[3 * (size_t)i] = ax[k];
-                    out[3 * (size_t)i + 1] = ay[k];
-                    out[3 * (size_t)i + 2] = az[k];
-                }
-            }
-        }
+    // sorted staging: if the arcs of A and B are out of each other's reach no pair of this super-tile can meet a
+    // critical radius -- the whole tile runs without the encounter test
+    bool far = false;
+    if (SORTED && !diag) {
+        const BlockBound ba = p.bnd[A], bb = p.bnd[B];
+        far = arcs_are_far(ba.phi_lo, ba.phi_hi, ba.r_min, ba.rc_max, bb.phi_lo, bb.phi_hi, bb.r_min, bb.rc_max);
     }
-    // j side (and, on the diagonal, both sides) -> slot A for B's bodies
-    double *out = p.part + (size_t)A * p.N * 3;
-    for (int n = t; n < S; n += kSymThreads) {
-        const long long g = (long long)B * S + n;
-        if (g < p.N) {
-            out[3 * g] = jsx[n];
-            out[3 * g + 1] = jsy[n];
-            out[3 * g + 2] = jsz[n];
-        }
-    }
+    if (SORTED && far) sym_tile<I, PAIRS, false, SORTED>(p, A, B, diag, S, bxy, bzg, bthr, jsx, jsy, jsz);
+    else sym_tile<I, PAIRS, true, SORTED>(p, A, B, diag, S, bxy, bzg, bthr, jsx, jsy, jsz);
 }
 
 }  // namespace nbk

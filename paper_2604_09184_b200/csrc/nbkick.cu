@@ -22,7 +22,7 @@ namespace {
 using namespace nbk;
 
 std::mutex g_mu;
-nb_config g_cfg = {nullptr, nullptr, 0, 0, 0, 0.01720209895 * 0.01720209895, 3.0, 0.4, 0, 0, 0, 1, 0, 0, 0, 0, 0, 0, 0, 1e-12, 1.0};
+nb_config g_cfg = {nullptr, nullptr, 0, 0, 0, 0.01720209895 * 0.01720209895, 3.0, 0.4, 0, 0, 0, 1, 0, 0, 0, 0, 0, 0, 0, 1e-12, 1.0, 0};
 char g_err[512] = "";
 int g_sm_count = 0;
 cudaEvent_t g_ev0 = nullptr, g_ev1 = nullptr;
@@ -97,6 +97,7 @@ struct Geometry {
     int pipe;             // software-pipelined j loop
     int sym;              // 1: Newton-III super-tile kernel (force_sym.cuh); nsplit = number of super-blocks
     int S, U, Npad_sym;   // super-block size, 32-blocks per skew unit, N padded to a multiple of S
+    int sorted;           // symmetric kernel: bodies staged in azimuthal order (sort_staging.cuh)
 };
 
 Geometry geometry(int64_t N, int64_t n_active) {
@@ -105,7 +106,7 @@ Geometry geometry(int64_t N, int64_t n_active) {
     g.tiles_total = (g.Nj + kTileJ - 1) / kTileJ;
     g.Njpad = g.tiles_total * kTileJ;
     const int sms = sm_count();
-    g.sym = 0; g.S = 0; g.U = 0; g.Npad_sym = 0;
+    g.sym = 0; g.S = 0; g.U = 0; g.Npad_sym = 0; g.sorted = 0;
     // Newton-III kernel: fully active case only (a passive body exerts nothing, so there is no second
     // side to serve), and only when there are enough super-tiles to fill the machine several times.
     const bool fully_active = (g.Nj == N);
@@ -133,6 +134,8 @@ Geometry geometry(int64_t N, int64_t n_active) {
         g.Npad_sym = (int)(((N + S - 1) / S) * S);
         g.nsplit = g.Npad_sym / S;
         g.iblocks = g.nsplit; g.tiles_per_split = 0;
+        // sorted staging pays off once the sort (a few small launches) is small against the evaluation
+        g.sorted = g_cfg.sort_staging == NB_SORT_ON || (g_cfg.sort_staging == NB_SORT_AUTO && N >= 32768);
         return g;
     }
     // I: register tile (i-bodies per thread).  I = 2 at 5 CTAs/SM (96 registers, 20 warps/SM) measured
@@ -194,6 +197,8 @@ struct Workspace {
     JRec *jrec;         // [Njpad]                 (one-sided kernel)
     double2 *sxy, *szg; // [2 Npad_sym]            (symmetric kernel, doubled-block layout)
     int *sthr;          // [2 Npad_sym]
+    int *perm, *pos_of; // [Npad_sym], [N]         (sorted staging: position <-> body)
+    BlockBound *bnd;    // [nsplit]                (bounds of the staged super-blocks)
     double *part;       // [nsplit, N, 3]
     size_t bytes;
 };
@@ -235,6 +240,9 @@ Workspace carve(void *base, int64_t N, const Geometry &g) {
     w.sxy = reinterpret_cast<double2 *>(b + off); off += align_up((size_t)2 * g.Npad_sym * sizeof(double2), 256);
     w.szg = reinterpret_cast<double2 *>(b + off); off += align_up((size_t)2 * g.Npad_sym * sizeof(double2), 256);
     w.sthr = reinterpret_cast<int *>(b + off); off += align_up((size_t)2 * g.Npad_sym * sizeof(int), 256);
+    w.perm = reinterpret_cast<int *>(b + off); off += align_up((size_t)g.Npad_sym * sizeof(int), 256);
+    w.pos_of = reinterpret_cast<int *>(b + off); off += align_up((size_t)(g.sym ? N : 0) * sizeof(int), 256);
+    w.bnd = reinterpret_cast<BlockBound *>(b + off); off += align_up((size_t)(g.sym ? g.nsplit : 0) * sizeof(BlockBound), 256);
     {   // partial accelerations; never smaller than 64 bytes per body (nb_merge's compaction buffer)
         size_t pb = (size_t)g.nsplit * (size_t)N * 3 * sizeof(double);
         if (pb < (size_t)N * 64) pb = (size_t)N * 64;
@@ -307,8 +315,8 @@ void launch_force(const ForceParams &fp, const Geometry &g, bool pairs) {
     else launch_force_I<1>(fp, g, pairs);
 }
 
-template <int I, int MINB>
-int launch_sym_IM(const SymParams &sp, const Geometry &g, bool pairs) {
+template <int I, int MINB, bool SORTED>
+int launch_sym_IMS(const SymParams &sp, const Geometry &g, bool pairs) {
     const size_t smem = sym_smem_bytes(g.S);
     const long long T = g.nsplit;
     const unsigned ctas = (unsigned)(T * (T + 1) / 2);
@@ -317,7 +325,12 @@ int launch_sym_IM(const SymParams &sp, const Geometry &g, bool pairs) {
         kern<<<ctas, kSymThreads, smem, stream()>>>(sp);
         return NB_OK;
     };
-    return pairs ? go(nb_force_sym_kernel<I, true, MINB>) : go(nb_force_sym_kernel<I, false, MINB>);
+    return pairs ? go(nb_force_sym_kernel<I, true, MINB, SORTED>) : go(nb_force_sym_kernel<I, false, MINB, SORTED>);
+}
+
+template <int I, int MINB>
+int launch_sym_IM(const SymParams &sp, const Geometry &g, bool pairs) {
+    return g.sorted ? launch_sym_IMS<I, MINB, true>(sp, g, pairs) : launch_sym_IMS<I, MINB, false>(sp, g, pairs);
 }
 
 template <int I>
@@ -346,9 +359,28 @@ int enqueue_eval(const Workspace &w, const Geometry &g, double *x, double *v, co
                  double dt_for_rc, double *rc_io, int update_rc, const double *mv_in, double dtc, double *acc,
                  int32_t *pairs, int64_t *npairs, double hk, int nhalf, double *mv_out, bool time_force) {
     const int nblk = body_blocks(N);
+    const bool sorted = g.sym && g.sorted;
+    if (sorted) {
+        // azimuthal order of the staged bodies (sort_staging.cuh), from the positions before the half-shift: the
+        // order only decides how many super-tiles can skip the encounter test, never a result
+        SortScratch ss;
+        ss.key = w.grp.parent; ss.hist = w.grp.size; ss.cursor = w.grp.cursor; ss.tmp = w.grp.tmp;
+        ss.perm = w.perm; ss.pos_of = w.pos_of;
+        long long nbk = g.Npad_sym / 8;
+        if (nbk > N - 1) nbk = N - 1;
+        if (nbk < 1) nbk = 1;
+        ss.NB = (int)nbk;
+        const int nbp = (g.Npad_sym + kGrpThreads - 1) / kGrpThreads, nbn = ((int)N + kGrpThreads - 1) / kGrpThreads;
+        nb_sort_clear_kernel<<<nbp, kGrpThreads, 0, stream()>>>(ss, (int)N, g.Npad_sym);
+        nb_sort_key_kernel<<<nbn, kGrpThreads, 0, stream()>>>(ss, x, (int)N);
+        nb_sort_scan_kernel<<<1, kGrpScanBlock, 0, stream()>>>(ss);
+        nb_sort_scatter_kernel<<<nbn, kGrpThreads, 0, stream()>>>(ss, (int)N);
+        nb_sort_rank_kernel<<<nbn, kGrpThreads, 0, stream()>>>(ss, (int)N);
+    }
     PrepParams pp;
     pp.x = x; pp.v = v; pp.m = m; pp.rcrit = rc_io; pp.jrec = g.sym ? nullptr : w.jrec; pp.mv_in = mv_in;
     pp.sxy = g.sym ? w.sxy : nullptr; pp.szg = w.szg; pp.sthr = w.sthr; pp.Npad_sym = g.Npad_sym;
+    pp.pos_of = sorted ? w.pos_of : nullptr;
     pp.npairs = pairs ? reinterpret_cast<unsigned long long *>(npairs) : nullptr;
     pp.status = w.status; pp.dtc = dtc; pp.M_star = M_star; pp.G = g_cfg.G; pp.n1 = g_cfg.n1; pp.n2 = g_cfg.n2;
     pp.absdt = std::fabs(dt_for_rc); pp.nblk_in = nblk; pp.N = (int)N; pp.Nj = g.Nj; pp.Njpad = g.Njpad;
@@ -376,6 +408,8 @@ int enqueue_eval(const Workspace &w, const Geometry &g, double *x, double *v, co
     }
     if (g.sym) {
         SymParams sp;
+        if (sorted) nb_sort_bounds_kernel<<<g.nsplit, kGrpThreads, 0, stream()>>>(w.sxy, w.perm, rc_io, (int)N, g.S, w.bnd);
+        sp.perm = sorted ? w.perm : nullptr; sp.bnd = sorted ? w.bnd : nullptr;
         sp.sxy = w.sxy; sp.szg = w.szg; sp.sthr = w.sthr; sp.rcrit = rc_io; sp.part = w.part; sp.pairs = pairs;
         sp.npairs = fp.npairs; sp.status = w.status; sp.cap = fp.cap; sp.N = (int)N; sp.S = g.S; sp.nsb = g.nsplit;
         sp.U = g.U; sp.kind = g_cfg.changeover_kind;
@@ -387,7 +421,8 @@ int enqueue_eval(const Workspace &w, const Geometry &g, double *x, double *v, co
     if (pool) { NB_CUDA(cudaEventRecord(g_tev[2 * g_tev_used + 1], stream())); ++g_tev_used; }
     else if (time_force) { NB_CUDA(cudaEventRecord(g_ev1, stream())); g_force_timed = true; }
 
-    nb_kickv_kernel<<<nblk, kBodyThreads, 0, stream()>>>(w.part, g.nsplit, acc, v, m, (int)N, hk, nhalf, mv_out);
+    nb_kickv_kernel<<<nblk, kBodyThreads, 0, stream()>>>(w.part, g.nsplit, acc, v, m, (int)N, hk, nhalf, mv_out,
+                                                         sorted ? w.perm : nullptr);
     NB_CUDA(cudaGetLastError());
     return NB_OK;
 }
@@ -501,7 +536,7 @@ int step_impl(double *x, double *v, const double *m, double M_star, int64_t N, d
 
     if (g_cfg.reuse_acc && nsteps > 0) {
         // acc already is the force at the current x: opening half-kick only (reads acc as a 1-split partial)
-        nb_kickv_kernel<<<nblk, kBodyThreads, 0, stream()>>>(acc, 1, acc, v, m, (int)N, hk, 1, w.mvA);
+        nb_kickv_kernel<<<nblk, kBodyThreads, 0, stream()>>>(acc, 1, acc, v, m, (int)N, hk, 1, w.mvA, nullptr);
     } else {
         // evaluation at t0 (+ opening half-kick of the first step)
         if ((rc = enqueue_eval(w, g, x, v, m, M_star, N, dt, rc_io, update_rc, nullptr, 0.0, acc, pairs, npairs, hk,
@@ -537,7 +572,7 @@ int step_impl(double *x, double *v, const double *m, double M_star, int64_t N, d
         key.x = x; key.v = v; key.m = m; key.rcrit = rc_io; key.acc = acc; key.pairs = pairs; key.npairs = npairs;
         key.ws = g_cfg.workspace; key.stream = g_cfg.stream; key.N = N; key.n_active = g_cfg.n_active;
         key.cap = g_cfg.pair_capacity; key.dt = dt; key.M_star = M_star; key.G = g_cfg.G; key.n1 = g_cfg.n1;
-        key.n2 = g_cfg.n2; key.kind = g_cfg.changeover_kind; key.bs_tol = g_cfg.bs_tol; key.enc = enc ? 1 : 0; key.ipt = g.S * 1000 + g.ipt * 100 + g.minb * 10 + g.pipe; key.jsplit = g.nsplit;
+        key.n2 = g_cfg.n2; key.kind = g_cfg.changeover_kind; key.bs_tol = g_cfg.bs_tol; key.enc = (enc ? 1 : 0) + 2 * g.sorted; key.ipt = g.S * 1000 + g.ipt * 100 + g.minb * 10 + g.pipe; key.jsplit = g.nsplit;
         key.ws_bytes = g_cfg.workspace_bytes;
         const bool hop = !stream_capturable();
         if (hop) {
@@ -617,6 +652,7 @@ void nb_default_config(nb_config *cfg) {
     cfg->resolve_encounters = 0;
     cfg->bs_tol = 1e-12;
     cfg->radius_factor = 1.0;
+    cfg->sort_staging = NB_SORT_AUTO;
 }
 
 int nb_configure(const nb_config *cfg) {
@@ -637,6 +673,8 @@ int nb_configure(const nb_config *cfg) {
     if (cfg->sym_block != 0 && cfg->sym_block != 256 && cfg->sym_block != 512 && cfg->sym_block != 1024 && cfg->sym_block != 2048)
         return fail(NB_E_BADARG, "sym_block must be 0, 256, 512, 1024 or 2048");
     if (!(cfg->bs_tol >= 0.0) || !std::isfinite(cfg->bs_tol)) return fail(NB_E_BADARG, "bs_tol must be finite and >= 0");
+    if (cfg->sort_staging != NB_SORT_AUTO && cfg->sort_staging != NB_SORT_ON && cfg->sort_staging != NB_SORT_OFF)
+        return fail(NB_E_BADARG, "unknown sort_staging %d", cfg->sort_staging);
     if (!(cfg->radius_factor >= 0.0) || !std::isfinite(cfg->radius_factor)) return fail(NB_E_BADARG, "radius_factor must be finite and >= 0");
     g_cfg = *cfg;
     return NB_OK;

@@ -199,3 +199,78 @@ def test_sym_randomized_shapes_against_oracle(seed):
                         what=f"random seed={seed} N={N} I={ipt} S={S} (Newton III)")
     info_t = _kick_case(x, v, m, rc, kind=kind, force_kernel=1, what=f"random seed={seed} N={N} (one-sided)")
     assert info_s["n_gpu"] == info_t["n_gpu"]
+
+
+# ---- sorted staging (sort_staging.cuh): the staged bodies are permuted into azimuthal order; everything the caller
+# sees (accelerations, pair indices, velocities) must be unchanged up to the summation order ----------------------
+SORT = dict(force_kernel=SYM, sort_staging=1)
+
+
+@pytest.mark.parametrize("ipt,S", [(1, 256), (2, 256), (4, 512)])
+@pytest.mark.parametrize("N", [1, 2, 33, 257, 700, 1100])
+def test_sorted_staging_cluster_with_changeover_and_pairs(N, ipt, S):
+    x, v, m = nb_inputs.random_cluster(N, seed=300 + N, scale=0.2)
+    rng = np.random.default_rng(N)
+    rc = rng.uniform(0.0, 0.06, N)
+    rc[::7] = 0.0
+    _kick_case(x, v, m, rc, dt=0.37, i_per_thread=ipt, sym_block=S, what=f"sorted N={N} I={ipt} S={S}", **SORT)
+
+
+def test_sorted_staging_counts_coincident_and_all_pairs():
+    N = 300
+    x, v, m = nb_inputs.chain_1d(N)
+    for rcv, expect in ((1.5, N - 1), (2.5, 2 * N - 3)):
+        assert _kick_case(x, v, m, np.full(N, rcv), G=1.0, what=f"sorted chain rc={rcv}", **SORT)["n_gpu"] == expect
+    x, v, m = nb_inputs.cubic_lattice(7)
+    assert _kick_case(x, v, m, np.full(343, 1.2), G=1.0, what="sorted lattice", **SORT)["n_gpu"] == 3 * 49 * 6
+    x, v, m = nb_inputs.random_cluster(300, seed=3)
+    x[7] = x[21]; x[40] = x[290]
+    assert _kick_case(x, v, m, np.full(300, 0.01), what="sorted coincident rc>0", **SORT)["n_gpu"] >= 2
+    _kick_case(x, v, m, np.zeros(300), what="sorted coincident rc=0", **SORT)
+    N = 700
+    x, v, m = nb_inputs.random_cluster(N, seed=23, scale=0.05)
+    assert _kick_case(x, v, m, np.full(N, 10.0), what="sorted all pairs", pair_capacity=1 << 19, **SORT)["n_gpu"] == N * (N - 1) // 2
+
+
+@pytest.mark.parametrize("cfg,n_override,n1,n2", [(0, 2048, 3.0, 0.4), (1, 3000, 3.0, 0.4), (2, 4096, 30.0, 0.0), (4, 5000, 3.0, 0.0)])
+def test_sorted_staging_disk_configs_reduced(cfg, n_override, n1, n2):
+    """Disks are where the order matters: most super-tiles skip the test, the near-diagonal ones and the ones that hold a
+    giant planet (critical radius ~1 AU) do not."""
+    d = nb_inputs.make_config(cfg, n_override=n_override)
+    rc = oracle.rcrit(d.x, d.v, d.m, d.M_star, d.dt, G_GAUSS, n1, n2)
+    for S in (256, 512):
+        info = _kick_case(d.x, d.v, d.m, rc, dt=0.5 * d.dt, sym_block=S, what=f"sorted {d.name} S={S}", **SORT)
+        assert info["n_sure"] > 0
+
+
+@pytest.mark.parametrize("nsteps", [3, 100])
+def test_sorted_staging_step_matches_oracle_and_is_reproducible(nsteps):
+    d = nb_inputs.make_config(1, n_override=1498)
+    out = []
+    for _ in range(2):
+        st = GpuState(d.x, d.v, d.m, d.M_star, G=G_GAUSS, n1=3.0, n2=0.4, sym_block=256, **SORT)
+        st.step(d.dt, nsteps)
+        out.append(st.host())
+    assert all(np.array_equal(a, b) for a, b in zip(out[0], out[1])), "sorted staging is not run-to-run reproducible"
+    xg, vg, ag, rcg = out[0]
+    ref = oracle.step(d.x, d.v, d.m, d.M_star, d.dt, G_GAUSS, nsteps, n1=3.0, n2=0.4)
+    tol = 1e-13 if nsteps <= 3 else 1e-9
+    assert np.max(np.abs(xg - ref["x"])) <= tol * np.max(np.abs(ref["x"]))
+    assert np.max(np.abs(vg - ref["v"])) <= tol * np.max(np.abs(ref["v"]))
+    acc_ref, ab, _ = oracle.accel(xg, d.m, rcg, G_GAUSS, want_abs=True)
+    assert_acc_close(ag, acc_ref, f"sorted step x{nsteps}: final acc", ab)
+    sure, border = oracle.pairs(xg, rcg)
+    gp, n = st.get_pairs()
+    assert_pairs_match(gp, n, sure, border, f"sorted step x{nsteps}")
+
+
+def test_sorted_staging_with_encounters_resolved():
+    d = nb_inputs.make_config(1, n_override=900)
+    st = GpuState(d.x, d.v, d.m, d.M_star, G=G_GAUSS, n1=3.0, n2=0.4, resolve_encounters=True, pair_capacity=1 << 16,
+                  sym_block=256, **SORT)
+    st.step(d.dt, 10)
+    xg, vg, _, _ = st.host()
+    ref = oracle.step_enc(d.x, d.v, d.m, d.M_star, d.dt, G_GAUSS, 10, n1=3.0, n2=0.4)
+    assert ref["stats"]["integrated"] > 0
+    assert np.max(np.abs(xg - ref["x"])) <= 1e-9 * np.max(np.abs(ref["x"]))
+    assert np.max(np.abs(vg - ref["v"])) <= 1e-9 * np.max(np.abs(ref["v"]))
