@@ -414,7 +414,10 @@ def run_cuda(args):
                       peak_measured_dfma=peak_tf, frac_of_measured_dfma=achieved_tf / peak_tf if peak_tf > 0 else None,
                       fp64_pipe_instr_per_interaction=pipe_instr,
                       fp64_pipe_util_est=pipe_instr * inter_per_step / (force_avg_ms * 1e-3) / (peak_tf * 1e12 / 2.0) if peak_tf > 0 else None),
-        clocks=clocks, gpu_launches=5 * K,  # per timed step: opening half-kick, drift, prep, force, slot sum + closing half-kick
+        clocks=clocks,
+        # per timed step: opening half-kick, drift, prep, force, slot sum + closing half-kick; with the Newton-III kernel's
+        # sorted staging (automatic for N >= 32768) also five sort kernels and the bounds kernel
+        gpu_launches=(11 if (geom.tile_j < 0 and N >= 32768) else 5) * K,
         groups=groups_info,
     )
     if e2e:
