@@ -83,8 +83,6 @@ typedef struct nb_config {
                                 as left by the previous nb_step/nb_kick(dt=0) call on this state: skip the
                                 evaluation at t0, so a run stepped in chunks costs one evaluation per step
                                 (default 0) */
-    int ctas_per_sm;         /* tuning: register cap of the force kernel, CTAs of 128 threads per SM (2..6), 0 = auto */
-    int pipeline_j;          /* tuning: 1 = software-pipelined j loop in the force kernel (default 0) */
     int time_force;          /* bracket every force-tile launch with CUDA events (nb_force_time); implies
                                 no graph replay (default 0) */
     int force_kernel;        /* NB_FORCE_AUTO (default), NB_FORCE_TILES, NB_FORCE_SYMMETRIC (see below) */

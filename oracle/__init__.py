@@ -38,6 +38,9 @@ def _L():
         dp, ip, lp = C.POINTER(C.c_double), C.POINTER(C.c_int32), C.POINTER(C.c_int64)
         i64, dbl, i32 = C.c_int64, C.c_double, C.c_int
         lib.oracle_num_threads.restype = i32
+        lib.oracle_long_double_digits.restype = i32
+        lib.oracle_encounter_rhs.argtypes = [dp, i32, dp, dp, i32, dbl, i32, dp]
+        lib.oracle_level_kick.argtypes = [dp, dp, dp, i64, dbl, i32, ip, i64, dp, i64, dbl]
         lib.oracle_set_num_threads.argtypes = [i32]
         lib.oracle_changeover.restype = dbl
         lib.oracle_changeover.argtypes = [dbl, dbl, i32]
@@ -55,8 +58,8 @@ def _L():
         lib.oracle_step.restype = i64
         lib.oracle_step.argtypes = [dp, dp, dp, dbl, i64, i64, dbl, dbl, dbl, dbl, i32, dp, dp, i64]
         lib.oracle_diagnostics.argtypes = [dp, dp, dp, dbl, i64, dbl, dp]
-        lib.oracle_encounter.argtypes = [dp, dp, dp, dp, i64, dbl, dbl, dbl, i32, dbl, ip, ip, i64, i64, lp]
-        lib.oracle_encounter_split.argtypes = [dp, dp, dp, dp, i64, i64, dbl, dbl, dbl, i32, dbl, ip, ip, i64, i64, lp]
+        lib.oracle_encounter.argtypes = [dp, dp, dp, dp, i64, i64, dbl, dbl, dbl, i32, dbl, ip, ip, i64, i64, lp]
+        lib.oracle_encounter_split.argtypes = [dp, dp, dp, dp, i64, i64, dbl, dbl, dbl, i32, dbl, ip, ip, i64, i64, i64, lp]
         lib.oracle_groups.restype = i32
         lib.oracle_groups.argtypes = [ip, i64, i64, ip, ip, ip, lp]
         _lib = lib
@@ -81,6 +84,11 @@ def num_threads() -> int:
 
 def set_num_threads(n: int) -> None:
     _L().oracle_set_num_threads(int(n))
+
+
+def long_double_digits() -> int:
+    """Significand bits of the type oracle_accel sums in (64 on x86-64; see the header of nb_oracle.c)."""
+    return int(_L().oracle_long_double_digits())
 
 
 def changeover(r: float, rc: float, kind: int = 0) -> float:
@@ -221,31 +229,53 @@ def groups(pairs_, N):
                 largest=int(gstat[2]))
 
 
-def encounter(x, v, m, rcrit_, M_star, dt, G, grp, kind=0, tol=1e-12, max_group=1024, n_active=0):
+def encounter_rhs(x, v, gm, rc, mu, kind=0):
+    """Right-hand side of the group equations of motion (Eq. 4): returns (dx/dt, dv/dt) of the n bodies
+    of ONE group, dv/dt = -mu x/r^3 + sum_j gm_j [1 - W(r_ij; max(rc_i, rc_j))] (x_j - x_i)/r_ij^3.  rc may be [nlev, n]
+    (multi-level scheme: the pair term carries the product of the levels' [1 - W_k])."""
+    x = np.ascontiguousarray(x, dtype=np.float64); v = np.ascontiguousarray(v, dtype=np.float64)
+    n = x.shape[0]
+    y = np.concatenate([x.reshape(-1), v.reshape(-1)])
+    gm = np.ascontiguousarray(gm, dtype=np.float64); rc = np.ascontiguousarray(rc, dtype=np.float64).reshape(-1, n)
+    f = np.empty(6 * n)
+    dp = C.POINTER(C.c_double)
+    _L().oracle_encounter_rhs(y.ctypes.data_as(dp), n, gm.ctypes.data_as(dp), rc.ctypes.data_as(dp), rc.shape[0], float(mu),
+                              int(kind), f.ctypes.data_as(dp))
+    return f[:3 * n].reshape(n, 3), f[3 * n:].reshape(n, 3)
+
+
+def encounter(x, v, m, rcrit_, M_star, dt, G, grp, kind=0, tol=1e-12, max_group=1024, n_active=0, split_max_core=-1):
     """H_A with encounters (Eq. 4, 98, 106): the members of every group of `grp` (a dict from
     groups()) are advanced by dt with the Bulirsch-Stoer integrator; returns (x, v, stats) with
-    stats = dict(integrated, skipped, failed, steps)."""
+    stats = dict(integrated, skipped, failed, steps).  Semi-active mode (0 < n_active < N, reading S22): every
+    group that has test particles is split into its active core and independent {core + particle} problems;
+    split_max_core >= 0 restricts the splitting to cores of at most that many members (what an implementation
+    with a bounded core size does; the tests pass the CUDA path's bound)."""
     x = np.array(x, dtype=np.float64, order="C"); v = np.array(v, dtype=np.float64, order="C")
-    m = np.ascontiguousarray(m, dtype=np.float64); rc = np.ascontiguousarray(rcrit_, dtype=np.float64)
+    m = np.ascontiguousarray(m, dtype=np.float64)
     N = m.shape[0]
+    rc = np.ascontiguousarray(rcrit_, dtype=np.float64).reshape(-1, N)     # [nlev, N]; nlev = 1: the plain hybrid scheme
+    nlev = rc.shape[0]
     members = np.ascontiguousarray(grp["members"], dtype=np.int32)
     gstart = np.ascontiguousarray(grp["gstart"], dtype=np.int32)
     stats = np.zeros(4, dtype=np.int64)
     dp, ip, lp = C.POINTER(C.c_double), C.POINTER(C.c_int32), C.POINTER(C.c_int64)
     if 0 < int(n_active) < N:
+        if nlev != 1:
+            raise ValueError("the multi-level scheme is defined for the fully active case only")
         # semi-active mode: cores and test particles are integrated separately (oracle_encounter_split)
         _L().oracle_encounter_split(x.ctypes.data_as(dp), v.ctypes.data_as(dp), m.ctypes.data_as(dp), rc.ctypes.data_as(dp),
                                     N, int(n_active), float(M_star), float(G), float(dt), int(kind), float(tol),
                                     members.ctypes.data_as(ip), gstart.ctypes.data_as(ip), int(grp["ngroups"]),
-                                    int(max_group), stats.ctypes.data_as(lp))
+                                    int(max_group), int(split_max_core), stats.ctypes.data_as(lp))
     else:
-        _L().oracle_encounter(x.ctypes.data_as(dp), v.ctypes.data_as(dp), m.ctypes.data_as(dp), rc.ctypes.data_as(dp), N,
+        _L().oracle_encounter(x.ctypes.data_as(dp), v.ctypes.data_as(dp), m.ctypes.data_as(dp), rc.ctypes.data_as(dp), nlev, N,
                               float(M_star), float(G), float(dt), int(kind), float(tol), members.ctypes.data_as(ip),
                               gstart.ctypes.data_as(ip), int(grp["ngroups"]), int(max_group), stats.ctypes.data_as(lp))
     return x, v, dict(integrated=int(stats[0]), skipped=int(stats[1]), failed=int(stats[2]), steps=int(stats[3]))
 
 
-def step_enc(x, v, m, M_star, dt, G, nsteps, n1=3.0, n2=0.4, kind=0, tol=1e-12, max_group=1024, n_active=0):
+def step_enc(x, v, m, M_star, dt, G, nsteps, n1=3.0, n2=0.4, kind=0, tol=1e-12, max_group=1024, n_active=0, split_max_core=-1):
     """nsteps of B(dt/2) C(dt/2) A(dt) C(dt/2) B(dt/2) with close encounters resolved:
     in A the members of the encounter groups of the step's opening pair list (groups of at most max_group
     bodies) are propagated by encounter(), every other body by the Kepler drift.  Composed of the pinned
@@ -270,14 +300,15 @@ def step_enc(x, v, m, M_star, dt, G, nsteps, n1=3.0, n2=0.4, kind=0, tol=1e-12, 
         x = shift(x, v, m, M_star, 0.5 * dt)
         grp = groups(pr, N)
         xk, vk, nfail = drift_kepler(x, v, M_star, dt, G)
-        xe, ve, st = encounter(x, v, m, rc, M_star, dt, G, grp, kind=kind, tol=tol, max_group=max_group, n_active=n_active)
+        xe, ve, st = encounter(x, v, m, rc, M_star, dt, G, grp, kind=kind, tol=tol, max_group=max_group, n_active=n_active,
+                               split_max_core=split_max_core)
         moved = np.zeros(N, dtype=bool)
         for g in range(grp["ngroups"]):
             seg = grp["members"][grp["gstart"][g]:grp["gstart"][g + 1]]
             size = seg.shape[0]
             if 0 < n_active < N:
                 nc = int(np.count_nonzero(seg < n_active))
-                if nc <= 31 and nc < size:
+                if nc < size and (split_max_core < 0 or nc <= split_max_core):
                     size = nc                      # split group: only the core counts against max_group
             if size <= max_group:
                 moved[seg] = True
@@ -289,6 +320,161 @@ def step_enc(x, v, m, M_star, dt, G, nsteps, n1=3.0, n2=0.4, kind=0, tol=1e-12, 
         rc, acc, pr = evaluate(x, v)
         v = v + (0.5 * dt) * acc
     return dict(x=x, v=v, acc=acc, rcrit=rc, pairs=pr, stats=tot)
+
+
+# ---------------------------------------------------------------------------------------------------------------------
+# Multi-level changeover (reading S23).  The statement of the recursion; the arithmetic pieces
+# are the C functions above (oracle_level_kick, oracle_drift_kepler, oracle_encounter with level radii, oracle_groups).
+# ---------------------------------------------------------------------------------------------------------------------
+def level_rcrit(x, v, m, M_star, dt, G, n1, n2, nlev, rcrit0=None):
+    """Critical radii of the levels 0 .. nlev-1, [nlev, N]: Eq. 7 evaluated with the level's own time step
+    dt / 2^l -- "a second term is used to increase the critical radius in situations where too few steps are used
+    through the changeover function", so the velocity term shrinks with the step while the Hill term
+    stays.  n1 == n2 == 0 (caller's radii, rcrit0): rc_l = rcrit0 / 2^l."""
+    if n1 == 0.0 and n2 == 0.0:
+        return np.stack([np.asarray(rcrit0, dtype=np.float64) / 2.0 ** l for l in range(nlev)])
+    return np.stack([rcrit(x, v, m, M_star, dt / 2.0 ** l, G, n1, n2) for l in range(nlev)])
+
+
+def level_weights(r, rcs, kind=0):
+    """Share of the Newtonian pair force each operator carries at separation r, for pairwise level radii rcs[0..L]:
+    [W_0, Omega_0 W_1, ..., Omega_{L-1} W_L, Omega_L] (L + 2 numbers: the outer kick, the L level kicks, the direct
+    solver).  They sum to 1 at every r."""
+    out, om = [], 1.0
+    for rc in rcs:
+        W = changeover(r, rc, kind)
+        out.append(om * W)
+        om = om * (1.0 - W)
+    out.append(om)
+    return out
+
+
+def level_kick(x, v, m, G, pairs_, rcl, level, h, kind=0):
+    """v_i += h sum_{j: {i,j} listed} G m_j Omega_level W_{level+1} (x_j - x_i)/r^3; returns the new v."""
+    x, px = _d(x); m, pm = _d(m)
+    v = np.array(v, dtype=np.float64, order="C", copy=True)
+    N = m.shape[0]
+    p = np.ascontiguousarray(np.asarray(pairs_, dtype=np.int32).reshape(-1, 2))
+    rcl = np.ascontiguousarray(rcl, dtype=np.float64).reshape(-1, N)
+    if rcl.shape[0] < level + 2:
+        raise ValueError("level_kick needs the radii of levels 0 .. level + 1")
+    dp = C.POINTER(C.c_double)
+    _L().oracle_level_kick(px, v.ctypes.data_as(dp), pm, N, float(G), int(kind), p.ctypes.data_as(C.POINTER(C.c_int32)),
+                           p.shape[0], rcl.ctypes.data_as(dp), int(level), float(h))
+    return v
+
+
+def _pairs_within(x, p, rc_level):
+    """Rows of the pair list p whose bodies are closer than max(rc_i, rc_j) of the given level (strict, fp64 on r^2 with
+    the definition's expression), in the order of p."""
+    if p.shape[0] == 0:
+        return p
+    i, j = p[:, 0], p[:, 1]
+    dx = x[j] - x[i]
+    r2 = (dx[:, 0] * dx[:, 0] + dx[:, 1] * dx[:, 1]) + dx[:, 2] * dx[:, 2]
+    rc = np.maximum(rc_level[i], rc_level[j])
+    return p[r2 < rc * rc]
+
+
+def encounter_ml(x, v, m, rcl, M_star, dt, G, pairs0, kind=0, tol=1e-12, max_group=1024):
+    """H_A over dt for the bodies of the pair list pairs0 with L = len(rcl) - 1 intermediate levels (reading S23).
+
+        advance(l, P, tau):                      # Kepler + sum_{pairs in P} (pair force) Omega_l, for the bodies of P
+            if l == L:  Bulirsch-Stoer over tau for the groups of P, pair weight Omega_L         (the direct solver)
+            else twice, with h = tau / 2:
+                P' = pairs of P closer than rc_{l+1} now
+                kick  h/2 with weight Omega_l W_{l+1} over P
+                bodies of P not in P': Kepler drift h;   advance(l + 1, P', h)
+                kick  h/2 with weight Omega_l W_{l+1} over P
+
+    L = 0 is oracle.encounter on the groups of pairs0.  Bodies outside pairs0 are not touched (the caller drifts them).
+    Returns (x, v, stats) with stats = dict(integrated, skipped, failed, steps, kicks, level_pairs[L+1])."""
+    x = np.array(x, dtype=np.float64, order="C"); v = np.array(v, dtype=np.float64, order="C")
+    m = np.ascontiguousarray(m, dtype=np.float64)
+    N = m.shape[0]
+    rcl = np.ascontiguousarray(rcl, dtype=np.float64).reshape(-1, N)
+    L = rcl.shape[0] - 1
+    stats = dict(integrated=0, skipped=0, failed=0, steps=0, kicks=0, level_pairs=[0] * (L + 1))
+    P0 = _canon(np.asarray(pairs0, dtype=np.int32).reshape(-1, 2))
+
+    def bodies(P):
+        return np.unique(P.reshape(-1)) if P.shape[0] else np.zeros(0, dtype=np.int64)
+
+    def advance(l, P, tau):
+        nonlocal x, v
+        stats["level_pairs"][l] += int(P.shape[0])
+        if P.shape[0] == 0:
+            return
+        if l == L:
+            grp = groups(P, N)
+            xe, ve, st = encounter(x, v, m, rcl, M_star, tau, G, grp, kind=kind, tol=tol, max_group=max_group)
+            # groups beyond max_group are left to the Kepler drift (counted), as in step_enc
+            big = np.zeros(N, dtype=bool)
+            for g in range(grp["ngroups"]):
+                seg = grp["members"][grp["gstart"][g]:grp["gstart"][g + 1]]
+                if seg.shape[0] > max_group:
+                    big[seg] = True
+            if big.any():
+                idx = np.flatnonzero(big)
+                xk, vk, _ = drift_kepler(x[idx], v[idx], M_star, tau, G)
+                xe[idx] = xk; ve[idx] = vk
+            x, v = xe, ve
+            for k in ("integrated", "skipped", "failed", "steps"):
+                stats[k] += st[k]
+            return
+        h = 0.5 * tau
+        for _ in range(2):
+            Pn = _pairs_within(x, P, rcl[l + 1])
+            v = level_kick(x, v, m, G, P, rcl, l, 0.5 * h, kind)
+            outer = np.setdiff1d(bodies(P), bodies(Pn))
+            if outer.size:
+                xk, vk, nf = drift_kepler(x[outer], v[outer], M_star, h, G)
+                stats["failed"] += nf
+                x[outer] = xk; v[outer] = vk
+            advance(l + 1, Pn, h)
+            v = level_kick(x, v, m, G, P, rcl, l, 0.5 * h, kind)
+            stats["kicks"] += 2
+
+    advance(0, P0, dt)
+    return x, v, stats
+
+
+def step_ml(x, v, m, M_star, dt, G, nsteps, nlev, n1=3.0, n2=0.4, kind=0, tol=1e-12, max_group=1024, rcrit0=None):
+    """nsteps of B(dt/2) C(dt/2) A(dt) C(dt/2) B(dt/2) with the close encounters of A resolved through nlev - 1 intermediate
+    levels (encounter_ml); nlev = 1 is step_enc.  Level radii by level_rcrit from the state at each force evaluation
+    (S17), held through the step.  Returns dict(x, v, acc, rcrit [nlev, N], pairs, stats)."""
+    x = np.array(x, dtype=np.float64, order="C"); v = np.array(v, dtype=np.float64, order="C")
+    m = np.ascontiguousarray(m, dtype=np.float64)
+    N = m.shape[0]
+    tot = dict(integrated=0, skipped=0, failed=0, steps=0, kicks=0, border=0, level_pairs=[0] * nlev)
+
+    def evaluate(x, v):
+        rcl = level_rcrit(x, v, m, M_star, dt, G, n1, n2, nlev, rcrit0)
+        acc, _, _ = accel(x, m, rcl[0], G, kind=kind)
+        sure, border = pairs(x, rcl[0])
+        tot["border"] += border.shape[0]
+        return rcl, acc, sure
+
+    rcl, acc, pr = evaluate(x, v)
+    for _ in range(int(nsteps)):
+        v = v + (0.5 * dt) * acc
+        x = shift(x, v, m, M_star, 0.5 * dt)
+        inside = np.zeros(N, dtype=bool)
+        inside[pr.reshape(-1)] = True
+        free = np.flatnonzero(~inside)
+        xe, ve, st = encounter_ml(x, v, m, rcl, M_star, dt, G, pr, kind=kind, tol=tol, max_group=max_group)
+        if free.size:
+            xk, vk, nf = drift_kepler(x[free], v[free], M_star, dt, G)
+            xe[free] = xk; ve[free] = vk
+            tot["failed"] += nf
+        x, v = xe, ve
+        for k in ("integrated", "skipped", "failed", "steps", "kicks"):
+            tot[k] += st[k]
+        tot["level_pairs"] = [a + b for a, b in zip(tot["level_pairs"], st["level_pairs"])]
+        x = shift(x, v, m, M_star, 0.5 * dt)
+        rcl, acc, pr = evaluate(x, v)
+        v = v + (0.5 * dt) * acc
+    return dict(x=x, v=v, acc=acc, rcrit=rcl, pairs=pr, stats=tot)
 
 
 def merge(x, v, m, radius, pairs_, f=1.0):

@@ -15,10 +15,15 @@
  *
  * It is the definition written out: explicit loops in the paper's index order, no blocking,
  * no fusion, no FMA contraction (build with -ffp-contract=off).  All inputs and outputs are
- * fp64.  Sums are Neumaier-compensated, and the O(N^2) acceleration sum carries its terms in the
- * host's extended precision (x87 long double) before one final rounding to fp64, so that the
- * whole 1e-12 error budget belongs to the CUDA path.  Decisions that produce integers (the
- * pair test r^2 < rc^2) are taken in plain fp64.  OpenMP parallelises over the OUTER body
+ * fp64.  O(N) sums are Neumaier-compensated, and the O(N^2) acceleration sum carries its terms
+ * in `long double` before one final rounding to fp64, so that the whole 1e-12 error budget
+ * belongs to the CUDA path.  HOST DEPENDENCE: this relies on x86-64, where `long double` is the
+ * x87 80-bit format (64-bit significand); oracle_long_double_digits() reports LDBL_MANT_DIG and
+ * a test requires >= 64 -- on a host whose long double is plain fp64 the oracle would still be
+ * the definition, only with its own rounding (~sqrt(N) eps) inside the tolerance it arbitrates.
+ * It is an extended-precision checker, not a tuned CPU kernel: its interactions/s understate
+ * what a vectorised fp64 CPU code would do by several times.  Decisions that produce integers
+ * (the pair test r^2 < rc^2) are taken in plain fp64.  OpenMP parallelises over the OUTER body
  * index i only; every per-body sum runs sequentially in j order.
  *
  * It shares no code, header, table or helper with paper_2604_09184_b200/ (the CUDA path) and
@@ -30,6 +35,7 @@
  * r_crit,ij and force-vs-potential weighting are "parity unpinned" against the paper (the
  * paper gives no formula for them) -- see DESIGN.md.
  */
+#include <float.h>
 #include <math.h>
 #include <stdint.h>
 #include <stdlib.h>
@@ -47,6 +53,9 @@ int oracle_num_threads(void) {
     return 1;
 #endif
 }
+
+/* significand bits of the type the O(N^2) sum is carried in (64 on x86-64: x87 extended) */
+int oracle_long_double_digits(void) { return LDBL_MANT_DIG; }
 
 void oracle_set_num_threads(int n) {
 #ifdef _OPENMP
@@ -243,22 +252,27 @@ void oracle_shift(double *x, const double *v, const double *m, double M_star, in
  * be solved analytically"; Eq. 4 first sum), advanced with Gauss'
  * f and g functions (BASELINE.json:north_star).
  *
- * Elliptic solver (alpha = 2/r0 - v^2/mu > 0), in the differenced eccentric anomaly dE:
+ * Elliptic solver (alpha = 2/r0 - v^2/mu with alpha r0 >= 0.05), in the differenced eccentric anomaly dE:
  *   a = 1/alpha, n = sqrt(mu/a^3), ec = 1 - r0/a, es = (x.v)/sqrt(mu a),
  *   dM = n h reduced to (-pi, pi],
  *   F(dE) = dE - ec sin dE + es (1 - cos dE) - dM = 0,   F' = r/a > 0   (unique root),
  *   Newton from dE = dM safeguarded by bisection on [dM - 3e, dM + 3e],
  *   c = 2 sin^2(dE/2), s = sin dE, r = a (1 - ec (1 - c) + es s),
  *   f = 1 - (a/r0) c,  g = [(r0/a) s + es c]/n,  fdot = -sqrt(mu a) s/(r r0),  gdot = 1 - (a/r) c.
+ * The elliptic elements lose their meaning as the orbit approaches a parabola (a -> inf: ec -> 1, n h -> 0, and
+ * for alpha = O(eps) by rounding alone the formulas return garbage without noticing -- found by the pin against
+ * numerical integration, tests/test_oracle_pins.py): this solver takes only orbits with r0/a >= 0.05 (every
+ * bound orbit with e <= 0.95 at any phase); the rest goes to the universal-variable solver, which is uniformly
+ * accurate across the parabola (reading S15).
  * Returns 0 on convergence, 1 if 64 iterations did not reach the fixed point (state then
- * left unchanged), 2 if not elliptic (state unchanged).
+ * left unchanged), 2 if not handled here: unbound or near-parabolic (state unchanged).
  * ------------------------------------------------------------------------------------------ */
 int oracle_kepler_elliptic(double *x, double *v, double mu, double h) {
     double r0 = sqrt((x[0] * x[0] + x[1] * x[1]) + x[2] * x[2]);
     double v2 = (v[0] * v[0] + v[1] * v[1]) + v[2] * v[2];
     double u = (x[0] * v[0] + x[1] * v[1]) + x[2] * v[2];
     double alpha = 2.0 / r0 - v2 / mu;
-    if (!(alpha > 0.0)) return 2;
+    if (!(alpha * r0 >= 0.05)) return 2;   /* unbound or near-parabolic (r0/a < 0.05): universal variables */
     double a = 1.0 / alpha;
     double n = sqrt(mu / (a * a * a));
     double ec = 1.0 - r0 / a;
@@ -301,6 +315,7 @@ int oracle_kepler_elliptic(double *x, double *v, double mu, double h) {
 /* Stumpff functions c0..c3 of z (Danby's argument-quartering + series + duplication). */
 static void stumpff(double z, double *c0, double *c1, double *c2, double *c3) {
     int nq = 0;
+    if (!isfinite(z)) { *c0 = *c1 = *c2 = *c3 = NAN; return; }   /* the caller treats it as "beyond the root" */
     while (fabs(z) > 0.1) { z *= 0.25; nq++; }
     /* series: c2 = sum (-z)^k/(2k+2)!, c3 = sum (-z)^k/(2k+3)! */
     double a2 = 1.0 / 2.0, a3 = 1.0 / 6.0, t2 = a2, t3 = a3;
@@ -324,7 +339,13 @@ static void stumpff(double z, double *c0, double *c1, double *c2, double *c3) {
  *    h = r0 G1 + u G2 + mu G3            (universal Kepler equation, dF/ds = r > 0)
  *    r = r0 G0 + u G1 + mu G2
  *    f = 1 - (mu/r0) G2, g = h - mu G3, fdot = -(mu/(r r0)) G1, gdot = 1 - (mu/r) G2.
- * Newton from s = h/r0, safeguarded by an expanding bracket + bisection.
+ * F(s) = r0 G1 + u G2 + mu G3 - h is strictly increasing with F(0) = -h, so the root lies on the
+ * side of sign(h): the bracket starts as [0, +inf) or (-inf, 0].  Newton from s = h/r0, safeguarded
+ * the textbook way: a Newton step is taken only if it stays inside the bracket AND is at most half
+ * the previous step; otherwise the bracket is expanded (while one end is infinite) or bisected.  On
+ * a strongly hyperbolic orbit F grows like exp(sqrt(-beta) s): plain Newton from far beyond the root
+ * creeps by 1/sqrt(-beta) per step, the half-step rule sends those iterations to bisection.  A
+ * non-finite F or r (overflow far beyond the root) counts as "beyond the root".
  * Returns 0 ok, 1 not converged (state unchanged). */
 int oracle_kepler_universal(double *x, double *v, double mu, double h) {
     double r0 = sqrt((x[0] * x[0] + x[1] * x[1]) + x[2] * x[2]);
@@ -332,24 +353,30 @@ int oracle_kepler_universal(double *x, double *v, double mu, double h) {
     double u = (x[0] * v[0] + x[1] * v[1]) + x[2] * v[2];
     double beta = 2.0 * mu / r0 - v2;
     double s = h / r0;
-    double lo = -INFINITY, hi = INFINITY;
+    double lo = (h > 0.0) ? 0.0 : -INFINITY, hi = (h < 0.0) ? 0.0 : INFINITY;
     double c0, c1, c2, c3, G0 = 1, G1 = 0, G2 = 0, G3 = 0, r = r0;
+    double prev = INFINITY;                       /* size of the previous step */
     int converged = 0;
-    for (int it = 0; it < 200; ++it) {
+    if (h == 0.0) return 0;
+    for (int it = 0; it < 300; ++it) {
         stumpff(beta * s * s, &c0, &c1, &c2, &c3);
         G0 = c0; G1 = s * c1; G2 = s * s * c2; G3 = s * s * s * c3;
         double F = r0 * G1 + u * G2 + mu * G3 - h;
         r = r0 * G0 + u * G1 + mu * G2;
+        if (!isfinite(F) || !isfinite(r)) { F = (s > 0.0) ? INFINITY : -INFINITY; r = NAN; }
+        if (F == 0.0) { converged = 1; break; }
         if (F > 0.0) hi = s; else lo = s;
-        double nxt = s - F / r;
-        if (!(nxt > lo && nxt < hi)) {
-            if (isinf(lo)) nxt = (hi == 0.0) ? -1.0 : hi - 2.0 * fabs(hi) - 1e-3;
-            else if (isinf(hi)) nxt = (lo == 0.0) ? 1.0 : lo + 2.0 * fabs(lo) + 1e-3;
+        const double scale = 2.220446049250313e-16 * fmax(fabs(s), fabs(h / r0));
+        double nxt = s - F / r;                    /* Newton */
+        if (fabs(nxt - s) <= scale) { s = nxt; converged = 1; break; }   /* F is monotone: s is the root to rounding */
+        if (!(nxt > lo && nxt < hi) || 2.0 * fabs(nxt - s) > prev) {
+            if (isinf(lo)) nxt = hi - 2.0 * fabs(hi) - 1e-3;
+            else if (isinf(hi)) nxt = lo + 2.0 * fabs(lo) + 1e-3;
             else nxt = 0.5 * (lo + hi);
         }
-        double delta = nxt - s;
+        prev = fabs(nxt - s);
+        if (prev <= scale) { s = nxt; converged = 1; break; }            /* the bracket has collapsed */
         s = nxt;
-        if (fabs(delta) <= 2.220446049250313e-16 * fmax(fabs(s), fabs(h / r0))) { converged = 1; break; }
     }
     if (!converged) return 1;
     stumpff(beta * s * s, &c0, &c1, &c2, &c3);
@@ -359,6 +386,7 @@ int oracle_kepler_universal(double *x, double *v, double mu, double h) {
     double g = h - mu * G3;
     double fd = -(mu / (r * r0)) * G1;
     double gd = 1.0 - (mu / r) * G2;
+    if (!(isfinite(f) && isfinite(g) && isfinite(fd) && isfinite(gd))) return 1;
     for (int k = 0; k < 3; ++k) {
         double xn = f * x[k] + g * v[k];
         double vn = fd * x[k] + gd * v[k];
@@ -556,8 +584,10 @@ static double one_minus_changeover(double r, double rc, int kind) {
     return (z * z) / (2.0 * y * y - 2.0 * y + 1.0);                    /* 1 - y^2/(2y^2 - 2y + 1)   */
 }
 
-/* y = (x[3n], v[3n]) -> f = (v, a) */
-static void group_rhs(const double *y, double *f, int n, const double *gm, const double *rc, double mu, int kind) {
+/* y = (x[3n], v[3n]) -> f = (v, a).  rc holds nlev critical radii per member, level-major (rc[k*n + i]); the pair
+ * term carries the product over the levels k = 0 .. nlev-1 of [1 - W(r; rc_k,ij)]: nlev = 1 is Eq. 4 as printed, nlev > 1
+ * is the innermost Hamiltonian of the multi-level scheme (oracle_level_kick below). */
+static void group_rhs(const double *y, double *f, int n, const double *gm, const double *rc, int nlev, double mu, int kind) {
     const double *x = y, *v = y + 3 * n;
     for (int i = 0; i < n; ++i) {
         double r2 = (x[3 * i] * x[3 * i] + x[3 * i + 1] * x[3 * i + 1]) + x[3 * i + 2] * x[3 * i + 2];
@@ -569,8 +599,11 @@ static void group_rhs(const double *y, double *f, int n, const double *gm, const
             double d2 = (dx * dx + dy * dy) + dz * dz;
             if (d2 == 0.0) continue;                       /* coincident: no direction, contributes nothing */
             double d = sqrt(d2);
-            double rcij = rc[i] > rc[j] ? rc[i] : rc[j];
-            double w = one_minus_changeover(d, rcij, kind);
+            double w = 1.0;
+            for (int k = 0; k < nlev && w != 0.0; ++k) {
+                double rcij = rc[k * n + i] > rc[k * n + j] ? rc[k * n + i] : rc[k * n + j];
+                w = w * one_minus_changeover(d, rcij, kind);
+            }
             if (w == 0.0) continue;
             double t = gm[j] * w / (d2 * d);
             ax += t * dx; ay += t * dy; az += t * dz;
@@ -580,9 +613,15 @@ static void group_rhs(const double *y, double *f, int n, const double *gm, const
     }
 }
 
+/* The right-hand side above for one group, exported so that the tests can pin the [1 - W] pair term
+ * directly (it must equal (1 - oracle_changeover) G m_j / r^2, and kick + encounter = Newton). */
+void oracle_encounter_rhs(const double *y, int n, const double *gm, const double *rc, int nlev, double mu, int kind, double *f) {
+    group_rhs(y, f, n, gm, rc, nlev, mu, kind);
+}
+
 #define BS_COLS 8
 
-int64_t oracle_encounter_group(double *y, int n, const double *gm, const double *rc, double mu, int kind,
+int64_t oracle_encounter_group(double *y, int n, const double *gm, const double *rc, int nlev, double mu, int kind,
                                double dt, double tol) {
     const int dim = 6 * n;
     double *buf = (double *)malloc(sizeof(double) * (size_t)dim * (5 + BS_COLS));
@@ -594,17 +633,17 @@ int64_t oracle_encounter_group(double *y, int n, const double *gm, const double 
     while (t != dt) {
         if (fabs(h) > fabs(dt - t)) h = dt - t;
         if (fabs(h) < 1e-14 * fabs(dt)) { free(buf); return -1; }
-        group_rhs(y, f0, n, gm, rc, mu, kind);
+        group_rhs(y, f0, n, gm, rc, nlev, mu, kind);
         int accepted = 0, cols = 0;
         for (int c = 1; c <= BS_COLS && !accepted; ++c) {
             const int nsub = 2 * c;
             const double hs = h / nsub;
             for (int k = 0; k < dim; ++k) { ym[k] = y[k]; yn[k] = y[k] + hs * f0[k]; }
             for (int s = 2; s <= nsub; ++s) {
-                group_rhs(yn, f, n, gm, rc, mu, kind);
+                group_rhs(yn, f, n, gm, rc, nlev, mu, kind);
                 for (int k = 0; k < dim; ++k) { tmp[k] = ym[k] + 2.0 * hs * f[k]; ym[k] = yn[k]; yn[k] = tmp[k]; }
             }
-            group_rhs(yn, f, n, gm, rc, mu, kind);
+            group_rhs(yn, f, n, gm, rc, nlev, mu, kind);
             /* new tableau row: tmp[] runs along the row, T[] holds the previous row */
             double err2 = 0.0;
             for (int k = 0; k < dim; ++k) {
@@ -654,22 +693,23 @@ int64_t oracle_encounter_group(double *y, int n, const double *gm, const double 
  * them), one after the other; x, v of the members are advanced in place by dt under H_A with
  * encounters, every other body is left alone.  stats = {groups integrated, groups skipped because they
  * exceed max_group, groups whose step size underflowed (left unchanged), accepted steps in total}. */
-void oracle_encounter(double *x, double *v, const double *m, const double *rcrit, int64_t N, double M_star,
+void oracle_encounter(double *x, double *v, const double *m, const double *rcrit, int64_t nlev, int64_t N, double M_star,
                       double G, double dt, int kind, double tol, const int32_t *members, const int32_t *gstart,
                       int64_t ngroups, int64_t max_group, int64_t *stats) {
-    (void)N;
+    /* rcrit: [nlev][N] critical radii, level-major (nlev = 1: the plain hybrid scheme) */
     stats[0] = stats[1] = stats[2] = stats[3] = 0;
     for (int64_t g = 0; g < ngroups; ++g) {
         const int n = gstart[g + 1] - gstart[g];
         if (n > max_group) { stats[1]++; continue; }
-        double *y = (double *)malloc(sizeof(double) * (size_t)(8 * n));
+        double *y = (double *)malloc(sizeof(double) * (size_t)((7 + nlev) * n));
         double *gm = y + 6 * n, *rc = y + 7 * n;
         for (int k = 0; k < n; ++k) {
             const int32_t b = members[gstart[g] + k];
             for (int c = 0; c < 3; ++c) { y[3 * k + c] = x[3 * (int64_t)b + c]; y[3 * n + 3 * k + c] = v[3 * (int64_t)b + c]; }
-            gm[k] = G * m[b]; rc[k] = rcrit[b];
+            gm[k] = G * m[b];
+            for (int64_t l = 0; l < nlev; ++l) rc[l * n + k] = rcrit[l * N + b];
         }
-        const int64_t st = oracle_encounter_group(y, n, gm, rc, G * M_star, kind, dt, tol);
+        const int64_t st = oracle_encounter_group(y, n, gm, rc, (int)nlev, G * M_star, kind, dt, tol);
         if (st < 0) { stats[2]++; free(y); continue; }
         for (int k = 0; k < n; ++k) {
             const int32_t b = members[gstart[g] + k];
@@ -683,22 +723,26 @@ void oracle_encounter(double *x, double *v, const double *m, const double *rcrit
 /* Semi-active mode (the first n_active bodies exert force, the others only feel it; BASELINE.json:north_star,
  * DESIGN.md readings S13, S22).  A test particle pulls on nobody, so inside a group the active members (the
  * "core"; the first members of the group, since members ascend) move exactly as if the test particles were not
- * there, and the test particles are mutually independent.  A group with at most 31 active members is therefore
+ * there, and the test particles are mutually independent.  A group that has test particles is therefore
  * split: the core is integrated alone, and every test particle s is integrated together with the core
- * (core + s, from the same initial state), of which only s is kept.  Groups whose core is larger are treated as
- * one problem, as in oracle_encounter.  max_group bounds the core (split groups) or the group (unsplit ones).
+ * (core + s, from the same initial state), of which only s is kept.  split_max_core < 0 (the definition): every
+ * such group is split; split_max_core >= 0: only groups whose core has at most that many members are split, the
+ * others are treated as one problem, as in oracle_encounter (an implementation may stop splitting at some core
+ * size; the two treatments agree to the Bulirsch-Stoer tolerance, not bit for bit).
+ * max_group bounds the core (split groups) or the group (unsplit ones).
  * stats = {groups integrated, groups skipped, sub-integrations whose step size underflowed (body/core left
  * unchanged), accepted steps in total}. */
 void oracle_encounter_split(double *x, double *v, const double *m, const double *rcrit, int64_t N, int64_t n_active,
                             double M_star, double G, double dt, int kind, double tol, const int32_t *members,
-                            const int32_t *gstart, int64_t ngroups, int64_t max_group, int64_t *stats) {
+                            const int32_t *gstart, int64_t ngroups, int64_t max_group, int64_t split_max_core,
+                            int64_t *stats) {
     (void)N;
     stats[0] = stats[1] = stats[2] = stats[3] = 0;
     for (int64_t g = 0; g < ngroups; ++g) {
         const int g0 = gstart[g], n = gstart[g + 1] - g0;
         int nc = 0;
         while (nc < n && members[g0 + nc] < n_active) ++nc;
-        const int split = (nc <= 31 && nc < n);
+        const int split = (nc < n && (split_max_core < 0 || nc <= split_max_core));
         if ((split ? nc : n) > max_group) { stats[1]++; continue; }
         const int nn = split ? nc + 1 : n;                   /* size of the largest sub-problem */
         double *y = (double *)malloc(sizeof(double) * (size_t)(8 * nn));
@@ -715,7 +759,7 @@ void oracle_encounter_split(double *x, double *v, const double *m, const double 
                 for (int c = 0; c < 3; ++c) { y[3 * k + c] = x0[3 * src + c]; y[3 * nb + 3 * k + c] = v0[3 * src + c]; }
                 gm[k] = G * m[b]; rc[k] = rcrit[b];
             }
-            const int64_t st = oracle_encounter_group(y, nb, gm, rc, G * M_star, kind, dt, tol);
+            const int64_t st = oracle_encounter_group(y, nb, gm, rc, 1, G * M_star, kind, dt, tol);
             if (st < 0) { stats[2]++; continue; }
             stats[3] += st;
             const int first = (split && sub > 0) ? nc : 0;   /* a satellite sub-problem keeps only the satellite */
@@ -728,4 +772,48 @@ void oracle_encounter_split(double *x, double *v, const double *m, const double 
         stats[0]++;
         free(y); free(x0);
     }
+}
+
+
+/* ---------------------------------------------------------------------------------------------
+ * Multi-level changeover ("introducing higher-level changeover functions ... to not switch from the
+ * symplectic integrator directly to the direct integrator but to introduce intermediate phases, where the symplectic
+ * integrator reduces the time step level by level for the affected bodies.  Only the last level is then performed with
+ * the inner direct integrator.  Every level needs again a smooth changeover function").  DESIGN.md reading S23: the
+ * hybrid split of PAPER.md:84-86 (Eq. 4, 5) is applied again to H_A, level after level.  With W_k(r) = W(r; rc_k,ij) the
+ * kick weight of level k (critical radii rc_k = Eq. 7 evaluated with the level's time step dt / 2^k) and
+ *     Omega_l(r) = prod_{k=0..l} [1 - W_k(r)]        (what is left of a pair force after levels 0 .. l took their share)
+ * the level-(l+1) kick Hamiltonian carries the pair force weighted by Omega_l W_{l+1} and the level-(l+1) "H_A" the
+ * pair force weighted by Omega_{l+1}; at every r:  W_0 + Omega_0 W_1 + ... + Omega_{L-1} W_L + Omega_L = 1.
+ *
+ * oracle_level_kick: v_i += h * sum_{j : {i,j} in pairs} G m_j Omega_level(r_ij) W_{level+1}(r_ij) (x_j - x_i)/r_ij^3
+ * for the listed pairs only (the pairs in a close encounter at this level; for every other pair Omega_level = 0 at the
+ * moment the list was made).  rcl: [nlev][N] level-major, nlev >= level + 2.  The pair terms of a body are summed in the
+ * order of the list, the sum is applied with one rounding (as in oracle_kick).  A massless body pulls on nobody.
+ * --------------------------------------------------------------------------------------------- */
+void oracle_level_kick(const double *x, double *v, const double *m, int64_t N, double G, int kind, const int32_t *pairs,
+                       int64_t npairs, const double *rcl, int64_t level, double h) {
+    double *acc = (double *)calloc((size_t)(3 * N > 0 ? 3 * N : 1), sizeof(double));
+    for (int64_t p = 0; p < npairs; ++p) {
+        const int64_t i = pairs[2 * p], j = pairs[2 * p + 1];
+        const double dx = x[3 * j] - x[3 * i], dy = x[3 * j + 1] - x[3 * i + 1], dz = x[3 * j + 2] - x[3 * i + 2];
+        const double r2 = (dx * dx + dy * dy) + dz * dz;
+        if (r2 == 0.0) continue;
+        const double r = sqrt(r2);
+        double w = 1.0;
+        for (int64_t k = 0; k <= level && w != 0.0; ++k) {
+            const double rck = rcl[k * N + i] > rcl[k * N + j] ? rcl[k * N + i] : rcl[k * N + j];
+            w = w * one_minus_changeover(r, rck, kind);
+        }
+        if (w == 0.0) continue;
+        const double rcn = rcl[(level + 1) * N + i] > rcl[(level + 1) * N + j] ? rcl[(level + 1) * N + i] : rcl[(level + 1) * N + j];
+        w = w * oracle_changeover(r, rcn, kind);
+        if (w == 0.0) continue;
+        const double f = w / (r2 * r);
+        const double fi = G * m[j] * f, fj = G * m[i] * f;
+        acc[3 * i] += fi * dx; acc[3 * i + 1] += fi * dy; acc[3 * i + 2] += fi * dz;
+        acc[3 * j] -= fj * dx; acc[3 * j + 1] -= fj * dy; acc[3 * j + 2] -= fj * dz;
+    }
+    for (int64_t k = 0; k < 3 * N; ++k) v[k] = v[k] + h * acc[k];
+    free(acc);
 }

@@ -42,8 +42,6 @@ class NbConfig(C.Structure):
         ("j_splits", C.c_int),
         ("use_graph", C.c_int),
         ("reuse_acc", C.c_int),
-        ("ctas_per_sm", C.c_int),
-        ("pipeline_j", C.c_int),
         ("time_force", C.c_int),
         ("force_kernel", C.c_int),
         ("sym_block", C.c_int),
@@ -157,8 +155,8 @@ def default_config() -> NbConfig:
 
 
 def configure(N=None, *, stream=None, pair_capacity=0, n_active=0, G=None, n1=3.0, n2=0.4, changeover_kind=0,
-              i_per_thread=0, j_splits=0, use_graph=True, reuse_acc=False, time_force=False, ctas_per_sm=0,
-              pipeline_j=0, force_kernel=0, sym_block=0, resolve_encounters=False, bs_tol=1e-12, radius_factor=1.0, sort_staging=0, workspace_bytes=None,
+              i_per_thread=0, j_splits=0, use_graph=True, reuse_acc=False, time_force=False,
+              force_kernel=0, sym_block=0, resolve_encounters=False, bs_tol=1e-12, radius_factor=1.0, sort_staging=0, workspace_bytes=None,
               device="cuda"):
     """nb_configure with a torch-allocated workspace sized for N bodies (N=None: no workspace,
     enough for the _host calls; workspace_bytes: explicit size, e.g. the head that the O(N) calls
@@ -175,7 +173,6 @@ def configure(N=None, *, stream=None, pair_capacity=0, n_active=0, G=None, n1=3.
     cfg.use_graph = 1 if use_graph else 0
     cfg.reuse_acc = 1 if reuse_acc else 0
     cfg.time_force = 1 if time_force else 0
-    cfg.ctas_per_sm, cfg.pipeline_j = int(ctas_per_sm), int(pipeline_j)
     cfg.force_kernel, cfg.sym_block = int(force_kernel), int(sym_block)
     cfg.resolve_encounters, cfg.bs_tol = (1 if resolve_encounters else 0), float(bs_tol)
     cfg.radius_factor = float(radius_factor)

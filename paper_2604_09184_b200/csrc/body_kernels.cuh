@@ -189,10 +189,9 @@ __global__ void __launch_bounds__(kBodyThreads) nb_drift_kernel(double *__restri
         // bodies of the encounter groups the direct solver takes (encounter.cuh) are left to it
         const bool in_group = enc_flag != nullptr && enc_flag[i] != 0;
         if (!in_group && kepler_elliptic_fast(X0, X1, X2, V0, V1, V2, mu, dt) != 0) {
-            // rare: not bound, or the fast iteration did not settle -> bracketed solvers (state untouched so far)
+            // rare: unbound, nearly parabolic, or the fast iteration did not settle -> universal variables (state untouched so far)
             double X[3] = {X0, X1, X2}, V[3] = {V0, V1, V2};
-            int rcode = kepler_elliptic(X, V, mu, dt);
-            if (rcode == 2) rcode = kepler_universal(X, V, mu, dt);
+            const int rcode = kepler_universal(X, V, mu, dt);
             if (rcode != 0) status_add(status, ST_KEPLER_FAIL, 1);
             X0 = X[0]; X1 = X[1]; X2 = X[2]; V0 = V[0]; V1 = V[1]; V2 = V[2];
         }

@@ -194,9 +194,8 @@ struct JWork {
     }
 };
 
-// MINB = CTAs per SM the register allocation is capped for; PIPE = software-pipeline the j loop
-// (differences and r^2 of j+1 are issued between the vote on j and its branch).
-template <int I, bool PAIRS, int MINB, bool PIPE>
+// MINB = CTAs per SM the register allocation is capped for.
+template <int I, bool PAIRS, int MINB>
 __global__ void __launch_bounds__(kForceThreads, MINB) nb_force_tiles_kernel(const ForceParams p) {
     __shared__ __align__(128) JRec sm[kStages][kTileJ];
     __shared__ __align__(8) uint64_t full[kStages];
@@ -288,40 +287,17 @@ __global__ void __launch_bounds__(kForceThreads, MINB) nb_force_tiles_kernel(con
             }
         };
 
-        if (PIPE) {
-            // ping-pong between two JWork sets (no register copies): while the vote on j resolves and
-            // its chain drains, the differences and r^2 of j+1 are already in flight
-            JWork<I> wa, wb;
-            wa.load(tile, xi, yi, zi, thr_i);
-#pragma unroll 1
-            for (int jj = 0; jj < kTileJ; jj += 2) {
-                double y0[I];
-#pragma unroll
-                for (int k = 0; k < I; ++k) y0[k] = rsqrt_seed(wa.r2[k]);  // speculative: unused on the slow path
-                const bool hit_a = __any_sync(0xffffffffu, wa.mn <= wa.thr);
-                wb.load(tile + jj + 1, xi, yi, zi, thr_i);
-                if (hit_a) slow_path<I, PAIRS>(p, wa.A, wa.B, jbase + jj, xi, yi, zi, rci, i0, ax, ay, az);
-                else fast(wa, y0);
-#pragma unroll
-                for (int k = 0; k < I; ++k) y0[k] = rsqrt_seed(wb.r2[k]);
-                const bool hit_b = __any_sync(0xffffffffu, wb.mn <= wb.thr);
-                if (jj + 2 < kTileJ) wa.load(tile + jj + 2, xi, yi, zi, thr_i);
-                if (hit_b) slow_path<I, PAIRS>(p, wb.A, wb.B, jbase + jj + 1, xi, yi, zi, rci, i0, ax, ay, az);
-                else fast(wb, y0);
-            }
-        } else {
 #pragma unroll 2
-            for (int jj = 0; jj < kTileJ; ++jj) {
-                JWork<I> cur;
-                cur.load(tile + jj, xi, yi, zi, thr_i);
-                double y0[I];
+        for (int jj = 0; jj < kTileJ; ++jj) {
+            JWork<I> cur;
+            cur.load(tile + jj, xi, yi, zi, thr_i);
+            double y0[I];
 #pragma unroll
-                for (int k = 0; k < I; ++k) y0[k] = rsqrt_seed(cur.r2[k]);
-                if (__any_sync(0xffffffffu, cur.mn <= cur.thr))
-                    slow_path<I, PAIRS>(p, cur.A, cur.B, jbase + jj, xi, yi, zi, rci, i0, ax, ay, az);
-                else
-                    fast(cur, y0);
-            }
+            for (int k = 0; k < I; ++k) y0[k] = rsqrt_seed(cur.r2[k]);
+            if (__any_sync(0xffffffffu, cur.mn <= cur.thr))
+                slow_path<I, PAIRS>(p, cur.A, cur.B, jbase + jj, xi, yi, zi, rci, i0, ax, ay, az);
+            else
+                fast(cur, y0);
         }
 #pragma unroll
         for (int k = 0; k < I; ++k) { ox[k] += ax[k]; oy[k] += ay[k]; oz[k] += az[k]; }

@@ -15,8 +15,9 @@ constexpr double kEps = 2.220446049250313e-16;
 // for the FP64 pipe: no IEEE divide or sqrt (MUFU seeds + one third-order correction, ~1 ulp), ONE
 // library sincos -- of the half angle dE/2, which gives sin dE = 2SC and 1 - cos dE = 2S^2 without
 // cancellation -- and Halley steps whose trigonometric update is a rotation of (S, C) by the small
-// correction.  Anything unusual (not bound, no convergence in 8 steps, non-finite) returns nonzero
-// with the state untouched, and the caller falls back to the bracketed solver.
+// correction.  Anything unusual (not bound or nearly parabolic, no convergence in 8 steps, non-finite)
+// returns nonzero with the state untouched, and the caller falls back to the universal-variable solver
+// below (a different formulation and a different iteration; the oracle's solvers are a third pair).
 
 __device__ __forceinline__ double rcp_fast(const double x) {
     double y;
@@ -48,7 +49,7 @@ __device__ __forceinline__ int kepler_elliptic_fast(double &x0, double &x1, doub
     const double r0 = sqrt_from_rsqrt(rr, ir0);
     const double imu = rcp_fast(mu);
     const double alpha = __fma_rn(-vv, imu, 2.0 * ir0);  // 1/a
-    if (!(alpha > 1e-100 && alpha < 1e100)) return 2;
+    if (!(alpha * r0 >= 0.05 && alpha < 1e100)) return 2;  // unbound or near-parabolic (r0/a < 0.05): universal variables
     const double a = rcp_fast(alpha);
     const double t = mu * alpha;
     const double irt = rsqrt_fast(t);                    // 1/sqrt(mu/a)
@@ -106,119 +107,107 @@ __device__ __forceinline__ int kepler_elliptic_fast(double &x0, double &x1, doub
     return 0;
 }
 
-// Bound orbit (alpha = 2/r0 - v^2/mu > 0), differenced eccentric anomaly dE:
-//   F(dE) = dE - ec sin dE + es (1 - cos dE) - dM = 0,  F' = r/a > 0
-// Newton from dE = dM, kept inside a shrinking bracket [dM - 3e, dM + 3e] by bisection.
-// Returns 0 ok, 1 not converged (state untouched), 2 not elliptic (state untouched).
-__device__ __noinline__ int kepler_elliptic(double (&x)[3], double (&v)[3], const double mu, const double h) {
-    const double r0 = sqrt(x[0] * x[0] + x[1] * x[1] + x[2] * x[2]);
-    const double v2 = v[0] * v[0] + v[1] * v[1] + v[2] * v[2];
-    const double u = x[0] * v[0] + x[1] * v[1] + x[2] * v[2];
-    const double alpha = 2.0 / r0 - v2 / mu;
-    if (!(alpha > 0.0)) return 2;
-    const double a = 1.0 / alpha;
-    const double n = sqrt(mu / (a * a * a));
-    const double ec = 1.0 - r0 / a;
-    const double sma = sqrt(mu * a);
-    const double es = u / sma;
-    const double e = sqrt(ec * ec + es * es);
-    double dM = n * h;
-    dM = dM - kTwoPi * rint(dM / kTwoPi);
-    double lo = dM - 3.0 * e, hi = dM + 3.0 * e;
-    double dE = dM;
-    bool converged = false;
-    for (int it = 0; it < 64; ++it) {
-        double sn, cs;
-        sincos(dE, &sn, &cs);
-        const double F = dE - ec * sn + es * (1.0 - cs) - dM;
-        const double Fp = 1.0 - ec * cs + es * sn;
-        if (F > 0.0) hi = dE; else lo = dE;
-        double nxt = dE - F / Fp;
-        if (!(nxt > lo && nxt < hi)) nxt = 0.5 * (lo + hi);
-        const double delta = nxt - dE;
-        dE = nxt;
-        if (fabs(delta) <= kEps * fmax(1.0, fabs(dE))) { converged = true; break; }
-    }
-    if (!converged) return 1;
-    const double sh = sin(0.5 * dE);
-    const double c = 2.0 * sh * sh;  // 1 - cos dE without cancellation
-    const double s = sin(dE);
-    const double r = a * (1.0 - ec * (1.0 - c) + es * s);
-    const double f = 1.0 - (a / r0) * c;
-    const double g = ((r0 / a) * s + es * c) / n;
-    const double fd = -sma * s / (r * r0);
-    const double gd = 1.0 - (a / r) * c;
+// ---- fall-back for everything the fast path declines: universal variables, Laguerre-Conway ------
+// Any conic (bound, parabolic, hyperbolic), one formulation.  With beta = 2 mu/r0 - v^2, u = x.v and the
+// universal functions G_k(s) = s^k c_k(beta s^2) (c_k: Stumpff functions), Kepler's equation reads
+//     F(s) = r0 G1 + u G2 + mu G3 - h = 0,   F' = r = r0 G0 + u G1 + mu G2 > 0,   F'' = u G0 + (mu - beta r0) G1,
+// and   f = 1 - (mu/r0) G2,  g = h - mu G3,  fdot = -(mu/(r r0)) G1,  gdot = 1 - (mu/r) G2.
+// The Stumpff functions come from their closed forms (circular functions for z > 1, hyperbolic ones for
+// z < -1, the power series in between), the root from Laguerre's iteration of order 5 (Conway's choice
+// for Kepler's equation: cubically convergent near the root and, unlike Newton, not fooled by the
+// exponential growth of F on a hyperbola or by the flat stretches of F near the pericentre of an
+// eccentric orbit), started at s = h/r0 clipped to the large-s asymptote of a hyperbola.  An overflow
+// (far beyond the root) halves s.  If 40 iterations do not settle, the interval [0, s_hi] is bisected
+// (F is monotone, F(0) = -h).  Returns 0 ok, 1 not converged / non-finite input (state untouched).
+__device__ __forceinline__ void stumpff_closed(const double z, double &c0, double &c1, double &c2, double &c3) {
+    if (fabs(z) <= 1.0) {
+        // c2 = sum_k (-z)^k / (2k+2)!,  c3 = sum_k (-z)^k / (2k+3)!;  k <= 10: next term < 1/24! ~ 2e-24
+        const double w = -z;
+        constexpr double k2[11] = {1.0 / 2.0, 1.0 / 24.0, 1.0 / 720.0, 1.0 / 40320.0, 1.0 / 3628800.0, 1.0 / 479001600.0, 1.0 / 87178291200.0, 1.0 / 20922789888000.0, 1.0 / 6402373705728000.0, 1.0 / 2432902008176640000.0, 1.0 / 1124000727777607680000.0};
+        constexpr double k3[11] = {1.0 / 6.0, 1.0 / 120.0, 1.0 / 5040.0, 1.0 / 362880.0, 1.0 / 39916800.0, 1.0 / 6227020800.0, 1.0 / 1307674368000.0, 1.0 / 355687428096000.0, 1.0 / 121645100408832000.0, 1.0 / 51090942171709440000.0, 1.0 / 25852016738884976640000.0};
+        double a2 = k2[10], a3 = k3[10];
 #pragma unroll
-    for (int k = 0; k < 3; ++k) {
-        const double xn = f * x[k] + g * v[k];
-        const double vn = fd * x[k] + gd * v[k];
-        x[k] = xn;
-        v[k] = vn;
+        for (int k = 9; k >= 0; --k) { a2 = __fma_rn(a2, w, k2[k]); a3 = __fma_rn(a3, w, k3[k]); }  // Horner
+        c2 = a2; c3 = a3;
+        c1 = __fma_rn(-z, a3, 1.0);
+        c0 = __fma_rn(-z, a2, 1.0);
+    } else if (z > 0.0) {
+        const double q = sqrt(z);
+        double sn, cs, sh, ch;
+        sincos(q, &sn, &cs);
+        sincos(0.5 * q, &sh, &ch);
+        c0 = cs; c1 = sn / q; c2 = 2.0 * sh * sh / z; c3 = (q - sn) / (z * q);
+    } else {
+        const double q = sqrt(-z);
+        const double sh = sinh(q), hh = sinh(0.5 * q);
+        c0 = cosh(q); c1 = sh / q; c2 = 2.0 * hh * hh / (-z); c3 = (sh - q) / ((-z) * q);
     }
-    return 0;
 }
 
-// Stumpff functions c0..c3(z): quarter the argument until |z| <= 0.1, Taylor series, then the
-// duplication formulas back up.
-__device__ __forceinline__ void stumpff(double z, double &c0, double &c1, double &c2, double &c3) {
-    int nq = 0;
-    while (fabs(z) > 0.1) { z *= 0.25; ++nq; }
-    double a2 = 0.5, a3 = 1.0 / 6.0, t2 = a2, t3 = a3;
-#pragma unroll 1
-    for (int k = 1; k < 12; ++k) {
-        t2 *= -z / ((2.0 * k + 1.0) * (2.0 * k + 2.0));
-        t3 *= -z / ((2.0 * k + 2.0) * (2.0 * k + 3.0));
-        a2 += t2;
-        a3 += t3;
-    }
-    double C2 = a2, C3 = a3, C1 = 1.0 - z * C3, C0 = 1.0 - z * C2;
-    for (; nq > 0; --nq) {
-        C3 = 0.25 * (C2 + C0 * C3);
-        C2 = 0.5 * C1 * C1;
-        C1 = C0 * C1;
-        C0 = 2.0 * C0 * C0 - 1.0;
-    }
-    c0 = C0; c1 = C1; c2 = C2; c3 = C3;
-}
-
-// Any conic, universal variable s with G_k(s) = s^k c_k(beta s^2), beta = 2 mu/r0 - v^2:
-//   h = r0 G1 + u G2 + mu G3   (dh/ds = r > 0),  r = r0 G0 + u G1 + mu G2,
-//   f = 1 - (mu/r0) G2, g = h - mu G3, fdot = -(mu/(r r0)) G1, gdot = 1 - (mu/r) G2.
-// Newton from s = h/r0 with an expanding bracket + bisection.  Returns 0 ok, 1 not converged.
 __device__ __noinline__ int kepler_universal(double (&x)[3], double (&v)[3], const double mu, const double h) {
     const double r0 = sqrt(x[0] * x[0] + x[1] * x[1] + x[2] * x[2]);
     const double v2 = v[0] * v[0] + v[1] * v[1] + v[2] * v[2];
     const double u = x[0] * v[0] + x[1] * v[1] + x[2] * v[2];
     const double beta = 2.0 * mu / r0 - v2;
+    if (!(isfinite(beta) && isfinite(u) && r0 > 0.0 && isfinite(h))) return 1;
+    if (h == 0.0) return 0;
     double s = h / r0;
-    double lo = -INFINITY, hi = INFINITY;
-    double c0, c1, c2, c3;
-    bool converged = false;
-#pragma unroll 1
-    for (int it = 0; it < 200; ++it) {
-        stumpff(beta * s * s, c0, c1, c2, c3);
-        const double G1 = s * c1, G2 = s * s * c2, G3 = s * s * s * c3;
-        const double F = r0 * G1 + u * G2 + mu * G3 - h;
-        const double r = r0 * c0 + u * G1 + mu * G2;
-        if (F > 0.0) hi = s; else lo = s;
-        double nxt = s - F / r;
-        if (!(nxt > lo && nxt < hi)) {
-            if (isinf(lo)) nxt = (hi == 0.0) ? -1.0 : hi - 2.0 * fabs(hi) - 1e-3;
-            else if (isinf(hi)) nxt = (lo == 0.0) ? 1.0 : lo + 2.0 * fabs(lo) + 1e-3;
-            else nxt = 0.5 * (lo + hi);
-        }
-        const double delta = nxt - s;
-        s = nxt;
-        if (fabs(delta) <= kEps * fmax(fabs(s), fabs(h / r0))) { converged = true; break; }
+    if (beta < 0.0) {
+        // hyperbola: for large k|s| (k = sqrt(-beta)) F ~ mu sinh(k s)/k^3, so the root is near asinh(k^3 h/mu)/k
+        const double k = sqrt(-beta);
+        const double cap = 1.5 * asinh(k * k * k * fabs(h) / mu) / k + 1.0 / k;
+        if (fabs(s) > cap) s = copysign(cap, h);
     }
-    if (!converged) return 1;
-    stumpff(beta * s * s, c0, c1, c2, c3);
-    const double G1 = s * c1, G2 = s * s * c2, G3 = s * s * s * c3;
-    const double r = r0 * c0 + u * G1 + mu * G2;
+    const double scale = fabs(h / r0);
+    double c0, c1, c2, c3, G1 = 0.0, G2 = 0.0, G3 = 0.0, r = r0;
+    bool converged = false;
+    double prev = INFINITY;
+#pragma unroll 1
+    for (int it = 0; it < 40; ++it) {
+        stumpff_closed(beta * s * s, c0, c1, c2, c3);
+        G1 = s * c1; G2 = s * s * c2; G3 = s * s * s * c3;
+        const double F = r0 * G1 + u * G2 + mu * G3 - h;
+        r = r0 * c0 + u * G1 + mu * G2;
+        const double Fpp = u * c0 + (mu - beta * r0) * G1;
+        if (!(isfinite(F) && isfinite(r) && isfinite(Fpp))) { s *= 0.5; prev = INFINITY; continue; }
+        if (F == 0.0) { converged = true; break; }
+        const double disc = fabs(16.0 * r * r - 20.0 * F * Fpp);
+        const double den = r + copysign(sqrt(disc), r);
+        const double ds = -5.0 * F / den;
+        if (!isfinite(ds)) { s *= 0.5; prev = INFINITY; continue; }
+        s += ds;
+        const double tol = kEps * fmax(fabs(s), scale);
+        // settled: the step is at rounding level, or it stopped shrinking while already tiny
+        if (fabs(ds) <= 2.0 * tol || (fabs(ds) >= prev && prev <= 512.0 * tol)) { converged = true; break; }
+        prev = fabs(ds);
+    }
+    if (!converged) {
+        // last resort: bisection on the monotone F between 0 and an end found by doubling
+        double lo = 0.0, hi = (h > 0.0) ? fmax(fabs(s), scale) : -fmax(fabs(s), scale);
+        auto Fof = [&](const double ss) {
+            stumpff_closed(beta * ss * ss, c0, c1, c2, c3);
+            const double val = r0 * (ss * c1) + u * (ss * ss * c2) + mu * (ss * ss * ss * c3) - h;
+            return isfinite(val) ? val : copysign(INFINITY, ss);
+        };
+        int guard = 0;
+        while (Fof(hi) * h < 0.0 && ++guard < 64) hi *= 2.0;   // F(hi) must have the sign of h
+        if (guard >= 64) return 1;
+#pragma unroll 1
+        for (int it = 0; it < 200; ++it) {
+            const double mid = 0.5 * (lo + hi);
+            if (mid == lo || mid == hi) break;
+            if (Fof(mid) * h < 0.0) lo = mid; else hi = mid;
+        }
+        s = 0.5 * (lo + hi);
+    }
+    stumpff_closed(beta * s * s, c0, c1, c2, c3);
+    G1 = s * c1; G2 = s * s * c2; G3 = s * s * s * c3;
+    r = r0 * c0 + u * G1 + mu * G2;
     const double f = 1.0 - (mu / r0) * G2;
     const double g = h - mu * G3;
     const double fd = -(mu / (r * r0)) * G1;
     const double gd = 1.0 - (mu / r) * G2;
+    if (!(isfinite(f) && isfinite(g) && isfinite(fd) && isfinite(gd))) return 1;
 #pragma unroll
     for (int k = 0; k < 3; ++k) {
         const double xn = f * x[k] + g * v[k];

@@ -22,7 +22,7 @@ namespace {
 using namespace nbk;
 
 std::mutex g_mu;
-nb_config g_cfg = {nullptr, nullptr, 0, 0, 0, 0.01720209895 * 0.01720209895, 3.0, 0.4, 0, 0, 0, 1, 0, 0, 0, 0, 0, 0, 0, 1e-12, 1.0, 0};
+nb_config g_cfg = {nullptr, nullptr, 0, 0, 0, 0.01720209895 * 0.01720209895, 3.0, 0.4, 0, 0, 0, 1, 0, 0, 0, 0, 0, 1e-12, 1.0, 0};
 char g_err[512] = "";
 int g_sm_count = 0;
 cudaEvent_t g_ev0 = nullptr, g_ev1 = nullptr;
@@ -94,7 +94,6 @@ struct Geometry {
     int nsplit;           // CTAs along j
     int Nj, Njpad;
     int minb;             // register cap: CTAs per SM the kernel variant is compiled for (3..6)
-    int pipe;             // software-pipelined j loop
     int sym;              // 1: Newton-III super-tile kernel (force_sym.cuh); nsplit = number of super-blocks
     int S, U, Npad_sym;   // super-block size, 32-blocks per skew unit, N padded to a multiple of S
     int sorted;           // symmetric kernel: bodies staged in azimuthal order (sort_staging.cuh)
@@ -115,7 +114,7 @@ Geometry geometry(int64_t N, int64_t n_active) {
         // problems take I = 2 so that S = 256 super-blocks (more CTAs) stay possible.
         int ipt = g_cfg.i_per_thread;
         if (ipt != 1 && ipt != 2 && ipt != 4) ipt = N >= 32768 ? 4 : 2;
-        int minb = g_cfg.ctas_per_sm >= 2 && g_cfg.ctas_per_sm <= 6 ? g_cfg.ctas_per_sm : (ipt == 4 ? 3 : 4);
+        const int minb = ipt == 4 ? 3 : 4;
         int S = g_cfg.sym_block;
         if (S != 256 && S != 512 && S != 1024 && S != 2048) {
             // S = 512 runs 3 CTAs/SM at I = 4 (48 KB of shared memory each) and measured fastest; smaller when
@@ -130,7 +129,7 @@ Geometry geometry(int64_t N, int64_t n_active) {
             while (S < 2048 && ((N + S - 1) / S) * N * 24 > ((int64_t)16 << 30)) S <<= 1;
         }
         if (S < 128 * ipt) S = 128 * ipt;
-        g.sym = 1; g.S = S; g.U = S / 128; g.ipt = ipt; g.minb = minb; g.pipe = 0;
+        g.sym = 1; g.S = S; g.U = S / 128; g.ipt = ipt; g.minb = minb;
         g.Npad_sym = (int)(((N + S - 1) / S) * S);
         g.nsplit = g.Npad_sym / S;
         g.iblocks = g.nsplit; g.tiles_per_split = 0;
@@ -149,8 +148,8 @@ Geometry geometry(int64_t N, int64_t n_active) {
             ipt >>= 1;
     }
     g.ipt = ipt;
-    g.minb = g_cfg.ctas_per_sm >= 3 && g_cfg.ctas_per_sm <= 6 ? g_cfg.ctas_per_sm : (ipt == 4 ? 3 : 5);
-    g.pipe = g_cfg.pipeline_j > 0 ? 1 : 0;
+    g.minb = ipt == 4 ? 3 : 5;
+
     g.iblocks = (int)((N + (int64_t)kForceThreads * ipt - 1) / ((int64_t)kForceThreads * ipt));
     int nsplit = g_cfg.j_splits;
     if (nsplit <= 0) {
@@ -286,33 +285,19 @@ int check_workspace_head(int64_t N, int level /* 0 status, 1 + momentum partials
 
 inline int body_blocks(int64_t n) { return (int)((n + kBodyThreads - 1) / kBodyThreads); }
 
-template <int I, int MINB, bool PIPE>
-void launch_force_IMP(const ForceParams &fp, const Geometry &g, bool pairs) {
-    dim3 grid(g.iblocks, g.nsplit);
-    if (pairs) nb_force_tiles_kernel<I, true, MINB, PIPE><<<grid, kForceThreads, 0, stream()>>>(fp);
-    else nb_force_tiles_kernel<I, false, MINB, PIPE><<<grid, kForceThreads, 0, stream()>>>(fp);
-}
-
+// register caps measured fastest on B200 (profiles/): one-sided kernel I = 1, 2 at 5 CTAs/SM, I = 4 at 3;
+// Newton-III kernel I = 1, 2 at 4 CTAs/SM, I = 4 at 3
 template <int I, int MINB>
 void launch_force_IM(const ForceParams &fp, const Geometry &g, bool pairs) {
-    if (g.pipe) launch_force_IMP<I, MINB, true>(fp, g, pairs);
-    else launch_force_IMP<I, MINB, false>(fp, g, pairs);
-}
-
-template <int I>
-void launch_force_I(const ForceParams &fp, const Geometry &g, bool pairs) {
-    switch (g.minb) {
-        case 3: launch_force_IM<I, 3>(fp, g, pairs); break;
-        case 4: launch_force_IM<I, 4>(fp, g, pairs); break;
-        case 5: launch_force_IM<I, 5>(fp, g, pairs); break;
-        default: launch_force_IM<I, 6>(fp, g, pairs); break;
-    }
+    dim3 grid(g.iblocks, g.nsplit);
+    if (pairs) nb_force_tiles_kernel<I, true, MINB><<<grid, kForceThreads, 0, stream()>>>(fp);
+    else nb_force_tiles_kernel<I, false, MINB><<<grid, kForceThreads, 0, stream()>>>(fp);
 }
 
 void launch_force(const ForceParams &fp, const Geometry &g, bool pairs) {
-    if (g.ipt == 4) launch_force_I<4>(fp, g, pairs);
-    else if (g.ipt == 2) launch_force_I<2>(fp, g, pairs);
-    else launch_force_I<1>(fp, g, pairs);
+    if (g.ipt == 4) launch_force_IM<4, 3>(fp, g, pairs);
+    else if (g.ipt == 2) launch_force_IM<2, 5>(fp, g, pairs);
+    else launch_force_IM<1, 5>(fp, g, pairs);
 }
 
 template <int I, int MINB, bool SORTED>
@@ -333,21 +318,10 @@ int launch_sym_IM(const SymParams &sp, const Geometry &g, bool pairs) {
     return g.sorted ? launch_sym_IMS<I, MINB, true>(sp, g, pairs) : launch_sym_IMS<I, MINB, false>(sp, g, pairs);
 }
 
-template <int I>
-int launch_sym_I(const SymParams &sp, const Geometry &g, bool pairs) {
-    switch (g.minb) {
-        case 2: return launch_sym_IM<I, 2>(sp, g, pairs);
-        case 3: return launch_sym_IM<I, 3>(sp, g, pairs);
-        case 4: return launch_sym_IM<I, 4>(sp, g, pairs);
-        case 5: return launch_sym_IM<I, 5>(sp, g, pairs);
-        default: return launch_sym_IM<I, 6>(sp, g, pairs);
-    }
-}
-
 int launch_sym(const SymParams &sp, const Geometry &g, bool pairs) {
-    if (g.ipt == 4) return launch_sym_I<4>(sp, g, pairs);
-    if (g.ipt == 2) return launch_sym_I<2>(sp, g, pairs);
-    return launch_sym_I<1>(sp, g, pairs);
+    if (g.ipt == 4) return launch_sym_IM<4, 3>(sp, g, pairs);
+    if (g.ipt == 2) return launch_sym_IM<2, 4>(sp, g, pairs);
+    return launch_sym_IM<1, 4>(sp, g, pairs);
 }
 
 // One force evaluation: [second half-shift] + rcrit + staging, tiles, reduce + kick.
@@ -573,7 +547,7 @@ int step_impl(double *x, double *v, const double *m, double M_star, int64_t N, d
         key.x = x; key.v = v; key.m = m; key.rcrit = rc_io; key.acc = acc; key.pairs = pairs; key.npairs = npairs;
         key.ws = g_cfg.workspace; key.stream = g_cfg.stream; key.N = N; key.n_active = g_cfg.n_active;
         key.cap = g_cfg.pair_capacity; key.dt = dt; key.M_star = M_star; key.G = g_cfg.G; key.n1 = g_cfg.n1;
-        key.n2 = g_cfg.n2; key.kind = g_cfg.changeover_kind; key.bs_tol = g_cfg.bs_tol; key.enc = (enc ? 1 : 0) + 2 * g.sorted; key.ipt = g.S * 1000 + g.ipt * 100 + g.minb * 10 + g.pipe; key.jsplit = g.nsplit;
+        key.n2 = g_cfg.n2; key.kind = g_cfg.changeover_kind; key.bs_tol = g_cfg.bs_tol; key.enc = (enc ? 1 : 0) + 2 * g.sorted; key.ipt = g.S * 1000 + g.ipt * 100 + g.minb * 10; key.jsplit = g.nsplit;
         key.ws_bytes = g_cfg.workspace_bytes;
         const bool hop = !stream_capturable();
         if (hop) {
@@ -668,7 +642,6 @@ int nb_configure(const nb_config *cfg) {
     if (cfg->i_per_thread != 0 && cfg->i_per_thread != 1 && cfg->i_per_thread != 2 && cfg->i_per_thread != 4)
         return fail(NB_E_BADARG, "i_per_thread must be 0, 1, 2 or 4");
     if (cfg->j_splits < 0) return fail(NB_E_BADARG, "j_splits must be >= 0");
-    if (cfg->ctas_per_sm != 0 && (cfg->ctas_per_sm < 2 || cfg->ctas_per_sm > 6)) return fail(NB_E_BADARG, "ctas_per_sm must be 0 or 2..6");
     if (cfg->force_kernel != NB_FORCE_AUTO && cfg->force_kernel != NB_FORCE_TILES && cfg->force_kernel != NB_FORCE_SYMMETRIC)
         return fail(NB_E_BADARG, "unknown force_kernel %d", cfg->force_kernel);
     if (cfg->sym_block != 0 && cfg->sym_block != 256 && cfg->sym_block != 512 && cfg->sym_block != 1024 && cfg->sym_block != 2048)

@@ -230,3 +230,36 @@ def test_encounter_semi_active_split_groups():
     print(f"semi-active split: {int(moved.sum())} bodies in {grp['ngroups']} groups, BS steps {st['steps']}, max rel dx {ex:.2e} dv {ev:.2e}")
     assert ex <= ENC_TOL and ev <= ENC_TOL
     assert np.max(np.abs(xr[moved] - x[moved])) > 0
+
+
+def test_encounter_semi_active_core_beyond_one_warp_against_the_always_split_definition():
+    """Reading S22: the definition (oracle default) splits EVERY semi-active group into its active core and independent
+    {core + particle} problems.  The CUDA path splits only while core + particle fit one warp (core <= 31) and otherwise
+    integrates the group as one problem -- the same motion, to the Bulirsch-Stoer tolerance.  A core of 36 embryos with 60
+    test particles: CUDA (unsplit) against the always-split oracle at ENC_TOL; and a core of 31 (split on both sides)."""
+    rng = np.random.default_rng(41)
+    for n_act, n_sat in ((36, 60), (31, 40)):
+        n = n_act + n_sat
+        N = n + 20
+        side = int(np.ceil(np.sqrt(n)))
+        cell = rng.permutation(side * side)[:n]
+        gi, gj = np.divmod(cell, side)
+        a = np.concatenate([1.0 + 3e-3 * (gi - side / 2) + rng.uniform(-4e-4, 4e-4, n), rng.uniform(2.0, 3.0, N - n)])
+        M = np.concatenate([0.4 + 3e-3 * (gj - side / 2) + rng.uniform(-4e-4, 4e-4, n), rng.uniform(0, 6, N - n)])
+        x, v = nb_inputs.elements_to_cartesian(a, rng.uniform(0, 2e-4, N), rng.uniform(0, 1e-4, N), np.zeros(N), np.zeros(N), M, G_GAUSS)
+        x = np.ascontiguousarray(x); v = np.ascontiguousarray(v)
+        # semi-active ordering: the embryos first
+        m = np.zeros(N); m[:n_act] = rng.uniform(1e-9, 1e-8, n_act)
+        rc = np.full(N, 0.02)
+        pairs = [[i, i + 1] for i in range(n_act - 1)] + [[int(rng.integers(0, n_act)), k] for k in range(n_act, n)]
+        grp = oracle.groups(np.array(pairs, dtype=np.int32), N)
+        assert grp["ngroups"] == 1 and grp["largest"] == n
+        xg, vg, status = _gpu_encounter(x, v, m, rc, 1.0, 3.0, grp, n_active=n_act)
+        xr, vr, st = oracle.encounter(x, v, m, rc, 1.0, 3.0, G_GAUSS, grp, tol=1e-12, n_active=n_act)   # always split
+        assert st["failed"] == 0 and st["skipped"] == 0 and status["bs_fail"] == 0 and status["groups_skipped"] == 0
+        mem = grp["members"]
+        ex = np.max(np.abs(xg[mem] - xr[mem]) / np.linalg.norm(xr[mem], axis=1, keepdims=True))
+        ev = np.max(np.abs(vg[mem] - vr[mem]) / np.linalg.norm(vr[mem], axis=1, keepdims=True))
+        print(f"semi-active core of {n_act}: CUDA vs always-split oracle: max rel dx {ex:.2e} dv {ev:.2e}")
+        assert ex <= ENC_TOL and ev <= ENC_TOL
+        assert np.array_equal(xg[n:], x[n:]) and np.max(np.abs(xr[mem] - x[mem])) > 0

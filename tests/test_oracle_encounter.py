@@ -192,3 +192,76 @@ def test_semi_active_groups_are_split_into_core_and_independent_test_particles()
     xk, vk, code = oracle.kepler_one(xr[0], vr[0], mu, 0.8 * P)
     assert code == 0 and np.max(np.abs((xe[1] - xe[0]) - xk)) <= 1e-10 * 0.01
     assert np.max(np.abs(xe[0] - (x2[0] + 0.8 * P * v2[0]))) <= 1e-13      # the embryo does not feel the particle
+
+
+@pytest.mark.parametrize("kind", [0, 1])
+def test_pair_term_inside_the_transition_shell_is_one_minus_W(kind):
+    """Pin of the [1 - W] factor BETWEEN its end values (Eq. 4 carries [1 - K], Eq. 5 carries K):
+    for a pair at r/rc in {0.15, 0.3, 0.7, 0.95} (all off the symmetric point 0.55, so W and 1 - W differ)
+      (i)  the group right-hand side gives exactly (1 - oracle.changeover(r, rc)) G m_j / r^2 along the line
+           (oracle.changeover is pinned on its own by P1: end points, midpoint, monotone, W(y) + W(1-y) = 1);
+      (ii) the kick acceleration (oracle.accel, weight W) plus the encounter acceleration is the full Newtonian
+           G m_j / r^2 -- the two Hamiltonians share one pair force (Eq. 4 [1 - K] + Eq. 5 K);
+      (iii) integrated: two bodies at relative rest around a star of negligible mass, tiny dt: dv/dt of each body
+           equals that acceleration."""
+    G = G_GAUSS
+    m = np.array([2e-3, 5e-4])
+    rcv = 0.04
+    d = np.array([0.36, -0.48, 0.8])                                     # unit vector
+    for frac in (0.15, 0.3, 0.7, 0.95):
+        r = frac * rcv
+        x = np.stack([np.array([1.0, 0.3, -0.2]), np.array([1.0, 0.3, -0.2]) + r * d])
+        v = np.tile(np.array([1e-6, 2e-6, -1e-6]), (2, 1))             # common drift: fixes the velocity scale of the error test
+        rc = np.array([rcv, 0.3 * rcv])                                   # max rule: rc_ij = rcv
+        r = float(np.linalg.norm(x[1] - x[0])); d = (x[1] - x[0]) / r      # the separation as stored (x ~ 1 rounds r at 1e-14)
+        W = oracle.changeover(r, rcv, kind)
+        assert 0.0 < W < 1.0 and abs(W - 0.5) > 0.05
+        # (i) right-hand side, star switched off
+        xd, vd = oracle.encounter_rhs(x, v, G * m, rc, 0.0, kind)
+        assert np.array_equal(xd, v)
+        # (1 - W formed here from the pinned W loses eps/(1 - W) to cancellation: allow eps of the FULL force on top)
+        full = G * m / r ** 2
+        np.testing.assert_allclose(vd[0], (1.0 - W) * full[1] * d, rtol=2e-14, atol=4e-16 * full[1])
+        np.testing.assert_allclose(vd[1], -(1.0 - W) * full[0] * d, rtol=2e-14, atol=4e-16 * full[0])
+        # (ii) sum rule with the kick
+        acc, _, _ = oracle.accel(x, m, rc, G, kind=kind)
+        np.testing.assert_allclose(acc[0] + vd[0], G * m[1] / r ** 2 * d, rtol=2e-14)
+        np.testing.assert_allclose(acc[1] + vd[1], -G * m[0] / r ** 2 * d, rtol=2e-14)
+        # (iii) through the integrator: dv = a dt + O(dt^3) (relative rest => no dt^2 term); a dt^2 / r ~ 1e-10
+        dt = 1e-5
+        xe, ve, st = oracle.encounter(x, v, m, rc, 1e-30, dt, G, _grp([[0, 1]], 2), kind=kind, tol=1e-14)
+        assert st["integrated"] == 1 and st["failed"] == 0
+        for b, sign, mj in ((0, 1.0, m[1]), (1, -1.0, m[0])):
+            a_num = (ve[b] - v[b]) / dt
+            a_ref = sign * (1.0 - W) * G * mj / r ** 2 * d
+            assert np.linalg.norm(a_num - a_ref) <= 1e-8 * np.linalg.norm(a_ref), (frac, kind, a_num, a_ref)
+    # outside rc the pair term vanishes, inside 0.1 rc it is the full force
+    for frac, w1 in ((1.2, 0.0), (0.05, 1.0)):
+        x = np.stack([np.zeros(3) + [1, 0, 0], np.array([1.0, 0, 0]) + frac * rcv * d])
+        r = float(np.linalg.norm(x[1] - x[0])); d = (x[1] - x[0]) / r
+        _, vd = oracle.encounter_rhs(x, np.zeros((2, 3)), G * m, np.full(2, rcv), 0.0, kind)
+        np.testing.assert_allclose(vd[0], w1 * G * m[1] / r ** 2 * d, rtol=2e-14, atol=0)
+
+
+def test_split_threshold_is_an_argument_not_a_constant():
+    """Reading S22: the definition splits EVERY group that has test particles; an implementation may stop splitting at
+    some core size (split_max_core).  Both treatments describe the same motion: they agree to the Bulirsch-Stoer
+    tolerance; with the threshold below the core size nothing is split (identical to the fully active routine)."""
+    G = G_GAUSS
+    rng = np.random.default_rng(12)
+    n_act, n_sat = 4, 6
+    N = n_act + n_sat
+    a = 1.0 + 3e-3 * rng.permutation(N) + rng.uniform(-3e-4, 3e-4, N)
+    M = 0.4 + 3e-3 * rng.permutation(N) + rng.uniform(-3e-4, 3e-4, N)
+    x, v = nb_inputs.elements_to_cartesian(a, np.full(N, 1e-3), np.full(N, 5e-4), np.zeros(N), np.zeros(N), M, G)
+    x = np.ascontiguousarray(x); v = np.ascontiguousarray(v)
+    m = np.zeros(N); m[:n_act] = rng.uniform(1e-7, 3e-7, n_act)
+    rc = np.full(N, 0.05)
+    grp = oracle.groups(np.array([[i, i + 1] for i in range(N - 1)], dtype=np.int32), N)
+    always = oracle.encounter(x, v, m, rc, 1.0, 3.0, G, grp, n_active=n_act, tol=1e-13)
+    wide = oracle.encounter(x, v, m, rc, 1.0, 3.0, G, grp, n_active=n_act, tol=1e-13, split_max_core=n_act)
+    never = oracle.encounter(x, v, m, rc, 1.0, 3.0, G, grp, n_active=n_act, tol=1e-13, split_max_core=n_act - 1)
+    plain = oracle.encounter(x, v, m, rc, 1.0, 3.0, G, grp, tol=1e-13)
+    assert np.array_equal(always[0], wide[0]) and np.array_equal(always[1], wide[1])
+    assert np.array_equal(never[0], plain[0]) and np.array_equal(never[1], plain[1])
+    assert np.max(np.abs(always[0] - never[0])) <= 1e-11 and np.max(np.abs(always[1] - never[1])) <= 1e-11 * np.max(np.abs(v))
