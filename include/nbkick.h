@@ -95,6 +95,11 @@ typedef struct nb_config {
     int sort_staging;        /* tuning (symmetric kernel): NB_SORT_ON stages the bodies sorted by azimuth, so that super-tiles whose
                                 arcs cannot hold an encounter pair skip the test (results keep the caller's indexing);
                                 NB_SORT_AUTO (default): on for N >= 32768; NB_SORT_OFF */
+    int levels;              /* nb_step with resolve_encounters, nb_encounter_levels: number L of intermediate changeover
+                                levels (0 .. 8, default 0 = the plain hybrid scheme).  Level l = 1 .. L runs
+                                with the time step dt / 2^l and the critical radii of Eq. 7 for that time step; only what
+                                is still in a close encounter at level L reaches the direct solver.  Needs workspace for
+                                two adjacency slots per row of the pair list (nb_workspace_bytes accounts for it). */
 } nb_config;
 
 void nb_default_config(nb_config *cfg);
@@ -201,6 +206,29 @@ int nb_groups(const int32_t *pairs, const int64_t *npairs, int64_t N, int32_t *l
 #define NB_MAX_GROUP 1024
 int nb_encounter(double *x, double *v, const double *m, const double *rcrit, double M_star, int64_t N,
                  double dt, const int32_t *members, const int32_t *gstart, const int64_t *gstat);
+
+/*
+ * Multi-level changeover ("introducing higher-level changeover functions ... to not switch from the
+ * symplectic integrator directly to the direct integrator but to introduce intermediate phases, where the symplectic
+ * integrator reduces the time step level by level for the affected bodies.  Only the last level is then performed with
+ * the inner direct integrator.  Every level needs again a smooth changeover function"; reading S23).
+ * H_A over dt for the bodies of a pair list with L = levels intermediate levels: with rc_k,i = max(rc_hill_i,
+ * rc_vel_i / 2^k) (the two terms of Eq. 7; the velocity term shrinks with the level's time step dt / 2^k),
+ * W_k = W(r; max(rc_k,i, rc_k,j)) and Omega_l = prod_{k <= l} [1 - W_k],
+ *     advance(l, tau):  l == L: the direct solver of nb_encounter over tau for the groups of P_L, pair weight Omega_L
+ *                       else twice, h = tau/2:  P_{l+1} = pairs of P_l with r < rc_{l+1} now (strict, fp64 on r^2)
+ *                                               v_i += (h/2) sum_{j: {i,j} in P_l} G m_j Omega_l W_{l+1} (x_j - x_i)/r^3
+ *                                               bodies of P_l in no pair of P_{l+1}: Kepler drift h;  advance(l + 1, h)
+ *                                               the same kick again
+ * starting with advance(0, dt) on P_0 = the given list.  At every r the weights W_0 (nb_kick), Omega_{l-1} W_l (level
+ * kicks) and Omega_L (direct solver) sum to 1.  Bodies in no listed pair are left alone; groups of P_L beyond
+ * NB_MAX_GROUP take the Kepler drift over tau and are counted in nb_status[4] (once per visit).  Sums run over a body's
+ * partners in ascending index order: bit-reproducible.  Fully active case only.
+ *   x, v [N,3] in/out; m, rc_hill, rc_vel [N] in; pairs / npairs in (device, as in nb_groups).
+ * Needs the head of the workspace up to and including the multi-level area (inside nb_workspace_bytes(N)).
+ */
+int nb_encounter_levels(double *x, double *v, const double *m, const double *rc_hill, const double *rc_vel, double M_star,
+                        int64_t N, double dt, const int32_t *pairs, const int64_t *npairs);
 
 /*
  * Perfect merging ("N-body simulations often treat collisions as perfect mergers";

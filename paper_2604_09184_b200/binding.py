@@ -22,7 +22,7 @@ FORCE_AUTO, FORCE_TILES, FORCE_SYMMETRIC = 0, 1, 2
 # every symbol include/nbkick.h declares (tests check the library exports each of them)
 SYMBOLS = (
     "nb_default_config", "nb_configure", "nb_workspace_bytes", "nb_rcrit", "nb_kick", "nb_shift",
-    "nb_drift_kepler", "nb_step", "nb_groups", "nb_encounter", "nb_merge", "nb_kick_host", "nb_step_host", "nb_status", "nb_status_reset",
+    "nb_drift_kepler", "nb_step", "nb_groups", "nb_encounter", "nb_encounter_levels", "nb_merge", "nb_kick_host", "nb_step_host", "nb_status", "nb_status_reset",
     "nb_last_force_ms", "nb_force_time", "nb_force_time_reset", "nb_force_geometry", "nb_fp64_peak", "nb_release", "nb_last_error", "nb_version",
 )
 
@@ -49,6 +49,7 @@ class NbConfig(C.Structure):
         ("bs_tol", C.c_double),
         ("radius_factor", C.c_double),
         ("sort_staging", C.c_int),
+        ("levels", C.c_int),
     ]
 
 
@@ -88,6 +89,7 @@ def load():
     lib.nb_step.argtypes = [vp, vp, vp, dbl, i64, dbl, vp, vp, vp, vp, i64]
     lib.nb_groups.argtypes = [vp, vp, i64, vp, vp, vp, vp]
     lib.nb_encounter.argtypes = [vp, vp, vp, vp, dbl, i64, dbl, vp, vp, vp]
+    lib.nb_encounter_levels.argtypes = [vp, vp, vp, vp, vp, dbl, i64, dbl, vp, vp]
     lib.nb_merge.argtypes = [vp, vp, vp, vp, i64, vp, vp, vp, vp]
     lib.nb_kick_host.argtypes = [vp, vp, vp, dbl, i64, dbl, vp, vp, vp, vp]
     lib.nb_step_host.argtypes = [vp, vp, vp, dbl, i64, dbl, vp, vp, vp, vp, i64]
@@ -156,7 +158,7 @@ def default_config() -> NbConfig:
 
 def configure(N=None, *, stream=None, pair_capacity=0, n_active=0, G=None, n1=3.0, n2=0.4, changeover_kind=0,
               i_per_thread=0, j_splits=0, use_graph=True, reuse_acc=False, time_force=False,
-              force_kernel=0, sym_block=0, resolve_encounters=False, bs_tol=1e-12, radius_factor=1.0, sort_staging=0, workspace_bytes=None,
+              force_kernel=0, sym_block=0, resolve_encounters=False, bs_tol=1e-12, radius_factor=1.0, sort_staging=0, levels=0, workspace_bytes=None,
               device="cuda"):
     """nb_configure with a torch-allocated workspace sized for N bodies (N=None: no workspace,
     enough for the _host calls; workspace_bytes: explicit size, e.g. the head that the O(N) calls
@@ -177,6 +179,7 @@ def configure(N=None, *, stream=None, pair_capacity=0, n_active=0, G=None, n1=3.
     cfg.resolve_encounters, cfg.bs_tol = (1 if resolve_encounters else 0), float(bs_tol)
     cfg.radius_factor = float(radius_factor)
     cfg.sort_staging = int(sort_staging)
+    cfg.levels = int(levels)
     if N is not None:
         import torch
         if stream is None:
@@ -257,6 +260,14 @@ def nb_encounter(x, v, m, rcrit, M_star, dt, members, gstart, gstat):
     _check(load().nb_encounter(_dev(x, 3 * N, torch.float64), _dev(v, 3 * N, torch.float64), _dev(m, N, torch.float64),
                                _dev(rcrit, N, torch.float64), float(M_star), N, float(dt), _dev(members, N, torch.int32),
                                _dev(gstart, N // 2 + 2, torch.int32), _dev(gstat, 4, torch.int64)))
+
+
+def nb_encounter_levels(x, v, m, rc_hill, rc_vel, M_star, dt, pairs, npairs):
+    import torch
+    N = m.numel()
+    _check(load().nb_encounter_levels(_dev(x, 3 * N, torch.float64), _dev(v, 3 * N, torch.float64), _dev(m, N, torch.float64),
+                                      _dev(rc_hill, N, torch.float64), _dev(rc_vel, N, torch.float64), float(M_star), N,
+                                      float(dt), _dev(pairs, None, torch.int32), _dev(npairs, 1, torch.int64)))
 
 
 def nb_merge(x, v, m, radius, pairs, npairs, survivor_of, mstat):

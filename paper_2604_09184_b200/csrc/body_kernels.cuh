@@ -13,13 +13,16 @@ namespace nbk {
 __device__ __forceinline__ double critical_radius(const double x, const double y, const double z, const double vx,
                                                   const double vy, const double vz, const double m,
                                                   const double M_star, const double G, const double n1,
-                                                  const double n2, const double absdt) {
+                                                  const double n2, const double absdt, double *hill_term = nullptr,
+                                                  double *vel_term = nullptr) {
     const double r = sqrt(x * x + y * y + z * z);
     const double v2 = vx * vx + vy * vy + vz * vz;
     const double inva = 2.0 / r - v2 / (G * M_star);
     const double a = (inva > 0.0) ? 1.0 / inva : r;
     const double rh = a * cbrt(m / (3.0 * M_star));
-    return fmax(n1 * rh, n2 * absdt * sqrt(v2));
+    const double t1 = n1 * rh, t2 = n2 * absdt * sqrt(v2);
+    if (hill_term != nullptr) { *hill_term = t1; *vel_term = t2; }   // multilevel.cuh: rc_k = max(t1, t2 / 2^k)
+    return fmax(t1, t2);
 }
 
 struct PrepParams {
@@ -27,6 +30,8 @@ struct PrepParams {
     const double *v;        // [N,3]; needed when update_rc
     const double *m;        // [N]
     double *rcrit;          // [N]; written when update_rc, read otherwise
+    double *rc_hill, *rc_vel;  // [N] the two terms of Eq. 7 for the multi-level scheme (nullptr: not wanted); with caller's
+                            // radii (update_rc = 0): hill = 0, vel = rcrit, i.e. rc_k = rcrit / 2^k
     JRec *jrec;             // [Njpad] one-sided kernel's records (nullptr: not staged)
     double2 *sxy, *szg;     // [2 Npad_sym] symmetric kernel's (x,y) and (z,Gm), doubled-block layout (nullptr: not staged)
     int *sthr;              // [2 Npad_sym] hi32(rcrit^2) + 1
@@ -63,13 +68,16 @@ __global__ void __launch_bounds__(kBodyThreads) nb_prep_kernel(const PrepParams 
         }
         const double m = p.m[i];
         double rc;
+        double t1 = 0.0, t2;
         if (p.update_rc) {
             rc = critical_radius(x, y, z, p.v[3 * (size_t)i], p.v[3 * (size_t)i + 1], p.v[3 * (size_t)i + 2], m,
-                                 p.M_star, p.G, p.n1, p.n2, p.absdt);
+                                 p.M_star, p.G, p.n1, p.n2, p.absdt, &t1, &t2);
             p.rcrit[i] = rc;
         } else {
             rc = p.rcrit[i];
+            t2 = rc;
         }
+        if (p.rc_hill != nullptr) { p.rc_hill[i] = t1; p.rc_vel[i] = t2; }
         if (i < p.Nj) {
             const double gm = p.G * m;
             r.x = x; r.y = y; r.z = z; r.gm = gm;

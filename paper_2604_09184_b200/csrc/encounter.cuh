@@ -21,14 +21,28 @@ namespace nbk {
 constexpr int kBsCols = 8;
 constexpr int kMaxGroup = 1024;  // larger groups are left to the Kepler drift and counted (NB_MAX_GROUP)
 
-// Acceleration of a body at q = (x, y, z) with critical radius my_rc: star term plus the [1 - W] pair terms of
-// the n members whose positions / G m / rc sit in the given (shared-memory) arrays; `self` is skipped.
+// 1 - W(r; rc): the complement of the kick weight, formed directly (no cancellation near W = 1)
+__device__ __forceinline__ double one_minus_weight(const double r, const double rc, const int kind) {
+    if (!(r < rc)) return 0.0;
+    const double t0 = r - 0.1 * rc;
+    if (t0 <= 0.0) return 1.0;
+    const double y = t0 * rcp_fast(0.9 * rc);
+    if (y >= 1.0) return 0.0;
+    const double z = 1.0 - y;
+    return kind == 1 ? z * z * z * (1.0 + y * (3.0 + 6.0 * y)) : (z * z) * rcp_fast(2.0 * y * y - 2.0 * y + 1.0);
+}
+
+// Acceleration of a body at q = (x, y, z) whose critical radius has the two terms (my_hill, my_vel): star term plus
+// the pair terms of the n members whose positions / G m / radius terms sit in the given (shared-memory) arrays;
+// `self` is skipped.  Level radii rc_k = max(hill, vel / 2^k) (multilevel.cuh); the pair weight is the product over
+// k < nlev of [1 - W(r; rc_k,ij)] -- nlev = 1 with vel = 0: Eq. 4 as printed, rc = hill.
 // No IEEE divide or sqrt on the common path (latency is what a small group pays for).
-__device__ __forceinline__ void enc_accel(const double qx, const double qy, const double qz, const double my_rc,
-                                          const int self, const int n, const double *__restrict__ px,
+__device__ __forceinline__ void enc_accel(const double qx, const double qy, const double qz, const double my_hill,
+                                          const double my_vel, const int self, const int n, const double *__restrict__ px,
                                           const double *__restrict__ py, const double *__restrict__ pz,
-                                          const double *__restrict__ sgm, const double *__restrict__ src,
-                                          const double mu, const int kind, double &ax, double &ay, double &az) {
+                                          const double *__restrict__ sgm, const double *__restrict__ shill,
+                                          const double *__restrict__ svel, const int nlev, const double mu, const int kind,
+                                          double &ax, double &ay, double &az) {
     const double r2 = (qx * qx + qy * qy) + qz * qz;
     const double ir = rsqrt_fast(r2);
     const double s = -mu * (ir * ir * ir);
@@ -37,18 +51,14 @@ __device__ __forceinline__ void enc_accel(const double qx, const double qy, cons
         if (j == self || sgm[j] == 0.0) continue;        // a massless member (semi-active mode) pulls on nobody
         const double dx = px[j] - qx, dy = py[j] - qy, dz = pz[j] - qz;
         const double d2 = (dx * dx + dy * dy) + dz * dz;
-        const double rc = fmax(my_rc, src[j]);
-        if (!(d2 < rc * rc) || d2 == 0.0) continue;      // 1 - W = 0 outside rc; coincident: no direction
+        const double hill = fmax(my_hill, shill[j]), vel = fmax(my_vel, svel[j]);
+        const double rc0 = fmax(hill, vel);
+        if (!(d2 < rc0 * rc0) || d2 == 0.0) continue;    // 1 - W_0 = 0 outside rc; coincident: no direction
         const double id = rsqrt_fast(d2);
         const double d = sqrt_from_rsqrt(d2, id);
-        double w = 1.0;
-        const double t0 = d - 0.1 * rc;
-        if (t0 > 0.0) {
-            const double y = t0 * rcp_fast(0.9 * rc);
-            if (y >= 1.0) continue;
-            const double z = 1.0 - y;
-            w = kind == 1 ? z * z * z * (1.0 + y * (3.0 + 6.0 * y)) : (z * z) * rcp_fast(2.0 * y * y - 2.0 * y + 1.0);
-        }
+        double w = one_minus_weight(d, rc0, kind), sc = 0.5;
+        for (int k = 1; k < nlev && w != 0.0; ++k, sc *= 0.5) w *= one_minus_weight(d, fmax(hill, vel * sc), kind);
+        if (w == 0.0) continue;
         const double tt = sgm[j] * w * (id * id * id);
         ax += tt * dx; ay += tt * dy; az += tt * dz;
     }
@@ -62,7 +72,9 @@ __device__ __forceinline__ double bs_weight(const int c, const int mc) {
 
 struct EncParams {
     double *x, *v;            // [N,3] in/out (members only)
-    const double *m, *rcrit;  // [N]
+    const double *m, *rcrit;  // [N]; rcrit: the critical radius, or its Hill term when rc_vel is given
+    const double *rc_vel;     // [N] velocity term of Eq. 7 (multilevel.cuh: rc_k = max(rcrit, rc_vel / 2^k)) or nullptr
+    int nlev;                 // levels whose [1 - W_k] multiply in the pair term (1: the plain hybrid scheme)
     const int *members, *gstart;
     const long long *gstat;   // [0] = number of groups
     long long *status;
@@ -94,9 +106,9 @@ __device__ __forceinline__ double cta_max(double val, double *red /* [32] */) {
 
 template <int THREADS>
 __global__ void __launch_bounds__(THREADS) nb_encounter_kernel(const EncParams p) {
-    extern __shared__ double enc_sm[];  // px[T] py[T] pz[T] gm[T] rc[T] red[32]
+    extern __shared__ double enc_sm[];  // px[T] py[T] pz[T] gm[T] rc[T] vel[T] red[32]
     double *px = enc_sm, *py = px + THREADS, *pz = py + THREADS, *sgm = pz + THREADS, *src = sgm + THREADS,
-           *red = src + THREADS;
+           *svel = src + THREADS, *red = svel + THREADS;
     const int t = threadIdx.x;
     const long long ngroups = p.gstat[0];
     for (long long g = blockIdx.x; g < ngroups; g += gridDim.x) {
@@ -117,8 +129,9 @@ __global__ void __launch_bounds__(THREADS) nb_encounter_kernel(const EncParams p
             for (int c = 0; c < 3; ++c) { y[c] = p.x[3 * (size_t)b + c]; y[3 + c] = p.v[3 * (size_t)b + c]; }
             sgm[t] = p.G * p.m[b];
             src[t] = p.rcrit[b];
+            svel[t] = p.rc_vel != nullptr ? p.rc_vel[b] : 0.0;
         }
-        const double my_rc = act ? src[t] : 0.0;
+        const double my_rc = act ? src[t] : 0.0, my_vel = act ? svel[t] : 0.0;
 
         // acceleration of this thread's body at position (qx,qy,qz), all members' positions taken from shared memory
         auto rhs = [&](const double (&q)[6], double (&f)[6]) {
@@ -127,7 +140,7 @@ __global__ void __launch_bounds__(THREADS) nb_encounter_kernel(const EncParams p
             __syncthreads();
             if (act) {
                 double ax, ay, az;
-                enc_accel(q[0], q[1], q[2], my_rc, t, n, px, py, pz, sgm, src, p.mu, p.kind, ax, ay, az);
+                enc_accel(q[0], q[1], q[2], my_rc, my_vel, t, n, px, py, pz, sgm, src, svel, p.nlev, p.mu, p.kind, ax, ay, az);
                 f[0] = q[3]; f[1] = q[4]; f[2] = q[5]; f[3] = ax; f[4] = ay; f[5] = az;
             }
         };
@@ -235,7 +248,7 @@ __global__ void __launch_bounds__(256) nb_enc_plan_kernel(const int *__restrict_
 // Lanes >= keep_from write their final state back (0: everybody; nc: only the test particle of a split group).
 __device__ __forceinline__ void bs_small_problem(const EncParams &p, const int b, const int n, const int keep_from) {
     __shared__ double px[kBsCols][32], py[kBsCols][32], pz[kBsCols][32];
-    __shared__ double sgm[32], src[32];
+    __shared__ double sgm[32], src[32], svel[32];
     __shared__ double col[kBsCols][6][32];   // T_{c,0} of every column
     __shared__ double ycur[6][32];
     __shared__ double ctrl_h, ctrl_t;
@@ -250,11 +263,12 @@ __device__ __forceinline__ void bs_small_problem(const EncParams &p, const int b
             for (int c = 0; c < 3; ++c) { ycur[c][lane] = p.x[3 * (size_t)b + c]; ycur[3 + c][lane] = p.v[3 * (size_t)b + c]; }
             sgm[lane] = p.G * p.m[b];
             src[lane] = p.rcrit[b];
+            svel[lane] = p.rc_vel != nullptr ? p.rc_vel[b] : 0.0;
         }
         if (lane == 0) { ctrl_h = p.dt; ctrl_t = 0.0; ctrl_done = (p.dt == 0.0) ? 1 : 0; }
     }
     __syncthreads();
-    const double my_rc = act ? src[lane] : 0.0;
+    const double my_rc = act ? src[lane] : 0.0, my_vel = act ? svel[lane] : 0.0;
     double T[kBsCols][6];                // warp 0: current row of the tableau
     while (true) {
         if (ctrl_done != 0) break;
@@ -273,7 +287,7 @@ __device__ __forceinline__ void bs_small_problem(const EncParams &p, const int b
                 __syncwarp();
                 if (act) {
                     double ax, ay, az;
-                    enc_accel(q[0], q[1], q[2], my_rc, lane, n, px[w], py[w], pz[w], sgm, src, p.mu, p.kind, ax, ay, az);
+                    enc_accel(q[0], q[1], q[2], my_rc, my_vel, lane, n, px[w], py[w], pz[w], sgm, src, svel, p.nlev, p.mu, p.kind, ax, ay, az);
                     f[0] = q[3]; f[1] = q[4]; f[2] = q[5]; f[3] = ax; f[4] = ay; f[5] = az;
                 }
             };

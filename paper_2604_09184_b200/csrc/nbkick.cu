@@ -16,13 +16,14 @@
 #include "force_tiles.cuh"
 #include "groups.cuh"
 #include "merge.cuh"
+#include "multilevel.cuh"
 
 namespace {
 
 using namespace nbk;
 
 std::mutex g_mu;
-nb_config g_cfg = {nullptr, nullptr, 0, 0, 0, 0.01720209895 * 0.01720209895, 3.0, 0.4, 0, 0, 0, 1, 0, 0, 0, 0, 0, 1e-12, 1.0, 0};
+nb_config g_cfg = {nullptr, nullptr, 0, 0, 0, 0.01720209895 * 0.01720209895, 3.0, 0.4, 0, 0, 0, 1, 0, 0, 0, 0, 0, 1e-12, 1.0, 0, 0};
 char g_err[512] = "";
 int g_sm_count = 0;
 cudaEvent_t g_ev0 = nullptr, g_ev1 = nullptr;
@@ -40,7 +41,7 @@ struct StepKey {
     const void *x, *v, *m, *rcrit, *acc, *pairs, *npairs, *ws, *stream;
     int64_t N, n_active, cap;
     double dt, M_star, G, n1, n2, bs_tol;
-    int kind, ipt, jsplit, enc;
+    int kind, ipt, jsplit, enc, levels;
     size_t ws_bytes;
 };
 StepKey g_graph_key;
@@ -191,7 +192,10 @@ struct Workspace {
     int32_t *g_label, *g_members, *g_start;  // the step driver's own group lists
     int64_t *g_stat;
     int *g_core, *enc_flag;                  // direct-solver plan: active members per group, per-body flag
-    char *head_mv_end, *head_grp_end;  // ends of the geometry-independent head
+    MlScratch ml;                            // multi-level changeover (multilevel.cuh), sized by pair_capacity; levels > 0 only
+    double *ml_hill, *ml_vel;                // [N] the two terms of Eq. 7 of the evaluation that opened the step
+    int *ml_listed;                          // [N] body is in a pair of the step's list
+    char *head_mv_end, *head_grp_end, *head_ml_end;  // ends of the geometry-independent head
     double *rc_scratch; // [N]
     JRec *jrec;         // [Njpad]                 (one-sided kernel)
     double2 *sxy, *szg; // [2 Npad_sym]            (symmetric kernel, doubled-block layout)
@@ -234,6 +238,27 @@ Workspace carve(void *base, int64_t N, const Geometry &g) {
         w.enc_flag = reinterpret_cast<int *>(b + off); off += n4;
     }
     w.head_grp_end = b + off;
+    {   // multi-level changeover: adjacency of the pair list (two slots per row) and the level radii
+        const bool on = g_cfg.levels > 0;
+        const size_t n4 = on ? align_up((size_t)(N + 1) * sizeof(int), 256) : 0;
+        const size_t n8 = on ? align_up((size_t)N * sizeof(double), 256) : 0;
+        const size_t slots = on ? (size_t)2 * (size_t)(g_cfg.pair_capacity > 0 ? g_cfg.pair_capacity : 0) : 0;
+        const size_t s4 = align_up(slots * sizeof(int), 256);
+        w.ml.deg = reinterpret_cast<int *>(b + off); off += n4;
+        w.ml.off = reinterpret_cast<int *>(b + off); off += n4;
+        w.ml.cur = reinterpret_cast<int *>(b + off); off += n4;
+        w.ml.bdepth = reinterpret_cast<int *>(b + off); off += n4;
+        w.ml_listed = reinterpret_cast<int *>(b + off); off += n4;
+        w.ml.bsum = reinterpret_cast<int *>(b + off); off += on ? align_up(((size_t)N / kGrpScanBlock + 2) * sizeof(int), 256) : 0;
+        w.ml_hill = reinterpret_cast<double *>(b + off); off += n8;
+        w.ml_vel = reinterpret_cast<double *>(b + off); off += n8;
+        w.ml.adj_tmp = reinterpret_cast<int *>(b + off); off += on ? s4 : 0;
+        w.ml.own = reinterpret_cast<int *>(b + off); off += on ? s4 : 0;
+        w.ml.adj = reinterpret_cast<int *>(b + off); off += on ? s4 : 0;
+        w.ml.depth = reinterpret_cast<signed char *>(b + off); off += on ? align_up(slots, 256) : 0;
+        w.ml.cap = g_cfg.pair_capacity;
+    }
+    w.head_ml_end = b + off;
     w.rc_scratch = reinterpret_cast<double *>(b + off); off += align_up((size_t)N * sizeof(double), 256);
     w.jrec = reinterpret_cast<JRec *>(b + off); off += align_up((size_t)(g.sym ? 0 : g.Njpad) * sizeof(JRec), 256);
     w.sxy = reinterpret_cast<double2 *>(b + off); off += align_up((size_t)2 * g.Npad_sym * sizeof(double2), 256);
@@ -270,14 +295,14 @@ int check_workspace(int64_t N, const Geometry &g, Workspace *w) {
 
 // The O(N) calls touch only the head of the workspace (status words, momentum partials): they must not
 // demand the O(N^2 / S) partial-sum area of the force kernels.
-int check_workspace_head(int64_t N, int level /* 0 status, 1 + momentum partials, 2 + group scratch */, Workspace *w) {
+int check_workspace_head(int64_t N, int level /* 0 status, 1 + momentum partials, 2 + group scratch, 3 + multi-level area */, Workspace *w) {
     if (g_cfg.workspace == nullptr) return fail(NB_E_WORKSPACE, "no workspace configured (nb_configure)");
     if ((reinterpret_cast<uintptr_t>(g_cfg.workspace) & 255u) != 0) return fail(NB_E_WORKSPACE, "workspace is not 256-byte aligned");
     Geometry g0;
     std::memset(&g0, 0, sizeof(g0));
     *w = carve(g_cfg.workspace, N, g0);
     const char *base = static_cast<char *>(g_cfg.workspace);
-    const size_t need = level == 0 ? 512 : (size_t)((level == 1 ? w->head_mv_end : w->head_grp_end) - base);
+    const size_t need = level == 0 ? 512 : (size_t)((level == 1 ? w->head_mv_end : (level == 2 ? w->head_grp_end : w->head_ml_end)) - base);
     if (need > g_cfg.workspace_bytes)
         return fail(NB_E_WORKSPACE, "workspace has %zu bytes, this call needs %zu", g_cfg.workspace_bytes, need);
     return NB_OK;
@@ -355,6 +380,7 @@ int enqueue_eval(const Workspace &w, const Geometry &g, double *x, double *v, co
     pp.x = x; pp.v = v; pp.m = m; pp.rcrit = rc_io; pp.jrec = g.sym ? nullptr : w.jrec; pp.mv_in = mv_in;
     pp.sxy = g.sym ? w.sxy : nullptr; pp.szg = w.szg; pp.sthr = w.sthr; pp.Npad_sym = g.Npad_sym;
     pp.pos_of = sorted ? w.pos_of : nullptr;
+    pp.rc_hill = g_cfg.levels > 0 ? w.ml_hill : nullptr; pp.rc_vel = g_cfg.levels > 0 ? w.ml_vel : nullptr;
     pp.npairs = pairs ? reinterpret_cast<unsigned long long *>(npairs) : nullptr;
     pp.status = w.status; pp.dtc = dtc; pp.M_star = M_star; pp.G = g_cfg.G; pp.n1 = g_cfg.n1; pp.n2 = g_cfg.n2;
     pp.absdt = std::fabs(dt_for_rc); pp.nblk_in = nblk; pp.N = (int)N; pp.Nj = g.Nj; pp.Njpad = g.Njpad;
@@ -424,7 +450,8 @@ void drop_graph() {
 
 // the nine launches of nb_groups (groups.cuh)
 void enqueue_groups(const Workspace &w, const int32_t *pairs, const int64_t *npairs, int64_t N, int32_t *label,
-                    int32_t *members, int32_t *gstart, int64_t *gstat, const GroupFilter flt = GroupFilter{nullptr, nullptr, 1.0, nullptr}) {
+                    int32_t *members, int32_t *gstart, int64_t *gstat, const GroupFilter flt = GroupFilter{nullptr, nullptr, 1.0, nullptr},
+                    const int ml_level = -1) {
     const int n = (int)N;
     const int nb256 = (n + kGrpThreads - 1) / kGrpThreads, nb1024 = (n + kGrpScanBlock - 1) / kGrpScanBlock;
     long long *gs = reinterpret_cast<long long *>(gstat);
@@ -433,9 +460,12 @@ void enqueue_groups(const Workspace &w, const int32_t *pairs, const int64_t *npa
     const long long max_blocks = (long long)sm_count() * 16;
     if (hook_blocks > max_blocks) hook_blocks = max_blocks;
     nb_grp_init_kernel<<<nb256, kGrpThreads, 0, stream()>>>(w.grp, label, members, gstart, gs, n);
-    nb_grp_hook_kernel<<<(unsigned)hook_blocks, kGrpThreads, 0, stream()>>>(w.grp, reinterpret_cast<const int2 *>(pairs),
-                                                                            reinterpret_cast<const long long *>(npairs), cap, n, gs,
-                                                                            w.status, flt);
+    if (ml_level >= 0)   // edges = the adjacency slots listed at the innermost level (multilevel.cuh)
+        nb_ml_hook_kernel<<<nb256, kGrpThreads, 0, stream()>>>(w.grp, w.ml, ml_level, n, gs);
+    else
+        nb_grp_hook_kernel<<<(unsigned)hook_blocks, kGrpThreads, 0, stream()>>>(w.grp, reinterpret_cast<const int2 *>(pairs),
+                                                                                reinterpret_cast<const long long *>(npairs), cap, n, gs,
+                                                                                w.status, flt);
     nb_grp_compress_kernel<<<nb256, kGrpThreads, 0, stream()>>>(w.grp, label, n);
     nb_grp_blocksum_kernel<<<nb1024, kGrpScanBlock, 0, stream()>>>(w.grp, label, n);
     nb_grp_topscan_kernel<<<1, kGrpScanBlock, 0, stream()>>>(w.grp, nb1024, gstart, gs);
@@ -460,14 +490,14 @@ void enqueue_encounter_plan(const Workspace &w, int64_t N, const int32_t *member
 // (one thread per member, columns in sequence)
 void enqueue_encounter(const Workspace &w, double *x, double *v, const double *m, const double *rcrit, double M_star,
                        int64_t N, double dt, const int32_t *members, const int32_t *gstart, const int64_t *gstat,
-                       bool plan_done) {
+                       bool plan_done, const double *rc_vel = nullptr, int nlev = 1) {
     const long long *gs = reinterpret_cast<const long long *>(gstat);
     if (!plan_done) enqueue_encounter_plan(w, N, members, gstart, gstat);
     EncParams ep;
     ep.x = x; ep.v = v; ep.m = m; ep.rcrit = rcrit; ep.members = members; ep.gstart = gstart;
     ep.gstat = gs; ep.status = w.status; ep.mu = g_cfg.G * M_star; ep.G = g_cfg.G;
     ep.dt = dt; ep.tol = g_cfg.bs_tol > 0.0 ? g_cfg.bs_tol : 1e-12; ep.kind = g_cfg.changeover_kind;
-    ep.gcore = w.g_core;
+    ep.gcore = w.g_core; ep.rc_vel = rc_vel; ep.nlev = nlev;
     long long small_blocks = N / 2 + 1;
     const long long cap_blocks = (long long)sm_count() * 8;
     if (small_blocks > cap_blocks) small_blocks = cap_blocks;
@@ -483,14 +513,66 @@ void enqueue_encounter(const Workspace &w, double *x, double *v, const double *m
     ep.min_size = 33; ep.max_size = 128;
     long long mid_blocks = N / 33 + 1;
     if (mid_blocks > 8LL * sm_count()) mid_blocks = 8LL * sm_count();
-    nb_encounter_kernel<128><<<(unsigned)mid_blocks, 128, (5 * 128 + 32) * sizeof(double), stream()>>>(ep);
+    nb_encounter_kernel<128><<<(unsigned)mid_blocks, 128, (6 * 128 + 32) * sizeof(double), stream()>>>(ep);
     ep.min_size = 129; ep.max_size = kMaxGroup;
     static bool attr_set = false;
-    const size_t big_smem = (5 * (size_t)kMaxGroup + 32) * sizeof(double);
+    const size_t big_smem = (6 * (size_t)kMaxGroup + 32) * sizeof(double);
     if (!attr_set) { cudaFuncSetAttribute(nb_encounter_kernel<kMaxGroup>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)big_smem); attr_set = true; }
     long long big_blocks = N / 129 + 1;
     if (big_blocks > 2LL * sm_count()) big_blocks = 2LL * sm_count();
     nb_encounter_kernel<kMaxGroup><<<(unsigned)big_blocks, kMaxGroup, big_smem, stream()>>>(ep);
+}
+
+// Multi-level changeover (multilevel.cuh): adjacency of the step's pair list, then the recursion
+//   advance(l, tau): l == L: direct solver over tau for the groups of P_L; else twice (h = tau/2): detect P_{l+1} +
+//   kick h/2 over P_l, Kepler drift h of the bodies that stay at level l, advance(l + 1, h), kick h/2 over P_l
+// (the closing kick of the first half and the opening kick of the second share one launch).
+void enqueue_ml_adjacency(const Workspace &w, const int32_t *pairs, const int64_t *npairs, int64_t N) {
+    const int n = (int)N;
+    const int nb256 = (n + kGrpThreads - 1) / kGrpThreads, nb1024 = (n + kGrpScanBlock - 1) / kGrpScanBlock;
+    const long long cap = g_cfg.pair_capacity;
+    long long pair_blocks = (cap + kGrpThreads - 1) / kGrpThreads;
+    const long long max_blocks = (long long)sm_count() * 16;
+    if (pair_blocks > max_blocks) pair_blocks = max_blocks;
+    if (pair_blocks < 1) pair_blocks = 1;
+    const int2 *p2 = reinterpret_cast<const int2 *>(pairs);
+    const long long *np = reinterpret_cast<const long long *>(npairs);
+    nb_ml_clear_kernel<<<nb256, kGrpThreads, 0, stream()>>>(w.ml, n);
+    nb_ml_degree_kernel<<<(unsigned)pair_blocks, kGrpThreads, 0, stream()>>>(w.ml, p2, np, cap, n, w.status);
+    nb_ml_scan1_kernel<<<nb1024, kGrpScanBlock, 0, stream()>>>(w.ml, n);
+    nb_ml_scan2_kernel<<<1, kGrpScanBlock, 0, stream()>>>(w.ml, nb1024, n);
+    nb_ml_scan3_kernel<<<nb1024, kGrpScanBlock, 0, stream()>>>(w.ml, n);
+    nb_ml_fill_kernel<<<(unsigned)pair_blocks, kGrpThreads, 0, stream()>>>(w.ml, p2, np, cap, n);
+    nb_ml_sort_kernel<<<(unsigned)(2 * pair_blocks), kGrpThreads, 0, stream()>>>(w.ml, n);
+    nb_ml_listed_kernel<<<nb256, kGrpThreads, 0, stream()>>>(w.ml, n, w.ml_listed);
+}
+
+void enqueue_ml_advance(const Workspace &w, const MlParams &mp, double M_star, int64_t N, int l, double tau) {
+    const int nb256 = ((int)N + kGrpThreads - 1) / kGrpThreads;
+    if (l == mp.L) {
+        // the innermost level: groups of P_L -> plan -> bodies of groups beyond the solver's cap drift -> direct solver
+        enqueue_groups(w, nullptr, nullptr, N, w.g_label, w.g_members, w.g_start, w.g_stat, GroupFilter{nullptr, nullptr, 1.0, nullptr}, l);
+        enqueue_encounter_plan(w, N, w.g_members, w.g_start, w.g_stat);
+        nb_ml_drift_kernel<<<nb256, kGrpThreads, 0, stream()>>>(mp, l, tau, w.enc_flag);
+        enqueue_encounter(w, mp.x, mp.v, mp.m, mp.hill, M_star, N, tau, w.g_members, w.g_start, w.g_stat, true, mp.vel, mp.L + 1);
+        return;
+    }
+    const double h = 0.5 * tau;
+    nb_ml_kick_kernel<true><<<nb256, kGrpThreads, 0, stream()>>>(mp, l, 0.5 * h, 1);
+    nb_ml_drift_kernel<<<nb256, kGrpThreads, 0, stream()>>>(mp, l, h, nullptr);
+    enqueue_ml_advance(w, mp, M_star, N, l + 1, h);
+    nb_ml_kick_kernel<true><<<nb256, kGrpThreads, 0, stream()>>>(mp, l, 0.5 * h, 2);
+    nb_ml_drift_kernel<<<nb256, kGrpThreads, 0, stream()>>>(mp, l, h, nullptr);
+    enqueue_ml_advance(w, mp, M_star, N, l + 1, h);
+    nb_ml_kick_kernel<false><<<nb256, kGrpThreads, 0, stream()>>>(mp, l, 0.5 * h, 1);
+}
+
+MlParams ml_params(const Workspace &w, double *x, double *v, const double *m, const double *hill, const double *vel,
+                   double M_star, int64_t N) {
+    MlParams mp;
+    mp.x = x; mp.v = v; mp.m = m; mp.hill = hill; mp.vel = vel; mp.s = w.ml; mp.status = w.status;
+    mp.G = g_cfg.G; mp.mu = g_cfg.G * M_star; mp.N = (int)N; mp.kind = g_cfg.changeover_kind; mp.L = g_cfg.levels;
+    return mp;
 }
 
 int step_impl(double *x, double *v, const double *m, double M_star, int64_t N, double dt, double *rcrit, double *acc,
@@ -521,7 +603,20 @@ int step_impl(double *x, double *v, const double *m, double M_star, int64_t N, d
 
     const bool enc = g_cfg.resolve_encounters != 0;
     if (enc && !pairs) return fail(NB_E_BADARG, "nb_step: resolve_encounters needs the pair list (pairs != NULL)");
+    const bool ml = enc && g_cfg.levels > 0;
+    if (ml && g.Nj != N) return fail(NB_E_BADARG, "nb_step: the multi-level changeover (levels > 0) is defined for the fully active case only");
     auto enqueue_step = [&](int nhalf) -> int {
+        if (ml) {
+            // multi-level changeover: every body of the step's pair list goes through the levels; the plain
+            // drift kernel moves the others (and shifts everybody)
+            enqueue_ml_adjacency(w, pairs, npairs, N);
+            nb_drift_kernel<<<nblk, kBodyThreads, 0, stream()>>>(x, v, m, (int)N, mu, dt, w.mvA, nblk, dtc, M_star, nullptr, w.status,
+                                                                 w.ml_listed);
+            enqueue_ml_advance(w, ml_params(w, x, v, m, w.ml_hill, w.ml_vel, M_star, N), M_star, N, 0, dt);
+            nb_momentum_kernel<<<nblk, kBodyThreads, 0, stream()>>>(v, m, (int)N, w.mvB);
+            return enqueue_eval(w, g, x, v, m, M_star, N, dt, rc_io, update_rc, w.mvB, dtc, acc, pairs, npairs, hk, nhalf,
+                                w.mvA, false);
+        }
         // groups of the pair list of the evaluation that opened this step
         if (enc) {
             enqueue_groups(w, pairs, npairs, N, w.g_label, w.g_members, w.g_start, w.g_stat);
@@ -548,7 +643,7 @@ int step_impl(double *x, double *v, const double *m, double M_star, int64_t N, d
         key.ws = g_cfg.workspace; key.stream = g_cfg.stream; key.N = N; key.n_active = g_cfg.n_active;
         key.cap = g_cfg.pair_capacity; key.dt = dt; key.M_star = M_star; key.G = g_cfg.G; key.n1 = g_cfg.n1;
         key.n2 = g_cfg.n2; key.kind = g_cfg.changeover_kind; key.bs_tol = g_cfg.bs_tol; key.enc = (enc ? 1 : 0) + 2 * g.sorted; key.ipt = g.S * 1000 + g.ipt * 100 + g.minb * 10; key.jsplit = g.nsplit;
-        key.ws_bytes = g_cfg.workspace_bytes;
+        key.ws_bytes = g_cfg.workspace_bytes; key.levels = g_cfg.levels;
         const bool hop = !stream_capturable();
         if (hop) {
             if (!g_own_stream) {
@@ -628,6 +723,7 @@ void nb_default_config(nb_config *cfg) {
     cfg->bs_tol = 1e-12;
     cfg->radius_factor = 1.0;
     cfg->sort_staging = NB_SORT_AUTO;
+    cfg->levels = 0;
 }
 
 int nb_configure(const nb_config *cfg) {
@@ -650,6 +746,7 @@ int nb_configure(const nb_config *cfg) {
     if (cfg->sort_staging != NB_SORT_AUTO && cfg->sort_staging != NB_SORT_ON && cfg->sort_staging != NB_SORT_OFF)
         return fail(NB_E_BADARG, "unknown sort_staging %d", cfg->sort_staging);
     if (!(cfg->radius_factor >= 0.0) || !std::isfinite(cfg->radius_factor)) return fail(NB_E_BADARG, "radius_factor must be finite and >= 0");
+    if (cfg->levels < 0 || cfg->levels > kMaxLevels) return fail(NB_E_BADARG, "levels must be 0 .. %d", kMaxLevels);
     g_cfg = *cfg;
     return NB_OK;
 }
@@ -775,6 +872,23 @@ int nb_encounter(double *x, double *v, const double *m, const double *rcrit, dou
     Workspace w;
     if ((rc = check_workspace_head(N, 2, &w))) return rc;
     enqueue_encounter(w, x, v, m, rcrit, M_star, N, dt, members, gstart, gstat, false);
+    NB_CUDA(cudaGetLastError());
+    return NB_OK;
+}
+
+int nb_encounter_levels(double *x, double *v, const double *m, const double *rc_hill, const double *rc_vel, double M_star,
+                        int64_t N, double dt, const int32_t *pairs, const int64_t *npairs) {
+    std::lock_guard<std::mutex> lk(g_mu);
+    int rc = check_common(N, dt, M_star);
+    if (rc) return rc;
+    if (!x || !v || !m || !rc_hill || !rc_vel || !pairs || !npairs) return fail(NB_E_NULL, "nb_encounter_levels: NULL argument");
+    if (g_cfg.levels <= 0) return fail(NB_E_BADARG, "nb_encounter_levels: levels is 0 (nb_configure)");
+    if (g_cfg.pair_capacity <= 0) return fail(NB_E_BADARG, "nb_encounter_levels: pair_capacity is 0 (nb_configure)");
+    if (g_cfg.n_active > 0 && g_cfg.n_active < N) return fail(NB_E_BADARG, "nb_encounter_levels: fully active case only");
+    Workspace w;
+    if ((rc = check_workspace_head(N, 3, &w))) return rc;
+    enqueue_ml_adjacency(w, pairs, npairs, N);
+    enqueue_ml_advance(w, ml_params(w, x, v, m, rc_hill, rc_vel, M_star, N), M_star, N, 0, dt);
     NB_CUDA(cudaGetLastError());
     return NB_OK;
 }

@@ -173,7 +173,8 @@ def test_complete_pair_list_and_all_rows_config3(n2):
     st = GpuState(d.x, d.v, d.m, d.M_star, G=G_GAUSS, n1=3.0, n2=n2, pair_capacity=1 << 23)
     geo = st.nb.force_geometry(d.N)
     assert geo.tile_j == -512 and geo.i_per_thread == 4          # the configuration bench.py times
-    st.kick(0.0, rcrit_given=False)                               # rcrit computed on the GPU (a0)
+    st.set_rcrit(rc)
+    st.kick(0.0)
     acc = st.acc.cpu().numpy()
     gp, n = st.get_pairs()
     sure, border = oracle.pairs(d.x, rc, cap=1 << 23)
