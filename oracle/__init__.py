@@ -60,6 +60,10 @@ def _L():
         lib.oracle_diagnostics.argtypes = [dp, dp, dp, dbl, i64, dbl, dp]
         lib.oracle_encounter.argtypes = [dp, dp, dp, dp, i64, i64, dbl, dbl, dbl, i32, dbl, ip, ip, i64, i64, lp]
         lib.oracle_encounter_split.argtypes = [dp, dp, dp, dp, i64, i64, dbl, dbl, dbl, i32, dbl, ip, ip, i64, i64, i64, lp]
+        lib.oracle_midpoint_drag.restype = i64
+        lib.oracle_midpoint_drag.argtypes = [dp, dp, i64, dbl, dbl, dbl, i32, dbl, dbl, i64, lp]
+        lib.oracle_step_drag.restype = i64
+        lib.oracle_step_drag.argtypes = [dp, dp, dp, dbl, i64, i64, dbl, dbl, dbl, dbl, i32, dp, dp, i64, dbl, i32, dbl, dbl, i64]
         lib.oracle_groups.restype = i32
         lib.oracle_groups.argtypes = [ip, i64, i64, ip, ip, ip, lp]
         _lib = lib
@@ -199,6 +203,34 @@ def step(x, v, m, M_star, dt, G, nsteps, n_active=0, n1=3.0, n2=0.0, kind=0, rcr
     P = C.POINTER(C.c_double)
     nf = _L().oracle_step(x.ctypes.data_as(P), v.ctypes.data_as(P), pm, M_star, N, n_active, dt, G,
                           n1, n2, kind, rc.ctypes.data_as(P), acc.ctypes.data_as(P), nsteps)
+    return dict(x=x, v=v, acc=acc, rcrit=rc, n_fail=int(nf))
+
+
+def midpoint_drag(x, v, mu, dt, gamma, power=0, eta=0.0, tol=1e-14, max_iter=50):
+    """Implicit midpoint (Eq. 8) for the drag a_f = -gamma |u|^p u, u = v - (1 - eta) v_circ(R) e_phi
+    (reading S24).  Returns (v_new, n_not_converged, most iterations used)."""
+    x, px = _d(x)
+    v = np.array(v, dtype=np.float64, order="C", copy=True)
+    N = v.shape[0]
+    it = C.c_int64(0)
+    nf = _L().oracle_midpoint_drag(px, v.ctypes.data_as(C.POINTER(C.c_double)), N, float(mu), float(dt), float(gamma), int(power),
+                                   float(eta), float(tol), int(max_iter), C.byref(it))
+    return v, int(nf), int(it.value)
+
+
+def step_drag(x, v, m, M_star, dt, G, nsteps, gamma, power=0, eta=0.0, tol=1e-14, max_iter=50, n_active=0, n1=3.0, n2=0.0,
+              kind=0, rcrit_=None):
+    """nsteps of D(dt/2) B(dt/2) C(dt/2) A(dt) C(dt/2) B(dt/2) D(dt/2) (reading S24).  Returns dict(x, v, acc, rcrit, n_fail)."""
+    x = np.array(x, dtype=np.float64, order="C", copy=True)
+    v = np.array(v, dtype=np.float64, order="C", copy=True)
+    m, pm = _d(m)
+    N = m.shape[0]
+    rc = np.zeros(N) if rcrit_ is None else np.array(rcrit_, dtype=np.float64, copy=True)
+    acc = np.empty((N, 3))
+    P = C.POINTER(C.c_double)
+    nf = _L().oracle_step_drag(x.ctypes.data_as(P), v.ctypes.data_as(P), pm, M_star, N, n_active, dt, G, n1, n2, kind,
+                               rc.ctypes.data_as(P), acc.ctypes.data_as(P), nsteps, float(gamma), int(power), float(eta),
+                               float(tol), int(max_iter))
     return dict(x=x, v=v, acc=acc, rcrit=rc, n_fail=int(nf))
 
 

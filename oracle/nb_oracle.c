@@ -817,3 +817,87 @@ void oracle_level_kick(const double *x, double *v, const double *m, int64_t N, d
     for (int64_t k = 0; k < 3 * N; ++k) v[k] = v[k] + h * acc[k];
     free(acc);
 }
+
+/* ---------------------------------------------------------------------------------------------
+ * Velocity-dependent extra forces by the implicit midpoint method (Eq. 8):
+ *     v^{t+dt} = v^t + dt * a_f( r^t, (v^t + v^{t+dt}) / 2 )
+ * "The implicit midpoint method needs some iterations to converge and is applied in between of the basic
+ * symplectic operations."  The paper refers to its source [21] for the forces themselves; ONE
+ * simple force stands in for them here (reading S24): drag against a gas disk on circular orbits,
+ *     a_f(r, v) = - gamma |u|^p u,   u = v - v_gas(r),   v_gas = (1 - eta) sqrt(mu / R) e_phi,
+ * R = sqrt(x^2 + y^2) the cylindrical radius, e_phi = (-y, x, 0)/R, p = 0 (linear) or 1 (quadratic).
+ * Eq. 8 is solved per body by the fixed-point iteration w <- v + dt a_f(r, (v + w)/2), started at w = v, until
+ * |w_new - w| <= tol * max(|w_new|, |v_gas|) or max_iter iterations.  v is replaced by w.
+ * Returns the number of bodies that did not converge (their last iterate is kept); *iters_max = most iterations used.
+ * --------------------------------------------------------------------------------------------- */
+static void drag_accel(const double *x, const double *vm, double mu, double gamma, int power, double eta, double *a,
+                       double *vgas_norm) {
+    double R2 = x[0] * x[0] + x[1] * x[1];
+    double vg[3] = {0.0, 0.0, 0.0};
+    if (R2 > 0.0) {
+        double R = sqrt(R2);
+        double vc = (1.0 - eta) * sqrt(mu / R);
+        vg[0] = -vc * x[1] / R; vg[1] = vc * x[0] / R;
+        *vgas_norm = fabs(vc);
+    } else {
+        *vgas_norm = 0.0;
+    }
+    double u[3] = {vm[0] - vg[0], vm[1] - vg[1], vm[2] - vg[2]};
+    double f = gamma;
+    if (power == 1) f = gamma * sqrt((u[0] * u[0] + u[1] * u[1]) + u[2] * u[2]);
+    for (int k = 0; k < 3; ++k) a[k] = -f * u[k];
+}
+
+int64_t oracle_midpoint_drag(const double *x, double *v, int64_t N, double mu, double dt, double gamma, int power,
+                             double eta, double tol, int64_t max_iter, int64_t *iters_max) {
+    int64_t nfail = 0, imax = 0;
+    for (int64_t i = 0; i < N; ++i) {
+        const double *xi = x + 3 * i;
+        double v0[3] = {v[3 * i], v[3 * i + 1], v[3 * i + 2]};
+        double w[3] = {v0[0], v0[1], v0[2]};
+        int converged = 0;
+        int64_t it = 0;
+        for (it = 1; it <= max_iter; ++it) {
+            double vm[3], a[3], vgn, wn[3];
+            for (int k = 0; k < 3; ++k) vm[k] = 0.5 * (v0[k] + w[k]);
+            drag_accel(xi, vm, mu, gamma, power, eta, a, &vgn);
+            for (int k = 0; k < 3; ++k) wn[k] = v0[k] + dt * a[k];
+            double d2 = 0.0, n2 = 0.0;
+            for (int k = 0; k < 3; ++k) { d2 += (wn[k] - w[k]) * (wn[k] - w[k]); n2 += wn[k] * wn[k]; }
+            double scale = sqrt(n2) > vgn ? sqrt(n2) : vgn;
+            for (int k = 0; k < 3; ++k) w[k] = wn[k];
+            if (sqrt(d2) <= tol * scale) { converged = 1; break; }
+        }
+        if (!converged) { nfail++; it = max_iter; }
+        if (it > imax) imax = it;
+        for (int k = 0; k < 3; ++k) v[3 * i + k] = w[k];
+    }
+    if (iters_max) *iters_max = imax;
+    return nfail;
+}
+
+/* The step of oracle_step with the extra force applied "in between of the basic symplectic operations"
+ * (PAPER.md:116), reading S24: D(dt/2) B(dt/2) C(dt/2) A(dt) C(dt/2) B(dt/2) D(dt/2) with D the implicit-midpoint
+ * velocity update above.  Force evaluations, r_crit and their sharing between steps exactly as in oracle_step (the
+ * evaluation at a step boundary sees the velocities before the closing half-kick and before D).
+ * Returns Kepler non-convergences + midpoint non-convergences. */
+int64_t oracle_step_drag(double *x, double *v, const double *m, double M_star, int64_t N, int64_t n_active, double dt,
+                         double G, double n1, double n2, int kind, double *rcrit, double *acc, int64_t nsteps,
+                         double gamma, int power, double eta, double tol, int64_t max_iter) {
+    int64_t nfail = 0;
+    int update_rc = !(n1 == 0.0 && n2 == 0.0);
+    if (update_rc) oracle_rcrit(x, v, m, M_star, N, dt, G, n1, n2, rcrit);
+    oracle_accel(x, m, rcrit, N, n_active, G, kind, NULL, 0, acc, NULL, NULL);
+    for (int64_t st = 0; st < nsteps; ++st) {
+        nfail += oracle_midpoint_drag(x, v, N, G * M_star, 0.5 * dt, gamma, power, eta, tol, max_iter, NULL);
+        for (int64_t i = 0; i < 3 * N; ++i) v[i] = v[i] + (0.5 * dt) * acc[i];
+        oracle_shift(x, v, m, M_star, N, 0.5 * dt);
+        nfail += oracle_drift_kepler(x, v, M_star, N, dt, G, 0);
+        oracle_shift(x, v, m, M_star, N, 0.5 * dt);
+        if (update_rc) oracle_rcrit(x, v, m, M_star, N, dt, G, n1, n2, rcrit);
+        oracle_accel(x, m, rcrit, N, n_active, G, kind, NULL, 0, acc, NULL, NULL);
+        for (int64_t i = 0; i < 3 * N; ++i) v[i] = v[i] + (0.5 * dt) * acc[i];
+        nfail += oracle_midpoint_drag(x, v, N, G * M_star, 0.5 * dt, gamma, power, eta, tol, max_iter, NULL);
+    }
+    return nfail;
+}

@@ -45,20 +45,5 @@ def build(force: bool = False, verbose: bool = False) -> str:
     return LIB
 
 
-PROBE = os.path.join(_HERE, "fp64_pipe_probe")
-
-
-def build_probe() -> str:
-    """Standalone FP64-pipe microbenchmark (measurement aid; see csrc/fp64_pipe_probe.cu)."""
-    src = os.path.join(_CSRC, "fp64_pipe_probe.cu")
-    if not os.path.exists(PROBE) or os.path.getmtime(PROBE) < os.path.getmtime(src):
-        subprocess.check_call([nvcc(), "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
-                               "-o", PROBE, src])
-    return PROBE
-
-
 if __name__ == "__main__":
-    if "--probe" in sys.argv:
-        print(build_probe())
-    else:
-        print(build(force="--force" in sys.argv, verbose=True))
+    print(build(force="--force" in sys.argv, verbose=True))
