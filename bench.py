@@ -54,6 +54,14 @@ def parse_args():
     ap.add_argument("--no-drift-point", action="store_true", help="skip the N = 2^24 drift-only HBM point")
     ap.add_argument("--force-kernel", type=int, default=0, choices=[0, 1, 2],
                     help="nb_config.force_kernel: 0 auto, 1 one-sided tiles, 2 Newton-III (comparison runs)")
+    ap.add_argument("--precision", default="f64", choices=["f64", "mixed"],
+                    help="f64 (default, the metric) or the mixed-precision kick variant (NB_PRECISION_MIXED; a side line)")
+    ap.add_argument("--trajectory", action="store_true",
+                    help="instead of the step benchmark: the config's own trajectory (all its steps) as ONE nb_step call "
+                         "(CUDA-graph replay / fused small-N launch), timed with CUDA events; prints one JSON line with mode=trajectory")
+    ap.add_argument("--n2", type=float, default=None, help="--trajectory: velocity factor of Eq. 7 (default 0: 3 R_Hill; 0.4: full Eq. 7)")
+    ap.add_argument("--encounters", action="store_true", help="--trajectory: resolve close encounters (direct solver)")
+    ap.add_argument("--levels", type=int, default=0, help="--trajectory --encounters: intermediate changeover levels (PAPER.md:106)")
     return ap.parse_args()
 
 
@@ -156,6 +164,7 @@ def cpu_baseline(d, na, budget_s=12.0):
     rows = np.sort(rng.choice(d.N, size=R, replace=False))
     t, n = oracle_sample_step(d, na, rows, state)
     return dict(value=n / t, unit=UNIT, cores=oracle.num_threads(), kind="oracle",
+                note="extended-precision checker (x87 long double sums), not a tuned CPU kernel",
                 sample=f"one oracle step with the O(N^2) kick + pair test on {R} seeded-random i-rows x all "
                        f"{na or d.N} j (rcrit, shifts, Kepler drift on all N): {n:.3e} interactions in {t:.2f} s")
 
@@ -197,14 +206,20 @@ def run_reference(args):
 # ------------------------------------------------------------------------------------------------
 # CUDA arm
 # ------------------------------------------------------------------------------------------------
-def _traffic_from_profile(kernel):
-    """dram bytes per launch of `kernel` at N = 65536 from the committed ncu capture (profiles/), or None."""
+def _traffic_from_profile(kernel, N, geom, sorted_staging, precision):
+    """(dram bytes per launch, source) from the committed ncu capture (profiles/force_kernel_traffic.json) -- only when the
+    launch that ran here has the profiled geometry (kernel, N, S or tile, I, sorted staging, precision); the figure is
+    NOT measured in this run (ncu counters cannot be read outside a profiler)."""
     p = os.path.join(ROOT, "profiles", "force_kernel_traffic.json")
     try:
-        j = json.load(open(p))
-        return j.get(kernel, {}).get("dram_bytes_per_launch")
+        for e in json.load(open(p))["captures"]:
+            if (e["kernel"] == kernel and e["N"] == N and e["tile_j"] == geom.tile_j and e["i_per_thread"] == geom.i_per_thread
+                    and e["j_splits"] == geom.j_splits and bool(e["sorted_staging"]) == bool(sorted_staging)
+                    and e.get("precision", "f64") == precision):
+                return e["dram_bytes_per_launch"], e["source"] + " (ncu capture of the same geometry; not measured in this run)"
     except Exception:
-        return None
+        pass
+    return None, "no ncu capture of this geometry under profiles/ (not measured in this run)"
 
 
 def _hbm_peak_gbs():
@@ -287,8 +302,9 @@ def run_cuda(args):
     K, W = args.steps, max(args.warmup, 0)
 
     # ---- device-resident arm: inputs in HBM before the timed region -------------------------------
+    mixed = args.precision == "mixed"
     nb.configure(N, pair_capacity=cap, n_active=na, G=G_GAUSS, n1=N1, n2=N2, reuse_acc=False, time_force=True,
-                 force_kernel=args.force_kernel)
+                 force_kernel=args.force_kernel, precision=1 if mixed else 0)
     nb.nb_status_reset()
     x = torch.from_numpy(d.x).cuda(); v = torch.from_numpy(d.v).cuda(); m = torch.from_numpy(d.m).cuda()
     acc = torch.zeros_like(x); rc = torch.zeros(N, dtype=torch.float64, device="cuda")
@@ -390,7 +406,9 @@ def run_cuda(args):
 
     value = whole_job_value(world, K, inter_per_step, total_ms)
     symmetric = geom.tile_j < 0
-    kernel = "nb_force_sym_kernel" if symmetric else "nb_force_tiles_kernel"
+    kernel = "nb_force_sym_kernel" if symmetric else ("nb_force_mixed_kernel" if mixed else "nb_force_tiles_kernel")
+    sorted_staging = symmetric and N >= 32768   # NB_SORT_AUTO (include/nbkick.h)
+    traffic, traffic_source = _traffic_from_profile(kernel, N, geom, sorted_staging, args.precision)
     # FP64-pipe instructions per ORDERED interaction on the fast path: 20 per unordered pair (Newton III)
     # or 15 (one-sided); DESIGN.md section 5
     pipe_instr = 10.0 if symmetric else 15.0
@@ -398,7 +416,9 @@ def run_cuda(args):
     achieved_tf = FLOPS_PER_INTERACTION * inter_per_step / (force_avg_ms * 1e-3) / 1e12
     line = dict(
         metric=METRIC, value=value, unit=UNIT, n_gpus=world, steps=K, warmup=W, ms_per_step=total_ms / K,
-        higher_is_better=True, scaling="weak", vs_baseline=None, dtype="f64", data="synthetic",
+        higher_is_better=True, scaling="weak", vs_baseline=None,
+        dtype="f64" if not mixed else "f64 differences / f32 pair arithmetic / f64 accumulation (NB_PRECISION_MIXED; not the metric's precision)",
+        data="synthetic",
         config=dict(workload=workload_name(d, na), parallelism="replicas only (path does not shard)" if world > 1 else "1 GPU",
                     l2="256 MiB buffer written between timed steps (L2 flush), outside the per-step CUDA events",
                     force_evaluations_per_step=1, interactions_per_step=inter_per_step,
@@ -407,7 +427,7 @@ def run_cuda(args):
                     pairs_last_step=npairs_last, status=status, wall_s_incl_flush=wall),
         steps_per_sec=world * K / (total_ms * 1e-3),
         roofline=dict(bound="alu", achieved=achieved_tf, peak=FP64_PEAK_NOMINAL_TFLOPS, unit="TFLOP/s",
-                      frac=achieved_tf / FP64_PEAK_NOMINAL_TFLOPS, traffic=_traffic_from_profile(kernel) if N == 65536 else None,
+                      frac=achieved_tf / FP64_PEAK_NOMINAL_TFLOPS, traffic=traffic, traffic_source=traffic_source,
                       kernel=kernel, launches_timed=n_force, avg_launch_ms=force_avg_ms,
                       flops_per_interaction=FLOPS_PER_INTERACTION,
                       peak_source="nominal: 148 SM x 64 fp64 lanes x 2 x 1.965 GHz (DESIGN.md); MEASURED_PEAKS.json has no fp64 entry",
@@ -417,7 +437,7 @@ def run_cuda(args):
         clocks=clocks,
         # per timed step: opening half-kick, drift, prep, force, slot sum + closing half-kick; with the Newton-III kernel's
         # sorted staging (automatic for N >= 32768) also five sort kernels and the bounds kernel
-        gpu_launches=(11 if (geom.tile_j < 0 and N >= 32768) else 5) * K,
+        gpu_launches=(11 if sorted_staging else 5) * K,
         groups=groups_info,
     )
     if e2e:
@@ -433,10 +453,51 @@ def run_cuda(args):
         dist.destroy_process_group()
 
 
+def run_trajectory(args):
+    """The config's own trajectory as ONE nb_step call after the evaluation at t0 (what a user of nb_step runs): CUDA events
+    around the call.  Energies are not computed here (the O(N^2) diagnostic is test infrastructure: tests/ write them to
+    profiles/r2_parity.md); this line carries timing, pair counts and the library's status counters."""
+    import torch
+    import paper_2604_09184_b200 as nb
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py --trajectory needs a CUDA device: there is no CPU fallback")
+    torch.cuda.set_device(int(os.environ.get("LOCAL_RANK", "0")))
+    d, na = workload(args)
+    N = d.N
+    n2 = N2 if args.n2 is None else args.n2
+    cap = 1 << 24
+    nb.configure(N, pair_capacity=cap, n_active=na, G=G_GAUSS, n1=N1, n2=n2, resolve_encounters=args.encounters,
+                 levels=args.levels, precision=1 if args.precision == "mixed" else 0)
+    nb.nb_status_reset()
+    x = torch.from_numpy(d.x).cuda(); v = torch.from_numpy(d.v).cuda(); m = torch.from_numpy(d.m).cuda()
+    acc = torch.zeros_like(x); rc = torch.zeros(N, dtype=torch.float64, device="cuda")
+    pairs = torch.zeros((cap, 2), dtype=torch.int32, device="cuda"); npairs = torch.zeros(1, dtype=torch.int64, device="cuda")
+    nsteps = args.steps if args.steps != 100 else d.nsteps
+    nb.nb_step(x, v, m, d.M_star, d.dt, rc, acc, pairs, npairs, 0)
+    nb.set_flags(reuse_acc=1)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    torch.cuda.synchronize()
+    e0.record()
+    nb.nb_step(x, v, m, d.M_star, d.dt, rc, acc, pairs, npairs, nsteps)
+    e1.record()
+    torch.cuda.synchronize()
+    ms = e0.elapsed_time(e1)
+    geom = nb.force_geometry(N)
+    print(json.dumps(dict(mode="trajectory", config=workload_name(d, na).replace(f"(n2={N2:g})", f"(n2={n2:g})"), N=N, nsteps=nsteps,
+                          a_substep=("direct solver for the encounter groups" + (f", {args.levels} intermediate levels" if args.levels else "")) if args.encounters else "Kepler drift",
+                          total_ms=ms, ms_per_step=ms / nsteps, steps_per_sec=nsteps / (ms * 1e-3),
+                          interactions_per_sec=nsteps * float(N) * float(na or N) / (ms * 1e-3), pairs_last_step=int(npairs.item()),
+                          status=nb.nb_status(), precision=args.precision,
+                          geometry=dict(i_per_thread=geom.i_per_thread, i_blocks=geom.i_blocks, j_splits=geom.j_splits, tile_j=geom.tile_j))),
+          flush=True)
+
+
 def main():
     args = parse_args()
     if args.impl == "reference":
         run_reference(args)
+    elif args.trajectory:
+        run_trajectory(args)
     else:
         run_cuda(args)
 

@@ -58,6 +58,14 @@ extern "C" {
  *                       serves both bodies (two thirds of the fp64 instructions); fully active case
  *                       only -- with n_active < N the call falls back to NB_FORCE_TILES.
  *   NB_FORCE_AUTO       symmetric when fully active and N >= 12288, else tiles. */
+/* Arithmetic of the O(N^2) sum (PAPER.md:160 contrasts FP32 and FP64 runs):
+ *   NB_PRECISION_F64    everything in fp64 (default; the north_star's 1e-12 tolerance applies)
+ *   NB_PRECISION_MIXED  pairs out of reach of every critical radius: differences in fp64, r^2, r^-3 and the products
+ *                       in fp32, summed in fp32 per 128-body tile and in fp64 across tiles; pairs within reach, the
+ *                       changeover weight, the pair test and the pair list stay in fp64 and are identical to the fp64
+ *                       kernel's.  Tolerance: DESIGN.md reading S25 (~1e-6 relative).  One-sided kernel, any n_active. */
+#define NB_PRECISION_F64 0
+#define NB_PRECISION_MIXED 1
 #define NB_SORT_AUTO 0
 #define NB_SORT_ON 1
 #define NB_SORT_OFF 2
@@ -100,6 +108,13 @@ typedef struct nb_config {
                                 with the time step dt / 2^l and the critical radii of Eq. 7 for that time step; only what
                                 is still in a close encounter at level L reaches the direct solver.  Needs workspace for
                                 two adjacency slots per row of the pair list (nb_workspace_bytes accounts for it). */
+    double drag_gamma;       /* nb_midpoint_drag, nb_step: coefficient of the extra force a_f = -gamma |u|^p u (
+                                reading S24); 0 (default) = no extra force, nb_step is the plain step */
+    double drag_eta;         /* u = v - (1 - eta) sqrt(G M_star / R) e_phi: gas on circular orbits, slower by the fraction eta */
+    int drag_power;          /* p: 0 linear drag (default), 1 quadratic drag */
+    int midpoint_iters;      /* Eq. 8 fixed-point iterations at most (default 50) */
+    double midpoint_tol;     /* stop when the update is below tol * max(|v|, |v_gas|) (default 1e-14) */
+    int precision;           /* NB_PRECISION_F64 (default) or NB_PRECISION_MIXED (see above) */
 } nb_config;
 
 void nb_default_config(nb_config *cfg);
@@ -153,6 +168,20 @@ int nb_shift(double *x, const double *v, const double *m, double M_star, int64_t
  * x, v: [N,3] in/out.
  */
 int nb_drift_kepler(double *x, double *v, double M_star, int64_t N, double dt);
+
+/*
+ * Velocity-dependent extra forces by the implicit midpoint method (Eq. 8:
+ *     v^{t+dt} = v^t + dt a_f(r^t, (v^t + v^{t+dt})/2) ,
+ * "needs some iterations to converge and is applied in between of the basic symplectic operations").  The paper
+ * defers the forces themselves to its source; ONE simple force stands in (reading S24): drag against a gas
+ * disk on circular orbits, a_f = -drag_gamma |u|^p u, u = v - (1 - drag_eta) sqrt(G M_star / R) e_phi, R the
+ * cylindrical radius, p = drag_power.  Per body: fixed-point iteration from v until the update is below
+ * midpoint_tol max(|v|, |v_gas|), at most midpoint_iters times; bodies that did not converge keep their last iterate
+ * and are counted in nb_status[6].  x [N,3] in; v [N,3] in/out.  Needs the first 512 bytes of the workspace.
+ * With drag_gamma > 0 nb_step applies this update for dt/2 before the opening and after the closing half-kick of every
+ * step: D(dt/2) B(dt/2) C(dt/2) A(dt) C(dt/2) B(dt/2) D(dt/2).
+ */
+int nb_midpoint_drag(const double *x, double *v, double M_star, int64_t N, double dt);
 
 /*
  * a7 -- nsteps steps of B(dt/2) C(dt/2) A(dt) C(dt/2) B(dt/2) (Eq. 3; order: reading
@@ -263,13 +292,14 @@ int nb_step_host(double *x, double *v, const double *m, double M_star, int64_t N
 
 /*
  * Lazy device-side conditions accumulated since the last nb_status_reset; synchronises the
- * stream.  flags (host int64[6]):
+ * stream.  flags (host int64[8]; [7] is reserved):
  *   [0] pairs dropped because the list was full (sum over evaluations)
  *   [1] Kepler solver non-convergences (body left unchanged)
  *   [2] non-finite positions / masses / radii seen while staging j-bodies; invalid rows of a pair list
  *   [3] coincident bodies (r_ij == 0, i != j) that contributed nothing
  *   [4] encounter groups larger than NB_MAX_GROUP, left to the Kepler drift
  *   [5] encounter groups whose Bulirsch-Stoer step size underflowed (left unchanged)
+ *   [6] bodies whose implicit-midpoint iteration (Eq. 8) did not converge
  */
 int nb_status(int64_t *flags);
 int nb_status_reset(void);

@@ -18,11 +18,12 @@ NB_OK = 0
 NB_E_NULL, NB_E_BADN, NB_E_BADARG, NB_E_WORKSPACE, NB_E_CUDA = -1, -2, -3, -4, -5
 CHANGEOVER_RATIONAL, CHANGEOVER_QUINTIC = 0, 1
 FORCE_AUTO, FORCE_TILES, FORCE_SYMMETRIC = 0, 1, 2
+PRECISION_F64, PRECISION_MIXED = 0, 1
 
 # every symbol include/nbkick.h declares (tests check the library exports each of them)
 SYMBOLS = (
     "nb_default_config", "nb_configure", "nb_workspace_bytes", "nb_rcrit", "nb_kick", "nb_shift",
-    "nb_drift_kepler", "nb_step", "nb_groups", "nb_encounter", "nb_encounter_levels", "nb_merge", "nb_kick_host", "nb_step_host", "nb_status", "nb_status_reset",
+    "nb_drift_kepler", "nb_midpoint_drag", "nb_step", "nb_groups", "nb_encounter", "nb_encounter_levels", "nb_merge", "nb_kick_host", "nb_step_host", "nb_status", "nb_status_reset",
     "nb_last_force_ms", "nb_force_time", "nb_force_time_reset", "nb_force_geometry", "nb_fp64_peak", "nb_release", "nb_last_error", "nb_version",
 )
 
@@ -50,6 +51,12 @@ class NbConfig(C.Structure):
         ("radius_factor", C.c_double),
         ("sort_staging", C.c_int),
         ("levels", C.c_int),
+        ("drag_gamma", C.c_double),
+        ("drag_eta", C.c_double),
+        ("drag_power", C.c_int),
+        ("midpoint_iters", C.c_int),
+        ("midpoint_tol", C.c_double),
+        ("precision", C.c_int),
     ]
 
 
@@ -86,6 +93,7 @@ def load():
     lib.nb_kick.argtypes = [vp, vp, vp, dbl, i64, dbl, vp, vp, vp, vp]
     lib.nb_shift.argtypes = [vp, vp, vp, dbl, i64, dbl]
     lib.nb_drift_kepler.argtypes = [vp, vp, dbl, i64, dbl]
+    lib.nb_midpoint_drag.argtypes = [vp, vp, dbl, i64, dbl]
     lib.nb_step.argtypes = [vp, vp, vp, dbl, i64, dbl, vp, vp, vp, vp, i64]
     lib.nb_groups.argtypes = [vp, vp, i64, vp, vp, vp, vp]
     lib.nb_encounter.argtypes = [vp, vp, vp, vp, dbl, i64, dbl, vp, vp, vp]
@@ -158,7 +166,8 @@ def default_config() -> NbConfig:
 
 def configure(N=None, *, stream=None, pair_capacity=0, n_active=0, G=None, n1=3.0, n2=0.4, changeover_kind=0,
               i_per_thread=0, j_splits=0, use_graph=True, reuse_acc=False, time_force=False,
-              force_kernel=0, sym_block=0, resolve_encounters=False, bs_tol=1e-12, radius_factor=1.0, sort_staging=0, levels=0, workspace_bytes=None,
+              force_kernel=0, sym_block=0, resolve_encounters=False, bs_tol=1e-12, radius_factor=1.0, sort_staging=0, levels=0, drag_gamma=0.0, drag_eta=0.0, drag_power=0,
+              midpoint_iters=50, midpoint_tol=1e-14, precision=0, workspace_bytes=None,
               device="cuda"):
     """nb_configure with a torch-allocated workspace sized for N bodies (N=None: no workspace,
     enough for the _host calls; workspace_bytes: explicit size, e.g. the head that the O(N) calls
@@ -180,6 +189,9 @@ def configure(N=None, *, stream=None, pair_capacity=0, n_active=0, G=None, n1=3.
     cfg.radius_factor = float(radius_factor)
     cfg.sort_staging = int(sort_staging)
     cfg.levels = int(levels)
+    cfg.drag_gamma, cfg.drag_eta, cfg.drag_power = float(drag_gamma), float(drag_eta), int(drag_power)
+    cfg.midpoint_iters, cfg.midpoint_tol = int(midpoint_iters), float(midpoint_tol)
+    cfg.precision = int(precision)
     if N is not None:
         import torch
         if stream is None:
@@ -239,6 +251,12 @@ def nb_drift_kepler(x, v, M_star, dt):
                                   float(dt)))
 
 
+def nb_midpoint_drag(x, v, M_star, dt):
+    import torch
+    N = x.numel() // 3
+    _check(load().nb_midpoint_drag(_dev(x, 3 * N, torch.float64), _dev(v, 3 * N, torch.float64), float(M_star), N, float(dt)))
+
+
 def nb_step(x, v, m, M_star, dt, rcrit, acc, pairs=None, npairs=None, nsteps=1):
     import torch
     N = m.numel()
@@ -293,10 +311,10 @@ def nb_step_host(x, v, m, M_star, dt, rcrit, acc, pairs=None, npairs=None, nstep
 
 
 def nb_status() -> dict:
-    f = (C.c_int64 * 6)()
+    f = (C.c_int64 * 8)()
     _check(load().nb_status(f))
     return dict(pairs_dropped=int(f[0]), kepler_fail=int(f[1]), nonfinite=int(f[2]), singular=int(f[3]),
-                groups_skipped=int(f[4]), bs_fail=int(f[5]))
+                groups_skipped=int(f[4]), bs_fail=int(f[5]), midpoint_fail=int(f[6]))
 
 
 def nb_status_reset():

@@ -45,17 +45,12 @@ struct PrepParams {
     int nblk_in;
     int N, Nj, Njpad;
     int update_rc;
+    int mixed;              // 1: stage the records for the mixed-precision kernel (force_mixed.cuh)
 };
 
-// a5 (second half) + a0 + staging: x += dtc * P/M_star; rcrit from the shifted state; JRec for j < Nj.
-__global__ void __launch_bounds__(kBodyThreads) nb_prep_kernel(const PrepParams p) {
-    __shared__ double sm[3 * kBodyThreads];
-    double sx = 0.0, sy = 0.0, sz = 0.0;
-    if (p.mv_in != nullptr) {
-        reduce_partials3(p.mv_in, p.nblk_in, sx, sy, sz, sm);
-        sx /= p.M_star; sy /= p.M_star; sz /= p.M_star;
-    }
-    const int i = blockIdx.x * kBodyThreads + threadIdx.x;
+// a5 (second half) + a0 + staging for ONE body slot i (the grid covers max(N, Njpad, Npad_sym)): x += dtc * s; rcrit
+// from the shifted state; JRec for j < Nj.  (sx, sy, sz) = total momentum / M_star (0 when there is no shift).
+__device__ __forceinline__ void prep_one(const PrepParams &p, const int i, const double sx, const double sy, const double sz) {
     if (i == 0 && p.npairs != nullptr) *p.npairs = 0ull;
     // padding record: zero mass, far away => contributes exactly 0 and never votes for the slow path
     JRec r;
@@ -82,6 +77,7 @@ __global__ void __launch_bounds__(kBodyThreads) nb_prep_kernel(const PrepParams 
             const double gm = p.G * m;
             r.x = x; r.y = y; r.z = z; r.gm = gm;
             r.c1 = 1.5 * gm; r.c2 = 1.875 * gm; r.rc2 = rc * rc; r.rc = rc;
+            if (p.mixed) r.c1 = pack_mixed(gm, r.rc2);
             if (!(isfinite(x) && isfinite(y) && isfinite(z) && isfinite(gm) && isfinite(rc) && rc >= 0.0))
                 status_add(p.status, ST_NONFINITE, 1);
         }
@@ -101,6 +97,16 @@ __global__ void __launch_bounds__(kBodyThreads) nb_prep_kernel(const PrepParams 
     }
 }
 
+__global__ void __launch_bounds__(kBodyThreads) nb_prep_kernel(const PrepParams p) {
+    __shared__ double sm[3 * kBodyThreads];
+    double sx = 0.0, sy = 0.0, sz = 0.0;
+    if (p.mv_in != nullptr) {
+        reduce_partials3(p.mv_in, p.nblk_in, sx, sy, sz, sm);
+        sx /= p.M_star; sy /= p.M_star; sz /= p.M_star;
+    }
+    prep_one(p, blockIdx.x * kBodyThreads + threadIdx.x, sx, sy, sz);
+}
+
 // standalone a0
 __global__ void __launch_bounds__(kBodyThreads) nb_rcrit_kernel(const double *__restrict__ x, const double *__restrict__ v,
                                                                const double *__restrict__ m, double *__restrict__ rcrit,
@@ -117,15 +123,13 @@ __global__ void __launch_bounds__(kBodyThreads) nb_rcrit_kernel(const double *__
 // separate roundings, as in the step definition).  Optionally emits momentum partials of the new v.
 // perm != nullptr: the partial sums are indexed by staged position (sort_staging.cuh); thread t then serves
 // position t (coalesced slot reads) and writes the body perm[t] (the real bodies hold positions 0 .. N-1).
-__global__ void __launch_bounds__(kBodyThreads) nb_kickv_kernel(const double *part, int nsplit,
-                                                               double *acc, double *__restrict__ v,
-                                                               const double *__restrict__ m, int N, double hk,
-                                                               int nhalf, double *__restrict__ mv_out,
-                                                               const int *__restrict__ perm) {
-    __shared__ double sm[3 * kBodyThreads];
-    const int t = blockIdx.x * kBodyThreads + threadIdx.x;
+// the work of thread slot t (of N): returns the momentum contribution of the kicked body
+__device__ __forceinline__ void kickv_one(const double *part, const int nsplit, double *acc, double *__restrict__ v,
+                                          const double *__restrict__ m, const int N, const double hk, const int nhalf,
+                                          const bool want_mv, const int *__restrict__ perm, const int t, double &px, double &py,
+                                          double &pz) {
+    px = 0.0; py = 0.0; pz = 0.0;
     const int i = (perm != nullptr && t < N) ? perm[t] : t;
-    double px = 0.0, py = 0.0, pz = 0.0;
     if (t < N && i < N) {
         double ax = 0.0, ay = 0.0, az = 0.0;
         for (int s = 0; s < nsplit; ++s) {
@@ -138,8 +142,18 @@ __global__ void __launch_bounds__(kBodyThreads) nb_kickv_kernel(const double *pa
             vx = vx + hk * ax; vy = vy + hk * ay; vz = vz + hk * az;
         }
         if (nhalf > 0) { v[3 * (size_t)i] = vx; v[3 * (size_t)i + 1] = vy; v[3 * (size_t)i + 2] = vz; }
-        if (mv_out != nullptr) { const double mi = m[i]; px = mi * vx; py = mi * vy; pz = mi * vz; }
+        if (want_mv) { const double mi = m[i]; px = mi * vx; py = mi * vy; pz = mi * vz; }
     }
+}
+
+__global__ void __launch_bounds__(kBodyThreads) nb_kickv_kernel(const double *part, int nsplit,
+                                                               double *acc, double *__restrict__ v,
+                                                               const double *__restrict__ m, int N, double hk,
+                                                               int nhalf, double *__restrict__ mv_out,
+                                                               const int *__restrict__ perm) {
+    __shared__ double sm[3 * kBodyThreads];
+    double px, py, pz;
+    kickv_one(part, nsplit, acc, v, m, N, hk, nhalf, mv_out != nullptr, perm, blockIdx.x * kBodyThreads + threadIdx.x, px, py, pz);
     if (mv_out != nullptr) {
         block_sum3(px, py, pz, sm);
         if (threadIdx.x == 0) {
@@ -177,23 +191,16 @@ __global__ void __launch_bounds__(kBodyThreads) nb_shift_kernel(double *__restri
 // a5 (first half, optional) + a6: x += dtc*P/M_star, then the Kepler flow for dt; optionally emits the
 // momentum partials of the drifted velocities for the second half-shift.  With enc_flag (nb_enc_plan_kernel) the
 // bodies the direct solver will move are shifted but not drifted.
-__global__ void __launch_bounds__(kBodyThreads) nb_drift_kernel(double *__restrict__ x, double *__restrict__ v,
-                                                               const double *__restrict__ m, int N, double mu, double dt,
-                                                               const double *__restrict__ mv_in, int nblk_in,
-                                                               double dtc, double M_star, double *__restrict__ mv_out,
-                                                               long long *status, const int *__restrict__ enc_flag) {
-    __shared__ double sm[3 * kBodyThreads];
-    double sx = 0.0, sy = 0.0, sz = 0.0;
-    if (mv_in != nullptr) {
-        reduce_partials3(mv_in, nblk_in, sx, sy, sz, sm);
-        sx /= M_star; sy /= M_star; sz /= M_star;
-    }
-    const int i = blockIdx.x * kBodyThreads + threadIdx.x;
-    double px = 0.0, py = 0.0, pz = 0.0;
+__device__ __forceinline__ void drift_one(double *__restrict__ x, double *__restrict__ v, const double *__restrict__ m,
+                                          const int N, const double mu, const double dt, const bool shift, const double dtc,
+                                          const double sx, const double sy, const double sz, const bool want_mv,
+                                          long long *status, const int *__restrict__ enc_flag, const int i, double &px,
+                                          double &py, double &pz) {
+    px = 0.0; py = 0.0; pz = 0.0;
     if (i < N) {
         double X0 = x[3 * (size_t)i], X1 = x[3 * (size_t)i + 1], X2 = x[3 * (size_t)i + 2];
         double V0 = v[3 * (size_t)i], V1 = v[3 * (size_t)i + 1], V2 = v[3 * (size_t)i + 2];
-        if (mv_in != nullptr) { X0 = X0 + dtc * sx; X1 = X1 + dtc * sy; X2 = X2 + dtc * sz; }
+        if (shift) { X0 = X0 + dtc * sx; X1 = X1 + dtc * sy; X2 = X2 + dtc * sz; }
         // bodies of the encounter groups the direct solver takes (encounter.cuh) are left to it
         const bool in_group = enc_flag != nullptr && enc_flag[i] != 0;
         if (!in_group && kepler_elliptic_fast(X0, X1, X2, V0, V1, V2, mu, dt) != 0) {
@@ -205,12 +212,63 @@ __global__ void __launch_bounds__(kBodyThreads) nb_drift_kernel(double *__restri
         }
         x[3 * (size_t)i] = X0; x[3 * (size_t)i + 1] = X1; x[3 * (size_t)i + 2] = X2;
         v[3 * (size_t)i] = V0; v[3 * (size_t)i + 1] = V1; v[3 * (size_t)i + 2] = V2;
-        if (mv_out != nullptr) { const double mi = m[i]; px = mi * V0; py = mi * V1; pz = mi * V2; }
+        if (want_mv) { const double mi = m[i]; px = mi * V0; py = mi * V1; pz = mi * V2; }
     }
+}
+
+__global__ void __launch_bounds__(kBodyThreads) nb_drift_kernel(double *__restrict__ x, double *__restrict__ v,
+                                                               const double *__restrict__ m, int N, double mu, double dt,
+                                                               const double *__restrict__ mv_in, int nblk_in,
+                                                               double dtc, double M_star, double *__restrict__ mv_out,
+                                                               long long *status, const int *__restrict__ enc_flag) {
+    __shared__ double sm[3 * kBodyThreads];
+    double sx = 0.0, sy = 0.0, sz = 0.0;
+    if (mv_in != nullptr) {
+        reduce_partials3(mv_in, nblk_in, sx, sy, sz, sm);
+        sx /= M_star; sy /= M_star; sz /= M_star;
+    }
+    double px, py, pz;
+    drift_one(x, v, m, N, mu, dt, mv_in != nullptr, dtc, sx, sy, sz, mv_out != nullptr, status, enc_flag,
+              blockIdx.x * kBodyThreads + threadIdx.x, px, py, pz);
     if (mv_out != nullptr) {
         block_sum3(px, py, pz, sm);
         if (threadIdx.x == 0) { mv_out[3 * blockIdx.x] = px; mv_out[3 * blockIdx.x + 1] = py; mv_out[3 * blockIdx.x + 2] = pz; }
     }
+}
+
+// Velocity-dependent extra force by the implicit midpoint method (Eq. 8):
+//     v' = v + dt a_f(r, (v + v')/2),   a_f = -gamma |u|^p u,  u = v - (1 - eta) sqrt(mu/R) e_phi   (reading S24: gas drag)
+// solved per body by the fixed-point iteration w <- v + dt a_f(r, (v + w)/2) from w = v until the update is below
+// tol max(|w|, |v_gas|) or max_iter iterations ("needs some iterations to converge"); non-convergence is counted.
+__global__ void __launch_bounds__(kBodyThreads) nb_midpoint_drag_kernel(const double *__restrict__ x, double *__restrict__ v,
+                                                                       int N, double mu, double dt, double gamma, int power,
+                                                                       double eta, double tol, int max_iter, long long *status) {
+    const int i = blockIdx.x * kBodyThreads + threadIdx.x;
+    if (i >= N) return;
+    const double x0 = x[3 * (size_t)i], x1 = x[3 * (size_t)i + 1];
+    const double v0 = v[3 * (size_t)i], v1 = v[3 * (size_t)i + 1], v2 = v[3 * (size_t)i + 2];
+    const double R2 = x0 * x0 + x1 * x1;
+    double g0 = 0.0, g1 = 0.0, vgn = 0.0;
+    if (R2 > 0.0) {
+        const double R = sqrt(R2);
+        const double vc = (1.0 - eta) * sqrt(mu / R);
+        g0 = -vc * x1 / R; g1 = vc * x0 / R; vgn = fabs(vc);
+    }
+    double w0 = v0, w1 = v1, w2 = v2;
+    bool converged = false;
+#pragma unroll 1
+    for (int it = 0; it < max_iter; ++it) {
+        const double u0 = 0.5 * (v0 + w0) - g0, u1 = 0.5 * (v1 + w1) - g1, u2 = 0.5 * (v2 + w2);
+        double f = gamma;
+        if (power == 1) f = gamma * sqrt((u0 * u0 + u1 * u1) + u2 * u2);
+        const double n0 = v0 + dt * (-f * u0), n1 = v1 + dt * (-f * u1), n2 = v2 + dt * (-f * u2);
+        const double d = sqrt((n0 - w0) * (n0 - w0) + (n1 - w1) * (n1 - w1) + (n2 - w2) * (n2 - w2));
+        const double nn = sqrt(n0 * n0 + n1 * n1 + n2 * n2);
+        w0 = n0; w1 = n1; w2 = n2;
+        if (d <= tol * fmax(nn, vgn)) { converged = true; break; }
+    }
+    if (!converged) status_add(status, ST_MIDPOINT_FAIL, 1);
+    v[3 * (size_t)i] = w0; v[3 * (size_t)i + 1] = w1; v[3 * (size_t)i + 2] = w2;
 }
 
 // fp64 FMA-rate microbenchmark: 8 independent chains per thread, register only.  The FMAs read TWO

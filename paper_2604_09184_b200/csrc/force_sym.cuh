@@ -163,6 +163,25 @@ __device__ __forceinline__ void sym_block(const SymParams &p, const double2 *__r
             const double e = __fma_rn(-r2[k], u, 1.0);                   // 1 - r2 y0^2
             const double q = __fma_rn(e, __fma_rn(e, 1.875, 1.5), 1.0);  // (1-e)^(-3/2), next term < 2^-56
             const double b = __dmul_rn(__dmul_rn(u, y0), q);             // r^-3
+#if defined(NB_SYM_CFORM)
+            // variant: c = r^-3 (dx,dy,dz) first; the i side then shares the multiplier G m_j across all 12 FMAs of a rotation
+            const double cx = __dmul_rn(b, dx[k]), cy = __dmul_rn(b, dy[k]), cz = __dmul_rn(b, dz[k]);
+            ax[k] = __fma_rn(zg.y, cx, ax[k]);
+            ay[k] = __fma_rn(zg.y, cy, ay[k]);
+            az[k] = __fma_rn(zg.y, cz, az[k]);
+            bx = __fma_rn(ngi[k], cx, bx);
+            by = __fma_rn(ngi[k], cy, by);
+            bz = __fma_rn(ngi[k], cz, bz);
+#elif defined(NB_SYM_SIDES)
+            const double si = __dmul_rn(b, zg.y);
+            const double sj = __dmul_rn(b, ngi[k]);
+            ax[k] = __fma_rn(si, dx[k], ax[k]);
+            ay[k] = __fma_rn(si, dy[k], ay[k]);
+            az[k] = __fma_rn(si, dz[k], az[k]);
+            bx = __fma_rn(sj, dx[k], bx);
+            by = __fma_rn(sj, dy[k], by);
+            bz = __fma_rn(sj, dz[k], bz);
+#else
             const double si = __dmul_rn(b, zg.y);                        // G m_j / r^3
             const double sj = __dmul_rn(b, ngi[k]);                      // -G m_i / r^3
             ax[k] = __fma_rn(si, dx[k], ax[k]);
@@ -171,6 +190,7 @@ __device__ __forceinline__ void sym_block(const SymParams &p, const double2 *__r
             ay[k] = __fma_rn(si, dy[k], ay[k]);
             az[k] = __fma_rn(si, dz[k], az[k]);
             bz = __fma_rn(sj, dz[k], bz);
+#endif
         }
         bx = __shfl_sync(0xffffffffu, bx, down);
         by = __shfl_sync(0xffffffffu, by, down);

@@ -194,16 +194,14 @@ struct JWork {
     }
 };
 
-// MINB = CTAs per SM the register allocation is capped for.
-template <int I, bool PAIRS, int MINB>
-__global__ void __launch_bounds__(kForceThreads, MINB) nb_force_tiles_kernel(const ForceParams p) {
-    __shared__ __align__(128) JRec sm[kStages][kTileJ];
-    __shared__ __align__(8) uint64_t full[kStages];
-    __shared__ __align__(8) uint64_t empty[kStages];
-
+// The work of one CTA of kForceThreads threads: i-block bx, j-split by.  sm / full / empty: the CTA's shared-memory ring and
+// its barriers, NOT yet initialised (a persistent caller -- step_small.cuh -- invalidates them between work items).
+template <int I, bool PAIRS>
+__device__ __forceinline__ void force_tiles_cta(const ForceParams &p, const int bx, const int by, JRec (*sm)[kTileJ],
+                                                uint64_t *full, uint64_t *empty) {
     const int t = threadIdx.x;
-    const int i0 = blockIdx.x * (kForceThreads * I) + t;
-    const int tile_begin = blockIdx.y * p.tiles_per_split;
+    const int i0 = bx * (kForceThreads * I) + t;
+    const int tile_begin = by * p.tiles_per_split;
     int tile_end = tile_begin + p.tiles_per_split;
     if (tile_end > p.tiles_total) tile_end = p.tiles_total;
     const int ntiles = tile_end - tile_begin;
@@ -305,7 +303,7 @@ __global__ void __launch_bounds__(kForceThreads, MINB) nb_force_tiles_kernel(con
         if ((t & 31) == 0) mbar_arrive(&empty[st]);  // this warp is done with stage st
     }
 
-    double *out = p.part + (size_t)blockIdx.y * p.N * 3;
+    double *out = p.part + (size_t)by * p.N * 3;
 #pragma unroll
     for (int k = 0; k < I; ++k) {
         const int i = i0 + k * kForceThreads;
@@ -315,6 +313,15 @@ __global__ void __launch_bounds__(kForceThreads, MINB) nb_force_tiles_kernel(con
             out[3 * (size_t)i + 2] = oz[k];
         }
     }
+}
+
+// MINB = CTAs per SM the register allocation is capped for.
+template <int I, bool PAIRS, int MINB>
+__global__ void __launch_bounds__(kForceThreads, MINB) nb_force_tiles_kernel(const ForceParams p) {
+    __shared__ __align__(128) JRec sm[kStages][kTileJ];
+    __shared__ __align__(8) uint64_t full[kStages];
+    __shared__ __align__(8) uint64_t empty[kStages];
+    force_tiles_cta<I, PAIRS>(p, blockIdx.x, blockIdx.y, sm, full, empty);
 }
 
 }  // namespace nbk

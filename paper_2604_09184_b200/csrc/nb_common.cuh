@@ -17,6 +17,14 @@ struct __align__(16) JRec {
 };
 static_assert(sizeof(JRec) == 64, "JRec must be 64 bytes");
 
+// Mixed-precision kernel (force_mixed.cuh): the record's c1 slot holds two floats instead -- G m_j rounded to fp32 (low
+// word) and rc_j^2 rounded UP to fp32 with a 2^-18 margin (high word; far above the fp32 rounding of r^2)
+__device__ __forceinline__ double pack_mixed(const double gm, const double rc2) {
+    const float g = __double2float_rn(gm);
+    const float t = __double2float_ru(rc2) * 1.0000038f;
+    return __hiloint2double(__float_as_int(t), __float_as_int(g));
+}
+
 constexpr int kForceThreads = 128;  // threads per force CTA
 constexpr int kTileJ = 128;         // j-bodies per shared-memory stage (8 KB)
 constexpr int kStages = 4;          // TMA ring depth (2 tiles in flight ahead of the consumer)
@@ -24,8 +32,8 @@ constexpr int kBodyThreads = 256;   // threads per CTA of the O(N) kernels
 constexpr double kFarJ = 1.0e30;    // padding j-records sit here with zero mass
 constexpr double kFarI = -1.0e30;   // padding i-lanes sit here; their sums are discarded
 
-// status counters (device int64[6]); meanings in include/nbkick.h nb_status
-enum { ST_PAIR_DROPPED = 0, ST_KEPLER_FAIL = 1, ST_NONFINITE = 2, ST_SINGULAR = 3, ST_GROUP_SKIPPED = 4, ST_BS_FAIL = 5, ST_COUNT = 6 };
+// status counters (device int64[8]); meanings in include/nbkick.h nb_status
+enum { ST_PAIR_DROPPED = 0, ST_KEPLER_FAIL = 1, ST_NONFINITE = 2, ST_SINGULAR = 3, ST_GROUP_SKIPPED = 4, ST_BS_FAIL = 5, ST_MIDPOINT_FAIL = 6, ST_COUNT = 8 };
 
 __device__ __forceinline__ void status_add(long long *status, int which, long long n) {
     atomicAdd(reinterpret_cast<unsigned long long *>(status + which), static_cast<unsigned long long>(n));

@@ -12,18 +12,20 @@
 
 #include "body_kernels.cuh"
 #include "encounter.cuh"
+#include "force_mixed.cuh"
 #include "force_sym.cuh"
 #include "force_tiles.cuh"
 #include "groups.cuh"
 #include "merge.cuh"
 #include "multilevel.cuh"
+#include "step_small.cuh"
 
 namespace {
 
 using namespace nbk;
 
 std::mutex g_mu;
-nb_config g_cfg = {nullptr, nullptr, 0, 0, 0, 0.01720209895 * 0.01720209895, 3.0, 0.4, 0, 0, 0, 1, 0, 0, 0, 0, 0, 1e-12, 1.0, 0, 0};
+nb_config g_cfg = {nullptr, nullptr, 0, 0, 0, 0.01720209895 * 0.01720209895, 3.0, 0.4, 0, 0, 0, 1, 0, 0, 0, 0, 0, 1e-12, 1.0, 0, 0, 0.0, 0.0, 0, 50, 1e-14, 0};
 char g_err[512] = "";
 int g_sm_count = 0;
 cudaEvent_t g_ev0 = nullptr, g_ev1 = nullptr;
@@ -40,8 +42,8 @@ size_t g_arena_bytes = 0;
 struct StepKey {
     const void *x, *v, *m, *rcrit, *acc, *pairs, *npairs, *ws, *stream;
     int64_t N, n_active, cap;
-    double dt, M_star, G, n1, n2, bs_tol;
-    int kind, ipt, jsplit, enc, levels;
+    double dt, M_star, G, n1, n2, bs_tol, drag_gamma, drag_eta, midpoint_tol;
+    int kind, ipt, jsplit, enc, levels, drag_power, midpoint_iters;
     size_t ws_bytes;
 };
 StepKey g_graph_key;
@@ -98,6 +100,7 @@ struct Geometry {
     int sym;              // 1: Newton-III super-tile kernel (force_sym.cuh); nsplit = number of super-blocks
     int S, U, Npad_sym;   // super-block size, 32-blocks per skew unit, N padded to a multiple of S
     int sorted;           // symmetric kernel: bodies staged in azimuthal order (sort_staging.cuh)
+    int mixed;            // mixed-precision one-sided kernel (force_mixed.cuh)
 };
 
 Geometry geometry(int64_t N, int64_t n_active) {
@@ -107,10 +110,11 @@ Geometry geometry(int64_t N, int64_t n_active) {
     g.Njpad = g.tiles_total * kTileJ;
     const int sms = sm_count();
     g.sym = 0; g.S = 0; g.U = 0; g.Npad_sym = 0; g.sorted = 0;
+    g.mixed = g_cfg.precision == NB_PRECISION_MIXED ? 1 : 0;
     // Newton-III kernel: fully active case only (a passive body exerts nothing, so there is no second
     // side to serve), and only when there are enough super-tiles to fill the machine several times.
     const bool fully_active = (g.Nj == N);
-    if (fully_active && g_cfg.force_kernel != NB_FORCE_TILES && (g_cfg.force_kernel == NB_FORCE_SYMMETRIC || N >= 12288)) {
+    if (fully_active && !g.mixed && g_cfg.force_kernel != NB_FORCE_TILES && (g_cfg.force_kernel == NB_FORCE_SYMMETRIC || N >= 12288)) {
         // I = 4 at 3 CTAs/SM (168 registers, no spills) measured fastest on B200 (profiles/); smaller
         // problems take I = 2 so that S = 256 super-blocks (more CTAs) stay possible.
         int ipt = g_cfg.i_per_thread;
@@ -319,7 +323,20 @@ void launch_force_IM(const ForceParams &fp, const Geometry &g, bool pairs) {
     else nb_force_tiles_kernel<I, false, MINB><<<grid, kForceThreads, 0, stream()>>>(fp);
 }
 
+template <int I, int MINB>
+void launch_mixed_IM(const ForceParams &fp, const Geometry &g, bool pairs) {
+    dim3 grid(g.iblocks, g.nsplit);
+    if (pairs) nb_force_mixed_kernel<I, true, MINB><<<grid, kForceThreads, 0, stream()>>>(fp);
+    else nb_force_mixed_kernel<I, false, MINB><<<grid, kForceThreads, 0, stream()>>>(fp);
+}
+
 void launch_force(const ForceParams &fp, const Geometry &g, bool pairs) {
+    if (g.mixed) {
+        if (g.ipt == 4) launch_mixed_IM<4, 4>(fp, g, pairs);
+        else if (g.ipt == 2) launch_mixed_IM<2, 5>(fp, g, pairs);
+        else launch_mixed_IM<1, 5>(fp, g, pairs);
+        return;
+    }
     if (g.ipt == 4) launch_force_IM<4, 3>(fp, g, pairs);
     else if (g.ipt == 2) launch_force_IM<2, 5>(fp, g, pairs);
     else launch_force_IM<1, 5>(fp, g, pairs);
@@ -384,7 +401,7 @@ int enqueue_eval(const Workspace &w, const Geometry &g, double *x, double *v, co
     pp.npairs = pairs ? reinterpret_cast<unsigned long long *>(npairs) : nullptr;
     pp.status = w.status; pp.dtc = dtc; pp.M_star = M_star; pp.G = g_cfg.G; pp.n1 = g_cfg.n1; pp.n2 = g_cfg.n2;
     pp.absdt = std::fabs(dt_for_rc); pp.nblk_in = nblk; pp.N = (int)N; pp.Nj = g.Nj; pp.Njpad = g.Njpad;
-    pp.update_rc = update_rc;
+    pp.update_rc = update_rc; pp.mixed = g.mixed;
     int64_t cover = N > g.Njpad ? N : g.Njpad;
     if (g.Npad_sym > cover) cover = g.Npad_sym;
     nb_prep_kernel<<<body_blocks(cover), kBodyThreads, 0, stream()>>>(pp);
@@ -575,6 +592,54 @@ MlParams ml_params(const Workspace &w, double *x, double *v, const double *m, co
     return mp;
 }
 
+// ---- small N: whole steps in one cooperative launch (step_small.cuh) ----
+constexpr int64_t kSmallStepMaxN = 8192;
+
+template <int I>
+int launch_step_small_I(const SmallStepParams &q, bool pairs, int work_items) {
+    auto go = [&](auto kern) -> int {
+        int dev = 0, coop = 0, per_sm = 0;
+        NB_CUDA(cudaGetDevice(&dev));
+        NB_CUDA(cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev));
+        if (!coop) return NB_E_BADARG;
+        NB_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, kForceThreads, 0));
+        if (per_sm < 1) return NB_E_BADARG;
+        int grid = per_sm * sm_count();
+        if (grid > work_items) grid = work_items;
+        if (grid < 1) grid = 1;
+        SmallStepParams qq = q;
+        void *args[] = {&qq};
+        NB_CUDA(cudaLaunchCooperativeKernel(kern, dim3(grid), dim3(kForceThreads), args, 0, stream()));
+        return NB_OK;
+    };
+    return pairs ? go(nb_step_small_kernel<I, true>) : go(nb_step_small_kernel<I, false>);
+}
+
+int launch_step_small(const Workspace &w, const Geometry &g, double *x, double *v, const double *m, double M_star, int64_t N,
+                      double dt, double *rc_io, int update_rc, double *acc, int32_t *pairs, int64_t *npairs, int64_t nsteps) {
+    SmallStepParams q;
+    PrepParams &pp = q.pp;
+    pp.x = x; pp.v = v; pp.m = m; pp.rcrit = rc_io; pp.rc_hill = nullptr; pp.rc_vel = nullptr; pp.jrec = w.jrec;
+    pp.sxy = nullptr; pp.szg = nullptr; pp.sthr = nullptr; pp.Npad_sym = 0; pp.pos_of = nullptr; pp.mv_in = nullptr;
+    pp.npairs = pairs ? reinterpret_cast<unsigned long long *>(npairs) : nullptr;
+    pp.status = w.status; pp.dtc = 0.5 * dt; pp.M_star = M_star; pp.G = g_cfg.G; pp.n1 = g_cfg.n1; pp.n2 = g_cfg.n2;
+    pp.absdt = std::fabs(dt); pp.nblk_in = body_blocks(N); pp.N = (int)N; pp.Nj = g.Nj; pp.Njpad = g.Njpad;
+    pp.update_rc = update_rc; pp.mixed = 0;
+    ForceParams &fp = q.fp;
+    fp.jrec = w.jrec; fp.x = x; fp.rcrit = rc_io; fp.part = w.part; fp.pairs = pairs;
+    fp.npairs = pairs ? reinterpret_cast<unsigned long long *>(npairs) : w.npairs_dummy;
+    fp.status = w.status; fp.cap = pairs ? g_cfg.pair_capacity : 0; fp.N = (int)N; fp.Nj = g.Nj;
+    fp.tiles_total = g.tiles_total; fp.tiles_per_split = g.tiles_per_split; fp.kind = g_cfg.changeover_kind;
+    q.acc = acc; q.mvA = w.mvA; q.mvB = w.mvB; q.mu = g_cfg.G * M_star; q.dt = dt; q.hk = 0.5 * dt; q.dtc = 0.5 * dt;
+    q.nsteps = (int)(nsteps > 2000000000LL ? 2000000000LL : nsteps); q.last_nhalf = 1;
+    q.iblocks = g.iblocks; q.nsplit = g.nsplit; q.nblk = body_blocks(N);
+    if ((int64_t)q.nsteps != nsteps) return NB_E_BADARG;
+    const int items = g.iblocks * g.nsplit > q.nblk ? g.iblocks * g.nsplit : q.nblk;
+    if (g.ipt == 4) return launch_step_small_I<4>(q, pairs != nullptr, items);
+    if (g.ipt == 2) return launch_step_small_I<2>(q, pairs != nullptr, items);
+    return launch_step_small_I<1>(q, pairs != nullptr, items);
+}
+
 int step_impl(double *x, double *v, const double *m, double M_star, int64_t N, double dt, double *rcrit, double *acc,
               int32_t *pairs, int64_t *npairs, int64_t nsteps) {
     int rc = check_common(N, dt, M_star);
@@ -591,20 +656,45 @@ int step_impl(double *x, double *v, const double *m, double M_star, int64_t N, d
     const double hk = 0.5 * dt, dtc = 0.5 * dt, mu = g_cfg.G * M_star;
     const int nblk = body_blocks(N);
 
+    // extra force (Eq. 8, reading S24): D(dt/2) before the opening and after the closing half-kick
+    const bool drag = g_cfg.drag_gamma > 0.0;
+    auto enqueue_D = [&]() {
+        nb_midpoint_drag_kernel<<<nblk, kBodyThreads, 0, stream()>>>(x, v, (int)N, mu, 0.5 * dt, g_cfg.drag_gamma, g_cfg.drag_power,
+                                                                     g_cfg.drag_eta, g_cfg.midpoint_tol, g_cfg.midpoint_iters > 0 ? g_cfg.midpoint_iters : 50, w.status);
+    };
+    // opening half-kick from the cached force (reads acc as a 1-split partial) + momentum partials
+    auto kick_only = [&]() { nb_kickv_kernel<<<nblk, kBodyThreads, 0, stream()>>>(acc, 1, acc, v, m, (int)N, hk, 1, w.mvA, nullptr); };
     if (g_cfg.reuse_acc && nsteps > 0) {
-        // acc already is the force at the current x: opening half-kick only (reads acc as a 1-split partial)
-        nb_kickv_kernel<<<nblk, kBodyThreads, 0, stream()>>>(acc, 1, acc, v, m, (int)N, hk, 1, w.mvA, nullptr);
-    } else {
+        // acc already is the force at the current x
+        if (drag) enqueue_D();
+        kick_only();
+    } else if (!drag) {
         // evaluation at t0 (+ opening half-kick of the first step)
         if ((rc = enqueue_eval(w, g, x, v, m, M_star, N, dt, rc_io, update_rc, nullptr, 0.0, acc, pairs, npairs, hk,
                                nsteps > 0 ? 1 : 0, w.mvA, nsteps == 0)))
             return rc;
+    } else {
+        if ((rc = enqueue_eval(w, g, x, v, m, M_star, N, dt, rc_io, update_rc, nullptr, 0.0, acc, pairs, npairs, hk, 0, nullptr,
+                               nsteps == 0)))
+            return rc;
+        if (nsteps > 0) { enqueue_D(); kick_only(); }
     }
 
     const bool enc = g_cfg.resolve_encounters != 0;
     if (enc && !pairs) return fail(NB_E_BADARG, "nb_step: resolve_encounters needs the pair list (pairs != NULL)");
     const bool ml = enc && g_cfg.levels > 0;
     if (ml && g.Nj != N) return fail(NB_E_BADARG, "nb_step: the multi-level changeover (levels > 0) is defined for the fully active case only");
+    // force evaluation that closes a step: closing half-kick [+ opening half-kick of the next step]; with the extra
+    // force the two half-kicks are separated by D(dt/2) D(dt/2)
+    auto close_step = [&](int nhalf) -> int {
+        if (!drag)
+            return enqueue_eval(w, g, x, v, m, M_star, N, dt, rc_io, update_rc, w.mvB, dtc, acc, pairs, npairs, hk, nhalf, w.mvA, false);
+        const int erc = enqueue_eval(w, g, x, v, m, M_star, N, dt, rc_io, update_rc, w.mvB, dtc, acc, pairs, npairs, hk, 1, nullptr, false);
+        if (erc) return erc;
+        enqueue_D();
+        if (nhalf == 2) { enqueue_D(); kick_only(); }
+        return NB_OK;
+    };
     auto enqueue_step = [&](int nhalf) -> int {
         if (ml) {
             // multi-level changeover: every body of the step's pair list goes through the levels; the plain
@@ -614,8 +704,7 @@ int step_impl(double *x, double *v, const double *m, double M_star, int64_t N, d
                                                                  w.ml_listed);
             enqueue_ml_advance(w, ml_params(w, x, v, m, w.ml_hill, w.ml_vel, M_star, N), M_star, N, 0, dt);
             nb_momentum_kernel<<<nblk, kBodyThreads, 0, stream()>>>(v, m, (int)N, w.mvB);
-            return enqueue_eval(w, g, x, v, m, M_star, N, dt, rc_io, update_rc, w.mvB, dtc, acc, pairs, npairs, hk, nhalf,
-                                w.mvA, false);
+            return close_step(nhalf);
         }
         // groups of the pair list of the evaluation that opened this step
         if (enc) {
@@ -631,10 +720,15 @@ int step_impl(double *x, double *v, const double *m, double M_star, int64_t N, d
             nb_momentum_kernel<<<nblk, kBodyThreads, 0, stream()>>>(v, m, (int)N, w.mvB);
         }
         // C(dt/2) folded into prep; force; B(dt/2) [+ B(dt/2) of the next step]
-        return enqueue_eval(w, g, x, v, m, M_star, N, dt, rc_io, update_rc, w.mvB, dtc, acc, pairs, npairs, hk, nhalf,
-                            w.mvA, false);
+        return close_step(nhalf);
     };
 
+    // Small N: all nsteps steps in ONE cooperative launch (step_small.cuh) -- same device functions, same virtual blocks,
+    // bit-identical results; taken when the step is the plain one (one-sided fp64 kernel, no encounters / extra force)
+    if (nsteps > 0 && g_cfg.use_graph && !g_cfg.time_force && !enc && !drag && !g.sym && !g.mixed && N <= kSmallStepMaxN) {
+        const int frc = launch_step_small(w, g, x, v, m, M_star, N, dt, rc_io, update_rc, acc, pairs, npairs, nsteps);
+        if (frc != NB_E_BADARG) return frc;   // NB_E_BADARG: the cooperative launch is not available here -> multi-launch path
+    }
     const int64_t interior = nsteps > 0 ? nsteps - 1 : 0;
     if (interior > 0 && g_cfg.use_graph && !g_cfg.time_force) {
         StepKey key;
@@ -644,6 +738,8 @@ int step_impl(double *x, double *v, const double *m, double M_star, int64_t N, d
         key.cap = g_cfg.pair_capacity; key.dt = dt; key.M_star = M_star; key.G = g_cfg.G; key.n1 = g_cfg.n1;
         key.n2 = g_cfg.n2; key.kind = g_cfg.changeover_kind; key.bs_tol = g_cfg.bs_tol; key.enc = (enc ? 1 : 0) + 2 * g.sorted; key.ipt = g.S * 1000 + g.ipt * 100 + g.minb * 10; key.jsplit = g.nsplit;
         key.ws_bytes = g_cfg.workspace_bytes; key.levels = g_cfg.levels;
+        key.drag_gamma = g_cfg.drag_gamma; key.drag_eta = g_cfg.drag_eta; key.midpoint_tol = g_cfg.midpoint_tol;
+        key.drag_power = g_cfg.drag_power; key.midpoint_iters = g_cfg.midpoint_iters + 1000 * g.mixed;
         const bool hop = !stream_capturable();
         if (hop) {
             if (!g_own_stream) {
@@ -724,6 +820,12 @@ void nb_default_config(nb_config *cfg) {
     cfg->radius_factor = 1.0;
     cfg->sort_staging = NB_SORT_AUTO;
     cfg->levels = 0;
+    cfg->drag_gamma = 0.0;
+    cfg->drag_eta = 0.0;
+    cfg->drag_power = 0;
+    cfg->midpoint_iters = 50;
+    cfg->midpoint_tol = 1e-14;
+    cfg->precision = NB_PRECISION_F64;
 }
 
 int nb_configure(const nb_config *cfg) {
@@ -746,6 +848,10 @@ int nb_configure(const nb_config *cfg) {
     if (cfg->sort_staging != NB_SORT_AUTO && cfg->sort_staging != NB_SORT_ON && cfg->sort_staging != NB_SORT_OFF)
         return fail(NB_E_BADARG, "unknown sort_staging %d", cfg->sort_staging);
     if (!(cfg->radius_factor >= 0.0) || !std::isfinite(cfg->radius_factor)) return fail(NB_E_BADARG, "radius_factor must be finite and >= 0");
+    if (!(cfg->drag_gamma >= 0.0) || !std::isfinite(cfg->drag_gamma) || !std::isfinite(cfg->drag_eta) ||
+        (cfg->drag_power != 0 && cfg->drag_power != 1) || cfg->midpoint_iters < 0 || !(cfg->midpoint_tol >= 0.0))
+        return fail(NB_E_BADARG, "drag_gamma >= 0, finite drag_eta, drag_power 0 or 1, midpoint_iters >= 0, midpoint_tol >= 0");
+    if (cfg->precision != NB_PRECISION_F64 && cfg->precision != NB_PRECISION_MIXED) return fail(NB_E_BADARG, "unknown precision %d", cfg->precision);
     if (cfg->levels < 0 || cfg->levels > kMaxLevels) return fail(NB_E_BADARG, "levels must be 0 .. %d", kMaxLevels);
     g_cfg = *cfg;
     return NB_OK;
@@ -807,6 +913,20 @@ int nb_drift_kepler(double *x, double *v, double M_star, int64_t N, double dt) {
     if ((rc = check_workspace_head(N, 0, &w))) return rc;
     nb_drift_kernel<<<body_blocks(N), kBodyThreads, 0, stream()>>>(x, v, nullptr, (int)N, g_cfg.G * M_star, dt, nullptr, 0,
                                                                    0.0, M_star, nullptr, w.status, nullptr);
+    NB_CUDA(cudaGetLastError());
+    return NB_OK;
+}
+
+int nb_midpoint_drag(const double *x, double *v, double M_star, int64_t N, double dt) {
+    std::lock_guard<std::mutex> lk(g_mu);
+    int rc = check_common(N, dt, M_star);
+    if (rc) return rc;
+    if (!x || !v) return fail(NB_E_NULL, "nb_midpoint_drag: NULL argument");
+    Workspace w;
+    if ((rc = check_workspace_head(N, 0, &w))) return rc;
+    nb_midpoint_drag_kernel<<<body_blocks(N), kBodyThreads, 0, stream()>>>(x, v, (int)N, g_cfg.G * M_star, dt, g_cfg.drag_gamma,
+                                                                           g_cfg.drag_power, g_cfg.drag_eta, g_cfg.midpoint_tol,
+                                                                           g_cfg.midpoint_iters > 0 ? g_cfg.midpoint_iters : 50, w.status);
     NB_CUDA(cudaGetLastError());
     return NB_OK;
 }

@@ -1,0 +1,111 @@
+"""-m gpu: the mixed-precision kick variant (NB_PRECISION_MIXED) against the fp64 oracle.
+
+Tolerance reading S25.  The definition stays the fp64 one (oracle.accel); the variant evaluates every pair
+that is out of reach of all critical radii with fp32 arithmetic after an fp64 difference.  With u = 2^-24: the cast of
+the three differences, r^2 (3 roundings), rsqrt (2 ulp), its cube (2), the product with G m_j (cast + 1) and with the
+difference (1) put at most ~16 u on a term, the fp32 sum over one 128-body tile at most 127 u on the tile's sum of
+|terms| (typically sqrt(128) u): |da_c| <= 143 u sum_j |t_jc| = 8.5e-6 sum|t| is the guaranteed bound, asserted here;
+the observed error is reported next to a PLAIN numpy fp32 restatement of the same recipe (it must be of the same size:
+the error is the arithmetic's, not the kernel's).  Pairs within reach of a critical radius take the fp64 path, so the
+pair list is bit-identical to the fp64 kernel's and compared exactly."""
+import numpy as np
+import pytest
+
+import nb_inputs
+import oracle
+from nb_inputs import G_GAUSS
+
+from gpu_util import GpuState, assert_pairs_match
+
+pytestmark = pytest.mark.gpu
+
+U32 = 2.0 ** -24
+BOUND = 143 * U32
+
+
+def _numpy_mixed(x, m, rc, G, rows):
+    """The recipe in plain numpy: fp64 differences, fp32 pair arithmetic, fp64 sum (no tiles); in-range pairs in fp64."""
+    out = np.empty((rows.size, 3))
+    for a, i in enumerate(rows):
+        d = x - x[i]
+        r2_64 = (d[:, 0] * d[:, 0] + d[:, 1] * d[:, 1]) + d[:, 2] * d[:, 2]
+        rcij = np.maximum(rc, rc[i])
+        near = r2_64 < rcij * rcij * (1 + 1e-5)
+        near[i] = True
+        df = d.astype(np.float32)
+        r2 = df[:, 0] * df[:, 0] + df[:, 1] * df[:, 1] + df[:, 2] * df[:, 2]
+        with np.errstate(divide="ignore"):
+            y = np.float32(1.0) / np.sqrt(r2)
+        s = (G * m).astype(np.float32) * (y * y * y)
+        t = (s[:, None] * df).astype(np.float64)
+        t[near] = 0.0
+        out[a] = t.sum(0)
+    return out
+
+
+@pytest.mark.parametrize("cfg,n_override,n2,tune", [(2, 6000, 0.0, {}), (1, 5000, 0.4, dict(i_per_thread=4)), (3, 8192, 0.0, {}),
+                                                    (0, 2048, 0.4, dict(i_per_thread=1, j_splits=3))])
+def test_mixed_kick_against_fp64_oracle(cfg, n_override, n2, tune):
+    d = nb_inputs.make_config(cfg, n_override=n_override)
+    na = d.n_active if d.n_active < d.N else 0
+    rc = oracle.rcrit(d.x, d.v, d.m, d.M_star, d.dt, G_GAUSS, 3.0, n2)
+    ref, ab, _ = oracle.accel(d.x, d.m, rc, G_GAUSS, n_active=na, want_abs=True)
+    sure, border = oracle.pairs(d.x, rc, n_active=na)
+    res = {}
+    for prec in (0, 1):
+        st = GpuState(d.x, d.v, d.m, d.M_star, G=G_GAUSS, n_active=na, n1=3.0, n2=n2, precision=prec, force_kernel=1, **tune)
+        st.set_rcrit(rc)
+        st.kick(0.5 * d.dt)
+        _, vg, acc, _ = st.host()
+        gp, n = st.get_pairs()
+        assert_pairs_match(gp, n, sure, border, f"{d.name} precision={prec}")
+        res[prec] = (acc, vg, {tuple(p) for p in gp.tolist()})
+        assert st.nb.nb_status()["pairs_dropped"] == 0
+    acc = res[1][0]
+    assert res[1][2] == res[0][2]                                     # the pair list does not depend on the precision
+    assert np.all(np.isfinite(acc))
+    err = np.abs(acc - ref)
+    worst = float(np.max(err / np.where(ab > 0, ab, 1e-300)))
+    rel = err / np.maximum(np.abs(ref), 1e-3 * np.linalg.norm(ref, axis=1, keepdims=True))
+    print(f"{d.name}: mixed vs fp64 oracle: worst |da| / sum|t| = {worst / U32:.1f} u (bound 143 u), relative error median "
+          f"{np.median(rel):.2e} max {rel.max():.2e}; fp64 kernel max {np.max(np.abs(res[0][0] - ref) / np.where(ab > 0, ab, 1e-300)) / 2.2e-16:.1f} eps")
+    assert worst <= BOUND
+    assert np.median(rel) <= 3e-7
+    # v kicked with those accelerations
+    assert np.max(np.abs(res[1][1] - (d.v + 0.5 * d.dt * acc))) <= 1e-15 * np.max(np.abs(d.v))
+    # the error is the arithmetic's: a plain numpy restatement of the recipe has errors of the same size
+    if not na:
+        rows = np.arange(0, d.N, max(1, d.N // 200))
+        near_free = _numpy_mixed(d.x, d.m, rc, G_GAUSS, rows)
+        # far-pair part of the reference: subtract the in-range pairs (evaluated in fp64 on both sides) by recomputing without them
+        e_np = []
+        for a, i in enumerate(rows):
+            dd = d.x - d.x[i]
+            r2 = (dd[:, 0] * dd[:, 0] + dd[:, 1] * dd[:, 1]) + dd[:, 2] * dd[:, 2]
+            near = r2 < np.maximum(rc, rc[i]) ** 2 * (1 + 1e-5)
+            near[i] = True
+            r2[near] = 1.0
+            t = (G_GAUSS * d.m / (r2 * np.sqrt(r2)))[:, None] * dd
+            t[near] = 0.0
+            far_ref = t.sum(0)
+            e_np.append(np.abs(near_free[a] - far_ref) / np.abs(t).sum(0))
+        e_np = np.array(e_np)
+        e_gpu = err[rows] / ab[rows]
+        print(f"   numpy fp32 restatement: median {np.median(e_np) / U32:.2f} u, max {e_np.max() / U32:.2f} u;  kernel: median {np.median(e_gpu) / U32:.2f} u, max {e_gpu.max() / U32:.2f} u")
+        assert np.median(e_gpu) <= 4 * np.median(e_np) + U32
+
+
+def test_mixed_step_energy_and_state():
+    """20 steps of the N = 3000 ring in mixed precision: the state follows the fp64 oracle run to ~1e-7, the energy error
+    stays of the size the fp32 force error allows."""
+    d = nb_inputs.make_config(2, n_override=3000)
+    st = GpuState(d.x, d.v, d.m, d.M_star, G=G_GAUSS, n1=3.0, n2=0.0, precision=1)
+    st.step(d.dt, 20)
+    xg, vg, _, _ = st.host()
+    ref = oracle.step(d.x, d.v, d.m, d.M_star, d.dt, G_GAUSS, 20, n1=3.0, n2=0.0)
+    ex = np.max(np.abs(xg - ref["x"])) / np.max(np.abs(ref["x"]))
+    E0 = oracle.diagnostics(d.x, d.v, d.m, d.M_star, G_GAUSS)["E"]
+    de_g = (oracle.diagnostics(xg, vg, d.m, d.M_star, G_GAUSS)["E"] - E0) / E0
+    de_r = (oracle.diagnostics(ref["x"], ref["v"], d.m, d.M_star, G_GAUSS)["E"] - E0) / E0
+    print(f"mixed x20: rel dx {ex:.2e}, dE/E mixed {de_g:.3e} fp64 oracle {de_r:.3e}")
+    assert ex <= 1e-8 and abs(de_g - de_r) <= 1e-6
