@@ -14,7 +14,7 @@ from gpu_util import GpuState, to_dev, torch_mod
 pytestmark = pytest.mark.gpu
 
 
-@pytest.mark.parametrize("power,gamma,eta", [(0, 0.02, 0.0), (0, 0.05, 0.01), (1, 5.0, 0.005), (1, 20.0, 1.0)])
+@pytest.mark.parametrize("power,gamma,eta", [(0, 0.02, 0.0), (0, 0.05, 0.01), (1, 5.0, 0.005), (1, 4.0, 1.0)])  # gas at rest: gamma |v| dt <= 0.3, the iteration contracts (gamma = 20 does not: 802 bodies diverge in the oracle itself)
 def test_midpoint_drag_against_oracle(power, gamma, eta):
     import paper_2604_09184_b200 as nb
     torch = torch_mod()
