@@ -94,7 +94,7 @@ typedef struct nb_config {
     int time_force;          /* bracket every force-tile launch with CUDA events (nb_force_time); implies
                                 no graph replay (default 0) */
     int force_kernel;        /* NB_FORCE_AUTO (default), NB_FORCE_TILES, NB_FORCE_SYMMETRIC (see below) */
-    int sym_block;           /* tuning: super-block size S of the symmetric kernel (256, 512, 1024, 2048), 0 = auto */
+    int sym_block;           /* tuning: super-block size S of the symmetric kernel (128, 256, 512, 1024, 2048), 0 = auto */
     int resolve_encounters;  /* nb_step: 1 = the members of the encounter groups of each step's pair list are
                                 propagated through A(dt) by the direct solver (nb_encounter) instead of the Kepler
                                 drift; needs pairs != NULL (default 0: pure Kepler drift) */

@@ -4,10 +4,12 @@
 // interaction, against 15 in the one-sided tile kernel (force_tiles.cuh), which stays the kernel of
 // the semi-active mode and of small N.
 //
-// Work unit: a super-tile (A, B), A <= B, of S x S bodies; one CTA of 4 warps per super-tile.
+// Work unit: a super-tile (A, B), A <= B, of S x S bodies; one CTA of W warps per super-tile (W = 4 for S >= 512,
+// 2 for S = 256, 1 for S = 128 at I = 4: always 12 warps per SM; the small tiles are what keeps the tail of a
+// mid-sized problem short -- a lone CTA runs hardly faster than one of many).
 //   * B's bodies (x, y | z, Gm | threshold word; doubled-block layout, see SymParams) are staged
 //     ONCE in shared memory by three TMA bulk copies; B's accelerations accumulate in shared memory (jS).
-//   * A's bodies are taken in chunks of 128*I; every lane holds I of them in registers together
+//   * A's bodies are taken in chunks of 32*W*I; every lane holds I of them in registers together
 //     with their accumulators.
 //   * A warp meets a block of 32 j-bodies by ROTATION: lane l starts with j = l, evaluates its I
 //     pairs, then the three j-accumulators move one lane down (6 SHFL) while the next j's constants
@@ -53,11 +55,8 @@ struct SymParams {
     int kind;   // changeover shape
 };
 
-constexpr int kSymThreads = 128;
-#ifndef NB_SYM_UNROLL
-#define NB_SYM_UNROLL 4
-#endif
-constexpr int kSymUnroll = NB_SYM_UNROLL;  // rotations unrolled in the hot loop
+// rotations unrolled in the hot loop: 4 with the encounter test, 2 without (measured)
+constexpr int kSymUnrollTest = 4, kSymUnrollFar = 2;
 __host__ __device__ constexpr size_t sym_smem_bytes(int S) { return (size_t)S * (32 + 32 + 24 + 8) + 16; }
 
 // Exact evaluation of the lane's I pairs against body j (deferred pass; entered by the lanes that
@@ -133,7 +132,7 @@ __device__ __forceinline__ void sym_block(const SymParams &p, const double2 *__r
     const double2 *__restrict__ lxy = qxy + lane;
     const double2 *__restrict__ lzg = qzg + lane;
     const int *__restrict__ lthr = qthr + lane;
-#pragma unroll kSymUnroll
+#pragma unroll(TEST ? kSymUnrollTest : kSymUnrollFar)
     for (int r = 0; r < 32; ++r) {
         const double2 xy = lxy[r];
         const double2 zg = lzg[r];
@@ -163,34 +162,25 @@ __device__ __forceinline__ void sym_block(const SymParams &p, const double2 *__r
             const double e = __fma_rn(-r2[k], u, 1.0);                   // 1 - r2 y0^2
             const double q = __fma_rn(e, __fma_rn(e, 1.875, 1.5), 1.0);  // (1-e)^(-3/2), next term < 2^-56
             const double b = __dmul_rn(__dmul_rn(u, y0), q);             // r^-3
-#if defined(NB_SYM_CFORM)
-            // variant: c = r^-3 (dx,dy,dz) first; the i side then shares the multiplier G m_j across all 12 FMAs of a rotation
-            const double cx = __dmul_rn(b, dx[k]), cy = __dmul_rn(b, dy[k]), cz = __dmul_rn(b, dz[k]);
-            ax[k] = __fma_rn(zg.y, cx, ax[k]);
-            ay[k] = __fma_rn(zg.y, cy, ay[k]);
-            az[k] = __fma_rn(zg.y, cz, az[k]);
-            bx = __fma_rn(ngi[k], cx, bx);
-            by = __fma_rn(ngi[k], cy, by);
-            bz = __fma_rn(ngi[k], cz, bz);
-#elif defined(NB_SYM_SIDES)
-            const double si = __dmul_rn(b, zg.y);
-            const double sj = __dmul_rn(b, ngi[k]);
-            ax[k] = __fma_rn(si, dx[k], ax[k]);
-            ay[k] = __fma_rn(si, dy[k], ay[k]);
-            az[k] = __fma_rn(si, dz[k], az[k]);
-            bx = __fma_rn(sj, dx[k], bx);
-            by = __fma_rn(sj, dy[k], by);
-            bz = __fma_rn(sj, dz[k], bz);
-#else
             const double si = __dmul_rn(b, zg.y);                        // G m_j / r^3
             const double sj = __dmul_rn(b, ngi[k]);                      // -G m_i / r^3
-            ax[k] = __fma_rn(si, dx[k], ax[k]);
-            bx = __fma_rn(sj, dx[k], bx);
-            by = __fma_rn(sj, dy[k], by);
-            ay[k] = __fma_rn(si, dy[k], ay[k]);
-            az[k] = __fma_rn(si, dz[k], az[k]);
-            bz = __fma_rn(sj, dz[k], bz);
-#endif
+            if (TEST) {
+                // neighbours share one operand (dx, sj, dy, si, dz): measured fastest in the loop with the test
+                ax[k] = __fma_rn(si, dx[k], ax[k]);
+                bx = __fma_rn(sj, dx[k], bx);
+                by = __fma_rn(sj, dy[k], by);
+                ay[k] = __fma_rn(si, dy[k], ay[k]);
+                az[k] = __fma_rn(si, dz[k], az[k]);
+                bz = __fma_rn(sj, dz[k], bz);
+            } else {
+                // side by side: -1.3 % in the test-free loop
+                ax[k] = __fma_rn(si, dx[k], ax[k]);
+                ay[k] = __fma_rn(si, dy[k], ay[k]);
+                az[k] = __fma_rn(si, dz[k], az[k]);
+                bx = __fma_rn(sj, dx[k], bx);
+                by = __fma_rn(sj, dy[k], by);
+                bz = __fma_rn(sj, dz[k], bz);
+            }
         }
         bx = __shfl_sync(0xffffffffu, bx, down);
         by = __shfl_sync(0xffffffffu, by, down);
@@ -225,15 +215,16 @@ __device__ __forceinline__ void sym_block(const SymParams &p, const double2 *__r
 
 
 // The work of one super-tile after B is staged: chunks of A against the blocks of B, then the slot writes.
-template <int I, bool PAIRS, bool TEST, bool SORTED>
+template <int I, int W, bool PAIRS, bool TEST, bool SORTED>
 __device__ __forceinline__ void sym_tile(const SymParams &p, const int A, const int B, const bool diag, const int S,
                                          const double2 *bxy, const double2 *bzg, const int *bthr, double *jsx, double *jsy,
                                          double *jsz) {
     const int t = threadIdx.x, lane = t & 31, w = t >> 5;
     const int nunits = S / (32 * p.U);
-    const int nchunks = S / (kSymThreads * I);
+    constexpr int kThreads = 32 * W;
+    const int nchunks = S / (kThreads * I);
     for (int c = 0; c < nchunks; ++c) {
-        const int P = (c * 4 + w) * I;                  // first 32-block of this warp's i-block within A
+        const int P = (c * W + w) * I;                  // first 32-block of this warp's i-block within A
         const int i0 = A * S + P * 32 + lane;           // global index of the lane's first i-body
         double xi[I], yi[I], zi[I], ngi[I], ax[I], ay[I], az[I];
         int thr_lane = 0;
@@ -289,7 +280,7 @@ __device__ __forceinline__ void sym_tile(const SymParams &p, const int A, const 
     }
     // j side (and, on the diagonal, both sides) -> slot A for B's bodies
     double *out = p.part + (size_t)A * p.N * 3;
-    for (int n = t; n < S; n += kSymThreads) {
+    for (int n = t; n < S; n += kThreads) {
         const long long g = (long long)B * S + n;
         if (g < p.N) {
             out[3 * g] = jsx[n];
@@ -299,8 +290,9 @@ __device__ __forceinline__ void sym_tile(const SymParams &p, const int A, const 
     }
 }
 
-template <int I, bool PAIRS, int MINB, bool SORTED>
-__global__ void __launch_bounds__(kSymThreads, MINB) nb_force_sym_kernel(const SymParams p) {
+template <int I, int W, bool PAIRS, int MINB, bool SORTED>
+__global__ void __launch_bounds__(32 * W, MINB) nb_force_sym_kernel(const SymParams p) {
+    constexpr int kThreads = 32 * W;
     extern __shared__ __align__(16) unsigned char sym_smem[];
     const int S = p.S;
     double2 *bxy = reinterpret_cast<double2 *>(sym_smem);
@@ -311,14 +303,15 @@ __global__ void __launch_bounds__(kSymThreads, MINB) nb_force_sym_kernel(const S
     int *bthr = reinterpret_cast<int *>(jsz + S);
     uint64_t *bar = reinterpret_cast<uint64_t *>(bthr + 2 * S);  // S*96 bytes in: 8-byte aligned
 
-    const int t = threadIdx.x, lane = t & 31, w = t >> 5;
+    const int t = threadIdx.x;
 
-    // super-tile of this CTA: strict pairs A < B first (all of equal cost), diagonal tiles (about half
-    // the work each) last, where they fill the tail wave
+    // super-tile of this CTA: the diagonal tiles (about half the work each) first, then the strict pairs A < B
     const int T = p.nsb;
     const long long nstrict = (long long)T * (T - 1) / 2;
-    const long long idx = blockIdx.x;
     int A, B;
+    // (measured: half-cost tiles at the START take the CTAs of an SM out of lock step, -1.9 % at N = 65536; at the end
+    // they do not shorten the tail, because a lone CTA runs hardly faster than one of three)
+    const long long idx = (long long)blockIdx.x < T ? nstrict + blockIdx.x : (long long)blockIdx.x - T;
     if (idx < nstrict) {
         B = (int)((1.0 + sqrt(1.0 + 8.0 * (double)idx)) * 0.5);
         while ((long long)B * (B - 1) / 2 > idx) --B;
@@ -339,7 +332,7 @@ __global__ void __launch_bounds__(kSymThreads, MINB) nb_force_sym_kernel(const S
         tma_bulk_g2s(bzg, p.szg + (size_t)B * S * 2, b16, bar);
         tma_bulk_g2s(bthr, p.sthr + (size_t)B * S * 2, b4, bar);
     }
-    for (int n = t; n < S; n += kSymThreads) { jsx[n] = 0.0; jsy[n] = 0.0; jsz[n] = 0.0; }
+    for (int n = t; n < S; n += kThreads) { jsx[n] = 0.0; jsy[n] = 0.0; jsz[n] = 0.0; }
     __syncthreads();  // barrier initialised and accumulators zeroed before anyone proceeds
     mbar_wait(bar, 0);
 
@@ -350,8 +343,8 @@ __global__ void __launch_bounds__(kSymThreads, MINB) nb_force_sym_kernel(const S
         const BlockBound ba = p.bnd[A], bb = p.bnd[B];
         far = arcs_are_far(ba.phi_lo, ba.phi_hi, ba.r_min, ba.rc_max, bb.phi_lo, bb.phi_hi, bb.r_min, bb.rc_max);
     }
-    if (SORTED && far) sym_tile<I, PAIRS, false, SORTED>(p, A, B, diag, S, bxy, bzg, bthr, jsx, jsy, jsz);
-    else sym_tile<I, PAIRS, true, SORTED>(p, A, B, diag, S, bxy, bzg, bthr, jsx, jsy, jsz);
+    if (SORTED && far) sym_tile<I, W, PAIRS, false, SORTED>(p, A, B, diag, S, bxy, bzg, bthr, jsx, jsy, jsz);
+    else sym_tile<I, W, PAIRS, true, SORTED>(p, A, B, diag, S, bxy, bzg, bthr, jsx, jsy, jsz);
 }
 
 }  // namespace nbk

@@ -99,6 +99,7 @@ struct Geometry {
     int minb;             // register cap: CTAs per SM the kernel variant is compiled for (3..6)
     int sym;              // 1: Newton-III super-tile kernel (force_sym.cuh); nsplit = number of super-blocks
     int S, U, Npad_sym;   // super-block size, 32-blocks per skew unit, N padded to a multiple of S
+    int warps;            // symmetric kernel: warps per CTA (1, 2 or 4)
     int sorted;           // symmetric kernel: bodies staged in azimuthal order (sort_staging.cuh)
     int mixed;            // mixed-precision one-sided kernel (force_mixed.cuh)
 };
@@ -109,32 +110,38 @@ Geometry geometry(int64_t N, int64_t n_active) {
     g.tiles_total = (g.Nj + kTileJ - 1) / kTileJ;
     g.Njpad = g.tiles_total * kTileJ;
     const int sms = sm_count();
-    g.sym = 0; g.S = 0; g.U = 0; g.Npad_sym = 0; g.sorted = 0;
+    g.sym = 0; g.S = 0; g.U = 0; g.Npad_sym = 0; g.sorted = 0; g.warps = 4;
     g.mixed = g_cfg.precision == NB_PRECISION_MIXED ? 1 : 0;
     // Newton-III kernel: fully active case only (a passive body exerts nothing, so there is no second
     // side to serve), and only when there are enough super-tiles to fill the machine several times.
     const bool fully_active = (g.Nj == N);
     if (fully_active && !g.mixed && g_cfg.force_kernel != NB_FORCE_TILES && (g_cfg.force_kernel == NB_FORCE_SYMMETRIC || N >= 12288)) {
-        // I = 4 at 3 CTAs/SM (168 registers, no spills) measured fastest on B200 (profiles/); smaller
-        // problems take I = 2 so that S = 256 super-blocks (more CTAs) stay possible.
+        // I = 4 at 12 warps per SM (160 registers, no spills) measured fastest on B200.
+        // The CTA shrinks with the super-block -- 4 warps for S >= 512, 2 for S = 256, 1 for S = 128 -- so that a
+        // mid-sized problem still has many short CTAs: the tail of the grid costs about one CTA duration, whatever
+        // the number of CTAs left (a lone CTA runs hardly faster than one of twelve warps' worth).
         int ipt = g_cfg.i_per_thread;
-        if (ipt != 1 && ipt != 2 && ipt != 4) ipt = N >= 32768 ? 4 : 2;
-        const int minb = ipt == 4 ? 3 : 4;
+        if (ipt != 1 && ipt != 2 && ipt != 4) ipt = 4;
         int S = g_cfg.sym_block;
-        if (S != 256 && S != 512 && S != 1024 && S != 2048) {
-            // S = 512 runs 3 CTAs/SM at I = 4 (48 KB of shared memory each) and measured fastest; smaller when
-            // that would leave fewer than 8 waves of CTAs; larger only to keep the N/S partial slots
-            // (24 N^2 / S bytes of workspace) under 16 GiB
-            S = 512;
-            while (S > 256 && S > 128 * ipt) {
-                const int64_t T = (N + S - 1) / S;
-                if (T * (T + 1) / 2 >= (int64_t)8 * minb * sms) break;
-                S >>= 1;
-            }
+        if (S != 128 && S != 256 && S != 512 && S != 1024 && S != 2048) {
+            // largest block whose grid still has enough waves of CTAs (measured crossovers: N ~ 24000 and ~ 60000);
+            // larger than 512 only to keep the N/S partial slots (24 N^2 / S bytes of workspace) under 16 GiB
+            auto waves = [&](int s) {
+                const int64_t T = (N + s - 1) / s;
+                return (double)(T * (T + 1) / 2) / (double)((int64_t)sms * (1536 / s));
+            };
+            S = ipt == 4 ? (waves(512) >= 16.0 ? 512 : (waves(256) >= 5.0 ? 256 : 128)) : (waves(512) >= 16.0 ? 512 : 256);
             while (S < 2048 && ((N + S - 1) / S) * N * 24 > ((int64_t)16 << 30)) S <<= 1;
         }
-        if (S < 128 * ipt) S = 128 * ipt;
-        g.sym = 1; g.S = S; g.U = S / 128; g.ipt = ipt; g.minb = minb;
+        if (ipt == 1 && S < 128) S = 128;
+        // warps per CTA: chunks of 32 W I bodies must tile the super-block
+        int W = S / (32 * ipt);
+        if (W > 4) W = 4;
+        if (ipt == 1) W = 4;
+        if (ipt == 2 && W == 1) W = 2;
+        if (S < 32 * ipt * W) S = 32 * ipt * W;
+        const int minb = ipt == 4 ? 12 / W : (W == 4 ? 4 : 8);
+        g.sym = 1; g.S = S; g.U = S / 128; g.ipt = ipt; g.minb = minb; g.warps = W;
         g.Npad_sym = (int)(((N + S - 1) / S) * S);
         g.nsplit = g.Npad_sym / S;
         g.iblocks = g.nsplit; g.tiles_per_split = 0;
@@ -342,28 +349,31 @@ void launch_force(const ForceParams &fp, const Geometry &g, bool pairs) {
     else launch_force_IM<1, 5>(fp, g, pairs);
 }
 
-template <int I, int MINB, bool SORTED>
+template <int I, int W, int MINB, bool SORTED>
 int launch_sym_IMS(const SymParams &sp, const Geometry &g, bool pairs) {
     const size_t smem = sym_smem_bytes(g.S);
     const long long T = g.nsplit;
     const unsigned ctas = (unsigned)(T * (T + 1) / 2);
     auto go = [&](auto kern) -> int {
         NB_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        kern<<<ctas, kSymThreads, smem, stream()>>>(sp);
+        kern<<<ctas, 32 * W, smem, stream()>>>(sp);
         return NB_OK;
     };
-    return pairs ? go(nb_force_sym_kernel<I, true, MINB, SORTED>) : go(nb_force_sym_kernel<I, false, MINB, SORTED>);
+    return pairs ? go(nb_force_sym_kernel<I, W, true, MINB, SORTED>) : go(nb_force_sym_kernel<I, W, false, MINB, SORTED>);
 }
 
-template <int I, int MINB>
+template <int I, int W, int MINB>
 int launch_sym_IM(const SymParams &sp, const Geometry &g, bool pairs) {
-    return g.sorted ? launch_sym_IMS<I, MINB, true>(sp, g, pairs) : launch_sym_IMS<I, MINB, false>(sp, g, pairs);
+    return g.sorted ? launch_sym_IMS<I, W, MINB, true>(sp, g, pairs) : launch_sym_IMS<I, W, MINB, false>(sp, g, pairs);
 }
 
 int launch_sym(const SymParams &sp, const Geometry &g, bool pairs) {
-    if (g.ipt == 4) return launch_sym_IM<4, 3>(sp, g, pairs);
-    if (g.ipt == 2) return launch_sym_IM<2, 4>(sp, g, pairs);
-    return launch_sym_IM<1, 4>(sp, g, pairs);
+    if (g.ipt == 4 && g.warps == 4) return launch_sym_IM<4, 4, 3>(sp, g, pairs);
+    if (g.ipt == 4 && g.warps == 2) return launch_sym_IM<4, 2, 6>(sp, g, pairs);
+    if (g.ipt == 4) return launch_sym_IM<4, 1, 12>(sp, g, pairs);
+    if (g.ipt == 2 && g.warps == 4) return launch_sym_IM<2, 4, 4>(sp, g, pairs);
+    if (g.ipt == 2) return launch_sym_IM<2, 2, 8>(sp, g, pairs);
+    return launch_sym_IM<1, 4, 4>(sp, g, pairs);
 }
 
 // One force evaluation: [second half-shift] + rcrit + staging, tiles, reduce + kick.
@@ -736,7 +746,7 @@ int step_impl(double *x, double *v, const double *m, double M_star, int64_t N, d
         key.x = x; key.v = v; key.m = m; key.rcrit = rc_io; key.acc = acc; key.pairs = pairs; key.npairs = npairs;
         key.ws = g_cfg.workspace; key.stream = g_cfg.stream; key.N = N; key.n_active = g_cfg.n_active;
         key.cap = g_cfg.pair_capacity; key.dt = dt; key.M_star = M_star; key.G = g_cfg.G; key.n1 = g_cfg.n1;
-        key.n2 = g_cfg.n2; key.kind = g_cfg.changeover_kind; key.bs_tol = g_cfg.bs_tol; key.enc = (enc ? 1 : 0) + 2 * g.sorted; key.ipt = g.S * 1000 + g.ipt * 100 + g.minb * 10; key.jsplit = g.nsplit;
+        key.n2 = g_cfg.n2; key.kind = g_cfg.changeover_kind; key.bs_tol = g_cfg.bs_tol; key.enc = (enc ? 1 : 0) + 2 * g.sorted; key.ipt = g.S * 1000 + g.ipt * 100 + g.minb * 10 + g.warps; key.jsplit = g.nsplit;
         key.ws_bytes = g_cfg.workspace_bytes; key.levels = g_cfg.levels;
         key.drag_gamma = g_cfg.drag_gamma; key.drag_eta = g_cfg.drag_eta; key.midpoint_tol = g_cfg.midpoint_tol;
         key.drag_power = g_cfg.drag_power; key.midpoint_iters = g_cfg.midpoint_iters + 1000 * g.mixed;
@@ -842,8 +852,8 @@ int nb_configure(const nb_config *cfg) {
     if (cfg->j_splits < 0) return fail(NB_E_BADARG, "j_splits must be >= 0");
     if (cfg->force_kernel != NB_FORCE_AUTO && cfg->force_kernel != NB_FORCE_TILES && cfg->force_kernel != NB_FORCE_SYMMETRIC)
         return fail(NB_E_BADARG, "unknown force_kernel %d", cfg->force_kernel);
-    if (cfg->sym_block != 0 && cfg->sym_block != 256 && cfg->sym_block != 512 && cfg->sym_block != 1024 && cfg->sym_block != 2048)
-        return fail(NB_E_BADARG, "sym_block must be 0, 256, 512, 1024 or 2048");
+    if (cfg->sym_block != 0 && cfg->sym_block != 128 && cfg->sym_block != 256 && cfg->sym_block != 512 && cfg->sym_block != 1024 && cfg->sym_block != 2048)
+        return fail(NB_E_BADARG, "sym_block must be 0, 128, 256, 512, 1024 or 2048");
     if (!(cfg->bs_tol >= 0.0) || !std::isfinite(cfg->bs_tol)) return fail(NB_E_BADARG, "bs_tol must be finite and >= 0");
     if (cfg->sort_staging != NB_SORT_AUTO && cfg->sort_staging != NB_SORT_ON && cfg->sort_staging != NB_SORT_OFF)
         return fail(NB_E_BADARG, "unknown sort_staging %d", cfg->sort_staging);
@@ -869,7 +879,7 @@ int nb_force_geometry(int64_t N, int64_t *out5) {
     if (!out5) return fail(NB_E_NULL, "out5 is NULL");
     if (N <= 0 || N > 2147483647LL) return fail(NB_E_BADN, "N out of range");
     const Geometry g = geometry(N, g_cfg.n_active <= N ? g_cfg.n_active : 0);
-    out5[0] = g.ipt; out5[1] = g.iblocks; out5[2] = g.nsplit; out5[3] = kForceThreads; out5[4] = g.sym ? -g.S : kTileJ;
+    out5[0] = g.ipt; out5[1] = g.iblocks; out5[2] = g.nsplit; out5[3] = g.sym ? 32 * g.warps : kForceThreads; out5[4] = g.sym ? -g.S : kTileJ;
     return NB_OK;
 }
 

@@ -93,7 +93,7 @@ def test_geometry_and_workspace(nb):
         c.n_active = n_active
         assert lib.nb_configure(C.byref(c)) == 0
         g = nb.force_geometry(N)
-        assert g.threads == 128 and g.i_per_thread in (1, 2, 4)
+        assert g.threads in (32, 64, 128) and g.i_per_thread in (1, 2, 4)
         nj = n_active or N
         ws = nb.workspace_bytes(N)
         if g.tile_j < 0:
@@ -101,12 +101,16 @@ def test_geometry_and_workspace(nb):
             # per unordered pair of super-blocks, one partial slot per super-block
             S = -g.tile_j
             assert not n_active and N >= 12288
-            assert S in (256, 512, 1024, 2048) and S % (128 * g.i_per_thread) == 0
+            # CTAs of W warps whose chunks of 32 W I bodies tile the super-block; always 12 warps per SM at I = 4
+            assert S in (128, 256, 512, 1024, 2048) and S % (g.threads * g.i_per_thread) == 0
+            assert g.threads == min(128, S // g.i_per_thread) or g.i_per_thread != 4
             assert g.i_blocks == g.j_splits == -(-N // S)
-            assert g.i_blocks * (g.i_blocks + 1) // 2 >= 8 * 148 or S == max(256, 128 * g.i_per_thread)
+            # enough waves of CTAs (16 at S = 512, 5 at S = 256), else the smallest block
+            slots = 148 * (1536 // min(S, 512))
+            assert g.i_blocks * (g.i_blocks + 1) // 2 >= (16 if S >= 512 else 5) * slots or S == 128
             assert ws >= 36 * N + 24 * N * g.j_splits
         else:
-            assert g.tile_j == 128
+            assert g.tile_j == 128 and g.threads == 128
             assert g.i_blocks * g.threads * g.i_per_thread >= N > (g.i_blocks - 1) * g.threads * g.i_per_thread
             tiles = -(-nj // g.tile_j)
             per = -(-tiles // g.j_splits)

@@ -23,7 +23,7 @@ def _geometry_is_symmetric(N):
     return nb.force_geometry(N).tile_j < 0
 
 
-@pytest.mark.parametrize("ipt,S", [(1, 256), (2, 256), (2, 512), (4, 512), (4, 1024)])
+@pytest.mark.parametrize("ipt,S", [(1, 256), (2, 256), (2, 512), (4, 512), (4, 1024), (4, 128), (4, 256), (2, 128), (1, 128)])
 @pytest.mark.parametrize("N", [1, 2, 31, 32, 33, 255, 256, 257, 700, 1100])
 def test_sym_random_cluster_newtonian(N, ipt, S):
     x, v, m = nb_inputs.random_cluster(N, seed=100 + N)
@@ -34,7 +34,7 @@ def test_sym_random_cluster_newtonian(N, ipt, S):
 
 
 @pytest.mark.parametrize("kind", [0, 1])
-@pytest.mark.parametrize("ipt,S", [(1, 256), (2, 256), (4, 512)])
+@pytest.mark.parametrize("ipt,S", [(1, 256), (2, 256), (4, 512), (4, 128), (4, 256), (2, 128)])
 def test_sym_cluster_with_changeover_and_pairs(kind, ipt, S):
     N = 1000
     x, v, m = nb_inputs.random_cluster(N, seed=5, scale=0.2)
@@ -46,7 +46,7 @@ def test_sym_cluster_with_changeover_and_pairs(kind, ipt, S):
     assert info["n_sure"] > 300
 
 
-@pytest.mark.parametrize("ipt,S", [(2, 256), (4, 512)])
+@pytest.mark.parametrize("ipt,S", [(2, 256), (4, 512), (4, 128), (4, 256)])
 def test_sym_chain_lattice_and_all_pairs(ipt, S):
     tune = dict(force_kernel=SYM, i_per_thread=ipt, sym_block=S)
     N = 300
@@ -65,7 +65,7 @@ def test_sym_chain_lattice_and_all_pairs(ipt, S):
     assert info["n_gpu"] == N * (N - 1) // 2
 
 
-@pytest.mark.parametrize("ipt,S", [(1, 256), (4, 512)])
+@pytest.mark.parametrize("ipt,S", [(1, 256), (4, 512), (4, 128), (4, 256)])
 def test_sym_coincident_bodies(ipt, S):
     tune = dict(force_kernel=SYM, i_per_thread=ipt, sym_block=S)
     x, v, m = nb_inputs.random_cluster(300, seed=3)
@@ -206,7 +206,7 @@ def test_sym_randomized_shapes_against_oracle(seed):
 SORT = dict(force_kernel=SYM, sort_staging=1)
 
 
-@pytest.mark.parametrize("ipt,S", [(1, 256), (2, 256), (4, 512)])
+@pytest.mark.parametrize("ipt,S", [(1, 256), (2, 256), (4, 512), (4, 128), (4, 256)])
 @pytest.mark.parametrize("N", [1, 2, 33, 257, 700, 1100])
 def test_sorted_staging_cluster_with_changeover_and_pairs(N, ipt, S):
     x, v, m = nb_inputs.random_cluster(N, seed=300 + N, scale=0.2)
