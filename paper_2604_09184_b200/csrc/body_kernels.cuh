@@ -123,11 +123,14 @@ __global__ void __launch_bounds__(kBodyThreads) nb_rcrit_kernel(const double *__
 // separate roundings, as in the step definition).  Optionally emits momentum partials of the new v.
 // perm != nullptr: the partial sums are indexed by staged position (sort_staging.cuh); thread t then serves
 // position t (coalesced slot reads) and writes the body perm[t] (the real bodies hold positions 0 .. N-1).
+// xcols > 0 (Newton-III kernel with tail splitting, force_sym.cuh kSymSplit): column nsplit-1-c of the tile grid was cut
+// into parts whose i sides sit in 3 extra slots, nsplit + 3 c + {0, 1, 2}, valid for the positions in front of that
+// column, t < (nsplit-1-c) S; they are added after the regular slots, in order.
 // the work of thread slot t (of N): returns the momentum contribution of the kicked body
 __device__ __forceinline__ void kickv_one(const double *part, const int nsplit, double *acc, double *__restrict__ v,
                                           const double *__restrict__ m, const int N, const double hk, const int nhalf,
                                           const bool want_mv, const int *__restrict__ perm, const int t, double &px, double &py,
-                                          double &pz) {
+                                          double &pz, const int xcols = 0, const int S = 0) {
     px = 0.0; py = 0.0; pz = 0.0;
     const int i = (perm != nullptr && t < N) ? perm[t] : t;
     if (t < N && i < N) {
@@ -135,6 +138,13 @@ __device__ __forceinline__ void kickv_one(const double *part, const int nsplit, 
         for (int s = 0; s < nsplit; ++s) {
             const double *q = part + ((size_t)s * N + t) * 3;
             ax += q[0]; ay += q[1]; az += q[2];
+        }
+        for (int c = 0; c < xcols; ++c) {
+            if (t >= (nsplit - 1 - c) * S) continue;
+            for (int e = 0; e < 3; ++e) {
+                const double *q = part + ((size_t)(nsplit + 3 * c + e) * N + t) * 3;
+                ax += q[0]; ay += q[1]; az += q[2];
+            }
         }
         acc[3 * (size_t)i] = ax; acc[3 * (size_t)i + 1] = ay; acc[3 * (size_t)i + 2] = az;
         double vx = v[3 * (size_t)i], vy = v[3 * (size_t)i + 1], vz = v[3 * (size_t)i + 2];
@@ -150,10 +160,10 @@ __global__ void __launch_bounds__(kBodyThreads) nb_kickv_kernel(const double *pa
                                                                double *acc, double *__restrict__ v,
                                                                const double *__restrict__ m, int N, double hk,
                                                                int nhalf, double *__restrict__ mv_out,
-                                                               const int *__restrict__ perm) {
+                                                               const int *__restrict__ perm, int xcols, int S) {
     __shared__ double sm[3 * kBodyThreads];
     double px, py, pz;
-    kickv_one(part, nsplit, acc, v, m, N, hk, nhalf, mv_out != nullptr, perm, blockIdx.x * kBodyThreads + threadIdx.x, px, py, pz);
+    kickv_one(part, nsplit, acc, v, m, N, hk, nhalf, mv_out != nullptr, perm, blockIdx.x * kBodyThreads + threadIdx.x, px, py, pz, xcols, S);
     if (mv_out != nullptr) {
         block_sum3(px, py, pz, sm);
         if (threadIdx.x == 0) {

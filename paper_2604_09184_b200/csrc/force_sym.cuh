@@ -52,11 +52,24 @@ struct SymParams {
     int S;      // super-block size: multiple of 128*I and of 128*U
     int nsb;    // super-blocks = Npad / S
     int U;      // 32-blocks per skew unit (S / (32 U) >= 4)
+    int xcols;  // TAIL SPLITTING: the strict tiles of the last xcols columns B run as kSymSplit CTAs each, one per
+                // part of B's bodies; part q > 0 of column T-1-c writes its i side to the extra slot nsb + c (kSymSplit-1) + q-1
     int kind;   // changeover shape
 };
 
 // rotations unrolled in the hot loop: 4 with the encounter test, 2 without (measured)
 constexpr int kSymUnrollTest = 4, kSymUnrollFar = 2;
+// Tail of the grid: a lone CTA runs hardly faster than one of many, so the end of the launch costs about one CTA
+// duration whatever the number of CTAs left.  The tiles launched last are therefore cut into kSymSplit parts along B
+// (S / kSymSplit j-bodies each, all of A): short CTAs, and many of them.  The j side of a part goes to slot A as usual
+// (its bodies are its own); the i sides of the parts are kSymSplit partial sums for A's bodies: part 0 takes slot B, the
+// others one extra slot each per split column (valid for the bodies in front of that column; nb_kickv_kernel knows).
+constexpr int kSymSplit = 4;
+__host__ __device__ constexpr long long sym_split_tiles(long long T, long long C) { return C * (T - 1) - C * (C - 1) / 2; }
+__host__ __device__ constexpr long long sym_grid(long long T, long long C) {
+    return T * (T + 1) / 2 + (kSymSplit - 1) * sym_split_tiles(T, C);
+}
+__host__ __device__ constexpr int sym_slots(int T, int C) { return T + (kSymSplit - 1) * C; }
 __host__ __device__ constexpr size_t sym_smem_bytes(int S) { return (size_t)S * (32 + 32 + 24 + 8) + 16; }
 
 // Exact evaluation of the lane's I pairs against body j (deferred pass; entered by the lanes that
@@ -217,10 +230,14 @@ __device__ __forceinline__ void sym_block(const SymParams &p, const double2 *__r
 // The work of one super-tile after B is staged: chunks of A against the blocks of B, then the slot writes.
 template <int I, int W, bool PAIRS, bool TEST, bool SORTED>
 __device__ __forceinline__ void sym_tile(const SymParams &p, const int A, const int B, const bool diag, const int S,
+                                         const volatile int *ti,
                                          const double2 *bxy, const double2 *bzg, const int *bthr, double *jsx, double *jsy,
                                          double *jsz) {
+    // ti (shared memory, re-read where needed so that none of it occupies a register across the rotation loops):
+    // [0] jS, the number of staged j-bodies (all of B unless the tile is split), [1] position of the first of them,
+    // [2] Uq, 32-blocks per skew unit, [3] the slot of the i side
     const int t = threadIdx.x, lane = t & 31, w = t >> 5;
-    const int nunits = S / (32 * p.U);
+    const int nunits = ti[0] / (32 * ti[2]);
     constexpr int kThreads = 32 * W;
     const int nchunks = S / (kThreads * I);
     for (int c = 0; c < nchunks; ++c) {
@@ -240,15 +257,16 @@ __device__ __forceinline__ void sym_tile(const SymParams &p, const int A, const 
         for (int step = 0; step < nunits; ++step) {
             int unit = step + w;
             if (unit >= nunits) unit -= nunits;
-            for (int uu = 0; uu < p.U; ++uu) {
-                const int q = unit * p.U + uu;  // 32-block of B
+            const int Uq = ti[2];
+            for (int uu = 0; uu < Uq; ++uu) {
+                const int q = unit * Uq + uu;  // 32-block of the staged part of B
                 bool mixed = false;
                 if (diag) {
                     if (q < P) continue;          // the mirrored visit covers it
                     mixed = q < P + I;
                 }
                 double bx, by, bz;
-                sym_block<I, PAIRS, TEST, SORTED>(p, bxy + q * 64, bzg + q * 64, bthr + q * 64, B * S + q * 32, mixed, xi, yi, zi,
+                sym_block<I, PAIRS, TEST, SORTED>(p, bxy + q * 64, bzg + q * 64, bthr + q * 64, ti[1] + q * 32, mixed, xi, yi, zi,
                                     ngi, thr_lane, i0, ax, ay, az, bx, by, bz);
                 if (!mixed) {
                     const int n = q * 32 + lane;
@@ -266,7 +284,7 @@ __device__ __forceinline__ void sym_tile(const SymParams &p, const int A, const 
             }
             __syncthreads();
         } else {
-            double *out = p.part + (size_t)B * p.N * 3;
+            double *out = p.part + (size_t)ti[3] * p.N * 3;
 #pragma unroll
             for (int k = 0; k < I; ++k) {
                 const int i = i0 + 32 * k;
@@ -280,8 +298,9 @@ __device__ __forceinline__ void sym_tile(const SymParams &p, const int A, const 
     }
     // j side (and, on the diagonal, both sides) -> slot A for B's bodies
     double *out = p.part + (size_t)A * p.N * 3;
-    for (int n = t; n < S; n += kThreads) {
-        const long long g = (long long)B * S + n;
+    const int jS = ti[0], j0 = ti[1];
+    for (int n = t; n < jS; n += kThreads) {
+        const long long g = (long long)j0 + n;
         if (g < p.N) {
             out[3 * g] = jsx[n];
             out[3 * g + 1] = jsy[n];
@@ -305,20 +324,35 @@ __global__ void __launch_bounds__(32 * W, MINB) nb_force_sym_kernel(const SymPar
 
     const int t = threadIdx.x;
 
-    // super-tile of this CTA: the diagonal tiles (about half the work each) first, then the strict pairs A < B
+    // super-tile of this CTA: the diagonal tiles (about half the work each) first -- measured: half-cost tiles at the
+    // START take the CTAs of an SM out of lock step, -1.9 % at N = 65536 --, then the strict pairs A < B column by
+    // column, the last xcols columns cut into kSymSplit parts each (see kSymSplit)
     const int T = p.nsb;
     const long long nstrict = (long long)T * (T - 1) / 2;
-    int A, B;
-    // (measured: half-cost tiles at the START take the CTAs of an SM out of lock step, -1.9 % at N = 65536; at the end
-    // they do not shorten the tail, because a lone CTA runs hardly faster than one of three)
-    const long long idx = (long long)blockIdx.x < T ? nstrict + blockIdx.x : (long long)blockIdx.x - T;
-    if (idx < nstrict) {
+    const long long nwhole = nstrict - sym_split_tiles(T, p.xcols);   // strict tiles that run as one CTA
+    int A, B, part = 0, nparts = 1;
+    if ((long long)blockIdx.x < T) {
+        A = B = (int)blockIdx.x;
+    } else {
+        long long idx = (long long)blockIdx.x - T;
+        if (idx >= nwhole) {
+            const long long k = idx - nwhole;
+            idx = nwhole + k / kSymSplit;
+            part = (int)(k % kSymSplit);
+            nparts = kSymSplit;
+        }
         B = (int)((1.0 + sqrt(1.0 + 8.0 * (double)idx)) * 0.5);
         while ((long long)B * (B - 1) / 2 > idx) --B;
         while ((long long)(B + 1) * B / 2 <= idx) ++B;
         A = (int)(idx - (long long)B * (B - 1) / 2);
-    } else {
-        A = B = (int)(idx - nstrict);
+    }
+    const int jS = S / nparts, joff = part * jS;
+    __shared__ int tinfo[4];
+    if (t == 0) {
+        tinfo[0] = jS;
+        tinfo[1] = B * S + joff;
+        tinfo[2] = nparts == 1 ? p.U : (p.U / kSymSplit > 0 ? p.U / kSymSplit : 1);
+        tinfo[3] = part == 0 ? B : T + (T - 1 - B) * (kSymSplit - 1) + part - 1;
     }
     const bool diag = (A == B);
 
@@ -326,13 +360,14 @@ __global__ void __launch_bounds__(32 * W, MINB) nb_force_sym_kernel(const SymPar
         mbar_init(bar, 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
         asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-        const unsigned b16 = (unsigned)S * 32u, b4 = (unsigned)S * 8u;
+        const unsigned b16 = (unsigned)jS * 32u, b4 = (unsigned)jS * 8u;
+        const size_t first = ((size_t)B * S + joff) * 2;   // doubled-block layout
         mbar_expect_tx(bar, 2u * b16 + b4);
-        tma_bulk_g2s(bxy, p.sxy + (size_t)B * S * 2, b16, bar);
-        tma_bulk_g2s(bzg, p.szg + (size_t)B * S * 2, b16, bar);
-        tma_bulk_g2s(bthr, p.sthr + (size_t)B * S * 2, b4, bar);
+        tma_bulk_g2s(bxy, p.sxy + first, b16, bar);
+        tma_bulk_g2s(bzg, p.szg + first, b16, bar);
+        tma_bulk_g2s(bthr, p.sthr + first, b4, bar);
     }
-    for (int n = t; n < S; n += kThreads) { jsx[n] = 0.0; jsy[n] = 0.0; jsz[n] = 0.0; }
+    for (int n = t; n < jS; n += kThreads) { jsx[n] = 0.0; jsy[n] = 0.0; jsz[n] = 0.0; }
     __syncthreads();  // barrier initialised and accumulators zeroed before anyone proceeds
     mbar_wait(bar, 0);
 
@@ -343,8 +378,8 @@ __global__ void __launch_bounds__(32 * W, MINB) nb_force_sym_kernel(const SymPar
         const BlockBound ba = p.bnd[A], bb = p.bnd[B];
         far = arcs_are_far(ba.phi_lo, ba.phi_hi, ba.r_min, ba.rc_max, bb.phi_lo, bb.phi_hi, bb.r_min, bb.rc_max);
     }
-    if (SORTED && far) sym_tile<I, W, PAIRS, false, SORTED>(p, A, B, diag, S, bxy, bzg, bthr, jsx, jsy, jsz);
-    else sym_tile<I, W, PAIRS, true, SORTED>(p, A, B, diag, S, bxy, bzg, bthr, jsx, jsy, jsz);
+    if (SORTED && far) sym_tile<I, W, PAIRS, false, SORTED>(p, A, B, diag, S, tinfo, bxy, bzg, bthr, jsx, jsy, jsz);
+    else sym_tile<I, W, PAIRS, true, SORTED>(p, A, B, diag, S, tinfo, bxy, bzg, bthr, jsx, jsy, jsz);
 }
 
 }  // namespace nbk

@@ -100,6 +100,8 @@ struct Geometry {
     int sym;              // 1: Newton-III super-tile kernel (force_sym.cuh); nsplit = number of super-blocks
     int S, U, Npad_sym;   // super-block size, 32-blocks per skew unit, N padded to a multiple of S
     int warps;            // symmetric kernel: warps per CTA (1, 2 or 4)
+    int xcols;            // symmetric kernel: trailing tile columns cut into kSymSplit CTAs each (force_sym.cuh kSymSplit)
+    int nslots;           // partial-acceleration slots nb_kickv_kernel sums (= nsplit + extra slots of the split columns)
     int sorted;           // symmetric kernel: bodies staged in azimuthal order (sort_staging.cuh)
     int mixed;            // mixed-precision one-sided kernel (force_mixed.cuh)
 };
@@ -110,7 +112,7 @@ Geometry geometry(int64_t N, int64_t n_active) {
     g.tiles_total = (g.Nj + kTileJ - 1) / kTileJ;
     g.Njpad = g.tiles_total * kTileJ;
     const int sms = sm_count();
-    g.sym = 0; g.S = 0; g.U = 0; g.Npad_sym = 0; g.sorted = 0; g.warps = 4;
+    g.sym = 0; g.S = 0; g.U = 0; g.Npad_sym = 0; g.sorted = 0; g.warps = 4; g.xcols = 0; g.nslots = 0;
     g.mixed = g_cfg.precision == NB_PRECISION_MIXED ? 1 : 0;
     // Newton-III kernel: fully active case only (a passive body exerts nothing, so there is no second
     // side to serve), and only when there are enough super-tiles to fill the machine several times.
@@ -145,6 +147,19 @@ Geometry geometry(int64_t N, int64_t n_active) {
         g.Npad_sym = (int)(((N + S - 1) / S) * S);
         g.nsplit = g.Npad_sym / S;
         g.iblocks = g.nsplit; g.tiles_per_split = 0;
+        {   // tail splitting: about one wave's worth of tiles (the ones launched last) run as kSymSplit short CTAs each;
+            // pointless once the grid is hundreds of waves long
+            const int64_t T = g.nsplit, slots = (int64_t)sms * (12 / W);
+            const int jS = S / kSymSplit, Uq = g.U / kSymSplit > 0 ? g.U / kSymSplit : 1;
+            int C = 0;
+            if (ipt == 4 && jS >= 32 && jS / (32 * Uq) >= W && T * (T + 1) / 2 < 100 * slots) {
+                C = (int)((slots + T - 1) / T);
+                if (C > T / 4) C = (int)(T / 4);
+                if (C > 16) C = 16;
+            }
+            g.xcols = C;
+        }
+        g.nslots = sym_slots(g.nsplit, g.xcols);
         // sorted staging pays off once the sort (a few small launches) is small against the evaluation
         g.sorted = g_cfg.sort_staging == NB_SORT_ON || (g_cfg.sort_staging == NB_SORT_AUTO && N >= 32768);
         return g;
@@ -191,6 +206,7 @@ Geometry geometry(int64_t N, int64_t n_active) {
     if (nsplit > 65535) nsplit = 65535;
     g.tiles_per_split = (g.tiles_total + nsplit - 1) / nsplit;
     g.nsplit = (g.tiles_total + g.tiles_per_split - 1) / g.tiles_per_split;
+    g.nslots = g.nsplit;
     return g;
 }
 
@@ -279,7 +295,7 @@ Workspace carve(void *base, int64_t N, const Geometry &g) {
     w.pos_of = reinterpret_cast<int *>(b + off); off += align_up((size_t)(g.sym ? N : 0) * sizeof(int), 256);
     w.bnd = reinterpret_cast<BlockBound *>(b + off); off += align_up((size_t)(g.sym ? g.nsplit : 0) * sizeof(BlockBound), 256);
     {   // partial accelerations; never smaller than 64 bytes per body (nb_merge's compaction buffer)
-        size_t pb = (size_t)g.nsplit * (size_t)N * 3 * sizeof(double);
+        size_t pb = (size_t)g.nslots * (size_t)N * 3 * sizeof(double);
         if (pb < (size_t)N * 64) pb = (size_t)N * 64;
         w.part = reinterpret_cast<double *>(b + off); off += align_up(pb, 256);
     }
@@ -353,7 +369,7 @@ template <int I, int W, int MINB, bool SORTED>
 int launch_sym_IMS(const SymParams &sp, const Geometry &g, bool pairs) {
     const size_t smem = sym_smem_bytes(g.S);
     const long long T = g.nsplit;
-    const unsigned ctas = (unsigned)(T * (T + 1) / 2);
+    const unsigned ctas = (unsigned)sym_grid(T, g.xcols);
     auto go = [&](auto kern) -> int {
         NB_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         kern<<<ctas, 32 * W, smem, stream()>>>(sp);
@@ -440,7 +456,7 @@ int enqueue_eval(const Workspace &w, const Geometry &g, double *x, double *v, co
         sp.perm = sorted ? w.perm : nullptr; sp.bnd = sorted ? w.bnd : nullptr;
         sp.sxy = w.sxy; sp.szg = w.szg; sp.sthr = w.sthr; sp.rcrit = rc_io; sp.part = w.part; sp.pairs = pairs;
         sp.npairs = fp.npairs; sp.status = w.status; sp.cap = fp.cap; sp.N = (int)N; sp.S = g.S; sp.nsb = g.nsplit;
-        sp.U = g.U; sp.kind = g_cfg.changeover_kind;
+        sp.U = g.U; sp.kind = g_cfg.changeover_kind; sp.xcols = g.xcols;
         const int lrc = launch_sym(sp, g, pairs != nullptr);
         if (lrc) return lrc;
     } else {
@@ -450,7 +466,7 @@ int enqueue_eval(const Workspace &w, const Geometry &g, double *x, double *v, co
     else if (time_force) { NB_CUDA(cudaEventRecord(g_ev1, stream())); g_force_timed = true; }
 
     nb_kickv_kernel<<<nblk, kBodyThreads, 0, stream()>>>(w.part, g.nsplit, acc, v, m, (int)N, hk, nhalf, mv_out,
-                                                         sorted ? w.perm : nullptr);
+                                                         sorted ? w.perm : nullptr, g.xcols, g.S);
     NB_CUDA(cudaGetLastError());
     return NB_OK;
 }
@@ -673,7 +689,7 @@ int step_impl(double *x, double *v, const double *m, double M_star, int64_t N, d
                                                                      g_cfg.drag_eta, g_cfg.midpoint_tol, g_cfg.midpoint_iters > 0 ? g_cfg.midpoint_iters : 50, w.status);
     };
     // opening half-kick from the cached force (reads acc as a 1-split partial) + momentum partials
-    auto kick_only = [&]() { nb_kickv_kernel<<<nblk, kBodyThreads, 0, stream()>>>(acc, 1, acc, v, m, (int)N, hk, 1, w.mvA, nullptr); };
+    auto kick_only = [&]() { nb_kickv_kernel<<<nblk, kBodyThreads, 0, stream()>>>(acc, 1, acc, v, m, (int)N, hk, 1, w.mvA, nullptr, 0, 0); };
     if (g_cfg.reuse_acc && nsteps > 0) {
         // acc already is the force at the current x
         if (drag) enqueue_D();
@@ -746,7 +762,7 @@ int step_impl(double *x, double *v, const double *m, double M_star, int64_t N, d
         key.x = x; key.v = v; key.m = m; key.rcrit = rc_io; key.acc = acc; key.pairs = pairs; key.npairs = npairs;
         key.ws = g_cfg.workspace; key.stream = g_cfg.stream; key.N = N; key.n_active = g_cfg.n_active;
         key.cap = g_cfg.pair_capacity; key.dt = dt; key.M_star = M_star; key.G = g_cfg.G; key.n1 = g_cfg.n1;
-        key.n2 = g_cfg.n2; key.kind = g_cfg.changeover_kind; key.bs_tol = g_cfg.bs_tol; key.enc = (enc ? 1 : 0) + 2 * g.sorted; key.ipt = g.S * 1000 + g.ipt * 100 + g.minb * 10 + g.warps; key.jsplit = g.nsplit;
+        key.n2 = g_cfg.n2; key.kind = g_cfg.changeover_kind; key.bs_tol = g_cfg.bs_tol; key.enc = (enc ? 1 : 0) + 2 * g.sorted; key.ipt = g.S * 1000 + g.ipt * 100 + g.minb * 10 + g.warps + 100000 * g.xcols; key.jsplit = g.nsplit;
         key.ws_bytes = g_cfg.workspace_bytes; key.levels = g_cfg.levels;
         key.drag_gamma = g_cfg.drag_gamma; key.drag_eta = g_cfg.drag_eta; key.midpoint_tol = g_cfg.midpoint_tol;
         key.drag_power = g_cfg.drag_power; key.midpoint_iters = g_cfg.midpoint_iters + 1000 * g.mixed;
