@@ -115,6 +115,9 @@ typedef struct nb_config {
     int midpoint_iters;      /* Eq. 8 fixed-point iterations at most (default 50) */
     double midpoint_tol;     /* stop when the update is below tol * max(|v|, |v_gas|) (default 1e-14) */
     int precision;           /* NB_PRECISION_F64 (default) or NB_PRECISION_MIXED (see above) */
+    int64_t slot_bytes_max;  /* tuning (symmetric kernel): cap of the partial-acceleration slots in the workspace; 0 (default) =
+                                4 GiB.  A grid whose slots (24 N^2 / S bytes) would pass it is evaluated in bands of tile
+                                columns, one launch and one fold into acc per band (same results to rounding order) */
 } nb_config;
 
 void nb_default_config(nb_config *cfg);

@@ -57,6 +57,7 @@ class NbConfig(C.Structure):
         ("midpoint_iters", C.c_int),
         ("midpoint_tol", C.c_double),
         ("precision", C.c_int),
+        ("slot_bytes_max", C.c_int64),
     ]
 
 
@@ -167,7 +168,7 @@ def default_config() -> NbConfig:
 def configure(N=None, *, stream=None, pair_capacity=0, n_active=0, G=None, n1=3.0, n2=0.4, changeover_kind=0,
               i_per_thread=0, j_splits=0, use_graph=True, reuse_acc=False, time_force=False,
               force_kernel=0, sym_block=0, resolve_encounters=False, bs_tol=1e-12, radius_factor=1.0, sort_staging=0, levels=0, drag_gamma=0.0, drag_eta=0.0, drag_power=0,
-              midpoint_iters=50, midpoint_tol=1e-14, precision=0, workspace_bytes=None,
+              midpoint_iters=50, midpoint_tol=1e-14, precision=0, slot_bytes_max=0, workspace_bytes=None,
               device="cuda"):
     """nb_configure with a torch-allocated workspace sized for N bodies (N=None: no workspace,
     enough for the _host calls; workspace_bytes: explicit size, e.g. the head that the O(N) calls
@@ -192,6 +193,7 @@ def configure(N=None, *, stream=None, pair_capacity=0, n_active=0, G=None, n1=3.
     cfg.drag_gamma, cfg.drag_eta, cfg.drag_power = float(drag_gamma), float(drag_eta), int(drag_power)
     cfg.midpoint_iters, cfg.midpoint_tol = int(midpoint_iters), float(midpoint_tol)
     cfg.precision = int(precision)
+    cfg.slot_bytes_max = int(slot_bytes_max)
     if N is not None:
         import torch
         if stream is None:

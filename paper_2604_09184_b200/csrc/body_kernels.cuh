@@ -135,7 +135,20 @@ __device__ __forceinline__ void kickv_one(const double *part, const int nsplit, 
     const int i = (perm != nullptr && t < N) ? perm[t] : t;
     if (t < N && i < N) {
         double ax = 0.0, ay = 0.0, az = 0.0;
-        for (int s = 0; s < nsplit; ++s) {
+        // the loads of 8 slots are issued together (the sum is latency-bound otherwise: up to 140 slots at N = 65536);
+        // the additions keep the slot order
+        int s = 0;
+        for (; s + 8 <= nsplit; s += 8) {
+            double b[8][3];
+#pragma unroll
+            for (int u = 0; u < 8; ++u) {
+                const double *q = part + ((size_t)(s + u) * N + t) * 3;
+                b[u][0] = q[0]; b[u][1] = q[1]; b[u][2] = q[2];
+            }
+#pragma unroll
+            for (int u = 0; u < 8; ++u) { ax += b[u][0]; ay += b[u][1]; az += b[u][2]; }
+        }
+        for (; s < nsplit; ++s) {
             const double *q = part + ((size_t)s * N + t) * 3;
             ax += q[0]; ay += q[1]; az += q[2];
         }
@@ -170,6 +183,35 @@ __global__ void __launch_bounds__(kBodyThreads) nb_kickv_kernel(const double *pa
             mv_out[3 * blockIdx.x] = px; mv_out[3 * blockIdx.x + 1] = py; mv_out[3 * blockIdx.x + 2] = pz;
         }
     }
+}
+
+// Banded evaluation of the Newton-III kernel (force_sym.cuh SymParams): folds the partial sums of the band of tile
+// columns col0 .. col0 + ncols - 1 into acc, in a fixed order -- the i sides part_i[b][N] (valid for the positions in
+// front of column col0 + b), then, for the band's own bodies, the j sides part_j[A][ncols S], A = 0 .. own block.
+// first != 0: acc starts from 0.  Thread t serves staged position t and writes body perm[t] (or t).
+__global__ void __launch_bounds__(kBodyThreads) nb_bandsum_kernel(const double *__restrict__ part_i, const double *__restrict__ part_j,
+                                                                 double *acc, int N, int S, int col0, int ncols, int first,
+                                                                 const int *__restrict__ perm) {
+    const int t = blockIdx.x * kBodyThreads + threadIdx.x;
+    if (t >= N) return;
+    const int i = perm != nullptr ? perm[t] : t;
+    if (i >= N) return;
+    double ax = 0.0, ay = 0.0, az = 0.0;
+    if (!first) { ax = acc[3 * (size_t)i]; ay = acc[3 * (size_t)i + 1]; az = acc[3 * (size_t)i + 2]; }
+    for (int b = 0; b < ncols; ++b) {
+        if (t >= (long long)(col0 + b) * S) continue;
+        const double *q = part_i + ((size_t)b * N + t) * 3;
+        ax += q[0]; ay += q[1]; az += q[2];
+    }
+    const int X = t / S;
+    if (X >= col0 && X < col0 + ncols) {
+        const size_t stride = (size_t)ncols * S, off = (size_t)t - (size_t)col0 * S;
+        for (int A = 0; A <= X; ++A) {
+            const double *q = part_j + ((size_t)A * stride + off) * 3;
+            ax += q[0]; ay += q[1]; az += q[2];
+        }
+    }
+    acc[3 * (size_t)i] = ax; acc[3 * (size_t)i + 1] = ay; acc[3 * (size_t)i + 2] = az;
 }
 
 // momentum partials of the current v (standalone nb_shift)

@@ -43,7 +43,14 @@ struct SymParams {
     const double *rcrit;         // [N]    exact critical radii (slow path only), indexed by BODY
     const int *perm;             // [Npad] staged position -> body (sorted staging, sort_staging.cuh) or nullptr
     const BlockBound *bnd;       // [nsb]  azimuth / radius / rc bounds of every staged super-block, or nullptr
-    double *part;                // [nsb, N, 3]
+    // partial accelerations.  Whole grid in one launch (col0 = 0, ncols = nsb): part_i = part_j = [slots, N, 3],
+    // stride_i = stride_j = N, goff = 0 -- tile (A, B) writes slot B for A's bodies and slot A for B's.
+    // BANDED (large N: the slots of the whole grid would be 24 N^2 / S bytes): one launch per band of ncols tile
+    // columns B = col0 .. col0 + ncols - 1; the i sides go to part_i[B - col0][N] and the j sides of the band's bodies to
+    // part_j[A][ncols S] (goff = col0 S), both folded into acc by nb_bandsum_kernel before the next band reuses them.
+    double *part_i, *part_j;
+    long long stride_i, stride_j;
+    int goff, col0, ncols;
     int32_t *pairs;              // [cap,2] or nullptr
     unsigned long long *npairs;  // device counter
     long long *status;           // device int64[ST_COUNT]
@@ -68,6 +75,10 @@ constexpr int kSymSplit = 4;
 __host__ __device__ constexpr long long sym_split_tiles(long long T, long long C) { return C * (T - 1) - C * (C - 1) / 2; }
 __host__ __device__ constexpr long long sym_grid(long long T, long long C) {
     return T * (T + 1) / 2 + (kSymSplit - 1) * sym_split_tiles(T, C);
+}
+// CTAs of the launch that covers the tile columns col0 .. col0 + ncols - 1 (banded evaluation, no tail splitting)
+__host__ __device__ constexpr long long sym_band_grid(long long col0, long long ncols) {
+    return ncols + (col0 + ncols) * (col0 + ncols - 1) / 2 - col0 * (col0 - 1) / 2;
 }
 __host__ __device__ constexpr int sym_slots(int T, int C) { return T + (kSymSplit - 1) * C; }
 __host__ __device__ constexpr size_t sym_smem_bytes(int S) { return (size_t)S * (32 + 32 + 24 + 8) + 16; }
@@ -284,7 +295,7 @@ __device__ __forceinline__ void sym_tile(const SymParams &p, const int A, const 
             }
             __syncthreads();
         } else {
-            double *out = p.part + (size_t)ti[3] * p.N * 3;
+            double *out = p.part_i + (size_t)ti[3] * p.stride_i * 3;
 #pragma unroll
             for (int k = 0; k < I; ++k) {
                 const int i = i0 + 32 * k;
@@ -297,14 +308,14 @@ __device__ __forceinline__ void sym_tile(const SymParams &p, const int A, const 
         }
     }
     // j side (and, on the diagonal, both sides) -> slot A for B's bodies
-    double *out = p.part + (size_t)A * p.N * 3;
+    double *out = p.part_j + (size_t)A * p.stride_j * 3;
     const int jS = ti[0], j0 = ti[1];
     for (int n = t; n < jS; n += kThreads) {
         const long long g = (long long)j0 + n;
         if (g < p.N) {
-            out[3 * g] = jsx[n];
-            out[3 * g + 1] = jsy[n];
-            out[3 * g + 2] = jsz[n];
+            out[3 * (g - p.goff)] = jsx[n];
+            out[3 * (g - p.goff) + 1] = jsy[n];
+            out[3 * (g - p.goff) + 2] = jsz[n];
         }
     }
 }
@@ -328,19 +339,22 @@ __global__ void __launch_bounds__(32 * W, MINB) nb_force_sym_kernel(const SymPar
     // START take the CTAs of an SM out of lock step, -1.9 % at N = 65536 --, then the strict pairs A < B column by
     // column, the last xcols columns cut into kSymSplit parts each (see kSymSplit)
     const int T = p.nsb;
-    const long long nstrict = (long long)T * (T - 1) / 2;
-    const long long nwhole = nstrict - sym_split_tiles(T, p.xcols);   // strict tiles that run as one CTA
+    const int c1 = p.col0 + p.ncols;                                  // columns of this launch: col0 .. c1 - 1
+    const long long first = (long long)p.col0 * (p.col0 - 1) / 2;     // strict tiles in front of the band
+    const long long nstrict = (long long)c1 * (c1 - 1) / 2 - first;
+    const long long nwhole = nstrict - sym_split_tiles(T, p.xcols);   // strict tiles that run as one CTA (xcols > 0: whole grid only)
     int A, B, part = 0, nparts = 1;
-    if ((long long)blockIdx.x < T) {
-        A = B = (int)blockIdx.x;
+    if ((int)blockIdx.x < p.ncols) {
+        A = B = p.col0 + (int)blockIdx.x;
     } else {
-        long long idx = (long long)blockIdx.x - T;
+        long long idx = (long long)blockIdx.x - p.ncols;
         if (idx >= nwhole) {
             const long long k = idx - nwhole;
             idx = nwhole + k / kSymSplit;
             part = (int)(k % kSymSplit);
             nparts = kSymSplit;
         }
+        idx += first;
         B = (int)((1.0 + sqrt(1.0 + 8.0 * (double)idx)) * 0.5);
         while ((long long)B * (B - 1) / 2 > idx) --B;
         while ((long long)(B + 1) * B / 2 <= idx) ++B;
@@ -352,7 +366,7 @@ __global__ void __launch_bounds__(32 * W, MINB) nb_force_sym_kernel(const SymPar
         tinfo[0] = jS;
         tinfo[1] = B * S + joff;
         tinfo[2] = nparts == 1 ? p.U : (p.U / kSymSplit > 0 ? p.U / kSymSplit : 1);
-        tinfo[3] = part == 0 ? B : T + (T - 1 - B) * (kSymSplit - 1) + part - 1;
+        tinfo[3] = part == 0 ? B - p.col0 : T + (T - 1 - B) * (kSymSplit - 1) + part - 1;
     }
     const bool diag = (A == B);
 

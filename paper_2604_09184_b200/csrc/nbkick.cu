@@ -43,7 +43,7 @@ struct StepKey {
     const void *x, *v, *m, *rcrit, *acc, *pairs, *npairs, *ws, *stream;
     int64_t N, n_active, cap;
     double dt, M_star, G, n1, n2, bs_tol, drag_gamma, drag_eta, midpoint_tol;
-    int kind, ipt, jsplit, enc, levels, drag_power, midpoint_iters;
+    int kind, ipt, jsplit, enc, levels, drag_power, midpoint_iters, band;
     size_t ws_bytes;
 };
 StepKey g_graph_key;
@@ -101,6 +101,7 @@ struct Geometry {
     int S, U, Npad_sym;   // super-block size, 32-blocks per skew unit, N padded to a multiple of S
     int warps;            // symmetric kernel: warps per CTA (1, 2 or 4)
     int xcols;            // symmetric kernel: trailing tile columns cut into kSymSplit CTAs each (force_sym.cuh kSymSplit)
+    int band;             // symmetric kernel: tile columns per launch of the banded evaluation (0: the whole grid in one launch)
     int nslots;           // partial-acceleration slots nb_kickv_kernel sums (= nsplit + extra slots of the split columns)
     int sorted;           // symmetric kernel: bodies staged in azimuthal order (sort_staging.cuh)
     int mixed;            // mixed-precision one-sided kernel (force_mixed.cuh)
@@ -112,7 +113,7 @@ Geometry geometry(int64_t N, int64_t n_active) {
     g.tiles_total = (g.Nj + kTileJ - 1) / kTileJ;
     g.Njpad = g.tiles_total * kTileJ;
     const int sms = sm_count();
-    g.sym = 0; g.S = 0; g.U = 0; g.Npad_sym = 0; g.sorted = 0; g.warps = 4; g.xcols = 0; g.nslots = 0;
+    g.sym = 0; g.S = 0; g.U = 0; g.Npad_sym = 0; g.sorted = 0; g.warps = 4; g.xcols = 0; g.nslots = 0; g.band = 0;
     g.mixed = g_cfg.precision == NB_PRECISION_MIXED ? 1 : 0;
     // Newton-III kernel: fully active case only (a passive body exerts nothing, so there is no second
     // side to serve), and only when there are enough super-tiles to fill the machine several times.
@@ -126,14 +127,13 @@ Geometry geometry(int64_t N, int64_t n_active) {
         if (ipt != 1 && ipt != 2 && ipt != 4) ipt = 4;
         int S = g_cfg.sym_block;
         if (S != 128 && S != 256 && S != 512 && S != 1024 && S != 2048) {
-            // largest block whose grid still has enough waves of CTAs (measured crossovers: N ~ 24000 and ~ 60000);
-            // larger than 512 only to keep the N/S partial slots (24 N^2 / S bytes of workspace) under 16 GiB
+            // largest block whose grid still has enough waves of CTAs (measured crossovers: N ~ 24000 and ~ 60000).  The
+            // N/S partial slots (24 N^2 / S bytes) are bounded by the banded evaluation below, not by a larger S
             auto waves = [&](int s) {
                 const int64_t T = (N + s - 1) / s;
                 return (double)(T * (T + 1) / 2) / (double)((int64_t)sms * (1536 / s));
             };
             S = ipt == 4 ? (waves(512) >= 16.0 ? 512 : (waves(256) >= 5.0 ? 256 : 128)) : (waves(512) >= 16.0 ? 512 : 256);
-            while (S < 2048 && ((N + S - 1) / S) * N * 24 > ((int64_t)16 << 30)) S <<= 1;
         }
         if (ipt == 1 && S < 128) S = 128;
         // warps per CTA: chunks of 32 W I bodies must tile the super-block
@@ -160,6 +160,16 @@ Geometry geometry(int64_t N, int64_t n_active) {
             g.xcols = C;
         }
         g.nslots = sym_slots(g.nsplit, g.xcols);
+        {   // banded evaluation: when the slots of the whole grid would pass the cap (nb_config.slot_bytes_max, default
+            // 4 GiB), the tile columns run in bands of `band` columns, one launch + one fold per band, on
+            // 24 N band (i sides) + 24 Npad band (j sides of the band's bodies) bytes
+            const int64_t cap = g_cfg.slot_bytes_max > 0 ? g_cfg.slot_bytes_max : ((int64_t)4 << 30);
+            if ((int64_t)g.nslots * N * 24 > cap) {
+                int64_t band = cap / (24 * (N + (int64_t)g.Npad_sym));
+                if (band < 1) band = 1;
+                if (band < g.nsplit) { g.band = (int)band; g.xcols = 0; g.nslots = g.nsplit; }
+            }
+        }
         // sorted staging pays off once the sort (a few small launches) is small against the evaluation
         g.sorted = g_cfg.sort_staging == NB_SORT_ON || (g_cfg.sort_staging == NB_SORT_AUTO && N >= 32768);
         return g;
@@ -295,7 +305,8 @@ Workspace carve(void *base, int64_t N, const Geometry &g) {
     w.pos_of = reinterpret_cast<int *>(b + off); off += align_up((size_t)(g.sym ? N : 0) * sizeof(int), 256);
     w.bnd = reinterpret_cast<BlockBound *>(b + off); off += align_up((size_t)(g.sym ? g.nsplit : 0) * sizeof(BlockBound), 256);
     {   // partial accelerations; never smaller than 64 bytes per body (nb_merge's compaction buffer)
-        size_t pb = (size_t)g.nslots * (size_t)N * 3 * sizeof(double);
+        size_t pb = g.band > 0 ? (size_t)g.band * ((size_t)N + (size_t)g.Npad_sym) * 3 * sizeof(double)
+                               : (size_t)g.nslots * (size_t)N * 3 * sizeof(double);
         if (pb < (size_t)N * 64) pb = (size_t)N * 64;
         w.part = reinterpret_cast<double *>(b + off); off += align_up(pb, 256);
     }
@@ -369,7 +380,7 @@ template <int I, int W, int MINB, bool SORTED>
 int launch_sym_IMS(const SymParams &sp, const Geometry &g, bool pairs) {
     const size_t smem = sym_smem_bytes(g.S);
     const long long T = g.nsplit;
-    const unsigned ctas = (unsigned)sym_grid(T, g.xcols);
+    const unsigned ctas = (unsigned)(sp.ncols == (int)T ? sym_grid(T, g.xcols) : sym_band_grid(sp.col0, sp.ncols));
     auto go = [&](auto kern) -> int {
         NB_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         kern<<<ctas, 32 * W, smem, stream()>>>(sp);
@@ -454,19 +465,36 @@ int enqueue_eval(const Workspace &w, const Geometry &g, double *x, double *v, co
     if (g.sym) {
         SymParams sp;
         sp.perm = sorted ? w.perm : nullptr; sp.bnd = sorted ? w.bnd : nullptr;
-        sp.sxy = w.sxy; sp.szg = w.szg; sp.sthr = w.sthr; sp.rcrit = rc_io; sp.part = w.part; sp.pairs = pairs;
+        sp.sxy = w.sxy; sp.szg = w.szg; sp.sthr = w.sthr; sp.rcrit = rc_io; sp.pairs = pairs;
         sp.npairs = fp.npairs; sp.status = w.status; sp.cap = fp.cap; sp.N = (int)N; sp.S = g.S; sp.nsb = g.nsplit;
         sp.U = g.U; sp.kind = g_cfg.changeover_kind; sp.xcols = g.xcols;
-        const int lrc = launch_sym(sp, g, pairs != nullptr);
-        if (lrc) return lrc;
+        if (g.band == 0) {
+            sp.part_i = w.part; sp.part_j = w.part; sp.stride_i = N; sp.stride_j = N; sp.goff = 0; sp.col0 = 0; sp.ncols = g.nsplit;
+            const int lrc = launch_sym(sp, g, pairs != nullptr);
+            if (lrc) return lrc;
+        } else {
+            // banded: i sides [band][N], then the j sides of the band's bodies [nsb][band S]; folded into acc band by band
+            sp.part_i = w.part; sp.part_j = w.part + (size_t)g.band * (size_t)N * 3; sp.stride_i = N;
+            for (int c0 = 0; c0 < g.nsplit; c0 += g.band) {
+                sp.col0 = c0; sp.ncols = g.nsplit - c0 < g.band ? g.nsplit - c0 : g.band;
+                sp.stride_j = (long long)sp.ncols * g.S; sp.goff = c0 * g.S;
+                const int lrc = launch_sym(sp, g, pairs != nullptr);
+                if (lrc) return lrc;
+                nb_bandsum_kernel<<<nblk, kBodyThreads, 0, stream()>>>(sp.part_i, sp.part_j, acc, (int)N, g.S, sp.col0, sp.ncols,
+                                                                      c0 == 0 ? 1 : 0, sorted ? w.perm : nullptr);
+            }
+        }
     } else {
         launch_force(fp, g, pairs != nullptr);
     }
     if (pool) { NB_CUDA(cudaEventRecord(g_tev[2 * g_tev_used + 1], stream())); ++g_tev_used; }
     else if (time_force) { NB_CUDA(cudaEventRecord(g_ev1, stream())); g_force_timed = true; }
 
-    nb_kickv_kernel<<<nblk, kBodyThreads, 0, stream()>>>(w.part, g.nsplit, acc, v, m, (int)N, hk, nhalf, mv_out,
-                                                         sorted ? w.perm : nullptr, g.xcols, g.S);
+    if (g.sym && g.band > 0)   // acc already holds the sum: it is read as one slot, indexed by body
+        nb_kickv_kernel<<<nblk, kBodyThreads, 0, stream()>>>(acc, 1, acc, v, m, (int)N, hk, nhalf, mv_out, nullptr, 0, 0);
+    else
+        nb_kickv_kernel<<<nblk, kBodyThreads, 0, stream()>>>(w.part, g.nsplit, acc, v, m, (int)N, hk, nhalf, mv_out,
+                                                             sorted ? w.perm : nullptr, g.xcols, g.S);
     NB_CUDA(cudaGetLastError());
     return NB_OK;
 }
@@ -762,7 +790,7 @@ int step_impl(double *x, double *v, const double *m, double M_star, int64_t N, d
         key.x = x; key.v = v; key.m = m; key.rcrit = rc_io; key.acc = acc; key.pairs = pairs; key.npairs = npairs;
         key.ws = g_cfg.workspace; key.stream = g_cfg.stream; key.N = N; key.n_active = g_cfg.n_active;
         key.cap = g_cfg.pair_capacity; key.dt = dt; key.M_star = M_star; key.G = g_cfg.G; key.n1 = g_cfg.n1;
-        key.n2 = g_cfg.n2; key.kind = g_cfg.changeover_kind; key.bs_tol = g_cfg.bs_tol; key.enc = (enc ? 1 : 0) + 2 * g.sorted; key.ipt = g.S * 1000 + g.ipt * 100 + g.minb * 10 + g.warps + 100000 * g.xcols; key.jsplit = g.nsplit;
+        key.n2 = g_cfg.n2; key.kind = g_cfg.changeover_kind; key.bs_tol = g_cfg.bs_tol; key.enc = (enc ? 1 : 0) + 2 * g.sorted; key.ipt = g.S * 1000 + g.ipt * 100 + g.minb * 10 + g.warps + 100000 * g.xcols; key.jsplit = g.nsplit; key.band = g.band;
         key.ws_bytes = g_cfg.workspace_bytes; key.levels = g_cfg.levels;
         key.drag_gamma = g_cfg.drag_gamma; key.drag_eta = g_cfg.drag_eta; key.midpoint_tol = g_cfg.midpoint_tol;
         key.drag_power = g_cfg.drag_power; key.midpoint_iters = g_cfg.midpoint_iters + 1000 * g.mixed;
@@ -852,6 +880,7 @@ void nb_default_config(nb_config *cfg) {
     cfg->midpoint_iters = 50;
     cfg->midpoint_tol = 1e-14;
     cfg->precision = NB_PRECISION_F64;
+    cfg->slot_bytes_max = 0;
 }
 
 int nb_configure(const nb_config *cfg) {
@@ -878,6 +907,7 @@ int nb_configure(const nb_config *cfg) {
         (cfg->drag_power != 0 && cfg->drag_power != 1) || cfg->midpoint_iters < 0 || !(cfg->midpoint_tol >= 0.0))
         return fail(NB_E_BADARG, "drag_gamma >= 0, finite drag_eta, drag_power 0 or 1, midpoint_iters >= 0, midpoint_tol >= 0");
     if (cfg->precision != NB_PRECISION_F64 && cfg->precision != NB_PRECISION_MIXED) return fail(NB_E_BADARG, "unknown precision %d", cfg->precision);
+    if (cfg->slot_bytes_max < 0) return fail(NB_E_BADARG, "slot_bytes_max < 0");
     if (cfg->levels < 0 || cfg->levels > kMaxLevels) return fail(NB_E_BADARG, "levels must be 0 .. %d", kMaxLevels);
     g_cfg = *cfg;
     return NB_OK;

@@ -274,3 +274,59 @@ def test_sorted_staging_with_encounters_resolved():
     assert ref["stats"]["integrated"] > 0
     assert np.max(np.abs(xg - ref["x"])) <= 1e-9 * np.max(np.abs(ref["x"]))
     assert np.max(np.abs(vg - ref["v"])) <= 1e-9 * np.max(np.abs(ref["v"]))
+
+
+# ---- banded evaluation (nb_config.slot_bytes_max): the tile columns in several launches, folded into acc band by band
+
+def _band_cap(N, S, band):
+    """slot_bytes_max that yields `band` tile columns per launch (24 (N + Npad) bytes per column)"""
+    npad = -(-N // S) * S
+    return 24 * (N + npad) * band + 8
+
+
+@pytest.mark.parametrize("N,ipt,S,band,sort", [(3000, 4, 128, 5, 0), (3000, 4, 128, 1, 0), (3333, 4, 256, 3, 1), (2500, 2, 256, 4, 0),
+                                               (5000, 4, 512, 2, 1), (3000, 4, 128, 23, 1)])
+def test_banded_evaluation_against_oracle(N, ipt, S, band, sort):
+    import paper_2604_09184_b200 as nb
+    x, v, m = nb_inputs.random_cluster(N, seed=700 + N + band, scale=0.2)
+    rng = np.random.default_rng(band)
+    rc = rng.uniform(0.0, 0.05, N)
+    rc[::5] = 0.0
+    tune = dict(force_kernel=SYM, i_per_thread=ipt, sym_block=S, sort_staging=1 if sort else 2, slot_bytes_max=_band_cap(N, S, band))
+    info = _kick_case(x, v, m, rc, dt=0.37, what=f"banded N={N} I={ipt} S={S} band={band} sorted={sort}", **tune)
+    assert info["n_sure"] > 100
+    # the banded workspace is the small one (two sets of `band` column slots against T slots)
+    T = -(-N // S)
+    if 3 * band <= T:
+        ws_band = nb.workspace_bytes(N)
+        nb.set_flags(slot_bytes_max=0)
+        assert ws_band < nb.workspace_bytes(N)
+    # same pair list and (to rounding order) the same accelerations as the one-launch evaluation; bit-reproducible
+    out = []
+    for cap in (_band_cap(N, S, band), _band_cap(N, S, band), 0):
+        st = GpuState(x, v, m, G=G_GAUSS, **dict(tune, slot_bytes_max=cap))
+        st.set_rcrit(rc)
+        st.kick(0.0)
+        gp, n = st.get_pairs()
+        out.append((st.acc.cpu().numpy().copy(), {tuple(p) for p in gp[:n].tolist()}))
+    assert np.array_equal(out[0][0], out[1][0]), "the banded evaluation is not run-to-run reproducible"
+    assert out[0][1] == out[1][1] == out[2][1]
+    scale = np.linalg.norm(out[2][0], axis=1, keepdims=True)
+    assert np.max(np.abs(out[0][0] - out[2][0]) / scale) < 1e-12
+
+
+@pytest.mark.parametrize("use_graph", [True, False])
+def test_banded_step_matches_oracle(use_graph):
+    d = nb_inputs.make_config(1, n_override=1498)
+    st = GpuState(d.x, d.v, d.m, d.M_star, G=G_GAUSS, n1=3.0, n2=0.4, force_kernel=SYM, sym_block=128, use_graph=use_graph,
+                  slot_bytes_max=_band_cap(d.N, 128, 5))
+    st.step(d.dt, 20)
+    xg, vg, ag, rcg = st.host()
+    ref = oracle.step(d.x, d.v, d.m, d.M_star, d.dt, G_GAUSS, 20, n1=3.0, n2=0.4)
+    ex = np.max(np.abs(xg - ref["x"])) / np.max(np.abs(ref["x"]))
+    ev = np.max(np.abs(vg - ref["v"])) / np.max(np.abs(ref["v"]))
+    print(f"banded step x20 graph={use_graph}: rel dx {ex:.2e} dv {ev:.2e}")
+    assert ex <= 1e-11 and ev <= 1e-11
+    sure, border = oracle.pairs(ref["x"], ref["rcrit"])
+    gp, n = st.get_pairs()
+    assert_pairs_match(gp, n, sure, border, "banded step")
