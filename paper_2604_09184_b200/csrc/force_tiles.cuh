@@ -136,11 +136,11 @@ template <int I, bool PAIRS>
 __device__ __forceinline__ void slow_path(const ForceParams &p, const double4 A, const double4 B, const int j,
                                           const double (&xi)[I], const double (&yi)[I], const double (&zi)[I],
                                           const double (&rci)[I], const int i0, double (&ax)[I], double (&ay)[I],
-                                          double (&az)[I]) {
+                                          double (&az)[I], const bool mine = true) {
 #pragma unroll
     for (int k = 0; k < I; ++k) {
         const int i = i0 + k * kForceThreads;
-        const bool valid = (i < p.N) && (j < p.Nj) && (i != j);
+        const bool valid = mine && (i < p.N) && (j < p.Nj) && (i != j);
         const double dx = A.x - xi[k], dy = A.y - yi[k], dz = A.z - zi[k];
         const double r2 = __fma_rn(dz, dz, __fma_rn(dy, dy, __dmul_rn(dx, dx)));
         const double rc = fmax(rci[k], B.w);
@@ -196,7 +196,9 @@ struct JWork {
 
 // The work of one CTA of kForceThreads threads: i-block bx, j-split by.  sm / full / empty: the CTA's shared-memory ring and
 // its barriers, NOT yet initialised (a persistent caller -- step_small.cuh -- invalidates them between work items).
-template <int I, bool PAIRS>
+// BF: branch-free tile loop (latency-bound launches: few CTAs of one or two tiles each -- small N; measured N = 2048:
+// 22.6 -> 16.5 us, but +6 % where the FP64 pipe is the limit, N = 65536 and the semi-active config)
+template <int I, bool PAIRS, bool BF>
 __device__ __forceinline__ void force_tiles_cta(const ForceParams &p, const int bx, const int by, JRec (*sm)[kTileJ],
                                                 uint64_t *full, uint64_t *empty) {
     const int t = threadIdx.x;
@@ -285,6 +287,35 @@ __device__ __forceinline__ void force_tiles_cta(const ForceParams &p, const int 
             }
         };
 
+        if (BF) {
+            // Branch-free form (as in force_sym.cuh): a lane within reach of a critical radius (always the self term)
+            // feeds +inf to its seeds -- its I pairs contribute exactly 0 -- and sets a bit; the flagged j of each
+            // group of 32 are then evaluated exactly by the lanes that flagged them.  No vote and no branch per j, so
+            // consecutive j overlap in the FP64 pipe: what a CTA with a single tile (small N, semi-active) is short of.
+            for (int g0 = 0; g0 < kTileJ; g0 += 32) {
+                unsigned bits = 0u;
+#pragma unroll 4
+                for (int jj = 0; jj < 32; ++jj) {
+                    JWork<I> cur;
+                    cur.load(tile + g0 + jj, xi, yi, zi, thr_i);
+                    const bool hit = cur.mn <= cur.thr;
+                    bits |= (hit ? 1u : 0u) << jj;
+                    const int kill = hit ? 0x7ff00000 : 0;
+                    double y0[I];
+#pragma unroll
+                    for (int k = 0; k < I; ++k)
+                        y0[k] = rsqrt_seed(__hiloint2double(max(__double2hiint(cur.r2[k]), kill), 0));
+                    fast(cur, y0);
+                }
+                unsigned any = __reduce_or_sync(0xffffffffu, bits);
+                while (any) {
+                    const int jj = __ffs(any) - 1;
+                    any &= any - 1u;
+                    const double4 *q = reinterpret_cast<const double4 *>(tile + g0 + jj);
+                    slow_path<I, PAIRS>(p, q[0], q[1], jbase + g0 + jj, xi, yi, zi, rci, i0, ax, ay, az, ((bits >> jj) & 1u) != 0u);
+                }
+            }
+        } else {
 #pragma unroll 2
         for (int jj = 0; jj < kTileJ; ++jj) {
             JWork<I> cur;
@@ -296,6 +327,7 @@ __device__ __forceinline__ void force_tiles_cta(const ForceParams &p, const int 
                 slow_path<I, PAIRS>(p, cur.A, cur.B, jbase + jj, xi, yi, zi, rci, i0, ax, ay, az);
             else
                 fast(cur, y0);
+        }
         }
 #pragma unroll
         for (int k = 0; k < I; ++k) { ox[k] += ax[k]; oy[k] += ay[k]; oz[k] += az[k]; }
@@ -316,12 +348,12 @@ __device__ __forceinline__ void force_tiles_cta(const ForceParams &p, const int 
 }
 
 // MINB = CTAs per SM the register allocation is capped for.
-template <int I, bool PAIRS, int MINB>
+template <int I, bool PAIRS, int MINB, bool BF>
 __global__ void __launch_bounds__(kForceThreads, MINB) nb_force_tiles_kernel(const ForceParams p) {
     __shared__ __align__(128) JRec sm[kStages][kTileJ];
     __shared__ __align__(8) uint64_t full[kStages];
     __shared__ __align__(8) uint64_t empty[kStages];
-    force_tiles_cta<I, PAIRS>(p, blockIdx.x, blockIdx.y, sm, full, empty);
+    force_tiles_cta<I, PAIRS, BF>(p, blockIdx.x, blockIdx.y, sm, full, empty);
 }
 
 }  // namespace nbk

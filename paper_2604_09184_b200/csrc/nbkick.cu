@@ -346,6 +346,8 @@ int check_workspace_head(int64_t N, int level /* 0 status, 1 + momentum partials
     return NB_OK;
 }
 
+constexpr int64_t kSmallStepMaxN = 8192;   // the fused small-N step (step_small.cuh) takes N up to this
+
 inline int body_blocks(int64_t n) { return (int)((n + kBodyThreads - 1) / kBodyThreads); }
 
 // register caps measured fastest on B200 (profiles/): one-sided kernel I = 1, 2 at 5 CTAs/SM, I = 4 at 3;
@@ -353,8 +355,16 @@ inline int body_blocks(int64_t n) { return (int)((n + kBodyThreads - 1) / kBodyT
 template <int I, int MINB>
 void launch_force_IM(const ForceParams &fp, const Geometry &g, bool pairs) {
     dim3 grid(g.iblocks, g.nsplit);
-    if (pairs) nb_force_tiles_kernel<I, true, MINB><<<grid, kForceThreads, 0, stream()>>>(fp);
-    else nb_force_tiles_kernel<I, false, MINB><<<grid, kForceThreads, 0, stream()>>>(fp);
+    // fewer than two waves of CTAs: the launch is latency-bound, the branch-free tile loop wins (force_tiles.cuh)
+    // (always for the sizes the fused small-N step takes, which runs the branch-free loop: the two paths stay bit-identical)
+    const bool bf = fp.N <= kSmallStepMaxN || (int64_t)g.iblocks * g.nsplit < (int64_t)2 * MINB * sm_count();
+    if (pairs) {
+        if (bf) nb_force_tiles_kernel<I, true, MINB, true><<<grid, kForceThreads, 0, stream()>>>(fp);
+        else nb_force_tiles_kernel<I, true, MINB, false><<<grid, kForceThreads, 0, stream()>>>(fp);
+    } else {
+        if (bf) nb_force_tiles_kernel<I, false, MINB, true><<<grid, kForceThreads, 0, stream()>>>(fp);
+        else nb_force_tiles_kernel<I, false, MINB, false><<<grid, kForceThreads, 0, stream()>>>(fp);
+    }
 }
 
 template <int I, int MINB>
@@ -647,7 +657,6 @@ MlParams ml_params(const Workspace &w, double *x, double *v, const double *m, co
 }
 
 // ---- small N: whole steps in one cooperative launch (step_small.cuh) ----
-constexpr int64_t kSmallStepMaxN = 8192;
 
 template <int I>
 int launch_step_small_I(const SmallStepParams &q, bool pairs, int work_items) {

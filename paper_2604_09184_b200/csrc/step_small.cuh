@@ -113,7 +113,7 @@ __global__ void __launch_bounds__(kForceThreads, I == 4 ? 3 : 4) nb_step_small_k
             // the ring was written through the generic proxy (reduction scratch) and is about to be written by TMA
             asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
             __syncthreads();   // nobody still reads the ring (scratch or the previous work item)
-            force_tiles_cta<I, PAIRS>(q.fp, w % q.iblocks, w / q.iblocks, ring, full, empty);
+            force_tiles_cta<I, PAIRS, true>(q.fp, w % q.iblocks, w / q.iblocks, ring, full, empty);
             __syncthreads();
             if (t == 0) {
 #pragma unroll
