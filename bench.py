@@ -222,6 +222,18 @@ def _traffic_from_profile(kernel, N, geom, sorted_staging, precision):
     return None, "no ncu capture of this geometry under profiles/ (not measured in this run)"
 
 
+def _extra_band_launches(N, geom, cap=4 << 30):
+    """Launches a banded evaluation of the Newton-III kernel adds to a step: 2 per band minus the one force launch already
+    counted (the library's rule: slots of the whole grid over nb_config.slot_bytes_max, default 4 GiB)."""
+    if geom.tile_j >= 0:
+        return 0
+    S, T = -geom.tile_j, geom.j_splits
+    if 24 * N * T <= cap:
+        return 0
+    band = max(1, cap // (24 * (N + T * S)))
+    return 2 * (-(-T // band)) - 1
+
+
 def _hbm_peak_gbs():
     """(GB/s, source): the driver-measured copy bandwidth, else the profiling guide's fallback."""
     try:
@@ -437,7 +449,8 @@ def run_cuda(args):
         clocks=clocks,
         # per timed step: opening half-kick, drift, prep, force, slot sum + closing half-kick; with the Newton-III kernel's
         # sorted staging (automatic for N >= 32768) also five sort kernels and the bounds kernel
-        gpu_launches=(11 if sorted_staging else 5) * K,
+        # banded evaluation (N beyond ~180 000: DESIGN.md 5.1d): one force launch and one fold per band instead of one launch
+        gpu_launches=((11 if sorted_staging else 5) + _extra_band_launches(N, geom)) * K,
         groups=groups_info,
     )
     if e2e:

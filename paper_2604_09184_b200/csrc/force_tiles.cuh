@@ -40,8 +40,6 @@ struct ForceParams {
     int Nj;           // number of force-exerting bodies (= n_active)
     int tiles_total;  // ceil(Nj / kTileJ)
     int tiles_per_split;
-    int sub;          // small N: pieces per j-tile (1, 2 or 4; > 1 only with tiles_per_split == 1 and the branch-free loop):
-                      // split by covers piece by % sub of tile by / sub -- 4x the CTAs, a quarter of the dependent iterations each
     int kind;  // changeover shape
 };
 
@@ -205,9 +203,8 @@ __device__ __forceinline__ void force_tiles_cta(const ForceParams &p, const int 
                                                 uint64_t *full, uint64_t *empty) {
     const int t = threadIdx.x;
     const int i0 = bx * (kForceThreads * I) + t;
-    const int sub = BF ? p.sub : 1;
-    const int tile_begin = sub > 1 ? by / sub : by * p.tiles_per_split;
-    int tile_end = tile_begin + (sub > 1 ? 1 : p.tiles_per_split);
+    const int tile_begin = by * p.tiles_per_split;
+    int tile_end = tile_begin + p.tiles_per_split;
     if (tile_end > p.tiles_total) tile_end = p.tiles_total;
     const int ntiles = tile_end - tile_begin;
     constexpr unsigned kTileBytes = kTileJ * sizeof(JRec);
@@ -295,8 +292,7 @@ __device__ __forceinline__ void force_tiles_cta(const ForceParams &p, const int 
             // feeds +inf to its seeds -- its I pairs contribute exactly 0 -- and sets a bit; the flagged j of each
             // group of 32 are then evaluated exactly by the lanes that flagged them.  No vote and no branch per j, so
             // consecutive j overlap in the FP64 pipe: what a CTA with a single tile (small N, semi-active) is short of.
-            const int g_lo = sub > 1 ? (by % sub) * (kTileJ / sub) : 0, g_hi = sub > 1 ? g_lo + kTileJ / sub : kTileJ;
-            for (int g0 = g_lo; g0 < g_hi; g0 += 32) {
+            for (int g0 = 0; g0 < kTileJ; g0 += 32) {
                 unsigned bits = 0u;
 #pragma unroll 4
                 for (int jj = 0; jj < 32; ++jj) {

@@ -101,7 +101,6 @@ struct Geometry {
     int S, U, Npad_sym;   // super-block size, 32-blocks per skew unit, N padded to a multiple of S
     int warps;            // symmetric kernel: warps per CTA (1, 2 or 4)
     int xcols;            // symmetric kernel: trailing tile columns cut into kSymSplit CTAs each (force_sym.cuh kSymSplit)
-    int sub;              // one-sided kernel at small N: pieces per j-tile (force_tiles.cuh ForceParams::sub)
     int band;             // symmetric kernel: tile columns per launch of the banded evaluation (0: the whole grid in one launch)
     int nslots;           // partial-acceleration slots nb_kickv_kernel sums (= nsplit + extra slots of the split columns)
     int sorted;           // symmetric kernel: bodies staged in azimuthal order (sort_staging.cuh)
@@ -116,7 +115,7 @@ Geometry geometry(int64_t N, int64_t n_active) {
     g.tiles_total = (g.Nj + kTileJ - 1) / kTileJ;
     g.Njpad = g.tiles_total * kTileJ;
     const int sms = sm_count();
-    g.sym = 0; g.S = 0; g.U = 0; g.Npad_sym = 0; g.sorted = 0; g.warps = 4; g.xcols = 0; g.nslots = 0; g.band = 0; g.sub = 1;
+    g.sym = 0; g.S = 0; g.U = 0; g.Npad_sym = 0; g.sorted = 0; g.warps = 4; g.xcols = 0; g.nslots = 0; g.band = 0;
     g.mixed = g_cfg.precision == NB_PRECISION_MIXED ? 1 : 0;
     // Newton-III kernel: fully active case only (a passive body exerts nothing, so there is no second
     // side to serve), and only when there are enough super-tiles to fill the machine several times.
@@ -219,13 +218,6 @@ Geometry geometry(int64_t N, int64_t n_active) {
     if (nsplit > 65535) nsplit = 65535;
     g.tiles_per_split = (g.tiles_total + nsplit - 1) / nsplit;
     g.nsplit = (g.tiles_total + g.tiles_per_split - 1) / g.tiles_per_split;
-    // small N (branch-free loop, one tile per CTA, still under two waves of CTAs): cut every tile into 2 or 4 pieces --
-    // the launch is bound by the chain of dependent j-iterations of a CTA, not by the FP64 pipe
-    if (g_cfg.j_splits <= 0 && N <= kSmallStepMaxN && !g.mixed && g.tiles_per_split == 1) {
-        const int64_t ctas = (int64_t)g.iblocks * g.nsplit, two_waves = (int64_t)2 * g.minb * sms;
-        g.sub = ctas * 4 <= two_waves ? 4 : (ctas * 2 <= two_waves ? 2 : 1);
-        g.nsplit *= g.sub;
-    }
     g.nslots = g.nsplit;
     return g;
 }
@@ -465,7 +457,7 @@ int enqueue_eval(const Workspace &w, const Geometry &g, double *x, double *v, co
     fp.jrec = w.jrec; fp.x = x; fp.rcrit = rc_io; fp.part = w.part; fp.pairs = pairs;
     fp.npairs = pairs ? reinterpret_cast<unsigned long long *>(npairs) : w.npairs_dummy;
     fp.status = w.status; fp.cap = pairs ? g_cfg.pair_capacity : 0; fp.N = (int)N; fp.Nj = g.Nj;
-    fp.tiles_total = g.tiles_total; fp.tiles_per_split = g.tiles_per_split; fp.sub = g.sub; fp.kind = g_cfg.changeover_kind;
+    fp.tiles_total = g.tiles_total; fp.tiles_per_split = g.tiles_per_split; fp.kind = g_cfg.changeover_kind;
     // bounds of the staged super-blocks (before the timing events: they bracket the force kernel alone)
     if (sorted) nb_sort_bounds_kernel<<<g.nsplit, kGrpThreads, 0, stream()>>>(w.sxy, w.perm, rc_io, (int)N, g.S, w.bnd);
     const bool pool = g_cfg.time_force && g_tev_used < kMaxTimed;
@@ -700,7 +692,7 @@ int launch_step_small(const Workspace &w, const Geometry &g, double *x, double *
     fp.jrec = w.jrec; fp.x = x; fp.rcrit = rc_io; fp.part = w.part; fp.pairs = pairs;
     fp.npairs = pairs ? reinterpret_cast<unsigned long long *>(npairs) : w.npairs_dummy;
     fp.status = w.status; fp.cap = pairs ? g_cfg.pair_capacity : 0; fp.N = (int)N; fp.Nj = g.Nj;
-    fp.tiles_total = g.tiles_total; fp.tiles_per_split = g.tiles_per_split; fp.sub = g.sub; fp.kind = g_cfg.changeover_kind;
+    fp.tiles_total = g.tiles_total; fp.tiles_per_split = g.tiles_per_split; fp.kind = g_cfg.changeover_kind;
     q.acc = acc; q.mvA = w.mvA; q.mvB = w.mvB; q.mu = g_cfg.G * M_star; q.dt = dt; q.hk = 0.5 * dt; q.dtc = 0.5 * dt;
     q.nsteps = (int)(nsteps > 2000000000LL ? 2000000000LL : nsteps); q.last_nhalf = 1;
     q.iblocks = g.iblocks; q.nsplit = g.nsplit; q.nblk = body_blocks(N);

@@ -54,7 +54,7 @@ def test_configure_validation(nb):
     cfg = nb.default_config()
     assert lib.nb_configure(C.byref(cfg)) == 0
     for field, bad in (("G", -1.0), ("n1", -3.0), ("n2", float("nan")), ("pair_capacity", -1), ("n_active", -5),
-                       ("changeover_kind", 7), ("i_per_thread", 3), ("j_splits", -2)):
+                       ("changeover_kind", 7), ("i_per_thread", 3), ("j_splits", -2), ("sym_block", 300), ("slot_bytes_max", -1)):
         c = nb.default_config()
         setattr(c, field, bad)
         assert lib.nb_configure(C.byref(c)) == nb.binding.NB_E_BADARG, field
@@ -118,12 +118,8 @@ def test_geometry_and_workspace(nb):
             assert g.tile_j == 128 and g.threads == 128
             assert g.i_blocks * g.threads * g.i_per_thread >= N > (g.i_blocks - 1) * g.threads * g.i_per_thread
             tiles = -(-nj // g.tile_j)
-            if g.j_splits > tiles:
-                # small N: every tile cut into 2 or 4 pieces (more, shorter CTAs: the launch is latency-bound)
-                assert N <= 8192 and g.j_splits % tiles == 0 and g.j_splits // tiles in (2, 4)
-            else:
-                per = -(-tiles // g.j_splits)
-                assert (g.j_splits - 1) * per < tiles <= g.j_splits * per
+            per = -(-tiles // g.j_splits)
+            assert (g.j_splits - 1) * per < tiles <= g.j_splits * per
             assert g.i_blocks * g.j_splits >= 148
             assert ws >= 64 * nj + 24 * N * g.j_splits
         if not n_active:

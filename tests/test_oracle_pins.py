@@ -643,3 +643,24 @@ def test_S9_plain_fp64_misses_the_literal_bound_where_terms_cancel():
     assert out[3.0][0] > 1.0 and out[30.0][0] > 1.0          # the S9-only bound is missed by plain fp64
     assert out[3.0][1] < 0.5 and out[30.0][1] < 0.5          # the backward-error form holds with margin
     assert out[30.0][2] > 1e4
+
+
+def test_golden_legs_are_consecutive_calls_of_step(tmp_path):
+    """oracle/make_golden.py can write a full-size trajectory in legs (a run that does not fit one session): the stored values
+    must be those of consecutive oracle.step calls, each from the state the previous one returned -- and, where no pair sits
+    inside a critical radius, of ONE call (the closing half-kick of a step and the opening half-kick of the next are separate
+    roundings of the same recomputed force; only r_crit of a call's first evaluation sees the call boundary, reading S17)."""
+    from oracle import make_golden
+    d = nbi.make_config(0, n_override=200)
+    state = str(tmp_path / "legs.npz")
+    make_golden.run(0, 4, 200, str(tmp_path), "1/2", state)
+    g = make_golden.load(make_golden.run(0, 4, 200, str(tmp_path), "2/2", state))
+    assert int(g["legs"]) == 2 and int(g["nsteps"]) == 4
+    b = oracle.step(d.x, d.v, d.m, d.M_star, d.dt, nbi.G_GAUSS, 2, n1=make_golden.N1, n2=make_golden.N2)
+    b = oracle.step(b["x"], b["v"], d.m, d.M_star, d.dt, nbi.G_GAUSS, 2, n1=make_golden.N1, n2=make_golden.N2)
+    rows = g["row_index"]
+    assert np.array_equal(g["x"], b["x"][rows]) and np.array_equal(g["v"], b["v"][rows]) and np.array_equal(g["acc"], b["acc"][rows])
+    one = oracle.step(d.x, d.v, d.m, d.M_star, d.dt, nbi.G_GAUSS, 4, n1=make_golden.N1, n2=make_golden.N2)
+    sure, border = oracle.pairs(one["x"], one["rcrit"])
+    if sure.shape[0] + border.shape[0] == 0:
+        assert np.array_equal(one["x"], b["x"]) and np.array_equal(one["v"], b["v"])
