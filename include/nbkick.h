@@ -121,7 +121,10 @@ typedef struct nb_config {
 } nb_config;
 
 void nb_default_config(nb_config *cfg);
-/* Copies *cfg; validates G > 0, n1,n2 >= 0 and finite, pair_capacity >= 0, n_active >= 0. */
+/* Copies *cfg; validates G > 0, n1,n2 >= 0 and finite, pair_capacity >= 0, n_active >= 0.
+ * The configuration is ONE per process (calls are serialised by a mutex): two simulations in one process re-issue
+ * nb_configure between their calls, and share the one cached CUDA graph of an interior step (it is re-captured
+ * whenever the pointers, sizes or tuning of the call differ from the cached ones). */
 int nb_configure(const nb_config *cfg);
 /* Bytes of scratch the device-pointer calls need for N bodies under the current tuning (the force
  * kernels' partial sums dominate: 24 N x slots).  The O(N) calls need only its head: nb_rcrit none,
@@ -324,6 +327,7 @@ int nb_force_geometry(int64_t N, int64_t *out5);
  * Measurement aid: runs a register-only chain of independent fp64 FMAs on every SM and returns
  * the achieved rate in *tflops (2 flops per FMA), the roofline denominator for the kick.
  * Synchronises.  iters = FMAs per chain step; 0 = default.
+ * Unlike the calls of the path this one allocates: a small result buffer (cudaMalloc / cudaFree inside the call).
  */
 int nb_fp64_peak(int64_t iters, double *tflops, double *ms);
 
