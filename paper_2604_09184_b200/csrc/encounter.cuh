@@ -82,6 +82,9 @@ struct EncParams {
     int kind;
     int min_size, max_size;   // this launch handles groups with min_size <= n <= max_size
     const int *gcore;         // [ngroups] active members per group (semi-active mode) or nullptr
+    unsigned long long *work; // [2] work counters of the small-group and the satellite kernel, zero at launch: the CTAs take the
+                              // next problem when they are done with one (a few hard encounters take ~70 Bulirsch-Stoer steps,
+                              // most take one or two: a fixed stride would leave the last CTAs with the hard ones)
 };
 
 __device__ __forceinline__ int enc_group_size(const EncParams &p, const long long g, const int n, bool &split);
@@ -383,9 +386,15 @@ __device__ __forceinline__ int enc_group_size(const EncParams &p, const long lon
 }
 
 __global__ void __launch_bounds__(32 * kBsCols) nb_encounter_small_kernel(const EncParams p) {
+    __shared__ long long sh_next;
     const int lane = threadIdx.x & 31;
     const long long ngroups = p.gstat[0];
-    for (long long g = blockIdx.x; g < ngroups; g += gridDim.x) {
+    while (true) {
+        __syncthreads();
+        if (threadIdx.x == 0) sh_next = (long long)atomicAdd(p.work, 1ull);
+        __syncthreads();
+        const long long g = sh_next;
+        if (g >= ngroups) break;
         const int g0 = p.gstart[g];
         bool split;
         const int n = enc_group_size(p, g, p.gstart[g + 1] - g0, split);
@@ -400,10 +409,15 @@ __global__ void __launch_bounds__(32 * kBsCols) nb_encounter_small_kernel(const 
 // latency-bound kernel above is faster uncapped).
 __global__ void __launch_bounds__(32 * kBsCols, 4) nb_encounter_sat_kernel(const EncParams p) {
     __shared__ int sh_g;
+    __shared__ long long sh_k;
     const int lane = threadIdx.x & 31;
     const long long ngroups = p.gstat[0], nslots = p.gstat[1];
-    for (long long k = blockIdx.x; k < nslots; k += gridDim.x) {
+    while (true) {
         __syncthreads();
+        if (threadIdx.x == 0) sh_k = (long long)atomicAdd(p.work + 1, 1ull);
+        __syncthreads();
+        const long long k = sh_k;
+        if (k >= nslots) break;
         if (threadIdx.x == 0) {  // group of member slot k: last g with gstart[g] <= k
             long long lo = 0, hi = ngroups - 1;
             while (lo < hi) { const long long mid = (lo + hi + 1) >> 1; if (p.gstart[mid] <= k) lo = mid; else hi = mid - 1; }

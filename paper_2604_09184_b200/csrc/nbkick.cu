@@ -579,6 +579,8 @@ void enqueue_encounter(const Workspace &w, double *x, double *v, const double *m
     ep.gstat = gs; ep.status = w.status; ep.mu = g_cfg.G * M_star; ep.G = g_cfg.G;
     ep.dt = dt; ep.tol = g_cfg.bs_tol > 0.0 ? g_cfg.bs_tol : 1e-12; ep.kind = g_cfg.changeover_kind;
     ep.gcore = w.g_core; ep.rc_vel = rc_vel; ep.nlev = nlev;
+    ep.work = reinterpret_cast<unsigned long long *>(w.status + 16);   // two spare words of the 512-byte status head
+    cudaMemsetAsync(ep.work, 0, 2 * sizeof(unsigned long long), stream());
     long long small_blocks = N / 2 + 1;
     const long long cap_blocks = (long long)sm_count() * 8;
     if (small_blocks > cap_blocks) small_blocks = cap_blocks;
