@@ -127,7 +127,8 @@ void nb_default_config(nb_config *cfg);
  * whenever the pointers, sizes or tuning of the call differ from the cached ones). */
 int nb_configure(const nb_config *cfg);
 /* Bytes of scratch the device-pointer calls need for N bodies under the current tuning (the force
- * kernels' partial sums dominate: 24 N x slots).  The O(N) calls need only its head: nb_rcrit none,
+ * kernels' partial sums dominate: 24 N x slots, never more than slot_bytes_max: beyond it the symmetric kernel's tile
+ * grid is evaluated in bands).  The O(N) calls need only its head: nb_rcrit none,
  * nb_drift_kepler the first 512 bytes (status words), nb_shift 512 + 2 x roundup256(24 ceil(N/256)) bytes. */
 size_t nb_workspace_bytes(int64_t N);
 
