@@ -480,7 +480,7 @@ def run_trajectory(args):
     n2 = N2 if args.n2 is None else args.n2
     cap = 1 << 24
     nb.configure(N, pair_capacity=cap, n_active=na, G=G_GAUSS, n1=N1, n2=n2, resolve_encounters=args.encounters,
-                 levels=args.levels, precision=1 if args.precision == "mixed" else 0)
+                 levels=args.levels, precision=1 if args.precision == "mixed" else 0, force_kernel=args.force_kernel)
     nb.nb_status_reset()
     x = torch.from_numpy(d.x).cuda(); v = torch.from_numpy(d.v).cuda(); m = torch.from_numpy(d.m).cuda()
     acc = torch.zeros_like(x); rc = torch.zeros(N, dtype=torch.float64, device="cuda")

@@ -282,3 +282,31 @@ def test_step_host_and_kick_host_match_the_oracle():
     assert all(tuple(p) in keys for p in ps.tolist()) and len({tuple(p) for p in ps.tolist()}) == small
     assert np.array_equal(vk3, d.v)
     nb.nb_release()
+
+
+def test_step_host_through_the_newton3_kernel_banded_and_not():
+    """nb_step_host with the Newton-III kernel forced (sorted staging, tail splitting) and with the banded evaluation on top
+    (nb_config.slot_bytes_max forced down): the private arena is sized by nb_workspace_bytes for either geometry; same
+    trajectory as oracle.step, same final pair list."""
+    import paper_2604_09184_b200 as nb
+    d = nb_inputs.make_config(1, n_override=3000)
+    N, cap = d.N, 1 << 16
+    ref = oracle.step(d.x, d.v, d.m, d.M_star, d.dt, G_GAUSS, 3, n1=3.0, n2=0.4)
+    sure, border = oracle.pairs(ref["x"], ref["rcrit"])
+    npad = -(-N // 128) * 128
+    for slot_cap in (0, 24 * (N + npad) * 4 + 8):
+        x, v = d.x.copy(), d.v.copy()
+        rc = np.zeros(N); acc = np.zeros((N, 3)); pairs = np.full((cap, 2), -1, dtype=np.int32); npairs = np.zeros(1, dtype=np.int64)
+        nb.nb_release()
+        nb.configure(None, pair_capacity=cap, G=G_GAUSS, n1=3.0, n2=0.4, force_kernel=2, sym_block=128, sort_staging=1,
+                     slot_bytes_max=slot_cap)
+        nb.nb_step_host(x, v, d.m, d.M_star, d.dt, rc, acc, pairs, npairs, 3)
+        ex = np.max(np.abs(x - ref["x"])) / np.max(np.abs(ref["x"]))
+        ev = np.max(np.abs(v - ref["v"])) / np.max(np.abs(ref["v"]))
+        assert ex <= 1e-13 and ev <= 1e-13, (slot_cap, ex, ev)
+        n = int(npairs[0])
+        assert_pairs_match(pairs[:n], n, sure, border, f"nb_step_host Newton-III, slot cap {slot_cap}")
+        acc_ref, ab, _ = oracle.accel(x, d.m, rc, G_GAUSS, want_abs=True)
+        assert_acc_close(acc, acc_ref, f"nb_step_host Newton-III acc, slot cap {slot_cap}", ab)
+        assert nb.nb_status()["kepler_fail"] == 0 and nb.nb_status()["pairs_dropped"] == 0
+    nb.nb_release()
