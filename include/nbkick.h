@@ -57,7 +57,7 @@ extern "C" {
  *   NB_FORCE_SYMMETRIC  Newton's third law: every unordered pair is evaluated once and its r^-3
  *                       serves both bodies (two thirds of the fp64 instructions); fully active case
  *                       only -- with n_active < N the call falls back to NB_FORCE_TILES.
- *   NB_FORCE_AUTO       symmetric when fully active and N >= 12288, else tiles. */
+ *   NB_FORCE_AUTO       symmetric when fully active and N >= 4096, else tiles. */
 /* Arithmetic of the O(N^2) sum (PAPER.md:160 contrasts FP32 and FP64 runs):
  *   NB_PRECISION_F64    everything in fp64 (default; the north_star's 1e-12 tolerance applies)
  *   NB_PRECISION_MIXED  pairs out of reach of every critical radius: differences in fp64, r^2, r^-3 and the products

@@ -107,6 +107,8 @@ struct Geometry {
     int mixed;            // mixed-precision one-sided kernel (force_mixed.cuh)
 };
 
+constexpr int64_t kSymMinN = 4096;         // fully active N from which the Newton-III kernel is taken (measured crossover with the
+                                           // fused one-sided step: 56 vs 53 us per step at N = 4096, 127 vs 95 at N = 8192)
 constexpr int64_t kSmallStepMaxN = 8192;   // the fused small-N step (step_small.cuh) takes N up to this
 
 Geometry geometry(int64_t N, int64_t n_active) {
@@ -120,7 +122,7 @@ Geometry geometry(int64_t N, int64_t n_active) {
     // Newton-III kernel: fully active case only (a passive body exerts nothing, so there is no second
     // side to serve), and only when there are enough super-tiles to fill the machine several times.
     const bool fully_active = (g.Nj == N);
-    if (fully_active && !g.mixed && g_cfg.force_kernel != NB_FORCE_TILES && (g_cfg.force_kernel == NB_FORCE_SYMMETRIC || N >= 12288)) {
+    if (fully_active && !g.mixed && g_cfg.force_kernel != NB_FORCE_TILES && (g_cfg.force_kernel == NB_FORCE_SYMMETRIC || N >= kSymMinN)) {
         // I = 4 at 12 warps per SM (160 registers, no spills) measured fastest on B200.
         // The CTA shrinks with the super-block -- 4 warps for S >= 512, 2 for S = 256, 1 for S = 128 -- so that a
         // mid-sized problem still has many short CTAs: the tail of the grid costs about one CTA duration, whatever

@@ -100,7 +100,7 @@ def test_geometry_and_workspace(nb):
             # Newton-III kernel: fully active and large enough; super-blocks of S bodies cover N, one CTA
             # per unordered pair of super-blocks, one partial slot per super-block
             S = -g.tile_j
-            assert not n_active and N >= 12288
+            assert not n_active and N >= 4096
             # CTAs of W warps whose chunks of 32 W I bodies tile the super-block; always 12 warps per SM at I = 4
             assert S in (128, 256, 512, 1024, 2048) and S % (g.threads * g.i_per_thread) == 0
             assert g.threads == min(128, S // g.i_per_thread) or g.i_per_thread != 4

@@ -21,8 +21,9 @@ def _run(d, nsteps, use_graph, with_pairs=True, n2=0.4, **tune):
     return xg, vg, ag, rcg, gp, n, st.nb.nb_status()
 
 
-@pytest.mark.parametrize("cfg,n_override,tune", [(0, 300, {}), (0, 2048, {}), (1, 5000, {}), (3, 4096, {}), (2, 8192, dict(i_per_thread=2)),
-                                                 (0, 1000, dict(i_per_thread=4, j_splits=2))])
+@pytest.mark.parametrize("cfg,n_override,tune", [(0, 300, {}), (0, 2048, {}), (1, 5000, dict(force_kernel=1)), (3, 4096, {}),
+                                                 (2, 8192, dict(i_per_thread=2, force_kernel=1)),    # one-sided kernel kept above the
+                                                 (0, 1000, dict(i_per_thread=4, j_splits=2))])      # Newton-III threshold (N >= 4096)
 @pytest.mark.parametrize("nsteps", [1, 2, 9])
 def test_fused_small_step_is_the_multi_launch_step_bit_for_bit(cfg, n_override, tune, nsteps):
     d = nb_inputs.make_config(cfg, n_override=n_override)

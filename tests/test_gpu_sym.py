@@ -164,10 +164,10 @@ def test_sym_everything_in_the_exact_path_at_larger_n():
 
 def test_auto_selection_threshold():
     import paper_2604_09184_b200 as nb
-    for N, want_sym in ((12287, False), (12288, True)):
+    for N, want_sym in ((4095, False), (4096, True)):
         nb.configure(N, G=G_GAUSS)
         assert (nb.force_geometry(N).tile_j < 0) == want_sym
-    d = nb_inputs.make_config(1, n_override=12300)       # just above the threshold, ragged: N = 12302
+    d = nb_inputs.make_config(1, n_override=4100)        # just above the threshold, ragged: N = 4102
     rc = oracle.rcrit(d.x, d.v, d.m, d.M_star, d.dt, G_GAUSS, 3.0, 0.4)
     rows = np.unique(np.concatenate([np.arange(0, d.N, 97), [d.N - 1, d.N - 2]]))
     st = GpuState(d.x, d.v, d.m, d.M_star, G=G_GAUSS, pair_capacity=1 << 20)
@@ -175,10 +175,10 @@ def test_auto_selection_threshold():
     st.set_rcrit(rc)
     st.kick(0.0)
     acc_ref, ab, _ = oracle.accel(d.x, d.m, rc, G_GAUSS, rows=rows, want_abs=True)
-    assert_acc_close(st.acc.cpu().numpy()[rows], acc_ref, "auto sym N=12302 sampled rows", ab)
+    assert_acc_close(st.acc.cpu().numpy()[rows], acc_ref, "auto sym N=4102 sampled rows", ab)
     sure, border = oracle.pairs(d.x, rc)
     gp, n = st.get_pairs()
-    assert_pairs_match(gp, n, sure, border, "auto sym N=12302")
+    assert_pairs_match(gp, n, sure, border, "auto sym N=4102")
 
 
 @pytest.mark.parametrize("seed", range(16))
