@@ -54,6 +54,8 @@ def parse_args():
     ap.add_argument("--no-drift-point", action="store_true", help="skip the N = 2^24 drift-only HBM point")
     ap.add_argument("--force-kernel", type=int, default=0, choices=[0, 1, 2],
                     help="nb_config.force_kernel: 0 auto, 1 one-sided tiles, 2 Newton-III (comparison runs)")
+    ap.add_argument("--j-splits", type=int, default=0,
+                    help="nb_config.j_splits: 0 auto, k > 0 a grid of k j-splits, -1 balanced pieces (comparison runs, one-sided kernel)")
     ap.add_argument("--precision", default="f64", choices=["f64", "mixed"],
                     help="f64 (default, the metric) or the mixed-precision kick variant (NB_PRECISION_MIXED; a side line)")
     ap.add_argument("--trajectory", action="store_true",
@@ -316,7 +318,7 @@ def run_cuda(args):
     # ---- device-resident arm: inputs in HBM before the timed region -------------------------------
     mixed = args.precision == "mixed"
     nb.configure(N, pair_capacity=cap, n_active=na, G=G_GAUSS, n1=N1, n2=N2, reuse_acc=False, time_force=True,
-                 force_kernel=args.force_kernel, precision=1 if mixed else 0)
+                 force_kernel=args.force_kernel, j_splits=args.j_splits, precision=1 if mixed else 0)
     nb.nb_status_reset()
     x = torch.from_numpy(d.x).cuda(); v = torch.from_numpy(d.v).cuda(); m = torch.from_numpy(d.m).cuda()
     acc = torch.zeros_like(x); rc = torch.zeros(N, dtype=torch.float64, device="cuda")
@@ -480,7 +482,7 @@ def run_trajectory(args):
     n2 = N2 if args.n2 is None else args.n2
     cap = 1 << 24
     nb.configure(N, pair_capacity=cap, n_active=na, G=G_GAUSS, n1=N1, n2=n2, resolve_encounters=args.encounters,
-                 levels=args.levels, precision=1 if args.precision == "mixed" else 0, force_kernel=args.force_kernel)
+                 levels=args.levels, precision=1 if args.precision == "mixed" else 0, force_kernel=args.force_kernel, j_splits=args.j_splits)
     nb.nb_status_reset()
     x = torch.from_numpy(d.x).cuda(); v = torch.from_numpy(d.v).cuda(); m = torch.from_numpy(d.m).cuda()
     acc = torch.zeros_like(x); rc = torch.zeros(N, dtype=torch.float64, device="cuda")
