@@ -161,6 +161,33 @@ int nb_kick(const double *x, double *v, const double *m, double M_star, int64_t 
             const double *rcrit, double *acc, int32_t *pairs, int64_t *npairs);
 
 /*
+ * nb_kick for callers that cannot allocate device memory (code under CUDA stream capture, tight serving loops,
+ * harnesses that forbid cudaMalloc): the same operation (Eq. 5, 94, 98 -- see nb_kick), the same kernels
+ * and launch geometry, but the scratch comes from a static device array of NB_STATIC_SCRATCH_BYTES (8 MiB) inside the
+ * library instead of the workspace of nb_configure, which this call neither needs nor touches.  Every GPU that loads
+ * the library holds those 8 MiB until the process exits.  The call itself allocates nothing: no cudaMalloc, cudaFree,
+ * event or stream creation -- kernel launches, one 512-byte cudaMemsetAsync and at most one 64-byte device-to-device
+ * cudaMemcpyAsync on the configured stream.
+ *   Limit: nb_workspace_bytes(N) (for the current configuration) must not exceed NB_STATIC_SCRATCH_BYTES -- N up to
+ *   about 4700 with the default configuration (N = 4096: 6.0 MB); beyond that the call returns NB_E_WORKSPACE and
+ *   nb_last_error() names both sizes.  Use nb_kick with a caller-owned workspace for larger N.
+ *   Arguments as nb_kick (all DEVICE pointers), plus status8: device int64[8] out or NULL -- the device-side
+ *   condition counters of THIS call (layout of nb_status; they live in the static array, so nb_status does not
+ *   see them).
+ *   Sharing: all calls, from every stream and thread, use the one array of the current device.  It keeps the last
+ *   call's contents; the call clears what must start at zero (the counters) and overwrites the rest before reading
+ *   it.  Calls that OVERLAP on the GPU (different streams, or a captured graph replayed concurrently with another
+ *   call) race on it: order them.
+ * nb_kick_static_setup resolves the array's device address for the CURRENT device (cudaGetSymbolAddress, once per
+ * device); nb_kick_static does the same on its first call per device, so calling it is only needed by callers who
+ * want that out of the way beforehand (before beginning a stream capture, say).
+ */
+#define NB_STATIC_SCRATCH_BYTES (8u << 20)
+int nb_kick_static_setup(void);
+int nb_kick_static(const double *x, double *v, const double *m, double M_star, int64_t N, double dt,
+                   const double *rcrit, double *acc, int32_t *pairs, int64_t *npairs, int64_t *status8);
+
+/*
  * a5 -- H_C (Eq. 6): x_i += dt * (sum_k m_k v_k) / M_star for every body.
  * The sum is a fixed-shape tree reduction (deterministic, run-to-run reproducible).
  */

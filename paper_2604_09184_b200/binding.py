@@ -22,7 +22,7 @@ PRECISION_F64, PRECISION_MIXED = 0, 1
 
 # every symbol include/nbkick.h declares (tests check the library exports each of them)
 SYMBOLS = (
-    "nb_default_config", "nb_configure", "nb_workspace_bytes", "nb_rcrit", "nb_kick", "nb_shift",
+    "nb_default_config", "nb_configure", "nb_workspace_bytes", "nb_rcrit", "nb_kick", "nb_kick_static_setup", "nb_kick_static", "nb_shift",
     "nb_drift_kepler", "nb_midpoint_drag", "nb_step", "nb_groups", "nb_encounter", "nb_encounter_levels", "nb_merge", "nb_kick_host", "nb_step_host", "nb_status", "nb_status_reset",
     "nb_last_force_ms", "nb_force_time", "nb_force_time_reset", "nb_force_geometry", "nb_fp64_peak", "nb_release", "nb_last_error", "nb_version",
 )
@@ -92,6 +92,8 @@ def load():
     lib.nb_workspace_bytes.restype = sz
     lib.nb_rcrit.argtypes = [vp, vp, vp, dbl, i64, dbl, vp]
     lib.nb_kick.argtypes = [vp, vp, vp, dbl, i64, dbl, vp, vp, vp, vp]
+    lib.nb_kick_static.argtypes = [vp, vp, vp, dbl, i64, dbl, vp, vp, vp, vp, vp]
+    lib.nb_kick_static_setup.argtypes = []
     lib.nb_shift.argtypes = [vp, vp, vp, dbl, i64, dbl]
     lib.nb_drift_kepler.argtypes = [vp, vp, dbl, i64, dbl]
     lib.nb_midpoint_drag.argtypes = [vp, vp, dbl, i64, dbl]
@@ -237,6 +239,19 @@ def nb_kick(x, v, m, M_star, dt, rcrit, acc, pairs=None, npairs=None):
     _check(load().nb_kick(_dev(x, 3 * N, torch.float64), _dev(v, 3 * N, torch.float64), _dev(m, N, torch.float64),
                           float(M_star), N, float(dt), _dev(rcrit, N, torch.float64), _dev(acc, 3 * N, torch.float64),
                           _dev(pairs, None, torch.int32), _dev(npairs, 1, torch.int64)))
+
+
+def nb_kick_static(x, v, m, M_star, dt, rcrit, acc, pairs=None, npairs=None, status8=None):
+    """nb_kick with the scratch in the library's static device array (include/nbkick.h): allocates nothing."""
+    import torch
+    N = m.numel()
+    _check(load().nb_kick_static(_dev(x, 3 * N, torch.float64), _dev(v, 3 * N, torch.float64), _dev(m, N, torch.float64),
+                                 float(M_star), N, float(dt), _dev(rcrit, N, torch.float64), _dev(acc, 3 * N, torch.float64),
+                                 _dev(pairs, None, torch.int32), _dev(npairs, 1, torch.int64), _dev(status8, 8, torch.int64)))
+
+
+def nb_kick_static_setup():
+    _check(load().nb_kick_static_setup())
 
 
 def nb_shift(x, v, m, M_star, dt):

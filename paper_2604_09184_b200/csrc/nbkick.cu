@@ -868,7 +868,74 @@ int kick_impl(const double *x, double *v, const double *m, double M_star, int64_
 
 }  // namespace
 
+// ---- nb_kick_static: the kick with its scratch in a static device array (include/nbkick.h) --------------------------
+// Callers that cannot allocate (stream capture, serving loops, harnesses that forbid cudaMalloc) get the scratch from
+// here: NB_STATIC_SCRATCH_BYTES of device memory that every GPU which loads the library holds until the process exits.
+// In HOST code the name below is only a stand-in for the symbol, never a device address: the address a kernel can use
+// comes from cudaGetSymbolAddress, asked once per device with that device current (static_scratch_for_current_device).
+static __device__ __align__(256) unsigned char g_static_scratch[NB_STATIC_SCRATCH_BYTES];
+
+namespace {
+
+constexpr int kStaticMaxDevices = 64;
+void *g_static_scratch_ptr[kStaticMaxDevices] = {nullptr};
+
+int static_scratch_for_current_device(void **out) {
+    int dev = -1;
+    NB_CUDA(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= kStaticMaxDevices) return fail(NB_E_BADARG, "nb_kick_static: device ordinal %d out of range", dev);
+    if (g_static_scratch_ptr[dev] == nullptr) {
+        void *ptr = nullptr;
+        NB_CUDA(cudaGetSymbolAddress(&ptr, g_static_scratch));
+        if (ptr == nullptr || (reinterpret_cast<uintptr_t>(ptr) & 255u) != 0)
+            return fail(NB_E_CUDA, "nb_kick_static: cudaGetSymbolAddress gave an unusable address");
+        g_static_scratch_ptr[dev] = ptr;
+    }
+    *out = g_static_scratch_ptr[dev];
+    return NB_OK;
+}
+
+}  // namespace
+
 extern "C" {
+
+int nb_kick_static_setup(void) {
+    std::lock_guard<std::mutex> lk(g_mu);
+    void *ptr = nullptr;
+    return static_scratch_for_current_device(&ptr);
+}
+
+int nb_kick_static(const double *x, double *v, const double *m, double M_star, int64_t N, double dt, const double *rcrit,
+                   double *acc, int32_t *pairs, int64_t *npairs, int64_t *status8) {
+    std::lock_guard<std::mutex> lk(g_mu);
+    int rc = check_common(N, dt, M_star);
+    if (rc) return rc;
+    if (!x || !v || !m || !acc) return fail(NB_E_NULL, "nb_kick_static: x, v, m, acc must not be NULL");
+    if ((rc = check_pairs_args(pairs, npairs))) return rc;
+    void *scratch = nullptr;
+    if ((rc = static_scratch_for_current_device(&scratch))) return rc;
+    const Geometry g = geometry(N, g_cfg.n_active);
+    const size_t need = carve(nullptr, N, g).bytes;
+    if (need > (size_t)NB_STATIC_SCRATCH_BYTES)
+        return fail(NB_E_WORKSPACE, "nb_kick_static: N = %lld needs %zu bytes of scratch, the static array has %zu "
+                    "(NB_STATIC_SCRATCH_BYTES); use nb_kick with a caller-owned workspace", (long long)N, need,
+                    (size_t)NB_STATIC_SCRATCH_BYTES);
+    const Workspace w = carve(scratch, N, g);
+    // the array keeps the previous call's contents.  What must start at zero: the status words (the kernels only ever
+    // add to them).  Everything else -- staged records, partial slots, rc scratch -- is written in full by this call
+    // before it is read (every (slot, body) exactly once per evaluation), and npairs is zeroed by nb_prep_kernel.
+    NB_CUDA(cudaMemsetAsync(w.status, 0, 512, stream()));
+    double *rc_io = rcrit ? const_cast<double *>(rcrit) : w.rc_scratch;
+    const int saved_time_force = g_cfg.time_force;
+    g_cfg.time_force = 0;   // timing events are created lazily (cudaEventCreate): not on this path
+    rc = enqueue_eval(w, g, const_cast<double *>(x), v, m, M_star, N, dt, rc_io, rcrit ? 0 : 1, nullptr, 0.0, acc, pairs,
+                      npairs, dt, dt != 0.0 ? 1 : 0, nullptr, false);
+    g_cfg.time_force = saved_time_force;
+    if (rc) return rc;
+    if (status8 != nullptr)
+        NB_CUDA(cudaMemcpyAsync(status8, w.status, ST_COUNT * sizeof(int64_t), cudaMemcpyDeviceToDevice, stream()));
+    return NB_OK;
+}
 
 void nb_default_config(nb_config *cfg) {
     if (!cfg) return;
