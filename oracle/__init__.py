@@ -59,6 +59,7 @@ def _L():
         lib.oracle_step.argtypes = [dp, dp, dp, dbl, i64, i64, dbl, dbl, dbl, dbl, i32, dp, dp, i64]
         lib.oracle_diagnostics.argtypes = [dp, dp, dp, dbl, i64, dbl, dp]
         lib.oracle_encounter.argtypes = [dp, dp, dp, dp, i64, i64, dbl, dbl, dbl, i32, dbl, ip, ip, i64, i64, lp]
+        lib.oracle_encounter_collide.argtypes = [dp, dp, dp, dp, dp, i64, i64, dbl, dbl, dbl, i32, dbl, dbl, ip, ip, i64, i64, ip, lp]
         lib.oracle_encounter_split.argtypes = [dp, dp, dp, dp, i64, i64, dbl, dbl, dbl, i32, dbl, ip, ip, i64, i64, i64, lp]
         lib.oracle_midpoint_drag.restype = i64
         lib.oracle_midpoint_drag.argtypes = [dp, dp, i64, dbl, dbl, dbl, i32, dbl, dbl, i64, lp]
@@ -276,13 +277,17 @@ def encounter_rhs(x, v, gm, rc, mu, kind=0):
     return f[:3 * n].reshape(n, 3), f[3 * n:].reshape(n, 3)
 
 
-def encounter(x, v, m, rcrit_, M_star, dt, G, grp, kind=0, tol=1e-12, max_group=1024, n_active=0, split_max_core=-1):
+def encounter(x, v, m, rcrit_, M_star, dt, G, grp, kind=0, tol=1e-12, max_group=1024, n_active=0, split_max_core=-1,
+              radius=None, radius_factor=1.0, absorbed_by=None):
     """H_A with encounters (Eq. 4, 98, 106): the members of every group of `grp` (a dict from
     groups()) are advanced by dt with the Bulirsch-Stoer integrator; returns (x, v, stats) with
     stats = dict(integrated, skipped, failed, steps).  Semi-active mode (0 < n_active < N, reading S22): every
     group that has test particles is split into its active core and independent {core + particle} problems;
     split_max_core >= 0 restricts the splitting to cores of at most that many members (what an implementation
-    with a bounded core size does; the tests pass the CUDA path's bound)."""
+    with a bounded core size does; the tests pass the CUDA path's bound).
+    radius given (fully active case): collisions are examined inside the solver after every accepted step and the
+    colliding members merged at once (reading S26); stats then also holds m, radius (new arrays),
+    absorbed_by (int32[N]: the body an absorbed body sits on, -1 otherwise; continues the array passed in) and absorbed."""
     x = np.array(x, dtype=np.float64, order="C"); v = np.array(v, dtype=np.float64, order="C")
     m = np.ascontiguousarray(m, dtype=np.float64)
     N = m.shape[0]
@@ -290,8 +295,19 @@ def encounter(x, v, m, rcrit_, M_star, dt, G, grp, kind=0, tol=1e-12, max_group=
     nlev = rc.shape[0]
     members = np.ascontiguousarray(grp["members"], dtype=np.int32)
     gstart = np.ascontiguousarray(grp["gstart"], dtype=np.int32)
-    stats = np.zeros(4, dtype=np.int64)
+    stats = np.zeros(5, dtype=np.int64)
     dp, ip, lp = C.POINTER(C.c_double), C.POINTER(C.c_int32), C.POINTER(C.c_int64)
+    if radius is not None:
+        if 0 < int(n_active) < N:
+            raise ValueError("collisions inside the solver are defined for the fully active case (reading S26)")
+        m2 = np.array(m, dtype=np.float64); R2 = np.array(radius, dtype=np.float64)
+        ab = np.full(N, -1, dtype=np.int32) if absorbed_by is None else np.array(absorbed_by, dtype=np.int32)
+        _L().oracle_encounter_collide(x.ctypes.data_as(dp), v.ctypes.data_as(dp), m2.ctypes.data_as(dp), R2.ctypes.data_as(dp),
+                                      rc.ctypes.data_as(dp), nlev, N, float(M_star), float(G), float(dt), int(kind), float(tol),
+                                      float(radius_factor), members.ctypes.data_as(ip), gstart.ctypes.data_as(ip),
+                                      int(grp["ngroups"]), int(max_group), ab.ctypes.data_as(ip), stats.ctypes.data_as(lp))
+        return x, v, dict(integrated=int(stats[0]), skipped=int(stats[1]), failed=int(stats[2]), steps=int(stats[3]),
+                          absorbed=int(stats[4]), m=m2, radius=R2, absorbed_by=ab)
     if 0 < int(n_active) < N:
         if nlev != 1:
             raise ValueError("the multi-level scheme is defined for the fully active case only")
@@ -307,17 +323,22 @@ def encounter(x, v, m, rcrit_, M_star, dt, G, grp, kind=0, tol=1e-12, max_group=
     return x, v, dict(integrated=int(stats[0]), skipped=int(stats[1]), failed=int(stats[2]), steps=int(stats[3]))
 
 
-def step_enc(x, v, m, M_star, dt, G, nsteps, n1=3.0, n2=0.4, kind=0, tol=1e-12, max_group=1024, n_active=0, split_max_core=-1):
+def step_enc(x, v, m, M_star, dt, G, nsteps, n1=3.0, n2=0.4, kind=0, tol=1e-12, max_group=1024, n_active=0, split_max_core=-1,
+             radius=None, radius_factor=1.0):
     """nsteps of B(dt/2) C(dt/2) A(dt) C(dt/2) B(dt/2) with close encounters resolved:
     in A the members of the encounter groups of the step's opening pair list (groups of at most max_group
     bodies) are propagated by encounter(), every other body by the Kepler drift.  Composed of the pinned
     pieces above; rcrit is recomputed before every force evaluation (S17) and held through the step.  With
     n_active (semi-active mode) only the first n_active bodies exert force and every pair has an active member.
-    Returns dict(x, v, acc, rcrit, pairs, stats)."""
+    radius given: collisions inside the solver (reading S26) -- m and radius change from step to step (an absorbed body
+    stays in the arrays with m = 0, R = 0 on top of its survivor until merge() compacts them) and are returned too.
+    Returns dict(x, v, acc, rcrit, pairs, stats [, m, radius, absorbed_by])."""
     x = np.array(x, dtype=np.float64, order="C"); v = np.array(v, dtype=np.float64, order="C")
-    m = np.ascontiguousarray(m, dtype=np.float64)
+    m = np.array(m, dtype=np.float64)
     N = m.shape[0]
-    tot = dict(integrated=0, skipped=0, failed=0, steps=0, border=0)
+    tot = dict(integrated=0, skipped=0, failed=0, steps=0, border=0, absorbed=0)
+    R = None if radius is None else np.array(radius, dtype=np.float64)
+    ab = np.full(N, -1, dtype=np.int32)
 
     def evaluate(x, v):
         rc = rcrit(x, v, m, M_star, dt, G, n1, n2)
@@ -333,7 +354,10 @@ def step_enc(x, v, m, M_star, dt, G, nsteps, n1=3.0, n2=0.4, kind=0, tol=1e-12, 
         grp = groups(pr, N)
         xk, vk, nfail = drift_kepler(x, v, M_star, dt, G)
         xe, ve, st = encounter(x, v, m, rc, M_star, dt, G, grp, kind=kind, tol=tol, max_group=max_group, n_active=n_active,
-                               split_max_core=split_max_core)
+                               split_max_core=split_max_core, radius=R, radius_factor=radius_factor, absorbed_by=ab)
+        if R is not None:
+            m, R, ab = st["m"], st["radius"], st["absorbed_by"]
+            tot["absorbed"] += st["absorbed"]
         moved = np.zeros(N, dtype=bool)
         for g in range(grp["ngroups"]):
             seg = grp["members"][grp["gstart"][g]:grp["gstart"][g + 1]]
@@ -351,7 +375,10 @@ def step_enc(x, v, m, M_star, dt, G, nsteps, n1=3.0, n2=0.4, kind=0, tol=1e-12, 
         x = shift(x, v, m, M_star, 0.5 * dt)
         rc, acc, pr = evaluate(x, v)
         v = v + (0.5 * dt) * acc
-    return dict(x=x, v=v, acc=acc, rcrit=rc, pairs=pr, stats=tot)
+    out = dict(x=x, v=v, acc=acc, rcrit=rc, pairs=pr, stats=tot)
+    if R is not None:
+        out.update(m=m, radius=R, absorbed_by=ab)
+    return out
 
 
 # ---------------------------------------------------------------------------------------------------------------------

@@ -12,6 +12,7 @@
  *   - step  B(dt/2) C(dt/2) A(dt) C(dt/2) B(dt/2)           PAPER.md:80 Eq. 3 (order: S6, S17)
  *   - diagnostics E, L               PAPER.md:84-92 Eq. 4-6 (K terms cancel in H_A + H_B)
  *   - independent encounter groups   PAPER.md:106           (connected components of the pair graph)
+ *   - collisions inside the direct solver  PAPER.md:98, 130, 168  (reading S26; "parity unpinned" against the paper)
  *
  * It is the definition written out: explicit loops in the paper's index order, no blocking,
  * no fusion, no FMA contraction (build with -ffp-contract=off).  All inputs and outputs are
@@ -621,8 +622,83 @@ void oracle_encounter_rhs(const double *y, int n, const double *gm, const double
 
 #define BS_COLS 8
 
+/* Collisions inside the direct solver ("N-body simulations often treat collisions as perfect mergers";
+ * PAPER.md:168 radii inflated by a constant factor f; PAPER.md:98 the solver "propagates the involved bodies through the
+ * close encounter phase" -- which is where bodies touch).  DESIGN.md reading S26: after every ACCEPTED Bulirsch-Stoer step
+ * the members are tested pairwise for contact, r_ij < f (R_i + R_j) (strict, fp64 on r^2 = (dx^2 + dy^2) + dz^2, the test
+ * of reading S21); members linked by a chain of contacts merge at once by the rule of S21 -- into the one with the
+ * smallest index: m <- sum m_k, x <- sum m_k x_k / sum m_k, v <- sum m_k v_k / sum m_k (index order, unfused),
+ * R <- cbrt(sum R_k^3).  The survivor goes on with the group (its critical radius is held, like every rc, through the
+ * step); an absorbed member keeps m = 0, R = 0 (it exerts nothing and is never tested again), is put on the survivor and
+ * carried along as a massless member; when the group's integration ends it is put on the body that holds it then (x, v
+ * equal), so that the perfect merging at the step boundary (oracle.merge / nb_merge) removes it when the arrays are
+ * compacted.  into[k] = member that absorbed member k (-1: none).  Returns the number of members absorbed by this test. */
+static int group_collide(double *y, int n, double *mm, double *gm, double *rad, double G, double f, int32_t *into) {
+    double *x = y, *v = y + 3 * n;
+    int *parent = (int *)malloc(sizeof(int) * (size_t)n);
+    int nabs = 0, any = 0;
+    for (int i = 0; i < n; ++i) parent[i] = i;
+    for (int i = 0; i < n; ++i) {
+        if (into[i] >= 0 || (mm[i] == 0.0 && rad[i] == 0.0)) continue;
+        for (int j = i + 1; j < n; ++j) {
+            if (into[j] >= 0 || (mm[j] == 0.0 && rad[j] == 0.0)) continue;
+            double dx = x[3 * j] - x[3 * i], dy = x[3 * j + 1] - x[3 * i + 1], dz = x[3 * j + 2] - x[3 * i + 2];
+            double r2 = (dx * dx + dy * dy) + dz * dz;
+            double sr = f * (rad[i] + rad[j]);
+            if (r2 < sr * sr) {
+                int a = i, b = j;
+                while (parent[a] != a) a = parent[a];
+                while (parent[b] != b) b = parent[b];
+                if (a < b) parent[b] = a; else if (b < a) parent[a] = b;   /* the smaller index is the root */
+                any = 1;
+            }
+        }
+    }
+    if (any) {
+        for (int s0 = 0; s0 < n; ++s0) {
+            if (parent[s0] != s0) continue;
+            double mt = 0.0, mx[3] = {0, 0, 0}, mv[3] = {0, 0, 0}, vol = 0.0;
+            int cnt = 0;
+            for (int k = s0; k < n; ++k) {                      /* members of the cluster in index order */
+                int r = k;
+                while (parent[r] != r) r = parent[r];
+                if (r != s0) continue;
+                mt = mt + mm[k];
+                for (int c = 0; c < 3; ++c) { mx[c] = mx[c] + mm[k] * x[3 * k + c]; mv[c] = mv[c] + mm[k] * v[3 * k + c]; }
+                vol = vol + rad[k] * rad[k] * rad[k];
+                ++cnt;
+            }
+            if (cnt < 2) continue;
+            if (mt > 0.0)
+                for (int c = 0; c < 3; ++c) { x[3 * s0 + c] = mx[c] / mt; v[3 * s0 + c] = mv[c] / mt; }
+            mm[s0] = mt; gm[s0] = G * mt; rad[s0] = cbrt(vol);
+            for (int k = s0 + 1; k < n; ++k) {
+                int r = k;
+                while (parent[r] != r) r = parent[r];
+                if (r != s0) continue;
+                mm[k] = 0.0; gm[k] = 0.0; rad[k] = 0.0; into[k] = s0; ++nabs;
+                for (int c = 0; c < 3; ++c) { x[3 * k + c] = x[3 * s0 + c]; v[3 * k + c] = v[3 * s0 + c]; }
+            }
+        }
+    }
+    free(parent);
+    return nabs;
+}
+
+static int64_t encounter_group_core(double *y, int n, double *gm, const double *rc, int nlev, double mu, int kind,
+                                    double dt, double tol, double *mm, double *rad, double G, double frad, int32_t *into,
+                                    int64_t *absorbed);
+
 int64_t oracle_encounter_group(double *y, int n, const double *gm, const double *rc, int nlev, double mu, int kind,
                                double dt, double tol) {
+    /* without radii: gm is only read */
+    return encounter_group_core(y, n, (double *)gm, rc, nlev, mu, kind, dt, tol, NULL, NULL, 0.0, 0.0, NULL, NULL);
+}
+
+/* mm != NULL: collisions on (reading S26); mm, gm, rad [n] in/out, into [n] out */
+static int64_t encounter_group_core(double *y, int n, double *gm, const double *rc, int nlev, double mu, int kind,
+                                    double dt, double tol, double *mm, double *rad, double G, double frad, int32_t *into,
+                                    int64_t *absorbed) {
     const int dim = 6 * n;
     double *buf = (double *)malloc(sizeof(double) * (size_t)dim * (5 + BS_COLS));
     double *f = buf, *ym = buf + dim, *yn = buf + 2 * dim, *tmp = buf + 3 * dim, *f0 = buf + 4 * dim;
@@ -679,9 +755,19 @@ int64_t oracle_encounter_group(double *y, int n, const double *gm, const double 
             for (int k = 0; k < dim; ++k) y[k] = T[(cols - 1) * dim + k];
             t = (fabs(dt - (t + h)) <= 1e-15 * fabs(dt)) ? dt : t + h;
             steps++;
+            if (mm != NULL) *absorbed += group_collide(y, n, mm, gm, rad, G, frad, into);
             if (cols <= 6) h *= 1.3; else if (cols == 8) h *= 0.55;
         } else {
             h *= 0.5;
+        }
+    }
+    if (mm != NULL) {
+        /* absorbed members end on the body that holds them now (a survivor may have been absorbed later itself) */
+        for (int k = 0; k < n; ++k) {
+            if (into[k] < 0) continue;
+            int s0 = into[k];
+            while (into[s0] >= 0) s0 = into[s0];
+            for (int c = 0; c < 3; ++c) { y[3 * k + c] = y[3 * s0 + c]; y[3 * n + 3 * k + c] = y[3 * n + 3 * s0 + c]; }
         }
     }
     free(buf);
@@ -717,6 +803,43 @@ void oracle_encounter(double *x, double *v, const double *m, const double *rcrit
         }
         stats[0]++; stats[3] += st;
         free(y);
+    }
+}
+
+/* oracle_encounter with collisions examined inside the solver (reading S26, group_collide above; fully active case):
+ * m, radius [N] in/out, absorbed_by [N] out (body that holds an absorbed body at the end of the call, -1 for everybody
+ * else; entries of earlier calls are kept).  stats[4] = bodies absorbed. */
+void oracle_encounter_collide(double *x, double *v, double *m, double *radius, const double *rcrit, int64_t nlev, int64_t N,
+                              double M_star, double G, double dt, int kind, double tol, double f, const int32_t *members,
+                              const int32_t *gstart, int64_t ngroups, int64_t max_group, int32_t *absorbed_by, int64_t *stats) {
+    stats[0] = stats[1] = stats[2] = stats[3] = stats[4] = 0;
+    for (int64_t g = 0; g < ngroups; ++g) {
+        const int n = gstart[g + 1] - gstart[g];
+        if (n > max_group) { stats[1]++; continue; }
+        double *y = (double *)malloc(sizeof(double) * (size_t)((9 + nlev) * n));
+        double *gm = y + 6 * n, *mm = y + 7 * n, *rad = y + 8 * n, *rc = y + 9 * n;
+        int32_t *into = (int32_t *)malloc(sizeof(int32_t) * (size_t)n);
+        for (int k = 0; k < n; ++k) {
+            const int32_t b = members[gstart[g] + k];
+            for (int c = 0; c < 3; ++c) { y[3 * k + c] = x[3 * (int64_t)b + c]; y[3 * n + 3 * k + c] = v[3 * (int64_t)b + c]; }
+            mm[k] = m[b]; gm[k] = G * m[b]; rad[k] = radius[b]; into[k] = -1;
+            for (int64_t l = 0; l < nlev; ++l) rc[l * n + k] = rcrit[l * N + b];
+        }
+        int64_t nabs = 0;
+        const int64_t st = encounter_group_core(y, n, gm, rc, (int)nlev, G * M_star, kind, dt, tol, mm, rad, G, f, into, &nabs);
+        if (st < 0) { stats[2]++; free(y); free(into); continue; }   /* step size underflow: the group is left unchanged */
+        for (int k = 0; k < n; ++k) {
+            const int32_t b = members[gstart[g] + k];
+            for (int c = 0; c < 3; ++c) { x[3 * (int64_t)b + c] = y[3 * k + c]; v[3 * (int64_t)b + c] = y[3 * n + 3 * k + c]; }
+            m[b] = mm[k]; radius[b] = rad[k];
+            if (into[k] >= 0) {
+                int s0 = into[k];
+                while (into[s0] >= 0) s0 = into[s0];
+                absorbed_by[b] = members[gstart[g] + s0];
+            }
+        }
+        stats[0]++; stats[3] += st; stats[4] += nabs;
+        free(y); free(into);
     }
 }
 
