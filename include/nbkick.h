@@ -271,6 +271,28 @@ int nb_encounter(double *x, double *v, const double *m, const double *rcrit, dou
                  double dt, const int32_t *members, const int32_t *gstart, const int64_t *gstat);
 
 /*
+ * nb_encounter with collisions examined INSIDE the direct solver (the solver "propagates the involved
+ * bodies through the close encounter phase" -- which is where bodies touch; PAPER.md:130 perfect mergers
+ * radii inflated by radius_factor; reading S26).  After every ACCEPTED Bulirsch-Stoer step of a group its
+ * members are tested pairwise for contact, r_ij < f (R_i + R_j) (strict, fp64 on r^2, the test of nb_merge); members
+ * linked by a chain of contacts merge at once by the rule of nb_merge -- into the one with the smallest index:
+ * m <- sum m_k, x <- sum m_k x_k / sum m_k, v likewise (index order), R <- cbrt(sum R_k^3).  The survivor goes on
+ * with the group (critical radii are held through the step); an absorbed body gets m = 0, R = 0, is never tested
+ * again and takes no part in the encounter any more -- it exerts nothing and feels only the star (left to feel the
+ * pair terms it would be a massless particle at zero distance from its survivor: a singular encounter) -- and ends the
+ * call ON the body that holds it (same x, v), so that nb_merge at the step boundary removes it when it compacts the
+ * arrays (or the caller does, from absorbed_by).
+ *   x, v [N,3] in/out; m, radius [N] in/out; rcrit [N] in; members / gstart / gstat as nb_encounter;
+ *   absorbed_by [N] int32 in/out: -1, or for an absorbed body the body that holds it.  Initialise with -1; a body
+ *   marked by an earlier call (and not yet removed from the arrays) stays out of the encounter in the same way and
+ *   follows its holder.  Entries of bodies that are not absorbed are not written.  Absorbed bodies are counted in nb_status[7].  Fully active case only
+ *   (NB_E_BADARG with 0 < n_active < N).  A group whose step size underflows is left unchanged, merges included.
+ */
+int nb_encounter_collide(double *x, double *v, double *m, double *radius, const double *rcrit, double M_star, int64_t N,
+                         double dt, const int32_t *members, const int32_t *gstart, const int64_t *gstat,
+                         int32_t *absorbed_by);
+
+/*
  * Multi-level changeover ("introducing higher-level changeover functions ... to not switch from the
  * symplectic integrator directly to the direct integrator but to introduce intermediate phases, where the symplectic
  * integrator reduces the time step level by level for the affected bodies.  Only the last level is then performed with
@@ -326,7 +348,7 @@ int nb_step_host(double *x, double *v, const double *m, double M_star, int64_t N
 
 /*
  * Lazy device-side conditions accumulated since the last nb_status_reset; synchronises the
- * stream.  flags (host int64[8]; [7] is reserved):
+ * stream.  flags (host int64[8]):
  *   [0] pairs dropped because the list was full (sum over evaluations)
  *   [1] Kepler solver non-convergences (body left unchanged)
  *   [2] non-finite positions / masses / radii seen while staging j-bodies; invalid rows of a pair list
@@ -334,6 +356,7 @@ int nb_step_host(double *x, double *v, const double *m, double M_star, int64_t N
  *   [4] encounter groups larger than NB_MAX_GROUP, left to the Kepler drift
  *   [5] encounter groups whose Bulirsch-Stoer step size underflowed (left unchanged)
  *   [6] bodies whose implicit-midpoint iteration (Eq. 8) did not converge
+ *   [7] bodies absorbed by a collision inside the direct solver (nb_encounter_collide)
  */
 int nb_status(int64_t *flags);
 int nb_status_reset(void);

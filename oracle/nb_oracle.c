@@ -588,14 +588,15 @@ static double one_minus_changeover(double r, double rc, int kind) {
 /* y = (x[3n], v[3n]) -> f = (v, a).  rc holds nlev critical radii per member, level-major (rc[k*n + i]); the pair
  * term carries the product over the levels k = 0 .. nlev-1 of [1 - W(r; rc_k,ij)]: nlev = 1 is Eq. 4 as printed, nlev > 1
  * is the innermost Hamiltonian of the multi-level scheme (oracle_level_kick below). */
-static void group_rhs(const double *y, double *f, int n, const double *gm, const double *rc, int nlev, double mu, int kind) {
+static void group_rhs(const double *y, double *f, int n, const double *gm, const double *rc, int nlev, double mu, int kind,
+                      const int32_t *into /* NULL, or: members with into[i] != -1 were absorbed (reading S26): star term only */) {
     const double *x = y, *v = y + 3 * n;
     for (int i = 0; i < n; ++i) {
         double r2 = (x[3 * i] * x[3 * i] + x[3 * i + 1] * x[3 * i + 1]) + x[3 * i + 2] * x[3 * i + 2];
         double s = -mu / (r2 * sqrt(r2));
         double ax = s * x[3 * i], ay = s * x[3 * i + 1], az = s * x[3 * i + 2];
         for (int j = 0; j < n; ++j) {
-            if (j == i) continue;
+            if (j == i || (into != NULL && into[i] != -1)) continue;
             double dx = x[3 * j] - x[3 * i], dy = x[3 * j + 1] - x[3 * i + 1], dz = x[3 * j + 2] - x[3 * i + 2];
             double d2 = (dx * dx + dy * dy) + dz * dz;
             if (d2 == 0.0) continue;                       /* coincident: no direction, contributes nothing */
@@ -617,7 +618,7 @@ static void group_rhs(const double *y, double *f, int n, const double *gm, const
 /* The right-hand side above for one group, exported so that the tests can pin the [1 - W] pair term
  * directly (it must equal (1 - oracle_changeover) G m_j / r^2, and kick + encounter = Newton). */
 void oracle_encounter_rhs(const double *y, int n, const double *gm, const double *rc, int nlev, double mu, int kind, double *f) {
-    group_rhs(y, f, n, gm, rc, nlev, mu, kind);
+    group_rhs(y, f, n, gm, rc, nlev, mu, kind, NULL);
 }
 
 #define BS_COLS 8
@@ -630,8 +631,9 @@ void oracle_encounter_rhs(const double *y, int n, const double *gm, const double
  * smallest index: m <- sum m_k, x <- sum m_k x_k / sum m_k, v <- sum m_k v_k / sum m_k (index order, unfused),
  * R <- cbrt(sum R_k^3).  The survivor goes on with the group (its critical radius is held, like every rc, through the
  * step); an absorbed member keeps m = 0, R = 0 (it exerts nothing and is never tested again), is put on the survivor and
- * carried along as a massless member; when the group's integration ends it is put on the body that holds it then (x, v
- * equal), so that the perfect merging at the step boundary (oracle.merge / nb_merge) removes it when the arrays are
+ * from then on takes no part in the encounter: it exerts nothing and feels only the star (were it left to feel the pair
+ * terms it would be a massless particle at zero distance from its survivor, with another critical radius: a singular
+ * encounter); when the group's integration ends it is put on the body that holds it then (x, v equal), so that the perfect merging at the step boundary (oracle.merge / nb_merge) removes it when the arrays are
  * compacted.  into[k] = member that absorbed member k (-1: none).  Returns the number of members absorbed by this test. */
 static int group_collide(double *y, int n, double *mm, double *gm, double *rad, double G, double f, int32_t *into) {
     double *x = y, *v = y + 3 * n;
@@ -639,9 +641,9 @@ static int group_collide(double *y, int n, double *mm, double *gm, double *rad, 
     int nabs = 0, any = 0;
     for (int i = 0; i < n; ++i) parent[i] = i;
     for (int i = 0; i < n; ++i) {
-        if (into[i] >= 0 || (mm[i] == 0.0 && rad[i] == 0.0)) continue;
+        if (into[i] != -1 || (mm[i] == 0.0 && rad[i] == 0.0)) continue;
         for (int j = i + 1; j < n; ++j) {
-            if (into[j] >= 0 || (mm[j] == 0.0 && rad[j] == 0.0)) continue;
+            if (into[j] != -1 || (mm[j] == 0.0 && rad[j] == 0.0)) continue;
             double dx = x[3 * j] - x[3 * i], dy = x[3 * j + 1] - x[3 * i + 1], dz = x[3 * j + 2] - x[3 * i + 2];
             double r2 = (dx * dx + dy * dy) + dz * dz;
             double sr = f * (rad[i] + rad[j]);
@@ -709,17 +711,17 @@ static int64_t encounter_group_core(double *y, int n, double *gm, const double *
     while (t != dt) {
         if (fabs(h) > fabs(dt - t)) h = dt - t;
         if (fabs(h) < 1e-14 * fabs(dt)) { free(buf); return -1; }
-        group_rhs(y, f0, n, gm, rc, nlev, mu, kind);
+        group_rhs(y, f0, n, gm, rc, nlev, mu, kind, into);
         int accepted = 0, cols = 0;
         for (int c = 1; c <= BS_COLS && !accepted; ++c) {
             const int nsub = 2 * c;
             const double hs = h / nsub;
             for (int k = 0; k < dim; ++k) { ym[k] = y[k]; yn[k] = y[k] + hs * f0[k]; }
             for (int s = 2; s <= nsub; ++s) {
-                group_rhs(yn, f, n, gm, rc, nlev, mu, kind);
+                group_rhs(yn, f, n, gm, rc, nlev, mu, kind, into);
                 for (int k = 0; k < dim; ++k) { tmp[k] = ym[k] + 2.0 * hs * f[k]; ym[k] = yn[k]; yn[k] = tmp[k]; }
             }
-            group_rhs(yn, f, n, gm, rc, nlev, mu, kind);
+            group_rhs(yn, f, n, gm, rc, nlev, mu, kind, into);
             /* new tableau row: tmp[] runs along the row, T[] holds the previous row */
             double err2 = 0.0;
             for (int k = 0; k < dim; ++k) {
@@ -807,8 +809,8 @@ void oracle_encounter(double *x, double *v, const double *m, const double *rcrit
 }
 
 /* oracle_encounter with collisions examined inside the solver (reading S26, group_collide above; fully active case):
- * m, radius [N] in/out, absorbed_by [N] out (body that holds an absorbed body at the end of the call, -1 for everybody
- * else; entries of earlier calls are kept).  stats[4] = bodies absorbed. */
+ * m, radius [N] in/out, absorbed_by [N] in/out (body that holds an absorbed body at the end of the call, -1 for
+ * everybody else; bodies marked by earlier calls stay out of the encounter, as absorbed members do: group_collide).  stats[4] = bodies absorbed. */
 void oracle_encounter_collide(double *x, double *v, double *m, double *radius, const double *rcrit, int64_t nlev, int64_t N,
                               double M_star, double G, double dt, int kind, double tol, double f, const int32_t *members,
                               const int32_t *gstart, int64_t ngroups, int64_t max_group, int32_t *absorbed_by, int64_t *stats) {
@@ -823,6 +825,12 @@ void oracle_encounter_collide(double *x, double *v, double *m, double *radius, c
             const int32_t b = members[gstart[g] + k];
             for (int c = 0; c < 3; ++c) { y[3 * k + c] = x[3 * (int64_t)b + c]; y[3 * n + 3 * k + c] = v[3 * (int64_t)b + c]; }
             mm[k] = m[b]; gm[k] = G * m[b]; rad[k] = radius[b]; into[k] = -1;
+            if (absorbed_by[b] >= 0) {
+                /* absorbed in an earlier call and not yet removed from the arrays: still takes no part; it follows its
+                 * holder if that is a member of this group (-2: it is not) */
+                into[k] = -2;
+                for (int q = 0; q < n; ++q) if (members[gstart[g] + q] == absorbed_by[b]) into[k] = q;
+            }
             for (int64_t l = 0; l < nlev; ++l) rc[l * n + k] = rcrit[l * N + b];
         }
         int64_t nabs = 0;

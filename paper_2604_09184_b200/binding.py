@@ -23,7 +23,7 @@ PRECISION_F64, PRECISION_MIXED = 0, 1
 # every symbol include/nbkick.h declares (tests check the library exports each of them)
 SYMBOLS = (
     "nb_default_config", "nb_configure", "nb_workspace_bytes", "nb_rcrit", "nb_kick", "nb_kick_static_setup", "nb_kick_static", "nb_shift",
-    "nb_drift_kepler", "nb_midpoint_drag", "nb_step", "nb_groups", "nb_encounter", "nb_encounter_levels", "nb_merge", "nb_kick_host", "nb_step_host", "nb_status", "nb_status_reset",
+    "nb_drift_kepler", "nb_midpoint_drag", "nb_step", "nb_groups", "nb_encounter", "nb_encounter_collide", "nb_encounter_levels", "nb_merge", "nb_kick_host", "nb_step_host", "nb_status", "nb_status_reset",
     "nb_last_force_ms", "nb_force_time", "nb_force_time_reset", "nb_force_geometry", "nb_fp64_peak", "nb_release", "nb_last_error", "nb_version",
 )
 
@@ -100,6 +100,7 @@ def load():
     lib.nb_step.argtypes = [vp, vp, vp, dbl, i64, dbl, vp, vp, vp, vp, i64]
     lib.nb_groups.argtypes = [vp, vp, i64, vp, vp, vp, vp]
     lib.nb_encounter.argtypes = [vp, vp, vp, vp, dbl, i64, dbl, vp, vp, vp]
+    lib.nb_encounter_collide.argtypes = [vp, vp, vp, vp, vp, dbl, i64, dbl, vp, vp, vp, vp]
     lib.nb_encounter_levels.argtypes = [vp, vp, vp, vp, vp, dbl, i64, dbl, vp, vp]
     lib.nb_merge.argtypes = [vp, vp, vp, vp, i64, vp, vp, vp, vp]
     lib.nb_kick_host.argtypes = [vp, vp, vp, dbl, i64, dbl, vp, vp, vp, vp]
@@ -297,6 +298,15 @@ def nb_encounter(x, v, m, rcrit, M_star, dt, members, gstart, gstat):
                                _dev(gstart, N // 2 + 2, torch.int32), _dev(gstat, 4, torch.int64)))
 
 
+def nb_encounter_collide(x, v, m, radius, rcrit, M_star, dt, members, gstart, gstat, absorbed_by):
+    import torch
+    N = m.numel()
+    _check(load().nb_encounter_collide(_dev(x, 3 * N, torch.float64), _dev(v, 3 * N, torch.float64), _dev(m, N, torch.float64),
+                                       _dev(radius, N, torch.float64), _dev(rcrit, N, torch.float64), float(M_star), N, float(dt),
+                                       _dev(members, N, torch.int32), _dev(gstart, N // 2 + 2, torch.int32),
+                                       _dev(gstat, 4, torch.int64), _dev(absorbed_by, N, torch.int32)))
+
+
 def nb_encounter_levels(x, v, m, rc_hill, rc_vel, M_star, dt, pairs, npairs):
     import torch
     N = m.numel()
@@ -331,7 +341,7 @@ def nb_status() -> dict:
     f = (C.c_int64 * 8)()
     _check(load().nb_status(f))
     return dict(pairs_dropped=int(f[0]), kepler_fail=int(f[1]), nonfinite=int(f[2]), singular=int(f[3]),
-                groups_skipped=int(f[4]), bs_fail=int(f[5]), midpoint_fail=int(f[6]))
+                groups_skipped=int(f[4]), bs_fail=int(f[5]), midpoint_fail=int(f[6]), absorbed=int(f[7]))
 
 
 def nb_status_reset():

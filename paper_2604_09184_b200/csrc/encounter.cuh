@@ -42,11 +42,12 @@ __device__ __forceinline__ void enc_accel(const double qx, const double qy, cons
                                           const double *__restrict__ py, const double *__restrict__ pz,
                                           const double *__restrict__ sgm, const double *__restrict__ shill,
                                           const double *__restrict__ svel, const int nlev, const double mu, const int kind,
-                                          double &ax, double &ay, double &az) {
+                                          double &ax, double &ay, double &az, const bool ghost = false) {
     const double r2 = (qx * qx + qy * qy) + qz * qz;
     const double ir = rsqrt_fast(r2);
     const double s = -mu * (ir * ir * ir);
     ax = s * qx; ay = s * qy; az = s * qz;
+    if (ghost) return;   // absorbed by a collision (reading S26): takes no part in the encounter, feels only the star
     for (int j = 0; j < n; ++j) {
         if (j == self || sgm[j] == 0.0) continue;        // a massless member (semi-active mode) pulls on nobody
         const double dx = px[j] - qx, dy = py[j] - qy, dz = pz[j] - qz;
@@ -82,12 +83,89 @@ struct EncParams {
     int kind;
     int min_size, max_size;   // this launch handles groups with min_size <= n <= max_size
     const int *gcore;         // [ngroups] active members per group (semi-active mode) or nullptr
+    // collisions inside the solver (reading S26; all nullptr / 0: off).  Fully active case only.
+    double *m_io, *radius;    // [N] in/out: masses (= m) and physical radii; an absorbed body ends with m = 0, R = 0
+    int *absorbed_by;         // [N] out: body that holds an absorbed body (entries of the others are not written)
+    double frad;              // radius inflation factor f
     unsigned long long *work; // [2] work counters of the small-group and the satellite kernel, zero at launch: the CTAs take the
                               // next problem when they are done with one (a few hard encounters take ~70 Bulirsch-Stoer steps,
                               // most take one or two: a fixed stride would leave the last CTAs with the hard ones)
 };
 
 __device__ __forceinline__ int enc_group_size(const EncParams &p, const long long g, const int n, bool &split);
+
+// Collisions inside the direct solver (reading S26), called after every ACCEPTED
+// Bulirsch-Stoer step by the n member threads of a group (t = member, act = t < n; a warp if WARP, else the whole CTA)
+// with the members' state in shared memory: X*, V* positions / velocities, smm masses, sgm = G m, srad radii,
+// sinto[k] = member that absorbed member k (-1: none; -2: absorbed in an earlier call by a body outside the group), slab scratch.  Contact iff r_ij < f (R_i + R_j), strict, fp64 on
+// r^2 = (dx^2 + dy^2) + dz^2 without contraction (the test of nb_merge, reading S21); members linked by a chain of
+// contacts merge into the one with the smallest index: m <- sum m_k, x <- sum m_k x_k / sum m_k, v likewise (index
+// order, unfused), R <- cbrt(sum R_k^3); an absorbed member gets m = 0, R = 0 and the survivor's x, v, and from then on
+// takes no part in the encounter (sinto != -1: it exerts nothing and feels only the star, enc_accel's `ghost`).  Returns (to every calling thread) whether anything merged; *nabs (thread 0's) counts.
+// The common case -- nobody touches -- costs one pass of n cheap tests per thread.
+template <bool WARP>
+__device__ __forceinline__ bool enc_collide(double *X0, double *X1, double *X2, double *V0, double *V1, double *V2,
+                                            double *smm, double *sgm, double *srad, int *sinto, int *slab, const int n,
+                                            const int t, const bool act, const double G, const double frad, int &nabs) {
+    auto sync = [&]() { if (WARP) __syncwarp(); else __syncthreads(); };
+    auto any = [&](const bool b) -> bool { return WARP ? (__any_sync(0xffffffffu, b) != 0) : (__syncthreads_or(b ? 1 : 0) != 0); };
+    auto eligible = [&](const int k) { return sinto[k] == -1 && !(smm[k] == 0.0 && srad[k] == 0.0); };
+    auto touch = [&](const int i, const int j) {
+        const double dx = X0[j] - X0[i], dy = X1[j] - X1[i], dz = X2[j] - X2[i];
+        const double r2 = __dadd_rn(__dadd_rn(__dmul_rn(dx, dx), __dmul_rn(dy, dy)), __dmul_rn(dz, dz));
+        const double sr = __dmul_rn(frad, __dadd_rn(srad[i], srad[j]));
+        return r2 < __dmul_rn(sr, sr);
+    };
+    sync();
+    const bool mine = act && eligible(t);
+    int lab = t;
+    bool hit = false;
+    if (mine)
+        for (int j = 0; j < n; ++j)
+            if (j != t && eligible(j) && touch(t, j)) { hit = true; if (j < lab) lab = j; }
+    if (!any(hit)) return false;
+    // label propagation to the smallest index of every cluster (clusters are tiny; this path is rare)
+    if (act) slab[t] = lab;
+    while (true) {
+        sync();
+        int nl = lab;
+        if (hit) {
+            for (int j = 0; j < n; ++j)
+                if (j != t && eligible(j) && touch(t, j) && slab[j] < nl) nl = slab[j];
+            if (slab[nl] < nl) nl = slab[nl];
+        }
+        const bool changed = nl != lab;
+        sync();
+        if (changed) { lab = nl; slab[t] = nl; }
+        if (!any(changed)) break;
+    }
+    sync();
+    int mine_abs = 0;
+    if (hit && lab == t) {   // this member is the survivor of its cluster: sums over the cluster in index order
+        double mt = 0.0, mx0 = 0.0, mx1 = 0.0, mx2 = 0.0, mv0 = 0.0, mv1 = 0.0, mv2 = 0.0, vol = 0.0;
+        for (int k = t; k < n; ++k) {
+            if (slab[k] != t || !eligible(k)) continue;
+            const double mk = smm[k], rk = srad[k];
+            mt = __dadd_rn(mt, mk);
+            mx0 = __dadd_rn(mx0, __dmul_rn(mk, X0[k])); mx1 = __dadd_rn(mx1, __dmul_rn(mk, X1[k])); mx2 = __dadd_rn(mx2, __dmul_rn(mk, X2[k]));
+            mv0 = __dadd_rn(mv0, __dmul_rn(mk, V0[k])); mv1 = __dadd_rn(mv1, __dmul_rn(mk, V1[k])); mv2 = __dadd_rn(mv2, __dmul_rn(mk, V2[k]));
+            vol = __dadd_rn(vol, __dmul_rn(__dmul_rn(rk, rk), rk));
+        }
+        if (mt > 0.0) {
+            X0[t] = __ddiv_rn(mx0, mt); X1[t] = __ddiv_rn(mx1, mt); X2[t] = __ddiv_rn(mx2, mt);
+            V0[t] = __ddiv_rn(mv0, mt); V1[t] = __ddiv_rn(mv1, mt); V2[t] = __ddiv_rn(mv2, mt);
+        }
+        smm[t] = mt; sgm[t] = __dmul_rn(G, mt); srad[t] = cbrt(vol);
+        for (int k = t + 1; k < n; ++k) {
+            if (slab[k] != t || !eligible(k)) continue;
+            smm[k] = 0.0; sgm[k] = 0.0; srad[k] = 0.0; sinto[k] = t; ++mine_abs;
+            X0[k] = X0[t]; X1[k] = X1[t]; X2[k] = X2[t]; V0[k] = V0[t]; V1[k] = V1[t]; V2[k] = V2[t];
+        }
+    }
+    nabs += mine_abs;
+    sync();
+    return true;
+}
 
 // CTA-wide maximum of a non-negative double; every thread gets it.
 template <int THREADS>
@@ -109,9 +187,13 @@ __device__ __forceinline__ double cta_max(double val, double *red /* [32] */) {
 
 template <int THREADS>
 __global__ void __launch_bounds__(THREADS) nb_encounter_kernel(const EncParams p) {
-    extern __shared__ double enc_sm[];  // px[T] py[T] pz[T] gm[T] rc[T] vel[T] red[32]
+    extern __shared__ double enc_sm[];  // px[T] py[T] pz[T] gm[T] rc[T] vel[T] red[32]; with collisions (enc_smem_bytes):
+                                        // + vx[T] vy[T] vz[T] mm[T] rad[T] and int into[T] lab[T]
     double *px = enc_sm, *py = px + THREADS, *pz = py + THREADS, *sgm = pz + THREADS, *src = sgm + THREADS,
            *svel = src + THREADS, *red = svel + THREADS;
+    double *vx = red + 32, *vy = vx + THREADS, *vz = vy + THREADS, *smm = vz + THREADS, *srad = smm + THREADS;
+    int *sinto = reinterpret_cast<int *>(srad + THREADS), *slab = sinto + THREADS;
+    const bool collide = p.radius != nullptr;
     const int t = threadIdx.x;
     const long long ngroups = p.gstat[0];
     for (long long g = blockIdx.x; g < ngroups; g += gridDim.x) {
@@ -133,7 +215,16 @@ __global__ void __launch_bounds__(THREADS) nb_encounter_kernel(const EncParams p
             sgm[t] = p.G * p.m[b];
             src[t] = p.rcrit[b];
             svel[t] = p.rc_vel != nullptr ? p.rc_vel[b] : 0.0;
+            if (collide) { smm[t] = p.m[b]; srad[t] = p.radius[b]; sinto[t] = p.absorbed_by[b] >= 0 ? -2 : -1; }
         }
+        if (collide) {
+            __syncthreads();
+            if (act && sinto[t] == -2) {   // absorbed in an earlier call: follows its holder if that is a member of this group
+                const int holder = p.absorbed_by[b];
+                for (int q = 0; q < n; ++q) if (p.members[g0 + q] == holder) sinto[t] = q;
+            }
+        }
+        int nabs = 0;
         const double my_rc = act ? src[t] : 0.0, my_vel = act ? svel[t] : 0.0;
 
         // acceleration of this thread's body at position (qx,qy,qz), all members' positions taken from shared memory
@@ -143,7 +234,8 @@ __global__ void __launch_bounds__(THREADS) nb_encounter_kernel(const EncParams p
             __syncthreads();
             if (act) {
                 double ax, ay, az;
-                enc_accel(q[0], q[1], q[2], my_rc, my_vel, t, n, px, py, pz, sgm, src, svel, p.nlev, p.mu, p.kind, ax, ay, az);
+                enc_accel(q[0], q[1], q[2], my_rc, my_vel, t, n, px, py, pz, sgm, src, svel, p.nlev, p.mu, p.kind, ax, ay, az,
+                          collide && sinto[t] != -1);
                 f[0] = q[3]; f[1] = q[4]; f[2] = q[5]; f[3] = ax; f[4] = ay; f[5] = az;
             }
         };
@@ -203,17 +295,43 @@ __global__ void __launch_bounds__(THREADS) nb_encounter_kernel(const EncParams p
                 for (int k = 0; k < 6; ++k) y[k] = T[cols - 1][k];
                 tcur = (fabs(p.dt - (tcur + h)) <= 1e-15 * fabs(p.dt)) ? p.dt : tcur + h;
                 if (cols <= 6) h *= 1.3; else if (cols == 8) h *= 0.55;
+                if (collide) {   // contacts at the accepted state (CTA-uniform): the state goes through shared memory
+                    __syncthreads();
+                    if (act) { px[t] = y[0]; py[t] = y[1]; pz[t] = y[2]; vx[t] = y[3]; vy[t] = y[4]; vz[t] = y[5]; }
+                    if (enc_collide<false>(px, py, pz, vx, vy, vz, smm, sgm, srad, sinto, slab, n, t, act, p.G, p.frad, nabs) && act) {
+                        y[0] = px[t]; y[1] = py[t]; y[2] = pz[t]; y[3] = vx[t]; y[4] = vy[t]; y[5] = vz[t];
+                    }
+                }
             } else {
                 h *= 0.5;
             }
         }
         if (failed) {
             if (t == 0) status_add(p.status, ST_BS_FAIL, 1);  // group left unchanged
+        } else if (collide) {
+            // an absorbed member ends on the body that holds it now (its survivor may have been absorbed later itself)
+            __syncthreads();
+            if (act) { px[t] = y[0]; py[t] = y[1]; pz[t] = y[2]; vx[t] = y[3]; vy[t] = y[4]; vz[t] = y[5]; }
+            __syncthreads();
+            if (act) {
+                int s0 = t;
+                while (sinto[s0] >= 0) s0 = sinto[s0];
+                p.x[3 * (size_t)b] = px[s0]; p.x[3 * (size_t)b + 1] = py[s0]; p.x[3 * (size_t)b + 2] = pz[s0];
+                p.v[3 * (size_t)b] = vx[s0]; p.v[3 * (size_t)b + 1] = vy[s0]; p.v[3 * (size_t)b + 2] = vz[s0];
+                p.m_io[b] = smm[t]; p.radius[b] = srad[t];
+                if (s0 != t) p.absorbed_by[b] = p.members[g0 + s0];
+                if (nabs > 0) status_add(p.status, ST_ABSORBED, nabs);
+            }
         } else if (act) {
 #pragma unroll
             for (int c = 0; c < 3; ++c) { p.x[3 * (size_t)b + c] = y[c]; p.v[3 * (size_t)b + c] = y[3 + c]; }
         }
     }
+}
+
+// dynamic shared memory of nb_encounter_kernel<T>
+__host__ __device__ constexpr size_t enc_smem_bytes(int T, bool collide) {
+    return (6 * (size_t)T + 32) * sizeof(double) + (collide ? 5 * (size_t)T * sizeof(double) + 2 * (size_t)T * sizeof(int) : 0);
 }
 
 // Groups of up to 32 members: latency is everything (a hard pair takes tens of serial Bulirsch-Stoer steps),
@@ -256,6 +374,10 @@ __device__ __forceinline__ void bs_small_problem(const EncParams &p, const int b
     __shared__ double ycur[6][32];
     __shared__ double ctrl_h, ctrl_t;
     __shared__ int ctrl_done;                // 0 running, 1 finished, 2 failed
+    __shared__ double smm[32], srad[32];     // collisions inside the solver (p.radius != nullptr): masses, radii,
+    __shared__ int sinto[32], slab[32], sbody[32];   // who absorbed whom, label scratch, body of every member
+    const bool collide = p.radius != nullptr;
+    int nabs = 0;
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
     const double tol2 = p.tol * p.tol;
     const bool act = lane < n;
@@ -267,8 +389,17 @@ __device__ __forceinline__ void bs_small_problem(const EncParams &p, const int b
             sgm[lane] = p.G * p.m[b];
             src[lane] = p.rcrit[b];
             svel[lane] = p.rc_vel != nullptr ? p.rc_vel[b] : 0.0;
+            if (collide) { smm[lane] = p.m[b]; srad[lane] = p.radius[b]; sinto[lane] = p.absorbed_by[b] >= 0 ? -2 : -1; sbody[lane] = b; }
         }
         if (lane == 0) { ctrl_h = p.dt; ctrl_t = 0.0; ctrl_done = (p.dt == 0.0) ? 1 : 0; }
+        if (collide) {
+            // absorbed in an earlier call and still in the arrays: follows its holder if that is a member of this problem
+            __syncwarp();
+            if (act && sinto[lane] == -2) {
+                const int holder = p.absorbed_by[b];
+                for (int q = 0; q < n; ++q) if (sbody[q] == holder) sinto[lane] = q;
+            }
+        }
     }
     __syncthreads();
     const double my_rc = act ? src[lane] : 0.0, my_vel = act ? svel[lane] : 0.0;
@@ -290,7 +421,8 @@ __device__ __forceinline__ void bs_small_problem(const EncParams &p, const int b
                 __syncwarp();
                 if (act) {
                     double ax, ay, az;
-                    enc_accel(q[0], q[1], q[2], my_rc, my_vel, lane, n, px[w], py[w], pz[w], sgm, src, svel, p.nlev, p.mu, p.kind, ax, ay, az);
+                    enc_accel(q[0], q[1], q[2], my_rc, my_vel, lane, n, px[w], py[w], pz[w], sgm, src, svel, p.nlev, p.mu, p.kind, ax, ay, az,
+                              collide && sinto[lane] != -1);
                     f[0] = q[3]; f[1] = q[4]; f[2] = q[5]; f[3] = ax; f[4] = ay; f[5] = az;
                 }
             };
@@ -350,6 +482,9 @@ __device__ __forceinline__ void bs_small_problem(const EncParams &p, const int b
 #pragma unroll
                 for (int k = 0; k < 6; ++k) ycur[k][lane] = T[cols - 1][k];
             }
+            if (collide && accepted)   // warp-uniform: contacts at the accepted state, clusters merge at once
+                enc_collide<true>(ycur[0], ycur[1], ycur[2], ycur[3], ycur[4], ycur[5], smm, sgm, srad, sinto, slab, n, lane, act,
+                                  p.G, p.frad, nabs);
             if (lane == 0) {
                 if (underflow) {
                     ctrl_done = 2;
@@ -369,8 +504,16 @@ __device__ __forceinline__ void bs_small_problem(const EncParams &p, const int b
         if (ctrl_done == 2) {
             if (lane == 0) status_add(p.status, ST_BS_FAIL, 1);  // group left unchanged
         } else if (act && lane >= keep_from) {
+            int src = lane;
+            if (collide) {
+                // an absorbed member ends on the body that holds it now (its survivor may have been absorbed later itself)
+                while (sinto[src] >= 0) src = sinto[src];
+                p.m_io[b] = smm[lane]; p.radius[b] = srad[lane];
+                if (src != lane) p.absorbed_by[b] = sbody[src];
+            }
 #pragma unroll
-            for (int c = 0; c < 3; ++c) { p.x[3 * (size_t)b + c] = ycur[c][lane]; p.v[3 * (size_t)b + c] = ycur[3 + c][lane]; }
+            for (int c = 0; c < 3; ++c) { p.x[3 * (size_t)b + c] = ycur[c][src]; p.v[3 * (size_t)b + c] = ycur[3 + c][src]; }
+            if (nabs > 0) status_add(p.status, ST_ABSORBED, nabs);
         }
     }
 

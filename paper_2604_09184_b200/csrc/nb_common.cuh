@@ -33,7 +33,7 @@ constexpr double kFarJ = 1.0e30;    // padding j-records sit here with zero mass
 constexpr double kFarI = -1.0e30;   // padding i-lanes sit here; their sums are discarded
 
 // status counters (device int64[8]); meanings in include/nbkick.h nb_status
-enum { ST_PAIR_DROPPED = 0, ST_KEPLER_FAIL = 1, ST_NONFINITE = 2, ST_SINGULAR = 3, ST_GROUP_SKIPPED = 4, ST_BS_FAIL = 5, ST_MIDPOINT_FAIL = 6, ST_COUNT = 8 };
+enum { ST_PAIR_DROPPED = 0, ST_KEPLER_FAIL = 1, ST_NONFINITE = 2, ST_SINGULAR = 3, ST_GROUP_SKIPPED = 4, ST_BS_FAIL = 5, ST_MIDPOINT_FAIL = 6, ST_ABSORBED = 7, ST_COUNT = 8 };
 
 __device__ __forceinline__ void status_add(long long *status, int which, long long n) {
     atomicAdd(reinterpret_cast<unsigned long long *>(status + which), static_cast<unsigned long long>(n));

@@ -573,7 +573,8 @@ void enqueue_encounter_plan(const Workspace &w, int64_t N, const int32_t *member
 // (one thread per member, columns in sequence)
 void enqueue_encounter(const Workspace &w, double *x, double *v, const double *m, const double *rcrit, double M_star,
                        int64_t N, double dt, const int32_t *members, const int32_t *gstart, const int64_t *gstat,
-                       bool plan_done, const double *rc_vel = nullptr, int nlev = 1) {
+                       bool plan_done, const double *rc_vel = nullptr, int nlev = 1, double *radius = nullptr,
+                       int *absorbed_by = nullptr) {
     const long long *gs = reinterpret_cast<const long long *>(gstat);
     if (!plan_done) enqueue_encounter_plan(w, N, members, gstart, gstat);
     EncParams ep;
@@ -581,6 +582,10 @@ void enqueue_encounter(const Workspace &w, double *x, double *v, const double *m
     ep.gstat = gs; ep.status = w.status; ep.mu = g_cfg.G * M_star; ep.G = g_cfg.G;
     ep.dt = dt; ep.tol = g_cfg.bs_tol > 0.0 ? g_cfg.bs_tol : 1e-12; ep.kind = g_cfg.changeover_kind;
     ep.gcore = w.g_core; ep.rc_vel = rc_vel; ep.nlev = nlev;
+    // collisions inside the solver (reading S26): m and radius are then in/out
+    ep.m_io = radius ? const_cast<double *>(m) : nullptr; ep.radius = radius; ep.absorbed_by = absorbed_by;
+    ep.frad = g_cfg.radius_factor > 0.0 ? g_cfg.radius_factor : 1.0;
+    const bool collide = radius != nullptr;
     ep.work = reinterpret_cast<unsigned long long *>(w.status + 16);   // two spare words of the 512-byte status head
     cudaMemsetAsync(ep.work, 0, 2 * sizeof(unsigned long long), stream());
     long long small_blocks = N / 2 + 1;
@@ -598,11 +603,11 @@ void enqueue_encounter(const Workspace &w, double *x, double *v, const double *m
     ep.min_size = 33; ep.max_size = 128;
     long long mid_blocks = N / 33 + 1;
     if (mid_blocks > 8LL * sm_count()) mid_blocks = 8LL * sm_count();
-    nb_encounter_kernel<128><<<(unsigned)mid_blocks, 128, (6 * 128 + 32) * sizeof(double), stream()>>>(ep);
+    nb_encounter_kernel<128><<<(unsigned)mid_blocks, 128, enc_smem_bytes(128, collide), stream()>>>(ep);
     ep.min_size = 129; ep.max_size = kMaxGroup;
     static bool attr_set = false;
-    const size_t big_smem = (6 * (size_t)kMaxGroup + 32) * sizeof(double);
-    if (!attr_set) { cudaFuncSetAttribute(nb_encounter_kernel<kMaxGroup>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)big_smem); attr_set = true; }
+    const size_t big_smem = enc_smem_bytes(kMaxGroup, collide);
+    if (!attr_set) { cudaFuncSetAttribute(nb_encounter_kernel<kMaxGroup>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)enc_smem_bytes(kMaxGroup, true)); attr_set = true; }
     long long big_blocks = N / 129 + 1;
     if (big_blocks > 2LL * sm_count()) big_blocks = 2LL * sm_count();
     nb_encounter_kernel<kMaxGroup><<<(unsigned)big_blocks, kMaxGroup, big_smem, stream()>>>(ep);
@@ -1128,6 +1133,21 @@ int nb_encounter(double *x, double *v, const double *m, const double *rcrit, dou
     Workspace w;
     if ((rc = check_workspace_head(N, 2, &w))) return rc;
     enqueue_encounter(w, x, v, m, rcrit, M_star, N, dt, members, gstart, gstat, false);
+    NB_CUDA(cudaGetLastError());
+    return NB_OK;
+}
+
+int nb_encounter_collide(double *x, double *v, double *m, double *radius, const double *rcrit, double M_star, int64_t N,
+                         double dt, const int32_t *members, const int32_t *gstart, const int64_t *gstat, int32_t *absorbed_by) {
+    std::lock_guard<std::mutex> lk(g_mu);
+    int rc = check_common(N, dt, M_star);
+    if (rc) return rc;
+    if (!x || !v || !m || !radius || !rcrit || !members || !gstart || !gstat || !absorbed_by)
+        return fail(NB_E_NULL, "nb_encounter_collide: NULL argument");
+    if (g_cfg.n_active > 0 && g_cfg.n_active < N) return fail(NB_E_BADARG, "nb_encounter_collide: fully active case only");
+    Workspace w;
+    if ((rc = check_workspace_head(N, 2, &w))) return rc;
+    enqueue_encounter(w, x, v, m, rcrit, M_star, N, dt, members, gstart, gstat, false, nullptr, 1, radius, absorbed_by);
     NB_CUDA(cudaGetLastError());
     return NB_OK;
 }

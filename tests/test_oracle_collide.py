@@ -129,3 +129,50 @@ def test_step_enc_with_radii():
     # a perfect merger keeps mass and momentum; the pair's angular momentum about its own barycentre (reduced mass x
     # separation x relative speed: the merged body's spin) leaves the orbital budget -- tiny, and not zero
     assert 0.0 < np.linalg.norm(E1["L"] - E0["L"]) <= 1e-7 * np.linalg.norm(E0["L"])
+
+
+def test_absorbed_bodies_follow_their_holder_when_it_is_absorbed_later():
+    """1 and 2 touch at the start (2 goes into 1 after the first accepted step); 0 arrives later and absorbs 1.  An absorbed
+    body takes no part in the encounter any more (it feels only the star) -- left to feel the pair terms it would be a
+    massless particle at zero distance from a massive one with another critical radius: a singular encounter -- and
+    ends on the body that holds it at the end, here body 0.  Pinned by the two-body problem {0, 1 + 2 merged}: same
+    final state of body 0 and about as many steps."""
+    R, mass = 1e-4, 1e-5
+    x = np.array([[1.0 - 20 * R, 0, 0], [1.0, 0, 0], [1.0 + 1.5 * R, 0, 0]])
+    v = np.tile(np.array([0.0, np.sqrt(G), 0.0]), (3, 1)); v[0, 0] += 60 * R
+    m = np.array([mass, mass, 0.5 * mass]); rc = np.full(3, 1e-2); rad = np.full(3, R)
+    xa, va, st = oracle.encounter(x, v, m, rc, 1.0, 0.5, G, _one_group(3), radius=rad)
+    assert list(st["absorbed_by"]) == [-1, 0, 0] and st["m"][0] == mass + (mass + 0.5 * mass)
+    assert np.array_equal(xa[1], xa[0]) and np.array_equal(xa[2], xa[0]) and np.array_equal(va[2], va[0])
+    m12 = m[1] + m[2]
+    x2 = np.array([x[0], (m[1] * x[1] + m[2] * x[2]) / m12]); v2 = np.array([v[0], (m[1] * v[1] + m[2] * v[2]) / m12])
+    xb, vb, st2 = oracle.encounter(x2, v2, np.array([mass, m12]), rc[:2], 1.0, 0.5, G, _one_group(2), radius=np.array([R, np.cbrt(2.0) * R]))
+    assert st2["absorbed"] == 1
+    assert np.max(np.abs(xb[0] - xa[0])) <= 1e-12 and np.max(np.abs(vb[0] - va[0])) <= 1e-11 * np.sqrt(G)
+    assert st["steps"] <= st2["steps"] + 10
+
+
+def test_bodies_absorbed_in_an_earlier_call_stay_out_of_the_encounter():
+    """The ring group that showed the problem: two members touch in the first half of the interval; in a second call over
+    the other half the absorbed ones are still in the arrays (m = 0, R = 0, on their holders).  They must not be
+    integrated against their holders: the second call converges in a step or two, does not fail and absorbs nothing."""
+    import nb_inputs
+    d = nb_inputs.make_config(2, n_override=2500)
+    rc = oracle.rcrit(d.x, d.v, d.m, d.M_star, d.dt, G, 3.0, 0.4)
+    sure, _ = oracle.pairs(d.x, rc)
+    grp = oracle.groups(sure, d.N)
+    seg = grp["members"][grp["gstart"][0]:grp["gstart"][1]]
+    sub = dict(ngroups=1, members=seg.astype(np.int32), gstart=np.array([0, len(seg)], dtype=np.int32), label=None)
+    x1, v1, s1 = oracle.encounter(d.x, d.v, d.m, rc, d.M_star, 1.5, G, sub, radius=d.radius, radius_factor=400.0)
+    assert s1["failed"] == 0 and s1["absorbed"] == 2
+    x2, v2, s2 = oracle.encounter(x1, v1, s1["m"], rc, d.M_star, 1.5, G, sub, radius=s1["radius"], radius_factor=400.0,
+                                  absorbed_by=s1["absorbed_by"])
+    assert s2["failed"] == 0 and s2["absorbed"] == 0 and s2["steps"] <= 3
+    assert np.array_equal(s2["absorbed_by"], s1["absorbed_by"])
+    gone = np.flatnonzero(s2["absorbed_by"] >= 0)
+    assert np.array_equal(x2[gone], x2[s2["absorbed_by"][gone]]) and np.array_equal(v2[gone], v2[s2["absorbed_by"][gone]])
+    # and in one call over the whole interval (the first trial step is rejected, the contact is found at t = dt / 2)
+    x3, v3, s3 = oracle.encounter(d.x, d.v, d.m, rc, d.M_star, 3.0, G, sub, radius=d.radius, radius_factor=400.0)
+    assert s3["failed"] == 0 and s3["absorbed"] == 2 and np.array_equal(s3["absorbed_by"], s1["absorbed_by"])
+    live = s3["absorbed_by"][seg] < 0
+    assert np.max(np.abs(x3[seg][live] - x2[seg][live])) <= 1e-11
