@@ -118,6 +118,14 @@ typedef struct nb_config {
     int64_t slot_bytes_max;  /* tuning (symmetric kernel): cap of the partial-acceleration slots in the workspace; 0 (default) =
                                 4 GiB.  A grid whose slots (24 N^2 / S bytes) would pass it is evaluated in bands of tile
                                 columns, one launch and one fold into acc per band (same results to rounding order) */
+    double *collide_radius;  /* nb_step with resolve_encounters: DEVICE double[N] in/out, physical radii; non-NULL switches on the
+                                collisions inside the direct solver (nb_encounter_collide; reading S26),
+                                inflated by radius_factor.  The step then CHANGES m (the caller's array, although nb_step
+                                takes it as const) and the radii: an absorbed body stays in the arrays with m = 0, R = 0
+                                on the body that holds it until nb_merge compacts them.  levels = 0, fully active case.
+                                Default NULL: off */
+    int32_t *collide_absorbed_by; /* with collide_radius: DEVICE int32[N] in/out, -1 or the body that holds an absorbed body
+                                (initialise with -1; required) */
 } nb_config;
 
 void nb_default_config(nb_config *cfg);

@@ -58,6 +58,8 @@ class NbConfig(C.Structure):
         ("midpoint_tol", C.c_double),
         ("precision", C.c_int),
         ("slot_bytes_max", C.c_int64),
+        ("collide_radius", C.c_void_p),
+        ("collide_absorbed_by", C.c_void_p),
     ]
 
 
@@ -171,7 +173,8 @@ def default_config() -> NbConfig:
 def configure(N=None, *, stream=None, pair_capacity=0, n_active=0, G=None, n1=3.0, n2=0.4, changeover_kind=0,
               i_per_thread=0, j_splits=0, use_graph=True, reuse_acc=False, time_force=False,
               force_kernel=0, sym_block=0, resolve_encounters=False, bs_tol=1e-12, radius_factor=1.0, sort_staging=0, levels=0, drag_gamma=0.0, drag_eta=0.0, drag_power=0,
-              midpoint_iters=50, midpoint_tol=1e-14, precision=0, slot_bytes_max=0, workspace_bytes=None,
+              midpoint_iters=50, midpoint_tol=1e-14, precision=0, slot_bytes_max=0, collide_radius=None, collide_absorbed_by=None,
+              workspace_bytes=None,
               device="cuda"):
     """nb_configure with a torch-allocated workspace sized for N bodies (N=None: no workspace,
     enough for the _host calls; workspace_bytes: explicit size, e.g. the head that the O(N) calls
@@ -197,6 +200,9 @@ def configure(N=None, *, stream=None, pair_capacity=0, n_active=0, G=None, n1=3.
     cfg.midpoint_iters, cfg.midpoint_tol = int(midpoint_iters), float(midpoint_tol)
     cfg.precision = int(precision)
     cfg.slot_bytes_max = int(slot_bytes_max)
+    cfg.collide_radius = _dev(collide_radius, None, None)
+    cfg.collide_absorbed_by = _dev(collide_absorbed_by, None, None)
+    _state["collide"] = (collide_radius, collide_absorbed_by)   # keep the tensors alive
     if N is not None:
         import torch
         if stream is None:

@@ -40,7 +40,7 @@ size_t g_arena_bytes = 0;
 
 // cached CUDA graph of one interior step of nb_step
 struct StepKey {
-    const void *x, *v, *m, *rcrit, *acc, *pairs, *npairs, *ws, *stream;
+    const void *x, *v, *m, *rcrit, *acc, *pairs, *npairs, *ws, *stream, *radius, *absorbed_by;
     int64_t N, n_active, cap;
     double dt, M_star, G, n1, n2, bs_tol, drag_gamma, drag_eta, midpoint_tol;
     int kind, ipt, jsplit, enc, levels, drag_power, midpoint_iters, band;
@@ -755,6 +755,10 @@ int step_impl(double *x, double *v, const double *m, double M_star, int64_t N, d
     const bool enc = g_cfg.resolve_encounters != 0;
     if (enc && !pairs) return fail(NB_E_BADARG, "nb_step: resolve_encounters needs the pair list (pairs != NULL)");
     const bool ml = enc && g_cfg.levels > 0;
+    // collisions examined inside the direct solver (reading S26): m and the radii change on the way
+    const bool coll = enc && g_cfg.collide_radius != nullptr;
+    if (coll && !g_cfg.collide_absorbed_by) return fail(NB_E_NULL, "nb_step: collide_radius is set but collide_absorbed_by is NULL");
+    if (coll && (ml || g.Nj != N)) return fail(NB_E_BADARG, "nb_step: collisions inside the solver (collide_radius) need levels = 0 and the fully active case");
     if (ml && g.Nj != N) return fail(NB_E_BADARG, "nb_step: the multi-level changeover (levels > 0) is defined for the fully active case only");
     // force evaluation that closes a step: closing half-kick [+ opening half-kick of the next step]; with the extra
     // force the two half-kicks are separated by D(dt/2) D(dt/2)
@@ -788,7 +792,8 @@ int step_impl(double *x, double *v, const double *m, double M_star, int64_t N, d
         nb_drift_kernel<<<nblk, kBodyThreads, 0, stream()>>>(x, v, m, (int)N, mu, dt, w.mvA, nblk, dtc, M_star,
                                                              enc ? nullptr : w.mvB, w.status, enc ? w.enc_flag : nullptr);
         if (enc) {
-            enqueue_encounter(w, x, v, m, rc_io, M_star, N, dt, w.g_members, w.g_start, w.g_stat, true);
+            enqueue_encounter(w, x, v, m, rc_io, M_star, N, dt, w.g_members, w.g_start, w.g_stat, true, nullptr, 1,
+                              coll ? g_cfg.collide_radius : nullptr, coll ? g_cfg.collide_absorbed_by : nullptr);
             nb_momentum_kernel<<<nblk, kBodyThreads, 0, stream()>>>(v, m, (int)N, w.mvB);
         }
         // C(dt/2) folded into prep; force; B(dt/2) [+ B(dt/2) of the next step]
@@ -810,6 +815,7 @@ int step_impl(double *x, double *v, const double *m, double M_star, int64_t N, d
         key.cap = g_cfg.pair_capacity; key.dt = dt; key.M_star = M_star; key.G = g_cfg.G; key.n1 = g_cfg.n1;
         key.n2 = g_cfg.n2; key.kind = g_cfg.changeover_kind; key.bs_tol = g_cfg.bs_tol; key.enc = (enc ? 1 : 0) + 2 * g.sorted; key.ipt = g.S * 1000 + g.ipt * 100 + g.minb * 10 + g.warps + 100000 * g.xcols; key.jsplit = g.nsplit; key.band = g.band;
         key.ws_bytes = g_cfg.workspace_bytes; key.levels = g_cfg.levels;
+        key.radius = coll ? g_cfg.collide_radius : nullptr; key.absorbed_by = coll ? g_cfg.collide_absorbed_by : nullptr;
         key.drag_gamma = g_cfg.drag_gamma; key.drag_eta = g_cfg.drag_eta; key.midpoint_tol = g_cfg.midpoint_tol;
         key.drag_power = g_cfg.drag_power; key.midpoint_iters = g_cfg.midpoint_iters + 1000 * g.mixed;
         const bool hop = !stream_capturable();

@@ -147,3 +147,44 @@ def test_absorbed_bodies_follow_their_holder():
     m = np.array([mass, mass, 0.5 * mass]); rc = np.full(3, 1e-2); rad = np.full(3, R)
     g, st = _compare(x, v, m, rad, rc, 1.0, 0.5, _grp_all(3), "sequential absorption", expect_absorbed=2)
     assert list(g["absorbed_by"]) == [-1, 0, 0]
+
+
+@pytest.mark.parametrize("use_graph", [True, False])
+def test_step_with_collisions_inside_the_solver(use_graph):
+    """nb_step(resolve_encounters, collide_radius) against oracle.step_enc(radius=...): 4 steps of a ring with radii
+    inflated by f = 400; the masses change from step to step, absorbed bodies stay in the arrays on their holders."""
+    import paper_2604_09184_b200 as nb
+    torch = torch_mod()
+    d = nb_inputs.make_config(2, n_override=1500)
+    nsteps, f = 4, 400.0
+    ref = oracle.step_enc(d.x, d.v, d.m, d.M_star, d.dt, G_GAUSS, nsteps, n1=3.0, n2=0.4, radius=d.radius, radius_factor=f)
+    assert ref["stats"]["absorbed"] >= 3 and ref["stats"]["failed"] == 0 and ref["stats"]["border"] == 0
+    x, v, m, R = to_dev(d.x), to_dev(d.v), to_dev(d.m), to_dev(d.radius)
+    ab = torch.full((d.N,), -1, dtype=torch.int32, device="cuda")
+    acc = torch.zeros_like(x); rcd = torch.zeros(d.N, dtype=torch.float64, device="cuda")
+    cap = 1 << 16
+    pairs = torch.zeros((cap, 2), dtype=torch.int32, device="cuda"); npairs = torch.zeros(1, dtype=torch.int64, device="cuda")
+    nb.configure(d.N, G=G_GAUSS, n1=3.0, n2=0.4, pair_capacity=cap, resolve_encounters=True, radius_factor=f,
+                 collide_radius=R, collide_absorbed_by=ab, use_graph=use_graph)
+    nb.nb_status_reset()
+    nb.nb_step(x, v, m, d.M_star, d.dt, rcd, acc, pairs, npairs, nsteps)
+    torch.cuda.synchronize()
+    st = nb.nb_status()
+    assert st["bs_fail"] == 0 and st["groups_skipped"] == 0 and st["absorbed"] == ref["stats"]["absorbed"]
+    assert np.array_equal(ab.cpu().numpy(), ref["absorbed_by"])
+    assert np.array_equal(m.cpu().numpy(), ref["m"])
+    assert np.max(np.abs(R.cpu().numpy() - ref["radius"])) <= 5e-16 * ref["radius"].max()
+    ex = np.max(np.abs(x.cpu().numpy() - ref["x"])) / np.max(np.abs(ref["x"]))
+    ev = np.max(np.abs(v.cpu().numpy() - ref["v"])) / np.max(np.abs(ref["v"]))
+    print(f"step with collisions (graph {use_graph}): absorbed {st['absorbed']}, rel dx {ex:.2e} dv {ev:.2e}")
+    assert ex <= ENC_TOL and ev <= ENC_TOL
+    n = int(npairs.item())
+    got = {tuple(p) for p in pairs[:n].cpu().numpy().tolist()}
+    assert got == {tuple(p) for p in ref["pairs"].tolist()}
+    # then the step-boundary merge removes the absorbed bodies: N shrinks by exactly their number
+    surv = torch.zeros(d.N, dtype=torch.int32, device="cuda"); mstat = torch.zeros(4, dtype=torch.int64, device="cuda")
+    nb.configure(d.N, G=G_GAUSS, pair_capacity=cap, radius_factor=1.0)
+    nb.nb_merge(x, v, m, R, pairs, npairs, surv, mstat)
+    torch.cuda.synchronize()
+    assert int(mstat[0].item()) == d.N - st["absorbed"]
+    assert float(m[: int(mstat[0].item())].min().item()) > 0.0
