@@ -420,8 +420,8 @@ def run_cuda(args):
 
     value = whole_job_value(world, K, inter_per_step, total_ms)
     symmetric = geom.tile_j < 0
-    kernel = "nb_force_sym_kernel" if symmetric else ("nb_force_mixed_kernel" if mixed else "nb_force_tiles_kernel")
-    sorted_staging = symmetric and N >= 32768   # NB_SORT_AUTO (include/nbkick.h)
+    kernel = ("nb_force_symds_kernel" if mixed else "nb_force_sym_kernel") if symmetric else ("nb_force_mixed_kernel" if mixed else "nb_force_tiles_kernel")
+    sorted_staging = symmetric and not mixed and N >= 32768   # NB_SORT_AUTO (include/nbkick.h); the mixed Newton-III kernel stages unsorted
     traffic, traffic_source = _traffic_from_profile(kernel, N, geom, sorted_staging, args.precision)
     # FP64-pipe instructions per ORDERED interaction on the fast path: 20 per unordered pair (Newton III)
     # or 15 (one-sided); DESIGN.md section 5
@@ -431,7 +431,7 @@ def run_cuda(args):
     line = dict(
         metric=METRIC, value=value, unit=UNIT, n_gpus=world, steps=K, warmup=W, ms_per_step=total_ms / K,
         higher_is_better=True, scaling="weak", vs_baseline=None,
-        dtype="f64" if not mixed else "f64 differences / f32 pair arithmetic / f64 accumulation (NB_PRECISION_MIXED; not the metric's precision)",
+        dtype="f64" if not mixed else "double-single (Newton-III kernel) or f64 differences, f32 pair arithmetic, f64 accumulation (NB_PRECISION_MIXED; not the metric's precision)",
         data="synthetic",
         config=dict(workload=workload_name(d, na), parallelism="replicas only (path does not shard)" if world > 1 else "1 GPU",
                     l2="256 MiB buffer written between timed steps (L2 flush), outside the per-step CUDA events",

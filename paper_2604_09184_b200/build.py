@@ -9,7 +9,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 _CSRC = os.path.join(_HERE, "csrc")
 LIB = os.path.join(_HERE, "libnbkick.so")
 SOURCES = [os.path.join(_CSRC, "nbkick.cu")]
-HEADERS = [os.path.join(_CSRC, f) for f in ("nb_common.cuh", "force_tiles.cuh", "force_sym.cuh", "body_kernels.cuh", "kepler.cuh", "groups.cuh", "encounter.cuh", "merge.cuh", "sort_staging.cuh", "multilevel.cuh", "force_mixed.cuh", "step_small.cuh")] + [
+HEADERS = [os.path.join(_CSRC, f) for f in ("nb_common.cuh", "force_tiles.cuh", "force_sym.cuh", "body_kernels.cuh", "kepler.cuh", "groups.cuh", "encounter.cuh", "merge.cuh", "sort_staging.cuh", "multilevel.cuh", "force_mixed.cuh", "force_symds.cuh", "step_small.cuh")] + [
     os.path.join(os.path.dirname(_HERE), "include", "nbkick.h")]
 
 NVCC_FLAGS = [

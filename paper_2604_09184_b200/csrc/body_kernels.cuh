@@ -35,6 +35,7 @@ struct PrepParams {
     JRec *jrec;             // [Njpad] one-sided kernel's records (nullptr: not staged)
     double2 *sxy, *szg;     // [2 Npad_sym] symmetric kernel's (x,y) and (z,Gm), doubled-block layout (nullptr: not staged)
     int *sthr;              // [2 Npad_sym] hi32(rcrit^2) + 1
+    float4 *sa, *sb;        // [2 Npad_sym] double-single records of the Newton-III mixed-precision kernel (nullptr: not staged)
     int Npad_sym;
     const int *pos_of;      // [N] staged position of each body (sort_staging.cuh) or nullptr: position = index
     const double *mv_in;    // [nblk_in,3] momentum partials or nullptr
@@ -94,6 +95,7 @@ __device__ __forceinline__ void prep_one(const PrepParams &p, const int i, const
         p.sxy[en] = make_double2(sx_, sy_); p.sxy[en + 32] = make_double2(sx_, sy_);
         p.szg[en] = make_double2(sz_, r.gm); p.szg[en + 32] = make_double2(sz_, r.gm);
         p.sthr[en] = thr; p.sthr[en + 32] = thr;
+        if (p.sa != nullptr) symds_stage(p.sa, p.sb, pos, sx_, sy_, sz_, r.gm, r.rc2);
     }
 }
 

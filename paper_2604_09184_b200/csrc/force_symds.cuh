@@ -1,0 +1,228 @@
+// force_symds.cuh -- Newton-III form of the MIXED-PRECISION kick (Fig. 1 contrasts FP32
+// and FP64 runs of the same code on both of its GPUs).  What is computed is the H_B kick of force_sym.cuh (PAPER.md:86
+// Eq. 5, 98) and the same pair list; what changes is the arithmetic of the pairs that are out of reach of every critical
+// radius (all but ~1e-6 of them), which runs ENTIRELY on the FP32 pipe:
+//   * positions are staged as double-single, x = xh + xl with xh = fl32(x), xl = fl32(x - xh) (48 bits together);
+//     dx = fl(fl(xjh - xih) + fl(xjl - xil)) carries a relative error of ~2.5 * 2^-24 OF THE DIFFERENCE ITSELF: the
+//     cancellation of nearby positions happens between the high parts (exactly, by Sterbenz, when they are close) and
+//     the low parts restore what fl32(x) lost -- no fp64 subtraction, no conversion;
+//   * r^2, MUFU.RSQ, its cube, the two mass products, six FFMA: 22 FP32 instructions per UNORDERED pair, both sides
+//     served (the fp64 kernel: 20 FP64 instructions, on a pipe half as wide);
+//   * the j-sums travel through the warp as in force_sym.cuh (3 SHFL per rotation instead of 6); fp32 sums over ONE
+//     visit of a 32-body block (32 terms on the i side, 128 on the j side), fp64 from there on.
+// Pairs whose fp32 r^2 is within reach of a critical radius (margin 2^-18: far above the fp32 rounding of r^2), and
+// every self term, are killed in the fp32 loop (rsqrt replaced by 0: they contribute exactly 0 to both sides) and
+// re-evaluated by the EXACT fp64 pass of force_sym.cuh (sym_exact) from the fp64 staged arrays: the changeover weight,
+// the pair test r^2 < rc^2 and the pair list are bit-identical to the fp64 kernel's.  Tolerance reading: DESIGN.md S25.
+// Same super-tile decomposition, skewed unit order, slots and determinism as nb_force_sym_kernel (no sorted staging, no
+// tail splitting, no bands: the host falls back to the one-sided mixed kernel where those would be needed).
+#pragma once
+#include "force_sym.cuh"
+
+namespace nbk {
+
+struct SymDsParams {
+    SymParams sp;      // fp64 staged arrays (exact pass), slots, pair list, geometry: as nb_force_sym_kernel, unsorted
+    const float4 *sa;  // [2 Npad] (xh, yh, zh, fl32(G m))              doubled-block layout
+    const float4 *sb;  // [2 Npad] (xl, yl, zl, rc^2 (1 + 2^-18) rounded up)
+};
+
+constexpr int kDsI = 4;   // i-bodies per lane
+__host__ __device__ constexpr size_t symds_smem_bytes(int S) { return (size_t)S * (32 + 32 + 24) + 16; }
+
+__device__ __forceinline__ float rsqrt_f32(const float a) {
+    float y;
+    asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(a));
+    return y;
+}
+
+// One warp, one block of 32 j-bodies, 32 rotations in fp32; then the exact fp64 pass for the flagged rotations.
+// On return lane l holds in (bx,by,bz) the fp64 sums for j = jbase + l; the i-side sums of the visit are ADDED to AX/AY/AZ.
+template <bool PAIRS>
+__device__ __forceinline__ void symds_block(const SymDsParams &p, const float4 *__restrict__ qa, const float4 *__restrict__ qb,
+                                            const int jbase, const bool mixed, const float (&xh)[kDsI], const float (&yh)[kDsI],
+                                            const float (&zh)[kDsI], const float (&xl)[kDsI], const float (&yl)[kDsI],
+                                            const float (&zl)[kDsI], const float (&ngi)[kDsI], const float thr_lane, const int i0,
+                                            double (&AX)[kDsI], double (&AY)[kDsI], double (&AZ)[kDsI], double &bx, double &by,
+                                            double &bz) {
+    constexpr int I = kDsI;
+    const int lane = threadIdx.x & 31;
+    const int down = (lane + 1) & 31;
+    float ax[I], ay[I], az[I], fx = 0.0f, fy = 0.0f, fz = 0.0f;
+#pragma unroll
+    for (int k = 0; k < I; ++k) { ax[k] = 0.0f; ay[k] = 0.0f; az[k] = 0.0f; }
+    unsigned bits = 0u, rbit = 1u;
+    const float4 *__restrict__ la = qa + lane;
+    const float4 *__restrict__ lb = qb + lane;
+#pragma unroll 4
+    for (int r = 0; r < 32; ++r) {
+        const float4 a = la[r];
+        const float4 b = lb[r];
+        float dx[I], dy[I], dz[I], r2[I];
+        float mn = 3.0e38f;
+#pragma unroll
+        for (int k = 0; k < I; ++k) {
+            dx[k] = __fadd_rn(__fsub_rn(a.x, xh[k]), __fsub_rn(b.x, xl[k]));
+            dy[k] = __fadd_rn(__fsub_rn(a.y, yh[k]), __fsub_rn(b.y, yl[k]));
+            dz[k] = __fadd_rn(__fsub_rn(a.z, zh[k]), __fsub_rn(b.z, zl[k]));
+            r2[k] = __fmaf_rn(dz[k], dz[k], __fmaf_rn(dy[k], dy[k], __fmul_rn(dx[k], dx[k])));
+            mn = fminf(mn, r2[k]);
+        }
+        const bool hit = mn <= fmaxf(thr_lane, b.w);
+        if (hit) bits |= rbit;
+        rbit <<= 1;
+#pragma unroll
+        for (int k = 0; k < I; ++k) {
+            const float y0 = hit ? 0.0f : rsqrt_f32(r2[k]);   // a flagged lane's I pairs contribute exactly 0
+            const float y3 = __fmul_rn(__fmul_rn(y0, y0), y0);
+            const float si = __fmul_rn(y3, a.w);             // G m_j / r^3
+            const float sj = __fmul_rn(y3, ngi[k]);          // -G m_i / r^3
+            ax[k] = __fmaf_rn(si, dx[k], ax[k]); ay[k] = __fmaf_rn(si, dy[k], ay[k]); az[k] = __fmaf_rn(si, dz[k], az[k]);
+            fx = __fmaf_rn(sj, dx[k], fx); fy = __fmaf_rn(sj, dy[k], fy); fz = __fmaf_rn(sj, dz[k], fz);
+        }
+        fx = __shfl_sync(0xffffffffu, fx, down);
+        fy = __shfl_sync(0xffffffffu, fy, down);
+        fz = __shfl_sync(0xffffffffu, fz, down);
+    }
+    bx = (double)fx; by = (double)fy; bz = (double)fz;
+#pragma unroll
+    for (int k = 0; k < I; ++k) { AX[k] += (double)ax[k]; AY[k] += (double)ay[k]; AZ[k] += (double)az[k]; }
+
+    unsigned any = __reduce_or_sync(0xffffffffu, bits);
+    if (any == 0u) return;
+    // exact fp64 pass (rare): the lane's i-bodies from the fp64 staged arrays
+    const SymParams &sp = p.sp;
+    double xi[I], yi[I], zi[I], ngd[I];
+#pragma unroll
+    for (int k = 0; k < I; ++k) {
+        const size_t en = (size_t)((i0 >> 5) + k) * 64 + lane;
+        const double2 u = sp.sxy[en], w = sp.szg[en];
+        xi[k] = u.x; yi[k] = u.y; zi[k] = w.x; ngd[k] = -w.y;
+    }
+    while (any) {
+        const int r = __ffs(any) - 1;
+        any &= any - 1u;
+        const int src = (lane + r) & 31;
+        double cx = 0.0, cy = 0.0, cz = 0.0;
+        bool emit[I];
+#pragma unroll
+        for (int k = 0; k < I; ++k) emit[k] = false;
+        if ((bits >> r) & 1u) {
+            const int j = jbase + src;
+            const size_t ej = (size_t)(j >> 5) * 64 + (j & 31);
+            sym_exact<I, false>(sp, sp.sxy[ej], sp.szg[ej], sp.sthr[ej], j, mixed, xi, yi, zi, ngd, i0, AX, AY, AZ, cx, cy, cz, emit);
+        }
+        if (PAIRS) {
+#pragma unroll
+            for (int k = 0; k < I; ++k) pair_append(sp.pairs, sp.npairs, sp.status, sp.cap, emit[k], i0 + 32 * k, jbase + src);
+        }
+        const int from = (lane - r) & 31;
+        bx += __shfl_sync(0xffffffffu, cx, from);
+        by += __shfl_sync(0xffffffffu, cy, from);
+        bz += __shfl_sync(0xffffffffu, cz, from);
+    }
+}
+
+// One CTA of W warps per super-tile (A, B), A <= B, S = 128 W bodies a side: B staged once (two TMA bulk copies of the
+// float4 arrays), B's fp64 sums in shared memory, A's bodies in registers four per lane; diagonal tiles first.
+template <int W, bool PAIRS>
+__global__ void __launch_bounds__(32 * W) nb_force_symds_kernel(const SymDsParams p) {
+    constexpr int I = kDsI, kThreads = 32 * W;
+    extern __shared__ __align__(16) unsigned char symds_smem[];
+    const SymParams &sp = p.sp;
+    const int S = sp.S;
+    float4 *ba = reinterpret_cast<float4 *>(symds_smem);
+    float4 *bb = ba + 2 * S;
+    double *jsx = reinterpret_cast<double *>(bb + 2 * S);
+    double *jsy = jsx + S;
+    double *jsz = jsy + S;
+    uint64_t *bar = reinterpret_cast<uint64_t *>(jsz + S);
+    const int t = threadIdx.x, lane = t & 31, w = t >> 5;
+
+    const int T = sp.nsb;
+    int A, B;
+    if ((int)blockIdx.x < T) {
+        A = B = (int)blockIdx.x;
+    } else {
+        const long long idx = (long long)blockIdx.x - T;
+        B = (int)((1.0 + sqrt(1.0 + 8.0 * (double)idx)) * 0.5);
+        while ((long long)B * (B - 1) / 2 > idx) --B;
+        while ((long long)(B + 1) * B / 2 <= idx) ++B;
+        A = (int)(idx - (long long)B * (B - 1) / 2);
+    }
+    const bool diag = (A == B);
+    if (t == 0) {
+        mbar_init(bar, 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+        const unsigned bytes = (unsigned)S * 32u;            // 2 S float4
+        const size_t first = (size_t)B * S * 2;
+        mbar_expect_tx(bar, 2u * bytes);
+        tma_bulk_g2s(ba, p.sa + first, bytes, bar);
+        tma_bulk_g2s(bb, p.sb + first, bytes, bar);
+    }
+    for (int n = t; n < S; n += kThreads) { jsx[n] = 0.0; jsy[n] = 0.0; jsz[n] = 0.0; }
+    __syncthreads();
+    mbar_wait(bar, 0);
+
+    const int nunits = S / (32 * sp.U);
+    const int nchunks = S / (kThreads * I);
+    for (int c = 0; c < nchunks; ++c) {
+        const int P = (c * W + w) * I;
+        const int i0 = A * S + P * 32 + lane;
+        float xh[I], yh[I], zh[I], xl[I], yl[I], zl[I], ngi[I];
+        double AX[I], AY[I], AZ[I];
+        float thr_lane = 0.0f;
+#pragma unroll
+        for (int k = 0; k < I; ++k) {
+            const size_t en = (size_t)((i0 >> 5) + k) * 64 + lane;
+            const float4 a = p.sa[en], b = p.sb[en];
+            xh[k] = a.x; yh[k] = a.y; zh[k] = a.z; ngi[k] = -a.w;
+            xl[k] = b.x; yl[k] = b.y; zl[k] = b.z;
+            thr_lane = fmaxf(thr_lane, b.w);
+            AX[k] = 0.0; AY[k] = 0.0; AZ[k] = 0.0;
+        }
+        for (int step = 0; step < nunits; ++step) {
+            int unit = step + w;
+            if (unit >= nunits) unit -= nunits;
+            for (int uu = 0; uu < sp.U; ++uu) {
+                const int q = unit * sp.U + uu;
+                bool mixed = false;
+                if (diag) {
+                    if (q < P) continue;
+                    mixed = q < P + I;
+                }
+                double bx, by, bz;
+                symds_block<PAIRS>(p, ba + q * 64, bb + q * 64, B * S + q * 32, mixed, xh, yh, zh, xl, yl, zl, ngi, thr_lane, i0,
+                                   AX, AY, AZ, bx, by, bz);
+                if (!mixed) {
+                    const int n = q * 32 + lane;
+                    jsx[n] += bx; jsy[n] += by; jsz[n] += bz;
+                }
+            }
+            __syncthreads();
+        }
+        if (diag) {
+#pragma unroll
+            for (int k = 0; k < I; ++k) {
+                const int n = P * 32 + 32 * k + lane;
+                jsx[n] += AX[k]; jsy[n] += AY[k]; jsz[n] += AZ[k];
+            }
+            __syncthreads();
+        } else {
+            double *out = sp.part_i + (size_t)B * sp.stride_i * 3;
+#pragma unroll
+            for (int k = 0; k < I; ++k) {
+                const int i = i0 + 32 * k;
+                if (i < sp.N) { out[3 * (size_t)i] = AX[k]; out[3 * (size_t)i + 1] = AY[k]; out[3 * (size_t)i + 2] = AZ[k]; }
+            }
+        }
+    }
+    double *out = sp.part_j + (size_t)A * sp.stride_j * 3;
+    for (int n = t; n < S; n += kThreads) {
+        const long long g = (long long)B * S + n;
+        if (g < sp.N) { out[3 * g] = jsx[n]; out[3 * g + 1] = jsy[n]; out[3 * g + 2] = jsz[n]; }
+    }
+}
+
+}  // namespace nbk

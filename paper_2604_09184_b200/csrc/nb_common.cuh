@@ -25,6 +25,19 @@ __device__ __forceinline__ double pack_mixed(const double gm, const double rc2) 
     return __hiloint2double(__float_as_int(t), __float_as_int(g));
 }
 
+// stages body `pos` (position in the doubled-block layout) for the Newton-III mixed-precision kernel (force_symds.cuh):
+// double-single position (xh + xl), fl32(G m), and rc^2 rounded up with a 2^-18 margin; called by nb_prep_kernel
+__device__ __forceinline__ void symds_stage(float4 *sa, float4 *sb, const int pos, const double x, const double y, const double z,
+                                            const double gm, const double rc2) {
+    const float xh = __double2float_rn(x), yh = __double2float_rn(y), zh = __double2float_rn(z);
+    const float xl = __double2float_rn(x - (double)xh), yl = __double2float_rn(y - (double)yh), zl = __double2float_rn(z - (double)zh);
+    const float thr = __double2float_ru(rc2) * 1.0000038f;
+    const size_t en = (size_t)(pos >> 5) * 64 + (pos & 31);
+    const float4 a = make_float4(xh, yh, zh, __double2float_rn(gm)), b = make_float4(xl, yl, zl, thr);
+    sa[en] = a; sa[en + 32] = a;
+    sb[en] = b; sb[en + 32] = b;
+}
+
 constexpr int kForceThreads = 128;  // threads per force CTA
 constexpr int kTileJ = 128;         // j-bodies per shared-memory stage (8 KB)
 constexpr int kStages = 4;          // TMA ring depth (2 tiles in flight ahead of the consumer)

@@ -14,6 +14,7 @@
 #include "encounter.cuh"
 #include "force_mixed.cuh"
 #include "force_sym.cuh"
+#include "force_symds.cuh"
 #include "force_tiles.cuh"
 #include "groups.cuh"
 #include "merge.cuh"
@@ -122,6 +123,23 @@ Geometry geometry(int64_t N, int64_t n_active) {
     // Newton-III kernel: fully active case only (a passive body exerts nothing, so there is no second
     // side to serve), and only when there are enough super-tiles to fill the machine several times.
     const bool fully_active = (g.Nj == N);
+    if (fully_active && g.mixed && g_cfg.force_kernel != NB_FORCE_TILES && (g_cfg.force_kernel == NB_FORCE_SYMMETRIC || N >= kSymMinN)) {
+        // Newton-III mixed-precision kernel (force_symds.cuh): I = 4, CTAs of 1 / 2 / 4 warps chosen as for the fp64 kernel;
+        // no sorted staging, tail splitting or bands -- where the slots would pass the cap the one-sided mixed kernel runs
+        auto waves = [&](int s) {
+            const int64_t T = (N + s - 1) / s;
+            return (double)(T * (T + 1) / 2) / (double)((int64_t)sms * (1536 / s));
+        };
+        int S = g_cfg.sym_block;
+        if (S != 128 && S != 256 && S != 512) S = waves(512) >= 16.0 ? 512 : (waves(256) >= 5.0 ? 256 : 128);
+        const int64_t Npad = ((N + S - 1) / S) * S, T = Npad / S;
+        const int64_t cap = g_cfg.slot_bytes_max > 0 ? g_cfg.slot_bytes_max : ((int64_t)4 << 30);
+        if (T * N * 24 <= cap) {
+            g.sym = 1; g.mixed = 2; g.S = S; g.U = S / 128; g.ipt = 4; g.warps = S / 128; g.minb = 12 / g.warps;
+            g.Npad_sym = (int)Npad; g.nsplit = (int)T; g.iblocks = (int)T; g.tiles_per_split = 0; g.nslots = (int)T;
+            return g;
+        }
+    }
     if (fully_active && !g.mixed && g_cfg.force_kernel != NB_FORCE_TILES && (g_cfg.force_kernel == NB_FORCE_SYMMETRIC || N >= kSymMinN)) {
         // I = 4 at 12 warps per SM (160 registers, no spills) measured fastest on B200.
         // The CTA shrinks with the super-block -- 4 warps for S >= 512, 2 for S = 256, 1 for S = 128 -- so that a
@@ -241,6 +259,7 @@ struct Workspace {
     JRec *jrec;         // [Njpad]                 (one-sided kernel)
     double2 *sxy, *szg; // [2 Npad_sym]            (symmetric kernel, doubled-block layout)
     int *sthr;          // [2 Npad_sym]
+    float4 *sa, *sb;    // [2 Npad_sym]            (Newton-III mixed-precision kernel: double-single records)
     int *perm, *pos_of; // [Npad_sym], [N]         (sorted staging: position <-> body)
     BlockBound *bnd;    // [nsplit]                (bounds of the staged super-blocks)
     double *part;       // [nsplit, N, 3]
@@ -305,6 +324,8 @@ Workspace carve(void *base, int64_t N, const Geometry &g) {
     w.sxy = reinterpret_cast<double2 *>(b + off); off += align_up((size_t)2 * g.Npad_sym * sizeof(double2), 256);
     w.szg = reinterpret_cast<double2 *>(b + off); off += align_up((size_t)2 * g.Npad_sym * sizeof(double2), 256);
     w.sthr = reinterpret_cast<int *>(b + off); off += align_up((size_t)2 * g.Npad_sym * sizeof(int), 256);
+    w.sa = reinterpret_cast<float4 *>(b + off); off += align_up((size_t)(g.mixed == 2 ? 2 * g.Npad_sym : 0) * sizeof(float4), 256);
+    w.sb = reinterpret_cast<float4 *>(b + off); off += align_up((size_t)(g.mixed == 2 ? 2 * g.Npad_sym : 0) * sizeof(float4), 256);
     w.perm = reinterpret_cast<int *>(b + off); off += align_up((size_t)g.Npad_sym * sizeof(int), 256);
     w.pos_of = reinterpret_cast<int *>(b + off); off += align_up((size_t)(g.sym ? N : 0) * sizeof(int), 256);
     w.bnd = reinterpret_cast<BlockBound *>(b + off); off += align_up((size_t)(g.sym ? g.nsplit : 0) * sizeof(BlockBound), 256);
@@ -406,6 +427,27 @@ int launch_sym_IM(const SymParams &sp, const Geometry &g, bool pairs) {
     return g.sorted ? launch_sym_IMS<I, W, MINB, true>(sp, g, pairs) : launch_sym_IMS<I, W, MINB, false>(sp, g, pairs);
 }
 
+template <int W>
+int launch_symds_W(const SymDsParams &dp, const Geometry &g, bool pairs) {
+    const long long T = g.nsplit;
+    const unsigned ctas = (unsigned)(T * (T + 1) / 2);
+    const size_t smem = symds_smem_bytes(g.S);
+    auto go = [&](auto kern) -> int {
+        NB_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        kern<<<ctas, 32 * W, smem, stream()>>>(dp);
+        return NB_OK;
+    };
+    return pairs ? go(nb_force_symds_kernel<W, true>) : go(nb_force_symds_kernel<W, false>);
+}
+
+int launch_symds(const SymParams &sp, const Workspace &w, const Geometry &g, bool pairs) {
+    SymDsParams dp;
+    dp.sp = sp; dp.sa = w.sa; dp.sb = w.sb;
+    if (g.warps == 4) return launch_symds_W<4>(dp, g, pairs);
+    if (g.warps == 2) return launch_symds_W<2>(dp, g, pairs);
+    return launch_symds_W<1>(dp, g, pairs);
+}
+
 int launch_sym(const SymParams &sp, const Geometry &g, bool pairs) {
     if (g.ipt == 4 && g.warps == 4) return launch_sym_IM<4, 4, 3>(sp, g, pairs);
     if (g.ipt == 4 && g.warps == 2) return launch_sym_IM<4, 2, 6>(sp, g, pairs);
@@ -445,12 +487,13 @@ int enqueue_eval(const Workspace &w, const Geometry &g, double *x, double *v, co
     PrepParams pp;
     pp.x = x; pp.v = v; pp.m = m; pp.rcrit = rc_io; pp.jrec = g.sym ? nullptr : w.jrec; pp.mv_in = mv_in;
     pp.sxy = g.sym ? w.sxy : nullptr; pp.szg = w.szg; pp.sthr = w.sthr; pp.Npad_sym = g.Npad_sym;
+    pp.sa = g.mixed == 2 ? w.sa : nullptr; pp.sb = w.sb;
     pp.pos_of = sorted ? w.pos_of : nullptr;
     pp.rc_hill = g_cfg.levels > 0 ? w.ml_hill : nullptr; pp.rc_vel = g_cfg.levels > 0 ? w.ml_vel : nullptr;
     pp.npairs = pairs ? reinterpret_cast<unsigned long long *>(npairs) : nullptr;
     pp.status = w.status; pp.dtc = dtc; pp.M_star = M_star; pp.G = g_cfg.G; pp.n1 = g_cfg.n1; pp.n2 = g_cfg.n2;
     pp.absdt = std::fabs(dt_for_rc); pp.nblk_in = nblk; pp.N = (int)N; pp.Nj = g.Nj; pp.Njpad = g.Njpad;
-    pp.update_rc = update_rc; pp.mixed = g.mixed;
+    pp.update_rc = update_rc; pp.mixed = g.mixed == 1;
     int64_t cover = N > g.Njpad ? N : g.Njpad;
     if (g.Npad_sym > cover) cover = g.Npad_sym;
     nb_prep_kernel<<<body_blocks(cover), kBodyThreads, 0, stream()>>>(pp);
@@ -482,7 +525,7 @@ int enqueue_eval(const Workspace &w, const Geometry &g, double *x, double *v, co
         sp.U = g.U; sp.kind = g_cfg.changeover_kind; sp.xcols = g.xcols;
         if (g.band == 0) {
             sp.part_i = w.part; sp.part_j = w.part; sp.stride_i = N; sp.stride_j = N; sp.goff = 0; sp.col0 = 0; sp.ncols = g.nsplit;
-            const int lrc = launch_sym(sp, g, pairs != nullptr);
+            const int lrc = g.mixed == 2 ? launch_symds(sp, w, g, pairs != nullptr) : launch_sym(sp, g, pairs != nullptr);
             if (lrc) return lrc;
         } else {
             // banded: i sides [band][N], then the j sides of the band's bodies [nsb][band S]; folded into acc band by band
@@ -693,6 +736,7 @@ int launch_step_small(const Workspace &w, const Geometry &g, double *x, double *
     PrepParams &pp = q.pp;
     pp.x = x; pp.v = v; pp.m = m; pp.rcrit = rc_io; pp.rc_hill = nullptr; pp.rc_vel = nullptr; pp.jrec = w.jrec;
     pp.sxy = nullptr; pp.szg = nullptr; pp.sthr = nullptr; pp.Npad_sym = 0; pp.pos_of = nullptr; pp.mv_in = nullptr;
+    pp.sa = nullptr; pp.sb = nullptr;
     pp.npairs = pairs ? reinterpret_cast<unsigned long long *>(npairs) : nullptr;
     pp.status = w.status; pp.dtc = 0.5 * dt; pp.M_star = M_star; pp.G = g_cfg.G; pp.n1 = g_cfg.n1; pp.n2 = g_cfg.n2;
     pp.absdt = std::fabs(dt); pp.nblk_in = body_blocks(N); pp.N = (int)N; pp.Nj = g.Nj; pp.Njpad = g.Njpad;

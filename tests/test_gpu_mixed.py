@@ -46,6 +46,28 @@ def _numpy_mixed(x, m, rc, G, rows):
 @pytest.mark.parametrize("cfg,n_override,n2,tune", [(2, 6000, 0.0, {}), (1, 5000, 0.4, dict(i_per_thread=4)), (3, 8192, 0.0, {}),
                                                     (0, 2048, 0.4, dict(i_per_thread=1, j_splits=3))])
 def test_mixed_kick_against_fp64_oracle(cfg, n_override, n2, tune):
+    _mixed_case(cfg, n_override, n2, tune, 1, BOUND)
+
+
+# Newton-III mixed-precision kernel (force_symds.cuh): double-single differences on the FP32 pipe.  Per term: the
+# difference 2.5 u, r^2 another 3 u on top of twice that, MUFU.RSQ 2 u, its cube, the mass (cast + product) and the
+# product with the difference: at most ~24 u; fp32 sums over one visit of a 32-body block: at most 127 u of the visit's
+# sum of |terms| on the j side (128 terms), 31 u on the i side.  Guaranteed: 151 u sum|t| (S25).
+BOUND_DS = 151 * U32
+
+
+@pytest.mark.parametrize("cfg,n_override,n2,tune", [(2, 6000, 0.0, {}),                                   # auto: S = 128, 1-warp CTAs
+                                                    (1, 5000, 0.4, dict(sym_block=256)),                   # giants, Eq. 7 radius, 2-warp CTAs
+                                                    (2, 8193, 0.4, dict(sym_block=512)),                   # ragged tail, 4-warp CTAs
+                                                    (0, 700, 0.4, dict(force_kernel=2, sym_block=128))])   # forced below the threshold
+def test_mixed_newton3_kick_against_fp64_oracle(cfg, n_override, n2, tune):
+    tune = dict(tune)
+    fk = tune.pop("force_kernel", 0)
+    geo = _mixed_case(cfg, n_override, n2, tune, fk, BOUND_DS)
+    assert geo.tile_j < 0 and geo.i_per_thread == 4               # the Newton-III kernel really ran
+
+
+def _mixed_case(cfg, n_override, n2, tune, force_kernel, bound):
     d = nb_inputs.make_config(cfg, n_override=n_override)
     na = d.n_active if d.n_active < d.N else 0
     rc = oracle.rcrit(d.x, d.v, d.m, d.M_star, d.dt, G_GAUSS, 3.0, n2)
@@ -53,7 +75,9 @@ def test_mixed_kick_against_fp64_oracle(cfg, n_override, n2, tune):
     sure, border = oracle.pairs(d.x, rc, n_active=na)
     res = {}
     for prec in (0, 1):
-        st = GpuState(d.x, d.v, d.m, d.M_star, G=G_GAUSS, n_active=na, n1=3.0, n2=n2, precision=prec, force_kernel=1, **tune)
+        st = GpuState(d.x, d.v, d.m, d.M_star, G=G_GAUSS, n_active=na, n1=3.0, n2=n2, precision=prec, force_kernel=force_kernel, **tune)
+        if prec == 1:
+            geo = st.nb.force_geometry(d.N)
         st.set_rcrit(rc)
         st.kick(0.5 * d.dt)
         _, vg, acc, _ = st.host()
@@ -68,8 +92,8 @@ def test_mixed_kick_against_fp64_oracle(cfg, n_override, n2, tune):
     worst = float(np.max(err / np.where(ab > 0, ab, 1e-300)))
     rel = err / np.maximum(np.abs(ref), 1e-3 * np.linalg.norm(ref, axis=1, keepdims=True))
     print(f"{d.name}: mixed vs fp64 oracle: worst |da| / sum|t| = {worst / U32:.1f} u (bound 143 u), relative error median "
-          f"{np.median(rel):.2e} max {rel.max():.2e}; fp64 kernel max {np.max(np.abs(res[0][0] - ref) / np.where(ab > 0, ab, 1e-300)) / 2.2e-16:.1f} eps")
-    assert worst <= BOUND
+          f"{np.median(rel):.2e} max {rel.max():.2e} [{geo}]; fp64 kernel max {np.max(np.abs(res[0][0] - ref) / np.where(ab > 0, ab, 1e-300)) / 2.2e-16:.1f} eps")
+    assert worst <= bound
     assert np.median(rel) <= 3e-7
     # v kicked with those accelerations
     assert np.max(np.abs(res[1][1] - (d.v + 0.5 * d.dt * acc))) <= 1e-15 * np.max(np.abs(d.v))
@@ -93,12 +117,22 @@ def test_mixed_kick_against_fp64_oracle(cfg, n_override, n2, tune):
         e_gpu = err[rows] / ab[rows]
         print(f"   numpy fp32 restatement: median {np.median(e_np) / U32:.2f} u, max {e_np.max() / U32:.2f} u;  kernel: median {np.median(e_gpu) / U32:.2f} u, max {e_gpu.max() / U32:.2f} u")
         assert np.median(e_gpu) <= 4 * np.median(e_np) + U32
+    return geo
 
 
 def test_mixed_step_energy_and_state():
     """20 steps of the N = 3000 ring in mixed precision: the state follows the fp64 oracle run to ~1e-7, the energy error
     stays of the size the fp32 force error allows."""
-    d = nb_inputs.make_config(2, n_override=3000)
+    _mixed_step(3000)
+
+
+def test_mixed_newton3_step_energy_and_state():
+    """The same through the Newton-III mixed-precision kernel (N = 6000: auto), graph replay included."""
+    _mixed_step(6000)
+
+
+def _mixed_step(n):
+    d = nb_inputs.make_config(2, n_override=n)
     st = GpuState(d.x, d.v, d.m, d.M_star, G=G_GAUSS, n1=3.0, n2=0.0, precision=1)
     st.step(d.dt, 20)
     xg, vg, _, _ = st.host()
