@@ -60,10 +60,14 @@ extern "C" {
  *   NB_FORCE_AUTO       symmetric when fully active and N >= 4096, else tiles. */
 /* Arithmetic of the O(N^2) sum (PAPER.md:160 contrasts FP32 and FP64 runs):
  *   NB_PRECISION_F64    everything in fp64 (default; the north_star's 1e-12 tolerance applies)
- *   NB_PRECISION_MIXED  pairs out of reach of every critical radius: differences in fp64, r^2, r^-3 and the products
- *                       in fp32, summed in fp32 per 128-body tile and in fp64 across tiles; pairs within reach, the
+ *   NB_PRECISION_MIXED  pairs out of reach of every critical radius are evaluated in fp32; pairs within reach, the
  *                       changeover weight, the pair test and the pair list stay in fp64 and are identical to the fp64
- *                       kernel's.  Tolerance: DESIGN.md reading S25 (~1e-6 relative).  One-sided kernel, any n_active. */
+ *                       kernel's.  Tolerance: DESIGN.md reading S25 (~1e-7 relative, typically).  Two kernels:
+ *                       fully active, N >= 4096 (or NB_FORCE_SYMMETRIC), slots within slot_bytes_max: the Newton-III
+ *                       kernel on double-single positions -- differences fl(fl(xjh - xih) + fl(xjl - xil)), r^2, r^-3,
+ *                       products and the sums over one visit of a 32-body block all on the FP32 pipe, fp64 from there on;
+ *                       otherwise (semi-active, small N, NB_FORCE_TILES): the one-sided kernel -- differences in fp64,
+ *                       the rest in fp32, summed in fp32 per 128-body tile and in fp64 across tiles. */
 #define NB_PRECISION_F64 0
 #define NB_PRECISION_MIXED 1
 #define NB_SORT_AUTO 0

@@ -8,8 +8,10 @@
 //     the low parts restore what fl32(x) lost -- no fp64 subtraction, no conversion;
 //   * r^2, MUFU.RSQ, its cube, the two mass products, six FFMA: 22 FP32 instructions per UNORDERED pair, both sides
 //     served (the fp64 kernel: 20 FP64 instructions, on a pipe half as wide);
-//   * the j-sums travel through the warp as in force_sym.cuh (3 SHFL per rotation instead of 6); fp32 sums over ONE
-//     visit of a 32-body block (32 terms on the i side, 128 on the j side), fp64 from there on.
+//   * the j-sums travel through the warp as in force_sym.cuh; fp32 sums over ONE visit of a 32-body block (32 terms on
+//     the i side, 64 + 64 on the j side), fp64 from there on;
+//   * packed fp32x2 instructions (FADD2 / FMUL2 / FFMA2) wherever two values take the same operation: the kernel is
+//     bound by instruction issue.
 // Pairs whose fp32 r^2 is within reach of a critical radius (margin 2^-18: far above the fp32 rounding of r^2), and
 // every self term, are killed in the fp32 loop (rsqrt replaced by 0: they contribute exactly 0 to both sides) and
 // re-evaluated by the EXACT fp64 pass of force_sym.cuh (sym_exact) from the fp64 staged arrays: the changeover weight,
@@ -23,8 +25,8 @@ namespace nbk {
 
 struct SymDsParams {
     SymParams sp;      // fp64 staged arrays (exact pass), slots, pair list, geometry: as nb_force_sym_kernel, unsorted
-    const float4 *sa;  // [2 Npad] (xh, yh, zh, fl32(G m))              doubled-block layout
-    const float4 *sb;  // [2 Npad] (xl, yl, zl, rc^2 (1 + 2^-18) rounded up)
+    const float4 *sa;  // [2 Npad] (xh, xl, yh, yl)                                  doubled-block layout
+    const float4 *sb;  // [2 Npad] (zh, zl, fl32(G m), rc^2 (1 + 2^-18) rounded up)
 };
 
 constexpr int kDsI = 4;   // i-bodies per lane
@@ -38,55 +40,71 @@ __device__ __forceinline__ float rsqrt_f32(const float a) {
 
 // One warp, one block of 32 j-bodies, 32 rotations in fp32; then the exact fp64 pass for the flagged rotations.
 // On return lane l holds in (bx,by,bz) the fp64 sums for j = jbase + l; the i-side sums of the visit are ADDED to AX/AY/AZ.
+// The kernel is bound by instruction issue, not by the FP32 pipe (ncu: issue slots 79 % busy, FMA pipe 62 %, with scalar
+// instructions), so the arithmetic is written with the packed fp32x2 instructions of sm_100 (FADD2 / FMUL2 / FFMA2: two
+// lanes per issue slot, each rounded as the scalar instruction would): the (high, low) partial differences of a coordinate
+// in one FADD2, everything after the differences on two i-bodies at a time.  nxa/nya/nza: the lane's i-bodies, NEGATED,
+// as (high, low) pairs; ngi2: -G m_i of bodies (2g, 2g+1).
 template <bool PAIRS>
 __device__ __forceinline__ void symds_block(const SymDsParams &p, const float4 *__restrict__ qa, const float4 *__restrict__ qb,
-                                            const int jbase, const bool mixed, const float (&xh)[kDsI], const float (&yh)[kDsI],
-                                            const float (&zh)[kDsI], const float (&xl)[kDsI], const float (&yl)[kDsI],
-                                            const float (&zl)[kDsI], const float (&ngi)[kDsI], const float thr_lane, const int i0,
-                                            double (&AX)[kDsI], double (&AY)[kDsI], double (&AZ)[kDsI], double &bx, double &by,
-                                            double &bz) {
-    constexpr int I = kDsI;
+                                            const int jbase, const bool mixed, const float2 (&nxa)[kDsI], const float2 (&nya)[kDsI],
+                                            const float2 (&nza)[kDsI], const float2 (&ngi2)[kDsI / 2], const float thr_lane,
+                                            const int i0, double (&AX)[kDsI], double (&AY)[kDsI], double (&AZ)[kDsI], double &bx,
+                                            double &by, double &bz) {
+    constexpr int I = kDsI, H = kDsI / 2;
     const int lane = threadIdx.x & 31;
     const int down = (lane + 1) & 31;
-    float ax[I], ay[I], az[I], fx = 0.0f, fy = 0.0f, fz = 0.0f;
+    float2 ax[H], ay[H], az[H];                       // i-side sums of bodies (2g, 2g+1)
+    float2 fx = make_float2(0.0f, 0.0f), fy = fx, fz = fx;   // travelling j-side sums: even and odd i-bodies apart
 #pragma unroll
-    for (int k = 0; k < I; ++k) { ax[k] = 0.0f; ay[k] = 0.0f; az[k] = 0.0f; }
+    for (int g = 0; g < H; ++g) { ax[g] = make_float2(0.0f, 0.0f); ay[g] = ax[g]; az[g] = ax[g]; }
     unsigned bits = 0u, rbit = 1u;
     const float4 *__restrict__ la = qa + lane;
     const float4 *__restrict__ lb = qb + lane;
+    const float kInf = __int_as_float(0x7f800000);
 #pragma unroll 4
     for (int r = 0; r < 32; ++r) {
-        const float4 a = la[r];
-        const float4 b = lb[r];
-        float dx[I], dy[I], dz[I], r2[I];
-        float mn = 3.0e38f;
+        const float4 a = la[r];                       // (xh, xl, yh, yl)
+        const float4 b = lb[r];                       // (zh, zl, G m, threshold)
+        const float2 jx = make_float2(a.x, a.y), jy = make_float2(a.z, a.w), jz = make_float2(b.x, b.y);
+        float2 dx[H], dy[H], dz[H], r2[H];
 #pragma unroll
-        for (int k = 0; k < I; ++k) {
-            dx[k] = __fadd_rn(__fsub_rn(a.x, xh[k]), __fsub_rn(b.x, xl[k]));
-            dy[k] = __fadd_rn(__fsub_rn(a.y, yh[k]), __fsub_rn(b.y, yl[k]));
-            dz[k] = __fadd_rn(__fsub_rn(a.z, zh[k]), __fsub_rn(b.z, zl[k]));
-            r2[k] = __fmaf_rn(dz[k], dz[k], __fmaf_rn(dy[k], dy[k], __fmul_rn(dx[k], dx[k])));
-            mn = fminf(mn, r2[k]);
+        for (int g = 0; g < H; ++g) {
+            const float2 x0 = __fadd2_rn(jx, nxa[2 * g]), x1 = __fadd2_rn(jx, nxa[2 * g + 1]);
+            const float2 y0 = __fadd2_rn(jy, nya[2 * g]), y1 = __fadd2_rn(jy, nya[2 * g + 1]);
+            const float2 z0 = __fadd2_rn(jz, nza[2 * g]), z1 = __fadd2_rn(jz, nza[2 * g + 1]);
+            dx[g] = make_float2(__fadd_rn(x0.x, x0.y), __fadd_rn(x1.x, x1.y));
+            dy[g] = make_float2(__fadd_rn(y0.x, y0.y), __fadd_rn(y1.x, y1.y));
+            dz[g] = make_float2(__fadd_rn(z0.x, z0.y), __fadd_rn(z1.x, z1.y));
+            r2[g] = __ffma2_rn(dz[g], dz[g], __ffma2_rn(dy[g], dy[g], __fmul2_rn(dx[g], dx[g])));
         }
+        float mn = fminf(r2[0].x, r2[0].y);
+#pragma unroll
+        for (int g = 1; g < H; ++g) mn = fminf(mn, fminf(r2[g].x, r2[g].y));
         const bool hit = mn <= fmaxf(thr_lane, b.w);
         if (hit) bits |= rbit;
         rbit <<= 1;
+        const float kill = hit ? kInf : 0.0f;         // rsqrt(+inf) = 0: a flagged lane's I pairs contribute exactly 0
+        const float2 gmj = make_float2(b.z, b.z);
 #pragma unroll
-        for (int k = 0; k < I; ++k) {
-            const float y0 = hit ? 0.0f : rsqrt_f32(r2[k]);   // a flagged lane's I pairs contribute exactly 0
-            const float y3 = __fmul_rn(__fmul_rn(y0, y0), y0);
-            const float si = __fmul_rn(y3, a.w);             // G m_j / r^3
-            const float sj = __fmul_rn(y3, ngi[k]);          // -G m_i / r^3
-            ax[k] = __fmaf_rn(si, dx[k], ax[k]); ay[k] = __fmaf_rn(si, dy[k], ay[k]); az[k] = __fmaf_rn(si, dz[k], az[k]);
-            fx = __fmaf_rn(sj, dx[k], fx); fy = __fmaf_rn(sj, dy[k], fy); fz = __fmaf_rn(sj, dz[k], fz);
+        for (int g = 0; g < H; ++g) {
+            const float2 y0 = make_float2(rsqrt_f32(fmaxf(r2[g].x, kill)), rsqrt_f32(fmaxf(r2[g].y, kill)));
+            const float2 y3 = __fmul2_rn(__fmul2_rn(y0, y0), y0);
+            const float2 si = __fmul2_rn(y3, gmj);            // G m_j / r^3
+            const float2 sj = __fmul2_rn(y3, ngi2[g]);        // -G m_i / r^3
+            ax[g] = __ffma2_rn(si, dx[g], ax[g]); ay[g] = __ffma2_rn(si, dy[g], ay[g]); az[g] = __ffma2_rn(si, dz[g], az[g]);
+            fx = __ffma2_rn(sj, dx[g], fx); fy = __ffma2_rn(sj, dy[g], fy); fz = __ffma2_rn(sj, dz[g], fz);
         }
-        fx = __shfl_sync(0xffffffffu, fx, down);
-        fy = __shfl_sync(0xffffffffu, fy, down);
-        fz = __shfl_sync(0xffffffffu, fz, down);
+        fx.x = __shfl_sync(0xffffffffu, fx.x, down); fx.y = __shfl_sync(0xffffffffu, fx.y, down);
+        fy.x = __shfl_sync(0xffffffffu, fy.x, down); fy.y = __shfl_sync(0xffffffffu, fy.y, down);
+        fz.x = __shfl_sync(0xffffffffu, fz.x, down); fz.y = __shfl_sync(0xffffffffu, fz.y, down);
     }
-    bx = (double)fx; by = (double)fy; bz = (double)fz;
+    bx = (double)fx.x + (double)fx.y; by = (double)fy.x + (double)fy.y; bz = (double)fz.x + (double)fz.y;
 #pragma unroll
-    for (int k = 0; k < I; ++k) { AX[k] += (double)ax[k]; AY[k] += (double)ay[k]; AZ[k] += (double)az[k]; }
+    for (int g = 0; g < H; ++g) {
+        AX[2 * g] += (double)ax[g].x; AY[2 * g] += (double)ay[g].x; AZ[2 * g] += (double)az[g].x;
+        AX[2 * g + 1] += (double)ax[g].y; AY[2 * g + 1] += (double)ay[g].y; AZ[2 * g + 1] += (double)az[g].y;
+    }
 
     unsigned any = __reduce_or_sync(0xffffffffu, bits);
     if (any == 0u) return;
@@ -126,7 +144,7 @@ __device__ __forceinline__ void symds_block(const SymDsParams &p, const float4 *
 // One CTA of W warps per super-tile (A, B), A <= B, S = 128 W bodies a side: B staged once (two TMA bulk copies of the
 // float4 arrays), B's fp64 sums in shared memory, A's bodies in registers four per lane; diagonal tiles first.
 template <int W, bool PAIRS>
-__global__ void __launch_bounds__(32 * W) nb_force_symds_kernel(const SymDsParams p) {
+__global__ void __launch_bounds__(32 * W, 16 / W) nb_force_symds_kernel(const SymDsParams p) {
     constexpr int I = kDsI, kThreads = 32 * W;
     extern __shared__ __align__(16) unsigned char symds_smem[];
     const SymParams &sp = p.sp;
@@ -170,18 +188,21 @@ __global__ void __launch_bounds__(32 * W) nb_force_symds_kernel(const SymDsParam
     for (int c = 0; c < nchunks; ++c) {
         const int P = (c * W + w) * I;
         const int i0 = A * S + P * 32 + lane;
-        float xh[I], yh[I], zh[I], xl[I], yl[I], zl[I], ngi[I];
+        float2 nxa[I], nya[I], nza[I], ngi2[I / 2];
+        float ngi[I];
         double AX[I], AY[I], AZ[I];
         float thr_lane = 0.0f;
 #pragma unroll
         for (int k = 0; k < I; ++k) {
             const size_t en = (size_t)((i0 >> 5) + k) * 64 + lane;
             const float4 a = p.sa[en], b = p.sb[en];
-            xh[k] = a.x; yh[k] = a.y; zh[k] = a.z; ngi[k] = -a.w;
-            xl[k] = b.x; yl[k] = b.y; zl[k] = b.z;
+            nxa[k] = make_float2(-a.x, -a.y); nya[k] = make_float2(-a.z, -a.w); nza[k] = make_float2(-b.x, -b.y);
+            ngi[k] = -b.z;
             thr_lane = fmaxf(thr_lane, b.w);
             AX[k] = 0.0; AY[k] = 0.0; AZ[k] = 0.0;
         }
+#pragma unroll
+        for (int g = 0; g < I / 2; ++g) ngi2[g] = make_float2(ngi[2 * g], ngi[2 * g + 1]);
         for (int step = 0; step < nunits; ++step) {
             int unit = step + w;
             if (unit >= nunits) unit -= nunits;
@@ -193,8 +214,7 @@ __global__ void __launch_bounds__(32 * W) nb_force_symds_kernel(const SymDsParam
                     mixed = q < P + I;
                 }
                 double bx, by, bz;
-                symds_block<PAIRS>(p, ba + q * 64, bb + q * 64, B * S + q * 32, mixed, xh, yh, zh, xl, yl, zl, ngi, thr_lane, i0,
-                                   AX, AY, AZ, bx, by, bz);
+                symds_block<PAIRS>(p, ba + q * 64, bb + q * 64, B * S + q * 32, mixed, nxa, nya, nza, ngi2, thr_lane, i0, AX, AY, AZ, bx, by, bz);
                 if (!mixed) {
                     const int n = q * 32 + lane;
                     jsx[n] += bx; jsy[n] += by; jsz[n] += bz;

@@ -33,7 +33,8 @@ __device__ __forceinline__ void symds_stage(float4 *sa, float4 *sb, const int po
     const float xl = __double2float_rn(x - (double)xh), yl = __double2float_rn(y - (double)yh), zl = __double2float_rn(z - (double)zh);
     const float thr = __double2float_ru(rc2) * 1.0000038f;
     const size_t en = (size_t)(pos >> 5) * 64 + (pos & 31);
-    const float4 a = make_float4(xh, yh, zh, __double2float_rn(gm)), b = make_float4(xl, yl, zl, thr);
+    // (high, low) of a coordinate sit side by side: one packed fp32x2 add forms both partial differences
+    const float4 a = make_float4(xh, xl, yh, yl), b = make_float4(zh, zl, __double2float_rn(gm), thr);
     sa[en] = a; sa[en + 32] = a;
     sb[en] = b; sb[en + 32] = b;
 }
