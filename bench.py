@@ -52,6 +52,7 @@ def parse_args():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-drift-point", action="store_true", help="skip the N = 2^24 drift-only HBM point")
+    ap.add_argument("--no-mixed-point", action="store_true", help="skip the mixed-precision side line (fully active configs)")
     ap.add_argument("--force-kernel", type=int, default=0, choices=[0, 1, 2],
                     help="nb_config.force_kernel: 0 auto, 1 one-sided tiles, 2 Newton-III (comparison runs)")
     ap.add_argument("--j-splits", type=int, default=0,
@@ -273,6 +274,41 @@ def drift_roofline(d, n_bodies=1 << 24, launches=5):
                 bodies_per_sec=n_bodies / (ms * 1e-3))
 
 
+def mixed_point(d, launches=10):
+    """Side line (PAPER.md:160 contrasts FP32 and FP64 runs): the same kick in NB_PRECISION_MIXED
+    (fully active N >= 4096: Newton-III kernel on double-single positions, FP32 pipe), nb_kick timed alone with CUDA
+    events, and its error against the fp64 kernel's accelerations on the same input (reading S25).  Not the metric."""
+    import torch
+    import paper_2604_09184_b200 as nb
+    N = d.N
+    x = torch.from_numpy(d.x).cuda(); v = torch.from_numpy(d.v).cuda(); m = torch.from_numpy(d.m).cuda()
+    rc = torch.zeros(N, dtype=torch.float64, device="cuda")
+    out = {}
+    for prec in (0, 1):
+        nb.configure(N, G=G_GAUSS, n1=N1, n2=N2, precision=prec)
+        nb.nb_rcrit(x, v, m, d.M_star, d.dt, rc)
+        acc = torch.zeros_like(x)
+        for _ in range(2):
+            nb.nb_kick(x, v, m, d.M_star, 0.0, rc, acc)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize()
+        e0.record()
+        for _ in range(launches):
+            nb.nb_kick(x, v, m, d.M_star, 0.0, rc, acc)
+        e1.record()
+        torch.cuda.synchronize()
+        out[prec] = (e0.elapsed_time(e1) / launches, acc, nb.force_geometry(N))
+    a64, a32 = out[0][1], out[1][1]
+    scale = torch.clamp(a64.abs(), min=1e-3 * float(a64.norm(dim=1).max()))
+    rel = ((a32 - a64).abs() / scale)
+    g = out[1][2]
+    return dict(precision="NB_PRECISION_MIXED", kernel="nb_force_symds_kernel" if g.tile_j < 0 else "nb_force_mixed_kernel",
+                ms_per_kick=out[1][0], interactions_per_sec=float(N) * float(N) / (out[1][0] * 1e-3),
+                ms_per_kick_f64=out[0][0], speedup_vs_f64=out[0][0] / out[1][0],
+                rel_err_vs_f64_median=float(rel.median()), rel_err_vs_f64_max=float(rel.max()),
+                note="whole nb_kick (staging + force + slot sum), no L2 flush; tolerance reading S25 (DESIGN.md)")
+
+
 def max_over_ranks(values, device="cuda"):
     """Replicas only: the single cross-rank step of the benchmark is this MAX over the ranks' timings (no
     data-path collective).  Works with any initialised backend (nccl on the GPUs, gloo in the CPU tests)."""
@@ -461,6 +497,8 @@ def run_cuda(args):
                            call="nb_step_host(nsteps=1, reuse_acc=1): pinned host buffers in, results out, stream synchronised")
     if not args.no_drift_point:
         line["drift_roofline"] = drift_roofline(d)
+    if not args.no_mixed_point and not mixed and not na:
+        line["mixed_precision"] = mixed_point(d)
     if not args.no_cpu_baseline:
         line["cpu_baseline"] = cpu_baseline(d, na)
     print(json.dumps(line), flush=True)
