@@ -457,7 +457,7 @@ def run_cuda(args):
     value = whole_job_value(world, K, inter_per_step, total_ms)
     symmetric = geom.tile_j < 0
     kernel = ("nb_force_symds_kernel" if mixed else "nb_force_sym_kernel") if symmetric else ("nb_force_mixed_kernel" if mixed else "nb_force_tiles_kernel")
-    sorted_staging = symmetric and not mixed and N >= 32768   # NB_SORT_AUTO (include/nbkick.h); the mixed Newton-III kernel stages unsorted
+    sorted_staging = symmetric and N >= 32768   # NB_SORT_AUTO (include/nbkick.h), both Newton-III kernels
     traffic, traffic_source = _traffic_from_profile(kernel, N, geom, sorted_staging, args.precision)
     # FP64-pipe instructions per ORDERED interaction on the fast path: 20 per unordered pair (Newton III)
     # or 15 (one-sided); DESIGN.md section 5

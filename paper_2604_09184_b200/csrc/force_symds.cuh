@@ -16,8 +16,9 @@
 // every self term, are killed in the fp32 loop (rsqrt replaced by 0: they contribute exactly 0 to both sides) and
 // re-evaluated by the EXACT fp64 pass of force_sym.cuh (sym_exact) from the fp64 staged arrays: the changeover weight,
 // the pair test r^2 < rc^2 and the pair list are bit-identical to the fp64 kernel's.  Tolerance reading: DESIGN.md S25.
-// Same super-tile decomposition, skewed unit order, slots and determinism as nb_force_sym_kernel (no sorted staging, no
-// tail splitting, no bands: the host falls back to the one-sided mixed kernel where those would be needed).
+// Same super-tile decomposition, skewed unit order, slots, determinism and sorted staging (test-free far tiles) as
+// nb_force_sym_kernel; no tail splitting and no bands (the host falls back to the one-sided mixed kernel where the slots
+// would pass the cap).
 #pragma once
 #include "force_sym.cuh"
 
@@ -45,7 +46,8 @@ __device__ __forceinline__ float rsqrt_f32(const float a) {
 // lanes per issue slot, each rounded as the scalar instruction would): the (high, low) partial differences of a coordinate
 // in one FADD2, everything after the differences on two i-bodies at a time.  nxa/nya/nza: the lane's i-bodies, NEGATED,
 // as (high, low) pairs; ngi2: -G m_i of bodies (2g, 2g+1).
-template <bool PAIRS>
+// TEST = false (sorted staging, super-tiles whose arcs are out of each other's reach): no pre-filter, no kill, no exact pass.
+template <bool PAIRS, bool TEST, bool SORTED>
 __device__ __forceinline__ void symds_block(const SymDsParams &p, const float4 *__restrict__ qa, const float4 *__restrict__ qb,
                                             const int jbase, const bool mixed, const float2 (&nxa)[kDsI], const float2 (&nya)[kDsI],
                                             const float2 (&nza)[kDsI], const float2 (&ngi2)[kDsI / 2], const float thr_lane,
@@ -78,17 +80,21 @@ __device__ __forceinline__ void symds_block(const SymDsParams &p, const float4 *
             dz[g] = make_float2(__fadd_rn(z0.x, z0.y), __fadd_rn(z1.x, z1.y));
             r2[g] = __ffma2_rn(dz[g], dz[g], __ffma2_rn(dy[g], dy[g], __fmul2_rn(dx[g], dx[g])));
         }
-        float mn = fminf(r2[0].x, r2[0].y);
+        float kill = 0.0f;
+        if (TEST) {
+            float mn = fminf(r2[0].x, r2[0].y);
 #pragma unroll
-        for (int g = 1; g < H; ++g) mn = fminf(mn, fminf(r2[g].x, r2[g].y));
-        const bool hit = mn <= fmaxf(thr_lane, b.w);
-        if (hit) bits |= rbit;
-        rbit <<= 1;
-        const float kill = hit ? kInf : 0.0f;         // rsqrt(+inf) = 0: a flagged lane's I pairs contribute exactly 0
+            for (int g = 1; g < H; ++g) mn = fminf(mn, fminf(r2[g].x, r2[g].y));
+            const bool hit = mn <= fmaxf(thr_lane, b.w);
+            if (hit) bits |= rbit;
+            rbit <<= 1;
+            kill = hit ? kInf : 0.0f;                 // rsqrt(+inf) = 0: a flagged lane's I pairs contribute exactly 0
+        }
         const float2 gmj = make_float2(b.z, b.z);
 #pragma unroll
         for (int g = 0; g < H; ++g) {
-            const float2 y0 = make_float2(rsqrt_f32(fmaxf(r2[g].x, kill)), rsqrt_f32(fmaxf(r2[g].y, kill)));
+            const float2 y0 = TEST ? make_float2(rsqrt_f32(fmaxf(r2[g].x, kill)), rsqrt_f32(fmaxf(r2[g].y, kill)))
+                                   : make_float2(rsqrt_f32(r2[g].x), rsqrt_f32(r2[g].y));
             const float2 y3 = __fmul2_rn(__fmul2_rn(y0, y0), y0);
             const float2 si = __fmul2_rn(y3, gmj);            // G m_j / r^3
             const float2 sj = __fmul2_rn(y3, ngi2[g]);        // -G m_i / r^3
@@ -106,6 +112,7 @@ __device__ __forceinline__ void symds_block(const SymDsParams &p, const float4 *
         AX[2 * g + 1] += (double)ax[g].y; AY[2 * g + 1] += (double)ay[g].y; AZ[2 * g + 1] += (double)az[g].y;
     }
 
+    if (!TEST) return;
     unsigned any = __reduce_or_sync(0xffffffffu, bits);
     if (any == 0u) return;
     // exact fp64 pass (rare): the lane's i-bodies from the fp64 staged arrays
@@ -128,11 +135,15 @@ __device__ __forceinline__ void symds_block(const SymDsParams &p, const float4 *
         if ((bits >> r) & 1u) {
             const int j = jbase + src;
             const size_t ej = (size_t)(j >> 5) * 64 + (j & 31);
-            sym_exact<I, false>(sp, sp.sxy[ej], sp.szg[ej], sp.sthr[ej], j, mixed, xi, yi, zi, ngd, i0, AX, AY, AZ, cx, cy, cz, emit);
+            sym_exact<I, SORTED>(sp, sp.sxy[ej], sp.szg[ej], sp.sthr[ej], j, mixed, xi, yi, zi, ngd, i0, AX, AY, AZ, cx, cy, cz, emit);
         }
         if (PAIRS) {
 #pragma unroll
-            for (int k = 0; k < I; ++k) pair_append(sp.pairs, sp.npairs, sp.status, sp.cap, emit[k], i0 + 32 * k, jbase + src);
+            for (int k = 0; k < I; ++k) {
+                int ib = i0 + 32 * k, jb = jbase + src;
+                if (SORTED && emit[k]) { ib = sp.perm[ib]; jb = sp.perm[jb]; }   // the list holds BODY indices
+                pair_append(sp.pairs, sp.npairs, sp.status, sp.cap, emit[k], ib, jb);
+            }
         }
         const int from = (lane - r) & 31;
         bx += __shfl_sync(0xffffffffu, cx, from);
@@ -143,7 +154,7 @@ __device__ __forceinline__ void symds_block(const SymDsParams &p, const float4 *
 
 // One CTA of W warps per super-tile (A, B), A <= B, S = 128 W bodies a side: B staged once (two TMA bulk copies of the
 // float4 arrays), B's fp64 sums in shared memory, A's bodies in registers four per lane; diagonal tiles first.
-template <int W, bool PAIRS>
+template <int W, bool PAIRS, bool SORTED>
 __global__ void __launch_bounds__(32 * W, 16 / W) nb_force_symds_kernel(const SymDsParams p) {
     constexpr int I = kDsI, kThreads = 32 * W;
     extern __shared__ __align__(16) unsigned char symds_smem[];
@@ -183,6 +194,12 @@ __global__ void __launch_bounds__(32 * W, 16 / W) nb_force_symds_kernel(const Sy
     __syncthreads();
     mbar_wait(bar, 0);
 
+    // sorted staging: arcs of A and B out of each other's reach => no pair of this super-tile can meet a critical radius
+    bool far = false;
+    if (SORTED && !diag) {
+        const BlockBound ba_ = sp.bnd[A], bb_ = sp.bnd[B];
+        far = arcs_are_far(ba_.phi_lo, ba_.phi_hi, ba_.r_min, ba_.rc_max, bb_.phi_lo, bb_.phi_hi, bb_.r_min, bb_.rc_max);
+    }
     const int nunits = S / (32 * sp.U);
     const int nchunks = S / (kThreads * I);
     for (int c = 0; c < nchunks; ++c) {
@@ -214,7 +231,10 @@ __global__ void __launch_bounds__(32 * W, 16 / W) nb_force_symds_kernel(const Sy
                     mixed = q < P + I;
                 }
                 double bx, by, bz;
-                symds_block<PAIRS>(p, ba + q * 64, bb + q * 64, B * S + q * 32, mixed, nxa, nya, nza, ngi2, thr_lane, i0, AX, AY, AZ, bx, by, bz);
+                if (SORTED && far)
+                    symds_block<PAIRS, false, SORTED>(p, ba + q * 64, bb + q * 64, B * S + q * 32, mixed, nxa, nya, nza, ngi2, thr_lane, i0, AX, AY, AZ, bx, by, bz);
+                else
+                    symds_block<PAIRS, true, SORTED>(p, ba + q * 64, bb + q * 64, B * S + q * 32, mixed, nxa, nya, nza, ngi2, thr_lane, i0, AX, AY, AZ, bx, by, bz);
                 if (!mixed) {
                     const int n = q * 32 + lane;
                     jsx[n] += bx; jsy[n] += by; jsz[n] += bz;

@@ -125,7 +125,8 @@ Geometry geometry(int64_t N, int64_t n_active) {
     const bool fully_active = (g.Nj == N);
     if (fully_active && g.mixed && g_cfg.force_kernel != NB_FORCE_TILES && (g_cfg.force_kernel == NB_FORCE_SYMMETRIC || N >= kSymMinN)) {
         // Newton-III mixed-precision kernel (force_symds.cuh): I = 4, CTAs of 1 / 2 / 4 warps chosen as for the fp64 kernel;
-        // no sorted staging, tail splitting or bands -- where the slots would pass the cap the one-sided mixed kernel runs
+        // sorted staging as for the fp64 kernel; no tail splitting or bands -- where the slots would pass the cap the one-sided
+        // mixed kernel runs
         auto waves = [&](int s) {
             const int64_t T = (N + s - 1) / s;
             return (double)(T * (T + 1) / 2) / (double)((int64_t)sms * (1536 / s));
@@ -137,6 +138,7 @@ Geometry geometry(int64_t N, int64_t n_active) {
         if (T * N * 24 <= cap) {
             g.sym = 1; g.mixed = 2; g.S = S; g.U = S / 128; g.ipt = 4; g.warps = S / 128; g.minb = 12 / g.warps;
             g.Npad_sym = (int)Npad; g.nsplit = (int)T; g.iblocks = (int)T; g.tiles_per_split = 0; g.nslots = (int)T;
+            g.sorted = g_cfg.sort_staging == NB_SORT_ON || (g_cfg.sort_staging == NB_SORT_AUTO && N >= 32768);
             return g;
         }
     }
@@ -437,7 +439,8 @@ int launch_symds_W(const SymDsParams &dp, const Geometry &g, bool pairs) {
         kern<<<ctas, 32 * W, smem, stream()>>>(dp);
         return NB_OK;
     };
-    return pairs ? go(nb_force_symds_kernel<W, true>) : go(nb_force_symds_kernel<W, false>);
+    if (g.sorted) return pairs ? go(nb_force_symds_kernel<W, true, true>) : go(nb_force_symds_kernel<W, false, true>);
+    return pairs ? go(nb_force_symds_kernel<W, true, false>) : go(nb_force_symds_kernel<W, false, false>);
 }
 
 int launch_symds(const SymParams &sp, const Workspace &w, const Geometry &g, bool pairs) {

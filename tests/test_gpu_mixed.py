@@ -59,7 +59,9 @@ BOUND_DS = 151 * U32
 @pytest.mark.parametrize("cfg,n_override,n2,tune", [(2, 6000, 0.0, {}),                                   # auto: S = 128, 1-warp CTAs
                                                     (1, 5000, 0.4, dict(sym_block=256)),                   # giants, Eq. 7 radius, 2-warp CTAs
                                                     (2, 8193, 0.4, dict(sym_block=512)),                   # ragged tail, 4-warp CTAs
-                                                    (0, 700, 0.4, dict(force_kernel=2, sym_block=128))])   # forced below the threshold
+                                                    (0, 700, 0.4, dict(force_kernel=2, sym_block=128)),    # forced below the threshold
+                                                    (2, 6000, 0.4, dict(sort_staging=1, sym_block=256)),   # sorted staging: test-free far tiles
+                                                    (2, 33000, 0.0, {})])                                  # auto: sorted staging from N = 32768
 def test_mixed_newton3_kick_against_fp64_oracle(cfg, n_override, n2, tune):
     tune = dict(tune)
     fk = tune.pop("force_kernel", 0)
