@@ -63,7 +63,7 @@ extern "C" {
  *   NB_PRECISION_MIXED  pairs out of reach of every critical radius are evaluated in fp32; pairs within reach, the
  *                       changeover weight, the pair test and the pair list stay in fp64 and are identical to the fp64
  *                       kernel's.  Tolerance: DESIGN.md reading S25 (~1e-7 relative, typically).  Two kernels:
- *                       fully active, N >= 4096 (or NB_FORCE_SYMMETRIC), slots within slot_bytes_max: the Newton-III
+ *                       fully active, N >= 4096 (or NB_FORCE_SYMMETRIC): the Newton-III
  *                       kernel on double-single positions -- differences fl(fl(xjh - xih) + fl(xjl - xil)), r^2, r^-3,
  *                       products and the sums over one visit of a 32-body block all on the FP32 pipe, fp64 from there on;
  *                       otherwise (semi-active, small N, NB_FORCE_TILES): the one-sided kernel -- differences in fp64,

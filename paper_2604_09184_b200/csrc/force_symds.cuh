@@ -17,8 +17,7 @@
 // re-evaluated by the EXACT fp64 pass of force_sym.cuh (sym_exact) from the fp64 staged arrays: the changeover weight,
 // the pair test r^2 < rc^2 and the pair list are bit-identical to the fp64 kernel's.  Tolerance reading: DESIGN.md S25.
 // Same super-tile decomposition, skewed unit order, slots, determinism and sorted staging (test-free far tiles) as
-// nb_force_sym_kernel; no tail splitting and no bands (the host falls back to the one-sided mixed kernel where the slots
-// would pass the cap).
+// nb_force_sym_kernel, banded evaluation included; no tail splitting.
 #pragma once
 #include "force_sym.cuh"
 
@@ -168,12 +167,13 @@ __global__ void __launch_bounds__(32 * W, 16 / W) nb_force_symds_kernel(const Sy
     uint64_t *bar = reinterpret_cast<uint64_t *>(jsz + S);
     const int t = threadIdx.x, lane = t & 31, w = t >> 5;
 
-    const int T = sp.nsb;
+    // tile of this CTA among the columns col0 .. col0 + ncols - 1 of the launch (the whole grid, or one band of the banded
+    // evaluation: force_sym.cuh SymParams): the diagonal tiles first, then the strict pairs A < B column by column
     int A, B;
-    if ((int)blockIdx.x < T) {
-        A = B = (int)blockIdx.x;
+    if ((int)blockIdx.x < sp.ncols) {
+        A = B = sp.col0 + (int)blockIdx.x;
     } else {
-        const long long idx = (long long)blockIdx.x - T;
+        const long long idx = (long long)blockIdx.x - sp.ncols + (long long)sp.col0 * (sp.col0 - 1) / 2;
         B = (int)((1.0 + sqrt(1.0 + 8.0 * (double)idx)) * 0.5);
         while ((long long)B * (B - 1) / 2 > idx) --B;
         while ((long long)(B + 1) * B / 2 <= idx) ++B;
@@ -250,7 +250,7 @@ __global__ void __launch_bounds__(32 * W, 16 / W) nb_force_symds_kernel(const Sy
             }
             __syncthreads();
         } else {
-            double *out = sp.part_i + (size_t)B * sp.stride_i * 3;
+            double *out = sp.part_i + (size_t)(B - sp.col0) * sp.stride_i * 3;
 #pragma unroll
             for (int k = 0; k < I; ++k) {
                 const int i = i0 + 32 * k;
@@ -261,7 +261,7 @@ __global__ void __launch_bounds__(32 * W, 16 / W) nb_force_symds_kernel(const Sy
     double *out = sp.part_j + (size_t)A * sp.stride_j * 3;
     for (int n = t; n < S; n += kThreads) {
         const long long g = (long long)B * S + n;
-        if (g < sp.N) { out[3 * g] = jsx[n]; out[3 * g + 1] = jsy[n]; out[3 * g + 2] = jsz[n]; }
+        if (g < sp.N) { out[3 * (g - sp.goff)] = jsx[n]; out[3 * (g - sp.goff) + 1] = jsy[n]; out[3 * (g - sp.goff) + 2] = jsz[n]; }
     }
 }
 

@@ -125,8 +125,7 @@ Geometry geometry(int64_t N, int64_t n_active) {
     const bool fully_active = (g.Nj == N);
     if (fully_active && g.mixed && g_cfg.force_kernel != NB_FORCE_TILES && (g_cfg.force_kernel == NB_FORCE_SYMMETRIC || N >= kSymMinN)) {
         // Newton-III mixed-precision kernel (force_symds.cuh): I = 4, CTAs of 1 / 2 / 4 warps chosen as for the fp64 kernel;
-        // sorted staging as for the fp64 kernel; no tail splitting or bands -- where the slots would pass the cap the one-sided
-        // mixed kernel runs
+        // sorted staging and the banded evaluation as for the fp64 kernel; no tail splitting
         auto waves = [&](int s) {
             const int64_t T = (N + s - 1) / s;
             return (double)(T * (T + 1) / 2) / (double)((int64_t)sms * (1536 / s));
@@ -135,12 +134,15 @@ Geometry geometry(int64_t N, int64_t n_active) {
         if (S != 128 && S != 256 && S != 512) S = waves(512) >= 16.0 ? 512 : (waves(256) >= 5.0 ? 256 : 128);
         const int64_t Npad = ((N + S - 1) / S) * S, T = Npad / S;
         const int64_t cap = g_cfg.slot_bytes_max > 0 ? g_cfg.slot_bytes_max : ((int64_t)4 << 30);
-        if (T * N * 24 <= cap) {
-            g.sym = 1; g.mixed = 2; g.S = S; g.U = S / 128; g.ipt = 4; g.warps = S / 128; g.minb = 12 / g.warps;
-            g.Npad_sym = (int)Npad; g.nsplit = (int)T; g.iblocks = (int)T; g.tiles_per_split = 0; g.nslots = (int)T;
-            g.sorted = g_cfg.sort_staging == NB_SORT_ON || (g_cfg.sort_staging == NB_SORT_AUTO && N >= 32768);
-            return g;
+        g.sym = 1; g.mixed = 2; g.S = S; g.U = S / 128; g.ipt = 4; g.warps = S / 128; g.minb = 12 / g.warps;
+        g.Npad_sym = (int)Npad; g.nsplit = (int)T; g.iblocks = (int)T; g.tiles_per_split = 0; g.nslots = (int)T;
+        g.sorted = g_cfg.sort_staging == NB_SORT_ON || (g_cfg.sort_staging == NB_SORT_AUTO && N >= 32768);
+        if (T * N * 24 > cap) {   // banded evaluation, as for the fp64 kernel (5.1d)
+            int64_t band = cap / (24 * (N + Npad));
+            if (band < 1) band = 1;
+            if (band < T) g.band = (int)band;
         }
+        return g;
     }
     if (fully_active && !g.mixed && g_cfg.force_kernel != NB_FORCE_TILES && (g_cfg.force_kernel == NB_FORCE_SYMMETRIC || N >= kSymMinN)) {
         // I = 4 at 12 warps per SM (160 registers, no spills) measured fastest on B200.
@@ -432,7 +434,7 @@ int launch_sym_IM(const SymParams &sp, const Geometry &g, bool pairs) {
 template <int W>
 int launch_symds_W(const SymDsParams &dp, const Geometry &g, bool pairs) {
     const long long T = g.nsplit;
-    const unsigned ctas = (unsigned)(T * (T + 1) / 2);
+    const unsigned ctas = (unsigned)(dp.sp.ncols == (int)T ? T * (T + 1) / 2 : sym_band_grid(dp.sp.col0, dp.sp.ncols));
     const size_t smem = symds_smem_bytes(g.S);
     auto go = [&](auto kern) -> int {
         NB_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
@@ -536,7 +538,7 @@ int enqueue_eval(const Workspace &w, const Geometry &g, double *x, double *v, co
             for (int c0 = 0; c0 < g.nsplit; c0 += g.band) {
                 sp.col0 = c0; sp.ncols = g.nsplit - c0 < g.band ? g.nsplit - c0 : g.band;
                 sp.stride_j = (long long)sp.ncols * g.S; sp.goff = c0 * g.S;
-                const int lrc = launch_sym(sp, g, pairs != nullptr);
+                const int lrc = g.mixed == 2 ? launch_symds(sp, w, g, pairs != nullptr) : launch_sym(sp, g, pairs != nullptr);
                 if (lrc) return lrc;
                 nb_bandsum_kernel<<<nblk, kBodyThreads, 0, stream()>>>(sp.part_i, sp.part_j, acc, (int)N, g.S, sp.col0, sp.ncols,
                                                                       c0 == 0 ? 1 : 0, sorted ? w.perm : nullptr);

@@ -61,7 +61,9 @@ BOUND_DS = 151 * U32
                                                     (2, 8193, 0.4, dict(sym_block=512)),                   # ragged tail, 4-warp CTAs
                                                     (0, 700, 0.4, dict(force_kernel=2, sym_block=128)),    # forced below the threshold
                                                     (2, 6000, 0.4, dict(sort_staging=1, sym_block=256)),   # sorted staging: test-free far tiles
-                                                    (2, 33000, 0.0, {})])                                  # auto: sorted staging from N = 32768
+                                                    (2, 33000, 0.0, {}),                                   # auto: sorted staging from N = 32768
+                                                    (2, 5000, 0.4, dict(sym_block=256, slot_bytes_max=24 * (5000 + 5120) * 3)),          # banded: 3 columns per launch
+                                                    (1, 6000, 0.4, dict(sym_block=128, sort_staging=1, slot_bytes_max=24 * (6002 + 6016) * 5))])  # banded + sorted
 def test_mixed_newton3_kick_against_fp64_oracle(cfg, n_override, n2, tune):
     tune = dict(tune)
     fk = tune.pop("force_kernel", 0)
