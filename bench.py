@@ -64,6 +64,8 @@ def parse_args():
                          "(CUDA-graph replay / fused small-N launch), timed with CUDA events; prints one JSON line with mode=trajectory")
     ap.add_argument("--n2", type=float, default=None, help="--trajectory: velocity factor of Eq. 7 (default 0: 3 R_Hill; 0.4: full Eq. 7)")
     ap.add_argument("--encounters", action="store_true", help="--trajectory: resolve close encounters (direct solver)")
+    ap.add_argument("--collide", type=float, default=0.0,
+                    help="--trajectory --encounters: examine collisions inside the direct solver with the radii (2 g/cm^3) inflated by this factor (PAPER.md:98, 130, 168); 0 = off")
     ap.add_argument("--levels", type=int, default=0, help="--trajectory --encounters: intermediate changeover levels (PAPER.md:106)")
     return ap.parse_args()
 
@@ -519,8 +521,12 @@ def run_trajectory(args):
     N = d.N
     n2 = N2 if args.n2 is None else args.n2
     cap = 1 << 24
+    collide = args.encounters and args.collide > 0.0
+    radius = torch.from_numpy(d.radius).cuda() if collide else None
+    absorbed_by = torch.full((N,), -1, dtype=torch.int32, device="cuda") if collide else None
     nb.configure(N, pair_capacity=cap, n_active=na, G=G_GAUSS, n1=N1, n2=n2, resolve_encounters=args.encounters,
-                 levels=args.levels, precision=1 if args.precision == "mixed" else 0, force_kernel=args.force_kernel, j_splits=args.j_splits)
+                 levels=args.levels, precision=1 if args.precision == "mixed" else 0, force_kernel=args.force_kernel, j_splits=args.j_splits,
+                 radius_factor=args.collide if collide else 1.0, collide_radius=radius, collide_absorbed_by=absorbed_by)
     nb.nb_status_reset()
     x = torch.from_numpy(d.x).cuda(); v = torch.from_numpy(d.v).cuda(); m = torch.from_numpy(d.m).cuda()
     acc = torch.zeros_like(x); rc = torch.zeros(N, dtype=torch.float64, device="cuda")
@@ -537,7 +543,7 @@ def run_trajectory(args):
     ms = e0.elapsed_time(e1)
     geom = nb.force_geometry(N)
     print(json.dumps(dict(mode="trajectory", config=workload_name(d, na).replace(f"(n2={N2:g})", f"(n2={n2:g})"), N=N, nsteps=nsteps,
-                          a_substep=("direct solver for the encounter groups" + (f", {args.levels} intermediate levels" if args.levels else "")) if args.encounters else "Kepler drift",
+                          a_substep=("direct solver for the encounter groups" + (f", {args.levels} intermediate levels" if args.levels else "") + (f", collisions inside the solver (f = {args.collide:g})" if collide else "")) if args.encounters else "Kepler drift",
                           total_ms=ms, ms_per_step=ms / nsteps, steps_per_sec=nsteps / (ms * 1e-3),
                           interactions_per_sec=nsteps * float(N) * float(na or N) / (ms * 1e-3), pairs_last_step=int(npairs.item()),
                           status=nb.nb_status(), precision=args.precision,

@@ -95,7 +95,7 @@ def _mixed_case(cfg, n_override, n2, tune, force_kernel, bound):
     err = np.abs(acc - ref)
     worst = float(np.max(err / np.where(ab > 0, ab, 1e-300)))
     rel = err / np.maximum(np.abs(ref), 1e-3 * np.linalg.norm(ref, axis=1, keepdims=True))
-    print(f"{d.name}: mixed vs fp64 oracle: worst |da| / sum|t| = {worst / U32:.1f} u (bound 143 u), relative error median "
+    print(f"{d.name}: mixed vs fp64 oracle: worst |da| / sum|t| = {worst / U32:.1f} u (bound {bound / U32:.0f} u), relative error median "
           f"{np.median(rel):.2e} max {rel.max():.2e} [{geo}]; fp64 kernel max {np.max(np.abs(res[0][0] - ref) / np.where(ab > 0, ab, 1e-300)) / 2.2e-16:.1f} eps")
     assert worst <= bound
     assert np.median(rel) <= 3e-7
