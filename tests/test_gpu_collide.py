@@ -188,3 +188,35 @@ def test_step_with_collisions_inside_the_solver(use_graph):
     torch.cuda.synchronize()
     assert int(mstat[0].item()) == d.N - st["absorbed"]
     assert float(m[: int(mstat[0].item())].min().item()) > 0.0
+
+
+def test_error_codes_of_the_collision_calls():
+    """Host-detectable misuse: semi-active mode, levels > 0, a missing absorbed_by array."""
+    import paper_2604_09184_b200 as nb
+    torch = torch_mod()
+    d = nb_inputs.make_config(2, n_override=600)
+    x, v, m, R = to_dev(d.x), to_dev(d.v), to_dev(d.m), to_dev(d.radius)
+    rc = torch.zeros(d.N, dtype=torch.float64, device="cuda"); acc = torch.zeros_like(x)
+    ab = torch.full((d.N,), -1, dtype=torch.int32, device="cuda")
+    members = torch.zeros(d.N, dtype=torch.int32, device="cuda"); gstart = torch.zeros(d.N // 2 + 2, dtype=torch.int32, device="cuda")
+    gstat = torch.zeros(4, dtype=torch.int64, device="cuda")
+    pairs = torch.zeros((1024, 2), dtype=torch.int32, device="cuda"); npairs = torch.zeros(1, dtype=torch.int64, device="cuda")
+    nb.configure(d.N, G=G_GAUSS, pair_capacity=1024, n_active=100)
+    with pytest.raises(nb.NbError) as e:
+        nb.nb_encounter_collide(x, v, m, R, rc, d.M_star, d.dt, members, gstart, gstat, ab)
+    assert e.value.code == nb.binding.NB_E_BADARG
+    nb.configure(d.N, G=G_GAUSS, pair_capacity=1024, resolve_encounters=True, collide_radius=R)
+    with pytest.raises(nb.NbError) as e:
+        nb.nb_step(x, v, m, d.M_star, d.dt, rc, acc, pairs, npairs, 1)
+    assert e.value.code == nb.binding.NB_E_NULL
+    nb.configure(d.N, G=G_GAUSS, pair_capacity=1024, resolve_encounters=True, levels=2, collide_radius=R, collide_absorbed_by=ab)
+    with pytest.raises(nb.NbError) as e:
+        nb.nb_step(x, v, m, d.M_star, d.dt, rc, acc, pairs, npairs, 1)
+    assert e.value.code == nb.binding.NB_E_BADARG
+    torch.cuda.synchronize()
+    assert np.array_equal(x.cpu().numpy(), d.x) and np.array_equal(m.cpu().numpy(), d.m)      # nothing ran
+    # zero groups: a no-op that returns
+    nb.configure(d.N, G=G_GAUSS, pair_capacity=1024)
+    nb.nb_encounter_collide(x, v, m, R, rc, d.M_star, d.dt, members, gstart, gstat, ab)
+    torch.cuda.synchronize()
+    assert np.array_equal(x.cpu().numpy(), d.x) and int(ab.max().item()) == -1
