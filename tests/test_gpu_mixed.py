@@ -147,3 +147,33 @@ def _mixed_step(n):
     de_r = (oracle.diagnostics(ref["x"], ref["v"], d.m, d.M_star, G_GAUSS)["E"] - E0) / E0
     print(f"mixed x20: rel dx {ex:.2e}, dE/E mixed {de_g:.3e} fp64 oracle {de_r:.3e}")
     assert ex <= 1e-8 and abs(de_g - de_r) <= 1e-6
+
+
+def test_mixed_config3_full_200_steps_against_the_stored_oracle_run():
+    """The bench workload (N = 65536 ring, 200 steps) in mixed precision against the stored fp64 oracle trajectory
+    (tests/golden/config3_trajectory.txt, written by oracle/make_golden.py): energy error within the 1e-9 of reading S16
+    although the force carries ~1e-7 relative error per pair (it is unbiased and the sums are long), angular momentum
+    conserved to fp32-sum level, sampled states within 1e-6."""
+    import os
+    from oracle import make_golden
+    g = make_golden.load(os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden", "config3_trajectory.txt"))
+    d = nb_inputs.make_config(2)
+    assert make_golden.input_sha(d) == g["input_sha256"]
+    nsteps = int(g["nsteps"])
+    st = GpuState(d.x, d.v, d.m, d.M_star, G=G_GAUSS, n1=3.0, n2=0.0, pair_capacity=1 << 22, precision=1)
+    geo = st.nb.force_geometry(d.N)
+    assert geo.tile_j == -512                                      # the Newton-III mixed-precision kernel
+    st.step(d.dt, nsteps)
+    xg, vg, _, _ = st.host()
+    E0 = oracle.diagnostics(d.x, d.v, d.m, d.M_star, G_GAUSS)
+    Eg = oracle.diagnostics(xg, vg, d.m, d.M_star, G_GAUSS)
+    de_g = (Eg["E"] - E0["E"]) / E0["E"]
+    de_r = float(g["dE_over_E"])
+    dL = np.linalg.norm(Eg["L"] - np.array(g["L1"])) / np.linalg.norm(np.array(g["L1"]))
+    rows = g["row_index"]
+    ex = np.max(np.abs(xg[rows] - g["x"]) / np.linalg.norm(g["x"], axis=1, keepdims=True), axis=1)
+    print(f"mixed, config 3 x {nsteps}: dE/E mixed {de_g:.6e} fp64 oracle {de_r:.6e} (difference {abs(de_g - de_r):.2e}), dL/L {dL:.2e}, "
+          f"rel dx max {ex.max():.2e} median {np.median(ex):.2e}, pairs {int(st.npairs.item())} (oracle {g['pairs_sure']})")
+    assert abs(de_g - de_r) <= 1e-9
+    assert dL <= 1e-9
+    assert np.quantile(ex, 0.99) <= 1e-6
