@@ -66,8 +66,9 @@ extern "C" {
  *                       fully active, N >= 4096 (or NB_FORCE_SYMMETRIC): the Newton-III
  *                       kernel on double-single positions -- differences fl(fl(xjh - xih) + fl(xjl - xil)), r^2, r^-3,
  *                       products and the sums over one visit of a 32-body block all on the FP32 pipe, fp64 from there on;
- *                       otherwise (semi-active, small N, NB_FORCE_TILES): the one-sided kernel -- differences in fp64,
- *                       the rest in fp32, summed in fp32 per 128-body tile and in fp64 across tiles. */
+ *                       otherwise (semi-active, small N, NB_FORCE_TILES): the one-sided kernel -- the same double-single
+ *                       arithmetic when it holds 2 or 4 i-bodies per thread, differences in fp64 and the rest in fp32
+ *                       when it holds one (small N); summed in fp32 per 128-body tile and in fp64 across tiles. */
 #define NB_PRECISION_F64 0
 #define NB_PRECISION_MIXED 1
 #define NB_SORT_AUTO 0

@@ -35,6 +35,7 @@ struct PrepParams {
     JRec *jrec;             // [Njpad] one-sided kernel's records (nullptr: not staged)
     double2 *sxy, *szg;     // [2 Npad_sym] symmetric kernel's (x,y) and (z,Gm), doubled-block layout (nullptr: not staged)
     int *sthr;              // [2 Npad_sym] hi32(rcrit^2) + 1
+    JRecDs *jds;            // [Njpad] double-single records of the one-sided mixed-precision kernel (nullptr: not staged)
     float4 *sa, *sb;        // [2 Npad_sym] double-single records of the Newton-III mixed-precision kernel (nullptr: not staged)
     int Npad_sym;
     const int *pos_of;      // [N] staged position of each body (sort_staging.cuh) or nullptr: position = index
@@ -84,6 +85,7 @@ __device__ __forceinline__ void prep_one(const PrepParams &p, const int i, const
         }
     }
     if (p.jrec != nullptr && i < p.Njpad) p.jrec[i] = r;  // grid covers max(N, Njpad, Npad_sym)
+    if (p.jds != nullptr && i < p.Njpad) p.jds[i] = make_jrecds(r.x, r.y, r.z, r.gm, r.rc2);
     if (p.sxy != nullptr && i < p.Npad_sym) {
         // symmetric kernel: every body is both an i- and a j-body; padding bodies get distinct far
         // positions (pad-pad distances stay huge and finite) and zero mass

@@ -29,6 +29,7 @@ namespace nbk {
 
 struct ForceParams {
     const JRec *jrec;            // [tiles_total * kTileJ] staged j-bodies (padded)
+    const JRecDs *jds;           // [tiles_total * kTileJ] double-single records (mixed-precision kernel, I >= 2) or nullptr
     const double *x;             // [N,3] i-side positions
     const double *rcrit;         // [N]   i-side critical radii
     double *part;                // [nsplit, N, 3] partial accelerations

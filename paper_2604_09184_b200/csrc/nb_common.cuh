@@ -39,6 +39,21 @@ __device__ __forceinline__ void symds_stage(float4 *sa, float4 *sb, const int po
     sb[en] = b; sb[en + 32] = b;
 }
 
+// One staged j-body of the one-sided mixed-precision kernel on double-single positions (force_mixed.cuh, nb_force_mixedds_kernel):
+// 32 bytes, (high, low) of a coordinate side by side.  Padding records sit far away with zero mass.
+struct __align__(16) JRecDs {
+    float xh, xl, yh, yl;
+    float zh, zl, gm, thr;   // thr = rc^2 (1 + 2^-18) rounded up
+};
+static_assert(sizeof(JRecDs) == 32, "JRecDs must be 32 bytes");
+__device__ __forceinline__ JRecDs make_jrecds(const double x, const double y, const double z, const double gm, const double rc2) {
+    JRecDs r;
+    r.xh = __double2float_rn(x); r.yh = __double2float_rn(y); r.zh = __double2float_rn(z);
+    r.xl = __double2float_rn(x - (double)r.xh); r.yl = __double2float_rn(y - (double)r.yh); r.zl = __double2float_rn(z - (double)r.zh);
+    r.gm = __double2float_rn(gm); r.thr = __double2float_ru(rc2) * 1.0000038f;
+    return r;
+}
+
 constexpr int kForceThreads = 128;  // threads per force CTA
 constexpr int kTileJ = 128;         // j-bodies per shared-memory stage (8 KB)
 constexpr int kStages = 4;          // TMA ring depth (2 tiles in flight ahead of the consumer)

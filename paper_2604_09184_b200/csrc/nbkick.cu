@@ -264,6 +264,7 @@ struct Workspace {
     double2 *sxy, *szg; // [2 Npad_sym]            (symmetric kernel, doubled-block layout)
     int *sthr;          // [2 Npad_sym]
     float4 *sa, *sb;    // [2 Npad_sym]            (Newton-III mixed-precision kernel: double-single records)
+    JRecDs *jds;        // [Njpad]                 (one-sided mixed-precision kernel, I >= 2: double-single records)
     int *perm, *pos_of; // [Npad_sym], [N]         (sorted staging: position <-> body)
     BlockBound *bnd;    // [nsplit]                (bounds of the staged super-blocks)
     double *part;       // [nsplit, N, 3]
@@ -328,6 +329,7 @@ Workspace carve(void *base, int64_t N, const Geometry &g) {
     w.sxy = reinterpret_cast<double2 *>(b + off); off += align_up((size_t)2 * g.Npad_sym * sizeof(double2), 256);
     w.szg = reinterpret_cast<double2 *>(b + off); off += align_up((size_t)2 * g.Npad_sym * sizeof(double2), 256);
     w.sthr = reinterpret_cast<int *>(b + off); off += align_up((size_t)2 * g.Npad_sym * sizeof(int), 256);
+    w.jds = reinterpret_cast<JRecDs *>(b + off); off += align_up((size_t)((!g.sym && g.mixed == 1 && g.ipt >= 2) ? g.Njpad : 0) * sizeof(JRecDs), 256);
     w.sa = reinterpret_cast<float4 *>(b + off); off += align_up((size_t)(g.mixed == 2 ? 2 * g.Npad_sym : 0) * sizeof(float4), 256);
     w.sb = reinterpret_cast<float4 *>(b + off); off += align_up((size_t)(g.mixed == 2 ? 2 * g.Npad_sym : 0) * sizeof(float4), 256);
     w.perm = reinterpret_cast<int *>(b + off); off += align_up((size_t)g.Npad_sym * sizeof(int), 256);
@@ -397,8 +399,13 @@ void launch_force_IM(const ForceParams &fp, const Geometry &g, bool pairs) {
 template <int I, int MINB>
 void launch_mixed_IM(const ForceParams &fp, const Geometry &g, bool pairs) {
     dim3 grid(g.iblocks, g.nsplit);
-    if (pairs) nb_force_mixed_kernel<I, true, MINB><<<grid, kForceThreads, 0, stream()>>>(fp);
-    else nb_force_mixed_kernel<I, false, MINB><<<grid, kForceThreads, 0, stream()>>>(fp);
+    if constexpr (I >= 2) {   // double-single records, everything on the FP32 pipe (force_mixed.cuh)
+        if (pairs) nb_force_mixedds_kernel<I, true, MINB><<<grid, kForceThreads, 0, stream()>>>(fp);
+        else nb_force_mixedds_kernel<I, false, MINB><<<grid, kForceThreads, 0, stream()>>>(fp);
+    } else {
+        if (pairs) nb_force_mixed_kernel<I, true, MINB><<<grid, kForceThreads, 0, stream()>>>(fp);
+        else nb_force_mixed_kernel<I, false, MINB><<<grid, kForceThreads, 0, stream()>>>(fp);
+    }
 }
 
 void launch_force(const ForceParams &fp, const Geometry &g, bool pairs) {
@@ -493,6 +500,7 @@ int enqueue_eval(const Workspace &w, const Geometry &g, double *x, double *v, co
     pp.x = x; pp.v = v; pp.m = m; pp.rcrit = rc_io; pp.jrec = g.sym ? nullptr : w.jrec; pp.mv_in = mv_in;
     pp.sxy = g.sym ? w.sxy : nullptr; pp.szg = w.szg; pp.sthr = w.sthr; pp.Npad_sym = g.Npad_sym;
     pp.sa = g.mixed == 2 ? w.sa : nullptr; pp.sb = w.sb;
+    pp.jds = (!g.sym && g.mixed == 1 && g.ipt >= 2) ? w.jds : nullptr;
     pp.pos_of = sorted ? w.pos_of : nullptr;
     pp.rc_hill = g_cfg.levels > 0 ? w.ml_hill : nullptr; pp.rc_vel = g_cfg.levels > 0 ? w.ml_vel : nullptr;
     pp.npairs = pairs ? reinterpret_cast<unsigned long long *>(npairs) : nullptr;
@@ -508,6 +516,7 @@ int enqueue_eval(const Workspace &w, const Geometry &g, double *x, double *v, co
     fp.npairs = pairs ? reinterpret_cast<unsigned long long *>(npairs) : w.npairs_dummy;
     fp.status = w.status; fp.cap = pairs ? g_cfg.pair_capacity : 0; fp.N = (int)N; fp.Nj = g.Nj;
     fp.tiles_total = g.tiles_total; fp.tiles_per_split = g.tiles_per_split; fp.kind = g_cfg.changeover_kind;
+    fp.jds = (!g.sym && g.mixed == 1 && g.ipt >= 2) ? w.jds : nullptr;
     // bounds of the staged super-blocks (before the timing events: they bracket the force kernel alone)
     if (sorted) nb_sort_bounds_kernel<<<g.nsplit, kGrpThreads, 0, stream()>>>(w.sxy, w.perm, rc_io, (int)N, g.S, w.bnd);
     const bool pool = g_cfg.time_force && g_tev_used < kMaxTimed;
@@ -741,7 +750,7 @@ int launch_step_small(const Workspace &w, const Geometry &g, double *x, double *
     PrepParams &pp = q.pp;
     pp.x = x; pp.v = v; pp.m = m; pp.rcrit = rc_io; pp.rc_hill = nullptr; pp.rc_vel = nullptr; pp.jrec = w.jrec;
     pp.sxy = nullptr; pp.szg = nullptr; pp.sthr = nullptr; pp.Npad_sym = 0; pp.pos_of = nullptr; pp.mv_in = nullptr;
-    pp.sa = nullptr; pp.sb = nullptr;
+    pp.sa = nullptr; pp.sb = nullptr; pp.jds = nullptr;
     pp.npairs = pairs ? reinterpret_cast<unsigned long long *>(npairs) : nullptr;
     pp.status = w.status; pp.dtc = 0.5 * dt; pp.M_star = M_star; pp.G = g_cfg.G; pp.n1 = g_cfg.n1; pp.n2 = g_cfg.n2;
     pp.absdt = std::fabs(dt); pp.nblk_in = body_blocks(N); pp.N = (int)N; pp.Nj = g.Nj; pp.Njpad = g.Njpad;
@@ -750,7 +759,7 @@ int launch_step_small(const Workspace &w, const Geometry &g, double *x, double *
     fp.jrec = w.jrec; fp.x = x; fp.rcrit = rc_io; fp.part = w.part; fp.pairs = pairs;
     fp.npairs = pairs ? reinterpret_cast<unsigned long long *>(npairs) : w.npairs_dummy;
     fp.status = w.status; fp.cap = pairs ? g_cfg.pair_capacity : 0; fp.N = (int)N; fp.Nj = g.Nj;
-    fp.tiles_total = g.tiles_total; fp.tiles_per_split = g.tiles_per_split; fp.kind = g_cfg.changeover_kind;
+    fp.tiles_total = g.tiles_total; fp.tiles_per_split = g.tiles_per_split; fp.kind = g_cfg.changeover_kind; fp.jds = nullptr;
     q.acc = acc; q.mvA = w.mvA; q.mvB = w.mvB; q.mu = g_cfg.G * M_star; q.dt = dt; q.hk = 0.5 * dt; q.dtc = 0.5 * dt;
     q.nsteps = (int)(nsteps > 2000000000LL ? 2000000000LL : nsteps); q.last_nhalf = 1;
     q.iblocks = g.iblocks; q.nsplit = g.nsplit; q.nblk = body_blocks(N);

@@ -44,7 +44,9 @@ def _numpy_mixed(x, m, rc, G, rows):
 
 
 @pytest.mark.parametrize("cfg,n_override,n2,tune", [(2, 6000, 0.0, {}), (1, 5000, 0.4, dict(i_per_thread=4)), (3, 8192, 0.0, {}),
-                                                    (0, 2048, 0.4, dict(i_per_thread=1, j_splits=3))])
+                                                    (0, 2048, 0.4, dict(i_per_thread=1, j_splits=3)),
+                                                    (3, 8192, 0.4, dict(i_per_thread=2)),                  # semi-active through the double-single one-sided kernel
+                                                    (3, 20000, 0.0, dict(i_per_thread=4, j_splits=2))])    # semi-active, I = 4, two tiles per CTA
 def test_mixed_kick_against_fp64_oracle(cfg, n_override, n2, tune):
     _mixed_case(cfg, n_override, n2, tune, 1, BOUND)
 
