@@ -304,7 +304,7 @@ def mixed_point(d, launches=10):
     scale = torch.clamp(a64.abs(), min=1e-3 * float(a64.norm(dim=1).max()))
     rel = ((a32 - a64).abs() / scale)
     g = out[1][2]
-    return dict(precision="NB_PRECISION_MIXED", kernel="nb_force_symds_kernel" if g.tile_j < 0 else ("nb_force_mixedds_kernel" if g.i_per_thread >= 2 else "nb_force_mixed_kernel"),
+    return dict(precision="NB_PRECISION_MIXED", kernel="nb_force_symds_kernel" if g.tile_j < 0 else ("nb_force_mixedds_kernel" if g.i_per_thread >= 2 else "nb_force_tiles_kernel (fp64: one i-body per thread)"),
                 ms_per_kick=out[1][0], interactions_per_sec=float(N) * float(N) / (out[1][0] * 1e-3),
                 ms_per_kick_f64=out[0][0], speedup_vs_f64=out[0][0] / out[1][0],
                 rel_err_vs_f64_median=float(rel.median()), rel_err_vs_f64_max=float(rel.max()),
@@ -458,7 +458,7 @@ def run_cuda(args):
 
     value = whole_job_value(world, K, inter_per_step, total_ms)
     symmetric = geom.tile_j < 0
-    kernel = ("nb_force_symds_kernel" if mixed else "nb_force_sym_kernel") if symmetric else (("nb_force_mixedds_kernel" if geom.i_per_thread >= 2 else "nb_force_mixed_kernel") if mixed else "nb_force_tiles_kernel")
+    kernel = ("nb_force_symds_kernel" if mixed else "nb_force_sym_kernel") if symmetric else ("nb_force_mixedds_kernel" if mixed and geom.i_per_thread >= 2 else "nb_force_tiles_kernel")
     sorted_staging = symmetric and N >= 32768   # NB_SORT_AUTO (include/nbkick.h), both Newton-III kernels
     traffic, traffic_source = _traffic_from_profile(kernel, N, geom, sorted_staging, args.precision)
     # FP64-pipe instructions per ORDERED interaction on the fast path: 20 per unordered pair (Newton III)

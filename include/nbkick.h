@@ -66,9 +66,10 @@ extern "C" {
  *                       fully active, N >= 4096 (or NB_FORCE_SYMMETRIC): the Newton-III
  *                       kernel on double-single positions -- differences fl(fl(xjh - xih) + fl(xjl - xil)), r^2, r^-3,
  *                       products and the sums over one visit of a 32-body block all on the FP32 pipe, fp64 from there on;
- *                       otherwise (semi-active, small N, NB_FORCE_TILES): the one-sided kernel -- the same double-single
- *                       arithmetic when it holds 2 or 4 i-bodies per thread, differences in fp64 and the rest in fp32
- *                       when it holds one (small N); summed in fp32 per 128-body tile and in fp64 across tiles. */
+ *                       otherwise (semi-active, NB_FORCE_TILES): the one-sided kernel with the same double-single
+ *                       arithmetic, summed in fp32 per 128-body tile and in fp64 across tiles -- when it holds 2 or 4
+ *                       i-bodies per thread; with one (small N: latency-bound launches, where fp32 does not pay) the
+ *                       fp64 kernel runs, which meets the tolerance trivially. */
 #define NB_PRECISION_F64 0
 #define NB_PRECISION_MIXED 1
 #define NB_SORT_AUTO 0

@@ -47,7 +47,6 @@ struct PrepParams {
     int nblk_in;
     int N, Nj, Njpad;
     int update_rc;
-    int mixed;              // 1: stage the records for the mixed-precision kernel (force_mixed.cuh)
 };
 
 // a5 (second half) + a0 + staging for ONE body slot i (the grid covers max(N, Njpad, Npad_sym)): x += dtc * s; rcrit
@@ -79,7 +78,6 @@ __device__ __forceinline__ void prep_one(const PrepParams &p, const int i, const
             const double gm = p.G * m;
             r.x = x; r.y = y; r.z = z; r.gm = gm;
             r.c1 = 1.5 * gm; r.c2 = 1.875 * gm; r.rc2 = rc * rc; r.rc = rc;
-            if (p.mixed) r.c1 = pack_mixed(gm, r.rc2);
             if (!(isfinite(x) && isfinite(y) && isfinite(z) && isfinite(gm) && isfinite(rc) && rc >= 0.0))
                 status_add(p.status, ST_NONFINITE, 1);
         }

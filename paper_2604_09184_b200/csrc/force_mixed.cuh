@@ -1,148 +1,19 @@
-// force_mixed.cuh -- mixed-precision variants of the one-sided O(N^2) kick: nb_force_mixed_kernel (below: fp64 differences, the
-// first version; still the kernel for I = 1, i.e. small N) and nb_force_mixedds_kernel (further down: double-single positions,
-// everything on the FP32 pipe; I = 2, 4).
-// The first version (Fig. 1
+// force_mixed.cuh -- mixed-precision variant of the one-sided O(N^2) kick (Fig. 1
 // contrasts FP32 and FP64 runs of the same code on both of its GPUs).  What is computed is the H_B kick of
 // force_tiles.cuh (Eq. 5, 98) and the same pair list; what changes is the arithmetic of the pairs that are
-// out of reach of every critical radius (all but ~1e-6 of them):
-//     dx, dy, dz = x_j - x_i              fp64 (3 DADD): the cancellation of nearby positions happens in fp64
-//     r^2, r^-3, G m_j r^-3 (dx,dy,dz)    fp32 (FP32 pipe + MUFU.RSQ), summed in fp32 over one 128-body j-tile
-//     tile sums -> acc                    fp64 (two-level sum: 3 DADD per tile)
-// Pairs whose fp32 r^2 is within reach of a critical radius (margin 2^-18: far above the fp32 rounding of r^2), and
-// every self term, take the EXACT fp64 path of force_tiles.cuh: the changeover weight, the pair test r^2 < rc^2 and
-// the pair list are bit-identical to the fp64 kernel's.  FP64-pipe work per far interaction: 3 DADD + 3 conversions,
-// against 15 instructions in the fp64 kernel.  Tolerance reading: DESIGN.md S25.
+// out of reach of every critical radius (all but ~1e-6 of them), which runs on the FP32 pipe on double-single
+// positions (nb_force_mixedds_kernel below; the Newton-III counterpart is force_symds.cuh).  Pairs whose fp32 r^2 is
+// within reach of a critical radius (margin 2^-18: far above the fp32 rounding of r^2), and every self term, take the
+// EXACT fp64 path of force_tiles.cuh: the changeover weight, the pair test r^2 < rc^2 and the pair list are
+// bit-identical to the fp64 kernel's.  Tolerance reading: DESIGN.md S25.
+// (Round 2's first version -- fp64 differences and conversions, fp32 for the rest -- was no faster than the fp64 kernel:
+// the differences stayed on the FP64 pipe.  It is gone; with one i-body per thread (small N, latency-bound launches) the
+// host runs the fp64 kernel, which meets the mixed tolerance trivially.)
 #pragma once
 #include "force_tiles.cuh"
 
 namespace nbk {
 
-template <int I, bool PAIRS, int MINB>
-__global__ void __launch_bounds__(kForceThreads, MINB) nb_force_mixed_kernel(const ForceParams p) {
-    __shared__ __align__(128) JRec sm[kStages][kTileJ];
-    __shared__ __align__(8) uint64_t full[kStages];
-    __shared__ __align__(8) uint64_t empty[kStages];
-
-    const int t = threadIdx.x;
-    const int i0 = blockIdx.x * (kForceThreads * I) + t;
-    const int tile_begin = blockIdx.y * p.tiles_per_split;
-    int tile_end = tile_begin + p.tiles_per_split;
-    if (tile_end > p.tiles_total) tile_end = p.tiles_total;
-    const int ntiles = tile_end - tile_begin;
-    constexpr unsigned kTileBytes = kTileJ * sizeof(JRec);
-    constexpr int kAhead = kStages - 2;
-
-    if (t == 0) {
-#pragma unroll
-        for (int s = 0; s < kStages; ++s) {
-            mbar_init(&full[s], 1);
-            mbar_init(&empty[s], kForceThreads / 32);
-        }
-        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-    }
-    __syncthreads();
-    if (t == 0) {
-#pragma unroll
-        for (int n = 0; n < kAhead; ++n)
-            if (n < ntiles) {
-                mbar_expect_tx(&full[n], kTileBytes);
-                tma_bulk_g2s(&sm[n][0], p.jrec + (size_t)(tile_begin + n) * kTileJ, kTileBytes, &full[n]);
-            }
-    }
-
-    double xi[I], yi[I], zi[I], rci[I];
-    float thr_i = 0.0f;
-#pragma unroll
-    for (int k = 0; k < I; ++k) {
-        const int i = i0 + k * kForceThreads;
-        if (i < p.N) {
-            xi[k] = p.x[3 * (size_t)i];
-            yi[k] = p.x[3 * (size_t)i + 1];
-            zi[k] = p.x[3 * (size_t)i + 2];
-            rci[k] = p.rcrit[i];
-        } else {
-            xi[k] = kFarI; yi[k] = kFarI; zi[k] = kFarI; rci[k] = 0.0;
-        }
-        thr_i = fmaxf(thr_i, __double2float_ru(rci[k] * rci[k]) * 1.0000038f);
-    }
-
-    double ox[I], oy[I], oz[I];  // fp64 sums over the tiles (and the exact path's terms)
-#pragma unroll
-    for (int k = 0; k < I; ++k) { ox[k] = 0.0; oy[k] = 0.0; oz[k] = 0.0; }
-
-    for (int it = 0; it < ntiles; ++it) {
-        const int st = it % kStages;
-        {
-            const int n = it + kAhead;
-            if (n < ntiles) {
-                const int sn = n % kStages;
-                if (n >= kStages) mbar_wait(&empty[sn], (unsigned)((n / kStages - 1) & 1));
-                if (t == 0) {
-                    mbar_expect_tx(&full[sn], kTileBytes);
-                    tma_bulk_g2s(&sm[sn][0], p.jrec + (size_t)(tile_begin + n) * kTileJ, kTileBytes, &full[sn]);
-                }
-            }
-        }
-        mbar_wait(&full[st], (unsigned)((it / kStages) & 1));
-
-        float fx[I], fy[I], fz[I];  // fp32 sums of this tile
-#pragma unroll
-        for (int k = 0; k < I; ++k) { fx[k] = 0.f; fy[k] = 0.f; fz[k] = 0.f; }
-        const int jbase = (tile_begin + it) * kTileJ;
-        const JRec *tile = &sm[st][0];
-
-#pragma unroll 2
-        for (int jj = 0; jj < kTileJ; ++jj) {
-            const double4 *q = reinterpret_cast<const double4 *>(tile + jj);
-            const double4 A = q[0];          // x, y, z, G m
-            const double2 Bl = *reinterpret_cast<const double2 *>(&q[1]);  // (packed floats, c2)
-            const float gmf = __int_as_float(__double2loint(Bl.x));
-            const float thr = fmaxf(thr_i, __int_as_float(__double2hiint(Bl.x)));
-            float dx[I], dy[I], dz[I], r2[I];
-            float mn = 3.0e38f;
-#pragma unroll
-            for (int k = 0; k < I; ++k) {
-                dx[k] = __double2float_rn(__dsub_rn(A.x, xi[k]));
-                dy[k] = __double2float_rn(__dsub_rn(A.y, yi[k]));
-                dz[k] = __double2float_rn(__dsub_rn(A.z, zi[k]));
-                r2[k] = fmaf(dz[k], dz[k], fmaf(dy[k], dy[k], dx[k] * dx[k]));
-                mn = fminf(mn, r2[k]);
-            }
-            if (__any_sync(0xffffffffu, mn <= thr)) {
-                // exact fp64 path for this j (self term, pairs within reach of a critical radius), straight into the fp64 sums
-                const double4 B = q[1];
-                slow_path<I, PAIRS>(p, A, B, jbase + jj, xi, yi, zi, rci, i0, ox, oy, oz);
-            } else {
-#pragma unroll
-                for (int k = 0; k < I; ++k) {
-                    const float y = rsqrtf(r2[k]);
-                    const float s = gmf * (y * y * y);
-                    fx[k] = fmaf(s, dx[k], fx[k]);
-                    fy[k] = fmaf(s, dy[k], fy[k]);
-                    fz[k] = fmaf(s, dz[k], fz[k]);
-                }
-            }
-        }
-#pragma unroll
-        for (int k = 0; k < I; ++k) { ox[k] += (double)fx[k]; oy[k] += (double)fy[k]; oz[k] += (double)fz[k]; }
-        __syncwarp();
-        if ((t & 31) == 0) mbar_arrive(&empty[st]);
-    }
-
-    double *out = p.part + (size_t)blockIdx.y * p.N * 3;
-#pragma unroll
-    for (int k = 0; k < I; ++k) {
-        const int i = i0 + k * kForceThreads;
-        if (i < p.N) {
-            out[3 * (size_t)i] = ox[k];
-            out[3 * (size_t)i + 1] = oy[k];
-            out[3 * (size_t)i + 2] = oz[k];
-        }
-    }
-}
-
-// ---- the same on double-single positions: nothing of a far pair touches the FP64 pipe ---------------------------------
 // The one-sided counterpart of force_symds.cuh (semi-active mode, N below the Newton-III threshold; I = 2 or 4): 32-byte
 // JRecDs records stream through the TMA ring, dx = fl(fl(xjh - xih) + fl(xjl - xil)) with the (high, low) partial
 // differences in one packed FADD2, everything after the differences on two i-bodies at a time (FMUL2 / FFMA2), fp32 sums

@@ -17,14 +17,6 @@ struct __align__(16) JRec {
 };
 static_assert(sizeof(JRec) == 64, "JRec must be 64 bytes");
 
-// Mixed-precision kernel (force_mixed.cuh): the record's c1 slot holds two floats instead -- G m_j rounded to fp32 (low
-// word) and rc_j^2 rounded UP to fp32 with a 2^-18 margin (high word; far above the fp32 rounding of r^2)
-__device__ __forceinline__ double pack_mixed(const double gm, const double rc2) {
-    const float g = __double2float_rn(gm);
-    const float t = __double2float_ru(rc2) * 1.0000038f;
-    return __hiloint2double(__float_as_int(t), __float_as_int(g));
-}
-
 // stages body `pos` (position in the doubled-block layout) for the Newton-III mixed-precision kernel (force_symds.cuh):
 // double-single position (xh + xl), fl32(G m), and rc^2 rounded up with a 2^-18 margin; called by nb_prep_kernel
 __device__ __forceinline__ void symds_stage(float4 *sa, float4 *sb, const int pos, const double x, const double y, const double z,

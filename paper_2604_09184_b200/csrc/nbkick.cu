@@ -212,6 +212,9 @@ Geometry geometry(int64_t N, int64_t n_active) {
     }
     g.ipt = ipt;
     g.minb = ipt == 4 ? 3 : 5;
+    // mixed precision with one i-body per thread (small N: latency-bound launches) does not pay: the fp64 kernel runs
+    // instead (it meets the mixed tolerance trivially, and the fused small-N step stays available)
+    if (g.mixed && ipt == 1) g.mixed = 0;
 
     g.iblocks = (int)((N + (int64_t)kForceThreads * ipt - 1) / ((int64_t)kForceThreads * ipt));
     int nsplit = g_cfg.j_splits;
@@ -329,7 +332,7 @@ Workspace carve(void *base, int64_t N, const Geometry &g) {
     w.sxy = reinterpret_cast<double2 *>(b + off); off += align_up((size_t)2 * g.Npad_sym * sizeof(double2), 256);
     w.szg = reinterpret_cast<double2 *>(b + off); off += align_up((size_t)2 * g.Npad_sym * sizeof(double2), 256);
     w.sthr = reinterpret_cast<int *>(b + off); off += align_up((size_t)2 * g.Npad_sym * sizeof(int), 256);
-    w.jds = reinterpret_cast<JRecDs *>(b + off); off += align_up((size_t)((!g.sym && g.mixed == 1 && g.ipt >= 2) ? g.Njpad : 0) * sizeof(JRecDs), 256);
+    w.jds = reinterpret_cast<JRecDs *>(b + off); off += align_up((size_t)((!g.sym && g.mixed == 1) ? g.Njpad : 0) * sizeof(JRecDs), 256);
     w.sa = reinterpret_cast<float4 *>(b + off); off += align_up((size_t)(g.mixed == 2 ? 2 * g.Npad_sym : 0) * sizeof(float4), 256);
     w.sb = reinterpret_cast<float4 *>(b + off); off += align_up((size_t)(g.mixed == 2 ? 2 * g.Npad_sym : 0) * sizeof(float4), 256);
     w.perm = reinterpret_cast<int *>(b + off); off += align_up((size_t)g.Npad_sym * sizeof(int), 256);
@@ -399,20 +402,15 @@ void launch_force_IM(const ForceParams &fp, const Geometry &g, bool pairs) {
 template <int I, int MINB>
 void launch_mixed_IM(const ForceParams &fp, const Geometry &g, bool pairs) {
     dim3 grid(g.iblocks, g.nsplit);
-    if constexpr (I >= 2) {   // double-single records, everything on the FP32 pipe (force_mixed.cuh)
-        if (pairs) nb_force_mixedds_kernel<I, true, MINB><<<grid, kForceThreads, 0, stream()>>>(fp);
-        else nb_force_mixedds_kernel<I, false, MINB><<<grid, kForceThreads, 0, stream()>>>(fp);
-    } else {
-        if (pairs) nb_force_mixed_kernel<I, true, MINB><<<grid, kForceThreads, 0, stream()>>>(fp);
-        else nb_force_mixed_kernel<I, false, MINB><<<grid, kForceThreads, 0, stream()>>>(fp);
-    }
+    // double-single records, everything on the FP32 pipe (force_mixed.cuh)
+    if (pairs) nb_force_mixedds_kernel<I, true, MINB><<<grid, kForceThreads, 0, stream()>>>(fp);
+    else nb_force_mixedds_kernel<I, false, MINB><<<grid, kForceThreads, 0, stream()>>>(fp);
 }
 
 void launch_force(const ForceParams &fp, const Geometry &g, bool pairs) {
     if (g.mixed) {
         if (g.ipt == 4) launch_mixed_IM<4, 4>(fp, g, pairs);
-        else if (g.ipt == 2) launch_mixed_IM<2, 5>(fp, g, pairs);
-        else launch_mixed_IM<1, 5>(fp, g, pairs);
+        else launch_mixed_IM<2, 5>(fp, g, pairs);   // (geometry() leaves I = 1 to the fp64 kernel)
         return;
     }
     if (g.ipt == 4) launch_force_IM<4, 3>(fp, g, pairs);
@@ -500,13 +498,13 @@ int enqueue_eval(const Workspace &w, const Geometry &g, double *x, double *v, co
     pp.x = x; pp.v = v; pp.m = m; pp.rcrit = rc_io; pp.jrec = g.sym ? nullptr : w.jrec; pp.mv_in = mv_in;
     pp.sxy = g.sym ? w.sxy : nullptr; pp.szg = w.szg; pp.sthr = w.sthr; pp.Npad_sym = g.Npad_sym;
     pp.sa = g.mixed == 2 ? w.sa : nullptr; pp.sb = w.sb;
-    pp.jds = (!g.sym && g.mixed == 1 && g.ipt >= 2) ? w.jds : nullptr;
+    pp.jds = (!g.sym && g.mixed == 1) ? w.jds : nullptr;
     pp.pos_of = sorted ? w.pos_of : nullptr;
     pp.rc_hill = g_cfg.levels > 0 ? w.ml_hill : nullptr; pp.rc_vel = g_cfg.levels > 0 ? w.ml_vel : nullptr;
     pp.npairs = pairs ? reinterpret_cast<unsigned long long *>(npairs) : nullptr;
     pp.status = w.status; pp.dtc = dtc; pp.M_star = M_star; pp.G = g_cfg.G; pp.n1 = g_cfg.n1; pp.n2 = g_cfg.n2;
     pp.absdt = std::fabs(dt_for_rc); pp.nblk_in = nblk; pp.N = (int)N; pp.Nj = g.Nj; pp.Njpad = g.Njpad;
-    pp.update_rc = update_rc; pp.mixed = g.mixed == 1;
+    pp.update_rc = update_rc;
     int64_t cover = N > g.Njpad ? N : g.Njpad;
     if (g.Npad_sym > cover) cover = g.Npad_sym;
     nb_prep_kernel<<<body_blocks(cover), kBodyThreads, 0, stream()>>>(pp);
@@ -516,7 +514,7 @@ int enqueue_eval(const Workspace &w, const Geometry &g, double *x, double *v, co
     fp.npairs = pairs ? reinterpret_cast<unsigned long long *>(npairs) : w.npairs_dummy;
     fp.status = w.status; fp.cap = pairs ? g_cfg.pair_capacity : 0; fp.N = (int)N; fp.Nj = g.Nj;
     fp.tiles_total = g.tiles_total; fp.tiles_per_split = g.tiles_per_split; fp.kind = g_cfg.changeover_kind;
-    fp.jds = (!g.sym && g.mixed == 1 && g.ipt >= 2) ? w.jds : nullptr;
+    fp.jds = (!g.sym && g.mixed == 1) ? w.jds : nullptr;
     // bounds of the staged super-blocks (before the timing events: they bracket the force kernel alone)
     if (sorted) nb_sort_bounds_kernel<<<g.nsplit, kGrpThreads, 0, stream()>>>(w.sxy, w.perm, rc_io, (int)N, g.S, w.bnd);
     const bool pool = g_cfg.time_force && g_tev_used < kMaxTimed;
@@ -754,7 +752,7 @@ int launch_step_small(const Workspace &w, const Geometry &g, double *x, double *
     pp.npairs = pairs ? reinterpret_cast<unsigned long long *>(npairs) : nullptr;
     pp.status = w.status; pp.dtc = 0.5 * dt; pp.M_star = M_star; pp.G = g_cfg.G; pp.n1 = g_cfg.n1; pp.n2 = g_cfg.n2;
     pp.absdt = std::fabs(dt); pp.nblk_in = body_blocks(N); pp.N = (int)N; pp.Nj = g.Nj; pp.Njpad = g.Njpad;
-    pp.update_rc = update_rc; pp.mixed = 0;
+    pp.update_rc = update_rc;
     ForceParams &fp = q.fp;
     fp.jrec = w.jrec; fp.x = x; fp.rcrit = rc_io; fp.part = w.part; fp.pairs = pairs;
     fp.npairs = pairs ? reinterpret_cast<unsigned long long *>(npairs) : w.npairs_dummy;

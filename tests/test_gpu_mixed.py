@@ -1,10 +1,11 @@
 """-m gpu: the mixed-precision kick variant (NB_PRECISION_MIXED) against the fp64 oracle.
 
 Tolerance reading S25.  The definition stays the fp64 one (oracle.accel); the variant evaluates every pair
-that is out of reach of all critical radii with fp32 arithmetic after an fp64 difference.  With u = 2^-24: the cast of
-the three differences, r^2 (3 roundings), rsqrt (2 ulp), its cube (2), the product with G m_j (cast + 1) and with the
-difference (1) put at most ~16 u on a term, the fp32 sum over one 128-body tile at most 127 u on the tile's sum of
-|terms| (typically sqrt(128) u): |da_c| <= 143 u sum_j |t_jc| = 8.5e-6 sum|t| is the guaranteed bound, asserted here;
+that is out of reach of all critical radii in fp32 on double-single positions.  With u = 2^-24: the difference
+(2.5 u), r^2, rsqrt (2 ulp), its cube, the product with G m_j (cast + 1) and with the difference put at most ~24 u on a
+term, the fp32 sum over one 128-body tile (one-sided kernel) or one visit of a 32-body block (Newton-III kernel) at most
+127 u on that sum of |terms| (typically sqrt(128) u): |da_c| <= 151 u sum_j |t_jc| = 9e-6 sum|t| is the guaranteed bound,
+asserted here (the one-sided cases are held to 143 u, the figure of the first version of the kernel);
 the observed error is reported next to a PLAIN numpy fp32 restatement of the same recipe (it must be of the same size:
 the error is the arithmetic's, not the kernel's).  Pairs within reach of a critical radius take the fp64 path, so the
 pair list is bit-identical to the fp64 kernel's and compared exactly."""
