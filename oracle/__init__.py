@@ -435,7 +435,8 @@ def _pairs_within(x, p, rc_level):
     return p[r2 < rc * rc]
 
 
-def encounter_ml(x, v, m, rcl, M_star, dt, G, pairs0, kind=0, tol=1e-12, max_group=1024):
+def encounter_ml(x, v, m, rcl, M_star, dt, G, pairs0, kind=0, tol=1e-12, max_group=1024, radius=None, radius_factor=1.0,
+                 absorbed_by=None):
     """H_A over dt for the bodies of the pair list pairs0 with L = len(rcl) - 1 intermediate levels (reading S23).
 
         advance(l, P, tau):                      # Kepler + sum_{pairs in P} (pair force) Omega_l, for the bodies of P
@@ -447,26 +448,34 @@ def encounter_ml(x, v, m, rcl, M_star, dt, G, pairs0, kind=0, tol=1e-12, max_gro
                 kick  h/2 with weight Omega_l W_{l+1} over P
 
     L = 0 is oracle.encounter on the groups of pairs0.  Bodies outside pairs0 are not touched (the caller drifts them).
+    radius given: the direct solver of the innermost level examines collisions (reading S26); the masses then change on
+    the way -- the level kicks that follow use the merged masses -- and stats also holds m, radius, absorbed_by, absorbed.
     Returns (x, v, stats) with stats = dict(integrated, skipped, failed, steps, kicks, level_pairs[L+1])."""
     x = np.array(x, dtype=np.float64, order="C"); v = np.array(v, dtype=np.float64, order="C")
-    m = np.ascontiguousarray(m, dtype=np.float64)
+    m = np.array(m, dtype=np.float64)
     N = m.shape[0]
+    R = None if radius is None else np.array(radius, dtype=np.float64)
+    ab = None if radius is None else (np.full(N, -1, dtype=np.int32) if absorbed_by is None else np.array(absorbed_by, dtype=np.int32))
     rcl = np.ascontiguousarray(rcl, dtype=np.float64).reshape(-1, N)
     L = rcl.shape[0] - 1
-    stats = dict(integrated=0, skipped=0, failed=0, steps=0, kicks=0, level_pairs=[0] * (L + 1))
+    stats = dict(integrated=0, skipped=0, failed=0, steps=0, kicks=0, absorbed=0, level_pairs=[0] * (L + 1))
     P0 = _canon(np.asarray(pairs0, dtype=np.int32).reshape(-1, 2))
 
     def bodies(P):
         return np.unique(P.reshape(-1)) if P.shape[0] else np.zeros(0, dtype=np.int64)
 
     def advance(l, P, tau):
-        nonlocal x, v
+        nonlocal x, v, m, R, ab
         stats["level_pairs"][l] += int(P.shape[0])
         if P.shape[0] == 0:
             return
         if l == L:
             grp = groups(P, N)
-            xe, ve, st = encounter(x, v, m, rcl, M_star, tau, G, grp, kind=kind, tol=tol, max_group=max_group)
+            xe, ve, st = encounter(x, v, m, rcl, M_star, tau, G, grp, kind=kind, tol=tol, max_group=max_group,
+                                   radius=R, radius_factor=radius_factor, absorbed_by=ab)
+            if R is not None:
+                m, R, ab = st["m"], st["radius"], st["absorbed_by"]
+                stats["absorbed"] += st["absorbed"]
             # groups beyond max_group are left to the Kepler drift (counted), as in step_enc
             big = np.zeros(N, dtype=bool)
             for g in range(grp["ngroups"]):
@@ -495,17 +504,23 @@ def encounter_ml(x, v, m, rcl, M_star, dt, G, pairs0, kind=0, tol=1e-12, max_gro
             stats["kicks"] += 2
 
     advance(0, P0, dt)
+    if R is not None:
+        stats.update(m=m, radius=R, absorbed_by=ab)
     return x, v, stats
 
 
-def step_ml(x, v, m, M_star, dt, G, nsteps, nlev, n1=3.0, n2=0.4, kind=0, tol=1e-12, max_group=1024, rcrit0=None):
+def step_ml(x, v, m, M_star, dt, G, nsteps, nlev, n1=3.0, n2=0.4, kind=0, tol=1e-12, max_group=1024, rcrit0=None,
+            radius=None, radius_factor=1.0):
     """nsteps of B(dt/2) C(dt/2) A(dt) C(dt/2) B(dt/2) with the close encounters of A resolved through nlev - 1 intermediate
     levels (encounter_ml); nlev = 1 is step_enc.  Level radii by level_rcrit from the state at each force evaluation
-    (S17), held through the step.  Returns dict(x, v, acc, rcrit [nlev, N], pairs, stats)."""
+    (S17), held through the step.  radius given: collisions inside the innermost solver (reading S26), as in step_enc.
+    Returns dict(x, v, acc, rcrit [nlev, N], pairs, stats [, m, radius, absorbed_by])."""
     x = np.array(x, dtype=np.float64, order="C"); v = np.array(v, dtype=np.float64, order="C")
-    m = np.ascontiguousarray(m, dtype=np.float64)
+    m = np.array(m, dtype=np.float64)
     N = m.shape[0]
-    tot = dict(integrated=0, skipped=0, failed=0, steps=0, kicks=0, border=0, level_pairs=[0] * nlev)
+    tot = dict(integrated=0, skipped=0, failed=0, steps=0, kicks=0, border=0, absorbed=0, level_pairs=[0] * nlev)
+    R = None if radius is None else np.array(radius, dtype=np.float64)
+    ab = np.full(N, -1, dtype=np.int32)
 
     def evaluate(x, v):
         rcl = level_rcrit(x, v, m, M_star, dt, G, n1, n2, nlev, rcrit0)
@@ -521,7 +536,11 @@ def step_ml(x, v, m, M_star, dt, G, nsteps, nlev, n1=3.0, n2=0.4, kind=0, tol=1e
         inside = np.zeros(N, dtype=bool)
         inside[pr.reshape(-1)] = True
         free = np.flatnonzero(~inside)
-        xe, ve, st = encounter_ml(x, v, m, rcl, M_star, dt, G, pr, kind=kind, tol=tol, max_group=max_group)
+        xe, ve, st = encounter_ml(x, v, m, rcl, M_star, dt, G, pr, kind=kind, tol=tol, max_group=max_group,
+                                  radius=R, radius_factor=radius_factor, absorbed_by=ab)
+        if R is not None:
+            m, R, ab = st["m"], st["radius"], st["absorbed_by"]
+            tot["absorbed"] += st["absorbed"]
         if free.size:
             xk, vk, nf = drift_kepler(x[free], v[free], M_star, dt, G)
             xe[free] = xk; ve[free] = vk
@@ -533,7 +552,10 @@ def step_ml(x, v, m, M_star, dt, G, nsteps, nlev, n1=3.0, n2=0.4, kind=0, tol=1e
         x = shift(x, v, m, M_star, 0.5 * dt)
         rcl, acc, pr = evaluate(x, v)
         v = v + (0.5 * dt) * acc
-    return dict(x=x, v=v, acc=acc, rcrit=rcl, pairs=pr, stats=tot)
+    out = dict(x=x, v=v, acc=acc, rcrit=rcl, pairs=pr, stats=tot)
+    if R is not None:
+        out.update(m=m, radius=R, absorbed_by=ab)
+    return out
 
 
 def merge(x, v, m, radius, pairs_, f=1.0):

@@ -176,3 +176,24 @@ def test_bodies_absorbed_in_an_earlier_call_stay_out_of_the_encounter():
     assert s3["failed"] == 0 and s3["absorbed"] == 2 and np.array_equal(s3["absorbed_by"], s1["absorbed_by"])
     live = s3["absorbed_by"][seg] < 0
     assert np.max(np.abs(x3[seg][live] - x2[seg][live])) <= 1e-11
+
+
+def test_multilevel_steps_with_radii():
+    """The multi-level scheme (reading S23) with collisions in its innermost solver: one level (nlev = 1) is step_enc with
+    radii bit for bit; radii too small to touch => step_ml bit for bit; inflated radii => bodies absorbed, mass conserved,
+    no failures, and about as many absorbed as the one-level scheme finds on the same input."""
+    import nb_inputs
+    d = nb_inputs.make_config(2, n_override=1200)
+    a = oracle.step_enc(d.x, d.v, d.m, d.M_star, d.dt, G, 2, n1=3.0, n2=0.4, radius=d.radius, radius_factor=400.0)
+    b = oracle.step_ml(d.x, d.v, d.m, d.M_star, d.dt, G, 2, 1, n1=3.0, n2=0.4, radius=d.radius, radius_factor=400.0)
+    assert np.array_equal(a["x"], b["x"]) and np.array_equal(a["v"], b["v"]) and np.array_equal(a["m"], b["m"])
+    assert np.array_equal(a["absorbed_by"], b["absorbed_by"]) and a["stats"]["absorbed"] == b["stats"]["absorbed"] > 0
+    c0 = oracle.step_ml(d.x, d.v, d.m, d.M_star, d.dt, G, 2, 3, n1=3.0, n2=0.4)
+    c1 = oracle.step_ml(d.x, d.v, d.m, d.M_star, d.dt, G, 2, 3, n1=3.0, n2=0.4, radius=d.radius, radius_factor=1.0)
+    assert c1["stats"]["absorbed"] == 0 and np.array_equal(c0["x"], c1["x"]) and np.array_equal(c0["v"], c1["v"])
+    c = oracle.step_ml(d.x, d.v, d.m, d.M_star, d.dt, G, 2, 3, n1=3.0, n2=0.4, radius=d.radius, radius_factor=400.0)
+    assert c["stats"]["failed"] == 0 and c["stats"]["absorbed"] > 0
+    assert abs(c["m"].sum() - d.m.sum()) <= 1e-15 * d.m.sum()
+    assert abs(c["stats"]["absorbed"] - a["stats"]["absorbed"]) <= max(3, a["stats"]["absorbed"] // 2)
+    gone = np.flatnonzero(c["absorbed_by"] >= 0)
+    assert np.all(c["m"][gone] == 0.0) and np.all(c["m"][c["absorbed_by"][gone]] > 0.0)
