@@ -128,7 +128,8 @@ typedef struct nb_config {
                                 collisions inside the direct solver (nb_encounter_collide; reading S26),
                                 inflated by radius_factor.  The step then CHANGES m (the caller's array, although nb_step
                                 takes it as const) and the radii: an absorbed body stays in the arrays with m = 0, R = 0
-                                on the body that holds it until nb_merge compacts them.  levels = 0, fully active case.
+                                on the body that holds it until nb_merge compacts them.  Fully active case; with levels > 0 the
+                                innermost solver examines the collisions and the level kicks that follow use the merged masses.
                                 Default NULL: off */
     int32_t *collide_absorbed_by; /* with collide_radius: DEVICE int32[N] in/out, -1 or the body that holds an absorbed body
                                 (initialise with -1; required) */

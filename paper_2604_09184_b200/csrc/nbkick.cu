@@ -692,23 +692,25 @@ void enqueue_ml_adjacency(const Workspace &w, const int32_t *pairs, const int64_
     nb_ml_listed_kernel<<<nb256, kGrpThreads, 0, stream()>>>(w.ml, n, w.ml_listed);
 }
 
-void enqueue_ml_advance(const Workspace &w, const MlParams &mp, double M_star, int64_t N, int l, double tau) {
+void enqueue_ml_advance(const Workspace &w, const MlParams &mp, double M_star, int64_t N, int l, double tau,
+                        double *radius = nullptr, int *absorbed_by = nullptr /* collisions in the innermost solver (S26) */) {
     const int nb256 = ((int)N + kGrpThreads - 1) / kGrpThreads;
     if (l == mp.L) {
         // the innermost level: groups of P_L -> plan -> bodies of groups beyond the solver's cap drift -> direct solver
         enqueue_groups(w, nullptr, nullptr, N, w.g_label, w.g_members, w.g_start, w.g_stat, GroupFilter{nullptr, nullptr, 1.0, nullptr}, l);
         enqueue_encounter_plan(w, N, w.g_members, w.g_start, w.g_stat);
         nb_ml_drift_kernel<<<nb256, kGrpThreads, 0, stream()>>>(mp, l, tau, w.enc_flag);
-        enqueue_encounter(w, mp.x, mp.v, mp.m, mp.hill, M_star, N, tau, w.g_members, w.g_start, w.g_stat, true, mp.vel, mp.L + 1);
+        enqueue_encounter(w, mp.x, mp.v, mp.m, mp.hill, M_star, N, tau, w.g_members, w.g_start, w.g_stat, true, mp.vel, mp.L + 1,
+                          radius, absorbed_by);
         return;
     }
     const double h = 0.5 * tau;
     nb_ml_kick_kernel<true><<<nb256, kGrpThreads, 0, stream()>>>(mp, l, 0.5 * h, 1);
     nb_ml_drift_kernel<<<nb256, kGrpThreads, 0, stream()>>>(mp, l, h, nullptr);
-    enqueue_ml_advance(w, mp, M_star, N, l + 1, h);
+    enqueue_ml_advance(w, mp, M_star, N, l + 1, h, radius, absorbed_by);
     nb_ml_kick_kernel<true><<<nb256, kGrpThreads, 0, stream()>>>(mp, l, 0.5 * h, 2);
     nb_ml_drift_kernel<<<nb256, kGrpThreads, 0, stream()>>>(mp, l, h, nullptr);
-    enqueue_ml_advance(w, mp, M_star, N, l + 1, h);
+    enqueue_ml_advance(w, mp, M_star, N, l + 1, h, radius, absorbed_by);
     nb_ml_kick_kernel<false><<<nb256, kGrpThreads, 0, stream()>>>(mp, l, 0.5 * h, 1);
 }
 
@@ -814,7 +816,7 @@ int step_impl(double *x, double *v, const double *m, double M_star, int64_t N, d
     // collisions examined inside the direct solver (reading S26): m and the radii change on the way
     const bool coll = enc && g_cfg.collide_radius != nullptr;
     if (coll && !g_cfg.collide_absorbed_by) return fail(NB_E_NULL, "nb_step: collide_radius is set but collide_absorbed_by is NULL");
-    if (coll && (ml || g.Nj != N)) return fail(NB_E_BADARG, "nb_step: collisions inside the solver (collide_radius) need levels = 0 and the fully active case");
+    if (coll && g.Nj != N) return fail(NB_E_BADARG, "nb_step: collisions inside the solver (collide_radius) are defined for the fully active case");
     if (ml && g.Nj != N) return fail(NB_E_BADARG, "nb_step: the multi-level changeover (levels > 0) is defined for the fully active case only");
     // force evaluation that closes a step: closing half-kick [+ opening half-kick of the next step]; with the extra
     // force the two half-kicks are separated by D(dt/2) D(dt/2)
@@ -834,7 +836,8 @@ int step_impl(double *x, double *v, const double *m, double M_star, int64_t N, d
             enqueue_ml_adjacency(w, pairs, npairs, N);
             nb_drift_kernel<<<nblk, kBodyThreads, 0, stream()>>>(x, v, m, (int)N, mu, dt, w.mvA, nblk, dtc, M_star, nullptr, w.status,
                                                                  w.ml_listed);
-            enqueue_ml_advance(w, ml_params(w, x, v, m, w.ml_hill, w.ml_vel, M_star, N), M_star, N, 0, dt);
+            enqueue_ml_advance(w, ml_params(w, x, v, m, w.ml_hill, w.ml_vel, M_star, N), M_star, N, 0, dt,
+                               coll ? g_cfg.collide_radius : nullptr, coll ? g_cfg.collide_absorbed_by : nullptr);
             nb_momentum_kernel<<<nblk, kBodyThreads, 0, stream()>>>(v, m, (int)N, w.mvB);
             return close_step(nhalf);
         }

@@ -191,7 +191,7 @@ def test_step_with_collisions_inside_the_solver(use_graph):
 
 
 def test_error_codes_of_the_collision_calls():
-    """Host-detectable misuse: semi-active mode, levels > 0, a missing absorbed_by array."""
+    """Host-detectable misuse: semi-active mode, a missing absorbed_by array."""
     import paper_2604_09184_b200 as nb
     torch = torch_mod()
     d = nb_inputs.make_config(2, n_override=600)
@@ -209,7 +209,7 @@ def test_error_codes_of_the_collision_calls():
     with pytest.raises(nb.NbError) as e:
         nb.nb_step(x, v, m, d.M_star, d.dt, rc, acc, pairs, npairs, 1)
     assert e.value.code == nb.binding.NB_E_NULL
-    nb.configure(d.N, G=G_GAUSS, pair_capacity=1024, resolve_encounters=True, levels=2, collide_radius=R, collide_absorbed_by=ab)
+    nb.configure(d.N, G=G_GAUSS, pair_capacity=1024, resolve_encounters=True, n_active=100, collide_radius=R, collide_absorbed_by=ab)
     with pytest.raises(nb.NbError) as e:
         nb.nb_step(x, v, m, d.M_star, d.dt, rc, acc, pairs, npairs, 1)
     assert e.value.code == nb.binding.NB_E_BADARG
@@ -220,3 +220,31 @@ def test_error_codes_of_the_collision_calls():
     nb.nb_encounter_collide(x, v, m, R, rc, d.M_star, d.dt, members, gstart, gstat, ab)
     torch.cuda.synchronize()
     assert np.array_equal(x.cpu().numpy(), d.x) and int(ab.max().item()) == -1
+
+
+def test_multilevel_step_with_collisions_inside_the_innermost_solver():
+    """nb_step(levels = 2, collide_radius) against oracle.step_ml(nlev = 3, radius=...): the masses change inside the
+    recursion and the level kicks that follow use them."""
+    import paper_2604_09184_b200 as nb
+    torch = torch_mod()
+    d = nb_inputs.make_config(2, n_override=1200)
+    nsteps, f, L = 2, 400.0, 2
+    ref = oracle.step_ml(d.x, d.v, d.m, d.M_star, d.dt, G_GAUSS, nsteps, L + 1, n1=3.0, n2=0.4, radius=d.radius, radius_factor=f)
+    assert ref["stats"]["absorbed"] >= 3 and ref["stats"]["failed"] == 0 and ref["stats"]["border"] == 0
+    x, v, m, R = to_dev(d.x), to_dev(d.v), to_dev(d.m), to_dev(d.radius)
+    ab = torch.full((d.N,), -1, dtype=torch.int32, device="cuda")
+    acc = torch.zeros_like(x); rcd = torch.zeros(d.N, dtype=torch.float64, device="cuda")
+    cap = 1 << 16
+    pairs = torch.zeros((cap, 2), dtype=torch.int32, device="cuda"); npairs = torch.zeros(1, dtype=torch.int64, device="cuda")
+    nb.configure(d.N, G=G_GAUSS, n1=3.0, n2=0.4, pair_capacity=cap, resolve_encounters=True, levels=L, radius_factor=f,
+                 collide_radius=R, collide_absorbed_by=ab)
+    nb.nb_status_reset()
+    nb.nb_step(x, v, m, d.M_star, d.dt, rcd, acc, pairs, npairs, nsteps)
+    torch.cuda.synchronize()
+    st = nb.nb_status()
+    assert st["bs_fail"] == 0 and st["groups_skipped"] == 0 and st["absorbed"] == ref["stats"]["absorbed"]
+    assert np.array_equal(ab.cpu().numpy(), ref["absorbed_by"]) and np.array_equal(m.cpu().numpy(), ref["m"])
+    ex = np.max(np.abs(x.cpu().numpy() - ref["x"])) / np.max(np.abs(ref["x"]))
+    ev = np.max(np.abs(v.cpu().numpy() - ref["v"])) / np.max(np.abs(ref["v"]))
+    print(f"levels = {L} with collisions: absorbed {st['absorbed']}, rel dx {ex:.2e} dv {ev:.2e}")
+    assert ex <= ENC_TOL and ev <= ENC_TOL
