@@ -361,7 +361,10 @@ __global__ void __launch_bounds__(256) nb_enc_plan_kernel(const int *__restrict_
         const bool split = nc <= 31 && nc < n;
         const int take = (split ? nc : n) <= kMaxGroup;
         if (lane == 0) gcore[g] = nc;
-        for (int k = lane; k < n; k += 32) flag[members[g0 + k]] = take;
+        // the flags start at 0 (memset by the host): a group the solver does not take -- the one giant group of a dense disk,
+        // 65 000 members written by one warp: 1.3 ms -- has nothing to write
+        if (take)
+            for (int k = lane; k < n; k += 32) flag[members[g0 + k]] = 1;
     }
 }
 
@@ -528,7 +531,9 @@ __device__ __forceinline__ int enc_group_size(const EncParams &p, const long lon
     return split ? nc : n;
 }
 
-__global__ void __launch_bounds__(32 * kBsCols) nb_encounter_small_kernel(const EncParams p) {
+// (two CTAs per SM: the collision code must not cost the second one -- 146 registers uncapped, measured 37.9 -> 52.1 ms per
+// step on config 3 with 4 levels)
+__global__ void __launch_bounds__(32 * kBsCols, 2) nb_encounter_small_kernel(const EncParams p) {
     __shared__ long long sh_next;
     const int lane = threadIdx.x & 31;
     const long long ngroups = p.gstat[0];
