@@ -407,80 +407,102 @@ __device__ __forceinline__ void bs_small_problem(const EncParams &p, const int b
     __syncthreads();
     const double my_rc = act ? src[lane] : 0.0, my_vel = act ? svel[lane] : 0.0;
     double T[kBsCols][6];                // warp 0: current row of the tableau
+    // A trial step whose first few columns already pass does not need the long ones: the columns are computed in two
+    // passes -- 1 .. first, then (only if none of them passed) first + 1 .. 8 -- with first = 4 for the FIRST trial step
+    // of the short intervals of the multi-level scheme (dt / 2^L: most problems are done in that one step, in 3 or 4
+    // columns), else 8 (one pass).  The tableau is still built column by column and the first column that passes is
+    // taken: the result is the sequential algorithm's; the critical path of such a step falls from 17 to 9 right-hand
+    // sides.  (Measured and rejected: first = 4 after every step accepted in <= 4 columns -- the step-size rule grows h
+    // until ~6 columns are needed, so the next step usually pays both passes: 3 R_Hill with encounters 7.0 -> 8.8 ms.)
+    __shared__ int ctrl_first, ctrl_more;
+    if (threadIdx.x == 0) ctrl_first = p.nlev > 1 ? 4 : kBsCols;
+    __syncthreads();
     while (true) {
         if (ctrl_done != 0) break;
         double h = ctrl_h;
         const double tcur = ctrl_t;
         if (fabs(h) > fabs(p.dt - tcur)) h = p.dt - tcur;
         const bool underflow = fabs(h) < 1e-14 * fabs(p.dt);
+        const int first = ctrl_first;
         double y[6];
 #pragma unroll
         for (int k = 0; k < 6; ++k) y[k] = act ? ycur[k][lane] : 0.0;
-        if (!underflow) {
-            // column c = w + 1: modified midpoint with 2c substeps
-            auto rhs = [&](const double (&q)[6], double (&f)[6]) {
-                __syncwarp();
-                if (act) { px[w][lane] = q[0]; py[w][lane] = q[1]; pz[w][lane] = q[2]; }
-                __syncwarp();
-                if (act) {
-                    double ax, ay, az;
-                    enc_accel(q[0], q[1], q[2], my_rc, my_vel, lane, n, px[w], py[w], pz[w], sgm, src, svel, p.nlev, p.mu, p.kind, ax, ay, az,
-                              collide && sinto[lane] != -1);
-                    f[0] = q[3]; f[1] = q[4]; f[2] = q[5]; f[3] = ax; f[4] = ay; f[5] = az;
-                }
-            };
-            const int c = w + 1, nsub = 2 * c;
-            const double hs = h / nsub;
-            double f0[6] = {0, 0, 0, 0, 0, 0}, f[6] = {0, 0, 0, 0, 0, 0}, ym[6], yn[6];
-            rhs(y, f0);
+        bool accepted = false;           // warp 0
+        int cols = 0;
+        for (int pass = 0; pass < 2; ++pass) {
+            const int c_lo = pass == 0 ? 1 : first + 1, c_hi = pass == 0 ? first : kBsCols;
+            if (c_lo > c_hi) break;                       // one pass held all eight columns
+            if (pass == 1 && ctrl_more == 0) break;       // a column of the first pass was accepted (or the step size underflowed)
+            if (!underflow && w + 1 >= c_lo && w + 1 <= c_hi) {
+                // column c = w + 1: modified midpoint with 2c substeps
+                auto rhs = [&](const double (&q)[6], double (&f)[6]) {
+                    __syncwarp();
+                    if (act) { px[w][lane] = q[0]; py[w][lane] = q[1]; pz[w][lane] = q[2]; }
+                    __syncwarp();
+                    if (act) {
+                        double ax, ay, az;
+                        enc_accel(q[0], q[1], q[2], my_rc, my_vel, lane, n, px[w], py[w], pz[w], sgm, src, svel, p.nlev, p.mu, p.kind, ax, ay, az,
+                                  collide && sinto[lane] != -1);
+                        f[0] = q[3]; f[1] = q[4]; f[2] = q[5]; f[3] = ax; f[4] = ay; f[5] = az;
+                    }
+                };
+                const int c = w + 1, nsub = 2 * c;
+                const double hs = h / nsub;
+                double f0[6] = {0, 0, 0, 0, 0, 0}, f[6] = {0, 0, 0, 0, 0, 0}, ym[6], yn[6];
+                rhs(y, f0);
 #pragma unroll
-            for (int k = 0; k < 6; ++k) { ym[k] = y[k]; yn[k] = y[k] + hs * f0[k]; }
-            for (int s = 2; s <= nsub; ++s) {
+                for (int k = 0; k < 6; ++k) { ym[k] = y[k]; yn[k] = y[k] + hs * f0[k]; }
+                for (int s = 2; s <= nsub; ++s) {
+                    rhs(yn, f);
+#pragma unroll
+                    for (int k = 0; k < 6; ++k) { const double tmp = ym[k] + 2.0 * hs * f[k]; ym[k] = yn[k]; yn[k] = tmp; }
+                }
                 rhs(yn, f);
 #pragma unroll
-                for (int k = 0; k < 6; ++k) { const double tmp = ym[k] + 2.0 * hs * f[k]; ym[k] = yn[k]; yn[k] = tmp; }
+                for (int k = 0; k < 6; ++k) col[w][k][lane] = 0.5 * (ym[k] + yn[k] + hs * f[k]);
             }
-            rhs(yn, f);
+            __syncthreads();
+            if (w == 0) {
+                if (!underflow) {
 #pragma unroll
-            for (int k = 0; k < 6; ++k) col[w][k][lane] = 0.5 * (ym[k] + yn[k] + hs * f[k]);
-        }
-        __syncthreads();
-        if (w == 0) {
-            bool accepted = false;
-            int cols = 0;
-            if (!underflow) {
-                for (int c = 1; c <= kBsCols && !accepted; ++c) {
-                    double dif[6];
+                    for (int c = 1; c <= kBsCols; ++c) {   // (compile-time column numbers: the tableau stays in registers)
+                        if (c < c_lo || c > c_hi || accepted) continue;
+                        double dif[6];
 #pragma unroll
-                    for (int k = 0; k < 6; ++k) {
-                        double cur = col[c - 1][k][lane];
-                        const double last_diag = c >= 2 ? T[c - 2][k] : 0.0;
-                        for (int mc = 1; mc < c; ++mc) {
-                            const double old = T[mc - 1][k];
-                            T[mc - 1][k] = cur;
-                            cur = cur + (cur - old) * bs_weight(c, mc);
+                        for (int k = 0; k < 6; ++k) {
+                            double cur = col[c - 1][k][lane];
+                            const double last_diag = c >= 2 ? T[c - 2][k] : 0.0;
+                            for (int mc = 1; mc < c; ++mc) {
+                                const double old = T[mc - 1][k];
+                                T[mc - 1][k] = cur;
+                                cur = cur + (cur - old) * bs_weight(c, mc);
+                            }
+                            T[c - 1][k] = cur;
+                            dif[k] = cur - last_diag;
                         }
-                        T[c - 1][k] = cur;
-                        dif[k] = cur - last_diag;
-                    }
-                    if (c >= 2) {
-                        double e2 = 0.0;
-                        if (act) {
-                            const double ex = (dif[0] * dif[0] + dif[1] * dif[1]) + dif[2] * dif[2];
-                            const double ev = (dif[3] * dif[3] + dif[4] * dif[4]) + dif[5] * dif[5];
-                            const double sx = (y[0] * y[0] + y[1] * y[1]) + y[2] * y[2];
-                            double sv = (y[3] * y[3] + y[4] * y[4]) + y[5] * y[5];
-                            const double vc2 = p.mu / sqrt(sx);
-                            if (sv < vc2) sv = vc2;
-                            e2 = fmax(ex / sx, ev / sv);
-                            if (!(e2 == e2)) e2 = INFINITY;
-                        }
+                        if (c >= 2) {
+                            double e2 = 0.0;
+                            if (act) {
+                                const double ex = (dif[0] * dif[0] + dif[1] * dif[1]) + dif[2] * dif[2];
+                                const double ev = (dif[3] * dif[3] + dif[4] * dif[4]) + dif[5] * dif[5];
+                                const double sx = (y[0] * y[0] + y[1] * y[1]) + y[2] * y[2];
+                                double sv = (y[3] * y[3] + y[4] * y[4]) + y[5] * y[5];
+                                const double vc2 = p.mu / sqrt(sx);
+                                if (sv < vc2) sv = vc2;
+                                e2 = fmax(ex / sx, ev / sv);
+                                if (!(e2 == e2)) e2 = INFINITY;
+                            }
 #pragma unroll
-                        for (int o = 16; o > 0; o >>= 1) e2 = fmax(e2, __shfl_xor_sync(0xffffffffu, e2, o));
-                        if (e2 <= tol2) { accepted = true; cols = c; }
+                            for (int o = 16; o > 0; o >>= 1) e2 = fmax(e2, __shfl_xor_sync(0xffffffffu, e2, o));
+                            if (e2 <= tol2) { accepted = true; cols = c; }
+                        }
                     }
                 }
+                if (lane == 0) ctrl_more = (!accepted && !underflow) ? 1 : 0;
             }
+            __syncthreads();
+        }
+        if (w == 0) {
             if (accepted && act) {
 #pragma unroll
                 for (int k = 0; k < 6; ++k) ycur[k][lane] = T[cols - 1][k];
@@ -495,9 +517,11 @@ __device__ __forceinline__ void bs_small_problem(const EncParams &p, const int b
                     const double tn = (fabs(p.dt - (tcur + h)) <= 1e-15 * fabs(p.dt)) ? p.dt : tcur + h;
                     ctrl_t = tn;
                     ctrl_h = cols <= 6 ? h * 1.3 : (cols == 8 ? h * 0.55 : h);
+                    ctrl_first = kBsCols;
                     if (tn == p.dt) ctrl_done = 1;
                 } else {
                     ctrl_h = h * 0.5;
+                    ctrl_first = kBsCols;
                 }
             }
         }
