@@ -408,12 +408,13 @@ __device__ __forceinline__ void bs_small_problem(const EncParams &p, const int b
     const double my_rc = act ? src[lane] : 0.0, my_vel = act ? svel[lane] : 0.0;
     double T[kBsCols][6];                // warp 0: current row of the tableau
     // A trial step whose first few columns already pass does not need the long ones: the columns are computed in two
-    // passes -- 1 .. first, then (only if none of them passed) first + 1 .. 8 -- with first = 4 for the FIRST trial step
+    // passes -- 1 .. first, then (only if none of them passed) first + 1 .. 8 -- with first = 4 for the first trial step
     // of the short intervals of the multi-level scheme (dt / 2^L: most problems are done in that one step, in 3 or 4
-    // columns), else 8 (one pass).  The tableau is still built column by column and the first column that passes is
-    // taken: the result is the sequential algorithm's; the critical path of such a step falls from 17 to 9 right-hand
-    // sides.  (Measured and rejected: first = 4 after every step accepted in <= 4 columns -- the step-size rule grows h
-    // until ~6 columns are needed, so the next step usually pays both passes: 3 R_Hill with encounters 7.0 -> 8.8 ms.)
+    // columns) and after a step that was accepted in at most 4 columns, else 8 (one pass).  The tableau is still built
+    // column by column and the first column that passes is taken: the result is the sequential algorithm's; the critical
+    // path of such a step falls from 17 to 9 right-hand sides.  Measured: config 3 with the Eq. 7 radius and 4 levels
+    // 37.2 -> 30.0 ms per step; single-level runs 1 - 2 % (the step-size rule grows h until ~6 columns are needed, so
+    // easy steps are rare there).
     __shared__ int ctrl_first, ctrl_more;
     if (threadIdx.x == 0) ctrl_first = p.nlev > 1 ? 4 : kBsCols;
     __syncthreads();
@@ -517,7 +518,7 @@ __device__ __forceinline__ void bs_small_problem(const EncParams &p, const int b
                     const double tn = (fabs(p.dt - (tcur + h)) <= 1e-15 * fabs(p.dt)) ? p.dt : tcur + h;
                     ctrl_t = tn;
                     ctrl_h = cols <= 6 ? h * 1.3 : (cols == 8 ? h * 0.55 : h);
-                    ctrl_first = kBsCols;
+                    ctrl_first = cols <= 4 ? 4 : kBsCols;
                     if (tn == p.dt) ctrl_done = 1;
                 } else {
                     ctrl_h = h * 0.5;
