@@ -370,8 +370,11 @@ __global__ void __launch_bounds__(256) nb_enc_plan_kernel(const int *__restrict_
 
 // One problem of up to 32 bodies, solved by the whole CTA (8 warps = 8 columns; lane = member, b = the lane's body).
 // Lanes >= keep_from write their final state back (0: everybody; nc: only the test particle of a split group).
+// NW = 8 warps: one per column.  NW = 4 (the multi-level scheme's innermost calls: thousands of easy problems, throughput-
+// bound): always two passes, columns 1 .. 4 and, if needed, 5 .. 8 on the same four warps -- half the CTA, twice as many per SM.
+template <int NW>
 __device__ __forceinline__ void bs_small_problem(const EncParams &p, const int b, const int n, const int keep_from) {
-    __shared__ double px[kBsCols][32], py[kBsCols][32], pz[kBsCols][32];
+    __shared__ double px[NW][32], py[NW][32], pz[NW][32];
     __shared__ double sgm[32], src[32], svel[32];
     __shared__ double col[kBsCols][6][32];   // T_{c,0} of every column
     __shared__ double ycur[6][32];
@@ -416,7 +419,7 @@ __device__ __forceinline__ void bs_small_problem(const EncParams &p, const int b
     // 37.2 -> 30.0 ms per step; single-level runs 1 - 2 % (the step-size rule grows h until ~6 columns are needed, so
     // easy steps are rare there).
     __shared__ int ctrl_first, ctrl_more;
-    if (threadIdx.x == 0) ctrl_first = p.nlev > 1 ? 4 : kBsCols;
+    if (threadIdx.x == 0) ctrl_first = (NW == 4 || p.nlev > 1) ? 4 : kBsCols;
     __syncthreads();
     while (true) {
         if (ctrl_done != 0) break;
@@ -434,8 +437,9 @@ __device__ __forceinline__ void bs_small_problem(const EncParams &p, const int b
             const int c_lo = pass == 0 ? 1 : first + 1, c_hi = pass == 0 ? first : kBsCols;
             if (c_lo > c_hi) break;                       // one pass held all eight columns
             if (pass == 1 && ctrl_more == 0) break;       // a column of the first pass was accepted (or the step size underflowed)
-            if (!underflow && w + 1 >= c_lo && w + 1 <= c_hi) {
-                // column c = w + 1: modified midpoint with 2c substeps
+            const int c = NW == 4 ? w + 1 + 4 * pass : w + 1;   // this warp's column in this pass
+            if (!underflow && c >= c_lo && c <= c_hi) {
+                // column c: modified midpoint with 2c substeps
                 auto rhs = [&](const double (&q)[6], double (&f)[6]) {
                     __syncwarp();
                     if (act) { px[w][lane] = q[0]; py[w][lane] = q[1]; pz[w][lane] = q[2]; }
@@ -447,7 +451,7 @@ __device__ __forceinline__ void bs_small_problem(const EncParams &p, const int b
                         f[0] = q[3]; f[1] = q[4]; f[2] = q[5]; f[3] = ax; f[4] = ay; f[5] = az;
                     }
                 };
-                const int c = w + 1, nsub = 2 * c;
+                const int nsub = 2 * c;
                 const double hs = h / nsub;
                 double f0[6] = {0, 0, 0, 0, 0, 0}, f[6] = {0, 0, 0, 0, 0, 0}, ym[6], yn[6];
                 rhs(y, f0);
@@ -460,7 +464,7 @@ __device__ __forceinline__ void bs_small_problem(const EncParams &p, const int b
                 }
                 rhs(yn, f);
 #pragma unroll
-                for (int k = 0; k < 6; ++k) col[w][k][lane] = 0.5 * (ym[k] + yn[k] + hs * f[k]);
+                for (int k = 0; k < 6; ++k) col[c - 1][k][lane] = 0.5 * (ym[k] + yn[k] + hs * f[k]);
             }
             __syncthreads();
             if (w == 0) {
@@ -518,11 +522,11 @@ __device__ __forceinline__ void bs_small_problem(const EncParams &p, const int b
                     const double tn = (fabs(p.dt - (tcur + h)) <= 1e-15 * fabs(p.dt)) ? p.dt : tcur + h;
                     ctrl_t = tn;
                     ctrl_h = cols <= 6 ? h * 1.3 : (cols == 8 ? h * 0.55 : h);
-                    ctrl_first = cols <= 4 ? 4 : kBsCols;
+                    ctrl_first = (NW == 4 || cols <= 4) ? 4 : kBsCols;
                     if (tn == p.dt) ctrl_done = 1;
                 } else {
                     ctrl_h = h * 0.5;
-                    ctrl_first = kBsCols;
+                    ctrl_first = NW == 4 ? 4 : kBsCols;
                 }
             }
         }
@@ -558,7 +562,8 @@ __device__ __forceinline__ int enc_group_size(const EncParams &p, const long lon
 
 // (two CTAs per SM: the collision code must not cost the second one -- 146 registers uncapped, measured 37.9 -> 52.1 ms per
 // step on config 3 with 4 levels)
-__global__ void __launch_bounds__(32 * kBsCols, 2) nb_encounter_small_kernel(const EncParams p) {
+template <int NW>
+__global__ void __launch_bounds__(32 * NW, 16 / NW) nb_encounter_small_kernel(const EncParams p) {
     __shared__ long long sh_next;
     const int lane = threadIdx.x & 31;
     const long long ngroups = p.gstat[0];
@@ -572,7 +577,7 @@ __global__ void __launch_bounds__(32 * kBsCols, 2) nb_encounter_small_kernel(con
         bool split;
         const int n = enc_group_size(p, g, p.gstart[g + 1] - g0, split);
         if (n < p.min_size || n > p.max_size) continue;
-        bs_small_problem(p, lane < n ? p.members[g0 + lane] : 0, n, 0);
+        bs_small_problem<NW>(p, lane < n ? p.members[g0 + lane] : 0, n, 0);
     }
 }
 
@@ -603,7 +608,7 @@ __global__ void __launch_bounds__(32 * kBsCols, 4) nb_encounter_sat_kernel(const
         const int nc = enc_group_size(p, g, p.gstart[g + 1] - g0, split);
         if (!split || k < g0 + nc) continue;  // not a test particle of a split group
         const int b = lane < nc ? p.members[g0 + lane] : (lane == nc ? p.members[k] : 0);
-        bs_small_problem(p, b, nc + 1, nc);
+        bs_small_problem<kBsCols>(p, b, nc + 1, nc);
     }
 }
 

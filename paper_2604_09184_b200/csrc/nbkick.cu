@@ -653,7 +653,14 @@ void enqueue_encounter(const Workspace &w, double *x, double *v, const double *m
         if (sat_blocks > cap_blocks) sat_blocks = cap_blocks;
         nb_encounter_sat_kernel<<<(unsigned)sat_blocks, 32 * kBsCols, 0, stream()>>>(ep);
     }
-    nb_encounter_small_kernel<<<(unsigned)small_blocks, 32 * kBsCols, 0, stream()>>>(ep);
+    if (nlev > 1) {
+        // the multi-level scheme's innermost calls: thousands of easy problems over dt / 2^L -- CTAs of 4 warps, twice as many per SM
+        long long b4 = N / 2 + 1;
+        if (b4 > 2 * cap_blocks) b4 = 2 * cap_blocks;
+        nb_encounter_small_kernel<4><<<(unsigned)b4, 32 * 4, 0, stream()>>>(ep);
+    } else {
+        nb_encounter_small_kernel<kBsCols><<<(unsigned)small_blocks, 32 * kBsCols, 0, stream()>>>(ep);
+    }
     // mid-size groups: CTAs of 128 threads (no register cap: the 1024-thread variant is held to 64 registers and spills)
     ep.min_size = 33; ep.max_size = 128;
     long long mid_blocks = N / 33 + 1;
