@@ -13,7 +13,7 @@
 //   * packed fp32x2 instructions (FADD2 / FMUL2 / FFMA2) wherever two values take the same operation: the kernel is
 //     bound by instruction issue.
 // Pairs whose fp32 r^2 is within reach of a critical radius (margin 2^-18: far above the fp32 rounding of r^2), and
-// every self term, are killed in the fp32 loop (rsqrt replaced by 0: they contribute exactly 0 to both sides) and
+// every self term, are killed in the fp32 loop (r^2 replaced by +inf, so rsqrt gives 0: they contribute exactly 0 to both sides) and
 // re-evaluated by the EXACT fp64 pass of force_sym.cuh (sym_exact) from the fp64 staged arrays: the changeover weight,
 // the pair test r^2 < rc^2 and the pair list are bit-identical to the fp64 kernel's.  Tolerance reading: DESIGN.md S25.
 // Same super-tile decomposition, skewed unit order, slots, determinism and sorted staging (test-free far tiles) as
@@ -24,7 +24,7 @@
 namespace nbk {
 
 struct SymDsParams {
-    SymParams sp;      // fp64 staged arrays (exact pass), slots, pair list, geometry: as nb_force_sym_kernel, unsorted
+    SymParams sp;      // fp64 staged arrays (exact pass), slots, pair list, geometry, perm / bnd of the sorted staging: as nb_force_sym_kernel
     const float4 *sa;  // [2 Npad] (xh, xl, yh, yl)                                  doubled-block layout
     const float4 *sb;  // [2 Npad] (zh, zl, fl32(G m), rc^2 (1 + 2^-18) rounded up)
 };
