@@ -308,6 +308,8 @@ def mixed_point(d, launches=10):
                 ms_per_kick=out[1][0], interactions_per_sec=float(N) * float(N) / (out[1][0] * 1e-3),
                 ms_per_kick_f64=out[0][0], speedup_vs_f64=out[0][0] / out[1][0],
                 rel_err_vs_f64_median=float(rel.median()), rel_err_vs_f64_max=float(rel.max()),
+                # 22 FP32 lane-operations per unordered pair (Newton-III kernel; S25 / 8.6) against 148 SM x 128 lanes x clock
+                fp32_lane_frac=(22.0 * float(N) * float(N) / 2.0 / (out[1][0] * 1e-3) / (148 * 128 * 1.965e9)) if g.tile_j < 0 else None,
                 note="whole nb_kick (staging + force + slot sum), no L2 flush; tolerance reading S25 (DESIGN.md)")
 
 
