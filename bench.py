@@ -55,6 +55,7 @@ def parse_args():
     ap.add_argument("--no-mixed-point", action="store_true", help="skip the mixed-precision side line (fully active configs)")
     ap.add_argument("--force-kernel", type=int, default=0, choices=[0, 1, 2],
                     help="nb_config.force_kernel: 0 auto, 1 one-sided tiles, 2 Newton-III (comparison runs)")
+    ap.add_argument("--i-per-thread", type=int, default=0, choices=[0, 1, 2, 4], help="nb_config.i_per_thread: 0 auto (comparison runs)")
     ap.add_argument("--j-splits", type=int, default=0,
                     help="nb_config.j_splits: 0 auto, k > 0 a grid of k j-splits, -1 balanced pieces (comparison runs, one-sided kernel)")
     ap.add_argument("--precision", default="f64", choices=["f64", "mixed"],
@@ -358,7 +359,7 @@ def run_cuda(args):
     # ---- device-resident arm: inputs in HBM before the timed region -------------------------------
     mixed = args.precision == "mixed"
     nb.configure(N, pair_capacity=cap, n_active=na, G=G_GAUSS, n1=N1, n2=N2, reuse_acc=False, time_force=True,
-                 force_kernel=args.force_kernel, j_splits=args.j_splits, precision=1 if mixed else 0)
+                 force_kernel=args.force_kernel, j_splits=args.j_splits, i_per_thread=args.i_per_thread, precision=1 if mixed else 0)
     nb.nb_status_reset()
     x = torch.from_numpy(d.x).cuda(); v = torch.from_numpy(d.v).cuda(); m = torch.from_numpy(d.m).cuda()
     acc = torch.zeros_like(x); rc = torch.zeros(N, dtype=torch.float64, device="cuda")
@@ -527,7 +528,7 @@ def run_trajectory(args):
     radius = torch.from_numpy(d.radius).cuda() if collide else None
     absorbed_by = torch.full((N,), -1, dtype=torch.int32, device="cuda") if collide else None
     nb.configure(N, pair_capacity=cap, n_active=na, G=G_GAUSS, n1=N1, n2=n2, resolve_encounters=args.encounters,
-                 levels=args.levels, precision=1 if args.precision == "mixed" else 0, force_kernel=args.force_kernel, j_splits=args.j_splits,
+                 levels=args.levels, precision=1 if args.precision == "mixed" else 0, force_kernel=args.force_kernel, j_splits=args.j_splits, i_per_thread=args.i_per_thread,
                  radius_factor=args.collide if collide else 1.0, collide_radius=radius, collide_absorbed_by=absorbed_by)
     nb.nb_status_reset()
     x = torch.from_numpy(d.x).cuda(); v = torch.from_numpy(d.v).cuda(); m = torch.from_numpy(d.m).cuda()
