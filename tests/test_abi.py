@@ -154,3 +154,38 @@ def test_product_path_does_not_touch_the_oracle():
             txt = open(os.path.join(ROOT, "oracle", f)).read()
             assert not re.search(r"^\s*(from|import)\s+paper_2604_09184_b200\b", txt, flags=re.M), f
             assert "nbkick" not in txt, f
+
+
+def test_geometry_of_the_mixed_precision_kernels(nb):
+    """NB_PRECISION_MIXED (host logic, no GPU): fully active N >= 4096 takes the Newton-III kernel on double-single positions
+    (same super-block rule as the fp64 kernel, 32 more bytes per staged body), bands when the slots would pass the cap;
+    semi-active mode takes the one-sided double-single kernel (32 bytes more per active body); with one i-body per thread
+    (small N) the fp64 kernel runs and the workspace is the fp64 one."""
+    lib = nb.load()
+
+    def geo(N, n_active=0, precision=1, **kw):
+        c = nb.default_config()
+        c.n_active, c.precision = n_active, precision
+        for k, v in kw.items():
+            setattr(c, k, v)
+        assert lib.nb_configure(C.byref(c)) == 0
+        return nb.force_geometry(N), nb.workspace_bytes(N)
+
+    for N in (4096, 16386, 65536):
+        g64, w64 = geo(N, precision=0)
+        g32, w32 = geo(N)
+        assert g32.tile_j == g64.tile_j < 0 and g32.i_per_thread == 4 and g32.threads == g64.threads
+        npad = -(-N // -g32.tile_j) * -g32.tile_j
+        T = npad // -g32.tile_j
+        # the fp64 staged arrays (72 B per body, doubled blocks; the exact pass reads them), two float4 arrays in the same
+        # layout (64 B per body), one slot per super-block
+        assert w32 >= 72 * npad + 64 * npad + 24 * N * T
+        assert w32 <= w64 + 64 * npad + 4096                                          # nothing else grows
+    g, w = geo(524288)
+    assert g.tile_j == -512 and w <= (4 << 30) + 200 * 524288                      # banded: slots within the 4 GiB cap
+    g, w = geo(131072, n_active=1024)
+    g0, w0 = geo(131072, n_active=1024, precision=0)
+    assert g.tile_j == 128 and g.i_per_thread == 2 and w - w0 == 1024 * 32         # one-sided double-single records
+    g, w = geo(2048)
+    g0, w0 = geo(2048, precision=0)
+    assert g.tile_j == 128 and g.i_per_thread == 1 and w == w0                     # small N: the fp64 kernel
