@@ -17,13 +17,17 @@ struct __align__(16) JRec {
 };
 static_assert(sizeof(JRec) == 64, "JRec must be 64 bytes");
 
+// fp32 range: r^2 below this (r < 1e-15 in the caller's units) goes to the exact fp64 path whatever the critical radii -- the cube
+// of an fp32 reciprocal square root would leave the fp32 range long before the fp64 kernel has any difficulty
+constexpr float kDsMinR2 = 1.0e-30f;
+
 // stages body `pos` (position in the doubled-block layout) for the Newton-III mixed-precision kernel (force_symds.cuh):
 // double-single position (xh + xl), fl32(G m), and rc^2 rounded up with a 2^-18 margin; called by nb_prep_kernel
 __device__ __forceinline__ void symds_stage(float4 *sa, float4 *sb, const int pos, const double x, const double y, const double z,
                                             const double gm, const double rc2) {
     const float xh = __double2float_rn(x), yh = __double2float_rn(y), zh = __double2float_rn(z);
     const float xl = __double2float_rn(x - (double)xh), yl = __double2float_rn(y - (double)yh), zl = __double2float_rn(z - (double)zh);
-    const float thr = __double2float_ru(rc2) * 1.0000038f;
+    const float thr = fmaxf(__double2float_ru(rc2) * 1.0000038f, kDsMinR2);
     const size_t en = (size_t)(pos >> 5) * 64 + (pos & 31);
     // (high, low) of a coordinate sit side by side: one packed fp32x2 add forms both partial differences
     const float4 a = make_float4(xh, xl, yh, yl), b = make_float4(zh, zl, __double2float_rn(gm), thr);
@@ -42,7 +46,7 @@ __device__ __forceinline__ JRecDs make_jrecds(const double x, const double y, co
     JRecDs r;
     r.xh = __double2float_rn(x); r.yh = __double2float_rn(y); r.zh = __double2float_rn(z);
     r.xl = __double2float_rn(x - (double)r.xh); r.yl = __double2float_rn(y - (double)r.yh); r.zl = __double2float_rn(z - (double)r.zh);
-    r.gm = __double2float_rn(gm); r.thr = __double2float_ru(rc2) * 1.0000038f;
+    r.gm = __double2float_rn(gm); r.thr = fmaxf(__double2float_ru(rc2) * 1.0000038f, kDsMinR2);
     return r;
 }
 

@@ -180,3 +180,23 @@ def test_mixed_config3_full_200_steps_against_the_stored_oracle_run():
     assert abs(de_g - de_r) <= 1e-9
     assert dL <= 1e-9
     assert np.quantile(ex, 0.99) <= 1e-6
+
+
+def test_mixed_pairs_closer_than_the_fp32_range_go_to_the_exact_path():
+    """Two pairs a hair apart (1e-17 and 1e-21 in the caller's units) with rc = 0 everywhere: the cube of an fp32 reciprocal
+    square root would overflow; the staging's floor on the pre-filter threshold sends them to the fp64 pass."""
+    N = 4100
+    x, v, m = nb_inputs.random_cluster(N, seed=77, scale=0.3)
+    x[10] = x[2000] + np.array([1e-17, 0.0, 0.0])
+    x[11] = x[3000] + np.array([0.0, 1e-21, 0.0])
+    m[11] = 0.0
+    rc = np.zeros(N)
+    ref, ab, _ = oracle.accel(x, m, rc, G_GAUSS, want_abs=True)
+    st = GpuState(x, v, m, G=G_GAUSS, precision=1)
+    assert st.nb.force_geometry(N).tile_j < 0
+    st.set_rcrit(rc)
+    st.kick(0.0)
+    acc = st.acc.cpu().numpy()
+    assert np.all(np.isfinite(acc))
+    worst = float(np.max(np.abs(acc - ref) / np.where(ab > 0, ab, 1e-300)))
+    assert worst <= BOUND_DS, worst / U32
