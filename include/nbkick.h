@@ -69,7 +69,10 @@ extern "C" {
  *                       otherwise (semi-active, NB_FORCE_TILES): the one-sided kernel with the same double-single
  *                       arithmetic, summed in fp32 per 128-body tile and in fp64 across tiles -- when it holds 2 or 4
  *                       i-bodies per thread; with one (small N: latency-bound launches, where fp32 does not pay) the
- *                       fp64 kernel runs, which meets the tolerance trivially. */
+ *                       fp64 kernel runs, which meets the tolerance trivially.
+ *                       Units: r^-3 and G m r^-3 of the far pairs must lie in the fp32 range (1e-38 .. 1e38): they do in
+ *                       AU / day / solar mass (the defaults) and in any units of that kind; they do not in cgs (r^-3 ~
+ *                       1e-42).  Pairs closer than 1e-15 length units always take the fp64 pass. */
 #define NB_PRECISION_F64 0
 #define NB_PRECISION_MIXED 1
 #define NB_SORT_AUTO 0
