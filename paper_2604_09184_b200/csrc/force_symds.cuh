@@ -63,7 +63,7 @@ __device__ __forceinline__ void symds_block(const SymDsParams &p, const float4 *
     const float4 *__restrict__ la = qa + lane;
     const float4 *__restrict__ lb = qb + lane;
     const float kInf = __int_as_float(0x7f800000);
-#pragma unroll 4
+#pragma unroll(TEST ? 4 : 8)
     for (int r = 0; r < 32; ++r) {
         const float4 a = la[r];                       // (xh, xl, yh, yl)
         const float4 b = lb[r];                       // (zh, zl, G m, threshold)
