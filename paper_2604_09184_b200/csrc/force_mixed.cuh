@@ -95,7 +95,7 @@ __global__ void __launch_bounds__(kForceThreads, MINB) nb_force_mixedds_kernel(c
         for (int g = 0; g < H; ++g) { fx[g] = make_float2(0.f, 0.f); fy[g] = fx[g]; fz[g] = fx[g]; }
         const int jbase = (tile_begin + it) * kTileJ;
         const float4 *tile = reinterpret_cast<const float4 *>(&sm[st][0]);
-#pragma unroll 2
+#pragma unroll 4
         for (int jj = 0; jj < kTileJ; ++jj) {
             const float4 a = tile[2 * jj];        // (xh, xl, yh, yl)
             const float4 b = tile[2 * jj + 1];    // (zh, zl, G m, threshold)
