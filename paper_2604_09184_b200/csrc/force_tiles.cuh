@@ -317,7 +317,7 @@ __device__ __forceinline__ void force_tiles_cta(const ForceParams &p, const int 
                 }
             }
         } else {
-#pragma unroll 2
+#pragma unroll 4
         for (int jj = 0; jj < kTileJ; ++jj) {
             JWork<I> cur;
             cur.load(tile + jj, xi, yi, zi, thr_i);
